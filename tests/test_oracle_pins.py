@@ -1,0 +1,377 @@
+"""Pins for the CPU oracle.  CPU only.
+
+None of these re-type the oracle's formula against itself: they check it
+against the worked example stored in tests/golden/ (hand-computed from
+PAPER.md Eq. 3), exact rational arithmetic in a different style, numpy's own
+float16 codec and matmul, the algebraic identities Eq. 2 / Eq. 4 of the paper,
+and hand-derived positions of the packed layout.
+"""
+import json
+import os
+from fractions import Fraction
+
+import numpy as np
+import pytest
+
+import oracle
+from workloads import make_layer
+
+GOLD = os.path.join(os.path.dirname(__file__), "golden")
+
+
+def f16(a):
+    return np.ascontiguousarray(np.asarray(a, dtype=np.float64).astype(np.float16))
+
+
+# ---------------------------------------------------------------- fp16 codec
+
+def test_f16_decode_all_bit_patterns_matches_numpy():
+    bits = np.arange(65536, dtype=np.uint16)
+    got = oracle.f16_to_f64(bits.view(np.float16))
+    want = bits.view(np.float16).astype(np.float64)
+    nan = np.isnan(want)
+    assert np.array_equal(np.isnan(got), nan)
+    assert np.array_equal(got[~nan], want[~nan])
+    assert np.array_equal(np.signbit(got[~nan]), np.signbit(want[~nan]))
+
+
+def test_f16_encode_matches_numpy_rne():
+    rng = np.random.default_rng(1)
+    v = np.concatenate([
+        rng.standard_normal(20000) * 10.0 ** rng.integers(-9, 6, 20000),
+        np.arange(65536, dtype=np.uint16).view(np.float16).astype(np.float64)[:0x7c00],
+        # exact ties between neighbouring fp16 values, both parities
+        (np.arange(1024, 2047) + 0.5) * 2.0 ** -10,
+        (np.arange(0, 1024) + 0.5) * 2.0 ** -24,
+        np.array([65504.0, 65519.99, 65520.0, 1e9, -1e9, 0.0, -0.0, 2.0 ** -25, 2.0 ** -25 * 1.0001]),
+    ])
+    with np.errstate(over="ignore"):
+        want = v.astype(np.float16)
+    got = oracle.f64_to_f16(v)
+    assert np.array_equal(got.view(np.uint16), want.view(np.uint16))
+
+
+# ---------------------------------------------------------------- P1 worked example
+
+def _gold():
+    with open(os.path.join(GOLD, "worked_example_P1.json")) as f:
+        return json.load(f)
+
+
+def test_P1_worked_example_dequant_and_base():
+    g = _gold()
+    codes = np.array(g["codes"], np.uint8)
+    scales = f16(g["scales"])
+    What = oracle.dequant(codes, scales, g["group"])
+    assert np.array_equal(What, np.array(g["What"]))
+    out = oracle.forward(f16(g["x"]), What, gate="none")
+    assert np.array_equal(out["ybase"], np.array(g["ybase"]))
+    assert np.array_equal(out["y"], np.array(g["ybase"]))
+
+
+@pytest.mark.parametrize("case", range(3))
+def test_P1_worked_example_gated(case):
+    g = _gold()
+    c = g["cases"][case]
+    What = oracle.dequant(np.array(g["codes"], np.uint8), f16(g["scales"]), g["group"])
+    kw = dict(gate=c["gate"], alpha=g["alpha"])
+    if c["gate"] == "scalar":
+        kw.update(w_g=f16(c["w_g"]), b_g=c["b_g"])
+    else:
+        kw.update(W1=f16(c["W1"]), b1=np.array(c["b1"], np.float32),
+                  W2=f16(c["W2"]), b2=np.array(c["b2"], np.float32))
+    out = oracle.forward(f16(g["x"]), What, f16(g["A"]), f16(g["B"]), **kw)
+    assert np.array_equal(out["z"], np.array(g["z"]))
+    np.testing.assert_allclose(np.ravel(out["gam"]), [c["gam"]], rtol=0, atol=1e-15)
+    np.testing.assert_allclose(out["y"], np.array(c["y"]), rtol=0, atol=1e-14)
+
+
+# ---------------------------------------------------------------- P8 brute force, exact rationals
+
+def _frac(a):
+    """fp16/fp32 array -> nested lists of exact Fractions (a float is a dyadic rational)."""
+    a = np.asarray(a)
+    return [[Fraction(float(v)) for v in row] for row in a.reshape(a.shape[0], -1)]
+
+
+def test_P8_bruteforce_rational_scalar_gate_none_and_static():
+    li = make_layer(seed=11, M=3, N=128, K=256, group=128, r=8, gate="none")
+    # restrict to the first 6 rows of W to keep the pure-Python loops short
+    Nn = 6
+    codes, scales, Bm = li.codes[:Nn], li.scales[:Nn], li.B[:Nn]
+    What = oracle.dequant(codes, scales, li.group)
+    out = oracle.forward(li.x, What, li.A, Bm, gate="none", alpha=0.75)
+    X, Af, Bf, S = _frac(li.x), _frac(li.A), _frac(Bm), _frac(scales)
+    alpha = Fraction(3, 4)
+    for m in range(li.M):
+        z = [sum(Af[j][k] * X[m][k] for k in range(li.K)) for j in range(li.r)]
+        for n in range(Nn):
+            base = sum(X[m][k] * (int(codes[n][k]) - 8) * S[n][k // li.group] for k in range(li.K))
+            y = base + alpha * sum(Bf[n][j] * z[j] for j in range(li.r))
+            assert abs(out["ybase"][m][n] - float(base)) <= 1e-12 * max(1.0, abs(float(base)))
+            assert abs(out["y"][m][n] - float(y)) <= 1e-12 * max(1.0, abs(float(y)))
+        for j in range(li.r):
+            assert abs(out["z"][m][j] - float(z[j])) <= 1e-13 * max(1.0, abs(float(z[j])))
+
+
+def test_P8_onehot_and_allones():
+    N, K, group = 128, 256, 128
+    li = make_layer(seed=5, M=1, N=N, K=K, group=group, r=0)
+    What = oracle.dequant(li.codes, li.scales, group)
+    for k in (0, 127, 128, 255):
+        x = np.zeros((1, K), np.float16)
+        x[0, k] = 1.0
+        out = oracle.forward(x, What, gate="none")
+        assert np.array_equal(out["y"][0], What[:, k])
+    codes = np.full((N, K), 9, np.uint8)
+    scales = np.ones((N, K // group), np.float16)
+    out = oracle.forward(li.x, oracle.dequant(codes, scales, group), gate="none")
+    want = float(sum(Fraction(float(v)) for v in li.x[0]))
+    assert np.allclose(out["y"][0], want, rtol=0, atol=1e-11)
+
+
+def test_numpy_matmul_cross_check_medium():
+    li = make_layer(seed=21, M=5, N=256, K=512, group=128, r=16, gate="scalar")
+    What = oracle.dequant(li.codes, li.scales, li.group)
+    out = oracle.forward(li.x, What, li.A, li.B, gate="scalar", w_g=li.w_g, b_g=0.25)
+    x = li.x.astype(np.float64)
+    # independent formulation: numpy broadcasting dequant + BLAS matmul + expit-style gate
+    W2d = (li.codes.astype(np.float64) - 8.0) * np.repeat(li.scales.astype(np.float64), li.group, axis=1)
+    assert np.array_equal(What, W2d)
+    z = x @ li.A.astype(np.float64).T
+    s = x @ li.w_g.astype(np.float64) + 0.25
+    g = np.exp(-np.logaddexp(0.0, -s))
+    y = x @ W2d.T + (z * g[:, None]) @ li.B.astype(np.float64).T
+    np.testing.assert_allclose(out["z"], z, rtol=1e-12, atol=1e-12)
+    np.testing.assert_allclose(out["gam"], g, rtol=1e-12, atol=1e-14)
+    np.testing.assert_allclose(out["y"], y, rtol=1e-11, atol=1e-10)
+
+
+# ---------------------------------------------------------------- P2 reductions to plain W4
+
+def test_P2_zero_A_or_B_or_closed_gate_is_plain_w4():
+    li = make_layer(seed=3, M=4, N=128, K=256, group=128, r=8, gate="mlp")
+    What = oracle.dequant(li.codes, li.scales, li.group)
+    base = oracle.forward(li.x, What, gate="none")["y"]
+    zA = oracle.forward(li.x, What, np.zeros_like(li.A), li.B, gate="mlp",
+                        W1=li.W1, b1=li.b1, W2=li.W2, b2=li.b2)
+    zB = oracle.forward(li.x, What, li.A, np.zeros_like(li.B), gate="mlp",
+                        W1=li.W1, b1=li.b1, W2=li.W2, b2=li.b2)
+    assert np.array_equal(zA["y"], base) and np.array_equal(zB["y"], base)
+    closed = oracle.forward(li.x, What, li.A, li.B, gate="mlp", W1=li.W1, b1=li.b1,
+                            W2=np.zeros_like(li.W2), b2=np.full(li.r, -40.0, np.float32))
+    assert np.array_equal(closed["gam"], np.zeros_like(closed["gam"]))
+    assert np.array_equal(closed["y"], base)
+    w_g = np.zeros(li.K, np.float16)
+    sc = oracle.forward(li.x, What, li.A, li.B, gate="scalar", w_g=w_g, b_g=-800.0)
+    assert np.array_equal(sc["gam"], np.zeros(li.M)) and np.array_equal(sc["y"], base)
+
+
+# ---------------------------------------------------------------- P3 / P4 effective-weight identities
+
+def test_P3_static_compensator_equals_effective_weight_Eq2():
+    li = make_layer(seed=7, M=6, N=128, K=384, group=128, r=16, gate="mlp")
+    What = oracle.dequant(li.codes, li.scales, li.group)
+    alpha = 0.5
+    out = oracle.forward(li.x, What, li.A, li.B, gate="mlp", alpha=alpha, W1=li.W1, b1=li.b1,
+                         W2=np.zeros_like(li.W2), b2=np.zeros(li.r, np.float32))
+    assert np.array_equal(out["gam"], np.ones_like(out["gam"]))
+    none = oracle.forward(li.x, What, li.A, li.B, gate="none", alpha=alpha)
+    assert np.array_equal(out["y"], none["y"])
+    Weff = What + alpha * li.B.astype(np.float64) @ li.A.astype(np.float64)     # [N][K], Eq. 2
+    want = li.x.astype(np.float64) @ Weff.T
+    np.testing.assert_allclose(out["y"], want, rtol=1e-11, atol=1e-10)
+    # orientation check: a transposed A or B would change the shapes; a swapped (A, B) pair would fail here
+    assert li.A.shape == (li.r, li.K) and li.B.shape == (li.N, li.r)
+
+
+@pytest.mark.parametrize("gate", ["mlp", "scalar"])
+def test_P4_per_token_effective_weight_Eq4(gate):
+    li = make_layer(seed=8, M=5, N=128, K=256, group=128, r=8, gate=gate)
+    What = oracle.dequant(li.codes, li.scales, li.group)
+    out = oracle.forward_layer(li)
+    A64, B64, x64 = li.A.astype(np.float64), li.B.astype(np.float64), li.x.astype(np.float64)
+    for m in range(li.M):
+        gam = out["gam"][m] if gate == "mlp" else np.full(li.r, out["gam"][m])
+        Weff = What + li.alpha * B64 @ np.diag(gam) @ A64
+        np.testing.assert_allclose(out["y"][m], Weff @ x64[m], rtol=1e-11, atol=1e-10)
+    assert np.ptp(out["gam"]) > 1e-3          # the gate really differs between tokens
+
+
+# ---------------------------------------------------------------- P5 linearity, rank
+
+def test_P5_linearity_in_B_homogeneity_in_alpha_and_rank():
+    li = make_layer(seed=9, M=24, N=128, K=256, group=128, r=8, gate="mlp")
+    li2 = make_layer(seed=10, M=24, N=128, K=256, group=128, r=8, gate="mlp")
+    What = oracle.dequant(li.codes, li.scales, li.group)
+    kw = dict(gate="mlp", W1=li.W1, b1=li.b1, W2=li.W2, b2=li.b2)
+    # B1, B2 on a coarse dyadic grid so that B1 + B2 is exactly representable in fp16
+    B1 = f16(np.round(li.B.astype(np.float64) * 64) / 64)
+    B2 = f16(np.round(li2.B.astype(np.float64) * 64) / 64)
+    B12 = f16(B1.astype(np.float64) + B2.astype(np.float64))
+    assert np.array_equal(B12.astype(np.float64), B1.astype(np.float64) + B2.astype(np.float64))
+    base = oracle.forward(li.x, What, gate="none")["y"]
+    d1 = oracle.forward(li.x, What, li.A, B1, **kw)["y"] - base
+    d2 = oracle.forward(li.x, What, li.A, B2, **kw)["y"] - base
+    d12 = oracle.forward(li.x, What, li.A, B12, **kw)["y"] - base
+    np.testing.assert_allclose(d12, d1 + d2, rtol=0, atol=1e-10)
+    d3 = oracle.forward(li.x, What, li.A, B1, alpha=3.0, **kw)["y"] - base
+    np.testing.assert_allclose(d3, 3.0 * d1, rtol=0, atol=1e-10)
+    sv = np.linalg.svd(d1, compute_uv=False)
+    assert sv[li.r - 1] > 1e-6 * sv[0]
+    assert sv[li.r] < 1e-10 * sv[0]          # numerical rank of Y - Ybase is <= r
+
+
+# ---------------------------------------------------------------- P6 gate bounds, token independence
+
+def test_P6_gate_bounds_and_neutral_points():
+    li = make_layer(seed=12, M=32, N=128, K=256, group=128, r=8, gate="mlp")
+    What = oracle.dequant(li.codes, li.scales, li.group)
+    out = oracle.forward_layer(li)
+    assert (out["gam"] > 0).all() and (out["gam"] < 2).all()
+    lo = oracle.forward(li.x, What, li.A, li.B, gate="mlp", W1=li.W1, b1=li.b1, W2=li.W2,
+                        b2=np.full(li.r, -0.5, np.float32))["gam"]
+    hi = oracle.forward(li.x, What, li.A, li.B, gate="mlp", W1=li.W1, b1=li.b1, W2=li.W2,
+                        b2=np.full(li.r, 0.5, np.float32))["gam"]
+    assert (hi > lo).all()                   # monotone in b2
+    ls = make_layer(seed=12, M=32, N=128, K=256, group=128, r=8, gate="scalar")
+    g0 = oracle.forward(ls.x, What, ls.A, ls.B, gate="scalar", w_g=np.zeros(ls.K, np.float16), b_g=0.0)["gam"]
+    assert np.array_equal(g0, np.full(ls.M, 0.5))
+    gs = oracle.forward_layer(ls)["gam"]
+    assert (gs > 0).all() and (gs < 1).all()
+    gp = oracle.forward(ls.x, What, ls.A, ls.B, gate="scalar", w_g=ls.w_g, b_g=1.0)["gam"]
+    assert (gp > gs).all()                   # monotone in b
+
+
+@pytest.mark.parametrize("gate", ["mlp", "scalar"])
+def test_P6_token_permutation_and_duplication(gate):
+    li = make_layer(seed=13, M=7, N=128, K=256, group=128, r=8, gate=gate)
+    out = oracle.forward_layer(li)
+    perm = np.array([3, 0, 6, 6, 1, 5, 2, 4, 3])
+    sub = oracle.forward_layer(li, rows=perm)
+    assert np.array_equal(sub["y"], out["y"][perm])
+    assert np.array_equal(sub["gam"], out["gam"][perm])
+    assert np.array_equal(sub["z"], out["z"][perm])
+
+
+# ---------------------------------------------------------------- P7 dequant grid, group indexing
+
+def test_P7_dequant_grid_all_codes_times_scales():
+    scales_list = [1e-3, 1.0, 0.5, 2.0 ** -10, 0.020004272, 0.0999755859375, 1023.0 / 1024, 6.1e-5, 3.0e-6]
+    K, group = 128, 128
+    N = 128
+    codes = np.zeros((N, K), np.uint8)
+    scales = np.ones((N, 1), np.float16)
+    for i, s in enumerate(scales_list):
+        scales[i, 0] = np.float16(s)
+        codes[i, :16] = np.arange(16)
+    What = oracle.dequant(codes, scales, group)
+    d16 = oracle.dequant16(codes, scales, group)
+    for i in range(len(scales_list)):
+        s = Fraction(float(scales[i, 0]))
+        for q in range(16):
+            assert Fraction(float(What[i, q])) == (q - 8) * s          # exact in fp64
+            with np.errstate(under="ignore"):
+                want16 = np.float64(float((q - 8) * s)).astype(np.float16)   # numpy's own RNE
+            assert d16[i, q].view(np.uint16) == want16.view(np.uint16)
+        assert What[i, 8] == 0.0 and not np.signbit(What[i, 8])
+
+
+def test_P7_group_boundaries_select_the_right_scale_and_x_slice():
+    N, K, group = 128, 512, 128
+    li = make_layer(seed=14, M=2, N=N, K=K, group=group, r=0)
+    for grp in range(K // group):
+        codes = np.full((N, K), 8, np.uint8)
+        codes[:, grp * group:(grp + 1) * group] = li.codes[:, grp * group:(grp + 1) * group]
+        y = oracle.forward(li.x, oracle.dequant(codes, li.scales, group), gate="none")["y"]
+        xs = li.x[:, grp * group:(grp + 1) * group].astype(np.float64)
+        ws = (li.codes[:, grp * group:(grp + 1) * group].astype(np.float64) - 8.0) \
+            * li.scales[:, grp].astype(np.float64)[:, None]
+        np.testing.assert_allclose(y, xs @ ws.T, rtol=1e-12, atol=1e-11)
+
+
+def test_A5_rtn_roundtrip_on_representable_grid():
+    rng = np.random.default_rng(4)
+    N, K, group = 128, 256, 128
+    codes = rng.integers(1, 16, (N, K)).astype(np.uint8)          # no code 0
+    codes[:, 0::group] = 15                                       # every group holds |q-8| = 7
+    scales = f16(np.abs(rng.standard_normal((N, K // group))) * 0.02 + 1e-3)
+    W = oracle.dequant(codes, scales, group)
+    q2, s2 = oracle.rtn_quantise(W, group)
+    assert np.array_equal(s2.view(np.uint16), scales.view(np.uint16))
+    assert np.array_equal(q2, codes)
+    assert np.array_equal(oracle.dequant(q2, s2, group), W)
+
+
+# ---------------------------------------------------------------- P9 workload statistics
+
+def test_P9_closed_form_statistics_of_config1():
+    li = make_layer(seed=0, M=4, N=2048, K=2048, group=128, r=16, gate="scalar")
+    assert li.outlier_channels.size == 20
+    out = oracle.forward_layer(li)
+    q = li.codes.astype(np.float64) - 8.0
+    assert abs((q ** 2).mean() - 21.5) < 0.1
+    assert abs((li.scales.astype(np.float64) ** 2).mean() - 4.33e-4) < 0.2e-4
+    rms = np.sqrt((out["ybase"] ** 2).mean())
+    # E[x^2] per token row = (K - 20 + 20*400)/K = 4.896; sqrt(K * 4.896 * 21.5 * 4.33e-4) = 9.66
+    assert 0.8 * 9.66 < rms < 1.2 * 9.66
+    zr = np.sqrt((out["z"] ** 2).mean())
+    assert 0.6 * 2.21 < zr < 1.5 * 2.21
+    ec = out["y"] - out["ybase"]
+    assert np.sqrt((ec ** 2).mean()) > 0.05 * rms      # an EC bug is far above the 1e-2*rms tolerance
+
+
+# ---------------------------------------------------------------- P10 packed layout
+
+def test_P10_pack_positions_hand_derived():
+    with open(os.path.join(GOLD, "pack_positions.json")) as f:
+        g = json.load(f)
+    N, K, group = g["N"], g["K"], g["group"]
+    G = K // group
+    for ent in g["entries"]:
+        codes = np.full((N, K), 0, np.uint8)
+        codes[ent["n"], ent["k"]] = 0xF
+        wq, _ = oracle.pack_w4(codes, np.ones((N, G), np.float16), group)
+        nz = np.flatnonzero(wq)
+        assert nz.tolist() == [ent["word"]], ent
+        assert int(wq[ent["word"]]) == 0xF << ent["shift"], ent
+    for ent in g["scale_entries"]:
+        sc = np.zeros((N, G), np.float16)
+        sc[ent["n"], ent["grp"]] = 1.0
+        _, sp = oracle.pack_w4(np.zeros((N, K), np.uint8), sc, group)
+        assert np.flatnonzero(sp).tolist() == [ent["index"]], ent
+
+
+def test_P10_pack_is_a_bijection_and_roundtrips():
+    rng = np.random.default_rng(2)
+    for (N, K, group) in [(128, 128, 128), (256, 384, 128), (128, 512, 512), (384, 256, 256)]:
+        codes = rng.integers(0, 16, (N, K)).astype(np.uint8)
+        scales = f16(rng.random((N, K // group)) + 0.01)
+        wq, sp = oracle.pack_w4(codes, scales, group)
+        assert wq.size * 4 == N * K // 2 and sp.size == N * (K // group)
+        assert np.array_equal(oracle.unpack_w4(wq, N, K), codes)
+        assert sorted(sp.view(np.uint16).tolist()) == sorted(scales.view(np.uint16).ravel().tolist())
+        n = np.arange(N)[:, None]
+        k = np.arange(K)[None, :]
+        structured = ((n + k) & 15).astype(np.uint8)
+        wq2, _ = oracle.pack_w4(structured, scales, group)
+        assert np.array_equal(oracle.unpack_w4(wq2, N, K), structured)
+    # every nibble position of the buffer is hit exactly once
+    N, K = 128, 128
+    seen = np.zeros(N * K // 8, np.uint32)
+    for nn in range(0, N, 5):
+        for kk in range(K):
+            c = np.zeros((N, K), np.uint8)
+            c[nn, kk] = 0xF
+            w, _ = oracle.pack_w4(c, np.ones((N, 1), np.float16), K)
+            assert (seen & w).sum() == 0
+            seen |= w
+
+
+def test_pack_rejects_bad_codes_and_shapes():
+    with pytest.raises(ValueError):
+        oracle.pack_w4(np.full((128, 128), 16, np.uint8), np.ones((128, 1), np.float16), 128)
+    with pytest.raises(ValueError):
+        oracle.pack_w4(np.zeros((64, 128), np.uint8), np.ones((64, 1), np.float16), 128)
+    with pytest.raises(ValueError):
+        oracle.dequant(np.full((4, 4), 17, np.uint8), np.ones((4, 1), np.float16), 4)
