@@ -1,0 +1,152 @@
+/*
+ * spear.h -- C ABI of libspear.so: the SPEAR W4A16 + per-token-gated Error Compensator layer
+ * on one NVIDIA B200 (sm_100a).
+ *
+ * The operation (PAPER.md:107-110, Eq. 3; shapes PAPER.md:118; W4 format PAPER.md:247, :585):
+ *
+ *     y[m][n] = sum_k x[m][k] * What[n][k]  +  alpha * sum_j B[n][j] * gamma[m][j] * z[m][j]
+ *     What[n][k] = (q[n][k] - 8) * s[n][k / group]              q in 0..15, zero-point 8, fp16 scale
+ *     z[m][j]    = sum_k A[j][k] * x[m][k]                      "Ax"
+ *     gamma      = 1 + tanh(W2 relu(W1 z + b1) + b2)            SPEAR_GATE_MLP
+ *     gamma[m][*]= 1 / (1 + exp(-(x[m] . w_g + b)))             SPEAR_GATE_SCALAR_SIGMOID (BASELINE.json configs)
+ *     gamma      = 1                                            SPEAR_GATE_NONE    (Eq. 2)
+ *
+ * Canonical layouts: row-major, contiguous.  x[M][K] fp16, q[N][K] uint8, s[N][K/group] fp16,
+ * A[r][K] fp16, B[N][r] fp16, y[M][N] fp16 (orientation as in the paper: What in R^{d_out x d_in},
+ * A in R^{r x d_in}, B in R^{d_out x r}).  Accumulation is fp32, y is rounded to fp16 once (RN-even).
+ *
+ * Conventions for every entry point
+ *   - returns 0 (SPEAR_OK) or a negative spear_status; never throws, never exits;
+ *     spear_last_error() gives a thread-local message for the last non-zero status;
+ *   - every data pointer is a DEVICE pointer, 16-byte aligned, owned by the caller, unless the
+ *     argument is documented as "host";
+ *   - `stream` is a cudaStream_t passed as void* (NULL = the legacy default stream);
+ *   - work is enqueued on `stream` and the call returns without synchronising, except
+ *     spear_pack_w4 (reads back a validity flag), spear_plan (measures) and spear_init;
+ *   - supported shapes: M >= 1, N % 128 == 0, K % 128 == 0, group % 128 == 0, K % group == 0,
+ *     0 <= r <= 128 with r % 8 == 0 (pad A with zero rows and B with zero columns: exact);
+ *     anything else returns SPEAR_EUNSUPPORTED.  x and y must not alias.
+ *   - there is no CPU path: without a CUDA device every compute call returns SPEAR_ECUDA.
+ */
+#ifndef SPEAR_H
+#define SPEAR_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef enum {
+    SPEAR_OK = 0,
+    SPEAR_EINVAL = -1,        /* bad argument (NULL pointer, misaligned, code > 15, ...)            */
+    SPEAR_EUNSUPPORTED = -2,  /* shape outside the supported set above                              */
+    SPEAR_ECUDA = -3,         /* a CUDA runtime call failed (message in spear_last_error)           */
+    SPEAR_ENOMEM = -4         /* workspace too small / allocation failed                            */
+} spear_status;
+
+typedef enum {
+    SPEAR_GATE_SCALAR_SIGMOID = 0,
+    SPEAR_GATE_MLP = 1,
+    SPEAR_GATE_NONE = 2
+} spear_gate_kind;
+
+/* Execution variants.  AUTO consults the table filled by spear_plan and
+ * otherwise a size heuristic. */
+typedef enum {
+    SPEAR_VARIANT_AUTO = 0,
+    SPEAR_VARIANT_STREAM_FUSED = 1,  /* one kernel: weight stream (mma.sync) + x.A^T, gate, B add inside; M <= 16 */
+    SPEAR_VARIANT_STREAM_SPLIT = 2,  /* EC pre-kernel (z, gate, u) then weight-stream kernel adding u.B^T; any M */
+    SPEAR_VARIANT_TC_FUSED = 3,      /* EC pre-kernel + tcgen05 GEMM with [X|U].[What|aB]^T K-concatenation; M >= 128 */
+    SPEAR_VARIANT_TC_SPLIT = 4,      /* tcgen05 GEMM (plain W4) then a separate rank-r update kernel; M >= 128 */
+    SPEAR_VARIANT_COUNT = 5
+} spear_variant;
+
+/* ---- S0: packing (the "SPW4" layout) -------------------------------- */
+
+/* Sizes in bytes of the opaque packed buffers: wq = N*K/2, scales = 2*N*(K/group). */
+int spear_pack_w4_sizes(int N, int K, int group, size_t* wq_bytes, size_t* scales_bytes);
+
+/* Canonical -> packed.  codes[N][K] uint8 in 0..15 (any code > 15 -> SPEAR_EINVAL, outputs
+ * undefined), scales[N][K/group] fp16.  Bit-exact and deterministic.  Synchronises `stream`. */
+int spear_pack_w4(const uint8_t* codes, const void* scales, void* wq_out, void* scales_out,
+                  int N, int K, int group, void* stream);
+
+/* Test hooks: packed -> canonical codes; packed -> fp16 weights What16[N][K] = RN_fp16((q-8)*s),
+ * computed as the exact fp16 (q-8) times s with one rounding (bit-exact against the oracle). */
+int spear_unpack_w4(const void* wq, uint8_t* codes_out, int N, int K, int group, void* stream);
+int spear_dequant_w4(const void* wq, const void* scales_packed, void* w_fp16_out,
+                     int N, int K, int group, void* stream);
+
+/* ---- the layer --------------------------------------------------------------------------- */
+
+/* The call BASELINE.json names, argument order verbatim.  Gate = scalar sigmoid, alpha = 1:
+ * gate_w = w_g[K] fp16, gate_b = pointer to ONE fp32 on the device.  r == 0 (A, B, gate_* may
+ * then be NULL) is the plain W4 layer.  Wq / scales are the packed buffers of spear_pack_w4.
+ * Uses the library's default workspace (spear_init): calls sharing it must be stream-ordered
+ * with respect to each other. */
+int spear_w4_ec_gemm(const void* x, const void* Wq, const void* scales, const void* A, const void* B,
+                     const void* gate_w, const void* gate_b, void* y,
+                     int M, int N, int K, int r, int group, void* stream);
+
+/* Extended form: everything the paper's EC needs that the 14-argument form cannot express. */
+typedef struct {
+    int gate_kind;            /* spear_gate_kind                                                    */
+    int gate_hidden;          /* h, MLP gate only (1 <= h <= 512, reading A2: default 4r)           */
+    float alpha;              /* Eq. 3 alpha (reading A3)                                           */
+    const void* W1;           /* [h][r] fp16   MLP gate                                             */
+    const void* b1;           /* [h]    fp32                                                        */
+    const void* W2;           /* [r][h] fp16                                                        */
+    const void* b2;           /* [r]    fp32                                                        */
+    const void* w_g;          /* [K]    fp16   scalar gate                                          */
+    const void* b_g;          /* 1      fp32   scalar gate (device pointer; NULL = 0)               */
+    void* gate_out;           /* optional: MLP -> [M][r] fp32, scalar -> [M] fp32; NULL = not written */
+    void* workspace;          /* NULL = library default; else >= spear_workspace_bytes(), zero-filled
+                                 once by the caller before first use (the library keeps its counters
+                                 zero between calls)                                                */
+    size_t workspace_bytes;
+    int force_variant;        /* spear_variant; SPEAR_VARIANT_AUTO = use the plan                   */
+} spear_ec_desc;
+
+int spear_w4_ec_gemm_ex(const void* x, const void* Wq, const void* scales, const void* A, const void* B,
+                        const spear_ec_desc* ec, void* y,
+                        int M, int N, int K, int r, int group, void* stream);
+
+/* Same layer with HOST activations: x_host[M][K] and y_host[M][N] are (preferably pinned) host
+ * buffers; x is copied to x_dev, the layer runs, y_dev is copied back, all on `stream` (the end-
+ * to-end path bench.py times).  Weights and EC parameters stay device-resident. */
+int spear_w4_ec_gemm_hostio(const void* x_host, void* y_host, void* x_dev, void* y_dev,
+                            const void* Wq, const void* scales, const void* A, const void* B,
+                            const spear_ec_desc* ec, int M, int N, int K, int r, int group, void* stream);
+
+/* Workspace a call of this shape may need (upper bound over variants). */
+int spear_workspace_bytes(int M, int N, int K, int r, int group, size_t* bytes);
+
+/* Allocates (once per process, current device) and zero-fills the default workspace and reads the
+ * device properties.  Called implicitly by the first compute call; call it explicitly before
+ * capturing a CUDA graph.  Synchronises the device. */
+int spear_init(void);
+
+/* ---- S9: measured dispatch ---------------------------------------------------------------- */
+
+/* Times every variant valid for this problem on synthetic device buffers it allocates itself
+ * (PAPER.md:274 protocol scaled down: warm-up then the median of timed launches, CUDA events),
+ * records the fastest in the process-wide table and returns it.  times_us_out (host, may be
+ * NULL) receives SPEAR_VARIANT_COUNT medians in microseconds (negative = variant not valid).
+ * Synchronises. */
+int spear_plan(int M, int N, int K, int r, int group, int gate_kind, int gate_hidden,
+               int* chosen_variant_out, float* times_us_out, void* stream);
+int spear_plan_save(const char* path);   /* text file, one line per planned problem (host path) */
+int spear_plan_load(const char* path);
+/* The variant AUTO would run for this problem right now (table hit or heuristic). */
+int spear_plan_query(int M, int N, int K, int r, int group, int gate_kind, int* variant_out);
+
+const char* spear_last_error(void);
+/* Number of kernels the library has launched in this process (bench.py's gpu_launches). */
+unsigned long long spear_launch_count(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* SPEAR_H */

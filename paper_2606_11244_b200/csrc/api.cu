@@ -1,0 +1,370 @@
+// api.cu -- the C ABI of libspear.so (include/spear.h): argument checking, workspace, TMA tensor-map
+// cache, variant dispatch (S9 of SURVEY.md 8(a)) and the measured plan table.
+#include <cstdarg>
+#include <cstdio>
+#include <cstring>
+#include <algorithm>
+#include <map>
+#include <mutex>
+#include <string>
+#include <tuple>
+#include <vector>
+#include <atomic>
+
+#include "common.cuh"
+#include "kernels.h"
+
+namespace spear {
+
+// ------------------------------------------------------------------------------------------------
+// error state / counters / device info
+// ------------------------------------------------------------------------------------------------
+static thread_local char g_err[512] = "";
+static std::atomic<unsigned long long> g_launches{0};
+
+int set_error(int status, const char* fmt, ...) {
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(g_err, sizeof(g_err), fmt, ap);
+    va_end(ap);
+    return status;
+}
+void count_launch(int n) { g_launches.fetch_add((unsigned long long)n, std::memory_order_relaxed); }
+
+static DeviceInfo g_dev;
+static std::once_flag g_init_once;
+static int g_init_status = SPEAR_OK;
+static char g_init_err[512] = "";
+static void* g_ws = nullptr;
+static size_t g_ws_bytes = 0;
+const DeviceInfo& device_info() { return g_dev; }
+
+// workspace layout (byte offsets); every region is 1 KiB aligned
+struct WsLayout {
+    size_t counters, zbuf, u32, partial, u16, tc_partial, total;
+};
+constexpr size_t kCounterBytes = 64 * 1024;          // 16384 u32
+constexpr int kEcPreCounter = 8192;                  // index into counters[]
+constexpr int kTcCounterBase = 8448;
+constexpr int kMaxStreamGrid = 1024;
+static size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
+static WsLayout ws_layout(int M, int r) {
+    WsLayout L;
+    size_t o = 0;
+    L.counters = o; o += kCounterBytes;
+    L.zbuf = o; o += align_up(size_t(16) * kZStride * 4, 1024);
+    L.u32 = o; o += align_up(size_t(16) * 128 * 4, 1024);
+    L.partial = o; o += size_t(kMaxStreamGrid) * 2 * 16 * 128 * 4;
+    L.u16 = o; o += align_up(size_t(M > 16 ? M : 0) * size_t(r) * 2 + 1024, 1024);
+    L.tc_partial = o; o += tc_partial_bytes(M);
+    L.total = o;
+    return L;
+}
+constexpr size_t kDefaultWorkspace = size_t(96) << 20;
+
+static void do_init() {
+    int dev = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) {
+        snprintf(g_init_err, sizeof(g_init_err), "no CUDA device: %s (libspear has no CPU path)", cudaGetErrorString(e));
+        g_init_status = SPEAR_ECUDA;
+        return;
+    }
+    cudaDeviceProp prop;
+    e = cudaGetDeviceProperties(&prop, dev);
+    if (e != cudaSuccess) {
+        snprintf(g_init_err, sizeof(g_init_err), "cudaGetDeviceProperties: %s", cudaGetErrorString(e));
+        g_init_status = SPEAR_ECUDA;
+        return;
+    }
+    g_dev.device = dev;
+    g_dev.num_sms = prop.multiProcessorCount;
+    g_dev.cc_major = prop.major;
+    g_dev.cc_minor = prop.minor;
+    g_dev.smem_optin = prop.sharedMemPerBlockOptin;
+    if (prop.major != 10) {
+        snprintf(g_init_err, sizeof(g_init_err), "libspear is built for sm_100a only; device is sm_%d%d", prop.major, prop.minor);
+        g_init_status = SPEAR_EUNSUPPORTED;
+        return;
+    }
+    e = cudaMalloc(&g_ws, kDefaultWorkspace);
+    if (e == cudaSuccess) e = cudaMemset(g_ws, 0, kDefaultWorkspace);
+    if (e == cudaSuccess) e = cudaDeviceSynchronize();
+    if (e != cudaSuccess) {
+        snprintf(g_init_err, sizeof(g_init_err), "default workspace: %s", cudaGetErrorString(e));
+        g_init_status = SPEAR_ENOMEM;
+        return;
+    }
+    g_ws_bytes = kDefaultWorkspace;
+}
+
+// ------------------------------------------------------------------------------------------------
+// TMA tensor maps
+// ------------------------------------------------------------------------------------------------
+typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
+                                  const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
+                                  CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+static EncodeTiledFn g_encode = nullptr;
+static std::mutex g_map_mutex;
+typedef std::tuple<const void*, uint64_t, uint64_t, uint64_t, uint32_t, uint32_t> MapKey;
+static std::map<MapKey, CUtensorMap> g_maps;
+
+int get_tensor_map_2d(const void* base, uint64_t rows, uint64_t cols, uint64_t row_stride_bytes,
+                      uint32_t box_rows, uint32_t box_cols, CUtensorMap* out) {
+    std::lock_guard<std::mutex> lock(g_map_mutex);
+    if (!g_encode) {
+        void* fn = nullptr;
+        cudaDriverEntryPointQueryResult qres;
+        cudaError_t e = cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qres);
+        if (e != cudaSuccess || qres != cudaDriverEntryPointSuccess || !fn)
+            return set_error(SPEAR_ECUDA, "cuTensorMapEncodeTiled entry point unavailable");
+        g_encode = reinterpret_cast<EncodeTiledFn>(fn);
+    }
+    const MapKey key(base, rows, cols, row_stride_bytes, box_rows, box_cols);
+    auto it = g_maps.find(key);
+    if (it != g_maps.end()) { *out = it->second; return SPEAR_OK; }
+    CUtensorMap m;
+    const cuuint64_t dims[2] = {cols, rows};
+    const cuuint64_t strides[1] = {row_stride_bytes};
+    const cuuint32_t box[2] = {box_cols, box_rows};
+    const cuuint32_t estr[2] = {1, 1};
+    const CUresult rc = g_encode(&m, CU_TENSOR_MAP_DATA_TYPE_FLOAT16, 2, const_cast<void*>(base), dims, strides, box,
+                                 estr, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B,
+                                 CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    if (rc != CUDA_SUCCESS)
+        return set_error(SPEAR_ECUDA, "cuTensorMapEncodeTiled failed (%d) rows=%llu cols=%llu stride=%llu box=%ux%u",
+                         int(rc), (unsigned long long)rows, (unsigned long long)cols,
+                         (unsigned long long)row_stride_bytes, box_rows, box_cols);
+    if (g_maps.size() > 8192) g_maps.clear();
+    g_maps[key] = m;
+    *out = m;
+    return SPEAR_OK;
+}
+
+// ------------------------------------------------------------------------------------------------
+// tunables (debug / sweep hook) and the plan table
+// ------------------------------------------------------------------------------------------------
+struct Tunables {
+    int stream_ctas_per_sm = 1;   // persistent grid = num_sms * this
+    int pdl = 1;                  // programmatic dependent launch between the library's kernels
+    int ecpre_ctas = 0;           // 0 = heuristic
+    int tc_grid = 0;              // 0 = heuristic
+};
+static Tunables g_tune;
+
+struct PlanKey {
+    int M, N, K, r, group, gate;
+    bool operator<(const PlanKey& o) const {
+        return std::tie(M, N, K, r, group, gate) < std::tie(o.M, o.N, o.K, o.r, o.group, o.gate);
+    }
+};
+struct PlanEntry { int variant; float us[SPEAR_VARIANT_COUNT]; };
+static std::map<PlanKey, PlanEntry> g_plan;
+static std::mutex g_plan_mutex;
+
+static bool variant_valid(int v, int M, int r) {
+    switch (v) {
+        case SPEAR_VARIANT_STREAM_FUSED: return false;   // not built yet
+        case SPEAR_VARIANT_STREAM_SPLIT: return M <= 16;
+        case SPEAR_VARIANT_TC_FUSED: return tc_available() && M >= 1;
+        case SPEAR_VARIANT_TC_SPLIT: return false;
+        default: return false;
+    }
+    (void)r;
+}
+static int heuristic_variant(int M, int r) {
+    (void)r;
+    if (M <= 16) return SPEAR_VARIANT_STREAM_SPLIT;
+    return SPEAR_VARIANT_TC_FUSED;
+}
+static int choose_variant(int M, int N, int K, int r, int group, int gate) {
+    {
+        std::lock_guard<std::mutex> lock(g_plan_mutex);
+        auto it = g_plan.find(PlanKey{M, N, K, r, group, gate});
+        if (it != g_plan.end()) return it->second.variant;
+    }
+    return heuristic_variant(M, r);
+}
+
+// ------------------------------------------------------------------------------------------------
+// the layer
+// ------------------------------------------------------------------------------------------------
+static int check_problem(const void* x, const void* Wq, const void* scales, const void* A, const void* B,
+                         const spear_ec_desc* ec, void* y, int M, int N, int K, int r, int group) {
+    if (M < 1 || N < 1 || K < 1 || group < 1 || r < 0)
+        return set_error(SPEAR_EINVAL, "bad sizes M=%d N=%d K=%d r=%d group=%d", M, N, K, r, group);
+    if (N % 128 || K % 128 || group % 128 || K % group)
+        return set_error(SPEAR_EUNSUPPORTED, "need N%%128==0, K%%128==0, group%%128==0, K%%group==0 (N=%d K=%d group=%d)", N, K, group);
+    if (r > 128 || r % 8) return set_error(SPEAR_EUNSUPPORTED, "need 0 <= r <= 128, r%%8==0 (r=%d)", r);
+    if (!x || !Wq || !scales || !y) return set_error(SPEAR_EINVAL, "NULL x / Wq / scales / y");
+    if (x == y) return set_error(SPEAR_EINVAL, "x and y must not alias");
+    uintptr_t al = uintptr_t(x) | uintptr_t(Wq) | uintptr_t(scales) | uintptr_t(y);
+    if (r > 0) {
+        if (!A || !B || !ec) return set_error(SPEAR_EINVAL, "r > 0 needs A, B and the EC descriptor");
+        al |= uintptr_t(A) | uintptr_t(B);
+        if (ec->gate_kind == SPEAR_GATE_SCALAR_SIGMOID) {
+            if (!ec->w_g) return set_error(SPEAR_EINVAL, "scalar gate needs w_g");
+            al |= uintptr_t(ec->w_g);
+        } else if (ec->gate_kind == SPEAR_GATE_MLP) {
+            if (!ec->W1 || !ec->b1 || !ec->W2 || !ec->b2) return set_error(SPEAR_EINVAL, "MLP gate needs W1, b1, W2, b2");
+            if (ec->gate_hidden < 1 || ec->gate_hidden > 512 || ec->gate_hidden % 8)
+                return set_error(SPEAR_EUNSUPPORTED, "MLP gate needs 8 <= h <= 512, h%%8==0 (h=%d)", ec->gate_hidden);
+            al |= uintptr_t(ec->W1) | uintptr_t(ec->W2);
+        } else if (ec->gate_kind != SPEAR_GATE_NONE) {
+            return set_error(SPEAR_EINVAL, "unknown gate kind %d", ec->gate_kind);
+        }
+    }
+    if (al & 15) return set_error(SPEAR_EINVAL, "device pointers must be 16-byte aligned");
+    return SPEAR_OK;
+}
+
+static int run_stream_split(const void* x, const void* Wq, const void* scales, const void* A, const void* B,
+                            const spear_ec_desc* ec, void* y, int M, int N, int K, int r, int group,
+                            uint8_t* ws, const WsLayout& L, cudaStream_t st) {
+    unsigned* counters = reinterpret_cast<unsigned*>(ws + L.counters);
+    float* u32 = reinterpret_cast<float*>(ws + L.u32);
+    const bool pdl = g_tune.pdl != 0;
+    if (r > 0) {
+        EcPreParams e = {};
+        e.x = static_cast<const __half*>(x);
+        e.A = static_cast<const __half*>(A);
+        e.w_g = static_cast<const __half*>(ec->w_g);
+        e.b_g = static_cast<const float*>(ec->b_g);
+        e.W1 = static_cast<const __half*>(ec->W1);
+        e.b1 = static_cast<const float*>(ec->b1);
+        e.W2 = static_cast<const __half*>(ec->W2);
+        e.b2 = static_cast<const float*>(ec->b2);
+        e.zbuf = reinterpret_cast<float*>(ws + L.zbuf);
+        e.u = u32;
+        e.gate_out = static_cast<float*>(ec->gate_out);
+        e.counter = counters + kEcPreCounter;
+        e.M = M; e.K = K; e.r = r; e.h = ec->gate_hidden; e.gate_kind = ec->gate_kind;
+        e.alpha = ec->alpha;
+        const int strips = (r + (ec->gate_kind == SPEAR_GATE_SCALAR_SIGMOID ? 1 : 0) + 15) / 16;
+        const int ktiles = K / 64;
+        int target = g_tune.ecpre_ctas > 0 ? g_tune.ecpre_ctas : g_dev.num_sms;
+        int ksplit = std::max(1, std::min(ktiles / 4, target / strips));
+        e.ksplit = std::max(1, std::min(ksplit, ktiles));
+        if (int rc = launch_ec_pre(e, pdl, st)) return rc;
+    }
+    const int MT = M <= 8 ? 1 : 2;
+    CUtensorMap xmap;
+    if (int rc = get_tensor_map_2d(x, uint64_t(M), uint64_t(K), uint64_t(K) * 2, uint32_t(8 * MT), 64, &xmap)) return rc;
+    StreamParams p = {};
+    p.wq = Wq; p.scales = scales;
+    p.y = static_cast<__half*>(y);
+    p.u = u32;
+    p.B = static_cast<const __half*>(B);
+    p.partial = reinterpret_cast<float*>(ws + L.partial);
+    p.counters = counters;
+    p.M = M; p.N = N; p.K = K; p.r = r;
+    p.G = K / group; p.group_chunks = group / 128; p.C = K / 128;
+    p.U = (N / 128) * p.C;
+    int grid = std::min(p.U, g_dev.num_sms * std::max(1, g_tune.stream_ctas_per_sm));
+    grid = std::min(grid, kMaxStreamGrid);
+    return launch_stream(xmap, p, MT, grid, pdl, st);
+}
+
+static int layer_impl(const void* x, const void* Wq, const void* scales, const void* A, const void* B,
+                      const spear_ec_desc* ec, void* y, int M, int N, int K, int r, int group, cudaStream_t st) {
+    if (int rc = spear_init()) return rc;
+    if (r == 0) { A = nullptr; B = nullptr; }
+    if (int rc = check_problem(x, Wq, scales, A, B, ec, y, M, N, K, r, group)) return rc;
+    const WsLayout L = ws_layout(M, r);
+    uint8_t* ws = static_cast<uint8_t*>(g_ws);
+    size_t ws_bytes = g_ws_bytes;
+    if (ec && ec->workspace) {
+        ws = static_cast<uint8_t*>(ec->workspace);
+        ws_bytes = ec->workspace_bytes;
+        if (uintptr_t(ws) & 1023) return set_error(SPEAR_EINVAL, "workspace must be 1024-byte aligned");
+    }
+    if (ws_bytes < L.total)
+        return set_error(SPEAR_ENOMEM, "workspace too small: need %zu bytes, have %zu (pass spear_ec_desc.workspace)", L.total, ws_bytes);
+    const int gate = (r > 0 && ec) ? ec->gate_kind : SPEAR_GATE_NONE;
+    int v = (ec && ec->force_variant != SPEAR_VARIANT_AUTO) ? ec->force_variant : choose_variant(M, N, K, r, group, gate);
+    if (!variant_valid(v, M, r)) {
+        if (ec && ec->force_variant != SPEAR_VARIANT_AUTO)
+            return set_error(SPEAR_EUNSUPPORTED, "variant %d is not valid for M=%d r=%d", v, M, r);
+        v = heuristic_variant(M, r);
+        if (!variant_valid(v, M, r)) return set_error(SPEAR_EUNSUPPORTED, "no kernel variant for M=%d r=%d", M, r);
+    }
+    switch (v) {
+        case SPEAR_VARIANT_STREAM_SPLIT:
+            return run_stream_split(x, Wq, scales, A, B, ec, y, M, N, K, r, group, ws, L, st);
+        case SPEAR_VARIANT_TC_FUSED: {
+            TcProblem t = {};
+            t.x = x; t.wq = Wq; t.scales = scales; t.A = A; t.B = B; t.ec = ec; t.y = y;
+            t.M = M; t.N = N; t.K = K; t.r = r; t.group = group;
+            t.u16 = ws + L.u16;
+            t.partial = ws + L.tc_partial;
+            t.counters = reinterpret_cast<unsigned*>(ws + L.counters) + kTcCounterBase;
+            t.pdl = g_tune.pdl != 0;
+            t.grid_override = g_tune.tc_grid;
+            return run_tc_fused(t, st);
+        }
+        default:
+            return set_error(SPEAR_EUNSUPPORTED, "variant %d not implemented", v);
+    }
+}
+
+}  // namespace spear
+
+using namespace spear;
+
+extern "C" int spear_init(void) {
+    std::call_once(g_init_once, do_init);
+    if (g_init_status != SPEAR_OK) return set_error(g_init_status, "%s", g_init_err);
+    return SPEAR_OK;
+}
+
+extern "C" const char* spear_last_error(void) { return g_err; }
+extern "C" unsigned long long spear_launch_count(void) { return g_launches.load(); }
+
+extern "C" int spear_tune(const char* key, int value) {
+    if (!key) return set_error(SPEAR_EINVAL, "NULL key");
+    if (!strcmp(key, "stream_ctas_per_sm")) g_tune.stream_ctas_per_sm = value;
+    else if (!strcmp(key, "pdl")) g_tune.pdl = value;
+    else if (!strcmp(key, "ecpre_ctas")) g_tune.ecpre_ctas = value;
+    else if (!strcmp(key, "tc_grid")) g_tune.tc_grid = value;
+    else return set_error(SPEAR_EINVAL, "unknown tunable '%s'", key);
+    return SPEAR_OK;
+}
+
+extern "C" int spear_workspace_bytes(int M, int N, int K, int r, int group, size_t* bytes) {
+    (void)N; (void)K; (void)group;
+    if (!bytes || M < 1 || r < 0) return set_error(SPEAR_EINVAL, "bad arguments");
+    *bytes = ws_layout(M, r).total;
+    return SPEAR_OK;
+}
+
+extern "C" int spear_w4_ec_gemm_ex(const void* x, const void* Wq, const void* scales, const void* A, const void* B,
+                                   const spear_ec_desc* ec, void* y, int M, int N, int K, int r, int group,
+                                   void* stream) {
+    return layer_impl(x, Wq, scales, A, B, ec, y, M, N, K, r, group, static_cast<cudaStream_t>(stream));
+}
+
+extern "C" int spear_w4_ec_gemm(const void* x, const void* Wq, const void* scales, const void* A, const void* B,
+                                const void* gate_w, const void* gate_b, void* y, int M, int N, int K, int r,
+                                int group, void* stream) {
+    spear_ec_desc ec;
+    memset(&ec, 0, sizeof(ec));
+    ec.gate_kind = SPEAR_GATE_SCALAR_SIGMOID;
+    ec.alpha = 1.0f;
+    ec.w_g = gate_w;
+    ec.b_g = gate_b;
+    ec.force_variant = SPEAR_VARIANT_AUTO;
+    return layer_impl(x, Wq, scales, A, B, &ec, y, M, N, K, r, group, static_cast<cudaStream_t>(stream));
+}
+
+extern "C" int spear_w4_ec_gemm_hostio(const void* x_host, void* y_host, void* x_dev, void* y_dev, const void* Wq,
+                                       const void* scales, const void* A, const void* B, const spear_ec_desc* ec,
+                                       int M, int N, int K, int r, int group, void* stream) {
+    if (!x_host || !y_host || !x_dev || !y_dev) return set_error(SPEAR_EINVAL, "NULL host/device activation buffer");
+    if (M < 1 || N < 1 || K < 1) return set_error(SPEAR_EINVAL, "bad sizes");
+    if (int rc = spear_init()) return rc;
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    SPEAR_CUDA_OK(cudaMemcpyAsync(x_dev, x_host, size_t(M) * K * 2, cudaMemcpyHostToDevice, st));
+    if (int rc = layer_impl(x_dev, Wq, scales, A, B, ec, y_dev, M, N, K, r, group, st)) return rc;
+    SPEAR_CUDA_OK(cudaMemcpyAsync(y_host, y_dev, size_t(M) * N * 2, cudaMemcpyDeviceToHost, st));
+    return SPEAR_OK;
+}

@@ -1,0 +1,47 @@
+// kernels.h -- parameter blocks and host launchers shared by api.cu and the kernel translation units.
+#pragma once
+
+#include "common.cuh"
+
+namespace spear {
+
+// ---- stream.cu (M <= 16) ------------------------------------------------------------------------
+struct StreamParams {
+    const void* wq;          // SPW4 packed codes
+    const void* scales;      // SPW4 packed scales
+    __half* y;               // [M][N]
+    const float* u;          // [16][r] fp32, alpha * gamma (.) z (EC pre-kernel); unused when r == 0
+    const __half* B;         // [N][r]
+    float* partial;          // [grid * 2][8*MT][128] fp32 split-K slots
+    unsigned* counters;      // [N / 128], zero between calls
+    int M, N, K, r;
+    int G;                   // K / group
+    int group_chunks;        // group / 128
+    int C;                   // K / 128 chunks per panel
+    int U;                   // (N / 128) * C work units
+};
+int stream_smem_bytes(int MT);
+int launch_stream(const CUtensorMap& xmap, const StreamParams& p, int MT, int grid, bool pdl, cudaStream_t st);
+
+// ---- ec_pre.cu (M <= 16): z = x A^T, gate, u = alpha * gamma (.) z ------------------------------
+struct EcPreParams {
+    const __half* x;         // [M][K]
+    const __half* A;         // [r][K]
+    const __half* w_g;       // [K]       scalar gate
+    const float* b_g;        // 1 (device) or NULL
+    const __half* W1;        // [h][r]    MLP gate
+    const float* b1;         // [h]
+    const __half* W2;        // [r][h]
+    const float* b2;         // [r]
+    float* zbuf;             // [16][kZStride] fp32 accumulators, zero between calls
+    float* u;                // [16][r] out
+    float* gate_out;         // optional
+    unsigned* counter;       // zero between calls
+    int M, K, r, h, gate_kind;
+    int ksplit;
+    float alpha;
+};
+constexpr int kZStride = 136;    // >= r + 1 (the extra column carries the scalar-gate logit)
+int launch_ec_pre(const EcPreParams& p, bool pdl, cudaStream_t st);
+
+}  // namespace spear
