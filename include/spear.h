@@ -142,6 +142,10 @@ int spear_plan_load(const char* path);
 /* The variant AUTO would run for this problem right now (table hit or heuristic). */
 int spear_plan_query(int M, int N, int K, int r, int group, int gate_kind, int* variant_out);
 
+/* Debug / sweep hook: sets a launch tunable ("stream_ctas_per_sm", "pdl", "ecpre_ctas", "tc_grid").
+ * Host-only, process-wide, not thread-safe against concurrent compute calls. */
+int spear_tune(const char* key, int value);
+
 const char* spear_last_error(void);
 /* Number of kernels the library has launched in this process (bench.py's gpu_launches). */
 unsigned long long spear_launch_count(void);

@@ -41,22 +41,20 @@ const DeviceInfo& device_info() { return g_dev; }
 
 // workspace layout (byte offsets); every region is 1 KiB aligned
 struct WsLayout {
-    size_t counters, zbuf, u32, partial, u16, tc_partial, total;
+    size_t counters, zbuf, u32, partial, u16, total;
 };
 constexpr size_t kCounterBytes = 64 * 1024;          // 16384 u32
 constexpr int kEcPreCounter = 8192;                  // index into counters[]
-constexpr int kTcCounterBase = 8448;
 constexpr int kMaxStreamGrid = 1024;
 static size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
 static WsLayout ws_layout(int M, int r) {
     WsLayout L;
     size_t o = 0;
     L.counters = o; o += kCounterBytes;
-    L.zbuf = o; o += align_up(size_t(16) * kZStride * 4, 1024);
+    L.zbuf = o; o += align_up(size_t(M > 16 ? M : 16) * kZStride * 4, 1024);
     L.u32 = o; o += align_up(size_t(16) * 128 * 4, 1024);
     L.partial = o; o += size_t(kMaxStreamGrid) * 2 * 16 * 128 * 4;
-    L.u16 = o; o += align_up(size_t(M > 16 ? M : 0) * size_t(r) * 2 + 1024, 1024);
-    L.tc_partial = o; o += tc_partial_bytes(M);
+    L.u16 = o; o += align_up(size_t(M) * size_t(r) * 2 + 1024, 1024);
     L.total = o;
     return L;
 }
@@ -265,6 +263,42 @@ static int run_stream_split(const void* x, const void* Wq, const void* scales, c
     return launch_stream(xmap, p, MT, grid, pdl, st);
 }
 
+// M > 16 (also valid for any M): EC pre-pass (z, gate, u16) then the tcgen05 GEMM whose K loop is
+// extended by ceil(r/64) blocks [X | U] . [What | B]^T  (SURVEY.md section 7 "Prefill EC fold").
+static int run_tc_fused(const void* x, const void* Wq, const void* scales, const void* A, const void* B,
+                        const spear_ec_desc* ec, void* y, int M, int N, int K, int r, int group,
+                        uint8_t* ws, const WsLayout& L, cudaStream_t st) {
+    const bool pdl = g_tune.pdl != 0;
+    if (r > 0) {
+        EcBigParams e = {};
+        e.x = static_cast<const __half*>(x);
+        e.A = static_cast<const __half*>(A);
+        e.w_g = static_cast<const __half*>(ec->w_g);
+        e.b_g = static_cast<const float*>(ec->b_g);
+        e.W1 = static_cast<const __half*>(ec->W1);
+        e.b1 = static_cast<const float*>(ec->b1);
+        e.W2 = static_cast<const __half*>(ec->W2);
+        e.b2 = static_cast<const float*>(ec->b2);
+        e.zbuf = reinterpret_cast<float*>(ws + L.zbuf);
+        e.u16 = reinterpret_cast<__half*>(ws + L.u16);
+        e.gate_out = static_cast<float*>(ec->gate_out);
+        e.M = M; e.K = K; e.r = r; e.h = ec->gate_hidden; e.gate_kind = ec->gate_kind;
+        e.alpha = ec->alpha;
+        const int mtiles = (M + 63) / 64, ktiles = K / 64;
+        int target = (g_tune.ecpre_ctas > 0 ? g_tune.ecpre_ctas : 2 * g_dev.num_sms);
+        int ksplit = std::max(1, target / mtiles);
+        e.ksplit = std::max(1, std::min(ksplit, ktiles / 4));
+        if (int rc = launch_ec_big(e, pdl, st)) return rc;
+    }
+    TcProblem t = {};
+    t.x = x; t.wq = Wq; t.scales = scales; t.B = B; t.y = y;
+    t.u16 = r > 0 ? ws + L.u16 : nullptr;
+    t.M = M; t.N = N; t.K = K; t.r = r; t.group = group;
+    t.pdl = pdl;
+    t.grid_override = g_tune.tc_grid;
+    return run_tc(t, st);
+}
+
 static int layer_impl(const void* x, const void* Wq, const void* scales, const void* A, const void* B,
                       const spear_ec_desc* ec, void* y, int M, int N, int K, int r, int group, cudaStream_t st) {
     if (int rc = spear_init()) return rc;
@@ -291,17 +325,8 @@ static int layer_impl(const void* x, const void* Wq, const void* scales, const v
     switch (v) {
         case SPEAR_VARIANT_STREAM_SPLIT:
             return run_stream_split(x, Wq, scales, A, B, ec, y, M, N, K, r, group, ws, L, st);
-        case SPEAR_VARIANT_TC_FUSED: {
-            TcProblem t = {};
-            t.x = x; t.wq = Wq; t.scales = scales; t.A = A; t.B = B; t.ec = ec; t.y = y;
-            t.M = M; t.N = N; t.K = K; t.r = r; t.group = group;
-            t.u16 = ws + L.u16;
-            t.partial = ws + L.tc_partial;
-            t.counters = reinterpret_cast<unsigned*>(ws + L.counters) + kTcCounterBase;
-            t.pdl = g_tune.pdl != 0;
-            t.grid_override = g_tune.tc_grid;
-            return run_tc_fused(t, st);
-        }
+        case SPEAR_VARIANT_TC_FUSED:
+            return run_tc_fused(x, Wq, scales, A, B, ec, y, M, N, K, r, group, ws, L, st);
         default:
             return set_error(SPEAR_EUNSUPPORTED, "variant %d not implemented", v);
     }
@@ -366,5 +391,154 @@ extern "C" int spear_w4_ec_gemm_hostio(const void* x_host, void* y_host, void* x
     SPEAR_CUDA_OK(cudaMemcpyAsync(x_dev, x_host, size_t(M) * K * 2, cudaMemcpyHostToDevice, st));
     if (int rc = layer_impl(x_dev, Wq, scales, A, B, ec, y_dev, M, N, K, r, group, st)) return rc;
     SPEAR_CUDA_OK(cudaMemcpyAsync(y_host, y_dev, size_t(M) * N * 2, cudaMemcpyDeviceToHost, st));
+    return SPEAR_OK;
+}
+
+// ------------------------------------------------------------------------------------------------
+// S9: measured dispatch (PAPER.md:181-193 phase-aware dispatch, :231 offline latency table; here the
+// table is measured per problem instead of fixed per phase -- north_star (4)).
+// ------------------------------------------------------------------------------------------------
+namespace spear {
+__global__ void fill_pattern_kernel(uint32_t* p, size_t n, uint32_t mul, uint32_t andm, uint32_t orm) {
+    for (size_t i = blockIdx.x * size_t(blockDim.x) + threadIdx.x; i < n; i += size_t(gridDim.x) * blockDim.x)
+        p[i] = ((uint32_t(i) * mul + 0x9e3779b9u) & andm) | orm;
+}
+struct DevBuf {
+    void* p = nullptr;
+    ~DevBuf() { if (p) cudaFree(p); }
+    cudaError_t alloc(size_t bytes) { return cudaMalloc(&p, bytes < 16 ? 16 : bytes); }
+};
+static void fill(void* p, size_t bytes, uint32_t mul, uint32_t andm, uint32_t orm, cudaStream_t st) {
+    fill_pattern_kernel<<<296, 256, 0, st>>>(static_cast<uint32_t*>(p), bytes / 4, mul, andm, orm);
+}
+}  // namespace spear
+
+extern "C" int spear_plan(int M, int N, int K, int r, int group, int gate_kind, int gate_hidden,
+                          int* chosen_variant_out, float* times_us_out, void* stream) {
+    if (int rc = spear_init()) return rc;
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    if (M < 1 || N % 128 || K % 128 || group % 128 || K % group || r < 0 || r > 128 || r % 8)
+        return set_error(SPEAR_EUNSUPPORTED, "spear_plan: unsupported problem");
+    const int G = K / group;
+    const int h = gate_kind == SPEAR_GATE_MLP ? (gate_hidden > 0 ? gate_hidden : 4 * r) : 0;
+    DevBuf x, wq, sc, A, B, y, wg, bg, W1, b1, W2, b2;
+    // finite, small fp16 patterns: 0x2xxx..0x2fff ~ [0.008, 0.12]; codes any nibble
+    if (x.alloc(size_t(M) * K * 2) || wq.alloc(size_t(N) * K / 2) || sc.alloc(size_t(N) * G * 2) ||
+        y.alloc(size_t(M) * N * 2) || A.alloc(size_t(r) * K * 2) || B.alloc(size_t(N) * r * 2) ||
+        wg.alloc(size_t(K) * 2) || bg.alloc(16) || W1.alloc(size_t(h) * r * 2) || b1.alloc(size_t(h) * 4) ||
+        W2.alloc(size_t(r) * h * 2) || b2.alloc(size_t(r) * 4))
+        return set_error(SPEAR_ENOMEM, "spear_plan: cudaMalloc failed");
+    fill(x.p, size_t(M) * K * 2, 2654435761u, 0x0fff0fffu, 0x20002000u, st);
+    fill(wq.p, size_t(N) * K / 2, 2246822519u, 0xffffffffu, 0u, st);
+    fill(sc.p, size_t(N) * G * 2, 3266489917u, 0x03ff03ffu, 0x20002000u, st);
+    if (r > 0) {
+        fill(A.p, size_t(r) * K * 2, 668265263u, 0x0fff0fffu, 0x20002000u, st);
+        fill(B.p, size_t(N) * r * 2, 374761393u, 0x0fff0fffu, 0x20002000u, st);
+        fill(wg.p, size_t(K) * 2, 1103515245u, 0x0fff0fffu, 0x20002000u, st);
+        if (h) {
+            fill(W1.p, size_t(h) * r * 2, 12345u, 0x0fff0fffu, 0x20002000u, st);
+            fill(W2.p, size_t(r) * h * 2, 54321u, 0x0fff0fffu, 0x20002000u, st);
+            cudaMemsetAsync(b1.p, 0, size_t(h) * 4, st);
+            cudaMemsetAsync(b2.p, 0, size_t(r) * 4, st);
+        }
+    }
+    cudaMemsetAsync(bg.p, 0, 16, st);
+    spear_ec_desc ec;
+    memset(&ec, 0, sizeof(ec));
+    ec.gate_kind = gate_kind; ec.gate_hidden = h; ec.alpha = 1.0f;
+    ec.W1 = W1.p; ec.b1 = b1.p; ec.W2 = W2.p; ec.b2 = b2.p; ec.w_g = wg.p; ec.b_g = bg.p;
+    // protocol of PAPER.md:274 (200 warm-up + 500 timed, median), scaled down for long kernels
+    const double flops = 2.0 * M * N * K;
+    int warm = 200, iters = 500;
+    if (flops > 2e11) { warm = 3; iters = 11; } else if (flops > 1e10) { warm = 10; iters = 51; }
+    PlanEntry ent;
+    ent.variant = -1;
+    float best = 1e30f;
+    cudaEvent_t e0, e1;
+    SPEAR_CUDA_OK(cudaEventCreate(&e0));
+    SPEAR_CUDA_OK(cudaEventCreate(&e1));
+    std::vector<float> t(iters);
+    int status = SPEAR_OK;
+    for (int v = 0; v < SPEAR_VARIANT_COUNT && status == SPEAR_OK; ++v) {
+        ent.us[v] = -1.f;
+        if (!variant_valid(v, M, r)) continue;
+        ec.force_variant = v;
+        for (int i = 0; i < warm + iters && status == SPEAR_OK; ++i) {
+            if (i >= warm) cudaEventRecord(e0, st);
+            status = spear_w4_ec_gemm_ex(x.p, wq.p, sc.p, A.p, B.p, &ec, y.p, M, N, K, r, group, st);
+            if (i >= warm) {
+                cudaEventRecord(e1, st);
+                if (cudaEventSynchronize(e1) != cudaSuccess) { status = set_error(SPEAR_ECUDA, "spear_plan: timing failed: %s", cudaGetErrorString(cudaGetLastError())); break; }
+                cudaEventElapsedTime(&t[i - warm], e0, e1);
+            }
+        }
+        if (status != SPEAR_OK) break;
+        std::sort(t.begin(), t.end());
+        ent.us[v] = t[iters / 2] * 1000.f;
+        if (ent.us[v] < best) { best = ent.us[v]; ent.variant = v; }
+    }
+    cudaEventDestroy(e0);
+    cudaEventDestroy(e1);
+    if (status != SPEAR_OK) return status;
+    if (ent.variant < 0) return set_error(SPEAR_EUNSUPPORTED, "spear_plan: no valid variant");
+    {
+        std::lock_guard<std::mutex> lock(g_plan_mutex);
+        g_plan[PlanKey{M, N, K, r, group, r > 0 ? gate_kind : SPEAR_GATE_NONE}] = ent;
+    }
+    if (chosen_variant_out) *chosen_variant_out = ent.variant;
+    if (times_us_out) for (int v = 0; v < SPEAR_VARIANT_COUNT; ++v) times_us_out[v] = ent.us[v];
+    return SPEAR_OK;
+}
+
+extern "C" int spear_plan_query(int M, int N, int K, int r, int group, int gate_kind, int* variant_out) {
+    if (!variant_out) return set_error(SPEAR_EINVAL, "NULL variant_out");
+    int v = choose_variant(M, N, K, r, group, r > 0 ? gate_kind : SPEAR_GATE_NONE);
+    if (!variant_valid(v, M, r)) v = heuristic_variant(M, r);
+    *variant_out = v;
+    return SPEAR_OK;
+}
+
+extern "C" int spear_plan_save(const char* path) {
+    if (!path) return set_error(SPEAR_EINVAL, "NULL path");
+    FILE* f = fopen(path, "w");
+    if (!f) return set_error(SPEAR_EINVAL, "cannot open %s for writing", path);
+    std::lock_guard<std::mutex> lock(g_plan_mutex);
+    fprintf(f, "# spear plan v1: M N K r group gate variant us[%d]\n", int(SPEAR_VARIANT_COUNT));
+    for (const auto& kv : g_plan) {
+        fprintf(f, "%d %d %d %d %d %d %d", kv.first.M, kv.first.N, kv.first.K, kv.first.r, kv.first.group,
+                kv.first.gate, kv.second.variant);
+        for (int v = 0; v < SPEAR_VARIANT_COUNT; ++v) fprintf(f, " %.3f", kv.second.us[v]);
+        fprintf(f, "\n");
+    }
+    fclose(f);
+    return SPEAR_OK;
+}
+
+extern "C" int spear_plan_load(const char* path) {
+    if (!path) return set_error(SPEAR_EINVAL, "NULL path");
+    FILE* f = fopen(path, "r");
+    if (!f) return set_error(SPEAR_EINVAL, "cannot open %s", path);
+    char line[1024];
+    int n_loaded = 0;
+    std::lock_guard<std::mutex> lock(g_plan_mutex);
+    while (fgets(line, sizeof(line), f)) {
+        if (line[0] == '#' || line[0] == '\n') continue;
+        PlanKey k; PlanEntry e;
+        int off = 0;
+        if (sscanf(line, "%d %d %d %d %d %d %d%n", &k.M, &k.N, &k.K, &k.r, &k.group, &k.gate, &e.variant, &off) != 7) {
+            fclose(f);
+            return set_error(SPEAR_EINVAL, "%s: malformed line", path);
+        }
+        const char* q = line + off;
+        for (int v = 0; v < SPEAR_VARIANT_COUNT; ++v) {
+            int adv = 0;
+            if (sscanf(q, "%f%n", &e.us[v], &adv) != 1) { e.us[v] = -1.f; break; }
+            q += adv;
+        }
+        if (e.variant <= 0 || e.variant >= SPEAR_VARIANT_COUNT) { fclose(f); return set_error(SPEAR_EINVAL, "%s: bad variant", path); }
+        g_plan[k] = e;
+        ++n_loaded;
+    }
+    fclose(f);
     return SPEAR_OK;
 }

@@ -37,6 +37,76 @@ __device__ __forceinline__ void load_x32(const __half* row, int col, uint32_t (&
     }
 }
 
+// S5 + S6 for up to 16 tokens whose fully reduced z rows sit in zs[m][0..r) (zs[m][r] = scalar-gate logit):
+//   MLP    gamma = 1 + tanh(W2 relu(W1 z + b1) + b2)
+//   scalar gamma = sigmoid(x . w_g + b)                  BASELINE.json configs (reading A1)
+//   none   gamma = 1                                     PAPER.md:96 (Eq. 2)
+// u = alpha * gamma (.) z goes to u32[m][r] (fp32, decode path) or u16[m_base + m][r] (fp16, tcgen05 path).
+struct GateArgs {
+    int gate_kind, r, h;
+    float alpha;
+    const float* b_g;
+    const __half* W1; const float* b1; const __half* W2; const float* b2;
+    float* u32; __half* u16; float* gate_out;
+};
+__device__ __forceinline__ void put_u(const GateArgs& ga, int m, int m_base, int j, float v) {
+    if (ga.u16) ga.u16[size_t(m_base + m) * ga.r + j] = __float2half_rn(v);
+    else ga.u32[m * ga.r + j] = v;
+}
+__device__ void apply_gate(const GateArgs& ga, float (*zs)[kZStride], float (*hid)[512], int m_count,
+                           int m_base, int tid, int nthreads) {
+    const int r = ga.r;
+    if (ga.gate_kind == SPEAR_GATE_SCALAR_SIGMOID) {
+        const float bias = ga.b_g ? *ga.b_g : 0.f;
+        for (int o = tid; o < m_count * r; o += nthreads) {
+            const int m = o / r, j = o - m * r;
+            const float gam = 1.f / (1.f + expf(-(zs[m][r] + bias)));
+            put_u(ga, m, m_base, j, ga.alpha * gam * zs[m][j]);
+            if (ga.gate_out && j == 0) ga.gate_out[m_base + m] = gam;
+        }
+    } else if (ga.gate_kind == SPEAR_GATE_MLP) {
+        const int h = ga.h;
+        for (int i = tid; i < h; i += nthreads) {
+            float a[16];
+#pragma unroll
+            for (int m = 0; m < 16; ++m) a[m] = 0.f;
+            const __half* w1 = ga.W1 + size_t(i) * r;
+            for (int j = 0; j < r; ++j) {
+                const float w = __half2float(w1[j]);
+#pragma unroll
+                for (int m = 0; m < 16; ++m) a[m] = fmaf(w, zs[m][j], a[m]);
+            }
+            const float bb = ga.b1[i];
+#pragma unroll
+            for (int m = 0; m < 16; ++m) hid[m][i] = fmaxf(a[m] + bb, 0.f);
+        }
+        __syncthreads();
+        for (int j = tid; j < r; j += nthreads) {
+            float a[16];
+#pragma unroll
+            for (int m = 0; m < 16; ++m) a[m] = 0.f;
+            const __half* w2 = ga.W2 + size_t(j) * h;
+            for (int i = 0; i < h; ++i) {
+                const float w = __half2float(w2[i]);
+#pragma unroll
+                for (int m = 0; m < 16; ++m) a[m] = fmaf(w, hid[m][i], a[m]);
+            }
+            const float bb = ga.b2[j];
+            for (int m = 0; m < m_count; ++m) {
+                const float gam = 1.f + tanhf(a[m] + bb);
+                put_u(ga, m, m_base, j, ga.alpha * gam * zs[m][j]);
+                if (ga.gate_out) ga.gate_out[size_t(m_base + m) * r + j] = gam;
+            }
+        }
+    } else {
+        for (int o = tid; o < m_count * r; o += nthreads) {
+            const int m = o / r, j = o - m * r;
+            put_u(ga, m, m_base, j, ga.alpha * zs[m][j]);
+        }
+    }
+}
+
+
 __global__ void __launch_bounds__(128) ec_pre_kernel(const EcPreParams p) {
     __shared__ float red[4][16][17];
     __shared__ float zs[16][kZStride];
@@ -109,55 +179,11 @@ __global__ void __launch_bounds__(128) ec_pre_kernel(const EcPreParams p) {
         p.zbuf[m * kZStride + rho] = 0.f;
     }
     __syncthreads();
-    const int r = p.r;
-    if (p.gate_kind == SPEAR_GATE_SCALAR_SIGMOID) {
-        const float bias = p.b_g ? *p.b_g : 0.f;
-        for (int o = threadIdx.x; o < p.M * r; o += 128) {
-            const int m = o / r, j = o - m * r;
-            const float gam = 1.f / (1.f + expf(-(zs[m][r] + bias)));
-            p.u[m * r + j] = p.alpha * gam * zs[m][j];
-            if (p.gate_out && j == 0) p.gate_out[m] = gam;
-        }
-    } else if (p.gate_kind == SPEAR_GATE_MLP) {
-        const int h = p.h;
-        for (int i = threadIdx.x; i < h; i += 128) {
-            float a[16];
-#pragma unroll
-            for (int m = 0; m < 16; ++m) a[m] = 0.f;
-            const __half* w1 = p.W1 + size_t(i) * r;
-            for (int j = 0; j < r; ++j) {
-                const float w = __half2float(w1[j]);
-#pragma unroll
-                for (int m = 0; m < 16; ++m) a[m] = fmaf(w, zs[m][j], a[m]);
-            }
-            const float bb = p.b1[i];
-#pragma unroll
-            for (int m = 0; m < 16; ++m) hid[m][i] = fmaxf(a[m] + bb, 0.f);
-        }
-        __syncthreads();
-        for (int j = threadIdx.x; j < r; j += 128) {
-            float a[16];
-#pragma unroll
-            for (int m = 0; m < 16; ++m) a[m] = 0.f;
-            const __half* w2 = p.W2 + size_t(j) * h;
-            for (int i = 0; i < h; ++i) {
-                const float w = __half2float(w2[i]);
-#pragma unroll
-                for (int m = 0; m < 16; ++m) a[m] = fmaf(w, hid[m][i], a[m]);
-            }
-            const float bb = p.b2[j];
-            for (int m = 0; m < p.M; ++m) {
-                const float gam = 1.f + tanhf(a[m] + bb);
-                p.u[m * r + j] = p.alpha * gam * zs[m][j];
-                if (p.gate_out) p.gate_out[m * r + j] = gam;
-            }
-        }
-    } else {
-        for (int o = threadIdx.x; o < p.M * r; o += 128) {
-            const int m = o / r, j = o - m * r;
-            p.u[m * r + j] = p.alpha * zs[m][j];
-        }
-    }
+    GateArgs ga;
+    ga.gate_kind = p.gate_kind; ga.r = p.r; ga.h = p.h; ga.alpha = p.alpha; ga.b_g = p.b_g;
+    ga.W1 = p.W1; ga.b1 = p.b1; ga.W2 = p.W2; ga.b2 = p.b2;
+    ga.u32 = p.u; ga.u16 = nullptr; ga.gate_out = p.gate_out;
+    apply_gate(ga, zs, hid, p.M, 0, threadIdx.x, 128);
 }
 
 int launch_ec_pre(const EcPreParams& p, bool pdl, cudaStream_t st) {
@@ -175,6 +201,121 @@ int launch_ec_pre(const EcPreParams& p, bool pdl, cudaStream_t st) {
     cfg.numAttrs = 1;
     SPEAR_CUDA_OK(cudaLaunchKernelEx(&cfg, ec_pre_kernel, p));
     count_launch();
+    return SPEAR_OK;
+}
+
+// ------------------------------------------------------------------------------------------------
+// M > 16: z = x [A; w_g]^T as a split-K mma.sync GEMM (tokens are the 16-row operand here), then a
+// gate kernel per 16 tokens.  Cost is r/N of the main GEMM (SURVEY.md section 7 "Prefill EC fold").
+// ------------------------------------------------------------------------------------------------
+template <int NT>   // NT = number of 8-row tiles of [A; w_g] (rows beyond r [+1] read as zero)
+__global__ void __launch_bounds__(128) ec_big_z_kernel(const EcBigParams p) {
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int g = lane >> 2, t = lane & 3;
+    const bool scalar = (p.gate_kind == SPEAR_GATE_SCALAR_SIGMOID);
+    const int rows_total = p.r + (scalar ? 1 : 0);
+    const int m0 = blockIdx.x * 64 + warp * 16;
+    pdl_launch_dependents();
+    if (m0 >= p.M) { pdl_wait(); return; }
+    const __half* px0 = (m0 + g) < p.M ? p.x + size_t(m0 + g) * p.K : nullptr;
+    const __half* px1 = (m0 + g + 8) < p.M ? p.x + size_t(m0 + g + 8) * p.K : nullptr;
+    const __half* pa[NT];
+#pragma unroll
+    for (int nt = 0; nt < NT; ++nt) {
+        const int rho = nt * 8 + g;
+        pa[nt] = rho < p.r ? p.A + size_t(rho) * p.K : (rho == p.r && scalar ? p.w_g : nullptr);
+    }
+    const int ktiles = p.K >> 6;
+    const int kt_begin = int((long long)blockIdx.y * ktiles / p.ksplit);
+    const int kt_end = int((long long)(blockIdx.y + 1) * ktiles / p.ksplit);
+    float acc[NT][4];
+#pragma unroll
+    for (int nt = 0; nt < NT; ++nt) acc[nt][0] = acc[nt][1] = acc[nt][2] = acc[nt][3] = 0.f;
+    pdl_wait();
+    for (int kt = kt_begin; kt < kt_end; ++kt) {
+        const int col = kt * 64 + 16 * t;
+        uint32_t x0l[4], x0h[4], x1l[4], x1h[4];
+        load_x32(px0, col, x0l, x0h);
+        load_x32(px1, col, x1l, x1h);
+#pragma unroll
+        for (int nt = 0; nt < NT; ++nt) {
+            uint32_t al[4], ah[4];
+            load_row32(pa[nt], col, al, ah);
+#pragma unroll
+            for (int jj = 0; jj < 4; ++jj)
+                mma_m16n8k16(acc[nt], x0l[jj], x1l[jj], x0h[jj], x1h[jj], al[jj], ah[jj]);
+        }
+    }
+    // C fragment: rows = tokens g, g+8; columns = EC rows nt*8 + 2t, +1
+#pragma unroll
+    for (int nt = 0; nt < NT; ++nt) {
+        const int rho = nt * 8 + 2 * t;
+        if (m0 + g < p.M) {
+            if (rho < rows_total) atomicAdd(p.zbuf + size_t(m0 + g) * kZStride + rho, acc[nt][0]);
+            if (rho + 1 < rows_total) atomicAdd(p.zbuf + size_t(m0 + g) * kZStride + rho + 1, acc[nt][1]);
+        }
+        if (m0 + g + 8 < p.M) {
+            if (rho < rows_total) atomicAdd(p.zbuf + size_t(m0 + g + 8) * kZStride + rho, acc[nt][2]);
+            if (rho + 1 < rows_total) atomicAdd(p.zbuf + size_t(m0 + g + 8) * kZStride + rho + 1, acc[nt][3]);
+        }
+    }
+}
+
+__global__ void __launch_bounds__(128) ec_big_gate_kernel(const EcBigParams p) {
+    __shared__ float zs[16][kZStride];
+    __shared__ float hid[16][512];
+    const int m_base = blockIdx.x * 16;
+    const int m_count = min(16, p.M - m_base);
+    const bool scalar = (p.gate_kind == SPEAR_GATE_SCALAR_SIGMOID);
+    const int rows_total = p.r + (scalar ? 1 : 0);
+    pdl_launch_dependents();
+    pdl_wait();
+    for (int o = threadIdx.x; o < 16 * rows_total; o += 128) {
+        const int m = o / rows_total, rho = o - m * rows_total;
+        float v = 0.f;
+        if (m < m_count) {
+            float* zp = p.zbuf + size_t(m_base + m) * kZStride + rho;
+            v = __ldcg(zp);
+            *zp = 0.f;                    // the workspace is left zero for the next call
+        }
+        zs[m][rho] = v;
+    }
+    __syncthreads();
+    GateArgs ga;
+    ga.gate_kind = p.gate_kind; ga.r = p.r; ga.h = p.h; ga.alpha = p.alpha; ga.b_g = p.b_g;
+    ga.W1 = p.W1; ga.b1 = p.b1; ga.W2 = p.W2; ga.b2 = p.b2;
+    ga.u32 = nullptr; ga.u16 = p.u16; ga.gate_out = p.gate_out;
+    apply_gate(ga, zs, hid, m_count, m_base, threadIdx.x, 128);
+}
+
+template <int NT>
+static int launch_ec_big_z(const EcBigParams& p, cudaLaunchConfig_t& cfg) {
+    SPEAR_CUDA_OK(cudaLaunchKernelEx(&cfg, ec_big_z_kernel<NT>, p));
+    return SPEAR_OK;
+}
+
+int launch_ec_big(const EcBigParams& p, bool pdl, cudaStream_t st) {
+    const bool scalar = (p.gate_kind == SPEAR_GATE_SCALAR_SIGMOID);
+    const int nt = (p.r + (scalar ? 1 : 0) + 7) / 8;
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3((p.M + 63) / 64, p.ksplit);
+    cfg.blockDim = dim3(128);
+    cfg.stream = st;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr[0].val.programmaticStreamSerializationAllowed = pdl ? 1 : 0;
+    cfg.attrs = attr;
+    cfg.numAttrs = 1;
+    int rc;
+    if (nt <= 3) rc = launch_ec_big_z<3>(p, cfg);
+    else if (nt <= 5) rc = launch_ec_big_z<5>(p, cfg);
+    else if (nt <= 9) rc = launch_ec_big_z<9>(p, cfg);
+    else if (nt <= 13) rc = launch_ec_big_z<13>(p, cfg);
+    else rc = launch_ec_big_z<17>(p, cfg);
+    if (rc) return rc;
+    cfg.gridDim = dim3((p.M + 15) / 16);
+    SPEAR_CUDA_OK(cudaLaunchKernelEx(&cfg, ec_big_gate_kernel, p));
+    count_launch(2);
     return SPEAR_OK;
 }
 

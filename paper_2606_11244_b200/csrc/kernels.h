@@ -44,4 +44,31 @@ struct EcPreParams {
 constexpr int kZStride = 136;    // >= r + 1 (the extra column carries the scalar-gate logit)
 int launch_ec_pre(const EcPreParams& p, bool pdl, cudaStream_t st);
 
+// ---- ec_big.cu (M > 16): z = x [A; w_g]^T (split-K, fp32 red.add), then gate -> u16 = fp16(alpha*gamma(.)z)
+struct EcBigParams {
+    const __half* x;         // [M][K]
+    const __half* A;         // [r][K]
+    const __half* w_g;       // [K] or NULL
+    const float* b_g;
+    const __half* W1; const float* b1; const __half* W2; const float* b2;
+    float* zbuf;             // [M][kZStride] fp32, zero between calls
+    __half* u16;             // [M][r] out
+    float* gate_out;         // optional
+    int M, K, r, h, gate_kind;
+    int ksplit;
+    float alpha;
+};
+int launch_ec_big(const EcBigParams& p, bool pdl, cudaStream_t st);
+
+// ---- tc.cu (M > 16): tcgen05 GEMM, int4 dequantised into shared memory, EC folded in as extra K blocks
+struct TcProblem {
+    const void* x; const void* wq; const void* scales; const void* B; void* y;
+    const void* u16;         // [M][r] fp16 (alpha * gamma (.) z) or NULL when r == 0
+    int M, N, K, r, group;
+    bool pdl;
+    int grid_override;
+};
+bool tc_available();
+int run_tc(const TcProblem& t, cudaStream_t st);
+
 }  // namespace spear
