@@ -1,0 +1,233 @@
+"""paper_2606_11244_b200 -- thin Python binding of libspear.so (include/spear.h).
+
+Argument marshalling only: every step of the SPEAR W4A16 + gated-EC layer (PAPER.md:107-110,
+Eq. 3) runs in the CUDA kernels behind the C ABI.  torch is used for device memory and streams.
+There is no CPU path: importing works without a GPU (so the symbol table can be checked), but
+every compute call needs the library and a CUDA device and raises otherwise.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+from dataclasses import dataclass
+from typing import Optional
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libspear.so")
+
+GATE_SCALAR_SIGMOID, GATE_MLP, GATE_NONE = 0, 1, 2
+GATE_KINDS = {"scalar": GATE_SCALAR_SIGMOID, "mlp": GATE_MLP, "none": GATE_NONE}
+VARIANT_AUTO, VARIANT_STREAM_FUSED, VARIANT_STREAM_SPLIT, VARIANT_TC_FUSED, VARIANT_TC_SPLIT = range(5)
+VARIANT_COUNT = 5
+VARIANT_NAMES = ["auto", "stream_fused", "stream_split", "tc_fused", "tc_split"]
+
+EXPORTS = [
+    "spear_pack_w4_sizes", "spear_pack_w4", "spear_unpack_w4", "spear_dequant_w4",
+    "spear_w4_ec_gemm", "spear_w4_ec_gemm_ex", "spear_w4_ec_gemm_hostio",
+    "spear_workspace_bytes", "spear_init", "spear_plan", "spear_plan_save", "spear_plan_load",
+    "spear_plan_query", "spear_tune", "spear_last_error", "spear_launch_count",
+]
+
+
+class SpearError(RuntimeError):
+    def __init__(self, status: int, msg: str):
+        super().__init__(f"libspear status {status}: {msg}")
+        self.status = status
+
+
+class EcDesc(ctypes.Structure):
+    """struct spear_ec_desc of include/spear.h."""
+    _fields_ = [
+        ("gate_kind", ctypes.c_int), ("gate_hidden", ctypes.c_int), ("alpha", ctypes.c_float),
+        ("W1", ctypes.c_void_p), ("b1", ctypes.c_void_p), ("W2", ctypes.c_void_p), ("b2", ctypes.c_void_p),
+        ("w_g", ctypes.c_void_p), ("b_g", ctypes.c_void_p), ("gate_out", ctypes.c_void_p),
+        ("workspace", ctypes.c_void_p), ("workspace_bytes", ctypes.c_size_t), ("force_variant", ctypes.c_int),
+    ]
+
+
+_lib = None
+
+
+def lib():
+    """Loads libspear.so; raises (loudly) if it has not been built."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(LIB_PATH):
+            raise ImportError(f"{LIB_PATH} is missing: run `python -m paper_2606_11244_b200.build` "
+                              "(there is no fallback path)")
+        L = ctypes.CDLL(LIB_PATH)
+        vp, ci = ctypes.c_void_p, ctypes.c_int
+        L.spear_pack_w4_sizes.argtypes = [ci, ci, ci, ctypes.POINTER(ctypes.c_size_t), ctypes.POINTER(ctypes.c_size_t)]
+        L.spear_pack_w4.argtypes = [vp, vp, vp, vp, ci, ci, ci, vp]
+        L.spear_unpack_w4.argtypes = [vp, vp, ci, ci, ci, vp]
+        L.spear_dequant_w4.argtypes = [vp, vp, vp, ci, ci, ci, vp]
+        L.spear_w4_ec_gemm.argtypes = [vp] * 8 + [ci] * 5 + [vp]
+        L.spear_w4_ec_gemm_ex.argtypes = [vp] * 5 + [ctypes.POINTER(EcDesc), vp] + [ci] * 5 + [vp]
+        L.spear_w4_ec_gemm_hostio.argtypes = [vp] * 8 + [ctypes.POINTER(EcDesc)] + [ci] * 5 + [vp]
+        L.spear_workspace_bytes.argtypes = [ci] * 5 + [ctypes.POINTER(ctypes.c_size_t)]
+        L.spear_init.argtypes = []
+        L.spear_plan.argtypes = [ci] * 7 + [ctypes.POINTER(ci), ctypes.POINTER(ctypes.c_float), vp]
+        L.spear_plan_save.argtypes = [ctypes.c_char_p]
+        L.spear_plan_load.argtypes = [ctypes.c_char_p]
+        L.spear_plan_query.argtypes = [ci] * 6 + [ctypes.POINTER(ci)]
+        L.spear_tune.argtypes = [ctypes.c_char_p, ci]
+        L.spear_last_error.restype = ctypes.c_char_p
+        L.spear_launch_count.restype = ctypes.c_ulonglong
+        for name in EXPORTS:
+            if name not in ("spear_last_error", "spear_launch_count"):
+                getattr(L, name).restype = ci
+        _lib = L
+    return _lib
+
+
+def _check(rc: int):
+    if rc != 0:
+        raise SpearError(rc, lib().spear_last_error().decode())
+
+
+def _ptr(t) -> Optional[int]:
+    return None if t is None else t.data_ptr()
+
+
+def _stream(stream) -> Optional[int]:
+    import torch
+    s = torch.cuda.current_stream() if stream is None else stream
+    return s.cuda_stream or None
+
+
+def init():
+    _check(lib().spear_init())
+
+
+def launch_count() -> int:
+    return int(lib().spear_launch_count())
+
+
+def tune(key: str, value: int):
+    _check(lib().spear_tune(key.encode(), int(value)))
+
+
+def pack_w4_sizes(N: int, K: int, group: int):
+    a, b = ctypes.c_size_t(), ctypes.c_size_t()
+    _check(lib().spear_pack_w4_sizes(N, K, group, ctypes.byref(a), ctypes.byref(b)))
+    return a.value, b.value
+
+
+@dataclass
+class PackedW4:
+    """Opaque packed weights of one layer (SPW4 layout) on the device."""
+    wq: "torch.Tensor"        # uint8 [N*K/2]
+    scales: "torch.Tensor"    # float16 [N*K/group] (packed order)
+    N: int
+    K: int
+    group: int
+
+
+def pack_w4(codes, scales, group: int, stream=None) -> PackedW4:
+    """spear_pack_w4: codes uint8 [N][K] in 0..15, scales float16 [N][K/group] (device tensors)."""
+    import torch
+    N, K = codes.shape
+    assert codes.dtype == torch.uint8 and codes.is_cuda and codes.is_contiguous()
+    assert scales.dtype == torch.float16 and scales.is_cuda and scales.is_contiguous()
+    wb, sb = pack_w4_sizes(N, K, group)
+    wq = torch.empty(wb, dtype=torch.uint8, device=codes.device)
+    sp = torch.empty(sb // 2, dtype=torch.float16, device=codes.device)
+    _check(lib().spear_pack_w4(_ptr(codes), _ptr(scales), _ptr(wq), _ptr(sp), N, K, group, _stream(stream)))
+    return PackedW4(wq, sp, N, K, group)
+
+
+def unpack_w4(pw: PackedW4, stream=None):
+    import torch
+    out = torch.empty((pw.N, pw.K), dtype=torch.uint8, device=pw.wq.device)
+    _check(lib().spear_unpack_w4(_ptr(pw.wq), _ptr(out), pw.N, pw.K, pw.group, _stream(stream)))
+    return out
+
+
+def dequant_w4(pw: PackedW4, stream=None):
+    import torch
+    out = torch.empty((pw.N, pw.K), dtype=torch.float16, device=pw.wq.device)
+    _check(lib().spear_dequant_w4(_ptr(pw.wq), _ptr(pw.scales), _ptr(out), pw.N, pw.K, pw.group, _stream(stream)))
+    return out
+
+
+def w4_ec_gemm(x, pw: PackedW4, A=None, B=None, gate_w=None, gate_b=None, y=None, stream=None):
+    """spear_w4_ec_gemm (the 14-argument call of BASELINE.json): scalar sigmoid gate, alpha = 1."""
+    import torch
+    M, K = x.shape
+    assert K == pw.K and x.dtype == torch.float16 and x.is_contiguous()
+    r = 0 if A is None else A.shape[0]
+    if y is None:
+        y = torch.empty((M, pw.N), dtype=torch.float16, device=x.device)
+    _check(lib().spear_w4_ec_gemm(_ptr(x), _ptr(pw.wq), _ptr(pw.scales), _ptr(A), _ptr(B), _ptr(gate_w),
+                                  _ptr(gate_b), _ptr(y), M, pw.N, K, r, pw.group, _stream(stream)))
+    return y
+
+
+def make_desc(gate="scalar", alpha=1.0, w_g=None, b_g=None, W1=None, b1=None, W2=None, b2=None,
+              gate_out=None, workspace=None, variant=VARIANT_AUTO) -> EcDesc:
+    d = EcDesc()
+    d.gate_kind = GATE_KINDS[gate] if isinstance(gate, str) else int(gate)
+    d.gate_hidden = 0 if W1 is None else int(W1.shape[0])
+    d.alpha = float(alpha)
+    d.W1, d.b1, d.W2, d.b2 = _ptr(W1), _ptr(b1), _ptr(W2), _ptr(b2)
+    d.w_g, d.b_g, d.gate_out = _ptr(w_g), _ptr(b_g), _ptr(gate_out)
+    d.workspace = _ptr(workspace)
+    d.workspace_bytes = 0 if workspace is None else workspace.numel() * workspace.element_size()
+    d.force_variant = int(variant)
+    return d
+
+
+def w4_ec_gemm_ex(x, pw: PackedW4, A=None, B=None, desc: Optional[EcDesc] = None, y=None, stream=None):
+    """spear_w4_ec_gemm_ex: the paper's MLP gate, alpha, gate_out, forced variants."""
+    import torch
+    M, K = x.shape
+    assert K == pw.K and x.dtype == torch.float16 and x.is_contiguous()
+    r = 0 if A is None else A.shape[0]
+    if desc is None:
+        desc = make_desc(gate="none")
+    if y is None:
+        y = torch.empty((M, pw.N), dtype=torch.float16, device=x.device)
+    _check(lib().spear_w4_ec_gemm_ex(_ptr(x), _ptr(pw.wq), _ptr(pw.scales), _ptr(A), _ptr(B),
+                                     ctypes.byref(desc), _ptr(y), M, pw.N, K, r, pw.group, _stream(stream)))
+    return y
+
+
+def w4_ec_gemm_hostio(x_host, y_host, x_dev, y_dev, pw: PackedW4, A=None, B=None,
+                      desc: Optional[EcDesc] = None, stream=None):
+    """spear_w4_ec_gemm_hostio: x from (pinned) host memory, y back to host, on `stream`."""
+    M, K = x_host.shape
+    r = 0 if A is None else A.shape[0]
+    if desc is None:
+        desc = make_desc(gate="none")
+    _check(lib().spear_w4_ec_gemm_hostio(_ptr(x_host), _ptr(y_host), _ptr(x_dev), _ptr(y_dev), _ptr(pw.wq),
+                                         _ptr(pw.scales), _ptr(A), _ptr(B), ctypes.byref(desc),
+                                         M, pw.N, K, r, pw.group, _stream(stream)))
+
+
+def workspace_bytes(M, N, K, r, group) -> int:
+    b = ctypes.c_size_t()
+    _check(lib().spear_workspace_bytes(M, N, K, r, group, ctypes.byref(b)))
+    return b.value
+
+
+def plan(M, N, K, r, group, gate="scalar", gate_hidden=0, stream=None):
+    """spear_plan: measures the valid variants, records and returns (chosen, [us per variant])."""
+    chosen = ctypes.c_int()
+    times = (ctypes.c_float * VARIANT_COUNT)()
+    _check(lib().spear_plan(M, N, K, r, group, GATE_KINDS[gate], gate_hidden, ctypes.byref(chosen), times,
+                            _stream(stream)))
+    return chosen.value, [float(t) for t in times]
+
+
+def plan_query(M, N, K, r, group, gate="scalar") -> int:
+    v = ctypes.c_int()
+    _check(lib().spear_plan_query(M, N, K, r, group, GATE_KINDS[gate], ctypes.byref(v)))
+    return v.value
+
+
+def plan_save(path: str):
+    _check(lib().spear_plan_save(path.encode()))
+
+
+def plan_load(path: str):
+    _check(lib().spear_plan_load(path.encode()))

@@ -1,0 +1,76 @@
+"""CPU-side checks of the boundary: libspear.so builds, loads and exports every symbol that
+include/spear.h declares; argument errors are reported without a GPU.  No compute calls here."""
+import ctypes
+import os
+import re
+
+import pytest
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+@pytest.fixture(scope="module")
+def spear():
+    from paper_2606_11244_b200 import build as b
+    b.build()
+    import paper_2606_11244_b200 as sp
+    sp.lib()
+    return sp
+
+
+def _declared():
+    src = open(os.path.join(ROOT, "include", "spear.h")).read()
+    src = re.sub(r"/\*.*?\*/", "", src, flags=re.S)
+    return sorted(set(re.findall(r"\b(spear_[a-z0-9_]+)\s*\(", src)))
+
+
+def test_header_symbols_all_exported(spear):
+    names = _declared()
+    assert "spear_w4_ec_gemm" in names and "spear_pack_w4" in names and "spear_plan" in names
+    L = ctypes.CDLL(spear.LIB_PATH)
+    for n in names:
+        assert hasattr(L, n), f"{n} declared in spear.h but not exported"
+    assert sorted(spear.EXPORTS) == names
+
+
+def test_ec_desc_layout_matches_header(spear):
+    # 2 ints + float + pad, 7 pointers, void* + size_t, int + pad
+    assert ctypes.sizeof(spear.EcDesc) == 16 + 7 * 8 + 16 + 8
+    assert spear.EcDesc.W1.offset == 16 and spear.EcDesc.force_variant.offset == 88
+
+
+def test_sizes_and_shape_errors_need_no_gpu(spear):
+    wb, sb = spear.pack_w4_sizes(2048, 2048, 128)
+    assert wb == 2048 * 2048 // 2 and sb == 2048 * 16 * 2
+    wb, sb = spear.pack_w4_sizes(4096, 14336, 14336)
+    assert wb == 4096 * 14336 // 2 and sb == 4096 * 2
+    with pytest.raises(spear.SpearError) as e:
+        spear.pack_w4_sizes(100, 2048, 128)
+    assert e.value.status == -2
+    with pytest.raises(spear.SpearError) as e:
+        spear.pack_w4_sizes(128, 2048, 96)
+    assert e.value.status == -2
+    with pytest.raises(spear.SpearError) as e:
+        spear.pack_w4_sizes(0, 2048, 128)
+    assert e.value.status == -1
+
+
+def test_no_cpu_fallback(spear):
+    import torch
+    if torch.cuda.is_available():
+        pytest.skip("GPU present")
+    with pytest.raises(spear.SpearError) as e:
+        spear.init()
+    assert e.value.status == -3   # SPEAR_ECUDA: the library refuses to run without a device
+
+
+def test_product_does_not_import_oracle():
+    pkg = os.path.join(ROOT, "paper_2606_11244_b200")
+    for dp, _, files in os.walk(pkg):
+        for f in files:
+            if f.endswith((".py", ".cu", ".cuh", ".h")):
+                txt = open(os.path.join(dp, f)).read()
+                assert not re.search(r"^\s*(import oracle|from oracle)\b", txt, flags=re.M), f
+                assert "spear_oracle" not in txt and "libspear_oracle" not in txt, f
+    osrc = open(os.path.join(ROOT, "oracle", "spear_oracle.c")).read() + open(os.path.join(ROOT, "oracle", "__init__.py")).read()
+    assert "paper_2606_11244_b200" not in osrc.replace("(paper_2606_11244_b200)", "")

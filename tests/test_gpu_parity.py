@@ -1,0 +1,215 @@
+"""GPU parity: libspear.so (through the C ABI) against the fp64 CPU oracle, element by element, on
+the same seeded inputs.  Bars (BASELINE.json north_star): packed bytes and dequantised fp16
+bit-exact; max|y - y_ref| <= 1e-2 * rms(y_ref); gate within 1e-3 absolute."""
+import numpy as np
+import pytest
+
+import oracle
+from workloads import make_layer, config_shapes
+
+pytestmark = pytest.mark.gpu
+
+Y_TOL = 1e-2      # x rms(y_ref)
+GATE_TOL = 1e-3   # absolute
+
+
+@pytest.fixture(scope="module")
+def sp():
+    import paper_2606_11244_b200 as sp
+    sp.init()
+    return sp
+
+
+def _harness():
+    from paper_2606_11244_b200 import harness
+    return harness
+
+
+def check_layer(li, variant=0, rows=None, use_14arg=False, label=""):
+    """Runs the layer on the GPU and compares against the oracle (all rows, or the given rows)."""
+    import torch
+    h = _harness()
+    dl = h.upload_layer(li)
+    x = h.dev(li.x)
+    y, gate = h.run_layer(dl, x, variant=variant, want_gate=True, use_14arg=use_14arg)
+    torch.cuda.synchronize()
+    yg = y.cpu().numpy().astype(np.float64)
+    ref = oracle.forward_layer(li, rows=rows)
+    yr = ref["y"]
+    if rows is not None:
+        yg = yg[rows]
+    rms = float(np.sqrt(np.mean(yr ** 2)))
+    err = float(np.max(np.abs(yg - yr)))
+    assert np.all(np.isfinite(yg)), label
+    assert err <= Y_TOL * rms, f"{label}: max err {err:.4g} > {Y_TOL} * rms {rms:.4g}"
+    if gate is not None and ref["gam"] is not None:
+        gg = gate.cpu().numpy().astype(np.float64)
+        if rows is not None:
+            gg = gg[rows]
+        gerr = float(np.max(np.abs(gg - ref["gam"])))
+        assert gerr <= GATE_TOL, f"{label}: gate err {gerr:.3g}"
+    return err / rms
+
+
+# ---------------------------------------------------------------- S0: pack / unpack / dequant, bit-exact
+
+@pytest.mark.parametrize("N,K,group", [(128, 128, 128), (256, 384, 128), (384, 512, 256), (2048, 2048, 128),
+                                       (256, 1792, 1792), (3072, 2048, 128)])
+def test_pack_bit_exact(sp, N, K, group):
+    import torch
+    h = _harness()
+    li = make_layer(11 + N + K, 1, N, K, group, 0)
+    pw = sp.pack_w4(h.dev(li.codes), h.dev(li.scales), group)
+    wq_ref, sc_ref = oracle.pack_w4(li.codes, li.scales, group)
+    assert np.array_equal(pw.wq.cpu().numpy().view(np.uint32), wq_ref)
+    assert np.array_equal(pw.scales.cpu().numpy().view(np.uint16), sc_ref.view(np.uint16))
+    assert np.array_equal(sp.unpack_w4(pw).cpu().numpy(), li.codes)
+    dq = sp.dequant_w4(pw).cpu().numpy()
+    assert np.array_equal(dq.view(np.uint16), oracle.dequant16(li.codes, li.scales, group).view(np.uint16))
+
+
+def test_pack_structured_codes(sp):
+    h = _harness()
+    N, K = 256, 256
+    n, k = np.meshgrid(np.arange(N), np.arange(K), indexing="ij")
+    codes = ((n + k) & 15).astype(np.uint8)
+    scales = np.full((N, 2), 1.0, np.float16)
+    pw = sp.pack_w4(h.dev(codes), h.dev(scales), 128)
+    wq_ref, _ = oracle.pack_w4(codes, scales, 128)
+    assert np.array_equal(pw.wq.cpu().numpy().view(np.uint32), wq_ref)
+    # a single non-8 nibble walking through one tile
+    for (nn, kk) in [(0, 0), (7, 63), (8, 64), (127, 127), (128, 1), (200, 255), (15, 9)]:
+        c = np.full((N, K), 8, np.uint8)
+        c[nn, kk] = 3
+        pw = sp.pack_w4(h.dev(c), h.dev(scales), 128)
+        assert np.array_equal(sp.unpack_w4(pw).cpu().numpy(), c)
+        ref, _ = oracle.pack_w4(c, scales, 128)
+        assert np.array_equal(pw.wq.cpu().numpy().view(np.uint32), ref)
+
+
+def test_pack_rejects_bad_code(sp):
+    h = _harness()
+    c = np.full((128, 128), 8, np.uint8)
+    c[5, 77] = 16
+    with pytest.raises(sp.SpearError) as e:
+        sp.pack_w4(h.dev(c), h.dev(np.ones((128, 1), np.float16)), 128)
+    assert e.value.status == -1
+
+
+def test_dequant_all_codes_and_scales(sp):
+    """P7 on the GPU: every code x scales incl. 1e-3, 1, powers of two, full-mantissa values."""
+    h = _harness()
+    N, K = 128, 128
+    scales = np.array([1e-3, 1.0, 0.5, 2.0, 0.02, 0.0123, 1.9990234375, 6.1e-5] * 16, np.float16).reshape(N, 1)
+    codes = ((np.arange(N)[:, None] + np.arange(K)[None, :]) & 15).astype(np.uint8)
+    pw = sp.pack_w4(h.dev(codes), h.dev(scales), 128)
+    dq = sp.dequant_w4(pw).cpu().numpy()
+    assert np.array_equal(dq.view(np.uint16), oracle.dequant16(codes, scales, 128).view(np.uint16))
+
+
+# ---------------------------------------------------------------- decode path (M <= 16)
+
+def test_config1_scalar_gate(sp):
+    s = config_shapes(0)[0]
+    li = make_layer(s.seed, s.M, s.N, s.K, s.group, s.r, gate="scalar")
+    check_layer(li, label="config1")
+    check_layer(li, use_14arg=True, label="config1/14arg")
+
+
+def test_config1_mlp_gate(sp):
+    s = config_shapes(0)[0]
+    for hh in (None, 2 * s.r, s.r):
+        li = make_layer(s.seed, s.M, s.N, s.K, s.group, s.r, gate="mlp", h=hh)
+        check_layer(li, label=f"config1/mlp h={hh}")
+
+
+@pytest.mark.parametrize("M", [1, 2, 3, 5, 8, 9, 13, 16])
+@pytest.mark.parametrize("gate", ["scalar", "mlp", "none"])
+def test_decode_small_shapes(sp, M, gate):
+    # several panels / chunks, ragged token counts, K not a power of two
+    li = make_layer(100 + M, M, 384, 640, 128, 24, gate=gate)
+    check_layer(li, label=f"decode M={M} {gate}")
+
+
+@pytest.mark.parametrize("r", [0, 8, 16, 32, 64, 128])
+def test_decode_ranks(sp, r):
+    li = make_layer(200 + r, 7, 512, 1024, 128, r, gate="scalar")
+    check_layer(li, label=f"decode r={r}")
+
+
+@pytest.mark.parametrize("group,K", [(128, 1024), (256, 1024), (1024, 1024), (1792, 1792)])
+def test_decode_groups(sp, group, K):
+    li = make_layer(300 + group, 4, 256, K, group, 16, gate="scalar")
+    check_layer(li, label=f"decode group={group}")
+
+
+@pytest.mark.parametrize("idx", range(12))
+def test_config2_llama1b_decode(sp, idx):
+    s = config_shapes(1)[idx]
+    li = make_layer(s.seed, s.M, s.N, s.K, s.group, s.r, gate="scalar")
+    check_layer(li, label=f"config2 {s.name} M={s.M}")
+
+
+@pytest.mark.parametrize("idx", [0, 1, 2, 3, 4, 5])
+def test_config3_per_channel_decode(sp, idx):
+    s = config_shapes(2)[idx]       # M = 1 and 16, per-channel scales (group = K)
+    li = make_layer(s.seed, s.M, s.N, s.K, s.group, s.r, gate="scalar")
+    check_layer(li, label=f"config3 {s.name} M={s.M}")
+
+
+# ---------------------------------------------------------------- invariants on the GPU (P2, P6)
+
+def test_gate_zero_or_A_zero_is_plain_w4(sp):
+    import torch
+    h = _harness()
+    li = make_layer(77, 6, 256, 512, 128, 16, gate="scalar")
+    plain = make_layer(77, 6, 256, 512, 128, 0)
+    y0, _ = h.run_layer(h.upload_layer(plain), h.dev(plain.x))
+    li.b_g = -100.0                                   # sigmoid(-100 + small) == 0 in fp32
+    y1, g1 = h.run_layer(h.upload_layer(li), h.dev(li.x), want_gate=True)
+    assert float(g1.abs().max()) < 1e-30
+    assert torch.equal(y0, y1)
+    li.b_g = 0.0
+    li.A = np.zeros_like(li.A)
+    y2, _ = h.run_layer(h.upload_layer(li), h.dev(li.x))
+    assert torch.equal(y0, y2)
+
+
+def test_token_permutation_equivariance(sp):
+    import torch
+    h = _harness()
+    li = make_layer(78, 8, 256, 512, 128, 16, gate="mlp")
+    dl = h.upload_layer(li)
+    x = h.dev(li.x)
+    perm = torch.tensor([3, 0, 7, 1, 6, 2, 5, 4], device=x.device)
+    y, g = h.run_layer(dl, x, want_gate=True)
+    yp, gp = h.run_layer(dl, x[perm].contiguous(), want_gate=True)
+    assert torch.allclose(yp.float(), y[perm].float(), atol=2e-2, rtol=2e-3)
+    assert torch.allclose(gp, g[perm], atol=1e-5)
+
+
+def test_back_to_back_calls_leave_workspace_clean(sp):
+    """The library's counters / z accumulators must be zero again after every call."""
+    import torch
+    h = _harness()
+    li = make_layer(79, 16, 384, 2048, 128, 32, gate="scalar")
+    dl = h.upload_layer(li)
+    x = h.dev(li.x)
+    ys = [h.run_layer(dl, x)[0].clone() for _ in range(5)]
+    torch.cuda.synchronize()
+    for y in ys[1:]:
+        assert torch.equal(ys[0], y)
+
+
+def test_errors(sp):
+    import torch
+    h = _harness()
+    li = make_layer(80, 4, 128, 128, 128, 8, gate="scalar")
+    dl = h.upload_layer(li)
+    x = h.dev(li.x)
+    with pytest.raises(sp.SpearError) as e:      # r not a multiple of 8
+        sp.w4_ec_gemm(x, dl.pw, dl.A[:4].contiguous(), dl.B[:, :4].contiguous(), dl.w_g, dl.b_g)
+    assert e.value.status == -2
+    with pytest.raises(sp.SpearError) as e:      # missing gate weights
+        sp.w4_ec_gemm(x, dl.pw, dl.A, dl.B, None, None)
+    assert e.value.status == -1
