@@ -1,0 +1,372 @@
+#!/usr/bin/env python
+"""bench.py -- BASELINE.json metric on one B200: the W4A16 + gated-EC layer's decode HBM GB/s.
+
+Workload (config.workload): BASELINE.json configs[1] -- Llama-3.2-1B-shaped decode projections
+(qkv 2048->3072, o 2048->2048, gate_up 2048->16384, down 8192->2048), int4 group=128, EC rank 32 with
+the scalar sigmoid gate on every projection, M in {1, 8, 16}.  One "step" = one pass of the whole hot
+path over that batch = 12 layer calls (3 token counts x 4 projections), all through the C ABI
+(spear_w4_ec_gemm_ex).  value = algorithmic bytes of the step (packed weights +
+scales + x + y + EC factors + gate vector) / device time, whole job.
+
+L2 hygiene: every step reads a different copy of the weights and EC factors from an arena of NCOPY
+copies (> 4x the 126 MB L2), so weights always come from HBM ("inputs larger than L2").
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl reference]
+
+N > 1 (torchrun): replicas only -- each rank runs the same per-GPU workload (weak scaling), no
+collective on the data path; rank 0 reports the sum.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import numpy as np
+
+from workloads import algorithmic_bytes, config_shapes, make_layer
+from workloads.synth import make_x
+
+METRIC = "W4A16+gated-EC layer: decode HBM GB/s (Llama-3.2-1B decode projections, r=32, M in {1,8,16})"
+UNIT = "GB/s"
+TOKENS = (1, 8, 16)
+NCOPY_TARGET_BYTES = 640 << 20
+
+
+def load_peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        with open(p) as f:
+            d = json.load(f)
+        return float(d["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+    return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
+
+
+def step_shapes():
+    """The 12 layer shapes of one step, grouped by token count."""
+    shapes = config_shapes(1)
+    return {M: [s for s in shapes if s.M == M] for M in TOKENS}
+
+
+def step_bytes(with_ec=True):
+    tot = 0
+    for M, ss in step_shapes().items():
+        for s in ss:
+            tot += algorithmic_bytes(s.M, s.N, s.K, s.group, s.r if with_ec else 0, "scalar")
+    return tot
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons sampled while the timed regions run."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,utilization.gpu,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index=0):
+        self.rows = []
+        self.proc = None
+        self.index = index
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(
+                ["nvidia-smi", "-i", str(self.index), f"--query-gpu={self.Q}", "--format=csv,noheader,nounits",
+                 "-lms", "100"], stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.t = threading.Thread(target=self._read, daemon=True)
+            self.t.start()
+        except Exception:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append(line.strip())
+
+    def stop(self):
+        if not self.proc:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=5)
+        except Exception:
+            self.proc.kill()
+        sm, mx, reasons = [], None, set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for r in self.rows:
+            f = [c.strip() for c in r.split(",")]
+            if len(f) < 8:
+                continue
+            try:
+                clk, mxc, util = float(f[0]), float(f[1]), float(f[3])
+            except ValueError:
+                continue
+            mx = mxc
+            if util > 0:
+                sm.append(clk)
+                for n, v in zip(names, f[4:8]):
+                    if v.lower().startswith("active"):
+                        reasons.add(n)
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": mx,
+                "reasons": sorted(reasons), "samples_under_load": len(sm)}
+
+
+# ------------------------------------------------------------------------------------------------
+# CUDA arm
+# ------------------------------------------------------------------------------------------------
+def run_cuda(args, rank, world):
+    import torch
+    import torch.distributed as dist
+    import paper_2606_11244_b200 as sp
+    from paper_2606_11244_b200 import harness
+
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    torch.cuda.set_device(local)
+    device = f"cuda:{local}"
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device(device))
+    sp.init()
+    if os.environ.get("SPEAR_PDL") is not None:
+        sp.tune("pdl", int(os.environ["SPEAR_PDL"]))
+
+    shapes = step_shapes()
+    # weights / EC factors: one seeded set per projection (the M=16 entry's seed), shared by the three
+    # token counts; activations per (M, projection) from that entry's own seed
+    base = {}
+    for s in shapes[16]:
+        li = make_layer(s.seed, 16, s.N, s.K, s.group, s.r, gate="scalar")
+        base[s.name] = harness.upload_layer(li, device)
+    set_bytes = sum(dl.pw.wq.numel() + dl.pw.scales.numel() * 2 + (dl.A.numel() + dl.B.numel() + dl.w_g.numel()) * 2
+                    for dl in base.values())
+    ncopy = max(3, -(-NCOPY_TARGET_BYTES // set_bytes))
+    ncopy = -(-ncopy // 3) * 3
+    copies = []
+    for c in range(ncopy):
+        d = {}
+        for name, dl in base.items():
+            pw = sp.PackedW4(dl.pw.wq.clone(), dl.pw.scales.clone(), dl.pw.N, dl.pw.K, dl.pw.group)
+            d[name] = harness.DeviceLayer(pw=pw, M=0, N=dl.N, K=dl.K, r=dl.r, group=dl.group, gate="scalar",
+                                          alpha=1.0, A=dl.A.clone(), B=dl.B.clone(), w_g=dl.w_g.clone(), b_g=dl.b_g)
+        copies.append(d)
+    xs, ys, xh, yh = {}, {}, {}, {}
+    for M in TOKENS:
+        for s in shapes[M]:
+            x, _ = make_x(s.seed, M, s.K)
+            xs[(M, s.name)] = harness.dev(x, device)
+            ys[(M, s.name)] = torch.empty((M, s.N), dtype=torch.float16, device=device)
+            xh[(M, s.name)] = torch.from_numpy(x).pin_memory()
+            yh[(M, s.name)] = torch.empty((M, s.N), dtype=torch.float16).pin_memory()
+
+    descs = {}   # keep EcDesc objects alive
+
+    def one_step(g, with_ec=True):
+        for mi, M in enumerate(TOKENS):
+            cp = copies[(3 * g + mi) % ncopy]
+            for s in shapes[M]:
+                dl = cp[s.name]
+                key = (g, mi, s.name, with_ec)
+                if key not in descs:
+                    descs[key] = dl.desc() if with_ec else sp.make_desc(gate="none")
+                if with_ec:
+                    sp.w4_ec_gemm_ex(xs[(M, s.name)], dl.pw, dl.A, dl.B, descs[key], y=ys[(M, s.name)])
+                else:
+                    sp.w4_ec_gemm_ex(xs[(M, s.name)], dl.pw, None, None, descs[key], y=ys[(M, s.name)])
+
+    stream = torch.cuda.Stream()
+    ngraph = ncopy // 3
+    use_graph = os.environ.get("SPEAR_BENCH_GRAPH", "1") != "0"
+
+    def make_graphs(with_ec):
+        gs = []
+        with torch.cuda.stream(stream):
+            one_step(0, with_ec)           # first-call work (tensor maps, attributes) outside capture
+            torch.cuda.synchronize()
+            for g in range(ngraph):
+                if use_graph:
+                    cg = torch.cuda.CUDAGraph()
+                    with torch.cuda.graph(cg, stream=stream):
+                        one_step(g, with_ec)
+                    gs.append(cg.replay)
+                else:
+                    gs.append(lambda g=g: one_step(g, with_ec))
+        return gs
+
+    def timed(fns, steps, warmup):
+        with torch.cuda.stream(stream):
+            for i in range(warmup):
+                fns[i % len(fns)]()
+            if world > 1:
+                dist.barrier()
+            torch.cuda.synchronize()
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record(stream)
+            for i in range(steps):
+                fns[i % len(fns)]()
+            e1.record(stream)
+            torch.cuda.synchronize()
+            if world > 1:
+                dist.barrier()
+        ms = e0.elapsed_time(e1)
+        if world > 1:
+            t = torch.tensor([ms], device=device)
+            dist.all_reduce(t, op=dist.ReduceOp.MAX)
+            ms = float(t.item())
+        return ms
+
+    sampler = ClockSampler(local)
+    if rank == 0:
+        sampler.start()
+    launches0 = sp.launch_count()
+    g_ec = make_graphs(True)
+    per_step_launches = (sp.launch_count() - launches0) // (ngraph + 1)
+    ms = timed(g_ec, args.steps, args.warmup)
+    g_w4 = make_graphs(False)
+    ms_w4 = timed(g_w4, args.steps, args.warmup)
+    # make the region long enough for nvidia-smi to see it under load
+    t_end = time.time() + 1.5
+    while rank == 0 and time.time() < t_end:
+        timed(g_ec, 200, 0)
+
+    # e2e: host x -> device -> layer -> host y, every call, through spear_w4_ec_gemm_hostio
+    e2e_steps = max(1, min(args.steps, 300))
+
+    def e2e_step(g):
+        for mi, M in enumerate(TOKENS):
+            cp = copies[(3 * g + mi) % ncopy]
+            for s in shapes[M]:
+                dl = cp[s.name]
+                k = (M, s.name)
+                sp.w4_ec_gemm_hostio(xh[k], yh[k], xs[k], ys[k], dl.pw, dl.A, dl.B, descs[(g, mi, s.name, True)])
+    ms_e2e = timed([lambda g=g: e2e_step(g) for g in range(ngraph)], e2e_steps, max(3, min(args.warmup, 20)))
+    clocks = sampler.stop() if rank == 0 else None
+
+    b_ec, b_w4 = step_bytes(True), step_bytes(False)
+    per = ms / args.steps
+    per_w4 = ms_w4 / args.steps
+    per_e2e = ms_e2e / e2e_steps
+    value = world * b_ec / (per * 1e-3) / 1e9
+    peak, peak_src = load_peaks()
+    ncalls = sum(len(v) for v in shapes.values())
+    ach = b_w4 / (per_w4 * 1e-3) / 1e9
+    out = {
+        "metric": METRIC, "value": round(value, 1), "unit": UNIT, "n_gpus": world, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": round(per, 6), "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "f16 (int4 weights, fp32 accumulate)", "data": "synthetic (seeded, workloads/)",
+        "config": {"workload": "BASELINE.json configs[1]: Llama-3.2-1B decode projections qkv/o/gate_up/down, "
+                               "group=128, EC r=32 scalar sigmoid gate, M in {1,8,16}; step = 12 layer calls",
+                   "l2": f"inputs larger than L2: weights+EC rotate over {ncopy} copies ({ncopy * set_bytes >> 20} MiB)",
+                   "cuda_graph": use_graph, "bytes_per_step": b_ec, "parallelism": f"replicas x{world}"},
+        "e2e": {"value": round(world * b_ec / (per_e2e * 1e-3) / 1e9, 1), "unit": UNIT,
+                "h2d_bytes_per_step": sum(t.numel() * 2 for t in xh.values()),
+                "d2h_bytes_per_step": sum(t.numel() * 2 for t in yh.values()), "ms_per_step": round(per_e2e, 6)},
+        "gpu_launches": int(per_step_launches * args.steps),
+        "clocks": clocks,
+        "roofline": {"bound": "hbm", "kernel": "spear::stream_kernel (plain W4 step: one launch per layer call)",
+                     "achieved": round(ach, 1), "peak": peak, "unit": "GB/s", "frac": round(ach / peak, 4),
+                     "peak_source": peak_src, "traffic": None,
+                     "avg_launch_us": round(per_w4 * 1e3 / ncalls, 3), "launches_per_step": ncalls},
+        "no_ec": {"value": round(world * b_w4 / (per_w4 * 1e-3) / 1e9, 1), "ms_per_step": round(per_w4, 6)},
+        "ec_overhead_time_frac": round(per / per_w4 - 1.0, 4),
+    }
+    if rank == 0:
+        out["cpu_baseline"] = cpu_baseline_sample()
+        print(json.dumps(out), flush=True)
+    if world > 1:
+        dist.destroy_process_group()
+
+
+# ------------------------------------------------------------------------------------------------
+# oracle legs (the only places bench.py executes oracle/): cpu_baseline and --impl reference
+# ------------------------------------------------------------------------------------------------
+def _oracle_pass(layers):
+    """One oracle pass (dequantise + forward, fp64) over prepared LayerInputs; returns seconds."""
+    import oracle
+    t0 = time.perf_counter()
+    for li in layers:
+        oracle.forward_layer(li)
+    return time.perf_counter() - t0
+
+
+def _sample_layers(which):
+    shapes = step_shapes()
+    if which == "step":
+        sel = [s for M in TOKENS for s in shapes[M]]
+    elif which == "m1":
+        sel = list(shapes[1])
+    else:
+        sel = [s for s in shapes[1] if s.name == "o"]
+    layers = [make_layer(s.seed, s.M, s.N, s.K, s.group, s.r, gate="scalar") for s in sel]
+    nbytes = sum(algorithmic_bytes(s.M, s.N, s.K, s.group, s.r, "scalar") for s in sel)
+    return layers, nbytes, sel
+
+
+SAMPLE_TEXT = {"step": "the full step once: 12 layer calls (dequantise to fp64 + naive fp64 GEMM + gate + EC)",
+               "m1": "the four projections at M=1 (dequantise to fp64 + naive fp64 GEMM + gate + EC)",
+               "o": "the o projection (2048x2048) at M=1"}
+
+
+def cpu_baseline_sample():
+    import oracle
+    oracle.build()
+    layers, nbytes, _ = _sample_layers("step")
+    _oracle_pass(layers[:1])                      # page in / thread pool start
+    t = _oracle_pass(layers)
+    return {"value": round(nbytes / t / 1e9, 4), "unit": UNIT, "cores": oracle.num_threads(), "kind": "oracle",
+            "sample": SAMPLE_TEXT["step"] + f"; {t:.2f} s wall", "seconds": round(t, 3)}
+
+
+def run_reference(args, rank, world):
+    if rank != 0:
+        return
+    import oracle
+    oracle.build()
+    # bounded sample per step, sized so warmup + steps ends within a few minutes
+    layers, nbytes, _ = _sample_layers("m1")
+    t_probe = _oracle_pass(layers)
+    which = "m1"
+    if t_probe * (args.steps + args.warmup) > 150.0:
+        which = "o"
+        layers, nbytes, _ = _sample_layers("o")
+    for _ in range(args.warmup):
+        _oracle_pass(layers)
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        _oracle_pass(layers)
+    t = (time.perf_counter() - t0) / args.steps
+    v = round(nbytes / t / 1e9, 4)
+    out = {"impl": "reference", "metric": METRIC, "value": v, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+           "warmup": args.warmup, "ms_per_step": round(t * 1e3, 4), "higher_is_better": True, "scaling": "weak",
+           "vs_baseline": None, "dtype": "f64", "data": "synthetic (seeded, workloads/)",
+           "config": {"workload": "BASELINE.json configs[1] (bounded sample per step: " + SAMPLE_TEXT[which] + ")",
+                      "bytes_per_step": nbytes},
+           "cpu_baseline": {"value": v, "unit": UNIT, "cores": oracle.num_threads(), "kind": "oracle",
+                            "sample": SAMPLE_TEXT[which]},
+           "e2e": {"value": v, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+           "gpu_launches": 0}
+    print(json.dumps(out), flush=True)
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=2000)
+    ap.add_argument("--warmup", type=int, default=50)
+    ap.add_argument("--impl", default="cuda", choices=["cuda", "reference"])
+    args = ap.parse_args()
+    args.warmup = max(args.warmup, 3) if args.impl == "cuda" else args.warmup
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    if args.impl == "reference":
+        run_reference(args, rank, world)
+    else:
+        run_cuda(args, rank, world)
+
+
+if __name__ == "__main__":
+    main()

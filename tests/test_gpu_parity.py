@@ -197,8 +197,13 @@ def test_back_to_back_calls_leave_workspace_clean(sp):
     x = h.dev(li.x)
     ys = [h.run_layer(dl, x)[0].clone() for _ in range(5)]
     torch.cuda.synchronize()
-    for y in ys[1:]:
-        assert torch.equal(ys[0], y)
+    ref = oracle.forward_layer(li)["y"]
+    rms = float(np.sqrt(np.mean(ref ** 2)))
+    for y in ys:
+        # z is reduced with fp32 red.add, so the last bit may differ run to run; a dirty workspace
+        # (stale z, counters) would be off by whole EC terms
+        assert float(np.max(np.abs(y.cpu().numpy().astype(np.float64) - ref))) <= Y_TOL * rms
+        assert float((y.float() - ys[0].float()).abs().max()) <= 1e-3 * rms
 
 
 def test_errors(sp):
