@@ -102,9 +102,11 @@ typedef struct {
     const void* w_g;          /* [K]    fp16   scalar gate                                          */
     const void* b_g;          /* 1      fp32   scalar gate (device pointer; NULL = 0)               */
     void* gate_out;           /* optional: MLP -> [M][r] fp32, scalar -> [M] fp32; NULL = not written */
-    void* workspace;          /* NULL = library default; else >= spear_workspace_bytes(), zero-filled
-                                 once by the caller before first use (the library keeps its counters
-                                 zero between calls)                                                */
+    void* workspace;          /* NULL = library default; else 1024-byte aligned, >= spear_workspace_bytes(),
+                                 zero-filled once by the caller before first use (the library keeps its
+                                 counters and accumulators zero between calls).  Every call sharing one
+                                 buffer must pass the same workspace_bytes (a scratch region is placed
+                                 relative to the END of the buffer).                                    */
     size_t workspace_bytes;
     int force_variant;        /* spear_variant; SPEAR_VARIANT_AUTO = use the plan                   */
 } spear_ec_desc;

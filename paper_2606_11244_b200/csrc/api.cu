@@ -47,15 +47,19 @@ constexpr size_t kCounterBytes = 64 * 1024;          // 16384 u32
 constexpr int kEcPreCounter = 8192;                  // index into counters[]
 constexpr int kMaxStreamGrid = 1024;
 static size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
-static WsLayout ws_layout(int M, int r) {
+// Fixed-size regions first; the two regions whose size depends on M must never alias a region that a
+// call with another M leaves non-zero: zbuf (kept zero between calls) grows up from a fixed offset and
+// u16 (scratch) grows DOWN from the end of the workspace.
+static WsLayout ws_layout(int M, int r, size_t ws_bytes) {
     WsLayout L;
     size_t o = 0;
     L.counters = o; o += kCounterBytes;
-    L.zbuf = o; o += align_up(size_t(M > 16 ? M : 16) * kZStride * 4, 1024);
     L.u32 = o; o += align_up(size_t(16) * 128 * 4, 1024);
     L.partial = o; o += size_t(kMaxStreamGrid) * 2 * 16 * 128 * 4;
-    L.u16 = o; o += align_up(size_t(M) * size_t(r) * 2 + 1024, 1024);
-    L.total = o;
+    L.zbuf = o; o += align_up(size_t(M > 16 ? M : 16) * kZStride * 4, 1024);
+    const size_t u16_bytes = align_up(size_t(M) * size_t(r) * 2 + 1024, 1024);
+    L.total = o + u16_bytes;
+    L.u16 = ws_bytes >= L.total ? (ws_bytes - u16_bytes) & ~size_t(1023) : o;
     return L;
 }
 constexpr size_t kDefaultWorkspace = size_t(96) << 20;
@@ -304,7 +308,6 @@ static int layer_impl(const void* x, const void* Wq, const void* scales, const v
     if (int rc = spear_init()) return rc;
     if (r == 0) { A = nullptr; B = nullptr; }
     if (int rc = check_problem(x, Wq, scales, A, B, ec, y, M, N, K, r, group)) return rc;
-    const WsLayout L = ws_layout(M, r);
     uint8_t* ws = static_cast<uint8_t*>(g_ws);
     size_t ws_bytes = g_ws_bytes;
     if (ec && ec->workspace) {
@@ -312,7 +315,8 @@ static int layer_impl(const void* x, const void* Wq, const void* scales, const v
         ws_bytes = ec->workspace_bytes;
         if (uintptr_t(ws) & 1023) return set_error(SPEAR_EINVAL, "workspace must be 1024-byte aligned");
     }
-    if (ws_bytes < L.total)
+    const WsLayout L = ws_layout(M, r, ws_bytes);
+    if (ws_bytes < L.total + 1024)
         return set_error(SPEAR_ENOMEM, "workspace too small: need %zu bytes, have %zu (pass spear_ec_desc.workspace)", L.total, ws_bytes);
     const int gate = (r > 0 && ec) ? ec->gate_kind : SPEAR_GATE_NONE;
     int v = (ec && ec->force_variant != SPEAR_VARIANT_AUTO) ? ec->force_variant : choose_variant(M, N, K, r, group, gate);
@@ -358,7 +362,7 @@ extern "C" int spear_tune(const char* key, int value) {
 extern "C" int spear_workspace_bytes(int M, int N, int K, int r, int group, size_t* bytes) {
     (void)N; (void)K; (void)group;
     if (!bytes || M < 1 || r < 0) return set_error(SPEAR_EINVAL, "bad arguments");
-    *bytes = ws_layout(M, r).total;
+    *bytes = ws_layout(M, r, 0).total + 1024;
     return SPEAR_OK;
 }
 

@@ -1,0 +1,159 @@
+"""GPU parity for the tcgen05 path (SPEAR_VARIANT_TC_FUSED, M > 16): libspear.so through the C ABI
+against the fp64 CPU oracle on the same seeded inputs.  Small shapes compare every element; the
+BASELINE.json prefill shapes compare all N columns of a seeded row sample (each y[m][:] depends on
+x[m][:] only, so sampling rows is exact -- SURVEY.md 8(c) large-shape policy)."""
+import numpy as np
+import pytest
+
+import oracle
+from workloads import make_layer, config_shapes
+
+pytestmark = pytest.mark.gpu
+
+Y_TOL = 1e-2
+GATE_TOL = 1e-3
+TC = 3          # SPEAR_VARIANT_TC_FUSED
+STREAM = 2      # SPEAR_VARIANT_STREAM_SPLIT
+
+
+@pytest.fixture(scope="module")
+def sp():
+    import paper_2606_11244_b200 as sp
+    sp.init()
+    return sp
+
+
+def _h():
+    from paper_2606_11244_b200 import harness
+    return harness
+
+
+def sample_rows(M, seed, extra=48):
+    """One seeded row per 128-row block + `extra` random rows + the first and last row."""
+    rng = np.random.default_rng(seed)
+    rows = {0, M - 1}
+    for b in range(0, M, 128):
+        rows.add(int(b + rng.integers(0, min(128, M - b))))
+    rows.update(int(v) for v in rng.integers(0, M, size=extra))
+    return np.array(sorted(rows))
+
+
+def check(li, variant=TC, rows=None, label=""):
+    import torch
+    h = _h()
+    dl = h.upload_layer(li)
+    x = h.dev(li.x)
+    y, gate = h.run_layer(dl, x, variant=variant, want_gate=True)
+    torch.cuda.synchronize()
+    yg = y.cpu().numpy().astype(np.float64)
+    ref = oracle.forward_layer(li, rows=rows)
+    yr = ref["y"]
+    if rows is not None:
+        yg = yg[rows]
+    rms = float(np.sqrt(np.mean(yr ** 2)))
+    err = float(np.max(np.abs(yg - yr)))
+    assert np.all(np.isfinite(yg)), label
+    assert err <= Y_TOL * rms, f"{label}: max err {err:.4g} > {Y_TOL} * rms {rms:.4g}"
+    if gate is not None and ref["gam"] is not None:
+        gg = gate.cpu().numpy().astype(np.float64)
+        if rows is not None:
+            gg = gg[rows]
+        assert float(np.max(np.abs(gg - ref["gam"]))) <= GATE_TOL, label
+    return y
+
+
+@pytest.mark.parametrize("M", [17, 32, 33, 64, 100, 128, 129, 256, 300, 520])
+def test_tc_token_counts(sp, M):
+    # every token-tile width (32/64/128/256), ragged tails, several panels, K not a power of two
+    li = make_layer(900 + M, M, 384, 640, 128, 24, gate="scalar")
+    check(li, label=f"tc M={M}")
+
+
+@pytest.mark.parametrize("r", [0, 8, 16, 64, 72, 128])
+@pytest.mark.parametrize("gate", ["scalar", "mlp", "none"])
+def test_tc_ranks_and_gates(sp, r, gate):
+    if r == 0 and gate != "scalar":
+        pytest.skip("r = 0 has no gate")
+    li = make_layer(1000 + r, 200, 256, 512, 128, r, gate=gate)
+    check(li, label=f"tc r={r} {gate}")
+
+
+@pytest.mark.parametrize("group,K", [(128, 1024), (256, 1024), (1024, 1024), (1792, 1792)])
+def test_tc_groups(sp, group, K):
+    li = make_layer(1100 + group, 96, 256, K, group, 16, gate="scalar")
+    check(li, label=f"tc group={group}")
+
+
+def test_tc_many_tiles_per_cta(sp):
+    # more tiles than SMs: exercises the persistent schedule, both TMEM accumulators and ring wrap-around
+    li = make_layer(1200, 1100, 6144, 256, 128, 16, gate="scalar")
+    check(li, rows=sample_rows(1100, 1), label="tc many tiles")
+
+
+def test_tc_matches_stream_variant(sp):
+    """P11: the same M = 16 problem through the decode kernel and through the tcgen05 kernel."""
+    import torch
+    h = _h()
+    li = make_layer(1300, 16, 512, 1024, 128, 32, gate="mlp")
+    dl = h.upload_layer(li)
+    x = h.dev(li.x)
+    ya, _ = h.run_layer(dl, x, variant=STREAM)
+    yb, _ = h.run_layer(dl, x, variant=TC)
+    ref = oracle.forward_layer(li)["y"]
+    rms = float(np.sqrt(np.mean(ref ** 2)))
+    assert float((ya.float() - yb.float()).abs().max()) <= Y_TOL * rms
+
+
+def test_tc_gate_zero_is_plain_w4(sp):
+    import torch
+    h = _h()
+    li = make_layer(1400, 150, 256, 512, 128, 16, gate="scalar")
+    plain = make_layer(1400, 150, 256, 512, 128, 0)
+    y0, _ = h.run_layer(h.upload_layer(plain), h.dev(plain.x), variant=TC)
+    li.b_g = -100.0
+    y1, _ = h.run_layer(h.upload_layer(li), h.dev(li.x), variant=TC)
+    assert torch.equal(y0, y1)
+
+
+def test_tc_back_to_back(sp):
+    import torch
+    h = _h()
+    li = make_layer(1500, 260, 384, 1024, 128, 32, gate="scalar")
+    dl = h.upload_layer(li)
+    x = h.dev(li.x)
+    ys = [h.run_layer(dl, x, variant=TC)[0].clone() for _ in range(4)]
+    torch.cuda.synchronize()
+    ref = oracle.forward_layer(li)["y"]
+    rms = float(np.sqrt(np.mean(ref ** 2)))
+    for y in ys:
+        assert float(np.max(np.abs(y.cpu().numpy().astype(np.float64) - ref))) <= Y_TOL * rms
+
+
+@pytest.mark.parametrize("idx", [6, 7, 8])
+def test_config3_prefill_M256(sp, idx):
+    s = config_shapes(2)[idx]
+    assert s.M == 256
+    li = make_layer(s.seed, s.M, s.N, s.K, s.group, s.r, gate="scalar")
+    check(li, variant=0, rows=sample_rows(s.M, s.seed, extra=16), label=f"config3 {s.name} M=256")
+
+
+@pytest.mark.parametrize("idx", [9, 11])
+def test_config3_prefill_M2048(sp, idx):
+    s = config_shapes(2)[idx]
+    assert s.M == 2048
+    li = make_layer(s.seed, s.M, s.N, s.K, s.group, s.r, gate="scalar")
+    check(li, variant=0, rows=sample_rows(s.M, s.seed, extra=8), label=f"config3 {s.name} M=2048")
+
+
+@pytest.mark.parametrize("r", [0, 64])
+def test_config4_M512(sp, r):
+    s = [c for c in config_shapes(3) if c.M == 512 and c.r == r][0]
+    li = make_layer(s.seed, s.M, s.N, s.K, s.group, s.r, gate="scalar")
+    check(li, variant=0, rows=sample_rows(s.M, s.seed, extra=8), label=f"config4 M=512 r={r}")
+
+
+@pytest.mark.parametrize("name", ["L0.qkv", "L0.o", "L0.gate_up", "L0.down", "L7.down"])
+def test_config5_M64(sp, name):
+    s = [c for c in config_shapes(4) if c.M == 64 and c.name == name][0]
+    li = make_layer(s.seed, s.M, s.N, s.K, s.group, s.r, gate="scalar")
+    check(li, variant=0, label=f"config5 {name} M=64")
