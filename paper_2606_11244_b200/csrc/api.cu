@@ -151,6 +151,7 @@ struct Tunables {
     int pdl = 1;                  // programmatic dependent launch between the library's kernels
     int ecpre_ctas = 0;           // 0 = heuristic
     int tc_grid = 0;              // 0 = heuristic
+    int tc_cluster = 0;           // 0 = heuristic, else 1 / 2 / 4
 };
 static Tunables g_tune;
 
@@ -300,6 +301,7 @@ static int run_tc_fused(const void* x, const void* Wq, const void* scales, const
     t.M = M; t.N = N; t.K = K; t.r = r; t.group = group;
     t.pdl = pdl;
     t.grid_override = g_tune.tc_grid;
+    t.cluster_override = g_tune.tc_cluster;
     return run_tc(t, st);
 }
 
@@ -355,6 +357,7 @@ extern "C" int spear_tune(const char* key, int value) {
     else if (!strcmp(key, "pdl")) g_tune.pdl = value;
     else if (!strcmp(key, "ecpre_ctas")) g_tune.ecpre_ctas = value;
     else if (!strcmp(key, "tc_grid")) g_tune.tc_grid = value;
+    else if (!strcmp(key, "tc_cluster")) g_tune.tc_cluster = value;
     else return set_error(SPEAR_EINVAL, "unknown tunable '%s'", key);
     return SPEAR_OK;
 }

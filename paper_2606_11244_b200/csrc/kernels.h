@@ -67,6 +67,7 @@ struct TcProblem {
     int M, N, K, r, group;
     bool pdl;
     int grid_override;
+    int cluster_override;    // 0 = heuristic, else 1 / 2 / 4 CTAs sharing x tiles by TMA multicast
 };
 bool tc_available();
 int run_tc(const TcProblem& t, cudaStream_t st);

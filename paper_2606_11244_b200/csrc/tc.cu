@@ -14,14 +14,14 @@
 // (lane = output channel, column = token), two accumulators in flight so that the epilogue of tile i
 // overlaps the main loop of tile i+1.
 //
-// Warp roles (448 threads, one CTA per SM, persistent over a static tile schedule):
+// Warp roles (704 threads, one CTA per SM, persistent over a static tile schedule):
 //   warp 0      producer: cp.async.bulk of the packed int4 (4 KiB per (panel, 64-k tile)) + 256 B of
 //               scales into a small ring; TMA tensor loads of the x tile (BT x 64 fp16, SWIZZLE_128B).
 //               int4 copies never wait for the previous kernel; x / u16 loads come after griddepcontrol.wait.
 //   warp 1      allocates TMEM; one elected lane issues tcgen05.mma (4 x K=16 per k-block) and commits
 //               to the mbarriers that free the operand stages / publish the accumulator.
 //   warps 2-5   epilogue: tcgen05.ld the accumulator, one RN-even cast to fp16, store y.
-//   warps 6-13  dequantisation: LDS.128 of int4 -> lop3 / sub / fma (exact q - 8) -> mul by the fp16
+//   warps 6-21  dequantisation (two groups of 8 warps taking k-blocks alternately): LDS.128 of int4 -> lop3 / sub / fma (exact q - 8) -> mul by the fp16
 //               group scale (one rounding: the same RN_fp16((q-8)*s) the dequant test hook exports)
 //               -> STS.128 into the K-major 128-byte-swizzled A-operand stage, fence.proxy.async, arrive.
 #include <algorithm>
@@ -72,6 +72,27 @@ __device__ __forceinline__ void tmem_ld32(uint32_t taddr, uint32_t (&v)[32]) {
         : "r"(taddr)
         : "memory");
 }
+// cluster variants: the commit arrives on the barrier at the same offset in every CTA of `mask`; the TMA
+// load writes the box into the same shared-memory offset of every CTA of `mask` and completes tx there.
+__device__ __forceinline__ void umma_commit_mc(uint64_t* bar, uint16_t mask) {
+    asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.multicast::cluster.b64 [%0], %1;" ::"r"(smem_u32(bar)), "h"(mask) : "memory");
+}
+__device__ __forceinline__ void tma_load_2d_mc(void* dst, const CUtensorMap* map, int c0, int c1, uint64_t* bar,
+                                               uint16_t mask, uint64_t policy) {
+    asm volatile(
+        "cp.async.bulk.tensor.2d.shared::cluster.global.tile.mbarrier::complete_tx::bytes.multicast::cluster.L2::cache_hint "
+        "[%0], [%1, {%3, %4}], [%2], %5, %6;" ::"r"(smem_u32(dst)),
+        "l"(map), "r"(smem_u32(bar)), "r"(c0), "r"(c1), "h"(mask), "l"(policy)
+        : "memory");
+}
+__device__ __forceinline__ uint32_t cluster_ctarank() {
+    uint32_t r;
+    asm volatile("mov.u32 %0, %%cluster_ctarank;" : "=r"(r));
+    return r;
+}
+__device__ __forceinline__ void cluster_sync_all() {
+    asm volatile("barrier.cluster.arrive.release.aligned;\n\tbarrier.cluster.wait.acquire.aligned;" ::: "memory");
+}
 __device__ __forceinline__ void tmem_ld_wait() { asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory"); }
 
 // ---- configuration -----------------------------------------------------------------------------
@@ -83,27 +104,30 @@ struct TcParams {
     int G, group;            // K / group, group
     int kb_w;                // K / 64 weight k-blocks
     int kb_ec;               // ceil(r / 64) EC k-blocks
-    int n_panels, n_mt;      // N / 128, ceil(M / BT)
+    int n_pp, n_mt;          // N / (128 * CS) panel groups (CS = cluster size), ceil(M / BT)
     int mt_group;            // token tiles per raster group (keeps the x slice L2-resident)
-    int n_tiles;
+    int n_tiles;             // n_pp * n_mt work items; each is taken by one cluster (CTA rank c -> panel pp * CS + c)
 };
 
 template <int BT>
 struct TcCfg {
-    static constexpr int kStages = BT == 256 ? 4 : (BT == 128 ? 5 : (BT == 64 ? 6 : 8));
-    static constexpr int kW4Stages = BT == 256 ? 6 : 8;
+    // the x ring hides an L2 round trip per stage (deep); the A ring only the local dequantisation (shallow)
+    static constexpr int kXStages = BT == 256 ? 5 : (BT == 128 ? 8 : 10);
+    static constexpr int kAStages = 3;
+    static constexpr int kW4Stages = BT == 256 ? 4 : 8;
     static constexpr int kABytes = 128 * 128;            // 128 channels x 64 k fp16
     static constexpr int kXBytes = BT * 128;             // BT tokens x 64 k fp16
     static constexpr int kW4Bytes = 4096 + 256;          // codes + scales of one (panel, 64-k tile)
     static constexpr int kTmemCols = 2 * BT < 32 ? 32 : 2 * BT;
-    static constexpr size_t kSmemBytes = 1024 + size_t(kStages) * (kABytes + kXBytes) + size_t(kW4Stages) * kW4Bytes + 512;
+    static constexpr size_t kSmemBytes = 1024 + size_t(kAStages) * kABytes + size_t(kXStages) * kXBytes + size_t(kW4Stages) * kW4Bytes + 512;
     static_assert(kSmemBytes <= 232448, "exceeds the 227 KiB opt-in shared memory of sm_100");
     static constexpr uint32_t kIdesc = (1u << 4) | (uint32_t(BT >> 3) << 17) | (uint32_t(128 >> 4) << 24);
 };
-constexpr int kTcThreads = 448;
+constexpr int kDequantGroups = 2;        // warp groups of 8 taking k-blocks round-robin (hides the per-k-block barrier latency)
+constexpr int kTcThreads = (7 + 8 * kDequantGroups) * 32;   // + x producer, MMA, 4 epilogue, int4 producer
 
 __device__ __forceinline__ void tile_coords(const TcParams& p, int tile, int& panel, int& mt) {
-    const int per_group = p.mt_group * p.n_panels;
+    const int per_group = p.mt_group * p.n_pp;
     const int grp = tile / per_group;
     const int mt0 = grp * p.mt_group;
     const int width = min(p.mt_group, p.n_mt - mt0);
@@ -112,22 +136,23 @@ __device__ __forceinline__ void tile_coords(const TcParams& p, int tile, int& pa
     mt = mt0 + rem - panel * width;
 }
 
-template <int BT>
+template <int BT, int CS>
 __global__ void __launch_bounds__(kTcThreads, 1)
 tc_kernel(const __grid_constant__ CUtensorMap xmap, const __grid_constant__ CUtensorMap umap,
           const __grid_constant__ CUtensorMap bmap, const TcParams p) {
     using Cfg = TcCfg<BT>;
-    constexpr int S = Cfg::kStages, S4 = Cfg::kW4Stages;
+    constexpr int SX = Cfg::kXStages, SA = Cfg::kAStages, S4 = Cfg::kW4Stages;
     extern __shared__ uint8_t smem_raw[];
     uint8_t* base = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
     uint8_t* a_ring = base;                                   // S x 16 KiB, 1024-aligned
-    uint8_t* x_ring = a_ring + size_t(S) * Cfg::kABytes;      // S x BT*128 B, 1024-aligned
-    uint8_t* w4_ring = x_ring + size_t(S) * Cfg::kXBytes;     // S4 x 4352 B
+    uint8_t* x_ring = a_ring + size_t(SA) * Cfg::kABytes;     // SX x BT*128 B, 1024-aligned
+    uint8_t* w4_ring = x_ring + size_t(SX) * Cfg::kXBytes;    // S4 x 4352 B
     uint64_t* bars = reinterpret_cast<uint64_t*>(w4_ring + size_t(S4) * Cfg::kW4Bytes);
-    uint64_t* x_full = bars;              // [S]  producer TMA (tx bytes)
-    uint64_t* a_full = x_full + S;        // [S]  8 dequant-warp arrivals (+ tx bytes for EC k-blocks)
-    uint64_t* xa_empty = a_full + S;      // [S]  tcgen05.commit
-    uint64_t* w4_full = xa_empty + S;     // [S4] producer bulk copy (tx bytes)
+    uint64_t* x_full = bars;              // [SX] producer TMA (tx bytes)
+    uint64_t* x_empty = x_full + SX;      // [SX] tcgen05.commit (from every CTA of the cluster)
+    uint64_t* a_full = x_empty + SX;      // [SA] 8 dequant-warp arrivals (+ tx bytes for EC k-blocks)
+    uint64_t* a_empty = a_full + SA;      // [SA] tcgen05.commit
+    uint64_t* w4_full = a_empty + SA;     // [S4] producer bulk copy (tx bytes)
     uint64_t* w4_empty = w4_full + S4;    // [S4] 8 dequant-warp arrivals
     uint64_t* acc_full = w4_empty + S4;   // [2]  tcgen05.commit
     uint64_t* acc_empty = acc_full + 2;   // [2]  4 epilogue-warp arrivals
@@ -135,9 +160,15 @@ tc_kernel(const __grid_constant__ CUtensorMap xmap, const __grid_constant__ CUte
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int kb_total = p.kb_w + p.kb_ec;
+    // a cluster of CS CTAs shares every x tile: each CTA fetches BT / CS token rows and multicasts them
+    const int cta_rank = CS > 1 ? int(cluster_ctarank()) : 0;
+    const int work0 = blockIdx.x / CS, work_stride = gridDim.x / CS;
+    constexpr uint16_t kMask = uint16_t((1u << CS) - 1);
+    constexpr int kXRows = BT / CS;
 
     if (threadIdx.x == 0) {
-        for (int s = 0; s < S; ++s) { mbar_init(&x_full[s], 1); mbar_init(&a_full[s], 8); mbar_init(&xa_empty[s], 1); }
+        for (int s = 0; s < SX; ++s) { mbar_init(&x_full[s], 1); mbar_init(&x_empty[s], CS); }
+        for (int s = 0; s < SA; ++s) { mbar_init(&a_full[s], 8); mbar_init(&a_empty[s], 1); }
         for (int s = 0; s < S4; ++s) { mbar_init(&w4_full[s], 1); mbar_init(&w4_empty[s], 8); }
         for (int s = 0; s < 2; ++s) { mbar_init(&acc_full[s], 1); mbar_init(&acc_empty[s], 4); }
         fence_mbar_init();
@@ -147,72 +178,77 @@ tc_kernel(const __grid_constant__ CUtensorMap xmap, const __grid_constant__ CUte
     if (warp == 1) tmem_alloc<Cfg::kTmemCols>(tmem_slot);
     tc_fence_before();
     __syncthreads();
+    if (CS > 1) cluster_sync_all();      // peers' barriers are initialised before anything arrives on them
     tc_fence_after();
     const uint32_t tmem_base = *tmem_slot;
     pdl_launch_dependents();
 
     if (warp == 0) {
-        // ---------------------------------- producer ----------------------------------
+        // ---------------------------------- x producer ----------------------------------
         if (lane == 0) {
-            const uint64_t pol_w = policy_evict_first(), pol_x = policy_evict_last();
-            // the two rings advance independently: int4 copies run ahead of the x loads by up to S4 k-blocks
-            int w_tile = blockIdx.x, w_kb = 0, w_it = 0;          // next int4 copy to issue
-            auto issue_w4 = [&]() {
-                int panel, mt;
-                tile_coords(p, w_tile, panel, mt);
-                const int s4 = w_it % S4;
-                mbar_wait(&w4_empty[s4], ((w_it / S4) & 1) ^ 1);
-                mbar_arrive_expect_tx(&w4_full[s4], Cfg::kW4Bytes);
-                uint8_t* dst = w4_ring + size_t(s4) * Cfg::kW4Bytes;
-                bulk_g2s(dst, p.wq + (size_t(panel) * p.kb_w + w_kb) * 4096, 4096, &w4_full[s4], pol_w);
-                bulk_g2s(dst + 4096, p.scales + (size_t(panel) * p.G + (w_kb * 64) / p.group) * 256, 256, &w4_full[s4], pol_x);
-                ++w_it;
-                if (++w_kb == p.kb_w) { w_kb = 0; w_tile += gridDim.x; }
-            };
-            // prologue: fill the int4 ring before waiting for the previous kernel (weights never depend on it)
-            for (int i = 0; i < S4 && w_tile < p.n_tiles; ++i) issue_w4();
-            pdl_wait();
+            const uint64_t pol_x = policy_evict_last();
+            pdl_wait();      // x / u16 may be written by the previous kernel in the stream
             int it = 0;
-            for (int tile = blockIdx.x; tile < p.n_tiles; tile += gridDim.x) {
+            for (int tile = work0; tile < p.n_tiles; tile += work_stride) {
                 int panel, mt;
                 tile_coords(p, tile, panel, mt);
+                const int c1 = mt * BT + cta_rank * kXRows;
                 for (int kb = 0; kb < kb_total; ++kb, ++it) {
-                    const int s = it % S;
-                    mbar_wait(&xa_empty[s], ((it / S) & 1) ^ 1);
+                    const int s = it % SX;
+                    mbar_wait(&x_empty[s], ((it / SX) & 1) ^ 1);
                     mbar_arrive_expect_tx(&x_full[s], Cfg::kXBytes);
-                    if (kb < p.kb_w) tma_load_2d(x_ring + size_t(s) * Cfg::kXBytes, &xmap, kb * 64, mt * BT, &x_full[s], pol_x);
-                    else tma_load_2d(x_ring + size_t(s) * Cfg::kXBytes, &umap, (kb - p.kb_w) * 64, mt * BT, &x_full[s], pol_x);
-                    if (w_tile < p.n_tiles) {
-                        // keep the int4 ring topped up without blocking on it
-                        const int s4 = w_it % S4;
-                        if (mbar_try_wait(&w4_empty[s4], ((w_it / S4) & 1) ^ 1)) issue_w4();
-                    }
+                    uint8_t* dst = x_ring + size_t(s) * Cfg::kXBytes + size_t(cta_rank) * kXRows * 128;
+                    const CUtensorMap* map = kb < p.kb_w ? &xmap : &umap;
+                    const int c0 = (kb < p.kb_w ? kb : kb - p.kb_w) * 64;
+                    if (CS > 1) tma_load_2d_mc(dst, map, c0, c1, &x_full[s], kMask, pol_x);
+                    else tma_load_2d(dst, map, c0, c1, &x_full[s], pol_x);
                 }
             }
-            // int4 copies the loop above did not get to (cannot happen unless kb_ec == 0 and try_wait lagged)
-            while (w_tile < p.n_tiles) issue_w4();
+        }
+    } else if (warp == kTcThreads / 32 - 1) {
+        // ---------------------------------- int4 producer ----------------------------------
+        // weights never depend on the previous kernel: no griddepcontrol.wait on this path
+        if (lane == 0) {
+            const uint64_t pol_w = policy_evict_first(), pol_s = policy_evict_last();
+            int w_it = 0;
+            for (int tile = work0; tile < p.n_tiles; tile += work_stride) {
+                int panel, mt;
+                tile_coords(p, tile, panel, mt);
+                panel = panel * CS + cta_rank;
+                const uint8_t* wsrc = p.wq + size_t(panel) * p.kb_w * 4096;
+                const uint8_t* ssrc = p.scales + size_t(panel) * p.G * 256;
+                for (int kb = 0; kb < p.kb_w; ++kb, ++w_it) {
+                    const int s4 = w_it % S4;
+                    mbar_wait(&w4_empty[s4], ((w_it / S4) & 1) ^ 1);
+                    mbar_arrive_expect_tx(&w4_full[s4], Cfg::kW4Bytes);
+                    uint8_t* dst = w4_ring + size_t(s4) * Cfg::kW4Bytes;
+                    bulk_g2s(dst, wsrc + size_t(kb) * 4096, 4096, &w4_full[s4], pol_w);
+                    bulk_g2s(dst + 4096, ssrc + size_t((kb * 64) / p.group) * 256, 256, &w4_full[s4], pol_s);
+                }
+            }
         }
     } else if (warp == 1) {
         // ---------------------------------- MMA issuer ----------------------------------
         int it = 0, tcount = 0;
-        for (int tile = blockIdx.x; tile < p.n_tiles; tile += gridDim.x, ++tcount) {
+        for (int tile = work0; tile < p.n_tiles; tile += work_stride, ++tcount) {
             const int acc = tcount & 1;
             mbar_wait(&acc_empty[acc], ((tcount >> 1) & 1) ^ 1);
             tc_fence_after();
             const uint32_t d_tmem = tmem_base + uint32_t(acc * BT);
             for (int kb = 0; kb < kb_total; ++kb, ++it) {
-                const int s = it % S;
-                const uint32_t ph = (it / S) & 1;
-                mbar_wait(&x_full[s], ph);
-                mbar_wait(&a_full[s], ph);
+                const int s = it % SX, sa = it % SA;
+                mbar_wait(&x_full[s], (it / SX) & 1);
+                mbar_wait(&a_full[sa], (it / SA) & 1);
                 tc_fence_after();
                 if (elect_one()) {
-                    const uint64_t a_desc = umma_desc_sw128(smem_u32(a_ring + size_t(s) * Cfg::kABytes));
+                    const uint64_t a_desc = umma_desc_sw128(smem_u32(a_ring + size_t(sa) * Cfg::kABytes));
                     const uint64_t b_desc = umma_desc_sw128(smem_u32(x_ring + size_t(s) * Cfg::kXBytes));
 #pragma unroll
                     for (int k = 0; k < 4; ++k)   // K = 16 per instruction: +32 bytes inside the swizzle atom
                         umma_f16(d_tmem, a_desc + uint64_t(k * 2), b_desc + uint64_t(k * 2), Cfg::kIdesc, (kb | k) != 0);
-                    umma_commit(&xa_empty[s]);
+                    if (CS > 1) umma_commit_mc(&x_empty[s], kMask);
+                    else umma_commit(&x_empty[s]);
+                    umma_commit(&a_empty[sa]);
                     if (kb == kb_total - 1) umma_commit(&acc_full[acc]);
                 }
                 __syncwarp();
@@ -222,9 +258,10 @@ tc_kernel(const __grid_constant__ CUtensorMap xmap, const __grid_constant__ CUte
         // ---------------------------------- epilogue ----------------------------------
         const int q = warp & 3;                 // TMEM lane quarter this warp may access
         int tcount = 0;
-        for (int tile = blockIdx.x; tile < p.n_tiles; tile += gridDim.x, ++tcount) {
+        for (int tile = work0; tile < p.n_tiles; tile += work_stride, ++tcount) {
             int panel, mt;
             tile_coords(p, tile, panel, mt);
+            panel = panel * CS + cta_rank;
             const int acc = tcount & 1;
             mbar_wait(&acc_full[acc], (tcount >> 1) & 1);
             tc_fence_after();
@@ -247,16 +284,22 @@ tc_kernel(const __grid_constant__ CUtensorMap xmap, const __grid_constant__ CUte
         }
     } else {
         // ---------------------------------- dequantisation ----------------------------------
-        const int strip = warp - 6;             // 16 output channels of the panel
+        const int strip = (warp - 6) & 7;       // 16 output channels of the panel
+        const int dgroup = (warp - 6) >> 3;     // this warp converts the k-blocks with it % kDequantGroups == dgroup
         const int g = lane >> 2, t = lane & 3;
         int it = 0, w_it = 0;
-        for (int tile = blockIdx.x; tile < p.n_tiles; tile += gridDim.x) {
+        for (int tile = work0; tile < p.n_tiles; tile += work_stride) {
             int panel, mt;
             tile_coords(p, tile, panel, mt);
+            panel = panel * CS + cta_rank;
             for (int kb = 0; kb < kb_total; ++kb, ++it) {
-                const int s = it % S;
+                const int s = it % SA;
                 uint8_t* a_stage = a_ring + size_t(s) * Cfg::kABytes;
-                mbar_wait(&xa_empty[s], ((it / S) & 1) ^ 1);
+                if (it % kDequantGroups != dgroup) {
+                    if (kb < p.kb_w) ++w_it;
+                    continue;
+                }
+                mbar_wait(&a_empty[s], ((it / SA) & 1) ^ 1);
                 if (kb < p.kb_w) {
                     const int s4 = w_it % S4;
                     mbar_wait(&w4_full[s4], (w_it / S4) & 1);
@@ -302,6 +345,7 @@ tc_kernel(const __grid_constant__ CUtensorMap xmap, const __grid_constant__ CUte
 
     tc_fence_before();
     __syncthreads();
+    if (CS > 1) cluster_sync_all();      // no CTA leaves while a peer may still multicast into it or arrive on its barriers
     if (warp == 1) {
         tc_fence_after();
         tmem_dealloc<Cfg::kTmemCols>(tmem_base);
@@ -311,32 +355,57 @@ tc_kernel(const __grid_constant__ CUtensorMap xmap, const __grid_constant__ CUte
 // ---- host side -----------------------------------------------------------------------------------
 bool tc_available() { return true; }
 
-template <int BT>
+template <int BT, int CS>
 static int launch_tc(const CUtensorMap& xmap, const CUtensorMap& umap, const CUtensorMap& bmap, const TcParams& p,
-                     int grid, bool pdl, cudaStream_t st) {
-    static bool attr_set = false;
-    if (!attr_set) {
-        SPEAR_CUDA_OK(cudaFuncSetAttribute(tc_kernel<BT>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                     int grid_override, bool pdl, cudaStream_t st) {
+    static int max_clusters = 0;     // co-resident clusters of CS CTAs (one CTA per SM)
+    if (!max_clusters) {
+        SPEAR_CUDA_OK(cudaFuncSetAttribute(tc_kernel<BT, CS>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                            int(TcCfg<BT>::kSmemBytes)));
-        attr_set = true;
+        int n = device_info().num_sms / CS;
+        if (CS > 1) {
+            cudaLaunchConfig_t q = {};
+            q.gridDim = dim3(device_info().num_sms / CS * CS);
+            q.blockDim = dim3(kTcThreads);
+            q.dynamicSmemBytes = TcCfg<BT>::kSmemBytes;
+            cudaLaunchAttribute qa[1];
+            qa[0].id = cudaLaunchAttributeClusterDimension;
+            qa[0].val.clusterDim.x = CS; qa[0].val.clusterDim.y = 1; qa[0].val.clusterDim.z = 1;
+            q.attrs = qa; q.numAttrs = 1;
+            int nc = 0;
+            SPEAR_CUDA_OK(cudaOccupancyMaxActiveClusters(&nc, tc_kernel<BT, CS>, &q));
+            if (nc < 1) return set_error(SPEAR_ECUDA, "tc_kernel<%d,%d>: no co-resident cluster fits", BT, CS);
+            n = std::min(n, nc);
+        }
+        max_clusters = n;
     }
+    int clusters = std::min(p.n_tiles, max_clusters);
+    if (grid_override > 0) clusters = std::min(clusters, std::max(1, grid_override / CS));
     cudaLaunchConfig_t cfg = {};
-    cfg.gridDim = dim3(grid);
+    cfg.gridDim = dim3(clusters * CS);
     cfg.blockDim = dim3(kTcThreads);
     cfg.dynamicSmemBytes = TcCfg<BT>::kSmemBytes;
     cfg.stream = st;
-    cudaLaunchAttribute attr[1];
+    cudaLaunchAttribute attr[2];
     attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
     attr[0].val.programmaticStreamSerializationAllowed = pdl ? 1 : 0;
+    attr[1].id = cudaLaunchAttributeClusterDimension;
+    attr[1].val.clusterDim.x = CS; attr[1].val.clusterDim.y = 1; attr[1].val.clusterDim.z = 1;
     cfg.attrs = attr;
-    cfg.numAttrs = 1;
-    SPEAR_CUDA_OK(cudaLaunchKernelEx(&cfg, tc_kernel<BT>, xmap, umap, bmap, p));
+    cfg.numAttrs = CS > 1 ? 2 : 1;
+    SPEAR_CUDA_OK(cudaLaunchKernelEx(&cfg, tc_kernel<BT, CS>, xmap, umap, bmap, p));
     count_launch();
     return SPEAR_OK;
 }
 
 int run_tc(const TcProblem& t, cudaStream_t st) {
     const int BT = t.M <= 32 ? 32 : (t.M <= 64 ? 64 : (t.M <= 128 ? 128 : 256));
+    const int n_panels = t.N / 128;
+    const int n_mt = (t.M + BT - 1) / BT;
+    // clusters share x tiles by TMA multicast; worth it once there are more tiles than SMs (L2 -> SM bound)
+    int CS = 1;
+    if (BT == 256 && n_panels * n_mt >= 2 * device_info().num_sms) CS = (n_panels % 4 == 0) ? 4 : (n_panels % 2 == 0 ? 2 : 1);
+    if (t.cluster_override > 0 && BT == 256 && n_panels % t.cluster_override == 0) CS = t.cluster_override;
     TcParams p = {};
     p.wq = static_cast<const uint8_t*>(t.wq);
     p.scales = static_cast<const uint8_t*>(t.scales);
@@ -345,27 +414,28 @@ int run_tc(const TcProblem& t, cudaStream_t st) {
     p.group = t.group; p.G = t.K / t.group;
     p.kb_w = t.K / 64;
     p.kb_ec = (t.r + 63) / 64;
-    p.n_panels = t.N / 128;
-    p.n_mt = (t.M + BT - 1) / BT;
+    p.n_pp = n_panels / CS;
+    p.n_mt = n_mt;
     // raster: token tiles in groups whose x slice (mt_group * BT * K * 2 bytes) stays L2-resident
     const size_t slice = size_t(BT) * t.K * 2;
     p.mt_group = int(std::max<size_t>(1, std::min<size_t>(size_t(p.n_mt), (size_t(48) << 20) / slice)));
-    p.n_tiles = p.n_panels * p.n_mt;
+    p.n_tiles = p.n_pp * p.n_mt;
     CUtensorMap xmap, umap, bmap;
-    if (int rc = get_tensor_map_2d(t.x, uint64_t(t.M), uint64_t(t.K), uint64_t(t.K) * 2, uint32_t(BT), 64, &xmap)) return rc;
+    if (int rc = get_tensor_map_2d(t.x, uint64_t(t.M), uint64_t(t.K), uint64_t(t.K) * 2, uint32_t(BT / CS), 64, &xmap)) return rc;
     if (t.r > 0) {
-        if (int rc = get_tensor_map_2d(t.u16, uint64_t(t.M), uint64_t(t.r), uint64_t(t.r) * 2, uint32_t(BT), 64, &umap)) return rc;
+        if (int rc = get_tensor_map_2d(t.u16, uint64_t(t.M), uint64_t(t.r), uint64_t(t.r) * 2, uint32_t(BT / CS), 64, &umap)) return rc;
         if (int rc = get_tensor_map_2d(t.B, uint64_t(t.N), uint64_t(t.r), uint64_t(t.r) * 2, 128, 64, &bmap)) return rc;
     } else {
         umap = xmap; bmap = xmap;
     }
-    int grid = std::min(p.n_tiles, device_info().num_sms);
-    if (t.grid_override > 0) grid = std::min(p.n_tiles, t.grid_override);
     switch (BT) {
-        case 32: return launch_tc<32>(xmap, umap, bmap, p, grid, t.pdl, st);
-        case 64: return launch_tc<64>(xmap, umap, bmap, p, grid, t.pdl, st);
-        case 128: return launch_tc<128>(xmap, umap, bmap, p, grid, t.pdl, st);
-        default: return launch_tc<256>(xmap, umap, bmap, p, grid, t.pdl, st);
+        case 32: return launch_tc<32, 1>(xmap, umap, bmap, p, t.grid_override, t.pdl, st);
+        case 64: return launch_tc<64, 1>(xmap, umap, bmap, p, t.grid_override, t.pdl, st);
+        case 128: return launch_tc<128, 1>(xmap, umap, bmap, p, t.grid_override, t.pdl, st);
+        default:
+            if (CS == 4) return launch_tc<256, 4>(xmap, umap, bmap, p, t.grid_override, t.pdl, st);
+            if (CS == 2) return launch_tc<256, 2>(xmap, umap, bmap, p, t.grid_override, t.pdl, st);
+            return launch_tc<256, 1>(xmap, umap, bmap, p, t.grid_override, t.pdl, st);
     }
 }
 
