@@ -165,9 +165,9 @@ struct PlanEntry { int variant; float us[SPEAR_VARIANT_COUNT]; };
 static std::map<PlanKey, PlanEntry> g_plan;
 static std::mutex g_plan_mutex;
 
-static bool variant_valid(int v, int M, int r) {
+static bool variant_valid(int v, int M, int r, int gate) {
     switch (v) {
-        case SPEAR_VARIANT_STREAM_FUSED: return false;   // not built yet
+        case SPEAR_VARIANT_STREAM_FUSED: return M <= 16 && r > 0 && gate != SPEAR_GATE_MLP;
         case SPEAR_VARIANT_STREAM_SPLIT: return M <= 16;
         case SPEAR_VARIANT_TC_FUSED: return tc_available() && M >= 1;
         case SPEAR_VARIANT_TC_SPLIT: return false;
@@ -175,9 +175,8 @@ static bool variant_valid(int v, int M, int r) {
     }
     (void)r;
 }
-static int heuristic_variant(int M, int r) {
-    (void)r;
-    if (M <= 16) return SPEAR_VARIANT_STREAM_SPLIT;
+static int heuristic_variant(int M, int r, int gate) {
+    if (M <= 16) return (r > 0 && gate != SPEAR_GATE_MLP) ? SPEAR_VARIANT_STREAM_FUSED : SPEAR_VARIANT_STREAM_SPLIT;
     return SPEAR_VARIANT_TC_FUSED;
 }
 static int choose_variant(int M, int N, int K, int r, int group, int gate) {
@@ -186,7 +185,7 @@ static int choose_variant(int M, int N, int K, int r, int group, int gate) {
         auto it = g_plan.find(PlanKey{M, N, K, r, group, gate});
         if (it != g_plan.end()) return it->second.variant;
     }
-    return heuristic_variant(M, r);
+    return heuristic_variant(M, r, gate);
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -221,13 +220,13 @@ static int check_problem(const void* x, const void* Wq, const void* scales, cons
     return SPEAR_OK;
 }
 
-static int run_stream_split(const void* x, const void* Wq, const void* scales, const void* A, const void* B,
-                            const spear_ec_desc* ec, void* y, int M, int N, int K, int r, int group,
-                            uint8_t* ws, const WsLayout& L, cudaStream_t st) {
+static int run_stream(const void* x, const void* Wq, const void* scales, const void* A, const void* B,
+                      const spear_ec_desc* ec, void* y, int M, int N, int K, int r, int group,
+                      uint8_t* ws, const WsLayout& L, bool fused, cudaStream_t st) {
     unsigned* counters = reinterpret_cast<unsigned*>(ws + L.counters);
     float* u32 = reinterpret_cast<float*>(ws + L.u32);
     const bool pdl = g_tune.pdl != 0;
-    if (r > 0) {
+    if (r > 0 && !fused) {
         EcPreParams e = {};
         e.x = static_cast<const __half*>(x);
         e.A = static_cast<const __half*>(A);
@@ -263,8 +262,22 @@ static int run_stream_split(const void* x, const void* Wq, const void* scales, c
     p.M = M; p.N = N; p.K = K; p.r = r;
     p.G = K / group; p.group_chunks = group / 128; p.C = K / 128;
     p.U = (N / 128) * p.C;
-    int grid = std::min(p.U, g_dev.num_sms * std::max(1, g_tune.stream_ctas_per_sm));
+    // the fused EC's device-wide arrive/wait needs every CTA resident: at most 2 per SM (launch bounds)
+    int grid = std::min(p.U, g_dev.num_sms * std::max(1, std::min(2, g_tune.stream_ctas_per_sm)));
     grid = std::min(grid, kMaxStreamGrid);
+    if (fused && r > 0) {
+        p.fused = 1;
+        p.gate_kind = ec->gate_kind;
+        p.alpha = ec->alpha;
+        p.x = static_cast<const __half*>(x);
+        p.A = static_cast<const __half*>(A);
+        p.w_g = static_cast<const __half*>(ec->w_g);
+        p.b_g = static_cast<const float*>(ec->b_g);
+        p.zbuf = reinterpret_cast<float*>(ws + L.zbuf);
+        p.u_out = u32;
+        p.gate_out = static_cast<float*>(ec->gate_out);
+        p.ec_sync = counters + kEcPreCounter + 16;
+    }
     return launch_stream(xmap, p, MT, grid, pdl, st);
 }
 
@@ -322,15 +335,17 @@ static int layer_impl(const void* x, const void* Wq, const void* scales, const v
         return set_error(SPEAR_ENOMEM, "workspace too small: need %zu bytes, have %zu (pass spear_ec_desc.workspace)", L.total, ws_bytes);
     const int gate = (r > 0 && ec) ? ec->gate_kind : SPEAR_GATE_NONE;
     int v = (ec && ec->force_variant != SPEAR_VARIANT_AUTO) ? ec->force_variant : choose_variant(M, N, K, r, group, gate);
-    if (!variant_valid(v, M, r)) {
+    if (!variant_valid(v, M, r, gate)) {
         if (ec && ec->force_variant != SPEAR_VARIANT_AUTO)
-            return set_error(SPEAR_EUNSUPPORTED, "variant %d is not valid for M=%d r=%d", v, M, r);
-        v = heuristic_variant(M, r);
-        if (!variant_valid(v, M, r)) return set_error(SPEAR_EUNSUPPORTED, "no kernel variant for M=%d r=%d", M, r);
+            return set_error(SPEAR_EUNSUPPORTED, "variant %d is not valid for M=%d r=%d gate=%d", v, M, r, gate);
+        v = heuristic_variant(M, r, gate);
+        if (!variant_valid(v, M, r, gate)) return set_error(SPEAR_EUNSUPPORTED, "no kernel variant for M=%d r=%d", M, r);
     }
     switch (v) {
+        case SPEAR_VARIANT_STREAM_FUSED:
+            return run_stream(x, Wq, scales, A, B, ec, y, M, N, K, r, group, ws, L, true, st);
         case SPEAR_VARIANT_STREAM_SPLIT:
-            return run_stream_split(x, Wq, scales, A, B, ec, y, M, N, K, r, group, ws, L, st);
+            return run_stream(x, Wq, scales, A, B, ec, y, M, N, K, r, group, ws, L, false, st);
         case SPEAR_VARIANT_TC_FUSED:
             return run_tc_fused(x, Wq, scales, A, B, ec, y, M, N, K, r, group, ws, L, st);
         default:
@@ -468,7 +483,7 @@ extern "C" int spear_plan(int M, int N, int K, int r, int group, int gate_kind, 
     int status = SPEAR_OK;
     for (int v = 0; v < SPEAR_VARIANT_COUNT && status == SPEAR_OK; ++v) {
         ent.us[v] = -1.f;
-        if (!variant_valid(v, M, r)) continue;
+        if (!variant_valid(v, M, r, r > 0 ? gate_kind : SPEAR_GATE_NONE)) continue;
         ec.force_variant = v;
         for (int i = 0; i < warm + iters && status == SPEAR_OK; ++i) {
             if (i >= warm) cudaEventRecord(e0, st);
@@ -499,8 +514,9 @@ extern "C" int spear_plan(int M, int N, int K, int r, int group, int gate_kind, 
 
 extern "C" int spear_plan_query(int M, int N, int K, int r, int group, int gate_kind, int* variant_out) {
     if (!variant_out) return set_error(SPEAR_EINVAL, "NULL variant_out");
-    int v = choose_variant(M, N, K, r, group, r > 0 ? gate_kind : SPEAR_GATE_NONE);
-    if (!variant_valid(v, M, r)) v = heuristic_variant(M, r);
+    const int gk = r > 0 ? gate_kind : SPEAR_GATE_NONE;
+    int v = choose_variant(M, N, K, r, group, gk);
+    if (!variant_valid(v, M, r, gk)) v = heuristic_variant(M, r, gk);
     *variant_out = v;
     return SPEAR_OK;
 }

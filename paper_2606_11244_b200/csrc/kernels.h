@@ -19,6 +19,18 @@ struct StreamParams {
     int group_chunks;        // group / 128
     int C;                   // K / 128 chunks per panel
     int U;                   // (N / 128) * C work units
+    // ---- fused EC (SPEAR_VARIANT_STREAM_FUSED): z = x [A; w_g]^T, gate and u are computed by this kernel ----
+    int fused;               // 0: u comes from the EC pre-kernel; 1: warp 9 of every CTA produces it
+    int gate_kind;           // SPEAR_GATE_SCALAR_SIGMOID or SPEAR_GATE_NONE
+    float alpha;
+    const __half* x;         // [M][K]
+    const __half* A;         // [r][K]
+    const __half* w_g;       // [K] (scalar gate)
+    const float* b_g;        // 1 or NULL
+    float* zbuf;             // [16][kZStride] fp32, zero between calls
+    float* u_out;            // [16][r] fp32 (same buffer as u)
+    float* gate_out;         // optional [M]
+    unsigned* ec_sync;       // [0] arrivals, [1] u-ready flag, [2] readers; zero between calls
 };
 int stream_smem_bytes(int MT);
 int launch_stream(const CUtensorMap& xmap, const StreamParams& p, int MT, int grid, bool pdl, cudaStream_t st);

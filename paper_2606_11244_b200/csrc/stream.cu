@@ -35,7 +35,7 @@ struct StreamCfg {
     static constexpr size_t kWBytes = size_t(kStages) * 8192;
     static constexpr size_t kScBytes = size_t(kStages) * 256;
     static constexpr size_t kRedBytes = size_t(8) * kTok * kRedStride * 4;
-    static constexpr size_t kBarBytes = size_t(kStages) * 16 + 16;
+    static constexpr size_t kBarBytes = size_t(kStages) * 16 + 32;
     static constexpr size_t kSmemBytes = 1024 + kXBytes + kWBytes + kScBytes + kRedBytes + kBarBytes;
 };
 
@@ -84,8 +84,126 @@ __device__ __forceinline__ void stream_task(const uint8_t* __restrict__ wst, con
     }
 }
 
+// ---- fused EC (warp 9): S4-S6 of SURVEY.md 8(a) inside the weight-stream kernel ---------------------
+// Every CTA reduces one (16-row strip of [A; w_g]) x (K slice) piece of z = x [A; w_g]^T with mma.sync,
+// adds it to the global fp32 z with red.add and ARRIVES on a device-wide counter right away; nobody
+// waits there.  The last CTA to arrive applies the gate (z must be complete before
+// the gate), writes u = alpha * gamma (.) z, re-zeroes z and raises a flag; the other
+// CTAs only look at the flag in their epilogue, long after everybody has arrived (arrive early / wait
+// late).  All CTAs of the grid are co-resident (grid <= SMs x occupancy), so the wait cannot deadlock.
+__device__ __forceinline__ void ec_load16(const __half* row, int col, bool readonly, uint32_t (&lo)[4], uint32_t (&hi)[4]) {
+    if (row) {
+        uint4 a, b;
+        if (readonly) {
+            a = __ldg(reinterpret_cast<const uint4*>(row + col));
+            b = __ldg(reinterpret_cast<const uint4*>(row + col + 8));
+        } else {
+            a = *reinterpret_cast<const uint4*>(row + col);
+            b = *reinterpret_cast<const uint4*>(row + col + 8);
+        }
+        lo[0] = a.x; lo[1] = a.y; lo[2] = a.z; lo[3] = a.w;
+        hi[0] = b.x; hi[1] = b.y; hi[2] = b.z; hi[3] = b.w;
+    } else {
+#pragma unroll
+        for (int i = 0; i < 4; ++i) lo[i] = hi[i] = 0u;
+    }
+}
+
+__device__ void ec_warp_fused(const StreamParams& p, int lane, uint64_t* u_ready) {
+    const int g = lane >> 2, t = lane & 3;
+    const bool scalar = (p.gate_kind == SPEAR_GATE_SCALAR_SIGMOID);
+    const int rows_total = p.r + (scalar ? 1 : 0);
+    const int strips = (rows_total + 15) >> 4;
+    const int G = gridDim.x;
+    const int ktiles = p.K >> 6;
+    const int ksplit = max(1, min(ktiles, G / strips));
+    const int n_tasks = strips * ksplit;
+    const __half* px0 = g < p.M ? p.x + size_t(g) * p.K : nullptr;
+    const __half* px1 = g + 8 < p.M ? p.x + size_t(g + 8) * p.K : nullptr;
+    bool waited = false;
+    for (int task = blockIdx.x; task < n_tasks; task += G) {
+        const int strip = task % strips, ks = task / strips;
+        const int rho0 = strip * 16 + g, rho1 = rho0 + 8;
+        const __half* pa0 = rho0 < p.r ? p.A + size_t(rho0) * p.K : (rho0 == p.r && scalar ? p.w_g : nullptr);
+        const __half* pa1 = rho1 < p.r ? p.A + size_t(rho1) * p.K : (rho1 == p.r && scalar ? p.w_g : nullptr);
+        const int kt_begin = int((long long)ks * ktiles / ksplit);
+        const int kt_end = int((long long)(ks + 1) * ktiles / ksplit);
+        float acc0[4] = {0.f, 0.f, 0.f, 0.f}, acc1[4] = {0.f, 0.f, 0.f, 0.f};
+        for (int kt = kt_begin; kt < kt_end; ++kt) {
+            const int col = kt * 64 + 16 * t;
+            uint32_t a0l[4], a0h[4], a1l[4], a1h[4], x0l[4], x0h[4], x1l[4], x1h[4];
+            ec_load16(pa0, col, true, a0l, a0h);     // EC factors are parameters: never written by a kernel
+            ec_load16(pa1, col, true, a1l, a1h);
+            if (!waited) { pdl_wait(); waited = true; }   // x may come from the previous kernel
+            ec_load16(px0, col, false, x0l, x0h);
+            ec_load16(px1, col, false, x1l, x1h);
+#pragma unroll
+            for (int jj = 0; jj < 4; ++jj) {
+                mma_m16n8k16(acc0, a0l[jj], a1l[jj], a0h[jj], a1h[jj], x0l[jj], x0h[jj]);
+                mma_m16n8k16(acc1, a0l[jj], a1l[jj], a0h[jj], a1h[jj], x1l[jj], x1h[jj]);
+            }
+        }
+        // C fragment: rows rho0 / rho1 of [A; w_g], tokens 2t, 2t+1 (acc0) and 8+2t, 9+2t (acc1)
+#pragma unroll
+        for (int i = 0; i < 4; ++i) {
+            const int rho = (i & 2) ? rho1 : rho0;
+            const int tok = 2 * t + (i & 1);
+            if (rho < rows_total) {
+                if (tok < p.M) atomicAdd(p.zbuf + tok * kZStride + rho, acc0[i]);
+                if (tok + 8 < p.M) atomicAdd(p.zbuf + (tok + 8) * kZStride + rho, acc1[i]);
+            }
+        }
+    }
+    if (!waited) pdl_wait();
+    __threadfence();
+    __syncwarp();
+    unsigned old = 0;
+    if (lane == 0) old = atomicAdd(p.ec_sync + 0, 1u);
+    old = __shfl_sync(0xffffffffu, old, 0);
+    if (old == unsigned(G - 1)) {
+        // ---- last arriver: gate, u, clean-up ----
+        __threadfence();
+        const float bias = (scalar && p.b_g) ? *p.b_g : 0.f;
+        const int n = p.M * p.r;
+        for (int idx = lane; idx < n; idx += 32) {
+            const int m = idx / p.r, j = idx - m * p.r;
+            const float z = __ldcg(p.zbuf + m * kZStride + j);
+            float gam = 1.f;
+            if (scalar) gam = 1.f / (1.f + expf(-(__ldcg(p.zbuf + m * kZStride + p.r) + bias)));
+            p.u_out[idx] = p.alpha * gam * z;
+            if (scalar && p.gate_out && j == 0) p.gate_out[m] = gam;
+        }
+        __syncwarp();
+        for (int idx = lane; idx < p.M * rows_total; idx += 32) {
+            const int m = idx / rows_total, rho = idx - m * rows_total;
+            p.zbuf[m * kZStride + rho] = 0.f;
+        }
+        __threadfence();
+        __syncwarp();
+        if (lane == 0) {
+            p.ec_sync[0] = 0;
+            if (G > 1) {
+                __threadfence();
+                asm volatile("st.release.gpu.global.u32 [%0], %1;" ::"l"(p.ec_sync + 1), "r"(1u) : "memory");
+            }
+        }
+    } else if (lane == 0) {
+        unsigned f = 0;
+        do {
+            asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(f) : "l"(p.ec_sync + 1) : "memory");
+        } while (f == 0);
+        const unsigned readers = atomicAdd(p.ec_sync + 2, 1u);
+        if (readers == unsigned(G - 2)) {      // every waiting CTA has seen the flag: leave the workspace clean
+            p.ec_sync[2] = 0;
+            p.ec_sync[1] = 0;
+        }
+    }
+    __syncwarp();
+    if (lane == 0) mbar_arrive(u_ready);
+}
+
 template <int MT>
-__global__ void __launch_bounds__(288, 2)
+__global__ void __launch_bounds__(320, 2)
 stream_kernel(const __grid_constant__ CUtensorMap xmap, const StreamParams p) {
     using Cfg = StreamCfg<MT>;
     constexpr int S = Cfg::kStages;
@@ -98,6 +216,7 @@ stream_kernel(const __grid_constant__ CUtensorMap xmap, const StreamParams p) {
     uint64_t* full = reinterpret_cast<uint64_t*>(reinterpret_cast<uint8_t*>(red) + Cfg::kRedBytes);
     uint64_t* empty = full + S;
     int* flag = reinterpret_cast<int*>(empty + S);
+    uint64_t* u_ready = reinterpret_cast<uint64_t*>(flag + 2);   // fused EC: u is in global memory, visible
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int G = gridDim.x, b = blockIdx.x;
@@ -108,11 +227,16 @@ stream_kernel(const __grid_constant__ CUtensorMap xmap, const StreamParams p) {
 
     if (threadIdx.x == 0) {
         for (int s = 0; s < S; ++s) { mbar_init(&full[s], 1); mbar_init(&empty[s], 4); }
+        mbar_init(u_ready, 1);
         fence_mbar_init();
         tma_prefetch_desc(&xmap);
     }
     __syncthreads();
     pdl_launch_dependents();
+    if (warp == 9) {
+        if (p.fused && p.r > 0) ec_warp_fused(p, lane, u_ready);
+        return;
+    }
     if (n_units == 0) return;
 
     if (warp == 0) {
@@ -247,7 +371,8 @@ stream_kernel(const __grid_constant__ CUtensorMap xmap, const StreamParams p) {
         if (finalize) {
             const int n = pnl * 128 + row;
             if (p.r > 0) {
-                // S7: y += sum_j u[m][j] * B[n][j]   (u = alpha * gamma (.) z, fp32, from the pre-kernel)
+                // S7: y += sum_j u[m][j] * B[n][j]   (u = alpha * gamma (.) z, fp32, from the pre-kernel or warp 9)
+                if (p.fused) mbar_wait(u_ready, 0);
                 const uint4* Brow = reinterpret_cast<const uint4*>(p.B + size_t(n) * p.r);
                 for (int j8 = 0; j8 < p.r / 8; ++j8) {
                     const uint4 bv = __ldg(Brow + j8);
@@ -298,7 +423,7 @@ int launch_stream(const CUtensorMap& xmap, const StreamParams& p, int MT, int gr
     }
     cudaLaunchConfig_t cfg = {};
     cfg.gridDim = dim3(grid);
-    cfg.blockDim = dim3(288);
+    cfg.blockDim = dim3(320);
     cfg.dynamicSmemBytes = stream_smem_bytes(MT);
     cfg.stream = st;
     cudaLaunchAttribute attr[1];

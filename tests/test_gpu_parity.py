@@ -218,3 +218,36 @@ def test_errors(sp):
     with pytest.raises(sp.SpearError) as e:      # missing gate weights
         sp.w4_ec_gemm(x, dl.pw, dl.A, dl.B, None, None)
     assert e.value.status == -1
+
+
+# ---------------------------------------------------------------- fused vs split EC on the decode path (S9 arms)
+
+@pytest.mark.parametrize("variant", [1, 2])      # SPEAR_VARIANT_STREAM_FUSED, SPEAR_VARIANT_STREAM_SPLIT
+@pytest.mark.parametrize("M,N,K,r,gate", [(1, 256, 512, 8, "scalar"), (4, 2048, 2048, 16, "scalar"),
+                                          (16, 384, 640, 24, "none"), (9, 3072, 2048, 32, "scalar"),
+                                          (16, 2048, 8192, 128, "scalar"), (3, 128, 128, 64, "scalar")])
+def test_decode_fused_and_split(sp, variant, M, N, K, r, gate):
+    li = make_layer(400 + M + r, M, N, K, 128, r, gate=gate)
+    check_layer(li, variant=variant, label=f"variant {variant} M={M} r={r} {gate}")
+
+
+def test_fused_variant_rejects_mlp_gate(sp):
+    h = _harness()
+    li = make_layer(81, 4, 128, 128, 128, 8, gate="mlp")
+    with pytest.raises(sp.SpearError) as e:
+        h.run_layer(h.upload_layer(li), h.dev(li.x), variant=1)
+    assert e.value.status == -2
+
+
+def test_fused_back_to_back_leaves_workspace_clean(sp):
+    import torch
+    h = _harness()
+    li = make_layer(82, 16, 384, 2048, 128, 32, gate="scalar")
+    dl = h.upload_layer(li)
+    x = h.dev(li.x)
+    ys = [h.run_layer(dl, x, variant=1)[0].clone() for _ in range(6)]
+    torch.cuda.synchronize()
+    ref = oracle.forward_layer(li)["y"]
+    rms = float(np.sqrt(np.mean(ref ** 2)))
+    for y in ys:
+        assert float(np.max(np.abs(y.cpu().numpy().astype(np.float64) - ref))) <= Y_TOL * rms
