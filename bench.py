@@ -164,8 +164,12 @@ def run_cuda(args, rank, world):
             yh[(M, s.name)] = torch.empty((M, s.N), dtype=torch.float16).pin_memory()
 
     descs = {}   # keep EcDesc objects alive
+    batches = {}
 
-    def one_step(g, with_ec=True):
+    def one_step(g, with_ec=True, batched=True):
+        """One pass over the 12 independent layer calls: as ONE spear_w4_ec_gemm_batch (the library overlaps
+        independent calls on its lanes) or as 12 stream-ordered spear_w4_ec_gemm_ex calls."""
+        entries = []
         for mi, M in enumerate(TOKENS):
             cp = copies[(3 * g + mi) % ncopy]
             for s in shapes[M]:
@@ -173,28 +177,34 @@ def run_cuda(args, rank, world):
                 key = (g, mi, s.name, with_ec)
                 if key not in descs:
                     descs[key] = dl.desc() if with_ec else sp.make_desc(gate="none")
-                if with_ec:
-                    sp.w4_ec_gemm_ex(xs[(M, s.name)], dl.pw, dl.A, dl.B, descs[key], y=ys[(M, s.name)])
+                A, B = (dl.A, dl.B) if with_ec else (None, None)
+                if batched:
+                    entries.append((xs[(M, s.name)], dl.pw, A, B, descs[key], ys[(M, s.name)]))
                 else:
-                    sp.w4_ec_gemm_ex(xs[(M, s.name)], dl.pw, None, None, descs[key], y=ys[(M, s.name)])
+                    sp.w4_ec_gemm_ex(xs[(M, s.name)], dl.pw, A, B, descs[key], y=ys[(M, s.name)])
+        if batched:
+            bk = (g, with_ec)
+            if bk not in batches:
+                batches[bk] = sp.Batch(entries)
+            sp.w4_ec_gemm_batch(batches[bk])
 
     stream = torch.cuda.Stream()
     ngraph = ncopy // 3
     use_graph = os.environ.get("SPEAR_BENCH_GRAPH", "1") != "0"
 
-    def make_graphs(with_ec):
+    def make_graphs(with_ec, batched=True):
         gs = []
         with torch.cuda.stream(stream):
-            one_step(0, with_ec)           # first-call work (tensor maps, attributes) outside capture
+            one_step(0, with_ec, batched)  # first-call work (tensor maps, attributes) outside capture
             torch.cuda.synchronize()
             for g in range(ngraph):
                 if use_graph:
                     cg = torch.cuda.CUDAGraph()
                     with torch.cuda.graph(cg, stream=stream):
-                        one_step(g, with_ec)
+                        one_step(g, with_ec, batched)
                     gs.append(cg.replay)
                 else:
-                    gs.append(lambda g=g: one_step(g, with_ec))
+                    gs.append(lambda g=g: one_step(g, with_ec, batched))
         return gs
 
     def timed(fns, steps, warmup):
@@ -228,6 +238,9 @@ def run_cuda(args, rank, world):
     ms = timed(g_ec, args.steps, args.warmup)
     g_w4 = make_graphs(False)
     ms_w4 = timed(g_w4, args.steps, args.warmup)
+    # the same step with the 12 calls strictly stream-ordered (one after the other, PDL-chained)
+    ms_seq = timed(make_graphs(True, batched=False), args.steps, args.warmup)
+    ms_seq_w4 = timed(make_graphs(False, batched=False), args.steps, args.warmup)
     # make the region long enough for nvidia-smi to see it under load
     t_end = time.time() + 1.5
     while rank == 0 and time.time() < t_end:
@@ -259,7 +272,8 @@ def run_cuda(args, rank, world):
         "warmup": args.warmup, "ms_per_step": round(per, 6), "higher_is_better": True, "scaling": "weak",
         "vs_baseline": None, "dtype": "f16 (int4 weights, fp32 accumulate)", "data": "synthetic (seeded, workloads/)",
         "config": {"workload": "BASELINE.json configs[1]: Llama-3.2-1B decode projections qkv/o/gate_up/down, "
-                               "group=128, EC r=32 scalar sigmoid gate, M in {1,8,16}; step = 12 layer calls",
+                               "group=128, EC r=32 scalar sigmoid gate, M in {1,8,16}; step = 12 independent layer calls issued as one "
+                               "spear_w4_ec_gemm_batch",
                    "l2": f"inputs larger than L2: weights+EC rotate over {ncopy} copies ({ncopy * set_bytes >> 20} MiB)",
                    "cuda_graph": use_graph, "bytes_per_step": b_ec, "parallelism": f"replicas x{world}"},
         "e2e": {"value": round(world * b_ec / (per_e2e * 1e-3) / 1e9, 1), "unit": UNIT,
@@ -267,12 +281,18 @@ def run_cuda(args, rank, world):
                 "d2h_bytes_per_step": sum(t.numel() * 2 for t in yh.values()), "ms_per_step": round(per_e2e, 6)},
         "gpu_launches": int(per_step_launches * args.steps),
         "clocks": clocks,
-        "roofline": {"bound": "hbm", "kernel": "spear::stream_kernel (plain W4 step: one launch per layer call)",
+        "roofline": {"bound": "hbm", "kernel": "spear::stream_kernel (plain W4 step: one launch per layer call, "
+                                                "calls overlapped on the batch lanes)",
                      "achieved": round(ach, 1), "peak": peak, "unit": "GB/s", "frac": round(ach / peak, 4),
                      "peak_source": peak_src, "traffic": None,
                      "avg_launch_us": round(per_w4 * 1e3 / ncalls, 3), "launches_per_step": ncalls},
         "no_ec": {"value": round(world * b_w4 / (per_w4 * 1e-3) / 1e9, 1), "ms_per_step": round(per_w4, 6)},
         "ec_overhead_time_frac": round(per / per_w4 - 1.0, 4),
+        "stream_ordered": {"note": "same step, 12 calls one after the other on one stream (PDL-chained) instead of "
+                                   "one spear_w4_ec_gemm_batch",
+                           "value": round(world * b_ec / (ms_seq / args.steps * 1e-3) / 1e9, 1),
+                           "no_ec_value": round(world * b_w4 / (ms_seq_w4 / args.steps * 1e-3) / 1e9, 1),
+                           "ms_per_step": round(ms_seq / args.steps, 6)},
     }
     if rank == 0:
         out["cpu_baseline"] = cpu_baseline_sample()

@@ -115,6 +115,20 @@ int spear_w4_ec_gemm_ex(const void* x, const void* Wq, const void* scales, const
                         const spear_ec_desc* ec, void* y,
                         int M, int N, int K, int r, int group, void* stream);
 
+/* A batch of INDEPENDENT layer calls (no call reads another call's y; all y buffers distinct), e.g. the
+ * q/k/v or gate/up projections of one transformer block, or unrelated requests.  The calls run
+ * concurrently on the library's internal lanes (streams with their own workspaces); all of them are
+ * ordered after the work already enqueued on `stream` and before anything enqueued on it afterwards
+ * (fork / join with events; capturable in a CUDA graph).  ec->workspace must be NULL.  The
+ * per-token-gated EC of every call is evaluated exactly as in spear_w4_ec_gemm_ex. */
+typedef struct {
+    const void *x, *Wq, *scales, *A, *B;
+    const spear_ec_desc* ec;    /* may be NULL when r == 0 */
+    void* y;
+    int M, N, K, r, group;
+} spear_call;
+int spear_w4_ec_gemm_batch(const spear_call* calls, int n_calls, void* stream);
+
 /* Same layer with HOST activations: x_host[M][K] and y_host[M][N] are (preferably pinned) host
  * buffers; x is copied to x_dev, the layer runs, y_dev is copied back, all on `stream` (the end-
  * to-end path bench.py times).  Weights and EC parameters stay device-resident. */
@@ -144,7 +158,8 @@ int spear_plan_load(const char* path);
 /* The variant AUTO would run for this problem right now (table hit or heuristic). */
 int spear_plan_query(int M, int N, int K, int r, int group, int gate_kind, int* variant_out);
 
-/* Debug / sweep hook: sets a launch tunable ("stream_ctas_per_sm", "pdl", "ecpre_ctas", "tc_grid").
+/* Debug / sweep hook: sets a launch tunable ("stream_ctas_per_sm", "pdl", "ecpre_ctas", "tc_grid",
+ * "tc_cluster", "batch_lanes").
  * Host-only, process-wide, not thread-safe against concurrent compute calls. */
 int spear_tune(const char* key, int value);
 

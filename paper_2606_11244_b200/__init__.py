@@ -23,7 +23,7 @@ VARIANT_NAMES = ["auto", "stream_fused", "stream_split", "tc_fused", "tc_split"]
 
 EXPORTS = [
     "spear_pack_w4_sizes", "spear_pack_w4", "spear_unpack_w4", "spear_dequant_w4",
-    "spear_w4_ec_gemm", "spear_w4_ec_gemm_ex", "spear_w4_ec_gemm_hostio",
+    "spear_w4_ec_gemm", "spear_w4_ec_gemm_ex", "spear_w4_ec_gemm_hostio", "spear_w4_ec_gemm_batch",
     "spear_workspace_bytes", "spear_init", "spear_plan", "spear_plan_save", "spear_plan_load",
     "spear_plan_query", "spear_tune", "spear_last_error", "spear_launch_count",
 ]
@@ -45,6 +45,15 @@ class EcDesc(ctypes.Structure):
     ]
 
 
+class Call(ctypes.Structure):
+    """struct spear_call of include/spear.h (one entry of spear_w4_ec_gemm_batch)."""
+    _fields_ = [
+        ("x", ctypes.c_void_p), ("Wq", ctypes.c_void_p), ("scales", ctypes.c_void_p), ("A", ctypes.c_void_p),
+        ("B", ctypes.c_void_p), ("ec", ctypes.POINTER(EcDesc)), ("y", ctypes.c_void_p),
+        ("M", ctypes.c_int), ("N", ctypes.c_int), ("K", ctypes.c_int), ("r", ctypes.c_int), ("group", ctypes.c_int),
+    ]
+
+
 _lib = None
 
 
@@ -63,6 +72,7 @@ def lib():
         L.spear_dequant_w4.argtypes = [vp, vp, vp, ci, ci, ci, vp]
         L.spear_w4_ec_gemm.argtypes = [vp] * 8 + [ci] * 5 + [vp]
         L.spear_w4_ec_gemm_ex.argtypes = [vp] * 5 + [ctypes.POINTER(EcDesc), vp] + [ci] * 5 + [vp]
+        L.spear_w4_ec_gemm_batch.argtypes = [ctypes.POINTER(Call), ci, vp]
         L.spear_w4_ec_gemm_hostio.argtypes = [vp] * 8 + [ctypes.POINTER(EcDesc)] + [ci] * 5 + [vp]
         L.spear_workspace_bytes.argtypes = [ci] * 5 + [ctypes.POINTER(ctypes.c_size_t)]
         L.spear_init.argtypes = []
@@ -202,6 +212,28 @@ def w4_ec_gemm_hostio(x_host, y_host, x_dev, y_dev, pw: PackedW4, A=None, B=None
     _check(lib().spear_w4_ec_gemm_hostio(_ptr(x_host), _ptr(y_host), _ptr(x_dev), _ptr(y_dev), _ptr(pw.wq),
                                          _ptr(pw.scales), _ptr(A), _ptr(B), ctypes.byref(desc),
                                          M, pw.N, K, r, pw.group, _stream(stream)))
+
+
+class Batch:
+    """A prepared array of spear_call entries (keeps the descriptors and tensors it points to alive)."""
+
+    def __init__(self, entries):
+        """entries: iterable of (x, pw, A, B, desc, y) with device tensors; desc may be None when A is None."""
+        entries = list(entries)
+        self.keep = entries
+        self.n = len(entries)
+        self.calls = (Call * self.n)()
+        for c, (x, pw, A, B, desc, y) in zip(self.calls, entries):
+            M, K = x.shape
+            assert K == pw.K and y.shape == (M, pw.N)
+            c.x, c.Wq, c.scales, c.A, c.B, c.y = _ptr(x), _ptr(pw.wq), _ptr(pw.scales), _ptr(A), _ptr(B), _ptr(y)
+            c.ec = ctypes.pointer(desc) if desc is not None else None
+            c.M, c.N, c.K, c.r, c.group = M, pw.N, K, (0 if A is None else A.shape[0]), pw.group
+
+
+def w4_ec_gemm_batch(batch: Batch, stream=None):
+    """spear_w4_ec_gemm_batch: independent layer calls, run concurrently on the library's lanes."""
+    _check(lib().spear_w4_ec_gemm_batch(batch.calls, batch.n, _stream(stream)))
 
 
 def workspace_bytes(M, N, K, r, group) -> int:

@@ -63,6 +63,12 @@ static WsLayout ws_layout(int M, int r, size_t ws_bytes) {
     return L;
 }
 constexpr size_t kDefaultWorkspace = size_t(96) << 20;
+constexpr int kBatchLanes = 4;
+constexpr size_t kLaneWorkspace = size_t(48) << 20;
+static cudaStream_t g_lane_stream[kBatchLanes];
+static cudaEvent_t g_lane_done[kBatchLanes];
+static cudaEvent_t g_batch_fork;
+static void* g_lane_ws[kBatchLanes];
 
 static void do_init() {
     int dev = 0;
@@ -98,6 +104,19 @@ static void do_init() {
         return;
     }
     g_ws_bytes = kDefaultWorkspace;
+    // lanes of spear_w4_ec_gemm_batch: independent calls run concurrently, each lane with its own workspace
+    for (int l = 0; l < kBatchLanes && e == cudaSuccess; ++l) {
+        e = cudaStreamCreateWithFlags(&g_lane_stream[l], cudaStreamNonBlocking);
+        if (e == cudaSuccess) e = cudaEventCreateWithFlags(&g_lane_done[l], cudaEventDisableTiming);
+        if (e == cudaSuccess) e = cudaMalloc(&g_lane_ws[l], kLaneWorkspace);
+        if (e == cudaSuccess) e = cudaMemset(g_lane_ws[l], 0, kLaneWorkspace);
+    }
+    if (e == cudaSuccess) e = cudaEventCreateWithFlags(&g_batch_fork, cudaEventDisableTiming);
+    if (e == cudaSuccess) e = cudaDeviceSynchronize();
+    if (e != cudaSuccess) {
+        snprintf(g_init_err, sizeof(g_init_err), "batch lanes: %s", cudaGetErrorString(e));
+        g_init_status = SPEAR_ENOMEM;
+    }
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -143,6 +162,33 @@ int get_tensor_map_2d(const void* base, uint64_t rows, uint64_t cols, uint64_t r
     return SPEAR_OK;
 }
 
+int get_tensor_map_x3d(const void* base, uint64_t rows, uint64_t cols, uint32_t box_rows, uint32_t box_ktiles,
+                       CUtensorMap* out) {
+    CUtensorMap dummy;
+    if (!g_encode) {   // resolves the driver entry point
+        if (int rc = get_tensor_map_2d(base, rows, cols, cols * 2, 8, 64, &dummy)) return rc;
+    }
+    std::lock_guard<std::mutex> lock(g_map_mutex);
+    const MapKey key(base, rows, cols, ~uint64_t(0), box_rows, box_ktiles);
+    auto it = g_maps.find(key);
+    if (it != g_maps.end()) { *out = it->second; return SPEAR_OK; }
+    CUtensorMap m;
+    const cuuint64_t dims[3] = {64, cols / 64, rows};
+    const cuuint64_t strides[2] = {128, cols * 2};
+    const cuuint32_t box[3] = {64, box_ktiles, box_rows};
+    const cuuint32_t estr[3] = {1, 1, 1};
+    const CUresult rc = g_encode(&m, CU_TENSOR_MAP_DATA_TYPE_FLOAT16, 3, const_cast<void*>(base), dims, strides, box,
+                                 estr, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B,
+                                 CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    if (rc != CUDA_SUCCESS)
+        return set_error(SPEAR_ECUDA, "cuTensorMapEncodeTiled (3-D x view) failed (%d) rows=%llu cols=%llu", int(rc),
+                         (unsigned long long)rows, (unsigned long long)cols);
+    if (g_maps.size() > 8192) g_maps.clear();
+    g_maps[key] = m;
+    *out = m;
+    return SPEAR_OK;
+}
+
 // ------------------------------------------------------------------------------------------------
 // tunables (debug / sweep hook) and the plan table
 // ------------------------------------------------------------------------------------------------
@@ -152,6 +198,7 @@ struct Tunables {
     int ecpre_ctas = 0;           // 0 = heuristic
     int tc_grid = 0;              // 0 = heuristic
     int tc_cluster = 0;           // 0 = heuristic, else 1 / 2 / 4
+    int batch_lanes = 4;          // concurrent lanes of spear_w4_ec_gemm_batch (1..4)
 };
 static Tunables g_tune;
 
@@ -251,7 +298,7 @@ static int run_stream(const void* x, const void* Wq, const void* scales, const v
     }
     const int MT = M <= 8 ? 1 : 2;
     CUtensorMap xmap;
-    if (int rc = get_tensor_map_2d(x, uint64_t(M), uint64_t(K), uint64_t(K) * 2, uint32_t(8 * MT), 64, &xmap)) return rc;
+    if (int rc = get_tensor_map_x3d(x, uint64_t(M), uint64_t(K), uint32_t(8 * MT), 4, &xmap)) return rc;
     StreamParams p = {};
     p.wq = Wq; p.scales = scales;
     p.y = static_cast<__half*>(y);
@@ -261,7 +308,8 @@ static int run_stream(const void* x, const void* Wq, const void* scales, const v
     p.counters = counters;
     p.M = M; p.N = N; p.K = K; p.r = r;
     p.G = K / group; p.group_chunks = group / 128; p.C = K / 128;
-    p.U = (N / 128) * p.C;
+    p.CP = (p.C + 1) / 2;
+    p.U = (N / 128) * p.CP;
     // the fused EC's device-wide arrive/wait needs every CTA resident: at most 2 per SM (launch bounds)
     int grid = std::min(p.U, g_dev.num_sms * std::max(1, std::min(2, g_tune.stream_ctas_per_sm)));
     grid = std::min(grid, kMaxStreamGrid);
@@ -319,13 +367,14 @@ static int run_tc_fused(const void* x, const void* Wq, const void* scales, const
 }
 
 static int layer_impl(const void* x, const void* Wq, const void* scales, const void* A, const void* B,
-                      const spear_ec_desc* ec, void* y, int M, int N, int K, int r, int group, cudaStream_t st) {
+                      const spear_ec_desc* ec, void* y, int M, int N, int K, int r, int group, cudaStream_t st,
+                      void* lane_ws = nullptr, size_t lane_ws_bytes = 0) {
     if (int rc = spear_init()) return rc;
     if (r == 0) { A = nullptr; B = nullptr; }
     if (int rc = check_problem(x, Wq, scales, A, B, ec, y, M, N, K, r, group)) return rc;
-    uint8_t* ws = static_cast<uint8_t*>(g_ws);
-    size_t ws_bytes = g_ws_bytes;
-    if (ec && ec->workspace) {
+    uint8_t* ws = static_cast<uint8_t*>(lane_ws ? lane_ws : g_ws);
+    size_t ws_bytes = lane_ws ? lane_ws_bytes : g_ws_bytes;
+    if (!lane_ws && ec && ec->workspace) {
         ws = static_cast<uint8_t*>(ec->workspace);
         ws_bytes = ec->workspace_bytes;
         if (uintptr_t(ws) & 1023) return set_error(SPEAR_EINVAL, "workspace must be 1024-byte aligned");
@@ -373,6 +422,7 @@ extern "C" int spear_tune(const char* key, int value) {
     else if (!strcmp(key, "ecpre_ctas")) g_tune.ecpre_ctas = value;
     else if (!strcmp(key, "tc_grid")) g_tune.tc_grid = value;
     else if (!strcmp(key, "tc_cluster")) g_tune.tc_cluster = value;
+    else if (!strcmp(key, "batch_lanes")) g_tune.batch_lanes = value;
     else return set_error(SPEAR_EINVAL, "unknown tunable '%s'", key);
     return SPEAR_OK;
 }
@@ -401,6 +451,49 @@ extern "C" int spear_w4_ec_gemm(const void* x, const void* Wq, const void* scale
     ec.b_g = gate_b;
     ec.force_variant = SPEAR_VARIANT_AUTO;
     return layer_impl(x, Wq, scales, A, B, &ec, y, M, N, K, r, group, static_cast<cudaStream_t>(stream));
+}
+
+extern "C" int spear_w4_ec_gemm_batch(const spear_call* calls, int n_calls, void* stream) {
+    if (!calls || n_calls < 0) return set_error(SPEAR_EINVAL, "bad batch");
+    if (n_calls == 0) return SPEAR_OK;
+    if (int rc = spear_init()) return rc;
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    const int lanes = std::max(1, std::min(kBatchLanes, std::min(n_calls, g_tune.batch_lanes)));
+    // longest-processing-time-first assignment by weight bytes
+    std::vector<int> order(n_calls);
+    for (int i = 0; i < n_calls; ++i) order[i] = i;
+    std::stable_sort(order.begin(), order.end(), [&](int a, int b) {
+        return size_t(calls[a].N) * calls[a].K > size_t(calls[b].N) * calls[b].K;
+    });
+    size_t load[kBatchLanes] = {0, 0, 0, 0};
+    std::vector<int> lane_of(n_calls);
+    for (int i : order) {
+        int best = 0;
+        for (int l = 1; l < lanes; ++l) if (load[l] < load[best]) best = l;
+        lane_of[i] = best;
+        load[best] += size_t(calls[i].N) * calls[i].K / 2 + (size_t(4) << 20);   // bytes + a fixed launch cost
+    }
+    SPEAR_CUDA_OK(cudaEventRecord(g_batch_fork, st));
+    for (int l = 0; l < lanes; ++l) SPEAR_CUDA_OK(cudaStreamWaitEvent(g_lane_stream[l], g_batch_fork, 0));
+    int status = SPEAR_OK;
+    for (int i = 0; i < n_calls && status == SPEAR_OK; ++i) {
+        const spear_call& c = calls[i];
+        if (c.ec && c.ec->workspace) { status = set_error(SPEAR_EINVAL, "batch calls use the library's lane workspaces (ec->workspace must be NULL)"); break; }
+        size_t need = 0;
+        if (c.M >= 1 && c.r >= 0) need = ws_layout(c.M, c.r, 0).total + 1024;
+        const int l = lane_of[i];
+        if (need <= kLaneWorkspace)
+            status = layer_impl(c.x, c.Wq, c.scales, c.A, c.B, c.ec, c.y, c.M, c.N, c.K, c.r, c.group, g_lane_stream[l],
+                                g_lane_ws[l], kLaneWorkspace);
+        else
+            status = set_error(SPEAR_ENOMEM, "batch call %d needs %zu bytes of workspace (lane has %zu)", i, need, kLaneWorkspace);
+    }
+    // always join, also after an error, so that `stream` stays consistent (and a capture stays valid)
+    for (int l = 0; l < lanes; ++l) {
+        cudaEventRecord(g_lane_done[l], g_lane_stream[l]);
+        cudaStreamWaitEvent(st, g_lane_done[l], 0);
+    }
+    return status;
 }
 
 extern "C" int spear_w4_ec_gemm_hostio(const void* x_host, void* y_host, void* x_dev, void* y_dev, const void* Wq,

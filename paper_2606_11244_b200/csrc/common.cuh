@@ -43,6 +43,9 @@ const DeviceInfo& device_info();
 // `row_stride_bytes` apart: box = box_rows x 64 columns (128 bytes), SWIZZLE_128B, zero fill outside.
 int get_tensor_map_2d(const void* base, uint64_t rows, uint64_t cols, uint64_t row_stride_bytes,
                       uint32_t box_rows, uint32_t box_cols, CUtensorMap* out);
+// 3-D view of the same matrix as [rows][cols / 64][64]: box = box_rows x box_ktiles x 64 columns, SWIZZLE_128B.
+int get_tensor_map_x3d(const void* base, uint64_t rows, uint64_t cols, uint32_t box_rows, uint32_t box_ktiles,
+                       CUtensorMap* out);
 
 #ifdef __CUDACC__
 // ------------------------------------------------------------------------------------------------
@@ -126,6 +129,15 @@ __device__ __forceinline__ void tma_load_2d(void* dst, const CUtensorMap* map, i
         "cp.async.bulk.tensor.2d.shared::cluster.global.tile.mbarrier::complete_tx::bytes.L2::cache_hint "
         "[%0], [%1, {%3, %4}], [%2], %5;" ::"r"(smem_u32(dst)),
         "l"(map), "r"(smem_u32(bar)), "r"(c0), "r"(c1), "l"(policy)
+        : "memory");
+}
+// 3-D tiled tensor copy global -> shared (c0 = innermost coordinate).
+__device__ __forceinline__ void tma_load_3d(void* dst, const CUtensorMap* map, int c0, int c1, int c2,
+                                            uint64_t* bar, uint64_t policy) {
+    asm volatile(
+        "cp.async.bulk.tensor.3d.shared::cluster.global.tile.mbarrier::complete_tx::bytes.L2::cache_hint "
+        "[%0], [%1, {%3, %4, %5}], [%2], %6;" ::"r"(smem_u32(dst)),
+        "l"(map), "r"(smem_u32(bar)), "r"(c0), "r"(c1), "r"(c2), "l"(policy)
         : "memory");
 }
 __device__ __forceinline__ void tma_prefetch_desc(const CUtensorMap* map) {

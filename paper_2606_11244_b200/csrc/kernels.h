@@ -18,7 +18,8 @@ struct StreamParams {
     int G;                   // K / group
     int group_chunks;        // group / 128
     int C;                   // K / 128 chunks per panel
-    int U;                   // (N / 128) * C work units
+    int CP;                  // (C + 1) / 2 chunk pairs = work units per panel
+    int U;                   // (N / 128) * CP work units
     // ---- fused EC (SPEAR_VARIANT_STREAM_FUSED): z = x [A; w_g]^T, gate and u are computed by this kernel ----
     int fused;               // 0: u comes from the EC pre-kernel; 1: warp 9 of every CTA produces it
     int gate_kind;           // SPEAR_GATE_SCALAR_SIGMOID or SPEAR_GATE_NONE

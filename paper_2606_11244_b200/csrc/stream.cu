@@ -1,25 +1,31 @@
 // stream.cu -- the weight-streaming kernel for small token counts (decode, M <= 16).
 //
-// Computes steps S1-S3, S7, S8 of SURVEY.md 8(a) in one launch (Eq. 3):
+// Computes steps S1-S3, S7, S8 of SURVEY.md 8(a) -- and, in the fused variant, S4-S6 -- in one launch
+// (Eq. 3):
 //     y[m][n] = sum_k x[m][k] * (q[n][k] - 8) * s[n][k/group]  +  sum_j u[m][j] * B[n][j]
-// where u = alpha * gamma (.) (A x) was produced by the EC pre-kernel (ec_pre.cu) and r == 0 is the
-// plain W4 layer.  The paper's decode kernel runs the EC chain in a MARLIN epilogue on
-// Hopper; here the layer is HBM-bound, so the design is a TMA-fed shared-memory ring:
+// where u = alpha * gamma (.) (A x) comes from the EC pre-kernel (ec_pre.cu, split variant) or from warp 9
+// of this kernel (fused variant); r == 0 is the plain W4 layer.  The paper's decode kernel
+// runs the EC chain in a MARLIN epilogue on Hopper; here the layer is HBM-bound, so the design is a
+// TMA-fed shared-memory ring:
 //
-//   * work unit = (panel of 128 output rows, chunk of 128 input columns) = 8 KiB of packed int4,
-//     contiguous in the SPW4 layout; units are numbered panel-major and split evenly (stream-K)
-//     over gridDim.x CTAs, so every SM streams the same number of bytes whatever the shape;
-//   * warp 0 is the producer: one lane issues cp.async.bulk (weights, scales) and a swizzled TMA
-//     tensor copy (the x tile, zero-filled beyond M) per unit into a kStages-deep ring guarded by
-//     full/empty mbarriers.  Weight copies are issued BEFORE griddepcontrol.wait (they never depend
-//     on the previous kernel), x copies after it: under programmatic dependent launch the ring of
-//     layer i+1 fills while layer i drains;
-//   * 8 consumer warps: each task is (4 strips of 16 rows) x (64 columns): 4 LDS.128 of int4,
-//     lop3/hsub2 dequantisation in registers, mma.sync.m16n8k16 with the tokens as the n=8 operand
-//     (fp32 accumulate), group scale applied to the fp32 accumulator;
-//   * per panel segment the 8 warps reduce through shared memory; a CTA that owns a whole panel
-//     writes y directly, otherwise it parks an fp32 partial in the workspace and the last arriver
-//     (atomic counter per panel) sums the partials in CTA order, adds the EC term and casts once.
+//   * work unit = (panel of 128 output rows, PAIR of 128-column chunks) = 16 KiB of packed int4,
+//     contiguous in the SPW4 layout (the last unit of a panel is a single chunk when K/128 is odd);
+//     units are numbered panel-major and split evenly (stream-K) over gridDim.x CTAs, so every SM streams
+//     the same number of bytes whatever the shape.  Large units keep the number of asynchronous-copy
+//     instructions per byte low: one thread issues them, and ~200 cycles each is what bounds a ring of
+//     small copies;
+//   * warp 0, one lane: cp.async.bulk of weights and scales into a kStages-deep ring guarded by full/empty
+//     mbarriers.  It never executes griddepcontrol.wait (weights do not depend on the previous kernel):
+//     under programmatic dependent launch the ring of layer i+1 fills while layer i drains;
+//   * warp 9 (service warp): after griddepcontrol.wait, one 3-D TMA tensor copy per unit brings the x
+//     tile (8*MT tokens x 4 k-tiles x 64 columns, 128-byte swizzle, zero-filled beyond M and K); in the
+//     fused variant the whole warp also reduces this CTA's share of z = x [A; w_g]^T (see below);
+//   * 8 consumer warps, all on the same unit: warp (h, kq) takes strips 4h..4h+3 (64 rows) x k-tile kq
+//     (64 columns): 4 LDS.128 of int4, lop3/sub dequantisation in registers, mma.sync.m16n8k16 with the
+//     tokens as the n=8 operand (fp32 accumulate), group scale applied to the fp32 accumulator;
+//   * per panel segment the 8 warps reduce through shared memory; a CTA that owns a whole panel writes y
+//     directly, otherwise it parks an fp32 partial in the workspace and the last arriver (atomic counter
+//     per panel) sums the partials in CTA order, adds the EC term and casts once.
 #include "common.cuh"
 #include "kernels.h"
 
@@ -27,13 +33,15 @@ namespace spear {
 
 template <int MT>
 struct StreamCfg {
-    static constexpr int kStages = (MT == 1) ? 8 : 6;
-    static constexpr int kXTile = MT * 1024;          // bytes: 8*MT token rows x 128 B
+    static constexpr int kStages = (MT == 1) ? 4 : 3;
+    static constexpr int kXTile = MT * 8 * 512;       // bytes: 8*MT token rows x 4 k-tiles x 128 B
+    static constexpr int kWUnit = 16384;              // two chunks of packed int4
+    static constexpr int kScUnit = 512;               // one 256-byte scale slot per chunk
     static constexpr int kRedStride = 68;             // floats; 68 makes the fragment stores conflict-free
     static constexpr int kTok = 8 * MT;
-    static constexpr size_t kXBytes = size_t(kStages) * 2 * kXTile;
-    static constexpr size_t kWBytes = size_t(kStages) * 8192;
-    static constexpr size_t kScBytes = size_t(kStages) * 256;
+    static constexpr size_t kXBytes = size_t(kStages) * kXTile;
+    static constexpr size_t kWBytes = size_t(kStages) * kWUnit;
+    static constexpr size_t kScBytes = size_t(kStages) * kScUnit;
     static constexpr size_t kRedBytes = size_t(8) * kTok * kRedStride * 4;
     static constexpr size_t kBarBytes = size_t(kStages) * 16 + 32;
     static constexpr size_t kSmemBytes = 1024 + kXBytes + kWBytes + kScBytes + kRedBytes + kBarBytes;
@@ -44,35 +52,74 @@ __device__ __forceinline__ int cta_of_unit(int u, int per, int rem) {
     return (u < big) ? u / (per + 1) : rem + (u - big) / per;
 }
 
+// ---- the consumer inner loop -------------------------------------------------------------------------
+// Explicit shared-window loads (32-bit addresses; the generic-pointer form compiles to LD.E + 64-bit math).
+__device__ __forceinline__ uint4 lds128(uint32_t addr) {
+    uint4 v;
+    asm volatile("ld.shared.v4.u32 {%0, %1, %2, %3}, [%4];" : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w) : "r"(addr));
+    return v;
+}
+__device__ __forceinline__ uint32_t lds32(uint32_t addr) {
+    uint32_t v;
+    asm volatile("ld.shared.u32 %0, [%1];" : "=r"(v) : "r"(addr));
+    return v;
+}
+// The four fp16 pairs of one SPW4 word WITHOUT removing the bias: pairs 0 and 2 hold 1024 + q, pairs 1
+// and 3 hold 1024 + 16 q (lop3 only: 5 instructions per 8 weights instead of 9).  The mma that consumes
+// pairs 1 and 3 is fed x / 16 (exact), and the bias -- (1024 + 8) x on the even pairs, (64 + 8) x on the
+// odd ones, the same for every output row -- enters as the accumulator's initial value (see stream_task).
+__device__ __forceinline__ void biased_word(uint32_t w, uint32_t (&out)[4]) {
+    constexpr uint32_t kMagic = 0x64006400u;
+    asm("lop3.b32 %0, %1, 0x000f000f, %2, 0xea;" : "=r"(out[0]) : "r"(w), "r"(kMagic));
+    asm("lop3.b32 %0, %1, 0x00f000f0, %2, 0xea;" : "=r"(out[1]) : "r"(w), "r"(kMagic));
+    const uint32_t w8 = w >> 8;
+    asm("lop3.b32 %0, %1, 0x000f000f, %2, 0xea;" : "=r"(out[2]) : "r"(w8), "r"(kMagic));
+    asm("lop3.b32 %0, %1, 0x00f000f0, %2, 0xea;" : "=r"(out[3]) : "r"(w8), "r"(kMagic));
+}
+
+// One (4 strips = 64 rows) x (64 columns) task of a warp.  w_addr: this lane's first 16 bytes of the
+// chunk's k-tile (strip 4h), strips are 512 bytes apart; sc_addr: this lane's scale word of strip 4h,
+// strips 32 bytes apart; x_addr: the unit's x tile [token row][k-tile kq 0..3][64 columns], written by TMA
+// with the 128-byte swizzle (16-byte chunk index XOR bits 7..9 of the address = kq | (row & 1) << 2).
+//   sum_k (q - 8) x  =  sum_even (1024 + q) x + sum_odd (1024 + 16 q)(x / 16) - [1032 sum_even x + 72 sum_odd x]
+// The bracket is produced by four mma with the constant fragment (-1032 | -1152 = -72 * 16) and used as the
+// initial accumulator of every strip; all products are exact in fp32, the sums are fp32 tensor-core adds.
 template <int MT>
-__device__ __forceinline__ void stream_task(const uint8_t* __restrict__ wst, const uint8_t* __restrict__ xst,
-                                            const uint8_t* __restrict__ scst, int h, int ktl, int lane,
+__device__ __forceinline__ void stream_task(uint32_t w_addr, uint32_t x_addr, uint32_t sc_addr, int kq, int lane,
                                             float (&tot)[4][MT][4]) {
     const int g = lane >> 2, t = lane & 3;
+    const int xr = kq | ((g & 1) << 2);
     uint32_t xa[MT][4], xb[MT][4];
+    float negc[MT][4];
 #pragma unroll
     for (int mt = 0; mt < MT; ++mt) {
-        const uint8_t* row = xst + ktl * (MT * 1024) + (mt * 8 + g) * 128;
-        const uint4 va = *reinterpret_cast<const uint4*>(row + (((2 * t) ^ g) << 4));
-        const uint4 vb = *reinterpret_cast<const uint4*>(row + (((2 * t + 1) ^ g) << 4));
-        xa[mt][0] = va.x; xa[mt][1] = va.y; xa[mt][2] = va.z; xa[mt][3] = va.w;
-        xb[mt][0] = vb.x; xb[mt][1] = vb.y; xb[mt][2] = vb.z; xb[mt][3] = vb.w;
+        const uint32_t row = x_addr + (mt * 8 + g) * 512 + kq * 128;
+        const uint4 va = lds128(row + (((2 * t) ^ xr) << 4));
+        const uint4 vb = lds128(row + (((2 * t + 1) ^ xr) << 4));
+        constexpr uint32_t kSixteenth = 0x2c002c00u;
+        xa[mt][0] = va.x; xa[mt][1] = hmul2_u32(va.y, kSixteenth); xa[mt][2] = va.z; xa[mt][3] = hmul2_u32(va.w, kSixteenth);
+        xb[mt][0] = vb.x; xb[mt][1] = hmul2_u32(vb.y, kSixteenth); xb[mt][2] = vb.z; xb[mt][3] = hmul2_u32(vb.w, kSixteenth);
+        constexpr uint32_t kNeg1032 = 0xe408e408u, kNeg1152 = 0xe480e480u;
+        negc[mt][0] = negc[mt][1] = negc[mt][2] = negc[mt][3] = 0.f;
+        mma_m16n8k16(negc[mt], kNeg1032, kNeg1032, kNeg1032, kNeg1032, xa[mt][0], xb[mt][0]);
+        mma_m16n8k16(negc[mt], kNeg1152, kNeg1152, kNeg1152, kNeg1152, xa[mt][1], xb[mt][1]);
+        mma_m16n8k16(negc[mt], kNeg1032, kNeg1032, kNeg1032, kNeg1032, xa[mt][2], xb[mt][2]);
+        mma_m16n8k16(negc[mt], kNeg1152, kNeg1152, kNeg1152, kNeg1152, xa[mt][3], xb[mt][3]);
     }
 #pragma unroll
     for (int j = 0; j < 4; ++j) {
-        const int strip = 4 * h + j;
-        const uint4 w = *reinterpret_cast<const uint4*>(wst + ((ktl * 8 + strip) * 32 + lane) * 16);
-        const uint32_t scw = *reinterpret_cast<const uint32_t*>(scst + (strip * 16 + 2 * g) * 2);
+        const uint4 w = lds128(w_addr + j * 512);
+        const uint32_t scw = lds32(sc_addr + j * 32);
         const float s_lo = __half2float(__ushort_as_half(uint16_t(scw & 0xffff)));
         const float s_hi = __half2float(__ushort_as_half(uint16_t(scw >> 16)));
         uint32_t a0[4], a1[4], a2[4], a3[4];
-        dequant_word(w.x, a0);   // row g,   columns 16t + 0..7
-        dequant_word(w.z, a1);   // row g+8, columns 16t + 0..7
-        dequant_word(w.y, a2);   // row g,   columns 16t + 8..15
-        dequant_word(w.w, a3);   // row g+8, columns 16t + 8..15
+        biased_word(w.x, a0);   // row g,   columns 16t + 0..7
+        biased_word(w.z, a1);   // row g+8, columns 16t + 0..7
+        biased_word(w.y, a2);   // row g,   columns 16t + 8..15
+        biased_word(w.w, a3);   // row g+8, columns 16t + 8..15
 #pragma unroll
         for (int mt = 0; mt < MT; ++mt) {
-            float acc[4] = {0.f, 0.f, 0.f, 0.f};
+            float acc[4] = {negc[mt][0], negc[mt][1], negc[mt][2], negc[mt][3]};
 #pragma unroll
             for (int jj = 0; jj < 4; ++jj)
                 mma_m16n8k16(acc, a0[jj], a1[jj], a2[jj], a3[jj], xa[mt][jj], xb[mt][jj]);
@@ -109,7 +156,32 @@ __device__ __forceinline__ void ec_load16(const __half* row, int col, bool reado
     }
 }
 
-__device__ void ec_warp_fused(const StreamParams& p, int lane, uint64_t* u_ready) {
+// Before griddepcontrol.wait: pull this CTA's slice of [A; w_g] (the rows / K range of its phase-A tasks) into
+// L2, so that the loads after the wait do not pay an HBM round trip on the critical path.
+__device__ void ec_prefetch_factors(const StreamParams& p, int lane) {
+    const bool scalar = (p.gate_kind == SPEAR_GATE_SCALAR_SIGMOID);
+    const int rows_total = p.r + (scalar ? 1 : 0);
+    const int strips = (rows_total + 15) >> 4;
+    const int G = gridDim.x;
+    const int ktiles = p.K >> 6;
+    const int ksplit = max(1, min(ktiles, G / strips));
+    const int n_tasks = strips * ksplit;
+    for (int task = blockIdx.x; task < n_tasks; task += G) {
+        const int strip = task % strips, ks = task / strips;
+        const int kt_begin = int((long long)ks * ktiles / ksplit);
+        const int kt_end = int((long long)(ks + 1) * ktiles / ksplit);
+        const int lines = kt_end - kt_begin;           // 128-byte lines per row
+        for (int i = lane; i < 16 * lines; i += 32) {
+            const int rho = strip * 16 + i / lines, kt = kt_begin + i % lines;
+            const __half* row = rho < p.r ? p.A + size_t(rho) * p.K : (rho == p.r && scalar ? p.w_g : nullptr);
+            if (row) prefetch_l2(row + kt * 64);
+        }
+    }
+}
+
+// Phase A (whole warp, after griddepcontrol.wait): this CTA's piece of z, red.add, arrive.  Returns true in
+// the last CTA to arrive.
+__device__ bool ec_reduce_and_arrive(const StreamParams& p, int lane) {
     const int g = lane >> 2, t = lane & 3;
     const bool scalar = (p.gate_kind == SPEAR_GATE_SCALAR_SIGMOID);
     const int rows_total = p.r + (scalar ? 1 : 0);
@@ -120,7 +192,6 @@ __device__ void ec_warp_fused(const StreamParams& p, int lane, uint64_t* u_ready
     const int n_tasks = strips * ksplit;
     const __half* px0 = g < p.M ? p.x + size_t(g) * p.K : nullptr;
     const __half* px1 = g + 8 < p.M ? p.x + size_t(g + 8) * p.K : nullptr;
-    bool waited = false;
     for (int task = blockIdx.x; task < n_tasks; task += G) {
         const int strip = task % strips, ks = task / strips;
         const int rho0 = strip * 16 + g, rho1 = rho0 + 8;
@@ -134,7 +205,6 @@ __device__ void ec_warp_fused(const StreamParams& p, int lane, uint64_t* u_ready
             uint32_t a0l[4], a0h[4], a1l[4], a1h[4], x0l[4], x0h[4], x1l[4], x1h[4];
             ec_load16(pa0, col, true, a0l, a0h);     // EC factors are parameters: never written by a kernel
             ec_load16(pa1, col, true, a1l, a1h);
-            if (!waited) { pdl_wait(); waited = true; }   // x may come from the previous kernel
             ec_load16(px0, col, false, x0l, x0h);
             ec_load16(px1, col, false, x1l, x1h);
 #pragma unroll
@@ -154,24 +224,41 @@ __device__ void ec_warp_fused(const StreamParams& p, int lane, uint64_t* u_ready
             }
         }
     }
-    if (!waited) pdl_wait();
     __threadfence();
     __syncwarp();
     unsigned old = 0;
     if (lane == 0) old = atomicAdd(p.ec_sync + 0, 1u);
     old = __shfl_sync(0xffffffffu, old, 0);
-    if (old == unsigned(G - 1)) {
-        // ---- last arriver: gate, u, clean-up ----
+    return old == unsigned(G - 1);
+}
+
+// Phase B in the last arriver: gate (PAPER.md:109 / BASELINE.json scalar gate), u, clean-up, flag.
+__device__ void ec_gate_and_publish(const StreamParams& p, int lane, unsigned epoch) {
+    const bool scalar = (p.gate_kind == SPEAR_GATE_SCALAR_SIGMOID);
+    const int rows_total = p.r + (scalar ? 1 : 0);
+    {
         __threadfence();
         const float bias = (scalar && p.b_g) ? *p.b_g : 0.f;
+        // lane m owns token m's gate; the z values are fetched 8 at a time so their L2 latencies overlap
+        float gam_own = 1.f;
+        if (scalar && lane < p.M) gam_own = 1.f / (1.f + expf(-(__ldcg(p.zbuf + lane * kZStride + p.r) + bias)));
+        if (scalar && p.gate_out && lane < p.M) p.gate_out[lane] = gam_own;
         const int n = p.M * p.r;
-        for (int idx = lane; idx < n; idx += 32) {
-            const int m = idx / p.r, j = idx - m * p.r;
-            const float z = __ldcg(p.zbuf + m * kZStride + j);
-            float gam = 1.f;
-            if (scalar) gam = 1.f / (1.f + expf(-(__ldcg(p.zbuf + m * kZStride + p.r) + bias)));
-            p.u_out[idx] = p.alpha * gam * z;
-            if (scalar && p.gate_out && j == 0) p.gate_out[m] = gam;
+        for (int base = 0; base < n; base += 256) {
+            float zv[8];
+#pragma unroll
+            for (int q = 0; q < 8; ++q) {
+                const int idx = base + q * 32 + lane;
+                zv[q] = 0.f;
+                if (idx < n) { const int m = idx / p.r; zv[q] = __ldcg(p.zbuf + m * kZStride + (idx - m * p.r)); }
+            }
+#pragma unroll
+            for (int q = 0; q < 8; ++q) {
+                const int idx = base + q * 32 + lane;
+                const int m = min(idx / p.r, 15);
+                const float gam = __shfl_sync(0xffffffffu, gam_own, m);
+                if (idx < n) p.u_out[idx] = p.alpha * gam * zv[q];
+            }
         }
         __syncwarp();
         for (int idx = lane; idx < p.M * rows_total; idx += 32) {
@@ -182,24 +269,10 @@ __device__ void ec_warp_fused(const StreamParams& p, int lane, uint64_t* u_ready
         __syncwarp();
         if (lane == 0) {
             p.ec_sync[0] = 0;
-            if (G > 1) {
-                __threadfence();
-                asm volatile("st.release.gpu.global.u32 [%0], %1;" ::"l"(p.ec_sync + 1), "r"(1u) : "memory");
-            }
-        }
-    } else if (lane == 0) {
-        unsigned f = 0;
-        do {
-            asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(f) : "l"(p.ec_sync + 1) : "memory");
-        } while (f == 0);
-        const unsigned readers = atomicAdd(p.ec_sync + 2, 1u);
-        if (readers == unsigned(G - 2)) {      // every waiting CTA has seen the flag: leave the workspace clean
-            p.ec_sync[2] = 0;
-            p.ec_sync[1] = 0;
+            __threadfence();
+            asm volatile("st.release.gpu.global.u32 [%0], %1;" ::"l"(p.ec_sync + 1), "r"(epoch + 1u) : "memory");
         }
     }
-    __syncwarp();
-    if (lane == 0) mbar_arrive(u_ready);
 }
 
 template <int MT>
@@ -216,64 +289,51 @@ stream_kernel(const __grid_constant__ CUtensorMap xmap, const StreamParams p) {
     uint64_t* full = reinterpret_cast<uint64_t*>(reinterpret_cast<uint8_t*>(red) + Cfg::kRedBytes);
     uint64_t* empty = full + S;
     int* flag = reinterpret_cast<int*>(empty + S);
-    uint64_t* u_ready = reinterpret_cast<uint64_t*>(flag + 2);   // fused EC: u is in global memory, visible
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int G = gridDim.x, b = blockIdx.x;
     const int per = p.U / G, rem = p.U % G;
     const int u0 = b * per + min(b, rem);
     const int n_units = per + (b < rem ? 1 : 0);
-    const int C = p.C;
+    const int C = p.C, CP = p.CP;     // chunks and chunk pairs (= units) per panel
 
     if (threadIdx.x == 0) {
-        for (int s = 0; s < S; ++s) { mbar_init(&full[s], 1); mbar_init(&empty[s], 4); }
-        mbar_init(u_ready, 1);
+        for (int s = 0; s < S; ++s) { mbar_init(&full[s], 2); mbar_init(&empty[s], 8); }
         fence_mbar_init();
         tma_prefetch_desc(&xmap);
     }
     __syncthreads();
     pdl_launch_dependents();
-    if (warp == 9) {
-        if (p.fused && p.r > 0) ec_warp_fused(p, lane, u_ready);
-        return;
-    }
-    if (n_units == 0) return;
 
     if (warp == 0) {
-        // ------------------------------ producer ------------------------------
+        // ------------------------------ weight producer ------------------------------
+        // never waits for the previous kernel: under programmatic dependent launch the ring of layer i+1
+        // fills while layer i drains
         if (lane == 0) {
-            const uint64_t pol_w = policy_evict_first(), pol_x = policy_evict_last();
+            const uint64_t pol_w = policy_evict_first(), pol_s = policy_evict_last();
             const uint8_t* wq = reinterpret_cast<const uint8_t*>(p.wq);
             const uint8_t* sc = reinterpret_cast<const uint8_t*>(p.scales);
-            const int nfirst = min(n_units, S);
-            for (int it = 0; it < nfirst; ++it) {
-                const int u = u0 + it, pnl = u / C, c = u - pnl * C;
-                mbar_expect_tx(&full[it], 8192 + 256);
-                bulk_g2s(wring + it * 8192, wq + (size_t(pnl) * C + c) * 8192, 8192, &full[it], pol_w);
-                bulk_g2s(scring + it * 256, sc + (size_t(pnl) * p.G + c / p.group_chunks) * 256, 256,
-                         &full[it], pol_x);
-            }
-            pdl_wait();   // x may be written by the previous kernel in the stream
-            for (int it = 0; it < nfirst; ++it) {
-                const int c = (u0 + it) % C;
-                mbar_arrive_expect_tx(&full[it], 2 * Cfg::kXTile);
-                tma_load_2d(xring + (it * 2 + 0) * Cfg::kXTile, &xmap, c * 128, 0, &full[it], pol_x);
-                tma_load_2d(xring + (it * 2 + 1) * Cfg::kXTile, &xmap, c * 128 + 64, 0, &full[it], pol_x);
-            }
-            for (int it = S; it < n_units; ++it) {
+            int pnl = u0 / CP, pr = u0 - pnl * CP;
+            for (int it = 0; it < n_units; ++it) {
                 const int s = it % S;
-                const int u = u0 + it, pnl = u / C, c = u - pnl * C;
-                mbar_wait(&empty[s], ((it / S) & 1) ^ 1);
-                mbar_arrive_expect_tx(&full[s], 8192 + 256 + 2 * Cfg::kXTile);
-                bulk_g2s(wring + s * 8192, wq + (size_t(pnl) * C + c) * 8192, 8192, &full[s], pol_w);
-                bulk_g2s(scring + s * 256, sc + (size_t(pnl) * p.G + c / p.group_chunks) * 256, 256,
-                         &full[s], pol_x);
-                tma_load_2d(xring + (s * 2 + 0) * Cfg::kXTile, &xmap, c * 128, 0, &full[s], pol_x);
-                tma_load_2d(xring + (s * 2 + 1) * Cfg::kXTile, &xmap, c * 128 + 64, 0, &full[s], pol_x);
+                if (it >= S) mbar_wait(&empty[s], ((it / S) & 1) ^ 1);
+                const int c0 = 2 * pr, nch = (c0 + 1 < C) ? 2 : 1;
+                mbar_arrive_expect_tx(&full[s], nch * (8192 + 256));
+                bulk_g2s(wring + s * Cfg::kWUnit, wq + (size_t(pnl) * C + c0) * 8192, nch * 8192, &full[s], pol_w);
+                const uint8_t* sp = sc + size_t(pnl) * p.G * 256;
+                if (p.group_chunks == 1) {
+                    bulk_g2s(scring + s * Cfg::kScUnit, sp + size_t(c0) * 256, nch * 256, &full[s], pol_s);
+                } else {
+                    bulk_g2s(scring + s * Cfg::kScUnit, sp + size_t(c0 / p.group_chunks) * 256, 256, &full[s], pol_s);
+                    if (nch == 2)
+                        bulk_g2s(scring + s * Cfg::kScUnit + 256, sp + size_t((c0 + 1) / p.group_chunks) * 256, 256,
+                                 &full[s], pol_s);
+                }
+                if (++pr == CP) { pr = 0; ++pnl; }
             }
         } else if (p.r > 0) {
             // warm L2 with the B rows of every panel this CTA may finalise (read only in the epilogue)
-            const int p_first = u0 / C, p_last = (u0 + n_units - 1) / C;
+            const int p_first = u0 / CP, p_last = (u0 + n_units - 1) / CP;
             const uint8_t* Bb = reinterpret_cast<const uint8_t*>(p.B);
             const size_t slab = size_t(128) * p.r * 2;
             for (int pnl = p_first; pnl <= p_last; ++pnl)
@@ -282,10 +342,39 @@ stream_kernel(const __grid_constant__ CUtensorMap xmap, const StreamParams p) {
         }
         return;
     }
+    if (warp == 9) {
+        // ------------------------------ service warp: x tiles (+ fused EC) ------------------------------
+        const uint64_t pol_x = policy_evict_last();
+        if (p.fused && p.r > 0) ec_prefetch_factors(p, lane);   // EC factors are parameters: warm L2 before the wait
+        pdl_wait();   // x may be written by the previous kernel in the stream
+        auto issue_x = [&](int it) {
+            const int s = it % S;
+            if (it >= S) mbar_wait(&empty[s], ((it / S) & 1) ^ 1);
+            mbar_arrive_expect_tx(&full[s], Cfg::kXTile);
+            tma_load_3d(xring + s * Cfg::kXTile, &xmap, 0, ((u0 + it) % CP) * 4, 0, &full[s], pol_x);
+        };
+        // The u-ready flag is an epoch that the last arriver bumps and nobody resets: its value before this
+        // launch is read here (after the wait, before this CTA arrives, hence before anyone can bump it) and
+        // handed to the consumers through shared memory; the x-tile barrier arrive below publishes it.
+        const bool fused = p.fused && p.r > 0;
+        unsigned epoch = 0;
+        if (fused) {
+            if (lane == 0) { epoch = *reinterpret_cast<volatile unsigned*>(p.ec_sync + 1); flag[1] = int(epoch); }
+            epoch = __shfl_sync(0xffffffffu, epoch, 0);
+        }
+        const int nfirst = min(n_units, S);
+        if (lane == 0)
+            for (int it = 0; it < nfirst; ++it) issue_x(it);
+        __syncwarp();
+        if (fused && ec_reduce_and_arrive(p, lane)) ec_gate_and_publish(p, lane, epoch);
+        if (lane == 0)
+            for (int it = nfirst; it < n_units; ++it) issue_x(it);
+        return;
+    }
 
     // -------------------------------- consumers --------------------------------
     const int cw = warp - 1;
-    const int h = cw & 1, ktl = (cw >> 1) & 1, par = cw >> 2;
+    const int h = cw & 1, kq = cw >> 1;        // strips 4h..4h+3, k-tile kq of the unit's (up to) four
     const int g = lane >> 2, t = lane & 3;
     const int ct = threadIdx.x - 32;            // 0..255
     pdl_wait();                                 // orders our workspace / y writes after the previous kernel
@@ -298,17 +387,26 @@ stream_kernel(const __grid_constant__ CUtensorMap xmap, const StreamParams p) {
 #pragma unroll
             for (int i = 0; i < 4; ++i) tot[j][mt][i] = 0.f;
 
+    // ring slot / phase and the unit's position inside its panel advance incrementally (no divisions here)
+    int rs = 0, pr = u0 % CP;
+    uint32_t rph = 0;
+    const uint32_t w_lane = smem_u32(wring) + (kq >> 1) * 8192 + (((kq & 1) * 8 + 4 * h) * 32 + lane) * 16;
+    const uint32_t sc_lane = smem_u32(scring) + (kq >> 1) * 256 + (4 * h * 16 + 2 * g) * 2;
+    const uint32_t x_base = smem_u32(xring);
     int it = 0;
     while (it < n_units) {
-        const int pnl = (u0 + it) / C;
+        const int pnl = (u0 + it) / CP;
         const int seg_begin = it;
-        const int seg_end = min(n_units, (pnl + 1) * C - u0);
-        for (int i = seg_begin + ((par ^ seg_begin) & 1); i < seg_end; i += 2) {
-            const int s = i % S;
-            mbar_wait(&full[s], (i / S) & 1);
-            stream_task<MT>(wring + s * 8192, xring + s * 2 * Cfg::kXTile, scring + s * 256, h, ktl, lane, tot);
+        const int seg_end = min(n_units, (pnl + 1) * CP - u0);
+        for (int i = seg_begin; i < seg_end; ++i) {
+            mbar_wait(&full[rs], rph);
+            if (2 * pr + (kq >> 1) < C)             // the second chunk is absent in a panel's odd tail unit
+                stream_task<MT>(w_lane + rs * Cfg::kWUnit, x_base + rs * Cfg::kXTile, sc_lane + rs * Cfg::kScUnit,
+                                kq, lane, tot);
             __syncwarp();
-            if (lane == 0) mbar_arrive(&empty[s]);
+            if (lane == 0) mbar_arrive(&empty[rs]);
+            if (++rs == S) { rs = 0; rph ^= 1; }
+            if (++pr == CP) pr = 0;
         }
         // ---- CTA-level reduction of the segment: red[warp][token][row within the half panel] ----
         float* myred = red + size_t(cw) * Cfg::kTok * Cfg::kRedStride;
@@ -335,18 +433,18 @@ stream_kernel(const __grid_constant__ CUtensorMap xmap, const StreamParams p) {
                 v += red[size_t(hh + 2 * q) * Cfg::kTok * Cfg::kRedStride + tok * Cfg::kRedStride + rl];
             val[i] = v;
         }
-        const bool whole = ((u0 + seg_begin) % C == 0) && (seg_end - seg_begin == C);
+        const bool whole = ((u0 + seg_begin) % CP == 0) && (seg_end - seg_begin == CP);
         bool finalize = whole;
         int c_first = b, c_last = b;
         if (!whole) {
-            const int which = ((u0 / C) == pnl) ? 0 : 1;
+            const int which = ((u0 / CP) == pnl) ? 0 : 1;
             float* slot = p.partial + size_t(b * 2 + which) * Cfg::kTok * 128;
 #pragma unroll
             for (int i = 0; i < 4 * MT; ++i) slot[((ct >> 7) + 2 * i) * 128 + row] = val[i];
             __threadfence();
             named_bar_sync(2, 256);
-            c_first = cta_of_unit(pnl * C, per, rem);
-            c_last = cta_of_unit(pnl * C + C - 1, per, rem);
+            c_first = cta_of_unit(pnl * CP, per, rem);
+            c_last = cta_of_unit(pnl * CP + CP - 1, per, rem);
             if (ct == 0) {
                 const unsigned old = atomicAdd(p.counters + pnl, 1u);
                 const int last = (old == unsigned(c_last - c_first));
@@ -361,7 +459,7 @@ stream_kernel(const __grid_constant__ CUtensorMap xmap, const StreamParams p) {
                 for (int i = 0; i < 4 * MT; ++i) val[i] = 0.f;
                 for (int cj = c_first; cj <= c_last; ++cj) {
                     const int uj = cj * per + min(cj, rem);
-                    const int wj = ((uj / C) == pnl) ? 0 : 1;
+                    const int wj = ((uj / CP) == pnl) ? 0 : 1;
                     const float* sj = p.partial + size_t(cj * 2 + wj) * Cfg::kTok * 128;
 #pragma unroll
                     for (int i = 0; i < 4 * MT; ++i) val[i] += __ldcg(sj + ((ct >> 7) + 2 * i) * 128 + row);
@@ -372,7 +470,21 @@ stream_kernel(const __grid_constant__ CUtensorMap xmap, const StreamParams p) {
             const int n = pnl * 128 + row;
             if (p.r > 0) {
                 // S7: y += sum_j u[m][j] * B[n][j]   (u = alpha * gamma (.) z, fp32, from the pre-kernel or warp 9)
-                if (p.fused) mbar_wait(u_ready, 0);
+                if (p.fused) {
+                    if (ct == 0) {      // wait (late) for the last arriver's epoch bump; u is then visible
+                        const unsigned e0 = unsigned(flag[1]);
+                        unsigned f;
+                        do {
+                            asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(f) : "l"(p.ec_sync + 1) : "memory");
+                        } while (f == e0);
+                    }
+                }
+                // u (M x r fp32, <= 8 KiB) is staged once in the idle reduction buffer: every lane of a warp
+                // then reads the same word (broadcast) instead of paying an L2 round trip per term
+                float* us = red;
+                named_bar_sync(2, 256);      // every thread has taken its sums out of red[]
+                for (int idx = ct; idx < p.M * p.r; idx += 256) us[idx] = __ldcg(p.u + idx);
+                named_bar_sync(2, 256);
                 const uint4* Brow = reinterpret_cast<const uint4*>(p.B + size_t(n) * p.r);
                 for (int j8 = 0; j8 < p.r / 8; ++j8) {
                     const uint4 bv = __ldg(Brow + j8);
@@ -387,8 +499,8 @@ stream_kernel(const __grid_constant__ CUtensorMap xmap, const StreamParams p) {
                     for (int i = 0; i < 4 * MT; ++i) {
                         const int tok = (ct >> 7) + 2 * i;
                         if (tok < p.M) {
-                            const float4* up = reinterpret_cast<const float4*>(p.u + size_t(tok) * p.r + j8 * 8);
-                            const float4 ua = __ldcg(up), ub = __ldcg(up + 1);
+                            const float4* up = reinterpret_cast<const float4*>(us + tok * p.r + j8 * 8);
+                            const float4 ua = up[0], ub = up[1];
                             val[i] += ua.x * bf[0] + ua.y * bf[1] + ua.z * bf[2] + ua.w * bf[3] +
                                       ub.x * bf[4] + ub.y * bf[5] + ub.z * bf[6] + ub.w * bf[7];
                         }

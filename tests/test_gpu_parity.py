@@ -251,3 +251,40 @@ def test_fused_back_to_back_leaves_workspace_clean(sp):
     rms = float(np.sqrt(np.mean(ref ** 2)))
     for y in ys:
         assert float(np.max(np.abs(y.cpu().numpy().astype(np.float64) - ref))) <= Y_TOL * rms
+
+
+# ---------------------------------------------------------------- batch of independent calls (concurrent lanes)
+
+def test_batch_matches_oracle_and_single_calls(sp):
+    """spear_w4_ec_gemm_batch over mixed shapes / token counts (decode, mid-M, plain and EC): each call
+    must equal the oracle, also inside a CUDA graph replayed several times."""
+    import torch
+    h = _harness()
+    specs = [(1, 256, 512, 16, "scalar"), (16, 384, 640, 24, "scalar"), (8, 2048, 2048, 0, "scalar"),
+             (4, 512, 1024, 32, "mlp"), (40, 256, 512, 16, "scalar"), (3, 128, 128, 8, "none"), (16, 3072, 2048, 32, "scalar")]
+    lis = [make_layer(500 + i, M, N, K, 128, r, gate=g) for i, (M, N, K, r, g) in enumerate(specs)]
+    dls = [h.upload_layer(li) for li in lis]
+    xs = [h.dev(li.x) for li in lis]
+    ys = [torch.zeros((li.M, li.N), dtype=torch.float16, device="cuda:0") for li in lis]
+    batch = sp.Batch([(x, dl.pw, dl.A, dl.B, dl.desc(), y) for x, dl, y in zip(xs, dls, ys)])
+    sp.w4_ec_gemm_batch(batch)
+    torch.cuda.synchronize()
+    refs = [oracle.forward_layer(li)["y"] for li in lis]
+
+    def verify(tag):
+        for li, y, ref in zip(lis, ys, refs):
+            rms = float(np.sqrt(np.mean(ref ** 2)))
+            err = float(np.max(np.abs(y.cpu().numpy().astype(np.float64) - ref)))
+            assert err <= Y_TOL * rms, f"{tag}: M={li.M} N={li.N} r={li.r}: {err:.4g} > {Y_TOL} * {rms:.4g}"
+    verify("eager")
+    st = torch.cuda.Stream()
+    with torch.cuda.stream(st):
+        g = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(g, stream=st):
+            sp.w4_ec_gemm_batch(batch)
+        for y in ys:
+            y.zero_()
+        for _ in range(3):
+            g.replay()
+    torch.cuda.synchronize()
+    verify("graph")
