@@ -134,6 +134,10 @@ def run_cuda(args, rank, world):
     sp.init()
     if os.environ.get("SPEAR_PDL") is not None:
         sp.tune("pdl", int(os.environ["SPEAR_PDL"]))
+    for kv in os.environ.get("SPEAR_TUNE", "").split(","):     # sweep hook: key=value,... for spear_tune
+        if "=" in kv:
+            k, v = kv.split("=")
+            sp.tune(k.strip(), int(v))
 
     shapes = step_shapes()
     # weights / EC factors: one seeded set per projection (the M=16 entry's seed), shared by the three

@@ -199,8 +199,11 @@ struct Tunables {
     int tc_grid = 0;              // 0 = heuristic
     int tc_cluster = 0;           // 0 = heuristic, else 1 / 2 / 4
     int batch_lanes = 4;          // concurrent lanes of spear_w4_ec_gemm_batch (1..4)
+    int stream_deep = -1;         // -1 = heuristic, 0 / 1 = force the shallow / deep decode ring
+    int stream_debug = 0;         // measurement hook, see StreamParams::debug
 };
 static Tunables g_tune;
+static thread_local bool t_in_batch = false;
 
 struct PlanKey {
     int M, N, K, r, group, gate;
@@ -310,8 +313,19 @@ static int run_stream(const void* x, const void* Wq, const void* scales, const v
     p.G = K / group; p.group_chunks = group / 128; p.C = K / 128;
     p.CP = (p.C + 1) / 2;
     p.U = (N / 128) * p.CP;
-    // the fused EC's device-wide arrive/wait needs every CTA resident: at most 2 per SM (launch bounds)
-    int grid = std::min(p.U, g_dev.num_sms * std::max(1, std::min(2, g_tune.stream_ctas_per_sm)));
+    // Ring depth: a CTA with many units to stream gets the deep ring (one CTA per SM, enough bytes in flight
+    // to cover the HBM latency); a CTA with few keeps the shallow one so that two CTAs fit an SM and the next
+    // layer's CTA can prefetch beside it.  The fused EC's device-wide arrive/wait needs every CTA resident,
+    // which both choices guarantee (grid <= SMs x resident CTAs per SM).
+    int per_sm = std::max(1, std::min(2, g_tune.stream_ctas_per_sm));
+    const int units_per_cta = (p.U + g_dev.num_sms - 1) / g_dev.num_sms;
+    // Inside a batch the lanes overlap whole kernels, which needs two CTAs per SM: keep the shallow ring there.
+    bool deep = !t_in_batch && units_per_cta > 2;
+    if (g_tune.stream_deep >= 0) deep = g_tune.stream_deep != 0;
+    if (deep) per_sm = 1;
+    p.stages = stream_stages(MT, deep);
+    p.debug = g_tune.stream_debug;
+    int grid = std::min(p.U, g_dev.num_sms * per_sm);
     grid = std::min(grid, kMaxStreamGrid);
     if (fused && r > 0) {
         p.fused = 1;
@@ -423,6 +437,8 @@ extern "C" int spear_tune(const char* key, int value) {
     else if (!strcmp(key, "tc_grid")) g_tune.tc_grid = value;
     else if (!strcmp(key, "tc_cluster")) g_tune.tc_cluster = value;
     else if (!strcmp(key, "batch_lanes")) g_tune.batch_lanes = value;
+    else if (!strcmp(key, "stream_deep")) g_tune.stream_deep = value;
+    else if (!strcmp(key, "stream_debug")) g_tune.stream_debug = value;
     else return set_error(SPEAR_EINVAL, "unknown tunable '%s'", key);
     return SPEAR_OK;
 }
@@ -476,6 +492,7 @@ extern "C" int spear_w4_ec_gemm_batch(const spear_call* calls, int n_calls, void
     SPEAR_CUDA_OK(cudaEventRecord(g_batch_fork, st));
     for (int l = 0; l < lanes; ++l) SPEAR_CUDA_OK(cudaStreamWaitEvent(g_lane_stream[l], g_batch_fork, 0));
     int status = SPEAR_OK;
+    t_in_batch = lanes > 1;
     for (int i = 0; i < n_calls && status == SPEAR_OK; ++i) {
         const spear_call& c = calls[i];
         if (c.ec && c.ec->workspace) { status = set_error(SPEAR_EINVAL, "batch calls use the library's lane workspaces (ec->workspace must be NULL)"); break; }
@@ -488,6 +505,7 @@ extern "C" int spear_w4_ec_gemm_batch(const spear_call* calls, int n_calls, void
         else
             status = set_error(SPEAR_ENOMEM, "batch call %d needs %zu bytes of workspace (lane has %zu)", i, need, kLaneWorkspace);
     }
+    t_in_batch = false;
     // always join, also after an error, so that `stream` stays consistent (and a capture stays valid)
     for (int l = 0; l < lanes; ++l) {
         cudaEventRecord(g_lane_done[l], g_lane_stream[l]);

@@ -20,6 +20,8 @@ struct StreamParams {
     int C;                   // K / 128 chunks per panel
     int CP;                  // (C + 1) / 2 chunk pairs = work units per panel
     int U;                   // (N / 128) * CP work units
+    int stages;              // ring depth (stream_stages)
+    int debug;               // bit 0: consumers skip the arithmetic (measures the bare memory pipeline; results are wrong)
     // ---- fused EC (SPEAR_VARIANT_STREAM_FUSED): z = x [A; w_g]^T, gate and u are computed by this kernel ----
     int fused;               // 0: u comes from the EC pre-kernel; 1: warp 9 of every CTA produces it
     int gate_kind;           // SPEAR_GATE_SCALAR_SIGMOID or SPEAR_GATE_NONE
@@ -33,7 +35,8 @@ struct StreamParams {
     float* gate_out;         // optional [M]
     unsigned* ec_sync;       // [0] arrivals, [1] u-ready flag, [2] readers; zero between calls
 };
-int stream_smem_bytes(int MT);
+int stream_stages(int MT, bool deep);
+int stream_smem_bytes(int MT, int stages);
 int launch_stream(const CUtensorMap& xmap, const StreamParams& p, int MT, int grid, bool pdl, cudaStream_t st);
 
 // ---- ec_pre.cu (M <= 16): z = x A^T, gate, u = alpha * gamma (.) z ------------------------------

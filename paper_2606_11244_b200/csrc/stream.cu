@@ -33,18 +33,25 @@ namespace spear {
 
 template <int MT>
 struct StreamCfg {
-    static constexpr int kStages = (MT == 1) ? 4 : 3;
+    // ring depth is a launch parameter: shallow (two CTAs per SM, the next layer's CTA prefetches beside this
+    // one under programmatic dependent launch) for small layers, deep (one CTA per SM, ~150 KiB in flight per
+    // SM to cover the HBM latency) for large ones
+    static constexpr int kStagesShallow = (MT == 1) ? 4 : 3;
+    static constexpr int kStagesDeep = (MT == 1) ? 10 : 7;
+    static constexpr int kMaxStages = 10;
     static constexpr int kXTile = MT * 8 * 512;       // bytes: 8*MT token rows x 4 k-tiles x 128 B
     static constexpr int kWUnit = 16384;              // two chunks of packed int4
     static constexpr int kScUnit = 512;               // one 256-byte scale slot per chunk
     static constexpr int kRedStride = 68;             // floats; 68 makes the fragment stores conflict-free
     static constexpr int kTok = 8 * MT;
-    static constexpr size_t kXBytes = size_t(kStages) * kXTile;
-    static constexpr size_t kWBytes = size_t(kStages) * kWUnit;
-    static constexpr size_t kScBytes = size_t(kStages) * kScUnit;
+    static constexpr size_t x_bytes(int S) { return size_t(S) * kXTile; }
+    static constexpr size_t w_bytes(int S) { return size_t(S) * kWUnit; }
+    static constexpr size_t sc_bytes(int S) { return size_t(S) * kScUnit; }
     static constexpr size_t kRedBytes = size_t(8) * kTok * kRedStride * 4;
-    static constexpr size_t kBarBytes = size_t(kStages) * 16 + 32;
-    static constexpr size_t kSmemBytes = 1024 + kXBytes + kWBytes + kScBytes + kRedBytes + kBarBytes;
+    static constexpr size_t kBarBytes = size_t(kMaxStages) * 16 + 32;
+    static constexpr size_t smem_bytes(int S) { return 1024 + x_bytes(S) + w_bytes(S) + sc_bytes(S) + kRedBytes + kBarBytes; }
+    static_assert(smem_bytes(kStagesDeep) <= 232448, "deep ring exceeds the 227 KiB opt-in shared memory");
+    static_assert(2 * (smem_bytes(kStagesShallow) + 1024) <= 233472, "two shallow CTAs must fit one SM");
 };
 
 __device__ __forceinline__ int cta_of_unit(int u, int per, int rem) {
@@ -100,11 +107,14 @@ __device__ __forceinline__ void stream_task(uint32_t w_addr, uint32_t x_addr, ui
         xa[mt][0] = va.x; xa[mt][1] = hmul2_u32(va.y, kSixteenth); xa[mt][2] = va.z; xa[mt][3] = hmul2_u32(va.w, kSixteenth);
         xb[mt][0] = vb.x; xb[mt][1] = hmul2_u32(vb.y, kSixteenth); xb[mt][2] = vb.z; xb[mt][3] = hmul2_u32(vb.w, kSixteenth);
         constexpr uint32_t kNeg1032 = 0xe408e408u, kNeg1152 = 0xe480e480u;
-        negc[mt][0] = negc[mt][1] = negc[mt][2] = negc[mt][3] = 0.f;
-        mma_m16n8k16(negc[mt], kNeg1032, kNeg1032, kNeg1032, kNeg1032, xa[mt][0], xb[mt][0]);
-        mma_m16n8k16(negc[mt], kNeg1152, kNeg1152, kNeg1152, kNeg1152, xa[mt][1], xb[mt][1]);
-        mma_m16n8k16(negc[mt], kNeg1032, kNeg1032, kNeg1032, kNeg1032, xa[mt][2], xb[mt][2]);
-        mma_m16n8k16(negc[mt], kNeg1152, kNeg1152, kNeg1152, kNeg1152, xa[mt][3], xb[mt][3]);
+        // short dependency chains: a dependent mma.sync costs far more than an independent one here
+        float n0[4] = {0.f, 0.f, 0.f, 0.f}, n1[4] = {0.f, 0.f, 0.f, 0.f};
+        mma_m16n8k16(n0, kNeg1032, kNeg1032, kNeg1032, kNeg1032, xa[mt][0], xb[mt][0]);
+        mma_m16n8k16(n1, kNeg1152, kNeg1152, kNeg1152, kNeg1152, xa[mt][1], xb[mt][1]);
+        mma_m16n8k16(n0, kNeg1032, kNeg1032, kNeg1032, kNeg1032, xa[mt][2], xb[mt][2]);
+        mma_m16n8k16(n1, kNeg1152, kNeg1152, kNeg1152, kNeg1152, xa[mt][3], xb[mt][3]);
+#pragma unroll
+        for (int i = 0; i < 4; ++i) negc[mt][i] = n0[i] + n1[i];
     }
 #pragma unroll
     for (int j = 0; j < 4; ++j) {
@@ -120,9 +130,13 @@ __device__ __forceinline__ void stream_task(uint32_t w_addr, uint32_t x_addr, ui
 #pragma unroll
         for (int mt = 0; mt < MT; ++mt) {
             float acc[4] = {negc[mt][0], negc[mt][1], negc[mt][2], negc[mt][3]};
+            float acd[4] = {0.f, 0.f, 0.f, 0.f};
+            mma_m16n8k16(acc, a0[0], a1[0], a2[0], a3[0], xa[mt][0], xb[mt][0]);
+            mma_m16n8k16(acd, a0[1], a1[1], a2[1], a3[1], xa[mt][1], xb[mt][1]);
+            mma_m16n8k16(acc, a0[2], a1[2], a2[2], a3[2], xa[mt][2], xb[mt][2]);
+            mma_m16n8k16(acd, a0[3], a1[3], a2[3], a3[3], xa[mt][3], xb[mt][3]);
 #pragma unroll
-            for (int jj = 0; jj < 4; ++jj)
-                mma_m16n8k16(acc, a0[jj], a1[jj], a2[jj], a3[jj], xa[mt][jj], xb[mt][jj]);
+            for (int i = 0; i < 4; ++i) acc[i] += acd[i];
             tot[j][mt][0] = fmaf(s_lo, acc[0], tot[j][mt][0]);
             tot[j][mt][1] = fmaf(s_lo, acc[1], tot[j][mt][1]);
             tot[j][mt][2] = fmaf(s_hi, acc[2], tot[j][mt][2]);
@@ -279,16 +293,16 @@ template <int MT>
 __global__ void __launch_bounds__(320, 2)
 stream_kernel(const __grid_constant__ CUtensorMap xmap, const StreamParams p) {
     using Cfg = StreamCfg<MT>;
-    constexpr int S = Cfg::kStages;
+    const int S = p.stages;
     extern __shared__ uint8_t smem_raw[];
     uint8_t* base = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
     uint8_t* xring = base;
-    uint8_t* wring = xring + Cfg::kXBytes;
-    uint8_t* scring = wring + Cfg::kWBytes;
-    float* red = reinterpret_cast<float*>(scring + Cfg::kScBytes);
+    uint8_t* wring = xring + Cfg::x_bytes(S);
+    uint8_t* scring = wring + Cfg::w_bytes(S);
+    float* red = reinterpret_cast<float*>(scring + Cfg::sc_bytes(S));
     uint64_t* full = reinterpret_cast<uint64_t*>(reinterpret_cast<uint8_t*>(red) + Cfg::kRedBytes);
-    uint64_t* empty = full + S;
-    int* flag = reinterpret_cast<int*>(empty + S);
+    uint64_t* empty = full + Cfg::kMaxStages;
+    int* flag = reinterpret_cast<int*>(empty + Cfg::kMaxStages);
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int G = gridDim.x, b = blockIdx.x;
@@ -314,9 +328,10 @@ stream_kernel(const __grid_constant__ CUtensorMap xmap, const StreamParams p) {
             const uint8_t* wq = reinterpret_cast<const uint8_t*>(p.wq);
             const uint8_t* sc = reinterpret_cast<const uint8_t*>(p.scales);
             int pnl = u0 / CP, pr = u0 - pnl * CP;
+            int s = 0;
+            uint32_t eph = 1;     // parity to wait for on empty[]: the first pass over the ring never waits
             for (int it = 0; it < n_units; ++it) {
-                const int s = it % S;
-                if (it >= S) mbar_wait(&empty[s], ((it / S) & 1) ^ 1);
+                if (it >= S) mbar_wait(&empty[s], eph);
                 const int c0 = 2 * pr, nch = (c0 + 1 < C) ? 2 : 1;
                 mbar_arrive_expect_tx(&full[s], nch * (8192 + 256));
                 bulk_g2s(wring + s * Cfg::kWUnit, wq + (size_t(pnl) * C + c0) * 8192, nch * 8192, &full[s], pol_w);
@@ -330,6 +345,7 @@ stream_kernel(const __grid_constant__ CUtensorMap xmap, const StreamParams p) {
                                  &full[s], pol_s);
                 }
                 if (++pr == CP) { pr = 0; ++pnl; }
+                if (++s == S) { s = 0; eph ^= 1; }
             }
         } else if (p.r > 0) {
             // warm L2 with the B rows of every panel this CTA may finalise (read only in the epilogue)
@@ -347,11 +363,14 @@ stream_kernel(const __grid_constant__ CUtensorMap xmap, const StreamParams p) {
         const uint64_t pol_x = policy_evict_last();
         if (p.fused && p.r > 0) ec_prefetch_factors(p, lane);   // EC factors are parameters: warm L2 before the wait
         pdl_wait();   // x may be written by the previous kernel in the stream
+        int xs = 0, xpr = u0 % CP;
+        uint32_t xeph = 1;
         auto issue_x = [&](int it) {
-            const int s = it % S;
-            if (it >= S) mbar_wait(&empty[s], ((it / S) & 1) ^ 1);
-            mbar_arrive_expect_tx(&full[s], Cfg::kXTile);
-            tma_load_3d(xring + s * Cfg::kXTile, &xmap, 0, ((u0 + it) % CP) * 4, 0, &full[s], pol_x);
+            if (it >= S) mbar_wait(&empty[xs], xeph);
+            mbar_arrive_expect_tx(&full[xs], Cfg::kXTile);
+            tma_load_3d(xring + xs * Cfg::kXTile, &xmap, 0, xpr * 4, 0, &full[xs], pol_x);
+            if (++xs == S) { xs = 0; xeph ^= 1; }
+            if (++xpr == CP) xpr = 0;
         };
         // The u-ready flag is an epoch that the last arriver bumps and nobody resets: its value before this
         // launch is read here (after the wait, before this CTA arrives, hence before anyone can bump it) and
@@ -400,7 +419,7 @@ stream_kernel(const __grid_constant__ CUtensorMap xmap, const StreamParams p) {
         const int seg_end = min(n_units, (pnl + 1) * CP - u0);
         for (int i = seg_begin; i < seg_end; ++i) {
             mbar_wait(&full[rs], rph);
-            if (2 * pr + (kq >> 1) < C)             // the second chunk is absent in a panel's odd tail unit
+            if (2 * pr + (kq >> 1) < C && !(p.debug & 1))   // the second chunk is absent in a panel's odd tail unit
                 stream_task<MT>(w_lane + rs * Cfg::kWUnit, x_base + rs * Cfg::kXTile, sc_lane + rs * Cfg::kScUnit,
                                 kq, lane, tot);
             __syncwarp();
@@ -519,8 +538,12 @@ stream_kernel(const __grid_constant__ CUtensorMap xmap, const StreamParams p) {
     }
 }
 
-int stream_smem_bytes(int MT) {
-    return int(MT == 1 ? StreamCfg<1>::kSmemBytes : StreamCfg<2>::kSmemBytes);
+int stream_stages(int MT, bool deep) {
+    if (MT == 1) return deep ? StreamCfg<1>::kStagesDeep : StreamCfg<1>::kStagesShallow;
+    return deep ? StreamCfg<2>::kStagesDeep : StreamCfg<2>::kStagesShallow;
+}
+int stream_smem_bytes(int MT, int stages) {
+    return int(MT == 1 ? StreamCfg<1>::smem_bytes(stages) : StreamCfg<2>::smem_bytes(stages));
 }
 
 int launch_stream(const CUtensorMap& xmap, const StreamParams& p, int MT, int grid, bool pdl,
@@ -528,15 +551,15 @@ int launch_stream(const CUtensorMap& xmap, const StreamParams& p, int MT, int gr
     static bool attr_set = false;
     if (!attr_set) {
         SPEAR_CUDA_OK(cudaFuncSetAttribute(stream_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                           int(StreamCfg<1>::kSmemBytes)));
+                                           int(StreamCfg<1>::smem_bytes(StreamCfg<1>::kStagesDeep))));
         SPEAR_CUDA_OK(cudaFuncSetAttribute(stream_kernel<2>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                           int(StreamCfg<2>::kSmemBytes)));
+                                           int(StreamCfg<2>::smem_bytes(StreamCfg<2>::kStagesDeep))));
         attr_set = true;
     }
     cudaLaunchConfig_t cfg = {};
     cfg.gridDim = dim3(grid);
     cfg.blockDim = dim3(320);
-    cfg.dynamicSmemBytes = stream_smem_bytes(MT);
+    cfg.dynamicSmemBytes = stream_smem_bytes(MT, p.stages);
     cfg.stream = st;
     cudaLaunchAttribute attr[1];
     attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
