@@ -404,7 +404,7 @@ int run_tc(const TcProblem& t, cudaStream_t st) {
     const int n_mt = (t.M + BT - 1) / BT;
     // clusters share x tiles by TMA multicast; worth it once there are more tiles than SMs (L2 -> SM bound)
     int CS = 1;
-    if (BT == 256 && n_panels * n_mt >= 2 * device_info().num_sms) CS = (n_panels % 4 == 0) ? 4 : (n_panels % 2 == 0 ? 2 : 1);
+    if (BT == 256 && n_panels * n_mt >= 2 * device_info().num_sms && n_panels % 2 == 0) CS = 2;   // measured: 2 > 1 > 4
     if (t.cluster_override > 0 && BT == 256 && n_panels % t.cluster_override == 0) CS = t.cluster_override;
     TcParams p = {};
     p.wq = static_cast<const uint8_t*>(t.wq);

@@ -1,0 +1,54 @@
+"""S9 on the GPU: spear_plan measures the valid variants of a problem, records the fastest, spear_plan_query
+returns it, the table survives save / load, and the planned variant still matches the oracle."""
+import os
+import numpy as np
+import pytest
+
+import oracle
+from workloads import make_layer
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def sp():
+    import paper_2606_11244_b200 as sp
+    sp.init()
+    return sp
+
+
+def test_plan_decode_times_fused_and_split(sp, tmp_path):
+    chosen, us = sp.plan(8, 2048, 2048, 32, 128, gate="scalar")
+    assert chosen in (sp.VARIANT_STREAM_FUSED, sp.VARIANT_STREAM_SPLIT)
+    assert us[sp.VARIANT_STREAM_FUSED] > 0 and us[sp.VARIANT_STREAM_SPLIT] > 0
+    assert us[chosen] == min(t for t in us if t > 0)
+    assert sp.plan_query(8, 2048, 2048, 32, 128, gate="scalar") == chosen
+    # the MLP gate has no fused decode arm: the plan must fall on the split one
+    chosen_mlp, us_mlp = sp.plan(8, 2048, 2048, 32, 128, gate="mlp", gate_hidden=128)
+    assert chosen_mlp == sp.VARIANT_STREAM_SPLIT and us_mlp[sp.VARIANT_STREAM_FUSED] < 0
+    path = str(tmp_path / "plan.txt")
+    sp.plan_save(path)
+    txt = open(path).read()
+    assert "8 2048 2048 32 128" in txt
+    sp.plan_load(path)
+    assert sp.plan_query(8, 2048, 2048, 32, 128, gate="scalar") == chosen
+
+
+def test_plan_crossover_shapes(sp):
+    # M <= 16: the decode kernel and the tcgen05 kernel are both valid; above 16 only the tcgen05 one
+    chosen, us = sp.plan(16, 4096, 4096, 64, 4096, gate="scalar")
+    assert us[sp.VARIANT_TC_FUSED] > 0 and us[sp.VARIANT_STREAM_FUSED] > 0
+    chosen64, us64 = sp.plan(64, 2048, 2048, 32, 128, gate="scalar")
+    assert chosen64 == sp.VARIANT_TC_FUSED and us64[sp.VARIANT_STREAM_FUSED] < 0
+
+
+def test_planned_variant_matches_oracle(sp):
+    import torch
+    from paper_2606_11244_b200 import harness as h
+    li = make_layer(1700, 16, 512, 1024, 128, 16, gate="scalar")
+    sp.plan(li.M, li.N, li.K, li.r, li.group, gate="scalar")
+    y, _ = h.run_layer(h.upload_layer(li), h.dev(li.x))          # AUTO -> the planned variant
+    torch.cuda.synchronize()
+    ref = oracle.forward_layer(li)["y"]
+    rms = float(np.sqrt(np.mean(ref ** 2)))
+    assert float(np.max(np.abs(y.cpu().numpy().astype(np.float64) - ref))) <= 1e-2 * rms
