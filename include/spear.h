@@ -56,10 +56,11 @@ typedef enum {
  * otherwise a size heuristic. */
 typedef enum {
     SPEAR_VARIANT_AUTO = 0,
-    SPEAR_VARIANT_STREAM_FUSED = 1,  /* one kernel: weight stream (mma.sync) + x.A^T, gate, B add inside; M <= 16 */
-    SPEAR_VARIANT_STREAM_SPLIT = 2,  /* EC pre-kernel (z, gate, u) then weight-stream kernel adding u.B^T; any M */
-    SPEAR_VARIANT_TC_FUSED = 3,      /* EC pre-kernel + tcgen05 GEMM with [X|U].[What|aB]^T K-concatenation; M >= 128 */
-    SPEAR_VARIANT_TC_SPLIT = 4,      /* tcgen05 GEMM (plain W4) then a separate rank-r update kernel; M >= 128 */
+    SPEAR_VARIANT_STREAM_FUSED = 1,  /* one kernel: weight stream (mma.sync) + x.A^T, gate, B add inside; M <= 16, scalar / none gate */
+    SPEAR_VARIANT_STREAM_SPLIT = 2,  /* EC pre-kernel (z, any gate, u) then weight-stream kernel adding u.B^T; M <= 16 */
+    SPEAR_VARIANT_TC_FUSED = 3,      /* EC pre-kernel + tcgen05 GEMM with [X|U].[What|B]^T K-concatenation; any M */
+    SPEAR_VARIANT_TC_SPLIT = 4,      /* EC pre-kernel + tcgen05 GEMM (plain W4) + a separate rank-r update pass over y (the
+                                        paper's unfused comparator; y is rounded twice); any M, r > 0 */
     SPEAR_VARIANT_COUNT = 5
 } spear_variant;
 

@@ -198,6 +198,7 @@ struct Tunables {
     int ecpre_ctas = 0;           // 0 = heuristic
     int tc_grid = 0;              // 0 = heuristic
     int tc_cluster = 0;           // 0 = heuristic, else 1 / 2 / 4
+    int tc_ksplit = 0;            // 0 = heuristic, else the tcgen05 kernel's split-K factor
     int batch_lanes = 4;          // concurrent lanes of spear_w4_ec_gemm_batch (1..4)
     int stream_deep = -1;         // -1 = heuristic, 0 / 1 = force the shallow / deep decode ring
     int stream_debug = 0;         // measurement hook, see StreamParams::debug
@@ -220,7 +221,7 @@ static bool variant_valid(int v, int M, int r, int gate) {
         case SPEAR_VARIANT_STREAM_FUSED: return M <= 16 && r > 0 && gate != SPEAR_GATE_MLP;
         case SPEAR_VARIANT_STREAM_SPLIT: return M <= 16;
         case SPEAR_VARIANT_TC_FUSED: return tc_available() && M >= 1;
-        case SPEAR_VARIANT_TC_SPLIT: return false;
+        case SPEAR_VARIANT_TC_SPLIT: return tc_available() && r > 0;
         default: return false;
     }
     (void)r;
@@ -347,7 +348,7 @@ static int run_stream(const void* x, const void* Wq, const void* scales, const v
 // extended by ceil(r/64) blocks [X | U] . [What | B]^T  (SURVEY.md section 7 "Prefill EC fold").
 static int run_tc_fused(const void* x, const void* Wq, const void* scales, const void* A, const void* B,
                         const spear_ec_desc* ec, void* y, int M, int N, int K, int r, int group,
-                        uint8_t* ws, const WsLayout& L, cudaStream_t st) {
+                        uint8_t* ws, const WsLayout& L, bool split, cudaStream_t st) {
     const bool pdl = g_tune.pdl != 0;
     if (r > 0) {
         EcBigParams e = {};
@@ -372,12 +373,21 @@ static int run_tc_fused(const void* x, const void* Wq, const void* scales, const
     }
     TcProblem t = {};
     t.x = x; t.wq = Wq; t.scales = scales; t.B = B; t.y = y;
-    t.u16 = r > 0 ? ws + L.u16 : nullptr;
-    t.M = M; t.N = N; t.K = K; t.r = r; t.group = group;
+    t.u16 = (r > 0 && !split) ? ws + L.u16 : nullptr;
+    t.M = M; t.N = N; t.K = K; t.r = split ? 0 : r; t.group = group;
     t.pdl = pdl;
     t.grid_override = g_tune.tc_grid;
     t.cluster_override = g_tune.tc_cluster;
-    return run_tc(t, st);
+    t.ksplit_override = g_tune.tc_ksplit;
+    t.partial = ws + L.partial;
+    t.partial_bytes = size_t(kMaxStreamGrid) * 2 * 16 * 128 * 4;
+    t.counters = reinterpret_cast<unsigned*>(ws + L.counters) + 1024;
+    t.max_counters = 4096;
+    if (int rc = run_tc(t, st)) return rc;
+    if (split && r > 0)     // TC_SPLIT: plain W4 GEMM, then the rank-r update as its own pass over y
+        return launch_ec_update(reinterpret_cast<const __half*>(ws + L.u16), static_cast<const __half*>(B),
+                                static_cast<__half*>(y), M, N, r, pdl, st);
+    return SPEAR_OK;
 }
 
 static int layer_impl(const void* x, const void* Wq, const void* scales, const void* A, const void* B,
@@ -410,7 +420,9 @@ static int layer_impl(const void* x, const void* Wq, const void* scales, const v
         case SPEAR_VARIANT_STREAM_SPLIT:
             return run_stream(x, Wq, scales, A, B, ec, y, M, N, K, r, group, ws, L, false, st);
         case SPEAR_VARIANT_TC_FUSED:
-            return run_tc_fused(x, Wq, scales, A, B, ec, y, M, N, K, r, group, ws, L, st);
+            return run_tc_fused(x, Wq, scales, A, B, ec, y, M, N, K, r, group, ws, L, false, st);
+        case SPEAR_VARIANT_TC_SPLIT:
+            return run_tc_fused(x, Wq, scales, A, B, ec, y, M, N, K, r, group, ws, L, true, st);
         default:
             return set_error(SPEAR_EUNSUPPORTED, "variant %d not implemented", v);
     }
@@ -436,6 +448,7 @@ extern "C" int spear_tune(const char* key, int value) {
     else if (!strcmp(key, "ecpre_ctas")) g_tune.ecpre_ctas = value;
     else if (!strcmp(key, "tc_grid")) g_tune.tc_grid = value;
     else if (!strcmp(key, "tc_cluster")) g_tune.tc_cluster = value;
+    else if (!strcmp(key, "tc_ksplit")) g_tune.tc_ksplit = value;
     else if (!strcmp(key, "batch_lanes")) g_tune.batch_lanes = value;
     else if (!strcmp(key, "stream_deep")) g_tune.stream_deep = value;
     else if (!strcmp(key, "stream_debug")) g_tune.stream_debug = value;

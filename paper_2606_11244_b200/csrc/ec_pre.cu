@@ -319,4 +319,72 @@ int launch_ec_big(const EcBigParams& p, bool pdl, cudaStream_t st) {
     return SPEAR_OK;
 }
 
+// ------------------------------------------------------------------------------------------------
+// Split arm for M > 16 (SPEAR_VARIANT_TC_SPLIT): the rank-r up-projection as its own pass over y,
+//     y[m][n] = RN_fp16( y[m][n] + sum_j u16[m][j] * B[n][j] )        (S7 of SURVEY.md 8(a))
+// i.e. the paper's naive "re-projection and accumulation" kernels kept as the comparator the
+// measured dispatch chooses against.  y was already rounded once by the plain W4 GEMM: this arm double-rounds
+// (reading A8) and reads + writes y a second time -- which is exactly why the fused arm usually wins.
+// Block = 256 threads, tile = 32 tokens x 128 channels; u and B tiles staged in shared memory as fp32 / fp16.
+// ------------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(256) ec_update_kernel(const __half* __restrict__ u16, const __half* __restrict__ B,
+                                                        __half* __restrict__ y, int M, int N, int r) {
+    extern __shared__ uint8_t ec_upd_smem[];
+    float* us = reinterpret_cast<float*>(ec_upd_smem);                 // [32][r]
+    __half* bs = reinterpret_cast<__half*>(us + 32 * r);               // [128][r + 2] (padded: conflict-free)
+    const int m0 = blockIdx.y * 32, n0 = blockIdx.x * 128;
+    const int tid = threadIdx.x;
+    pdl_launch_dependents();
+    pdl_wait();
+    for (int i = tid; i < 32 * r; i += 256) {
+        const int m = m0 + i / r;
+        us[i] = m < M ? __half2float(u16[size_t(m) * r + (i % r)]) : 0.f;
+    }
+    const int rs = r + 2;
+    for (int i = tid; i < 128 * r; i += 256) {
+        const int nn = i / r, j = i - nn * r;
+        bs[nn * rs + j] = B[size_t(n0 + nn) * r + j];
+    }
+    __syncthreads();
+    const int nl = tid & 127, tg = tid >> 7;        // channel, token half (16 tokens each)
+    float acc[16];
+#pragma unroll
+    for (int t = 0; t < 16; ++t) acc[t] = 0.f;
+    for (int j = 0; j < r; ++j) {
+        const float b = __half2float(bs[nl * rs + j]);
+#pragma unroll
+        for (int t = 0; t < 16; ++t) acc[t] = fmaf(us[(tg * 16 + t) * r + j], b, acc[t]);
+    }
+#pragma unroll
+    for (int t = 0; t < 16; ++t) {
+        const int m = m0 + tg * 16 + t;
+        if (m < M) {
+            __half* yp = y + size_t(m) * N + n0 + nl;
+            *yp = __float2half_rn(__half2float(*yp) + acc[t]);
+        }
+    }
+}
+
+int launch_ec_update(const __half* u16, const __half* B, __half* y, int M, int N, int r, bool pdl, cudaStream_t st) {
+    const size_t smem = size_t(32) * r * 4 + size_t(128) * (r + 2) * 2;
+    static bool attr_set = false;
+    if (!attr_set) {
+        SPEAR_CUDA_OK(cudaFuncSetAttribute(ec_update_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 64 * 1024));
+        attr_set = true;
+    }
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3(N / 128, (M + 31) / 32);
+    cfg.blockDim = dim3(256);
+    cfg.dynamicSmemBytes = smem;
+    cfg.stream = st;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr[0].val.programmaticStreamSerializationAllowed = pdl ? 1 : 0;
+    cfg.attrs = attr;
+    cfg.numAttrs = 1;
+    SPEAR_CUDA_OK(cudaLaunchKernelEx(&cfg, ec_update_kernel, u16, B, y, M, N, r));
+    count_launch();
+    return SPEAR_OK;
+}
+
 }  // namespace spear

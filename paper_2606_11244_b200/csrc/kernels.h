@@ -75,6 +75,8 @@ struct EcBigParams {
     float alpha;
 };
 int launch_ec_big(const EcBigParams& p, bool pdl, cudaStream_t st);
+// split arm for M > 16: y += u16 . B^T as a separate pass (SPEAR_VARIANT_TC_SPLIT)
+int launch_ec_update(const __half* u16, const __half* B, __half* y, int M, int N, int r, bool pdl, cudaStream_t st);
 
 // ---- tc.cu (M > 16): tcgen05 GEMM, int4 dequantised into shared memory, EC folded in as extra K blocks
 struct TcProblem {
@@ -84,6 +86,11 @@ struct TcProblem {
     bool pdl;
     int grid_override;
     int cluster_override;    // 0 = heuristic, else 1 / 2 / 4 CTAs sharing x tiles by TMA multicast
+    int ksplit_override;     // 0 = heuristic, else the split-K factor
+    void* partial;           // fp32 split-K slots (workspace)
+    size_t partial_bytes;
+    unsigned* counters;      // zero between calls
+    int max_counters;
 };
 bool tc_available();
 int run_tc(const TcProblem& t, cudaStream_t st);

@@ -106,14 +106,39 @@ struct TcParams {
     int kb_ec;               // ceil(r / 64) EC k-blocks
     int n_pp, n_mt;          // N / (128 * CS) panel groups (CS = cluster size), ceil(M / BT)
     int mt_group;            // token tiles per raster group (keeps the x slice L2-resident)
-    int n_tiles;             // n_pp * n_mt work items; each is taken by one cluster (CTA rank c -> panel pp * CS + c)
+    int n_tiles;             // n_pp * n_mt output tiles; each is taken by one cluster (CTA rank c -> panel pp * CS + c)
+    int ksplit;              // split-K factor: a tile's weight k-blocks are shared by `ksplit` work items
+    int n_work;              // n_tiles * ksplit
+    float* partial;          // [n_tiles * CS][ksplit][BT][128] fp32, split-K partial sums (ksplit > 1)
+    unsigned* counters;      // [n_tiles * CS], zero between calls
 };
+
+// One work item: output tile (panel group, token tile) and its share of the reduction axis.  The EC k-blocks
+// belong to the last split.
+struct TcWork {
+    int panel, mt, ks, kb0, nw, ne;
+};
+__device__ __forceinline__ void tile_coords(const TcParams& p, int tile, int& panel, int& mt);
+__device__ __forceinline__ TcWork get_work(const TcParams& p, int w) {
+    TcWork t;
+    const int tile = w / p.ksplit;
+    t.ks = w - tile * p.ksplit;
+    tile_coords(p, tile, t.panel, t.mt);
+    t.kb0 = int((long long)t.ks * p.kb_w / p.ksplit);
+    t.nw = int((long long)(t.ks + 1) * p.kb_w / p.ksplit) - t.kb0;
+    t.ne = (t.ks == p.ksplit - 1) ? p.kb_ec : 0;
+    return t;
+}
 
 template <int BT>
 struct TcCfg {
     // the x ring hides an L2 round trip per stage (deep); the A ring only the local dequantisation (shallow)
-    static constexpr int kXStages = BT == 256 ? 5 : (BT == 128 ? 8 : 10);
-    static constexpr int kAStages = 3;
+    static constexpr int kXStages = BT == 256 ? 5 : (BT == 128 ? 6 : 10);
+    // dequantisation warp groups of 8 taking k-blocks round-robin: a k-block costs one barrier round trip
+    // (~0.7 us) whatever its MMA time, so narrow token tiles (short MMAs) get three groups and a deeper A ring
+    static constexpr int kDequantGroups = BT == 256 ? 2 : 3;
+    static constexpr int kThreads = (7 + 8 * kDequantGroups) * 32;   // + x producer, MMA, 4 epilogue, int4 producer
+    static constexpr int kAStages = BT == 256 ? 3 : 5;
     static constexpr int kW4Stages = BT == 256 ? 4 : 8;
     static constexpr int kABytes = 128 * 128;            // 128 channels x 64 k fp16
     static constexpr int kXBytes = BT * 128;             // BT tokens x 64 k fp16
@@ -123,8 +148,6 @@ struct TcCfg {
     static_assert(kSmemBytes <= 232448, "exceeds the 227 KiB opt-in shared memory of sm_100");
     static constexpr uint32_t kIdesc = (1u << 4) | (uint32_t(BT >> 3) << 17) | (uint32_t(128 >> 4) << 24);
 };
-constexpr int kDequantGroups = 2;        // warp groups of 8 taking k-blocks round-robin (hides the per-k-block barrier latency)
-constexpr int kTcThreads = (7 + 8 * kDequantGroups) * 32;   // + x producer, MMA, 4 epilogue, int4 producer
 
 __device__ __forceinline__ void tile_coords(const TcParams& p, int tile, int& panel, int& mt) {
     const int per_group = p.mt_group * p.n_pp;
@@ -137,7 +160,7 @@ __device__ __forceinline__ void tile_coords(const TcParams& p, int tile, int& pa
 }
 
 template <int BT, int CS>
-__global__ void __launch_bounds__(kTcThreads, 1)
+__global__ void __launch_bounds__(TcCfg<BT>::kThreads, 1)
 tc_kernel(const __grid_constant__ CUtensorMap xmap, const __grid_constant__ CUtensorMap umap,
           const __grid_constant__ CUtensorMap bmap, const TcParams p) {
     using Cfg = TcCfg<BT>;
@@ -159,7 +182,6 @@ tc_kernel(const __grid_constant__ CUtensorMap xmap, const __grid_constant__ CUte
     uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(acc_empty + 2);
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    const int kb_total = p.kb_w + p.kb_ec;
     // a cluster of CS CTAs shares every x tile: each CTA fetches BT / CS token rows and multicasts them
     const int cta_rank = CS > 1 ? int(cluster_ctarank()) : 0;
     const int work0 = blockIdx.x / CS, work_stride = gridDim.x / CS;
@@ -189,35 +211,33 @@ tc_kernel(const __grid_constant__ CUtensorMap xmap, const __grid_constant__ CUte
             const uint64_t pol_x = policy_evict_last();
             pdl_wait();      // x / u16 may be written by the previous kernel in the stream
             int it = 0;
-            for (int tile = work0; tile < p.n_tiles; tile += work_stride) {
-                int panel, mt;
-                tile_coords(p, tile, panel, mt);
-                const int c1 = mt * BT + cta_rank * kXRows;
-                for (int kb = 0; kb < kb_total; ++kb, ++it) {
+            for (int w = work0; w < p.n_work; w += work_stride) {
+                const TcWork t = get_work(p, w);
+                const int c1 = t.mt * BT + cta_rank * kXRows;
+                for (int j = 0; j < t.nw + t.ne; ++j, ++it) {
                     const int s = it % SX;
                     mbar_wait(&x_empty[s], ((it / SX) & 1) ^ 1);
                     mbar_arrive_expect_tx(&x_full[s], Cfg::kXBytes);
                     uint8_t* dst = x_ring + size_t(s) * Cfg::kXBytes + size_t(cta_rank) * kXRows * 128;
-                    const CUtensorMap* map = kb < p.kb_w ? &xmap : &umap;
-                    const int c0 = (kb < p.kb_w ? kb : kb - p.kb_w) * 64;
+                    const CUtensorMap* map = j < t.nw ? &xmap : &umap;
+                    const int c0 = (j < t.nw ? t.kb0 + j : j - t.nw) * 64;
                     if (CS > 1) tma_load_2d_mc(dst, map, c0, c1, &x_full[s], kMask, pol_x);
                     else tma_load_2d(dst, map, c0, c1, &x_full[s], pol_x);
                 }
             }
         }
-    } else if (warp == kTcThreads / 32 - 1) {
+    } else if (warp == Cfg::kThreads / 32 - 1) {
         // ---------------------------------- int4 producer ----------------------------------
         // weights never depend on the previous kernel: no griddepcontrol.wait on this path
         if (lane == 0) {
             const uint64_t pol_w = policy_evict_first(), pol_s = policy_evict_last();
             int w_it = 0;
-            for (int tile = work0; tile < p.n_tiles; tile += work_stride) {
-                int panel, mt;
-                tile_coords(p, tile, panel, mt);
-                panel = panel * CS + cta_rank;
+            for (int w = work0; w < p.n_work; w += work_stride) {
+                const TcWork t = get_work(p, w);
+                const int panel = t.panel * CS + cta_rank;
                 const uint8_t* wsrc = p.wq + size_t(panel) * p.kb_w * 4096;
                 const uint8_t* ssrc = p.scales + size_t(panel) * p.G * 256;
-                for (int kb = 0; kb < p.kb_w; ++kb, ++w_it) {
+                for (int kb = t.kb0; kb < t.kb0 + t.nw; ++kb, ++w_it) {
                     const int s4 = w_it % S4;
                     mbar_wait(&w4_empty[s4], ((w_it / S4) & 1) ^ 1);
                     mbar_arrive_expect_tx(&w4_full[s4], Cfg::kW4Bytes);
@@ -230,7 +250,9 @@ tc_kernel(const __grid_constant__ CUtensorMap xmap, const __grid_constant__ CUte
     } else if (warp == 1) {
         // ---------------------------------- MMA issuer ----------------------------------
         int it = 0, tcount = 0;
-        for (int tile = work0; tile < p.n_tiles; tile += work_stride, ++tcount) {
+        for (int w = work0; w < p.n_work; w += work_stride, ++tcount) {
+            const TcWork t = get_work(p, w);
+            const int kb_total = t.nw + t.ne;
             const int acc = tcount & 1;
             mbar_wait(&acc_empty[acc], ((tcount >> 1) & 1) ^ 1);
             tc_fence_after();
@@ -258,49 +280,95 @@ tc_kernel(const __grid_constant__ CUtensorMap xmap, const __grid_constant__ CUte
         // ---------------------------------- epilogue ----------------------------------
         const int q = warp & 3;                 // TMEM lane quarter this warp may access
         int tcount = 0;
-        for (int tile = work0; tile < p.n_tiles; tile += work_stride, ++tcount) {
-            int panel, mt;
-            tile_coords(p, tile, panel, mt);
-            panel = panel * CS + cta_rank;
+        for (int w = work0; w < p.n_work; w += work_stride, ++tcount) {
+            const TcWork t = get_work(p, w);
+            const int panel = t.panel * CS + cta_rank;
             const int acc = tcount & 1;
             mbar_wait(&acc_full[acc], (tcount >> 1) & 1);
             tc_fence_after();
-            const int n = panel * 128 + q * 32 + lane;
-            const int m0 = mt * BT;
+            const int nl = q * 32 + lane;
+            const int n = panel * 128 + nl;
+            const int m0 = t.mt * BT;
             __half* yp = p.y + size_t(m0) * p.N + n;
+            if (p.ksplit == 1) {
 #pragma unroll 1
-            for (int c = 0; c < BT; c += 32) {
-                if (m0 + c >= p.M) break;       // warp-uniform: nothing left in this tile
-                uint32_t v[32];
-                tmem_ld32(tmem_base + (uint32_t(q * 32) << 16) + uint32_t(acc * BT + c), v);
-                tmem_ld_wait();
+                for (int c = 0; c < BT; c += 32) {
+                    if (m0 + c >= p.M) break;       // warp-uniform: nothing left in this tile
+                    uint32_t v[32];
+                    tmem_ld32(tmem_base + (uint32_t(q * 32) << 16) + uint32_t(acc * BT + c), v);
+                    tmem_ld_wait();
 #pragma unroll
-                for (int i = 0; i < 32; ++i)
-                    if (m0 + c + i < p.M) yp[size_t(c + i) * p.N] = __float2half_rn(__uint_as_float(v[i]));
+                    for (int i = 0; i < 32; ++i)
+                        if (m0 + c + i < p.M) yp[size_t(c + i) * p.N] = __float2half_rn(__uint_as_float(v[i]));
+                }
+                tc_fence_before();
+                __syncwarp();
+                if (lane == 0) mbar_arrive(&acc_empty[acc]);
+            } else {
+                // split-K: park the fp32 partial, the last of the tile's `ksplit` work items to arrive sums them
+                // in split order, casts once and stores y (same pattern as the decode kernel's panels)
+                const int out_id = (w / p.ksplit) * CS + cta_rank;
+                float* slots = p.partial + size_t(out_id) * p.ksplit * (BT * 128);
+                float* mine = slots + size_t(t.ks) * (BT * 128);
+#pragma unroll 1
+                for (int c = 0; c < BT; c += 32) {
+                    if (m0 + c >= p.M) break;
+                    uint32_t v[32];
+                    tmem_ld32(tmem_base + (uint32_t(q * 32) << 16) + uint32_t(acc * BT + c), v);
+                    tmem_ld_wait();
+#pragma unroll
+                    for (int i = 0; i < 32; ++i)
+                        if (m0 + c + i < p.M) mine[(c + i) * 128 + nl] = __uint_as_float(v[i]);
+                }
+                tc_fence_before();
+                __syncwarp();
+                if (lane == 0) mbar_arrive(&acc_empty[acc]);     // the accumulator is drained
+                __threadfence();
+                named_bar_sync(3, 128);
+                if (warp == 2 && lane == 0) {
+                    const unsigned old = atomicAdd(p.counters + out_id, 1u);
+                    const unsigned last = (old == unsigned(p.ksplit - 1));
+                    if (last) p.counters[out_id] = 0;           // self-cleaning
+                    tmem_slot[1] = last;
+                }
+                named_bar_sync(3, 128);
+                if (tmem_slot[1]) {
+                    __threadfence();
+                    const int rows = min(BT, p.M - m0);
+                    for (int mm = 0; mm < rows; mm += 4) {
+                        float sum[4] = {0.f, 0.f, 0.f, 0.f};
+                        for (int ks = 0; ks < p.ksplit; ++ks) {
+                            const float* sk = slots + size_t(ks) * (BT * 128) + nl;
+#pragma unroll
+                            for (int u = 0; u < 4; ++u)
+                                if (mm + u < rows) sum[u] += __ldcg(sk + (mm + u) * 128);
+                        }
+#pragma unroll
+                        for (int u = 0; u < 4; ++u)
+                            if (mm + u < rows) yp[size_t(mm + u) * p.N] = __float2half_rn(sum[u]);
+                    }
+                }
+                named_bar_sync(3, 128);      // tmem_slot[1] is reused by the next work item
             }
-            tc_fence_before();
-            __syncwarp();
-            if (lane == 0) mbar_arrive(&acc_empty[acc]);
         }
     } else {
         // ---------------------------------- dequantisation ----------------------------------
         const int strip = (warp - 6) & 7;       // 16 output channels of the panel
-        const int dgroup = (warp - 6) >> 3;     // this warp converts the k-blocks with it % kDequantGroups == dgroup
+        const int dgroup = (warp - 6) >> 3;     // this warp converts the k-blocks with it % Cfg::kDequantGroups == dgroup
         const int g = lane >> 2, t = lane & 3;
         int it = 0, w_it = 0;
-        for (int tile = work0; tile < p.n_tiles; tile += work_stride) {
-            int panel, mt;
-            tile_coords(p, tile, panel, mt);
-            panel = panel * CS + cta_rank;
-            for (int kb = 0; kb < kb_total; ++kb, ++it) {
+        for (int w = work0; w < p.n_work; w += work_stride) {
+            const TcWork tw = get_work(p, w);
+            const int panel = tw.panel * CS + cta_rank;
+            for (int kb = 0; kb < tw.nw + tw.ne; ++kb, ++it) {
                 const int s = it % SA;
                 uint8_t* a_stage = a_ring + size_t(s) * Cfg::kABytes;
-                if (it % kDequantGroups != dgroup) {
-                    if (kb < p.kb_w) ++w_it;
+                if (it % Cfg::kDequantGroups != dgroup) {
+                    if (kb < tw.nw) ++w_it;
                     continue;
                 }
                 mbar_wait(&a_empty[s], ((it / SA) & 1) ^ 1);
-                if (kb < p.kb_w) {
+                if (kb < tw.nw) {
                     const int s4 = w_it % S4;
                     mbar_wait(&w4_full[s4], (w_it / S4) & 1);
                     ++w_it;
@@ -333,7 +401,7 @@ tc_kernel(const __grid_constant__ CUtensorMap xmap, const __grid_constant__ CUte
                     if (lane == 0) {
                         if (strip == 0) {
                             mbar_arrive_expect_tx(&a_full[s], Cfg::kABytes);
-                            tma_load_2d(a_stage, &bmap, (kb - p.kb_w) * 64, panel * 128, &a_full[s], policy_evict_last());
+                            tma_load_2d(a_stage, &bmap, (kb - tw.nw) * 64, panel * 128, &a_full[s], policy_evict_last());
                         } else {
                             mbar_arrive(&a_full[s]);
                         }
@@ -366,7 +434,7 @@ static int launch_tc(const CUtensorMap& xmap, const CUtensorMap& umap, const CUt
         if (CS > 1) {
             cudaLaunchConfig_t q = {};
             q.gridDim = dim3(device_info().num_sms / CS * CS);
-            q.blockDim = dim3(kTcThreads);
+            q.blockDim = dim3(TcCfg<BT>::kThreads);
             q.dynamicSmemBytes = TcCfg<BT>::kSmemBytes;
             cudaLaunchAttribute qa[1];
             qa[0].id = cudaLaunchAttributeClusterDimension;
@@ -379,11 +447,11 @@ static int launch_tc(const CUtensorMap& xmap, const CUtensorMap& umap, const CUt
         }
         max_clusters = n;
     }
-    int clusters = std::min(p.n_tiles, max_clusters);
+    int clusters = std::min(p.n_work, max_clusters);
     if (grid_override > 0) clusters = std::min(clusters, std::max(1, grid_override / CS));
     cudaLaunchConfig_t cfg = {};
     cfg.gridDim = dim3(clusters * CS);
-    cfg.blockDim = dim3(kTcThreads);
+    cfg.blockDim = dim3(TcCfg<BT>::kThreads);
     cfg.dynamicSmemBytes = TcCfg<BT>::kSmemBytes;
     cfg.stream = st;
     cudaLaunchAttribute attr[2];
@@ -420,6 +488,20 @@ int run_tc(const TcProblem& t, cudaStream_t st) {
     const size_t slice = size_t(BT) * t.K * 2;
     p.mt_group = int(std::max<size_t>(1, std::min<size_t>(size_t(p.n_mt), (size_t(48) << 20) / slice)));
     p.n_tiles = p.n_pp * p.n_mt;
+    // split-K when there are fewer output tiles than SMs (mid-M on small layers): work items = tiles x ksplit
+    int ks = 1;
+    if (CS == 1 && p.n_tiles < device_info().num_sms) {
+        ks = std::min(std::min(device_info().num_sms / p.n_tiles, std::max(1, p.kb_w / 32)), 16);   // measured: a split must keep >= 32 k-blocks to pay for its reduction
+        while (ks > 1 && size_t(p.n_tiles) * ks * BT * 128 * 4 > t.partial_bytes) --ks;
+        if (p.n_tiles > t.max_counters || !t.partial || !t.counters) ks = 1;
+    }
+    if (t.ksplit_override > 0) ks = std::max(1, std::min(t.ksplit_override, p.kb_w));
+    if (ks > 1 && (size_t(p.n_tiles) * ks * BT * 128 * 4 > t.partial_bytes || p.n_tiles * CS > t.max_counters))
+        return set_error(SPEAR_ENOMEM, "tc split-K %d needs more workspace", ks);
+    p.ksplit = ks;
+    p.n_work = p.n_tiles * ks;
+    p.partial = static_cast<float*>(t.partial);
+    p.counters = t.counters;
     CUtensorMap xmap, umap, bmap;
     if (int rc = get_tensor_map_2d(t.x, uint64_t(t.M), uint64_t(t.K), uint64_t(t.K) * 2, uint32_t(BT / CS), 64, &xmap)) return rc;
     if (t.r > 0) {

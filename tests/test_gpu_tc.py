@@ -157,3 +157,30 @@ def test_config5_M64(sp, name):
     s = [c for c in config_shapes(4) if c.M == 64 and c.name == name][0]
     li = make_layer(s.seed, s.M, s.N, s.K, s.group, s.r, gate="scalar")
     check(li, variant=0, label=f"config5 {name} M=64")
+
+
+@pytest.mark.parametrize("ksplit", [2, 3, 7])
+@pytest.mark.parametrize("M,r", [(40, 0), (64, 32), (200, 72)])
+def test_tc_split_k(sp, ksplit, M, r):
+    """Split-K arm of the tcgen05 kernel (fp32 partial slots + last-arriver reduction), forced through the
+    tuning hook; repeated calls must leave the counters clean."""
+    import torch
+    li = make_layer(1600 + M + ksplit, M, 384, 1792, 128, r, gate="scalar")
+    sp.tune("tc_ksplit", ksplit)
+    try:
+        check(li, label=f"tc split-K {ksplit} M={M} r={r}")
+        check(li, label=f"tc split-K {ksplit} M={M} r={r} (second call)")
+    finally:
+        sp.tune("tc_ksplit", 0)
+
+
+@pytest.mark.parametrize("M,r,gate", [(40, 16, "scalar"), (200, 72, "mlp"), (300, 128, "scalar"), (16, 32, "none")])
+def test_tc_split_variant(sp, M, r, gate):
+    """SPEAR_VARIANT_TC_SPLIT: plain W4 tcgen05 GEMM, then the rank-r update as its own pass over y (rounded
+    twice, reading A8) -- still inside the y tolerance, and close to the fused arm."""
+    li = make_layer(1800 + M, M, 384, 640, 128, r, gate=gate)
+    y_split = check(li, variant=4, label=f"tc split M={M} r={r} {gate}")
+    y_fused = check(li, variant=TC, label=f"tc fused M={M} r={r} {gate}")
+    ref = oracle.forward_layer(li)["y"]
+    rms = float(np.sqrt(np.mean(ref ** 2)))
+    assert float((y_split.float() - y_fused.float()).abs().max()) <= Y_TOL * rms
