@@ -202,6 +202,7 @@ struct Tunables {
     int batch_lanes = 4;          // concurrent lanes of spear_w4_ec_gemm_batch (1..4)
     int stream_deep = -1;         // -1 = heuristic, 0 / 1 = force the shallow / deep decode ring
     int stream_debug = 0;         // measurement hook, see StreamParams::debug
+    int stream_whole_panels = 1;  // 1 = whole-panel partition when N/128 is within 1/5 of the grid
 };
 static Tunables g_tune;
 static thread_local bool t_in_batch = false;
@@ -328,6 +329,10 @@ static int run_stream(const void* x, const void* Wq, const void* scales, const v
     p.debug = g_tune.stream_debug;
     int grid = std::min(p.U, g_dev.num_sms * per_sm);
     grid = std::min(grid, kMaxStreamGrid);
+    // When the panels nearly fill the machine, give every CTA whole panels: an even stream-K split would cut almost
+    // every panel in two and pay the cross-CTA reduction (partials through L2 + a counter) on all of them.
+    const int n_panels = N / 128;
+    if (g_tune.stream_whole_panels && n_panels <= grid && n_panels * 5 >= grid * 4) grid = n_panels;
     if (fused && r > 0) {
         p.fused = 1;
         p.gate_kind = ec->gate_kind;
@@ -452,6 +457,7 @@ extern "C" int spear_tune(const char* key, int value) {
     else if (!strcmp(key, "batch_lanes")) g_tune.batch_lanes = value;
     else if (!strcmp(key, "stream_deep")) g_tune.stream_deep = value;
     else if (!strcmp(key, "stream_debug")) g_tune.stream_debug = value;
+    else if (!strcmp(key, "stream_whole_panels")) g_tune.stream_whole_panels = value;
     else return set_error(SPEAR_EINVAL, "unknown tunable '%s'", key);
     return SPEAR_OK;
 }

@@ -412,6 +412,7 @@ stream_kernel(const __grid_constant__ CUtensorMap xmap, const StreamParams p) {
     const uint32_t w_lane = smem_u32(wring) + (kq >> 1) * 8192 + (((kq & 1) * 8 + 4 * h) * 32 + lane) * 16;
     const uint32_t sc_lane = smem_u32(scring) + (kq >> 1) * 256 + (4 * h * 16 + 2 * g) * 2;
     const uint32_t x_base = smem_u32(xring);
+    bool u_seen = false;
     int it = 0;
     while (it < n_units) {
         const int pnl = (u0 + it) / CP;
@@ -489,7 +490,7 @@ stream_kernel(const __grid_constant__ CUtensorMap xmap, const StreamParams p) {
             const int n = pnl * 128 + row;
             if (p.r > 0) {
                 // S7: y += sum_j u[m][j] * B[n][j]   (u = alpha * gamma (.) z, fp32, from the pre-kernel or warp 9)
-                if (p.fused) {
+                if (p.fused && !u_seen) {
                     if (ct == 0) {      // wait (late) for the last arriver's epoch bump; u is then visible
                         const unsigned e0 = unsigned(flag[1]);
                         unsigned f;
@@ -497,6 +498,7 @@ stream_kernel(const __grid_constant__ CUtensorMap xmap, const StreamParams p) {
                             asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(f) : "l"(p.ec_sync + 1) : "memory");
                         } while (f == e0);
                     }
+                    u_seen = true;      // later panels of this CTA need not look again
                 }
                 // u (M x r fp32, <= 8 KiB) is staged once in the idle reduction buffer: every lane of a warp
                 // then reads the same word (broadcast) instead of paying an L2 round trip per term
@@ -505,6 +507,7 @@ stream_kernel(const __grid_constant__ CUtensorMap xmap, const StreamParams p) {
                 for (int idx = ct; idx < p.M * p.r; idx += 256) us[idx] = __ldcg(p.u + idx);
                 named_bar_sync(2, 256);
                 const uint4* Brow = reinterpret_cast<const uint4*>(p.B + size_t(n) * p.r);
+#pragma unroll 4
                 for (int j8 = 0; j8 < p.r / 8; ++j8) {
                     const uint4 bv = __ldg(Brow + j8);
                     const __half2* bh = reinterpret_cast<const __half2*>(&bv);
