@@ -59,6 +59,15 @@ __device__ __forceinline__ int cta_of_unit(int u, int per, int rem) {
     return (u < big) ? u / (per + 1) : rem + (u - big) / per;
 }
 
+// Device-wide arrive: one acq_rel RMW at gpu scope.  Executed after a warp / named barrier it releases the
+// writes of every thread that synchronised with the caller (cumulativity) and acquires what earlier arrivers
+// released -- no separate __threadfence round trips on the critical path.
+__device__ __forceinline__ unsigned arrive_acq_rel(unsigned* ctr) {
+    unsigned old;
+    asm volatile("atom.add.acq_rel.gpu.global.u32 %0, [%1], 1;" : "=r"(old) : "l"(ctr) : "memory");
+    return old;
+}
+
 // ---- the consumer inner loop -------------------------------------------------------------------------
 // Explicit shared-window loads (32-bit addresses; the generic-pointer form compiles to LD.E + 64-bit math).
 __device__ __forceinline__ uint4 lds128(uint32_t addr) {
@@ -238,10 +247,9 @@ __device__ bool ec_reduce_and_arrive(const StreamParams& p, int lane) {
             }
         }
     }
-    __threadfence();
     __syncwarp();
     unsigned old = 0;
-    if (lane == 0) old = atomicAdd(p.ec_sync + 0, 1u);
+    if (lane == 0) old = arrive_acq_rel(p.ec_sync + 0);
     old = __shfl_sync(0xffffffffu, old, 0);
     return old == unsigned(G - 1);
 }
@@ -251,7 +259,7 @@ __device__ void ec_gate_and_publish(const StreamParams& p, int lane, unsigned ep
     const bool scalar = (p.gate_kind == SPEAR_GATE_SCALAR_SIGMOID);
     const int rows_total = p.r + (scalar ? 1 : 0);
     {
-        __threadfence();
+        __syncwarp();       // lane 0's acquire (arrive_acq_rel) covers the whole warp
         const float bias = (scalar && p.b_g) ? *p.b_g : 0.f;
         // lane m owns token m's gate; the z values are fetched 8 at a time so their L2 latencies overlap
         float gam_own = 1.f;
@@ -279,11 +287,10 @@ __device__ void ec_gate_and_publish(const StreamParams& p, int lane, unsigned ep
             const int m = idx / rows_total, rho = idx - m * rows_total;
             p.zbuf[m * kZStride + rho] = 0.f;
         }
-        __threadfence();
         __syncwarp();
         if (lane == 0) {
             p.ec_sync[0] = 0;
-            __threadfence();
+            // release at gpu scope, cumulative over the warp's u stores and z zeroing (ordered by __syncwarp)
             asm volatile("st.release.gpu.global.u32 [%0], %1;" ::"l"(p.ec_sync + 1), "r"(epoch + 1u) : "memory");
         }
     }
@@ -461,12 +468,11 @@ stream_kernel(const __grid_constant__ CUtensorMap xmap, const StreamParams p) {
             float* slot = p.partial + size_t(b * 2 + which) * Cfg::kTok * 128;
 #pragma unroll
             for (int i = 0; i < 4 * MT; ++i) slot[((ct >> 7) + 2 * i) * 128 + row] = val[i];
-            __threadfence();
             named_bar_sync(2, 256);
             c_first = cta_of_unit(pnl * CP, per, rem);
             c_last = cta_of_unit(pnl * CP + CP - 1, per, rem);
             if (ct == 0) {
-                const unsigned old = atomicAdd(p.counters + pnl, 1u);
+                const unsigned old = arrive_acq_rel(p.counters + pnl);   // releases the CTA's partial, acquires the others'
                 const int last = (old == unsigned(c_last - c_first));
                 if (last) p.counters[pnl] = 0;      // self-cleaning: the next call finds zero
                 *flag = last;
@@ -474,15 +480,27 @@ stream_kernel(const __grid_constant__ CUtensorMap xmap, const StreamParams p) {
             named_bar_sync(2, 256);
             finalize = (*flag != 0);
             if (finalize) {
-                __threadfence();
 #pragma unroll
                 for (int i = 0; i < 4 * MT; ++i) val[i] = 0.f;
-                for (int cj = c_first; cj <= c_last; ++cj) {
-                    const int uj = cj * per + min(cj, rem);
-                    const int wj = ((uj / CP) == pnl) ? 0 : 1;
-                    const float* sj = p.partial + size_t(cj * 2 + wj) * Cfg::kTok * 128;
+                // partials are summed in CTA order; four CTAs' loads are issued before the first add so that their
+                // L2 round trips overlap instead of queueing one behind the other
+                for (int cj = c_first; cj <= c_last; cj += 4) {
+                    float tmp[4][4 * MT];
 #pragma unroll
-                    for (int i = 0; i < 4 * MT; ++i) val[i] += __ldcg(sj + ((ct >> 7) + 2 * i) * 128 + row);
+                    for (int q = 0; q < 4; ++q) {
+                        const int cq = min(cj + q, c_last);
+                        const int uj = cq * per + min(cq, rem);
+                        const int wj = ((uj / CP) == pnl) ? 0 : 1;
+                        const float* sj = p.partial + size_t(cq * 2 + wj) * Cfg::kTok * 128;
+#pragma unroll
+                        for (int i = 0; i < 4 * MT; ++i) tmp[q][i] = __ldcg(sj + ((ct >> 7) + 2 * i) * 128 + row);
+                    }
+#pragma unroll
+                    for (int q = 0; q < 4; ++q)
+                        if (cj + q <= c_last) {
+#pragma unroll
+                            for (int i = 0; i < 4 * MT; ++i) val[i] += tmp[q][i];
+                        }
                 }
             }
         }
