@@ -310,6 +310,7 @@ stream_kernel(const __grid_constant__ CUtensorMap xmap, const StreamParams p) {
     uint64_t* full = reinterpret_cast<uint64_t*>(reinterpret_cast<uint8_t*>(red) + Cfg::kRedBytes);
     uint64_t* empty = full + Cfg::kMaxStages;
     int* flag = reinterpret_cast<int*>(empty + Cfg::kMaxStages);
+    uint64_t* e_ready = reinterpret_cast<uint64_t*>(flag + 2);     // fused EC: flag[1] holds the epoch to wait past
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int G = gridDim.x, b = blockIdx.x;
@@ -320,6 +321,7 @@ stream_kernel(const __grid_constant__ CUtensorMap xmap, const StreamParams p) {
 
     if (threadIdx.x == 0) {
         for (int s = 0; s < S; ++s) { mbar_init(&full[s], 2); mbar_init(&empty[s], 8); }
+        mbar_init(e_ready, 1);
         fence_mbar_init();
         tma_prefetch_desc(&xmap);
     }
@@ -327,18 +329,16 @@ stream_kernel(const __grid_constant__ CUtensorMap xmap, const StreamParams p) {
     pdl_launch_dependents();
 
     if (warp == 0) {
-        // ------------------------------ weight producer ------------------------------
-        // never waits for the previous kernel: under programmatic dependent launch the ring of layer i+1
-        // fills while layer i drains
+        // ------------------------------ producer: weights, scales, x tiles ------------------------------
+        // The first ring-full of weights is issued WITHOUT waiting for the previous kernel (weights never depend
+        // on it): under programmatic dependent launch the ring of layer i+1 fills while layer i drains.  x tiles
+        // (which may be the previous kernel's output) follow griddepcontrol.wait.
         if (lane == 0) {
             const uint64_t pol_w = policy_evict_first(), pol_s = policy_evict_last();
             const uint8_t* wq = reinterpret_cast<const uint8_t*>(p.wq);
             const uint8_t* sc = reinterpret_cast<const uint8_t*>(p.scales);
-            int pnl = u0 / CP, pr = u0 - pnl * CP;
-            int s = 0;
-            uint32_t eph = 1;     // parity to wait for on empty[]: the first pass over the ring never waits
-            for (int it = 0; it < n_units; ++it) {
-                if (it >= S) mbar_wait(&empty[s], eph);
+            int pnl = u0 / CP, pr = u0 - pnl * CP, s = 0;
+            auto issue_w = [&]() {
                 const int c0 = 2 * pr, nch = (c0 + 1 < C) ? 2 : 1;
                 mbar_arrive_expect_tx(&full[s], nch * (8192 + 256));
                 bulk_g2s(wring + s * Cfg::kWUnit, wq + (size_t(pnl) * C + c0) * 8192, nch * 8192, &full[s], pol_w);
@@ -351,8 +351,27 @@ stream_kernel(const __grid_constant__ CUtensorMap xmap, const StreamParams p) {
                         bulk_g2s(scring + s * Cfg::kScUnit + 256, sp + size_t((c0 + 1) / p.group_chunks) * 256, 256,
                                  &full[s], pol_s);
                 }
+            };
+            auto issue_x = [&]() {
+                mbar_arrive_expect_tx(&full[s], Cfg::kXTile);
+                tma_load_3d(xring + s * Cfg::kXTile, &xmap, 0, pr * 4, 0, &full[s], pol_s);
+            };
+            auto advance = [&]() {
                 if (++pr == CP) { pr = 0; ++pnl; }
-                if (++s == S) { s = 0; eph ^= 1; }
+                if (++s == S) s = 0;
+            };
+            const int nfirst = min(n_units, S);
+            for (int it = 0; it < nfirst; ++it) { issue_w(); advance(); }
+            pdl_wait();   // x may be written by the previous kernel in the stream
+            pnl = u0 / CP; pr = u0 - pnl * CP; s = 0;
+            for (int it = 0; it < nfirst; ++it) { issue_x(); advance(); }
+            uint32_t eph = 0;     // parity of the first completion of empty[]
+            for (int it = nfirst; it < n_units; ++it) {
+                mbar_wait(&empty[s], eph);
+                issue_w();
+                issue_x();
+                advance();
+                if (s == 0) eph ^= 1;
             }
         } else if (p.r > 0) {
             // warm L2 with the B rows of every panel this CTA may finalise (read only in the epilogue)
@@ -366,35 +385,21 @@ stream_kernel(const __grid_constant__ CUtensorMap xmap, const StreamParams p) {
         return;
     }
     if (warp == 9) {
-        // ------------------------------ service warp: x tiles (+ fused EC) ------------------------------
-        const uint64_t pol_x = policy_evict_last();
-        if (p.fused && p.r > 0) ec_prefetch_factors(p, lane);   // EC factors are parameters: warm L2 before the wait
-        pdl_wait();   // x may be written by the previous kernel in the stream
-        int xs = 0, xpr = u0 % CP;
-        uint32_t xeph = 1;
-        auto issue_x = [&](int it) {
-            if (it >= S) mbar_wait(&empty[xs], xeph);
-            mbar_arrive_expect_tx(&full[xs], Cfg::kXTile);
-            tma_load_3d(xring + xs * Cfg::kXTile, &xmap, 0, xpr * 4, 0, &full[xs], pol_x);
-            if (++xs == S) { xs = 0; xeph ^= 1; }
-            if (++xpr == CP) xpr = 0;
-        };
-        // The u-ready flag is an epoch that the last arriver bumps and nobody resets: its value before this
+        // ------------------------------ EC warp (fused variant only) ------------------------------
+        if (!(p.fused && p.r > 0)) return;
+        ec_prefetch_factors(p, lane);   // EC factors are parameters: warm L2 before the wait
+        pdl_wait();
+        // The u-ready word is an epoch that the last arriver bumps and nobody resets: its value before this
         // launch is read here (after the wait, before this CTA arrives, hence before anyone can bump it) and
-        // handed to the consumers through shared memory; the x-tile barrier arrive below publishes it.
-        const bool fused = p.fused && p.r > 0;
+        // handed to the consumers through shared memory + an mbarrier.
         unsigned epoch = 0;
-        if (fused) {
-            if (lane == 0) { epoch = *reinterpret_cast<volatile unsigned*>(p.ec_sync + 1); flag[1] = int(epoch); }
-            epoch = __shfl_sync(0xffffffffu, epoch, 0);
+        if (lane == 0) {
+            epoch = *reinterpret_cast<volatile unsigned*>(p.ec_sync + 1);
+            flag[1] = int(epoch);
+            mbar_arrive(e_ready);
         }
-        const int nfirst = min(n_units, S);
-        if (lane == 0)
-            for (int it = 0; it < nfirst; ++it) issue_x(it);
-        __syncwarp();
-        if (fused && ec_reduce_and_arrive(p, lane)) ec_gate_and_publish(p, lane, epoch);
-        if (lane == 0)
-            for (int it = nfirst; it < n_units; ++it) issue_x(it);
+        epoch = __shfl_sync(0xffffffffu, epoch, 0);
+        if (ec_reduce_and_arrive(p, lane)) ec_gate_and_publish(p, lane, epoch);
         return;
     }
 
@@ -506,10 +511,11 @@ stream_kernel(const __grid_constant__ CUtensorMap xmap, const StreamParams p) {
         }
         if (finalize) {
             const int n = pnl * 128 + row;
-            if (p.r > 0) {
+            if (p.r > 0 && !(p.debug & 4)) {
                 // S7: y += sum_j u[m][j] * B[n][j]   (u = alpha * gamma (.) z, fp32, from the pre-kernel or warp 9)
-                if (p.fused && !u_seen) {
+                if (p.fused && !u_seen && !(p.debug & 2)) {
                     if (ct == 0) {      // wait (late) for the last arriver's epoch bump; u is then visible
+                        mbar_wait(e_ready, 0);
                         const unsigned e0 = unsigned(flag[1]);
                         unsigned f;
                         do {
