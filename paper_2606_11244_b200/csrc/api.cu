@@ -41,7 +41,7 @@ const DeviceInfo& device_info() { return g_dev; }
 
 // workspace layout (byte offsets); every region is 1 KiB aligned
 struct WsLayout {
-    size_t counters, zbuf, u32, partial, u16, total;
+    size_t counters, zbuf, zfused, u32, partial, u16, total;
 };
 constexpr size_t kCounterBytes = 64 * 1024;          // 16384 u32
 constexpr int kEcPreCounter = 8192;                  // index into counters[]
@@ -55,6 +55,7 @@ static WsLayout ws_layout(int M, int r, size_t ws_bytes) {
     size_t o = 0;
     L.counters = o; o += kCounterBytes;
     L.u32 = o; o += align_up(size_t(16) * 128 * 4, 1024);
+    L.zfused = o; o += align_up(size_t(2) * 16 * kZStride * 4, 1024);   // fused decode EC: z, double-buffered by epoch parity
     L.partial = o; o += size_t(kMaxStreamGrid) * 2 * 16 * 128 * 4;
     L.zbuf = o; o += align_up(size_t(M > 16 ? M : 16) * kZStride * 4, 1024);
     const size_t u16_bytes = align_up(size_t(M) * size_t(r) * 2 + 1024, 1024);
@@ -341,7 +342,7 @@ static int run_stream(const void* x, const void* Wq, const void* scales, const v
         p.A = static_cast<const __half*>(A);
         p.w_g = static_cast<const __half*>(ec->w_g);
         p.b_g = static_cast<const float*>(ec->b_g);
-        p.zbuf = reinterpret_cast<float*>(ws + L.zbuf);
+        p.zbuf = reinterpret_cast<float*>(ws + L.zfused);
         p.u_out = u32;
         p.gate_out = static_cast<float*>(ec->gate_out);
         p.ec_sync = counters + kEcPreCounter + 16;

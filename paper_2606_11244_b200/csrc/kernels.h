@@ -31,10 +31,10 @@ struct StreamParams {
     const __half* A;         // [r][K]
     const __half* w_g;       // [K] (scalar gate)
     const float* b_g;        // 1 or NULL
-    float* zbuf;             // [16][kZStride] fp32, zero between calls
-    float* u_out;            // [16][r] fp32 (same buffer as u)
+    float* zbuf;             // [2][16][kZStride] fp32, double-buffered by the parity of the epoch word
+    float* u_out;            // unused by the fused variant (u is formed in shared memory)
     float* gate_out;         // optional [M]
-    unsigned* ec_sync;       // [0] arrivals, [1] u-ready flag, [2] readers; zero between calls
+    unsigned* ec_sync;       // [0] epoch (bumped once per fused launch), [1], [2] arrival counters of buffer 0 / 1
 };
 int stream_stages(int MT, bool deep);
 int stream_smem_bytes(int MT, int stages);

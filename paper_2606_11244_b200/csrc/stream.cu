@@ -156,11 +156,15 @@ __device__ __forceinline__ void stream_task(uint32_t w_addr, uint32_t x_addr, ui
 
 // ---- fused EC (warp 9): S4-S6 of SURVEY.md 8(a) inside the weight-stream kernel ---------------------
 // Every CTA reduces one (16-row strip of [A; w_g]) x (K slice) piece of z = x [A; w_g]^T with mma.sync,
-// adds it to the global fp32 z with red.add and ARRIVES on a device-wide counter right away; nobody
-// waits there.  The last CTA to arrive applies the gate (z must be complete before
-// the gate), writes u = alpha * gamma (.) z, re-zeroes z and raises a flag; the other
-// CTAs only look at the flag in their epilogue, long after everybody has arrived (arrive early / wait
-// late).  All CTAs of the grid are co-resident (grid <= SMs x occupancy), so the wait cannot deadlock.
+// adds it to the global fp32 z with red.add and ARRIVES on a device-wide counter right away; nobody waits
+// there.  A CTA that finalises a panel looks at the counter only in its epilogue, long after everybody has
+// arrived (arrive early / wait late), then reads the complete z (z must be complete before the gate,
+// PAPER.md:199-211), applies the gate (PAPER.md:107-109 / BASELINE.json scalar gate) and forms
+// u = alpha * gamma (.) z in shared memory.  z and the counter are double-buffered by the parity of an epoch
+// word that the last arriver bumps: launch n uses buffer n & 1 and CTA 0 re-zeroes the other buffer for launch
+// n + 1 (its previous user, launch n - 1, is complete once griddepcontrol.wait returns), so nothing has to be
+// cleaned on the critical path.  All CTAs of the grid are co-resident (grid <= SMs x resident CTAs), so the
+// late wait cannot deadlock.
 __device__ __forceinline__ void ec_load16(const __half* row, int col, bool readonly, uint32_t (&lo)[4], uint32_t (&hi)[4]) {
     if (row) {
         uint4 a, b;
@@ -204,7 +208,7 @@ __device__ void ec_prefetch_factors(const StreamParams& p, int lane) {
 
 // Phase A (whole warp, after griddepcontrol.wait): this CTA's piece of z, red.add, arrive.  Returns true in
 // the last CTA to arrive.
-__device__ bool ec_reduce_and_arrive(const StreamParams& p, int lane) {
+__device__ void ec_reduce_and_arrive(const StreamParams& p, int lane, int* par_smem, uint64_t* e_ready) {
     const int g = lane >> 2, t = lane & 3;
     const bool scalar = (p.gate_kind == SPEAR_GATE_SCALAR_SIGMOID);
     const int rows_total = p.r + (scalar ? 1 : 0);
@@ -215,6 +219,11 @@ __device__ bool ec_reduce_and_arrive(const StreamParams& p, int lane) {
     const int n_tasks = strips * ksplit;
     const __half* px0 = g < p.M ? p.x + size_t(g) * p.K : nullptr;
     const __half* px1 = g + 8 < p.M ? p.x + size_t(g + 8) * p.K : nullptr;
+    // the epoch load is issued first and consumed after the first loads / mma (one L2 round trip, overlapped)
+    unsigned epoch;
+    asm volatile("ld.relaxed.gpu.global.u32 %0, [%1];" : "=r"(epoch) : "l"(p.ec_sync) : "memory");
+    bool announced = false;
+    float* zpar = nullptr;
     for (int task = blockIdx.x; task < n_tasks; task += G) {
         const int strip = task % strips, ks = task / strips;
         const int rho0 = strip * 16 + g, rho1 = rho0 + 8;
@@ -236,63 +245,34 @@ __device__ bool ec_reduce_and_arrive(const StreamParams& p, int lane) {
                 mma_m16n8k16(acc1, a0l[jj], a1l[jj], a0h[jj], a1h[jj], x1l[jj], x1h[jj]);
             }
         }
+        if (!announced) {
+            zpar = p.zbuf + (epoch & 1u) * (16 * kZStride);
+            if (lane == 0) { *par_smem = int(epoch & 1u); mbar_arrive(e_ready); }
+            announced = true;
+        }
         // C fragment: rows rho0 / rho1 of [A; w_g], tokens 2t, 2t+1 (acc0) and 8+2t, 9+2t (acc1)
 #pragma unroll
         for (int i = 0; i < 4; ++i) {
             const int rho = (i & 2) ? rho1 : rho0;
             const int tok = 2 * t + (i & 1);
             if (rho < rows_total) {
-                if (tok < p.M) atomicAdd(p.zbuf + tok * kZStride + rho, acc0[i]);
-                if (tok + 8 < p.M) atomicAdd(p.zbuf + (tok + 8) * kZStride + rho, acc1[i]);
+                if (tok < p.M) atomicAdd(zpar + tok * kZStride + rho, acc0[i]);
+                if (tok + 8 < p.M) atomicAdd(zpar + (tok + 8) * kZStride + rho, acc1[i]);
             }
         }
     }
+    const unsigned par = epoch & 1u;
+    if (!announced && lane == 0) { *par_smem = int(par); mbar_arrive(e_ready); }
+    if (blockIdx.x == 0) {
+        // prepare the other buffer for the next fused launch on this workspace
+        float* zo = p.zbuf + (par ^ 1u) * (16 * kZStride);
+        for (int i = lane; i < 16 * kZStride; i += 32) zo[i] = 0.f;
+        if (lane == 0) p.ec_sync[1 + (par ^ 1u)] = 0;
+    }
     __syncwarp();
-    unsigned old = 0;
-    if (lane == 0) old = arrive_acq_rel(p.ec_sync + 0);
-    old = __shfl_sync(0xffffffffu, old, 0);
-    return old == unsigned(G - 1);
-}
-
-// Phase B in the last arriver: gate (PAPER.md:109 / BASELINE.json scalar gate), u, clean-up, flag.
-__device__ void ec_gate_and_publish(const StreamParams& p, int lane, unsigned epoch) {
-    const bool scalar = (p.gate_kind == SPEAR_GATE_SCALAR_SIGMOID);
-    const int rows_total = p.r + (scalar ? 1 : 0);
-    {
-        __syncwarp();       // lane 0's acquire (arrive_acq_rel) covers the whole warp
-        const float bias = (scalar && p.b_g) ? *p.b_g : 0.f;
-        // lane m owns token m's gate; the z values are fetched 8 at a time so their L2 latencies overlap
-        float gam_own = 1.f;
-        if (scalar && lane < p.M) gam_own = 1.f / (1.f + expf(-(__ldcg(p.zbuf + lane * kZStride + p.r) + bias)));
-        if (scalar && p.gate_out && lane < p.M) p.gate_out[lane] = gam_own;
-        const int n = p.M * p.r;
-        for (int base = 0; base < n; base += 256) {
-            float zv[8];
-#pragma unroll
-            for (int q = 0; q < 8; ++q) {
-                const int idx = base + q * 32 + lane;
-                zv[q] = 0.f;
-                if (idx < n) { const int m = idx / p.r; zv[q] = __ldcg(p.zbuf + m * kZStride + (idx - m * p.r)); }
-            }
-#pragma unroll
-            for (int q = 0; q < 8; ++q) {
-                const int idx = base + q * 32 + lane;
-                const int m = min(idx / p.r, 15);
-                const float gam = __shfl_sync(0xffffffffu, gam_own, m);
-                if (idx < n) p.u_out[idx] = p.alpha * gam * zv[q];
-            }
-        }
-        __syncwarp();
-        for (int idx = lane; idx < p.M * rows_total; idx += 32) {
-            const int m = idx / rows_total, rho = idx - m * rows_total;
-            p.zbuf[m * kZStride + rho] = 0.f;
-        }
-        __syncwarp();
-        if (lane == 0) {
-            p.ec_sync[0] = 0;
-            // release at gpu scope, cumulative over the warp's u stores and z zeroing (ordered by __syncwarp)
-            asm volatile("st.release.gpu.global.u32 [%0], %1;" ::"l"(p.ec_sync + 1), "r"(epoch + 1u) : "memory");
-        }
+    if (lane == 0) {
+        const unsigned old = arrive_acq_rel(p.ec_sync + 1 + par);
+        if (old == unsigned(G - 1)) p.ec_sync[0] = epoch + 1u;      // the next launch takes the other buffer
     }
 }
 
@@ -389,17 +369,7 @@ stream_kernel(const __grid_constant__ CUtensorMap xmap, const StreamParams p) {
         if (!(p.fused && p.r > 0)) return;
         ec_prefetch_factors(p, lane);   // EC factors are parameters: warm L2 before the wait
         pdl_wait();
-        // The u-ready word is an epoch that the last arriver bumps and nobody resets: its value before this
-        // launch is read here (after the wait, before this CTA arrives, hence before anyone can bump it) and
-        // handed to the consumers through shared memory + an mbarrier.
-        unsigned epoch = 0;
-        if (lane == 0) {
-            epoch = *reinterpret_cast<volatile unsigned*>(p.ec_sync + 1);
-            flag[1] = int(epoch);
-            mbar_arrive(e_ready);
-        }
-        epoch = __shfl_sync(0xffffffffu, epoch, 0);
-        if (ec_reduce_and_arrive(p, lane)) ec_gate_and_publish(p, lane, epoch);
+        ec_reduce_and_arrive(p, lane, flag + 1, e_ready);
         return;
     }
 
@@ -513,22 +483,37 @@ stream_kernel(const __grid_constant__ CUtensorMap xmap, const StreamParams p) {
             const int n = pnl * 128 + row;
             if (p.r > 0 && !(p.debug & 4)) {
                 // S7: y += sum_j u[m][j] * B[n][j]   (u = alpha * gamma (.) z, fp32, from the pre-kernel or warp 9)
-                if (p.fused && !u_seen && !(p.debug & 2)) {
-                    if (ct == 0) {      // wait (late) for the last arriver's epoch bump; u is then visible
+                if (p.fused && !u_seen) {
+                    if (ct == 0 && !(p.debug & 2)) {   // wait (late) until every CTA has added its piece of z
                         mbar_wait(e_ready, 0);
-                        const unsigned e0 = unsigned(flag[1]);
+                        const unsigned* ctr = p.ec_sync + 1 + flag[1];
                         unsigned f;
                         do {
-                            asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(f) : "l"(p.ec_sync + 1) : "memory");
-                        } while (f == e0);
+                            asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(f) : "l"(ctr) : "memory");
+                        } while (f < gridDim.x);
                     }
                     u_seen = true;      // later panels of this CTA need not look again
                 }
-                // u (M x r fp32, <= 8 KiB) is staged once in the idle reduction buffer: every lane of a warp
-                // then reads the same word (broadcast) instead of paying an L2 round trip per term
+                // u (M x r fp32, <= 8 KiB) is staged in the idle reduction buffer: every lane of a warp then reads
+                // the same word (broadcast) instead of paying an L2 round trip per term
                 float* us = red;
-                named_bar_sync(2, 256);      // every thread has taken its sums out of red[]
-                for (int idx = ct; idx < p.M * p.r; idx += 256) us[idx] = __ldcg(p.u + idx);
+                named_bar_sync(2, 256);      // every thread has taken its sums out of red[]; the counter was seen
+                if (p.fused) {
+                    // S5 + S6 here: gamma from the complete z, u = alpha * gamma (.) z
+                    const bool scalar = (p.gate_kind == SPEAR_GATE_SCALAR_SIGMOID);
+                    const float* zc = p.zbuf + flag[1] * (16 * kZStride);
+                    const float bias = (scalar && p.b_g) ? __ldg(p.b_g) : 0.f;
+                    for (int idx = ct; idx < p.M * p.r; idx += 256) {
+                        const int m = idx / p.r, j = idx - m * p.r;
+                        const float zz = __ldcg(zc + m * kZStride + j);
+                        float gam = 1.f;
+                        if (scalar) gam = 1.f / (1.f + expf(-(__ldcg(zc + m * kZStride + p.r) + bias)));
+                        us[idx] = p.alpha * gam * zz;
+                        if (scalar && p.gate_out && pnl == 0 && j == 0) p.gate_out[m] = gam;
+                    }
+                } else {
+                    for (int idx = ct; idx < p.M * p.r; idx += 256) us[idx] = __ldcg(p.u + idx);
+                }
                 named_bar_sync(2, 256);
                 const uint4* Brow = reinterpret_cast<const uint4*>(p.B + size_t(n) * p.r);
 #pragma unroll 4
