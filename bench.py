@@ -288,7 +288,9 @@ def run_cuda(args, rank, world):
         "roofline": {"bound": "hbm", "kernel": "spear::stream_kernel (plain W4 step: one launch per layer call, "
                                                 "calls overlapped on the batch lanes)",
                      "achieved": round(ach, 1), "peak": peak, "unit": "GB/s", "frac": round(ach / peak, 4),
-                     "peak_source": peak_src, "traffic": None,
+                     "peak_source": peak_src, "traffic": 17400320,
+                     "traffic_note": "dram__bytes_read+write of ONE launch (gate_up 2048->16384, M=8, r=0; algorithmic "
+                                     "17.35 MB) from profiles/r01_ncu_summary.md; the step is 12 such launches of 4 shapes",
                      "avg_launch_us": round(per_w4 * 1e3 / ncalls, 3), "launches_per_step": ncalls},
         "no_ec": {"value": round(world * b_w4 / (per_w4 * 1e-3) / 1e9, 1), "ms_per_step": round(per_w4, 6)},
         "ec_overhead_time_frac": round(per / per_w4 - 1.0, 4),
@@ -351,7 +353,7 @@ def prefill_numbers(sp, device):
     tf0 = algorithmic_flops(M, N, K, group, 0) / (res[0] * 1e-3) / 1e12
     tf1 = algorithmic_flops(M, N, K, group, 64, "scalar") / (res[64] * 1e-3) / 1e12
     return {"workload": "BASELINE.json configs[3]: M=4096, K=8192, N=28672, group=128, one layer call, median of 7",
-            "kernel": "spear::tc_kernel<256,1> (tcgen05, TMEM accumulators, EC folded in as extra k-blocks)",
+            "kernel": "spear::tc_kernel<256,2> (tcgen05, TMEM accumulators, EC folded in as extra k-blocks)",
             "tflops_no_ec": round(tf0, 1), "ms_no_ec": round(res[0], 4),
             "tflops_ec_r64": round(tf1, 1), "ms_ec_r64": round(res[64], 4),
             "ec_overhead_time_frac": round(res[64] / res[0] - 1.0, 4),
