@@ -14,12 +14,12 @@
 //     the same number of bytes whatever the shape.  Large units keep the number of asynchronous-copy
 //     instructions per byte low: one thread issues them, and ~200 cycles each is what bounds a ring of
 //     small copies;
-//   * warp 0, one lane: cp.async.bulk of weights and scales into a kStages-deep ring guarded by full/empty
-//     mbarriers.  It never executes griddepcontrol.wait (weights do not depend on the previous kernel):
-//     under programmatic dependent launch the ring of layer i+1 fills while layer i drains;
-//   * warp 9 (service warp): after griddepcontrol.wait, one 3-D TMA tensor copy per unit brings the x
-//     tile (8*MT tokens x 4 k-tiles x 64 columns, 128-byte swizzle, zero-filled beyond M and K); in the
-//     fused variant the whole warp also reduces this CTA's share of z = x [A; w_g]^T (see below);
+//   * warp 0, one lane: cp.async.bulk of weights and scales into a ring (depth = launch parameter) guarded by
+//     full/empty mbarriers.  The first ring-full is issued BEFORE griddepcontrol.wait (weights do not depend on
+//     the previous kernel): under programmatic dependent launch the ring of layer i+1 fills while layer i
+//     drains.  After the wait the same lane adds one 3-D TMA tensor copy per unit for the x tile (8*MT tokens x
+//     4 k-tiles x 64 columns, 128-byte swizzle, zero-filled beyond M and K);
+//   * warp 9 (fused variant only): reduces this CTA's share of z = x [A; w_g]^T and arrives (see below);
 //   * 8 consumer warps, all on the same unit: warp (h, kq) takes strips 4h..4h+3 (64 rows) x k-tile kq
 //     (64 columns): 4 LDS.128 of int4, lop3/sub dequantisation in registers, mma.sync.m16n8k16 with the
 //     tokens as the n=8 operand (fp32 accumulate), group scale applied to the fp32 accumulator;

@@ -14,16 +14,22 @@
 // (lane = output channel, column = token), two accumulators in flight so that the epilogue of tile i
 // overlaps the main loop of tile i+1.
 //
-// Warp roles (704 threads, one CTA per SM, persistent over a static tile schedule):
-//   warp 0      producer: cp.async.bulk of the packed int4 (4 KiB per (panel, 64-k tile)) + 256 B of
-//               scales into a small ring; TMA tensor loads of the x tile (BT x 64 fp16, SWIZZLE_128B).
-//               int4 copies never wait for the previous kernel; x / u16 loads come after griddepcontrol.wait.
+// Warp roles (736 threads for BT = 256, 992 for narrower token tiles; one CTA per SM, persistent over a static
+// schedule of work items = output tile x split-K share):
+//   warp 0      x producer: after griddepcontrol.wait, TMA tensor loads of the x tile (BT x 64 fp16,
+//               SWIZZLE_128B; for the EC k-blocks the u16 tile), multicast to the CTAs of a cluster that share
+//               the token tile.
+//   last warp   int4 producer: cp.async.bulk of the packed int4 (4 KiB per (panel, 64-k tile)) + 256 B of
+//               scales into a small ring; never waits for the previous kernel.  (One thread issuing both kinds
+//               of copies was the bottleneck of the first version: 39 % -> 72 % tensor-pipe activity.)
 //   warp 1      allocates TMEM; one elected lane issues tcgen05.mma (4 x K=16 per k-block) and commits
 //               to the mbarriers that free the operand stages / publish the accumulator.
-//   warps 2-5   epilogue: tcgen05.ld the accumulator, one RN-even cast to fp16, store y.
-//   warps 6-21  dequantisation (two groups of 8 warps taking k-blocks alternately): LDS.128 of int4 -> lop3 / sub / fma (exact q - 8) -> mul by the fp16
-//               group scale (one rounding: the same RN_fp16((q-8)*s) the dequant test hook exports)
-//               -> STS.128 into the K-major 128-byte-swizzled A-operand stage, fence.proxy.async, arrive.
+//   warps 2-5   epilogue: tcgen05.ld the accumulator, one RN-even cast to fp16, store y; with split-K: park
+//               the fp32 partial, last arriver of the tile sums the partials in split order and stores.
+//   warps 6-... dequantisation, 2 (BT = 256) or 3 groups of 8 warps taking k-blocks round-robin: LDS.128 of
+//               int4 -> lop3 / sub / fma (exact q - 8) -> mul by the fp16 group scale (one rounding: the same
+//               RN_fp16((q-8)*s) the dequant test hook exports) -> STS.128 into the K-major 128-byte-swizzled
+//               A-operand stage, fence.proxy.async, arrive.  For an EC k-block one lane TMA-loads the B slab.
 #include <algorithm>
 
 #include "common.cuh"
