@@ -88,6 +88,7 @@ struct TcProblem {
     int grid_override;
     int cluster_override;    // 0 = heuristic, else 1 / 2 / 4 CTAs sharing x tiles by TMA multicast
     int ksplit_override;     // 0 = heuristic, else the split-K factor
+    int bt_override;         // 0 = heuristic, else the token-tile width (32 / 64 need M <= width)
     void* partial;           // fp32 split-K slots (workspace)
     size_t partial_bytes;
     unsigned* counters;      // zero between calls

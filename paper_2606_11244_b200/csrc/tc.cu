@@ -108,8 +108,8 @@ struct TcParams {
     __half* y;               // [M][N]
     int M, N, K, r;
     int G, group;            // K / group, group
-    int kb_w;                // K / 64 weight k-blocks
-    int kb_ec;               // ceil(r / 64) EC k-blocks
+    int kb_w;                // weight k-blocks (= pipeline stages of kKT x 64 columns)
+    int kb_ec;               // EC k-blocks: ceil(r / (kKT x 64))
     int n_pp, n_mt;          // N / (128 * CS) panel groups (CS = cluster size), ceil(M / BT)
     int mt_group;            // token tiles per raster group (keeps the x slice L2-resident)
     int n_tiles;             // n_pp * n_mt output tiles; each is taken by one cluster (CTA rank c -> panel pp * CS + c)
@@ -139,16 +139,19 @@ __device__ __forceinline__ TcWork get_work(const TcParams& p, int w) {
 template <int BT>
 struct TcCfg {
     // the x ring hides an L2 round trip per stage (deep); the A ring only the local dequantisation (shallow)
-    static constexpr int kXStages = BT == 256 ? 5 : (BT == 128 ? 6 : 10);
+    // k-tiles (64 columns) per pipeline stage: a stage costs one barrier round trip (~0.45 us measured) whatever
+    // its MMA time, so narrow token tiles (short MMAs) take 128 columns per stage
+    static constexpr int kKT = BT == 256 ? 1 : 2;
+    static constexpr int kXStages = BT == 256 ? 5 : (BT == 128 ? 3 : (BT == 64 ? 6 : 8));
     // dequantisation warp groups of 8 taking k-blocks round-robin: a k-block costs one barrier round trip
     // (~0.7 us) whatever its MMA time, so narrow token tiles (short MMAs) get three groups and a deeper A ring
     static constexpr int kDequantGroups = BT == 256 ? 2 : 3;
     static constexpr int kThreads = (7 + 8 * kDequantGroups) * 32;   // + x producer, MMA, 4 epilogue, int4 producer
-    static constexpr int kAStages = BT == 256 ? 3 : 5;
-    static constexpr int kW4Stages = BT == 256 ? 4 : 8;
-    static constexpr int kABytes = 128 * 128;            // 128 channels x 64 k fp16
-    static constexpr int kXBytes = BT * 128;             // BT tokens x 64 k fp16
-    static constexpr int kW4Bytes = 4096 + 256;          // codes + scales of one (panel, 64-k tile)
+    static constexpr int kAStages = 3;
+    static constexpr int kW4Stages = 4;
+    static constexpr int kABytes = kKT * 128 * 128;      // kKT sub-tiles of 128 channels x 64 k fp16
+    static constexpr int kXBytes = kKT * BT * 128;       // kKT sub-tiles of BT tokens x 64 k fp16
+    static constexpr int kW4Bytes = kKT * 4096 + 256;    // codes of kKT (panel, 64-k tile)s + one scale block
     static constexpr int kTmemCols = 2 * BT < 32 ? 32 : 2 * BT;
     static constexpr size_t kSmemBytes = 1024 + size_t(kAStages) * kABytes + size_t(kXStages) * kXBytes + size_t(kW4Stages) * kW4Bytes + 512;
     static_assert(kSmemBytes <= 232448, "exceeds the 227 KiB opt-in shared memory of sm_100");
@@ -170,7 +173,7 @@ __global__ void __launch_bounds__(TcCfg<BT>::kThreads, 1)
 tc_kernel(const __grid_constant__ CUtensorMap xmap, const __grid_constant__ CUtensorMap umap,
           const __grid_constant__ CUtensorMap bmap, const TcParams p) {
     using Cfg = TcCfg<BT>;
-    constexpr int SX = Cfg::kXStages, SA = Cfg::kAStages, S4 = Cfg::kW4Stages;
+    constexpr int SX = Cfg::kXStages, SA = Cfg::kAStages, S4 = Cfg::kW4Stages, KT = Cfg::kKT;
     extern __shared__ uint8_t smem_raw[];
     uint8_t* base = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
     uint8_t* a_ring = base;                                   // S x 16 KiB, 1024-aligned
@@ -224,11 +227,14 @@ tc_kernel(const __grid_constant__ CUtensorMap xmap, const __grid_constant__ CUte
                     const int s = it % SX;
                     mbar_wait(&x_empty[s], ((it / SX) & 1) ^ 1);
                     mbar_arrive_expect_tx(&x_full[s], Cfg::kXBytes);
-                    uint8_t* dst = x_ring + size_t(s) * Cfg::kXBytes + size_t(cta_rank) * kXRows * 128;
                     const CUtensorMap* map = j < t.nw ? &xmap : &umap;
-                    const int c0 = (j < t.nw ? t.kb0 + j : j - t.nw) * 64;
-                    if (CS > 1) tma_load_2d_mc(dst, map, c0, c1, &x_full[s], kMask, pol_x);
-                    else tma_load_2d(dst, map, c0, c1, &x_full[s], pol_x);
+#pragma unroll
+                    for (int kt = 0; kt < KT; ++kt) {
+                        uint8_t* dst = x_ring + size_t(s) * Cfg::kXBytes + size_t(kt) * (BT * 128) + size_t(cta_rank) * kXRows * 128;
+                        const int c0 = ((j < t.nw ? t.kb0 + j : j - t.nw) * KT + kt) * 64;
+                        if (CS > 1) tma_load_2d_mc(dst, map, c0, c1, &x_full[s], kMask, pol_x);
+                        else tma_load_2d(dst, map, c0, c1, &x_full[s], pol_x);
+                    }
                 }
             }
         }
@@ -241,15 +247,15 @@ tc_kernel(const __grid_constant__ CUtensorMap xmap, const __grid_constant__ CUte
             for (int w = work0; w < p.n_work; w += work_stride) {
                 const TcWork t = get_work(p, w);
                 const int panel = t.panel * CS + cta_rank;
-                const uint8_t* wsrc = p.wq + size_t(panel) * p.kb_w * 4096;
+                const uint8_t* wsrc = p.wq + size_t(panel) * p.kb_w * (KT * 4096);
                 const uint8_t* ssrc = p.scales + size_t(panel) * p.G * 256;
                 for (int kb = t.kb0; kb < t.kb0 + t.nw; ++kb, ++w_it) {
                     const int s4 = w_it % S4;
                     mbar_wait(&w4_empty[s4], ((w_it / S4) & 1) ^ 1);
                     mbar_arrive_expect_tx(&w4_full[s4], Cfg::kW4Bytes);
                     uint8_t* dst = w4_ring + size_t(s4) * Cfg::kW4Bytes;
-                    bulk_g2s(dst, wsrc + size_t(kb) * 4096, 4096, &w4_full[s4], pol_w);
-                    bulk_g2s(dst + 4096, ssrc + size_t((kb * 64) / p.group) * 256, 256, &w4_full[s4], pol_s);
+                    bulk_g2s(dst, wsrc + size_t(kb) * (KT * 4096), KT * 4096, &w4_full[s4], pol_w);
+                    bulk_g2s(dst + KT * 4096, ssrc + size_t((kb * 64 * KT) / p.group) * 256, 256, &w4_full[s4], pol_s);
                 }
             }
         }
@@ -272,8 +278,11 @@ tc_kernel(const __grid_constant__ CUtensorMap xmap, const __grid_constant__ CUte
                     const uint64_t a_desc = umma_desc_sw128(smem_u32(a_ring + size_t(sa) * Cfg::kABytes));
                     const uint64_t b_desc = umma_desc_sw128(smem_u32(x_ring + size_t(s) * Cfg::kXBytes));
 #pragma unroll
-                    for (int k = 0; k < 4; ++k)   // K = 16 per instruction: +32 bytes inside the swizzle atom
-                        umma_f16(d_tmem, a_desc + uint64_t(k * 2), b_desc + uint64_t(k * 2), Cfg::kIdesc, (kb | k) != 0);
+                    for (int kt = 0; kt < KT; ++kt)
+#pragma unroll
+                        for (int k = 0; k < 4; ++k)   // K = 16 per instruction: +32 bytes inside the swizzle atom
+                            umma_f16(d_tmem, a_desc + uint64_t(kt * (16384 >> 4) + k * 2),
+                                     b_desc + uint64_t(kt * ((BT * 128) >> 4) + k * 2), Cfg::kIdesc, (kb | kt | k) != 0);
                     if (CS > 1) umma_commit_mc(&x_empty[s], kMask);
                     else umma_commit(&x_empty[s]);
                     umma_commit(&a_empty[sa]);
@@ -379,26 +388,29 @@ tc_kernel(const __grid_constant__ CUtensorMap xmap, const __grid_constant__ CUte
                     mbar_wait(&w4_full[s4], (w_it / S4) & 1);
                     ++w_it;
                     const uint8_t* src = w4_ring + size_t(s4) * Cfg::kW4Bytes;
-                    const uint4 w = *reinterpret_cast<const uint4*>(src + (strip * 32 + lane) * 16);
-                    const uint32_t scw = *reinterpret_cast<const uint32_t*>(src + 4096 + (strip * 16 + 2 * g) * 2);
+                    const uint32_t scw = *reinterpret_cast<const uint32_t*>(src + KT * 4096 + (strip * 16 + 2 * g) * 2);
                     const uint32_t s_lo = __byte_perm(scw, scw, 0x1010), s_hi = __byte_perm(scw, scw, 0x3232);
-                    uint32_t c0[4], c1[4], c2[4], c3[4];
-                    dequant_word(w.x, c0);      // row g,     columns 16t + 0..7   -> 16-byte chunk 2t
-                    dequant_word(w.y, c1);      // row g,     columns 16t + 8..15  -> chunk 2t + 1
-                    dequant_word(w.z, c2);      // row g + 8, columns 16t + 0..7
-                    dequant_word(w.w, c3);      // row g + 8, columns 16t + 8..15
 #pragma unroll
-                    for (int i = 0; i < 4; ++i) {
-                        c0[i] = hmul2_u32(c0[i], s_lo); c1[i] = hmul2_u32(c1[i], s_lo);
-                        c2[i] = hmul2_u32(c2[i], s_hi); c3[i] = hmul2_u32(c3[i], s_hi);
+                    for (int kt = 0; kt < KT; ++kt) {
+                        const uint4 w = *reinterpret_cast<const uint4*>(src + kt * 4096 + (strip * 32 + lane) * 16);
+                        uint32_t c0[4], c1[4], c2[4], c3[4];
+                        dequant_word(w.x, c0);      // row g,     columns 16t + 0..7   -> 16-byte chunk 2t
+                        dequant_word(w.y, c1);      // row g,     columns 16t + 8..15  -> chunk 2t + 1
+                        dequant_word(w.z, c2);      // row g + 8, columns 16t + 0..7
+                        dequant_word(w.w, c3);      // row g + 8, columns 16t + 8..15
+#pragma unroll
+                        for (int i = 0; i < 4; ++i) {
+                            c0[i] = hmul2_u32(c0[i], s_lo); c1[i] = hmul2_u32(c1[i], s_lo);
+                            c2[i] = hmul2_u32(c2[i], s_hi); c3[i] = hmul2_u32(c3[i], s_hi);
+                        }
+                        // K-major SWIZZLE_128B: row n at n * 128, 16-byte chunk c at position c ^ (n & 7); (n & 7) == g
+                        uint8_t* r0 = a_stage + kt * 16384 + (strip * 16 + g) * 128;
+                        uint8_t* r1 = r0 + 8 * 128;
+                        *reinterpret_cast<uint4*>(r0 + (((2 * t) ^ g) << 4)) = make_uint4(c0[0], c0[1], c0[2], c0[3]);
+                        *reinterpret_cast<uint4*>(r0 + (((2 * t + 1) ^ g) << 4)) = make_uint4(c1[0], c1[1], c1[2], c1[3]);
+                        *reinterpret_cast<uint4*>(r1 + (((2 * t) ^ g) << 4)) = make_uint4(c2[0], c2[1], c2[2], c2[3]);
+                        *reinterpret_cast<uint4*>(r1 + (((2 * t + 1) ^ g) << 4)) = make_uint4(c3[0], c3[1], c3[2], c3[3]);
                     }
-                    // K-major SWIZZLE_128B: row n at n * 128, 16-byte chunk c at position c ^ (n & 7); (n & 7) == g
-                    uint8_t* r0 = a_stage + (strip * 16 + g) * 128;
-                    uint8_t* r1 = r0 + 8 * 128;
-                    *reinterpret_cast<uint4*>(r0 + (((2 * t) ^ g) << 4)) = make_uint4(c0[0], c0[1], c0[2], c0[3]);
-                    *reinterpret_cast<uint4*>(r0 + (((2 * t + 1) ^ g) << 4)) = make_uint4(c1[0], c1[1], c1[2], c1[3]);
-                    *reinterpret_cast<uint4*>(r1 + (((2 * t) ^ g) << 4)) = make_uint4(c2[0], c2[1], c2[2], c2[3]);
-                    *reinterpret_cast<uint4*>(r1 + (((2 * t + 1) ^ g) << 4)) = make_uint4(c3[0], c3[1], c3[2], c3[3]);
                     fence_proxy_async_smem();   // generic-proxy writes -> visible to the tensor core's async proxy
                     __syncwarp();
                     if (lane == 0) { mbar_arrive(&w4_empty[s4]); mbar_arrive(&a_full[s]); }
@@ -407,7 +419,10 @@ tc_kernel(const __grid_constant__ CUtensorMap xmap, const __grid_constant__ CUte
                     if (lane == 0) {
                         if (strip == 0) {
                             mbar_arrive_expect_tx(&a_full[s], Cfg::kABytes);
-                            tma_load_2d(a_stage, &bmap, (kb - tw.nw) * 64, panel * 128, &a_full[s], policy_evict_last());
+#pragma unroll
+                            for (int kt = 0; kt < KT; ++kt)
+                                tma_load_2d(a_stage + kt * 16384, &bmap, ((kb - tw.nw) * KT + kt) * 64, panel * 128,
+                                            &a_full[s], policy_evict_last());
                         } else {
                             mbar_arrive(&a_full[s]);
                         }
@@ -473,8 +488,13 @@ static int launch_tc(const CUtensorMap& xmap, const CUtensorMap& umap, const CUt
 }
 
 int run_tc(const TcProblem& t, cudaStream_t st) {
-    const int BT = t.M <= 32 ? 32 : (t.M <= 64 ? 64 : (t.M <= 128 ? 128 : 256));
+    int BT = t.M <= 32 ? 32 : (t.M <= 64 ? 64 : (t.M <= 128 ? 128 : 256));
     const int n_panels = t.N / 128;
+    // few, wide tiles leave SMs idle and pay one barrier round trip per 64 columns: with too few 256-token tiles
+    // to fill the machine, 128-token tiles (two k-tiles per stage, twice the CTAs) are faster (measured at M = 256)
+    if (BT == 256 && t.M <= 512 && n_panels * ((t.M + 255) / 256) < device_info().num_sms) BT = 128;
+    if (t.bt_override == 32 || t.bt_override == 64 || t.bt_override == 128 || t.bt_override == 256)
+        if (t.bt_override >= 32 && (t.bt_override >= t.M || t.bt_override >= 128)) BT = t.bt_override;
     const int n_mt = (t.M + BT - 1) / BT;
     // clusters share x tiles by TMA multicast; worth it once there are more tiles than SMs (L2 -> SM bound)
     int CS = 1;
@@ -486,8 +506,9 @@ int run_tc(const TcProblem& t, cudaStream_t st) {
     p.y = static_cast<__half*>(t.y);
     p.M = t.M; p.N = t.N; p.K = t.K; p.r = t.r;
     p.group = t.group; p.G = t.K / t.group;
-    p.kb_w = t.K / 64;
-    p.kb_ec = (t.r + 63) / 64;
+    const int KT = BT == 256 ? 1 : 2;        // TcCfg<BT>::kKT: 64-column k-tiles per pipeline stage
+    p.kb_w = t.K / (64 * KT);               // from here on a "k-block" is one stage
+    p.kb_ec = (t.r + 64 * KT - 1) / (64 * KT);
     p.n_pp = n_panels / CS;
     p.n_mt = n_mt;
     // raster: token tiles in groups whose x slice (mt_group * BT * K * 2 bytes) stays L2-resident
@@ -497,7 +518,7 @@ int run_tc(const TcProblem& t, cudaStream_t st) {
     // split-K when there are fewer output tiles than SMs (mid-M on small layers): work items = tiles x ksplit
     int ks = 1;
     if (CS == 1 && p.n_tiles < device_info().num_sms) {
-        ks = std::min(std::min(device_info().num_sms / p.n_tiles, std::max(1, p.kb_w / 32)), 16);   // measured: a split must keep >= 32 k-blocks to pay for its reduction
+        ks = std::min(std::min(device_info().num_sms / p.n_tiles, std::max(1, p.kb_w * KT / 32)), 16);   // measured: a split must keep >= 32 k-tiles to pay for its reduction
         while (ks > 1 && size_t(p.n_tiles) * ks * BT * 128 * 4 > t.partial_bytes) --ks;
         if (p.n_tiles > t.max_counters || !t.partial || !t.counters) ks = 1;
     }
