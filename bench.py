@@ -117,6 +117,22 @@ class ClockSampler:
                 "reasons": sorted(reasons), "samples_under_load": len(sm)}
 
 
+def max_over_ranks(ms, world, device):
+    """Replicas only: the job's step time is the slowest rank's device time."""
+    if world <= 1:
+        return ms
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor([ms], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def aggregate_value(bytes_per_rank_step, ms_per_step, world):
+    """Whole-job throughput in GB/s: every rank moves the same algorithmic bytes per step (weak scaling)."""
+    return world * bytes_per_rank_step / (ms_per_step * 1e-3) / 1e9
+
+
 # ------------------------------------------------------------------------------------------------
 # CUDA arm
 # ------------------------------------------------------------------------------------------------
@@ -226,12 +242,7 @@ def run_cuda(args, rank, world):
             torch.cuda.synchronize()
             if world > 1:
                 dist.barrier()
-        ms = e0.elapsed_time(e1)
-        if world > 1:
-            t = torch.tensor([ms], device=device)
-            dist.all_reduce(t, op=dist.ReduceOp.MAX)
-            ms = float(t.item())
-        return ms
+        return max_over_ranks(e0.elapsed_time(e1), world, device)
 
     sampler = ClockSampler(local)
     if rank == 0:
@@ -267,7 +278,7 @@ def run_cuda(args, rank, world):
     per = ms / args.steps
     per_w4 = ms_w4 / args.steps
     per_e2e = ms_e2e / e2e_steps
-    value = world * b_ec / (per * 1e-3) / 1e9
+    value = aggregate_value(b_ec, per, world)
     peak, peak_src = load_peaks()
     ncalls = sum(len(v) for v in shapes.values())
     ach = b_w4 / (per_w4 * 1e-3) / 1e9

@@ -74,3 +74,35 @@ def test_product_does_not_import_oracle():
                 assert "spear_oracle" not in txt and "libspear_oracle" not in txt, f
     osrc = open(os.path.join(ROOT, "oracle", "spear_oracle.c")).read() + open(os.path.join(ROOT, "oracle", "__init__.py")).read()
     assert "paper_2606_11244_b200" not in osrc.replace("(paper_2606_11244_b200)", "")
+
+
+def test_plan_table_file_roundtrip_and_heuristics_without_gpu(tmp_path):
+    """Host logic of S9 that needs no device: the plan file format, and the heuristic AUTO falls back on."""
+    import ctypes
+    L = ctypes.CDLL(os.path.join(ROOT, "paper_2606_11244_b200", "libspear.so"))
+    L.spear_plan_query.argtypes = [ctypes.c_int] * 6 + [ctypes.POINTER(ctypes.c_int)]
+    L.spear_plan_load.argtypes = [ctypes.c_char_p]
+    L.spear_plan_save.argtypes = [ctypes.c_char_p]
+    v = ctypes.c_int()
+
+    def query(M, N, K, r, group, gate):
+        assert L.spear_plan_query(M, N, K, r, group, gate, ctypes.byref(v)) == 0
+        return v.value
+    # heuristics: decode kernel up to 16 tokens (fused unless the MLP gate), tcgen05 kernel above
+    assert query(4, 2048, 2048, 16, 128, 0) == 1
+    assert query(4, 2048, 2048, 16, 128, 1) == 2
+    assert query(4, 2048, 2048, 0, 128, 0) == 2
+    assert query(64, 2048, 2048, 32, 128, 0) == 3
+    # a hand-written table overrides them and survives save -> load
+    src = tmp_path / "plan.txt"
+    src.write_text("# spear plan v1\n4 2048 2048 16 128 0 2 17.2 16.5 26.4 32.2 -1\n64 2048 2048 32 128 0 4 -1 -1 30.0 28.0 -1\n")
+    assert L.spear_plan_load(str(src).encode()) == 0
+    assert query(4, 2048, 2048, 16, 128, 0) == 2
+    assert query(64, 2048, 2048, 32, 128, 0) == 4
+    out = tmp_path / "saved.txt"
+    assert L.spear_plan_save(str(out).encode()) == 0
+    txt = out.read_text()
+    assert "4 2048 2048 16 128 0 2" in txt and "64 2048 2048 32 128 0 4" in txt
+    bad = tmp_path / "bad.txt"
+    bad.write_text("1 2 3\n")
+    assert L.spear_plan_load(str(bad).encode()) == -1
