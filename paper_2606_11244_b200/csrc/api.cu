@@ -201,6 +201,7 @@ struct Tunables {
     int tc_cluster = 0;           // 0 = heuristic, else 1 / 2 / 4
     int tc_ksplit = 0;            // 0 = heuristic, else the tcgen05 kernel's split-K factor
     int tc_bt = 0;                // 0 = heuristic, else the tcgen05 kernel's token-tile width
+    int tc_xslice_mb = 0;         // 0 = default (16), MiB of x per raster group
     int batch_lanes = 4;          // concurrent lanes of spear_w4_ec_gemm_batch (1..4)
     int stream_deep = -1;         // -1 = heuristic, 0 / 1 = force the shallow / deep decode ring
     int stream_debug = 0;         // measurement hook, see StreamParams::debug
@@ -387,6 +388,7 @@ static int run_tc_fused(const void* x, const void* Wq, const void* scales, const
     t.cluster_override = g_tune.tc_cluster;
     t.ksplit_override = g_tune.tc_ksplit;
     t.bt_override = g_tune.tc_bt;
+    t.xslice_mb = g_tune.tc_xslice_mb;
     t.partial = ws + L.partial;
     t.partial_bytes = size_t(kMaxStreamGrid) * 2 * 16 * 128 * 4;
     t.counters = reinterpret_cast<unsigned*>(ws + L.counters) + 1024;
@@ -458,6 +460,7 @@ extern "C" int spear_tune(const char* key, int value) {
     else if (!strcmp(key, "tc_cluster")) g_tune.tc_cluster = value;
     else if (!strcmp(key, "tc_ksplit")) g_tune.tc_ksplit = value;
     else if (!strcmp(key, "tc_bt")) g_tune.tc_bt = value;
+    else if (!strcmp(key, "tc_xslice_mb")) g_tune.tc_xslice_mb = value;
     else if (!strcmp(key, "batch_lanes")) g_tune.batch_lanes = value;
     else if (!strcmp(key, "stream_deep")) g_tune.stream_deep = value;
     else if (!strcmp(key, "stream_debug")) g_tune.stream_debug = value;

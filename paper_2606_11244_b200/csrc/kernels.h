@@ -89,6 +89,7 @@ struct TcProblem {
     int cluster_override;    // 0 = heuristic, else 1 / 2 / 4 CTAs sharing x tiles by TMA multicast
     int ksplit_override;     // 0 = heuristic, else the split-K factor
     int bt_override;         // 0 = heuristic, else the token-tile width (32 / 64 need M <= width)
+    int xslice_mb;           // 0 = default: MiB of x a raster group of token tiles may cover (L2 residency)
     void* partial;           // fp32 split-K slots (workspace)
     size_t partial_bytes;
     unsigned* counters;      // zero between calls

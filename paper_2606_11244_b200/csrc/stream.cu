@@ -488,8 +488,19 @@ stream_kernel(const __grid_constant__ CUtensorMap xmap, const StreamParams p) {
                         mbar_wait(e_ready, 0);
                         const unsigned* ctr = p.ec_sync + 1 + flag[1];
                         unsigned f;
+                        unsigned long long t0 = 0;
+                        unsigned spins = 0;
                         do {
                             asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(f) : "l"(ctr) : "memory");
+                            // Watchdog: every CTA arrives within microseconds of its start, so seconds of waiting
+                            // can only mean that the grid is not co-resident (see api.cu); fail loudly (sticky launch
+                            // error) instead of hanging the device.
+                            if (f < gridDim.x && (++spins & 0x3ffu) == 0) {
+                                unsigned long long now;
+                                asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(now));
+                                if (t0 == 0) t0 = now;
+                                else if (now - t0 > 4000000000ull) __trap();
+                            }
                         } while (f < gridDim.x);
                     }
                     u_seen = true;      // later panels of this CTA need not look again

@@ -511,9 +511,9 @@ int run_tc(const TcProblem& t, cudaStream_t st) {
     p.kb_ec = (t.r + 64 * KT - 1) / (64 * KT);
     p.n_pp = n_panels / CS;
     p.n_mt = n_mt;
-    // raster: token tiles in groups whose x slice (mt_group * BT * K * 2 bytes) stays L2-resident
+    // raster: token tiles in groups whose x slice (mt_group * BT * K * 2 bytes, <= 16 MiB) stays L2-resident next to the weights in flight
     const size_t slice = size_t(BT) * t.K * 2;
-    p.mt_group = int(std::max<size_t>(1, std::min<size_t>(size_t(p.n_mt), (size_t(48) << 20) / slice)));
+    p.mt_group = int(std::max<size_t>(1, std::min<size_t>(size_t(p.n_mt), (size_t(t.xslice_mb > 0 ? t.xslice_mb : 16) << 20) / slice)));   // measured: 8-16 MiB > 32-96 MiB
     p.n_tiles = p.n_pp * p.n_mt;
     // split-K when there are fewer output tiles than SMs (mid-M on small layers): work items = tiles x ksplit
     int ks = 1;
