@@ -130,6 +130,16 @@ typedef struct {
 } spear_call;
 int spear_w4_ec_gemm_batch(const spear_call* calls, int n_calls, void* stream);
 
+/* The same batch with HOST activations: for call i, io[i].x_host [M][K] fp16 is copied to calls[i].x (the device
+ * staging buffer the caller provides), the layer runs, and calls[i].y is copied back to io[i].y_host [M][N] --
+ * all on that call's lane, inside the fork / join (preferably pinned host memory; the end-to-end path bench.py
+ * times).  The host buffers are valid once `stream` has been synchronised. */
+typedef struct {
+    const void* x_host;
+    void* y_host;
+} spear_host_io;
+int spear_w4_ec_gemm_batch_hostio(const spear_call* calls, const spear_host_io* io, int n_calls, void* stream);
+
 /* Same layer with HOST activations: x_host[M][K] and y_host[M][N] are (preferably pinned) host
  * buffers; x is copied to x_dev, the layer runs, y_dev is copied back, all on `stream` (the end-
  * to-end path bench.py times).  Weights and EC parameters stay device-resident. */

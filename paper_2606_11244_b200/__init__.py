@@ -23,7 +23,7 @@ VARIANT_NAMES = ["auto", "stream_fused", "stream_split", "tc_fused", "tc_split"]
 
 EXPORTS = [
     "spear_pack_w4_sizes", "spear_pack_w4", "spear_unpack_w4", "spear_dequant_w4",
-    "spear_w4_ec_gemm", "spear_w4_ec_gemm_ex", "spear_w4_ec_gemm_hostio", "spear_w4_ec_gemm_batch",
+    "spear_w4_ec_gemm", "spear_w4_ec_gemm_ex", "spear_w4_ec_gemm_hostio", "spear_w4_ec_gemm_batch", "spear_w4_ec_gemm_batch_hostio",
     "spear_workspace_bytes", "spear_init", "spear_plan", "spear_plan_save", "spear_plan_load",
     "spear_plan_query", "spear_tune", "spear_last_error", "spear_launch_count",
 ]
@@ -54,6 +54,11 @@ class Call(ctypes.Structure):
     ]
 
 
+class HostIO(ctypes.Structure):
+    """struct spear_host_io of include/spear.h."""
+    _fields_ = [("x_host", ctypes.c_void_p), ("y_host", ctypes.c_void_p)]
+
+
 _lib = None
 
 
@@ -73,6 +78,7 @@ def lib():
         L.spear_w4_ec_gemm.argtypes = [vp] * 8 + [ci] * 5 + [vp]
         L.spear_w4_ec_gemm_ex.argtypes = [vp] * 5 + [ctypes.POINTER(EcDesc), vp] + [ci] * 5 + [vp]
         L.spear_w4_ec_gemm_batch.argtypes = [ctypes.POINTER(Call), ci, vp]
+        L.spear_w4_ec_gemm_batch_hostio.argtypes = [ctypes.POINTER(Call), ctypes.POINTER(HostIO), ci, vp]
         L.spear_w4_ec_gemm_hostio.argtypes = [vp] * 8 + [ctypes.POINTER(EcDesc)] + [ci] * 5 + [vp]
         L.spear_workspace_bytes.argtypes = [ci] * 5 + [ctypes.POINTER(ctypes.c_size_t)]
         L.spear_init.argtypes = []
@@ -229,6 +235,15 @@ class Batch:
             c.x, c.Wq, c.scales, c.A, c.B, c.y = _ptr(x), _ptr(pw.wq), _ptr(pw.scales), _ptr(A), _ptr(B), _ptr(y)
             c.ec = ctypes.pointer(desc) if desc is not None else None
             c.M, c.N, c.K, c.r, c.group = M, pw.N, K, (0 if A is None else A.shape[0]), pw.group
+
+
+def w4_ec_gemm_batch_hostio(batch: Batch, x_hosts, y_hosts, stream=None):
+    """spear_w4_ec_gemm_batch_hostio: per call, x from (pinned) host memory and y back to host, on the lanes."""
+    assert len(x_hosts) == batch.n and len(y_hosts) == batch.n
+    io = (HostIO * batch.n)()
+    for e, xh, yh in zip(io, x_hosts, y_hosts):
+        e.x_host, e.y_host = _ptr(xh), _ptr(yh)
+    _check(lib().spear_w4_ec_gemm_batch_hostio(batch.calls, io, batch.n, _stream(stream)))
 
 
 def w4_ec_gemm_batch(batch: Batch, stream=None):

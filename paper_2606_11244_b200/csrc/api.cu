@@ -495,7 +495,18 @@ extern "C" int spear_w4_ec_gemm(const void* x, const void* Wq, const void* scale
     return layer_impl(x, Wq, scales, A, B, &ec, y, M, N, K, r, group, static_cast<cudaStream_t>(stream));
 }
 
+static int batch_impl(const spear_call* calls, const spear_host_io* io, int n_calls, void* stream);
+
 extern "C" int spear_w4_ec_gemm_batch(const spear_call* calls, int n_calls, void* stream) {
+    return batch_impl(calls, nullptr, n_calls, stream);
+}
+
+extern "C" int spear_w4_ec_gemm_batch_hostio(const spear_call* calls, const spear_host_io* io, int n_calls, void* stream) {
+    if (!io) return set_error(SPEAR_EINVAL, "NULL host io array");
+    return batch_impl(calls, io, n_calls, stream);
+}
+
+static int batch_impl(const spear_call* calls, const spear_host_io* io, int n_calls, void* stream) {
     if (!calls || n_calls < 0) return set_error(SPEAR_EINVAL, "bad batch");
     if (n_calls == 0) return SPEAR_OK;
     if (int rc = spear_init()) return rc;
@@ -525,10 +536,23 @@ extern "C" int spear_w4_ec_gemm_batch(const spear_call* calls, int n_calls, void
         size_t need = 0;
         if (c.M >= 1 && c.r >= 0) need = ws_layout(c.M, c.r, 0).total + 1024;
         const int l = lane_of[i];
-        if (need <= kLaneWorkspace)
-            status = layer_impl(c.x, c.Wq, c.scales, c.A, c.B, c.ec, c.y, c.M, c.N, c.K, c.r, c.group, g_lane_stream[l],
-                                g_lane_ws[l], kLaneWorkspace);
-        else
+        if (io && (!io[i].x_host || !io[i].y_host || c.M < 1 || c.N < 1 || c.K < 1)) {
+            status = set_error(SPEAR_EINVAL, "batch call %d: NULL host buffer", i);
+            break;
+        }
+        if (need <= kLaneWorkspace) {
+            // host activations: x goes up and y comes back on the call's own lane, so the copies of one call overlap
+            // the kernels of the others
+            if (io && cudaMemcpyAsync(const_cast<void*>(c.x), io[i].x_host, size_t(c.M) * c.K * 2, cudaMemcpyHostToDevice,
+                                      g_lane_stream[l]) != cudaSuccess)
+                status = set_error(SPEAR_ECUDA, "batch call %d: H2D copy failed", i);
+            if (status == SPEAR_OK)
+                status = layer_impl(c.x, c.Wq, c.scales, c.A, c.B, c.ec, c.y, c.M, c.N, c.K, c.r, c.group, g_lane_stream[l],
+                                    g_lane_ws[l], kLaneWorkspace);
+            if (status == SPEAR_OK && io &&
+                cudaMemcpyAsync(io[i].y_host, c.y, size_t(c.M) * c.N * 2, cudaMemcpyDeviceToHost, g_lane_stream[l]) != cudaSuccess)
+                status = set_error(SPEAR_ECUDA, "batch call %d: D2H copy failed", i);
+        } else
             status = set_error(SPEAR_ENOMEM, "batch call %d needs %zu bytes of workspace (lane has %zu)", i, need, kLaneWorkspace);
     }
     t_in_batch = false;

@@ -288,3 +288,23 @@ def test_batch_matches_oracle_and_single_calls(sp):
             g.replay()
     torch.cuda.synchronize()
     verify("graph")
+
+
+def test_batch_hostio_matches_oracle(sp):
+    """spear_w4_ec_gemm_batch_hostio: pinned-host x in, pinned-host y out, per call, on the lanes."""
+    import torch
+    h = _harness()
+    specs = [(1, 256, 512, 16, "scalar"), (16, 384, 640, 24, "scalar"), (40, 256, 512, 16, "scalar"), (8, 2048, 2048, 0, "scalar")]
+    lis = [make_layer(600 + i, M, N, K, 128, r, gate=g) for i, (M, N, K, r, g) in enumerate(specs)]
+    dls = [h.upload_layer(li) for li in lis]
+    xs = [torch.zeros((li.M, li.K), dtype=torch.float16, device="cuda:0") for li in lis]      # staging buffers
+    ys = [torch.zeros((li.M, li.N), dtype=torch.float16, device="cuda:0") for li in lis]
+    xh = [torch.from_numpy(li.x).pin_memory() for li in lis]
+    yh = [torch.zeros((li.M, li.N), dtype=torch.float16).pin_memory() for li in lis]
+    batch = sp.Batch([(x, dl.pw, dl.A, dl.B, dl.desc(), y) for x, dl, y in zip(xs, dls, ys)])
+    sp.w4_ec_gemm_batch_hostio(batch, xh, yh)
+    torch.cuda.synchronize()
+    for li, y in zip(lis, yh):
+        ref = oracle.forward_layer(li)["y"]
+        rms = float(np.sqrt(np.mean(ref ** 2)))
+        assert float(np.max(np.abs(y.numpy().astype(np.float64) - ref))) <= Y_TOL * rms
