@@ -318,14 +318,15 @@ static int run_stream(const void* x, const void* Wq, const void* scales, const v
     p.G = K / group; p.group_chunks = group / 128; p.C = K / 128;
     p.CP = (p.C + 1) / 2;
     p.U = (N / 128) * p.CP;
-    // Ring depth: a CTA with many units to stream gets the deep ring (one CTA per SM, enough bytes in flight
-    // to cover the HBM latency); a CTA with few keeps the shallow one so that two CTAs fit an SM and the next
-    // layer's CTA can prefetch beside it.  The fused EC's device-wide arrive/wait needs every CTA resident,
+    // Ring depth: stream-ordered calls get the deep ring (one CTA per SM, ~200 KiB in flight, and the kernel
+    // instance compiled for one resident CTA, whose consumer loop does not spill); inside a batch the shallow ring
+    // keeps two CTAs per SM so that the kernels of different lanes overlap.  The fused EC's device-wide arrive/wait needs every CTA resident,
     // which both choices guarantee (grid <= SMs x resident CTAs per SM).
     int per_sm = std::max(1, std::min(2, g_tune.stream_ctas_per_sm));
     const int units_per_cta = (p.U + g_dev.num_sms - 1) / g_dev.num_sms;
     // Inside a batch the lanes overlap whole kernels, which needs two CTAs per SM: keep the shallow ring there.
-    bool deep = !t_in_batch && units_per_cta > 2;
+    bool deep = !t_in_batch;     // measured: the deep instance (168 registers, no spills) wins stream-ordered even on the smallest layers
+    (void)units_per_cta;
     if (g_tune.stream_deep >= 0) deep = g_tune.stream_deep != 0;
     if (deep) per_sm = 1;
     p.stages = stream_stages(MT, deep);

@@ -276,8 +276,10 @@ __device__ void ec_reduce_and_arrive(const StreamParams& p, int lane, int* par_s
     }
 }
 
-template <int MT>
-__global__ void __launch_bounds__(320, 2)
+// MINB = resident CTAs per SM the register allocation must allow: 2 for the shallow ring (96 registers), 1 for the
+// deep ring, where the consumer loop gets the registers to keep its four strips in flight without spilling.
+template <int MT, int MINB>
+__global__ void __launch_bounds__(320, MINB)
 stream_kernel(const __grid_constant__ CUtensorMap xmap, const StreamParams p) {
     using Cfg = StreamCfg<MT>;
     const int S = p.stages;
@@ -573,9 +575,13 @@ int launch_stream(const CUtensorMap& xmap, const StreamParams& p, int MT, int gr
                   cudaStream_t st) {
     static bool attr_set = false;
     if (!attr_set) {
-        SPEAR_CUDA_OK(cudaFuncSetAttribute(stream_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+        SPEAR_CUDA_OK(cudaFuncSetAttribute(stream_kernel<1, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                           int(StreamCfg<1>::smem_bytes(StreamCfg<1>::kStagesShallow))));
+        SPEAR_CUDA_OK(cudaFuncSetAttribute(stream_kernel<2, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                           int(StreamCfg<2>::smem_bytes(StreamCfg<2>::kStagesShallow))));
+        SPEAR_CUDA_OK(cudaFuncSetAttribute(stream_kernel<1, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                            int(StreamCfg<1>::smem_bytes(StreamCfg<1>::kStagesDeep))));
-        SPEAR_CUDA_OK(cudaFuncSetAttribute(stream_kernel<2>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+        SPEAR_CUDA_OK(cudaFuncSetAttribute(stream_kernel<2, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                            int(StreamCfg<2>::smem_bytes(StreamCfg<2>::kStagesDeep))));
         attr_set = true;
     }
@@ -589,8 +595,11 @@ int launch_stream(const CUtensorMap& xmap, const StreamParams& p, int MT, int gr
     attr[0].val.programmaticStreamSerializationAllowed = pdl ? 1 : 0;
     cfg.attrs = attr;
     cfg.numAttrs = 1;
-    if (MT == 1) SPEAR_CUDA_OK(cudaLaunchKernelEx(&cfg, stream_kernel<1>, xmap, p));
-    else SPEAR_CUDA_OK(cudaLaunchKernelEx(&cfg, stream_kernel<2>, xmap, p));
+    const bool deep = p.stages > stream_stages(MT, false);
+    if (MT == 1 && !deep) SPEAR_CUDA_OK(cudaLaunchKernelEx(&cfg, stream_kernel<1, 2>, xmap, p));
+    else if (MT == 1) SPEAR_CUDA_OK(cudaLaunchKernelEx(&cfg, stream_kernel<1, 1>, xmap, p));
+    else if (!deep) SPEAR_CUDA_OK(cudaLaunchKernelEx(&cfg, stream_kernel<2, 2>, xmap, p));
+    else SPEAR_CUDA_OK(cudaLaunchKernelEx(&cfg, stream_kernel<2, 1>, xmap, p));
     count_launch();
     return SPEAR_OK;
 }
