@@ -22,7 +22,8 @@ struct StreamParams {
     int U;                   // (N / 128) * CP work units
     int stages;              // ring depth (stream_stages)
     int debug;               // measurement hooks (results are wrong): bit 0 consumers skip the arithmetic; bit 1 the
-                             // epilogue does not wait for u; bit 2 the epilogue skips the rank-r add
+                             // epilogue does not wait for z; bit 2 the epilogue skips the rank-r add; bit 3 every
+                             // role returns after the prologue (launch machinery only)
     // ---- fused EC (SPEAR_VARIANT_STREAM_FUSED): z = x [A; w_g]^T, gate and u are computed by this kernel ----
     int fused;               // 0: u comes from the EC pre-kernel; 1: warp 9 of every CTA produces it
     int gate_kind;           // SPEAR_GATE_SCALAR_SIGMOID or SPEAR_GATE_NONE

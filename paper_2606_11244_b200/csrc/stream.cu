@@ -309,6 +309,7 @@ stream_kernel(const __grid_constant__ CUtensorMap xmap, const StreamParams p) {
     }
     __syncthreads();
     pdl_launch_dependents();
+    if (p.debug & 8) return;     // measurement hook: launch machinery only
 
     if (warp == 0) {
         // ------------------------------ producer: weights, scales, x tiles ------------------------------
