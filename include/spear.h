@@ -118,7 +118,7 @@ int spear_w4_ec_gemm_ex(const void* x, const void* Wq, const void* scales, const
 
 /* A batch of INDEPENDENT layer calls (no call reads another call's y; all y buffers distinct), e.g. the
  * q/k/v or gate/up projections of one transformer block, or unrelated requests.  The calls run
- * concurrently on the library's internal lanes (streams with their own workspaces); all of them are
+ * concurrently on the library's internal lanes (up to 16 streams with their own workspaces); all of them are
  * ordered after the work already enqueued on `stream` and before anything enqueued on it afterwards
  * (fork / join with events; capturable in a CUDA graph).  ec->workspace must be NULL.  The
  * per-token-gated EC of every call is evaluated exactly as in spear_w4_ec_gemm_ex. */

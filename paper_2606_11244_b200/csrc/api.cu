@@ -64,7 +64,7 @@ static WsLayout ws_layout(int M, int r, size_t ws_bytes) {
     return L;
 }
 constexpr size_t kDefaultWorkspace = size_t(96) << 20;
-constexpr int kBatchLanes = 4;
+constexpr int kBatchLanes = 16;
 constexpr size_t kLaneWorkspace = size_t(48) << 20;
 static cudaStream_t g_lane_stream[kBatchLanes];
 static cudaEvent_t g_lane_done[kBatchLanes];
@@ -202,9 +202,10 @@ struct Tunables {
     int tc_ksplit = 0;            // 0 = heuristic, else the tcgen05 kernel's split-K factor
     int tc_bt = 0;                // 0 = heuristic, else the tcgen05 kernel's token-tile width
     int tc_xslice_mb = 0;         // 0 = default (16), MiB of x per raster group
-    int batch_lanes = 4;          // concurrent lanes of spear_w4_ec_gemm_batch (1..4)
+    int batch_lanes = 16;         // concurrent lanes of spear_w4_ec_gemm_batch (1..16); measured 12 > 8 > 4 on the 12-call step
     int stream_deep = -1;         // -1 = heuristic, 0 / 1 = force the shallow / deep decode ring
     int stream_debug = 0;         // measurement hook, see StreamParams::debug
+    int stream_batch_grid = 128;  // cap of the decode grid inside a batch (0 = off); measured 128 > 148 > 96
     int stream_whole_panels = 1;  // 1 = whole-panel partition when N/128 is within 1/5 of the grid
 };
 static Tunables g_tune;
@@ -337,6 +338,9 @@ static int run_stream(const void* x, const void* Wq, const void* scales, const v
     // every panel in two and pay the cross-CTA reduction (partials through L2 + a counter) on all of them.
     const int n_panels = N / 128;
     if (g_tune.stream_whole_panels && n_panels <= grid && n_panels * 5 >= grid * 4) grid = n_panels;
+    // inside a batch smaller grids let more kernels of different lanes be resident at once (the step is bound by
+    // un-overlapped pipeline latency, not by bandwidth)
+    if (t_in_batch && g_tune.stream_batch_grid > 0) grid = std::min(grid, g_tune.stream_batch_grid);
     if (fused && r > 0) {
         p.fused = 1;
         p.gate_kind = ec->gate_kind;
@@ -466,6 +470,7 @@ extern "C" int spear_tune(const char* key, int value) {
     else if (!strcmp(key, "stream_deep")) g_tune.stream_deep = value;
     else if (!strcmp(key, "stream_debug")) g_tune.stream_debug = value;
     else if (!strcmp(key, "stream_whole_panels")) g_tune.stream_whole_panels = value;
+    else if (!strcmp(key, "stream_batch_grid")) g_tune.stream_batch_grid = value;
     else return set_error(SPEAR_EINVAL, "unknown tunable '%s'", key);
     return SPEAR_OK;
 }
@@ -519,7 +524,7 @@ static int batch_impl(const spear_call* calls, const spear_host_io* io, int n_ca
     std::stable_sort(order.begin(), order.end(), [&](int a, int b) {
         return size_t(calls[a].N) * calls[a].K > size_t(calls[b].N) * calls[b].K;
     });
-    size_t load[kBatchLanes] = {0, 0, 0, 0};
+    size_t load[kBatchLanes] = {};
     std::vector<int> lane_of(n_calls);
     for (int i : order) {
         int best = 0;
