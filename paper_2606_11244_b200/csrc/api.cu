@@ -206,6 +206,7 @@ struct Tunables {
     int stream_deep = -1;         // -1 = heuristic, 0 / 1 = force the shallow / deep decode ring
     int stream_debug = 0;         // measurement hook, see StreamParams::debug
     int stream_batch_grid = 128;  // cap of the decode grid inside a batch (0 = off); measured 128 > 148 > 96
+    int stream_batch_units = 8;   // target units per CTA inside a batch (0 = off); measured 8-10 > 4 > 16 > even split
     int stream_whole_panels = 1;  // 1 = whole-panel partition when N/128 is within 1/5 of the grid
 };
 static Tunables g_tune;
@@ -341,6 +342,12 @@ static int run_stream(const void* x, const void* Wq, const void* scales, const v
     // inside a batch smaller grids let more kernels of different lanes be resident at once (the step is bound by
     // un-overlapped pipeline latency, not by bandwidth)
     if (t_in_batch && g_tune.stream_batch_grid > 0) grid = std::min(grid, g_tune.stream_batch_grid);
+    // ... and a CTA that streams several units amortises its fill / reduction latency over them: aim at
+    // `stream_batch_units` units per CTA, cutting each panel into equal parts (whole panels when that is enough)
+    if (t_in_batch && g_tune.stream_batch_units > 0) {
+        const int parts = (p.CP + g_tune.stream_batch_units - 1) / g_tune.stream_batch_units;
+        grid = std::max(1, std::min(grid, n_panels * parts));
+    }
     if (fused && r > 0) {
         p.fused = 1;
         p.gate_kind = ec->gate_kind;
@@ -471,6 +478,7 @@ extern "C" int spear_tune(const char* key, int value) {
     else if (!strcmp(key, "stream_debug")) g_tune.stream_debug = value;
     else if (!strcmp(key, "stream_whole_panels")) g_tune.stream_whole_panels = value;
     else if (!strcmp(key, "stream_batch_grid")) g_tune.stream_batch_grid = value;
+    else if (!strcmp(key, "stream_batch_units")) g_tune.stream_batch_units = value;
     else return set_error(SPEAR_EINVAL, "unknown tunable '%s'", key);
     return SPEAR_OK;
 }
