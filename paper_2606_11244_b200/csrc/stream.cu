@@ -498,6 +498,7 @@ stream_kernel(const __grid_constant__ CUtensorMap xmap, const StreamParams p) {
                             // Watchdog: every CTA arrives within microseconds of its start, so seconds of waiting
                             // can only mean that the grid is not co-resident (see api.cu); fail loudly (sticky launch
                             // error) instead of hanging the device.
+                            if (f < gridDim.x) __nanosleep(200);     // do not hammer the line the arrivals need
                             if (f < gridDim.x && (++spins & 0x3ffu) == 0) {
                                 unsigned long long now;
                                 asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(now));
