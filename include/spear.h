@@ -169,9 +169,11 @@ int spear_plan_load(const char* path);
 /* The variant AUTO would run for this problem right now (table hit or heuristic). */
 int spear_plan_query(int M, int N, int K, int r, int group, int gate_kind, int* variant_out);
 
-/* Debug / sweep hook: sets a launch tunable ("stream_ctas_per_sm", "pdl", "ecpre_ctas", "tc_grid",
- * "tc_cluster", "batch_lanes").
- * Host-only, process-wide, not thread-safe against concurrent compute calls. */
+/* Debug / sweep hook: sets a launch tunable.  Decode kernel: "stream_ctas_per_sm", "stream_deep" (-1 heuristic,
+ * 0 / 1 shallow / deep ring), "stream_whole_panels", "stream_batch_grid", "stream_batch_units", "stream_units",
+ * "stream_debug" (measurement bits, results are wrong); EC pre-kernel: "ecpre_ctas"; tcgen05 kernel: "tc_grid",
+ * "tc_cluster", "tc_ksplit", "tc_bt", "tc_xslice_mb"; all: "pdl"; batch: "batch_lanes".  Unknown key ->
+ * SPEAR_EINVAL.  Host-only, process-wide, not thread-safe against concurrent compute calls. */
 int spear_tune(const char* key, int value);
 
 const char* spear_last_error(void);

@@ -207,6 +207,7 @@ struct Tunables {
     int stream_debug = 0;         // measurement hook, see StreamParams::debug
     int stream_batch_grid = 128;  // cap of the decode grid inside a batch (0 = off); measured 128 > 148 > 96
     int stream_batch_units = 8;   // target units per CTA inside a batch (0 = off); measured 8-10 > 4 > 16 > even split
+    int stream_units = 0;         // the same target for stream-ordered calls (0 = off: use every SM)
     int stream_whole_panels = 1;  // 1 = whole-panel partition when N/128 is within 1/5 of the grid
 };
 static Tunables g_tune;
@@ -344,8 +345,9 @@ static int run_stream(const void* x, const void* Wq, const void* scales, const v
     if (t_in_batch && g_tune.stream_batch_grid > 0) grid = std::min(grid, g_tune.stream_batch_grid);
     // ... and a CTA that streams several units amortises its fill / reduction latency over them: aim at
     // `stream_batch_units` units per CTA, cutting each panel into equal parts (whole panels when that is enough)
-    if (t_in_batch && g_tune.stream_batch_units > 0) {
-        const int parts = (p.CP + g_tune.stream_batch_units - 1) / g_tune.stream_batch_units;
+    const int units_target = t_in_batch ? g_tune.stream_batch_units : g_tune.stream_units;
+    if (units_target > 0) {
+        const int parts = (p.CP + units_target - 1) / units_target;
         grid = std::max(1, std::min(grid, n_panels * parts));
     }
     if (fused && r > 0) {
@@ -479,6 +481,7 @@ extern "C" int spear_tune(const char* key, int value) {
     else if (!strcmp(key, "stream_whole_panels")) g_tune.stream_whole_panels = value;
     else if (!strcmp(key, "stream_batch_grid")) g_tune.stream_batch_grid = value;
     else if (!strcmp(key, "stream_batch_units")) g_tune.stream_batch_units = value;
+    else if (!strcmp(key, "stream_units")) g_tune.stream_units = value;
     else return set_error(SPEAR_EINVAL, "unknown tunable '%s'", key);
     return SPEAR_OK;
 }
