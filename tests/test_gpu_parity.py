@@ -308,3 +308,19 @@ def test_batch_hostio_matches_oracle(sp):
         ref = oracle.forward_layer(li)["y"]
         rms = float(np.sqrt(np.mean(ref ** 2)))
         assert float(np.max(np.abs(y.numpy().astype(np.float64) - ref))) <= Y_TOL * rms
+
+
+# ---------------------------------------------------------------- degenerate sizes
+
+@pytest.mark.parametrize("M,N,K,group,r,gate", [
+    (1, 128, 128, 128, 8, "scalar"),       # one unit, one CTA: the device-wide EC arrive / wait with a grid of 1
+    (16, 128, 128, 128, 128, "scalar"),    # maximum rank on the smallest layer
+    (5, 128, 1152, 128, 16, "scalar"),     # odd chunk count: the panel's tail unit holds a single chunk
+    (16, 256, 1152, 384, 24, "none"),      # group of three chunks: a unit's two chunks fall in different groups
+    (2, 128, 128, 128, 0, "scalar"),       # plain W4, smallest
+    (9, 18432, 256, 128, 8, "scalar"),     # more panels than CTAs, whole panels per CTA
+])
+@pytest.mark.parametrize("variant", [0, 2, 3])
+def test_degenerate_shapes(sp, M, N, K, group, r, gate, variant):
+    li = make_layer(700 + M + N + K, M, N, K, group, r, gate=gate)
+    check_layer(li, variant=variant, label=f"degenerate M={M} N={N} K={K} g={group} r={r} v={variant}")
