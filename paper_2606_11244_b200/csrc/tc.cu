@@ -145,10 +145,12 @@ struct TcCfg {
     static constexpr int kXStages = BT == 256 ? 4 : (BT == 128 ? 3 : (BT == 64 ? 4 : 6));
     // dequantisation warp groups of 8 taking k-blocks round-robin: a k-block costs one barrier round trip
     // (~0.7 us) whatever its MMA time, so narrow token tiles (short MMAs) get three groups and a deeper A ring
-    static constexpr int kDequantGroups = BT == 256 ? 2 : 3;
+    // The A ring must be deeper than the number of groups, or a group's next stage waits for the MMA of its previous
+    // one (same slot) and nothing overlaps: 2 groups x 4 slots where shared memory allows (BT <= 64)
+    static constexpr int kDequantGroups = BT == 128 ? 3 : 2;
     static constexpr int kThreads = (7 + 8 * kDequantGroups) * 32;   // + x producer, MMA, 4 epilogue, int4 producer
-    static constexpr int kAStages = 3;
-    static constexpr int kW4Stages = BT == 256 ? 10 : (BT == 128 ? 4 : (BT == 64 ? 7 : 9));     // ncu: with 4 the dequantisation warps spun on w4_full (HBM latency x 4 KiB per stage)
+    static constexpr int kAStages = BT <= 64 ? 4 : 3;
+    static constexpr int kW4Stages = BT == 256 ? 10 : (BT == 128 ? 4 : (BT == 64 ? 4 : 6));     // ncu: with 4 the dequantisation warps spun on w4_full (HBM latency x 4 KiB per stage)
     static constexpr int kABytes = kKT * 128 * 128;      // kKT sub-tiles of 128 channels x 64 k fp16
     static constexpr int kXBytes = kKT * BT * 128;       // kKT sub-tiles of BT tokens x 64 k fp16
     static constexpr int kW4Bytes = kKT * 4096 + 256;    // codes of kKT (panel, 64-k tile)s + one scale block
