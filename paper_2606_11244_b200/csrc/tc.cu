@@ -149,8 +149,8 @@ struct TcCfg {
     // one (same slot) and nothing overlaps: 2 groups x 4 slots where shared memory allows (BT <= 64)
     static constexpr int kDequantGroups = BT == 128 ? 3 : 2;
     static constexpr int kThreads = (7 + 8 * kDequantGroups) * 32;   // + x producer, MMA, 4 epilogue, int4 producer
-    static constexpr int kAStages = BT <= 64 ? 4 : 3;
-    static constexpr int kW4Stages = BT == 256 ? 10 : (BT == 128 ? 4 : (BT == 64 ? 4 : 6));     // ncu: with 4 the dequantisation warps spun on w4_full (HBM latency x 4 KiB per stage)
+    static constexpr int kAStages = BT == 128 ? 3 : 4;
+    static constexpr int kW4Stages = BT == 256 ? 6 : (BT == 128 ? 4 : (BT == 64 ? 4 : 6));     // ncu: with 4 the dequantisation warps spun on w4_full (HBM latency x 4 KiB per stage)
     static constexpr int kABytes = kKT * 128 * 128;      // kKT sub-tiles of 128 channels x 64 k fp16
     static constexpr int kXBytes = kKT * BT * 128;       // kKT sub-tiles of BT tokens x 64 k fp16
     static constexpr int kW4Bytes = kKT * 4096 + 256;    // codes of kKT (panel, 64-k tile)s + one scale block
