@@ -324,3 +324,24 @@ def test_batch_hostio_matches_oracle(sp):
 def test_degenerate_shapes(sp, M, N, K, group, r, gate, variant):
     li = make_layer(700 + M + N + K, M, N, K, group, r, gate=gate)
     check_layer(li, variant=variant, label=f"degenerate M={M} N={N} K={K} g={group} r={r} v={variant}")
+
+
+def test_empty_and_misaligned_inputs_are_rejected(sp):
+    """Edge cases of the boundary: no tokens, a misaligned activation pointer, an unsupported shape."""
+    import torch
+    h = _harness()
+    li = make_layer(90, 4, 128, 128, 128, 0)
+    dl = h.upload_layer(li)
+    with pytest.raises(sp.SpearError) as e:                      # M = 0
+        sp.w4_ec_gemm(torch.empty((0, 128), dtype=torch.float16, device="cuda:0"), dl.pw)
+    assert e.value.status == -1
+    buf = torch.zeros(4 * 128 + 8, dtype=torch.float16, device="cuda:0")
+    x_mis = buf[1:1 + 4 * 128].view(4, 128)                      # 2 bytes off a 16-byte boundary
+    assert x_mis.data_ptr() % 16 != 0
+    with pytest.raises(sp.SpearError) as e:
+        sp.w4_ec_gemm(x_mis, dl.pw)
+    assert e.value.status == -1
+    with pytest.raises(sp.SpearError) as e:                      # K not a multiple of 128
+        sp.pack_w4(torch.zeros((128, 64), dtype=torch.uint8, device="cuda:0"),
+                   torch.ones((128, 1), dtype=torch.float16, device="cuda:0"), 64)
+    assert e.value.status == -2
