@@ -345,3 +345,34 @@ def test_empty_and_misaligned_inputs_are_rejected(sp):
         sp.pack_w4(torch.zeros((128, 64), dtype=torch.uint8, device="cuda:0"),
                    torch.ones((128, 1), dtype=torch.float16, device="cuda:0"), 64)
     assert e.value.status == -2
+
+
+def test_config2_step_in_the_bench_launch_configuration(sp):
+    """The 12 calls of BASELINE.json configs[1] issued exactly as bench.py times them: ONE
+    spear_w4_ec_gemm_batch (lanes, shallow-ring instance, ~8 units per CTA), captured in a CUDA graph and replayed;
+    every call against the oracle, every output element."""
+    import torch
+    h = _harness()
+    shapes = config_shapes(1)
+    lis = [make_layer(s.seed, s.M, s.N, s.K, s.group, s.r, gate="scalar") for s in shapes]
+    dls = [h.upload_layer(li) for li in lis]
+    xs = [h.dev(li.x) for li in lis]
+    ys = [torch.zeros((li.M, li.N), dtype=torch.float16, device="cuda:0") for li in lis]
+    batch = sp.Batch([(x, dl.pw, dl.A, dl.B, dl.desc(), y) for x, dl, y in zip(xs, dls, ys)])
+    st = torch.cuda.Stream()
+    with torch.cuda.stream(st):
+        sp.w4_ec_gemm_batch(batch)
+        torch.cuda.synchronize()
+        g = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(g, stream=st):
+            sp.w4_ec_gemm_batch(batch)
+        for y in ys:
+            y.zero_()
+        for _ in range(5):
+            g.replay()
+    torch.cuda.synchronize()
+    for s, li, y in zip(shapes, lis, ys):
+        ref = oracle.forward_layer(li)["y"]
+        rms = float(np.sqrt(np.mean(ref ** 2)))
+        err = float(np.max(np.abs(y.cpu().numpy().astype(np.float64) - ref)))
+        assert err <= Y_TOL * rms, f"config2 {s.name} M={s.M} in the batch: {err:.4g} > {Y_TOL} * {rms:.4g}"
