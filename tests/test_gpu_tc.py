@@ -184,3 +184,13 @@ def test_tc_split_variant(sp, M, r, gate):
     ref = oracle.forward_layer(li)["y"]
     rms = float(np.sqrt(np.mean(ref ** 2)))
     assert float((y_split.float() - y_fused.float()).abs().max()) <= Y_TOL * rms
+
+
+def test_config4_M4096_r64_sampled_rows(sp):
+    """The prefill shape bench.py times (configs[3]: M = 4096, K = 8192, N = 28672, r = 64) at full size: all N
+    columns of a seeded sample of token rows against the oracle (rows are independent, so sampling is exact)."""
+    s = [c for c in config_shapes(3) if c.M == 4096 and c.r == 64][0]
+    li = make_layer(s.seed, s.M, s.N, s.K, s.group, s.r, gate="scalar")
+    rng = np.random.default_rng(s.seed)
+    rows = np.array(sorted({0, s.M - 1, 255, 256, *[int(v) for v in rng.integers(0, s.M, size=8)]}))
+    check(li, variant=0, rows=rows, label="config4 M=4096 r=64")
