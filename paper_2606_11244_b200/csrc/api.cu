@@ -207,6 +207,7 @@ struct Tunables {
     int stream_debug = 0;         // measurement hook, see StreamParams::debug
     int stream_batch_grid = 128;  // cap of the decode grid inside a batch (0 = off); measured 128 > 148 > 96
     int stream_batch_units = 8;   // target units per CTA inside a batch (0 = off); measured 8-10 > 4 > 16 > even split
+    int ecbig_kdiv = 0;           // 0 = default 2 (measured 1-2 > 4): minimum k-tiles per K split of the M > 16 EC pre-pass
     int stream_units = 0;         // the same target for stream-ordered calls (0 = off: use every SM)
     int stream_whole_panels = 1;  // 1 = whole-panel partition when N/128 is within 1/5 of the grid
 };
@@ -390,7 +391,7 @@ static int run_tc_fused(const void* x, const void* Wq, const void* scales, const
         const int mtiles = (M + 63) / 64, ktiles = K / 64;
         int target = (g_tune.ecpre_ctas > 0 ? g_tune.ecpre_ctas : 2 * g_dev.num_sms);
         int ksplit = std::max(1, target / mtiles);
-        e.ksplit = std::max(1, std::min(ksplit, ktiles / 4));
+        e.ksplit = std::max(1, std::min(ksplit, ktiles / (g_tune.ecbig_kdiv > 0 ? g_tune.ecbig_kdiv : 2)));
         if (int rc = launch_ec_big(e, pdl, st)) return rc;
     }
     TcProblem t = {};
@@ -482,6 +483,7 @@ extern "C" int spear_tune(const char* key, int value) {
     else if (!strcmp(key, "stream_batch_grid")) g_tune.stream_batch_grid = value;
     else if (!strcmp(key, "stream_batch_units")) g_tune.stream_batch_units = value;
     else if (!strcmp(key, "stream_units")) g_tune.stream_units = value;
+    else if (!strcmp(key, "ecbig_kdiv")) g_tune.ecbig_kdiv = value;
     else return set_error(SPEAR_EINVAL, "unknown tunable '%s'", key);
     return SPEAR_OK;
 }
