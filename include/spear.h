@@ -171,7 +171,7 @@ int spear_plan_query(int M, int N, int K, int r, int group, int gate_kind, int* 
 
 /* Debug / sweep hook: sets a launch tunable.  Decode kernel: "stream_ctas_per_sm", "stream_deep" (-1 heuristic,
  * 0 / 1 shallow / deep ring), "stream_whole_panels", "stream_batch_grid", "stream_batch_units", "stream_units",
- * "stream_debug" (measurement bits, results are wrong); EC pre-kernel: "ecpre_ctas"; tcgen05 kernel: "tc_grid",
+ * "stream_debug" (measurement bits, results are wrong); EC pre-kernels: "ecpre_ctas", "ecbig_kdiv"; tcgen05 kernel: "tc_grid",
  * "tc_cluster", "tc_ksplit", "tc_bt", "tc_xslice_mb"; all: "pdl"; batch: "batch_lanes".  Unknown key ->
  * SPEAR_EINVAL.  Host-only, process-wide, not thread-safe against concurrent compute calls. */
 int spear_tune(const char* key, int value);
