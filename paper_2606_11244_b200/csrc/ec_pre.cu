@@ -66,15 +66,24 @@ __device__ void apply_gate(const GateArgs& ga, float (*zs)[kZStride], float (*hi
         }
     } else if (ga.gate_kind == SPEAR_GATE_MLP) {
         const int h = ga.h;
+        // rows of W1 / W2 are read as 16-byte vectors, four in flight, so that the L2 latency is paid per row and
+        // not per element (r % 8 == 0 and h % 8 == 0: every row is 16-byte aligned)
         for (int i = tid; i < h; i += nthreads) {
             float a[16];
 #pragma unroll
             for (int m = 0; m < 16; ++m) a[m] = 0.f;
-            const __half* w1 = ga.W1 + size_t(i) * r;
-            for (int j = 0; j < r; ++j) {
-                const float w = __half2float(w1[j]);
+            const uint4* w1 = reinterpret_cast<const uint4*>(ga.W1 + size_t(i) * r);
+#pragma unroll 4
+            for (int j8 = 0; j8 < r / 8; ++j8) {
+                const uint4 wv = __ldg(w1 + j8);
+                const __half2* wh = reinterpret_cast<const __half2*>(&wv);
 #pragma unroll
-                for (int m = 0; m < 16; ++m) a[m] = fmaf(w, zs[m][j], a[m]);
+                for (int q = 0; q < 4; ++q) {
+                    const float2 w = __half22float2(wh[q]);
+                    const int j = j8 * 8 + 2 * q;
+#pragma unroll
+                    for (int m = 0; m < 16; ++m) a[m] = fmaf(w.y, zs[m][j + 1], fmaf(w.x, zs[m][j], a[m]));
+                }
             }
             const float bb = ga.b1[i];
 #pragma unroll
@@ -85,11 +94,18 @@ __device__ void apply_gate(const GateArgs& ga, float (*zs)[kZStride], float (*hi
             float a[16];
 #pragma unroll
             for (int m = 0; m < 16; ++m) a[m] = 0.f;
-            const __half* w2 = ga.W2 + size_t(j) * h;
-            for (int i = 0; i < h; ++i) {
-                const float w = __half2float(w2[i]);
+            const uint4* w2 = reinterpret_cast<const uint4*>(ga.W2 + size_t(j) * h);
+#pragma unroll 4
+            for (int i8 = 0; i8 < h / 8; ++i8) {
+                const uint4 wv = __ldg(w2 + i8);
+                const __half2* wh = reinterpret_cast<const __half2*>(&wv);
 #pragma unroll
-                for (int m = 0; m < 16; ++m) a[m] = fmaf(w, hid[m][i], a[m]);
+                for (int q = 0; q < 4; ++q) {
+                    const float2 w = __half22float2(wh[q]);
+                    const int i = i8 * 8 + 2 * q;
+#pragma unroll
+                    for (int m = 0; m < 16; ++m) a[m] = fmaf(w.y, hid[m][i + 1], fmaf(w.x, hid[m][i], a[m]));
+                }
             }
             const float bb = ga.b2[j];
             for (int m = 0; m < m_count; ++m) {
