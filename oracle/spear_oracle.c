@@ -29,7 +29,8 @@
  *   A5  spo_rtn_quantise: test-only round-to-nearest quantiser.
  *
  * Pins (tests/test_oracle_pins.py): worked example P1 of SURVEY.md 8(c) stored in
- * tests/golden/, exact-rational brute force, numpy.matmul on the dequantised
+ * tests/golden/, the MLP-gate worked example (h != r, ReLU active, non-zero biases) stored in
+ * tests/golden/, exact-rational brute force with and without the gate, numpy.matmul on the dequantised
  * weight, Eq. 2 / Eq. 4 effective-weight identities, rank / linearity, gate
  * bounds, token-permutation equivariance, fp16 codec against numpy.float16.
  */

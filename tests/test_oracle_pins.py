@@ -147,6 +147,92 @@ def test_numpy_matmul_cross_check_medium():
     np.testing.assert_allclose(out["y"], y, rtol=1e-11, atol=1e-10)
 
 
+# ---------------------------------------------------------------- the paper's MLP gate
+
+def _exp_fraction(v, terms=60):
+    """exp of a small rational by its Taylor series in exact rationals (independent of libm)."""
+    s, t = Fraction(1), Fraction(1)
+    for i in range(1, terms):
+        t = t * v / i
+        s += t
+    return s
+
+
+def _tanh_fraction(v):
+    e = _exp_fraction(2 * v)
+    return (e - 1) / (e + 1)
+
+
+def test_mlp_gate_worked_example_h3_r2_relu_active():
+    """Hand-computed golden for gamma = 1 + tanh(W2 ReLU(W1 z + b1) + b2): h != r,
+    non-zero biases, one hidden unit clipped by the ReLU.  A transposed W1 or W2, a missing ReLU
+    or a dropped b1 each change gamma by far more than the tolerance."""
+    with open(os.path.join(GOLD, "mlp_gate_worked_example.json")) as f:
+        g = json.load(f)
+    # the stored transcendental values against the exact-rational series (no libm on this side)
+    for logit, gam in zip(g["logit"], g["gam"][0]):
+        assert abs(float(1 + _tanh_fraction(Fraction(logit))) - gam) <= 1e-15
+    What = oracle.dequant(np.array(g["codes"], np.uint8), f16(g["scales"]), g["group"])
+    out = oracle.forward(f16(g["x"]), What, f16(g["A"]), f16(g["B"]), gate="mlp", alpha=g["alpha"],
+                         W1=f16(g["W1"]), b1=np.array(g["b1"], np.float32),
+                         W2=f16(g["W2"]), b2=np.array(g["b2"], np.float32))
+    assert np.array_equal(out["ybase"], np.array(g["ybase"]))
+    assert np.array_equal(out["z"], np.array(g["z"]))
+    np.testing.assert_allclose(out["gam"], np.array(g["gam"]), rtol=0, atol=2e-15)
+    np.testing.assert_allclose(out["y"], np.array(g["y"]), rtol=0, atol=1e-14)
+
+
+@pytest.mark.parametrize("gate,h", [("mlp", 24), ("mlp", 16), ("mlp", 8), ("scalar", 0)])
+def test_P8_bruteforce_rational_with_the_gate(gate, h):
+    """P8 with the gate on: pre-activations / logits in exact rationals (triple loops over Fractions,
+    indices written from PAPER.md:109: W1 is h x r, W2 is r x h), the transcendental through
+    math.tanh / math.exp of the correctly rounded rational."""
+    import math
+    li = make_layer(seed=17, M=3, N=128, K=256, group=128, r=8, gate=gate, h=h if h else None)
+    if gate == "mlp":
+        # non-zero biases (the workload recipe has b1 = b2 = 0): dyadic, exact in fp32
+        rng = np.random.default_rng(5)
+        li.b1 = (rng.integers(-8, 9, li.W1.shape[0]) / 8.0).astype(np.float32)
+        li.b2 = (rng.integers(-4, 5, li.r) / 16.0).astype(np.float32)
+    Nn = 5
+    codes, scales, Bm = li.codes[:Nn], li.scales[:Nn], li.B[:Nn]
+    What = oracle.dequant(codes, scales, li.group)
+    alpha = Fraction(5, 4)
+    kw = dict(gate=gate, alpha=float(alpha))
+    if gate == "mlp":
+        kw.update(W1=li.W1, b1=li.b1, W2=li.W2, b2=li.b2)
+    else:
+        kw.update(w_g=li.w_g, b_g=0.375)
+    out = oracle.forward(li.x, What, li.A, Bm, **kw)
+    X, Af, Bf, S = _frac(li.x), _frac(li.A), _frac(Bm), _frac(scales)
+    n_clipped = 0
+    for m in range(li.M):
+        z = [sum(Af[j][k] * X[m][k] for k in range(li.K)) for j in range(li.r)]
+        if gate == "mlp":
+            W1f, W2f = _frac(li.W1), _frac(li.W2)          # [h][r], [r][h]
+            hh = li.W1.shape[0]
+            pre = [sum(W1f[i][j] * z[j] for j in range(li.r)) + Fraction(float(li.b1[i])) for i in range(hh)]
+            n_clipped += sum(1 for v in pre if v < 0)
+            hid = [v if v > 0 else Fraction(0) for v in pre]
+            logit = [sum(W2f[j][i] * hid[i] for i in range(hh)) + Fraction(float(li.b2[j])) for j in range(li.r)]
+            gam = [1.0 + math.tanh(float(v)) for v in logit]
+            for j in range(li.r):
+                assert abs(out["gam"][m][j] - gam[j]) <= 1e-12, (m, j)
+        else:
+            wg = [Fraction(float(v)) for v in li.w_g]
+            logit = sum(X[m][k] * wg[k] for k in range(li.K)) + Fraction(3, 8)
+            gs = 1.0 / (1.0 + math.exp(-float(logit)))
+            assert abs(out["gam"][m] - gs) <= 1e-12
+            gam = [gs] * li.r
+        for n in range(Nn):
+            base = sum(X[m][k] * (int(codes[n][k]) - 8) * S[n][k // li.group] for k in range(li.K))
+            # gamma enters as the fp64 value checked above; everything around it stays exact
+            y = base + alpha * sum(Bf[n][j] * Fraction(gam[j]) * z[j] for j in range(li.r))
+            assert abs(out["y"][m][n] - float(y)) <= 1e-11 * max(1.0, abs(float(y)))
+    if gate == "mlp":
+        assert n_clipped > 0          # the ReLU really clips on this input
+
+
 # ---------------------------------------------------------------- P2 reductions to plain W4
 
 def test_P2_zero_A_or_B_or_closed_gate_is_plain_w4():
