@@ -61,7 +61,9 @@ typedef enum {
     SPEAR_VARIANT_TC_FUSED = 3,      /* EC pre-kernel + tcgen05 GEMM with [X|U].[What|B]^T K-concatenation; any M */
     SPEAR_VARIANT_TC_SPLIT = 4,      /* EC pre-kernel + tcgen05 GEMM (plain W4) + a separate rank-r update pass over y (the
                                         paper's unfused comparator; y is rounded twice); any M, r > 0 */
-    SPEAR_VARIANT_COUNT = 5
+    SPEAR_VARIANT_LSTREAM = 5,       /* persistent layer-stream kernel (tcgen05, weights through TMEM), EC fused; M <= 16,
+                                        scalar / none gate; also what spear_w4_ec_gemm_batch runs for such calls */
+    SPEAR_VARIANT_COUNT = 6
 } spear_variant;
 
 /* ---- S0: packing (the "SPW4" layout) -------------------------------- */

@@ -70,6 +70,22 @@ static cudaStream_t g_lane_stream[kBatchLanes];
 static cudaEvent_t g_lane_done[kBatchLanes];
 static cudaEvent_t g_batch_fork;
 static void* g_lane_ws[kBatchLanes];
+// layer-stream kernel (lstream.cu): split-K slots, panel counters, phase counters, EC state
+struct LsWs { size_t partial, counters, done, zbuf, ubuf, ec_sync, total; };
+constexpr int kLsMaxPanels = 1 << 16;
+static LsWs ls_ws_layout(int grid) {
+    LsWs L;
+    size_t o = 0;
+    L.partial = o; o += size_t(grid) * 2 * 2 * 2048 * 4;
+    L.counters = o; o += size_t(kLsMaxPanels) * 4;
+    L.done = o; o += align_up(size_t(kLsMaxCalls + 1) * 4, 1024);
+    L.zbuf = o; o += align_up(size_t(kLsMaxCalls) * 16 * kZStride * 4, 1024);
+    L.ubuf = o; o += size_t(kLsMaxCalls) * 2048 * 4;
+    L.ec_sync = o; o += align_up(size_t(kLsMaxCalls) * 2 * 4, 1024);
+    L.total = o;
+    return L;
+}
+static void* g_ls_ws = nullptr;
 
 static void do_init() {
     int dev = 0;
@@ -113,6 +129,11 @@ static void do_init() {
         if (e == cudaSuccess) e = cudaMemset(g_lane_ws[l], 0, kLaneWorkspace);
     }
     if (e == cudaSuccess) e = cudaEventCreateWithFlags(&g_batch_fork, cudaEventDisableTiming);
+    if (e == cudaSuccess) {
+        const size_t ls_bytes = ls_ws_layout(g_dev.num_sms).total;
+        e = cudaMalloc(&g_ls_ws, ls_bytes);
+        if (e == cudaSuccess) e = cudaMemset(g_ls_ws, 0, ls_bytes);
+    }
     if (e == cudaSuccess) e = cudaDeviceSynchronize();
     if (e != cudaSuccess) {
         snprintf(g_init_err, sizeof(g_init_err), "batch lanes: %s", cudaGetErrorString(e));
@@ -209,6 +230,7 @@ struct Tunables {
     int stream_batch_units = 8;   // target units per CTA inside a batch (0 = off); measured 8-10 > 4 > 16 > even split
     int ecbig_kdiv = 0;           // 0 = default 2 (measured 1-2 > 4): minimum k-tiles per K split of the M > 16 EC pre-pass
     int stream_units = 0;         // the same target for stream-ordered calls (0 = off: use every SM)
+    int lstream = 1;              // 1 = M <= 16 calls (single and batched) take the persistent layer-stream kernel
     int stream_whole_panels = 1;  // 1 = whole-panel partition when N/128 is within 1/5 of the grid
 };
 static Tunables g_tune;
@@ -228,6 +250,7 @@ static bool variant_valid(int v, int M, int r, int gate) {
     switch (v) {
         case SPEAR_VARIANT_STREAM_FUSED: return M <= 16 && r > 0 && gate != SPEAR_GATE_MLP;
         case SPEAR_VARIANT_STREAM_SPLIT: return M <= 16;
+        case SPEAR_VARIANT_LSTREAM: return M <= 16 && gate != SPEAR_GATE_MLP;
         case SPEAR_VARIANT_TC_FUSED: return tc_available() && M >= 1;
         case SPEAR_VARIANT_TC_SPLIT: return tc_available() && r > 0;
         default: return false;
@@ -235,6 +258,7 @@ static bool variant_valid(int v, int M, int r, int gate) {
     (void)r;
 }
 static int heuristic_variant(int M, int r, int gate) {
+    if (M <= 16 && g_tune.lstream && gate != SPEAR_GATE_MLP) return SPEAR_VARIANT_LSTREAM;
     if (M <= 16) return (r > 0 && gate != SPEAR_GATE_MLP) ? SPEAR_VARIANT_STREAM_FUSED : SPEAR_VARIANT_STREAM_SPLIT;
     return SPEAR_VARIANT_TC_FUSED;
 }
@@ -415,6 +439,97 @@ static int run_tc_fused(const void* x, const void* Wq, const void* scales, const
     return SPEAR_OK;
 }
 
+// ------------------------------------------------------------------------------------------------
+// The persistent layer-stream kernel (lstream.cu): builds the call table of ONE launch.  Calls are grouped
+// into phases: a call whose x (or y) overlaps the y of an earlier call of the current phase opens a new
+// phase, so dependent chains (call i+1 reads call i's y) are legal and ordered inside the launch.
+// ------------------------------------------------------------------------------------------------
+static bool overlaps(const void* a, size_t an, const void* b, size_t bn) {
+    const uintptr_t a0 = uintptr_t(a), b0 = uintptr_t(b);
+    return a0 < b0 + bn && b0 < a0 + an;
+}
+static bool ls_eligible(const spear_call& c) {
+    if (c.M < 1 || c.M > 16) return false;
+    if (c.r > 0 && c.ec && c.ec->gate_kind == SPEAR_GATE_MLP) return false;
+    if (c.ec && c.ec->workspace) return false;
+    return true;
+}
+static int run_lstream(const spear_call* calls, int n_calls, cudaStream_t st) {
+    int done_calls = 0;
+    while (done_calls < n_calls) {
+        LsParams p;
+        memset(&p, 0, sizeof(p));
+        const LsWs L = ls_ws_layout(g_dev.num_sms);
+        uint8_t* ws = static_cast<uint8_t*>(g_ls_ws);
+        p.partial = reinterpret_cast<float*>(ws + L.partial);
+        p.counters = reinterpret_cast<unsigned*>(ws + L.counters);
+        p.done = reinterpret_cast<unsigned*>(ws + L.done);
+        p.zbuf = reinterpret_cast<float*>(ws + L.zbuf);
+        p.ubuf = reinterpret_cast<float*>(ws + L.ubuf);
+        p.ec_sync = reinterpret_cast<unsigned*>(ws + L.ec_sync);
+        int n = 0, ph = -1, phase_begin = 0, panels = 0, ec_slots = 0;
+        long long phase_chunks = 0;
+        for (int i = done_calls; i < n_calls && n < kLsMaxCalls; ++i) {
+            const spear_call& c = calls[i];
+            const void* A = c.r ? c.A : nullptr;
+            const void* Bm = c.r ? c.B : nullptr;
+            if (int rc = check_problem(c.x, c.Wq, c.scales, A, Bm, c.ec, c.y, c.M, c.N, c.K, c.r, c.group)) return rc;
+            if (panels + c.N / 128 > kLsMaxPanels) break;
+            bool dep = (ph < 0);
+            for (int j = phase_begin; j < n && !dep; ++j) {
+                const LsCall& e = p.calls[j];
+                const size_t yb = size_t(e.M) * e.N * 2;
+                dep = overlaps(c.x, size_t(c.M) * c.K * 2, e.y, yb) || overlaps(c.y, size_t(c.M) * c.N * 2, e.y, yb) ||
+                      overlaps(c.y, size_t(c.M) * c.N * 2, e.x, size_t(e.M) * e.K * 2);
+            }
+            const long long chunks = (long long)(c.N / 128) * (c.K / 128);
+            if (dep || phase_chunks + chunks > 0x3fffffff) {
+                if (ph >= 0) { p.phase_chunks[ph] = int(phase_chunks); }
+                ++ph;
+                p.phase_first_call[ph] = n;
+                phase_begin = n;
+                phase_chunks = 0;
+            }
+            LsCall& d = p.calls[n];
+            d.wq = static_cast<const uint8_t*>(c.Wq);
+            d.scales = static_cast<const uint8_t*>(c.scales);
+            d.x = static_cast<const __half*>(c.x);
+            d.y = static_cast<__half*>(c.y);
+            d.M = c.M; d.N = c.N; d.K = c.K; d.r = c.r;
+            d.group_chunks = c.group / 128;
+            d.C = c.K / 128;
+            d.P = c.N / 128;
+            d.chunk_base = int(phase_chunks);
+            d.panel_base = panels;
+            d.ec_slot = -1;
+            d.gate_kind = SPEAR_GATE_NONE;
+            d.alpha = 1.f;
+            if (c.r > 0) {
+                d.A = static_cast<const __half*>(c.A);
+                d.B = static_cast<const __half*>(c.B);
+                d.gate_kind = c.ec->gate_kind;
+                d.alpha = c.ec->alpha;
+                d.w_g = static_cast<const __half*>(c.ec->w_g);
+                d.b_g = static_cast<const float*>(c.ec->b_g);
+                d.gate_out = static_cast<float*>(c.ec->gate_out);
+                d.ec_slot = ec_slots++;
+            }
+            phase_chunks += chunks;
+            p.phase_panels[ph] += d.P;
+            panels += d.P;
+            ++n;
+        }
+        if (n == 0) return set_error(SPEAR_EUNSUPPORTED, "layer-stream: a single call exceeds the counter capacity");
+        p.phase_chunks[ph] = int(phase_chunks);
+        p.n_calls = n;
+        p.n_phases = ph + 1;
+        p.phase_first_call[p.n_phases] = n;
+        if (int rc = launch_lstream(p, st)) return rc;
+        done_calls += n;
+    }
+    return SPEAR_OK;
+}
+
 static int layer_impl(const void* x, const void* Wq, const void* scales, const void* A, const void* B,
                       const spear_ec_desc* ec, void* y, int M, int N, int K, int r, int group, cudaStream_t st,
                       void* lane_ws = nullptr, size_t lane_ws_bytes = 0) {
@@ -438,6 +553,13 @@ static int layer_impl(const void* x, const void* Wq, const void* scales, const v
             return set_error(SPEAR_EUNSUPPORTED, "variant %d is not valid for M=%d r=%d gate=%d", v, M, r, gate);
         v = heuristic_variant(M, r, gate);
         if (!variant_valid(v, M, r, gate)) return set_error(SPEAR_EUNSUPPORTED, "no kernel variant for M=%d r=%d", M, r);
+    }
+    if (v == SPEAR_VARIANT_LSTREAM && ec && ec->workspace && ec->force_variant == SPEAR_VARIANT_AUTO)
+        v = (r > 0 && gate != SPEAR_GATE_MLP) ? SPEAR_VARIANT_STREAM_FUSED : SPEAR_VARIANT_STREAM_SPLIT;   // caller-owned workspace
+    if (v == SPEAR_VARIANT_LSTREAM) {
+        if (ec && ec->workspace) return set_error(SPEAR_EUNSUPPORTED, "the layer-stream variant uses the library's own workspace");
+        spear_call c = {x, Wq, scales, A, B, ec, y, M, N, K, r, group};
+        return run_lstream(&c, 1, st);
     }
     switch (v) {
         case SPEAR_VARIANT_STREAM_FUSED:
@@ -479,6 +601,7 @@ extern "C" int spear_tune(const char* key, int value) {
     else if (!strcmp(key, "batch_lanes")) g_tune.batch_lanes = value;
     else if (!strcmp(key, "stream_deep")) g_tune.stream_deep = value;
     else if (!strcmp(key, "stream_debug")) g_tune.stream_debug = value;
+    else if (!strcmp(key, "lstream")) g_tune.lstream = value;
     else if (!strcmp(key, "stream_whole_panels")) g_tune.stream_whole_panels = value;
     else if (!strcmp(key, "stream_batch_grid")) g_tune.stream_batch_grid = value;
     else if (!strcmp(key, "stream_batch_units")) g_tune.stream_batch_units = value;
@@ -530,6 +653,11 @@ static int batch_impl(const spear_call* calls, const spear_host_io* io, int n_ca
     if (n_calls == 0) return SPEAR_OK;
     if (int rc = spear_init()) return rc;
     cudaStream_t st = static_cast<cudaStream_t>(stream);
+    if (!io && g_tune.lstream) {
+        bool all = true;
+        for (int i = 0; i < n_calls && all; ++i) all = ls_eligible(calls[i]);
+        if (all) return run_lstream(calls, n_calls, st);
+    }
     const int lanes = std::max(1, std::min(kBatchLanes, std::min(n_calls, g_tune.batch_lanes)));
     // longest-processing-time-first assignment by weight bytes
     std::vector<int> order(n_calls);

@@ -5,6 +5,8 @@
 
 namespace spear {
 
+constexpr int kZStride = 136;    // >= r + 1 (the extra column carries the scalar-gate logit)
+
 // ---- stream.cu (M <= 16) ------------------------------------------------------------------------
 struct StreamParams {
     const void* wq;          // SPW4 packed codes
@@ -41,6 +43,47 @@ int stream_stages(int MT, bool deep);
 int stream_smem_bytes(int MT, int stages);
 int launch_stream(const CUtensorMap& xmap, const StreamParams& p, int MT, int grid, bool pdl, cudaStream_t st);
 
+// ---- lstream.cu (M <= 16): persistent "layer stream" -- ONE cooperative launch consumes a table of layer
+// calls as a single queue of (call, panel, 128-column chunk) work items; int4 -> fp16 in registers -> TMEM
+// (tcgen05.st) -> tcgen05.mma with the tokens as N = 16 (A operand in tensor memory), fp32 accumulators in TMEM.
+constexpr int kLsMaxCalls = 64;
+struct LsCall {
+    const uint8_t* wq;       // SPW4 packed codes
+    const uint8_t* scales;   // SPW4 packed scales
+    const __half* x;         // [M][K]
+    __half* y;               // [M][N]
+    const __half* A;         // [r][K] or NULL
+    const __half* B;         // [N][r] or NULL
+    const __half* w_g;       // [K] (scalar gate) or NULL
+    const float* b_g;        // 1 (device) or NULL
+    float* gate_out;         // optional [M]
+    int M, N, K, r;
+    int group_chunks;        // group / 128
+    int C;                   // K / 128 chunks per panel
+    int P;                   // N / 128 panels
+    int gate_kind;           // SPEAR_GATE_SCALAR_SIGMOID or SPEAR_GATE_NONE
+    float alpha;
+    int chunk_base;          // first chunk of this call inside its phase's chunk sequence
+    int panel_base;          // first split-K counter of this call
+    int ec_slot;             // EC state slot (z, u, counters) or -1
+};
+struct LsParams {
+    LsCall calls[kLsMaxCalls];
+    int n_calls, n_phases;
+    int phase_first_call[kLsMaxCalls + 1];   // calls of phase ph: [phase_first_call[ph], phase_first_call[ph + 1])
+    int phase_chunks[kLsMaxCalls];           // chunks of the phase (all its calls)
+    int phase_panels[kLsMaxCalls];           // panels of the phase = y completions to wait for
+    float* partial;          // [2 phase parities][grid][2][16][128] fp32 split-K slots
+    unsigned* counters;      // per-panel split-K counters, zero between launches (self-cleaning)
+    unsigned* done;          // [n_phases] finalised panels per phase + [kLsMaxCalls] exit counter; zeroed by the last CTA
+    float* zbuf;             // [ec slots][16][kZStride] fp32, zero between launches
+    float* ubuf;             // [ec slots][16][128] fp32: u = alpha * gamma (.) z
+    unsigned* ec_sync;       // [ec slots][2]: z arrivals, u-ready flag; zeroed by the last arriver / last CTA
+};
+size_t ls_workspace_bytes(int grid);
+int ls_grid();
+int launch_lstream(const LsParams& p, cudaStream_t st);
+
 // ---- ec_pre.cu (M <= 16): z = x A^T, gate, u = alpha * gamma (.) z ------------------------------
 struct EcPreParams {
     const __half* x;         // [M][K]
@@ -59,7 +102,6 @@ struct EcPreParams {
     int ksplit;
     float alpha;
 };
-constexpr int kZStride = 136;    // >= r + 1 (the extra column carries the scalar-gate logit)
 int launch_ec_pre(const EcPreParams& p, bool pdl, cudaStream_t st);
 
 // ---- ec_big.cu (M > 16): z = x [A; w_g]^T (split-K, fp32 red.add), then gate -> u16 = fp16(alpha*gamma(.)z)
