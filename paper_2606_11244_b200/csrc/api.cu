@@ -71,17 +71,19 @@ static cudaEvent_t g_lane_done[kBatchLanes];
 static cudaEvent_t g_batch_fork;
 static void* g_lane_ws[kBatchLanes];
 // layer-stream kernel (lstream.cu): split-K slots, panel counters, phase counters, EC state
-struct LsWs { size_t partial, counters, done, zbuf, ubuf, ec_sync, total; };
+struct LsWs { size_t partial, counters, done, zbuf, ubuf, ec_sync, xperm, total; };
+constexpr size_t kLsXpermBytes = size_t(32) << 20;     // x in the MMA operand layout: 2 or 4 KiB per (call, 128-column chunk)
 constexpr int kLsMaxPanels = 1 << 16;
 static LsWs ls_ws_layout(int grid) {
     LsWs L;
     size_t o = 0;
     L.partial = o; o += size_t(grid) * 2 * 2 * 2048 * 4;
     L.counters = o; o += size_t(kLsMaxPanels) * 4;
-    L.done = o; o += align_up(size_t(kLsMaxCalls + 1) * 4, 1024);
+    L.done = o; o += align_up(size_t(kLsMaxCalls + 2) * 4, 1024);
     L.zbuf = o; o += align_up(size_t(kLsMaxCalls) * 16 * kZStride * 4, 1024);
     L.ubuf = o; o += size_t(kLsMaxCalls) * 2048 * 4;
     L.ec_sync = o; o += align_up(size_t(kLsMaxCalls) * 2 * 4, 1024);
+    L.xperm = o; o += kLsXpermBytes;
     L.total = o;
     return L;
 }
@@ -234,6 +236,7 @@ struct Tunables {
     int stream_whole_panels = 1;  // 1 = whole-panel partition when N/128 is within 1/5 of the grid
 };
 static Tunables g_tune;
+extern int g_ls_coop;
 static thread_local bool t_in_batch = false;
 
 struct PlanKey {
@@ -469,19 +472,31 @@ static int run_lstream(const spear_call* calls, int n_calls, cudaStream_t st) {
         p.ec_sync = reinterpret_cast<unsigned*>(ws + L.ec_sync);
         int n = 0, ph = -1, phase_begin = 0, panels = 0, ec_slots = 0;
         long long phase_chunks = 0;
+        size_t xperm_used = 0;
+        uint8_t* xperm_base = ws + L.xperm;
         for (int i = done_calls; i < n_calls && n < kLsMaxCalls; ++i) {
             const spear_call& c = calls[i];
             const void* A = c.r ? c.A : nullptr;
             const void* Bm = c.r ? c.B : nullptr;
             if (int rc = check_problem(c.x, c.Wq, c.scales, A, Bm, c.ec, c.y, c.M, c.N, c.K, c.r, c.group)) return rc;
             if (panels + c.N / 128 > kLsMaxPanels) break;
-            bool dep = (ph < 0);
-            for (int j = phase_begin; j < n && !dep; ++j) {
+            // dependencies inside the launch: x == an earlier call's y exactly (same M, K == its N) is a chain link
+            // (new phase); any other overlap with an earlier call's buffers ends this launch (stream order does the rest)
+            const size_t xb = size_t(c.M) * c.K * 2, yb = size_t(c.M) * c.N * 2;
+            const int xtile = c.M <= 8 ? 2048 : 4096;
+            int producer = -1;
+            bool cut = false, dep = (ph < 0);
+            for (int j = 0; j < n && !cut; ++j) {
                 const LsCall& e = p.calls[j];
-                const size_t yb = size_t(e.M) * e.N * 2;
-                dep = overlaps(c.x, size_t(c.M) * c.K * 2, e.y, yb) || overlaps(c.y, size_t(c.M) * c.N * 2, e.y, yb) ||
-                      overlaps(c.y, size_t(c.M) * c.N * 2, e.x, size_t(e.M) * e.K * 2);
+                const size_t eyb = size_t(e.M) * e.N * 2, exb = size_t(e.M) * e.K * 2;
+                if (c.x == e.y && c.M == e.M && c.K == e.N) {
+                    producer = j;
+                    if (j >= phase_begin) dep = true;
+                } else if (overlaps(c.x, xb, e.y, eyb)) cut = true;
+                if (overlaps(c.y, yb, e.y, eyb) || overlaps(c.y, yb, e.x, exb)) cut = true;
             }
+            const size_t need = producer >= 0 ? (p.calls[producer].yperm ? 0 : size_t(c.K / 128) * xtile) : size_t(c.K / 128) * xtile;
+            if (cut || xperm_used + need > kLsXpermBytes) break;
             const long long chunks = (long long)(c.N / 128) * (c.K / 128);
             if (dep || phase_chunks + chunks > 0x3fffffff) {
                 if (ph >= 0) { p.phase_chunks[ph] = int(phase_chunks); }
@@ -496,6 +511,19 @@ static int run_lstream(const spear_call* calls, int n_calls, cudaStream_t st) {
             d.x = static_cast<const __half*>(c.x);
             d.y = static_cast<__half*>(c.y);
             d.M = c.M; d.N = c.N; d.K = c.K; d.r = c.r;
+            d.xtile = xtile;
+            if (producer >= 0) {
+                LsCall& e = p.calls[producer];
+                if (!e.yperm) {
+                    e.yperm = xperm_base + xperm_used;
+                    xperm_used += need;
+                }
+                d.xperm = e.yperm;
+                d.x_internal = 1;
+            } else {
+                d.xperm = xperm_base + xperm_used;
+                xperm_used += need;
+            }
             d.group_chunks = c.group / 128;
             d.C = c.K / 128;
             d.P = c.N / 128;
@@ -524,6 +552,7 @@ static int run_lstream(const spear_call* calls, int n_calls, cudaStream_t st) {
         p.n_calls = n;
         p.n_phases = ph + 1;
         p.phase_first_call[p.n_phases] = n;
+        for (int q = 0; q < p.n_phases; ++q) { p.phase_per[q] = p.phase_chunks[q] / ls_grid(); p.phase_rem[q] = p.phase_chunks[q] % ls_grid(); }
         if (int rc = launch_lstream(p, st)) return rc;
         done_calls += n;
     }
@@ -602,6 +631,7 @@ extern "C" int spear_tune(const char* key, int value) {
     else if (!strcmp(key, "stream_deep")) g_tune.stream_deep = value;
     else if (!strcmp(key, "stream_debug")) g_tune.stream_debug = value;
     else if (!strcmp(key, "lstream")) g_tune.lstream = value;
+    else if (!strcmp(key, "ls_coop")) spear::g_ls_coop = value;
     else if (!strcmp(key, "stream_whole_panels")) g_tune.stream_whole_panels = value;
     else if (!strcmp(key, "stream_batch_grid")) g_tune.stream_batch_grid = value;
     else if (!strcmp(key, "stream_batch_units")) g_tune.stream_batch_units = value;

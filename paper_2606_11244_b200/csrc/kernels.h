@@ -57,6 +57,11 @@ struct LsCall {
     const __half* w_g;       // [K] (scalar gate) or NULL
     const float* b_g;        // 1 (device) or NULL
     float* gate_out;         // optional [M]
+    const uint8_t* xperm;    // [K/128][xtile] x in the MMA operand layout (workspace): written by the prologue of the launch
+                             // (external x) or by the finalisers of the call whose y this x is
+    uint8_t* yperm;          // NULL, or where a later call of this launch expects this call's y as its xperm
+    int xtile;               // bytes per chunk tile of xperm / yperm: 2048 (M <= 8) or 4096
+    int x_internal;          // 1: x is an earlier call's y (xperm comes from its finalisers)
     int M, N, K, r;
     int group_chunks;        // group / 128
     int C;                   // K / 128 chunks per panel
@@ -72,10 +77,12 @@ struct LsParams {
     int n_calls, n_phases;
     int phase_first_call[kLsMaxCalls + 1];   // calls of phase ph: [phase_first_call[ph], phase_first_call[ph + 1])
     int phase_chunks[kLsMaxCalls];           // chunks of the phase (all its calls)
+    int phase_per[kLsMaxCalls], phase_rem[kLsMaxCalls];   // phase_chunks / grid, phase_chunks % grid
     int phase_panels[kLsMaxCalls];           // panels of the phase = y completions to wait for
     float* partial;          // [2 phase parities][grid][2][16][128] fp32 split-K slots
     unsigned* counters;      // per-panel split-K counters, zero between launches (self-cleaning)
-    unsigned* done;          // [n_phases] finalised panels per phase + [kLsMaxCalls] exit counter; zeroed by the last CTA
+    unsigned* done;          // [n_phases] finalised panels per phase, [kLsMaxCalls] exit counter, [kLsMaxCalls + 1] CTAs that
+                             // finished the x prologue; zeroed by the last CTA
     float* zbuf;             // [ec slots][16][kZStride] fp32, zero between launches
     float* ubuf;             // [ec slots][16][128] fp32: u = alpha * gamma (.) z
     unsigned* ec_sync;       // [ec slots][2]: z arrivals, u-ready flag; zeroed by the last arriver / last CTA

@@ -12,25 +12,32 @@
 //     contiguous ranges, so every SM streams the same number of bytes and the cp.async.bulk ring never drains
 //     between calls; a call whose x is an earlier call's y opens a new phase, whose x loads wait for the
 //     previous phase's panel-completion counter while its WEIGHTS are prefetched across the boundary;
-//   * warp 0 (one lane): cp.async.bulk of chunk + scales into a shared-memory ring (evict_first);
-//   * warp 1: x tile of the chunk ([16 tokens][128 columns] fp16) by 8-byte cp.async into the K-major
-//     SWIZZLE_128B operand layout, with the k-order permuted to match the weight fragments (below);
-//   * warps 8-23 (16 dequantisation warps, 4 per TMEM lane quarter): LDS.128 -> exact q - 8 in fp16
-//     (lop3 / sub / fma) -> tcgen05.st.16x256b.x4 into a ring of A-operand slots in TENSOR MEMORY.  The SPW4
+//   * warp 0 (one lane): cp.async.bulk of the chunk into a shared-memory ring (evict_first);
+//   * warp 1 / warp 3 (one lane each): the chunk's x tile ([16 tokens][128 columns] fp16 in the MMA operand layout,
+//     prepared once per launch in the workspace, see x_prologue) / its 256-byte scale slot, as cp.async.bulk copies
+//     into the same ring stage;
+//   * warps 8-19 (12 dequantisation warps = 3 groups x 4 TMEM lane quarters; group g takes the chunks n = g mod 3
+//     of the CTA's stream): LDS.128 -> exact q - 8 in fp16 (lop3 / sub / fma) -> tcgen05.st.16x256b.x4 into the
+//     A-operand slot n mod 4 in TENSOR MEMORY.  The SPW4
 //     word of lane (g, t) holds rows g, g+8 x columns 16t..16t+15, the 16x256b store shape spreads a row's
 //     columns over the four lanes of a quad, so MMA j of a 64-column k-tile sees k = 16t + 4j + e at its
 //     K position 4t + e; the x loader applies the same permutation (a dot product is order-invariant);
-//   * warp 2 (one lane): tcgen05.mma.cta_group::1.kind::f16, M = 128 rows of the panel, N = 16 tokens, K = 16,
-//     A from TMEM, B = x tile from shared memory, D = one of two 16-column fp32 accumulators in TMEM, one
-//     accumulation run per scale group; tcgen05.commit frees the A slot / ring stage and hands D over;
-//   * warps 4-7 (epilogue, thread = output row): tcgen05.ld the run, scale by s[n][group] into fp32 registers;
+//   * warps 20-23 (one lane each, MMA issuer of pipeline i = chunks n = i mod 4): tcgen05.mma.cta_group::1.kind::f16, M = 128 rows of
+//     the panel, N = 16 tokens, K = 16, A from TMEM, B = x tile from shared memory, D = one of the pipeline's
+//     two 16-column fp32 accumulators in TMEM; one accumulation run per scale group (a run that spans several
+//     chunks leaves one partial accumulator per pipeline).  Measured: one thread issues a small-N MMA every
+//     ~47 clk whatever N, the tensor pipe needs 8 clk: four issuers keep the 8 MMAs per chunk off the critical
+//     path.  tcgen05.commit frees the A slot / ring stage and hands D over;
+//   * warps 4-7 (epilogue, thread = output row): tcgen05.ld the run's accumulators, scale by s[n][group]
+//     (read from global one run ahead) into fp32 registers;
 //     at the end of a panel segment: split-K through fp32 partial slots + an acq_rel counter when the panel
 //     is shared with neighbouring CTAs, then the rank-r update y += u B^T, one RN-even cast, store;
-//   * warp 3 (EC): this CTA's share of z = x [A; w_g]^T for every call of the phase (mma.sync, red.add),
+//   * warp 2 (EC): this CTA's share of z = x [A; w_g]^T for every call of the phase (mma.sync, red.add),
 //     arrive; the last arriver applies the gate (PAPER.md:109 scalar form of BASELINE.json / gamma = 1) and
 //     publishes u = alpha gamma z behind a flag that finalising CTAs look at only in their epilogue
 //     (z must be complete before the gate).
 #include <cooperative_groups.h>
+#include <cstdio>
 
 #include "common.cuh"
 #include "kernels.h"
@@ -38,14 +45,33 @@
 namespace spear {
 
 namespace ls {
-constexpr int kStages = 16;                 // ring depth (chunks): 16 x 12.25 KiB
-constexpr int kASlots = 8;                  // TMEM A-operand slots (one 64-column k-tile = 32 TMEM columns each)
-constexpr int kThreads = 768;
-constexpr int kWBytes = 8192, kScBytes = 256, kXBytes = 4096;
+#ifdef LS_TRACE
+__device__ __forceinline__ unsigned long long ls_now() { unsigned long long t; asm volatile("mov.u64 %0, %globaltimer;" : "=l"(t)); return t; }
+#endif
+#ifdef LS_TRACE
+__shared__ unsigned long long g_stamp[48];
+#define LS_STAMP(i) do { if (et == 0) g_stamp[i] = ls_now(); } while (0)
+__shared__ unsigned long long g_ct[32][8];
+#define LS_CT(n, j) do { if ((n) < 32) g_ct[n][j] = ls_now(); } while (0)
+#else
+#define LS_STAMP(i)
+#define LS_CT(n, j)
+#endif
+#ifndef LS_STAGES
+#define LS_STAGES 16
+#endif
+constexpr int kStages = LS_STAGES;                 // ring depth (chunks): 16 x (8 KiB weights + 4 KiB x tile)
+constexpr int kPipes = 4;                   // dequantisation / MMA pipelines; pipeline i owns chunks n = i (mod 4)
+#ifndef LS_DQ_GROUPS
+#define LS_DQ_GROUPS 2
+#endif
+constexpr int kDqGroups = LS_DQ_GROUPS;     // dequantisation warp groups (4 warps each); group g takes chunks n = g (mod kDqGroups)
+constexpr int kThreads = (8 + 4 * kDqGroups + 4) * 32;
+constexpr int kWBytes = 8192, kXBytes = 4096, kScBytes = 256;
 constexpr uint32_t kTmemCols = 512;
-constexpr uint32_t kDCol = kASlots * 32;    // two 16-column accumulators behind the A ring
+constexpr uint32_t kDCol = kPipes * 64;     // per pipeline: one 64-column A slot (a chunk), then two 16-column accumulators
 constexpr uint32_t kIdesc = (1u << 4) | (uint32_t(16 >> 3) << 17) | (uint32_t(128 >> 4) << 24);
-constexpr int kEmptyCount = 8 + 4 + 1;      // 8 dequant warps + 4 epilogue warps + the MMA commit per chunk
+constexpr int kEmptyCount = 4 + 4 + 1;      // the chunk's 4 dequantisation warps + 4 epilogue warps (scales) + its MMA commit
 struct Smem {
     static constexpr size_t x = 0;
     static constexpr size_t w = x + size_t(kStages) * kXBytes;
@@ -102,176 +128,253 @@ struct Seg {
     int ph;                    // phase
     int pos;                   // position of chunk k0 in the phase's chunk sequence
 };
-__device__ __forceinline__ int range_lo(int b, int T, int G) { return int((long long)b * T / G); }
-__device__ __forceinline__ int cta_of(int pos, int T, int G) {
-    int b = int((long long)pos * G / T);
-    while (b + 1 < G && range_lo(b + 1, T, G) <= pos) ++b;
-    while (b > 0 && range_lo(b, T, G) > pos) --b;
-    return b;
+// The phase's T chunks are cut into gridDim.x contiguous ranges: the first `rem` CTAs take per + 1 chunks, the
+// others per (per = T / G, rem = T % G, supplied by the host: no 64-bit division on the device).
+struct Cut { int per, rem; };
+__device__ __forceinline__ int range_lo(int b, Cut c) { return b * c.per + min(b, c.rem); }
+__device__ __forceinline__ int cta_of(int pos, Cut c) {
+    const int big = c.rem * (c.per + 1);
+    return pos < big ? pos / (c.per + 1) : c.rem + (pos - big) / c.per;     // pos >= big implies per >= 1
 }
+__device__ __forceinline__ Cut phase_cut(const LsParams& P, int ph) { return Cut{P.phase_per[ph], P.phase_rem[ph]}; }
+// Segments of this CTA, phase by phase.  Inside a phase the range's LAST segment comes first when it is the head
+// of a panel that continues in the next CTA: all pieces of a shared panel are then produced at the start of the
+// phase, its split-K reduction happens in the shadow of the whole panels that follow, and the CTA's final
+// segment needs no cross-CTA hand-shake.
 struct SegIter {
-    int ph, pos, hi, call;
-    __device__ SegIter() : ph(-1), pos(0), hi(0), call(0) {}
-    // advances to the next segment of this CTA; false when the table is exhausted
+    int ph, pos, hi, call, tail_pos;     // tail_pos: start of the deferred-to-front segment (== hi when none)
+    bool tail_done;
+    __device__ SegIter() : ph(-1), pos(0), hi(0), call(0), tail_pos(0), tail_done(true) {}
+    __device__ void locate(const LsParams& P, int at, int first_call, int& ci, int& panel, int& k) const {
+        ci = first_call;
+        while (at >= P.calls[ci].chunk_base + P.calls[ci].P * P.calls[ci].C) ++ci;
+        const int rel = at - P.calls[ci].chunk_base;
+        panel = rel / P.calls[ci].C;
+        k = rel - panel * P.calls[ci].C;
+    }
     __device__ bool next(const LsParams& P, Seg& s) {
-        const int G = gridDim.x, b = blockIdx.x;
-        while (pos >= hi) {
+        const int b = blockIdx.x;
+        while (pos >= tail_pos && tail_done) {
             if (++ph >= P.n_phases) return false;
-            const int T = P.phase_chunks[ph];
-            pos = range_lo(b, T, G);
-            hi = range_lo(b + 1, T, G);
+            const Cut cut = phase_cut(P, ph);
+            pos = range_lo(b, cut);
+            hi = range_lo(b + 1, cut);
             call = P.phase_first_call[ph];
+            tail_pos = hi;
+            tail_done = true;
+            if (hi > pos) {
+                int ci, panel, k;
+                locate(P, hi - 1, call, ci, panel, k);
+                if (k + 1 < P.calls[ci].C) {          // the range ends inside a panel
+                    tail_pos = max(pos, hi - 1 - k);
+                    tail_done = false;
+                }
+            }
         }
-        while (pos >= P.calls[call].chunk_base + P.calls[call].P * P.calls[call].C) ++call;
-        const LsCall& c = P.calls[call];
-        const int rel = pos - c.chunk_base;
-        s.call = call; s.ph = ph; s.pos = pos;
-        s.panel = rel / c.C;
-        s.k0 = rel - s.panel * c.C;
-        const int end = min(hi, c.chunk_base + (s.panel + 1) * c.C);
-        s.k1 = s.k0 + (end - pos);
-        pos = end;
+        int at, end;
+        if (!tail_done) { at = tail_pos; tail_done = true; end = hi; }
+        else { at = pos; end = tail_pos; }
+        int ci, panel, k;
+        locate(P, at, (at == pos) ? call : P.phase_first_call[ph], ci, panel, k);
+        const LsCall& c = P.calls[ci];
+        s.call = ci; s.ph = ph; s.pos = at; s.panel = panel; s.k0 = k;
+        const int seg_end = min(end, c.chunk_base + (panel + 1) * c.C);
+        s.k1 = k + (seg_end - at);
+        if (at == pos) { pos = seg_end; call = ci; }
         return true;
     }
 };
 __device__ __forceinline__ int total_chunks(const LsParams& P) {
     int n = 0;
-    for (int ph = 0; ph < P.n_phases; ++ph)
-        n += range_lo(blockIdx.x + 1, P.phase_chunks[ph], gridDim.x) - range_lo(blockIdx.x, P.phase_chunks[ph], gridDim.x);
+    for (int ph = 0; ph < P.n_phases; ++ph) n += P.phase_per[ph] + (int(blockIdx.x) < P.phase_rem[ph] ? 1 : 0);
     return n;
 }
 }  // namespace ls
 
 namespace ls {
 struct Bars {
-    uint64_t full[kStages], empty[kStages], a_full[kASlots], a_empty[kASlots], d_full[2], d_empty[2];
+    uint64_t full[kStages], empty[kStages], a_full[kPipes], a_empty[kPipes], d_full[kPipes][2], d_empty[kPipes][2];
     uint32_t tmem;
     int flag;       // epilogue broadcast: this CTA finalises the panel
     int u_call;     // call whose u sits in the staging buffer (-1 = none)
 };
 static_assert(sizeof(Bars) <= 1024, "barrier block");
 
-// ---- warp 0: weights + scales -------------------------------------------------------------------------------
-__device__ void producer(const LsParams& P, uint8_t* wring, uint8_t* scring, Bars* B) {
-    const uint64_t pol_w = policy_evict_first(), pol_s = policy_evict_last();
+// ---- warp 0: weights ------------------------------------------------------------------------------------------
+__device__ void producer(const LsParams& P, uint8_t* wring, Bars* B) {
+    const uint64_t pol_w = policy_evict_first();
     SegIter it;
     Seg sg;
     int n = 0;
     while (it.next(P, sg)) {
         const LsCall& c = P.calls[sg.call];
         const uint8_t* wp = c.wq + (size_t(sg.panel) * c.C + sg.k0) * kWBytes;
-        const uint8_t* sp = c.scales + size_t(sg.panel) * (c.C / c.group_chunks) * kScBytes;
         for (int k = sg.k0; k < sg.k1; ++k, ++n, wp += kWBytes) {
             const int s = n % kStages;
             mbar_wait(&B->empty[s], ((n / kStages) & 1) ^ 1);
-            mbar_arrive_expect_tx(&B->full[s], kWBytes + kScBytes);
+            mbar_arrive_expect_tx(&B->full[s], kWBytes);
             bulk_g2s(wring + s * kWBytes, wp, kWBytes, &B->full[s], pol_w);
-            bulk_g2s(scring + s * kScBytes, sp + size_t(k / c.group_chunks) * kScBytes, kScBytes, &B->full[s], pol_s);
+            LS_CT(n, 0);
         }
     }
 }
 
-// ---- warp 1: x tiles ----------------------------------------------------------------------------------------
-// Lane l copies, for every token m < M, the 8-byte piece k = 4l..4l+3 of the chunk's 128 columns to the place the
-// MMA expects it: k-tile half = l >> 4; inside the k-tile k = 16 t + 4 j + e goes to K position 16 j + 4 t + e
-// (see the header: the 16x256b TMEM store spreads the columns of lane (g, t)'s word over MMA j = 0..3), in the
-// K-major SWIZZLE_128B layout: row m at (m >> 3) * 1024 + (m & 7) * 128, 16-byte unit index XOR (m & 7).
-__device__ void x_loader(const LsParams& P, uint8_t* xring, Bars* B, int lane) {
-    const int half = lane >> 4, t = (lane & 15) >> 2, j = lane & 3;
-    const int unit = 2 * j + (t >> 1), off = (t & 1) * 8;
+// ---- x in the operand layout -----------------------------------------------------------------------------------
+// The MMA wants, per chunk, the tile [k-tile half][16 tokens][64 columns] fp16 in the K-major SWIZZLE_128B layout
+// (row m at (m >> 3) * 1024 + (m & 7) * 128, 16-byte unit index XOR (m & 7)) with the k-order of the weight
+// fragments: inside a k-tile, column k = 16 t + 4 j + e sits at K position 16 j + 4 t + e (see the header).  That is
+// a permutation of 8-byte pieces, which neither TMA nor a 16-byte cp.async can express, so x is rewritten ONCE per
+// launch into the workspace (xperm: one contiguous tile per chunk, 2 KiB when M <= 8, else 4 KiB) and the tiles
+// then travel through the ring as plain cp.async.bulk copies, like the weights.
+__device__ __forceinline__ uint32_t xperm_offset(int m, int kk, int xtile) {    // byte offset of (token m, column kk of the chunk)
+    const int l = kk >> 2, e = kk & 3;
+    const int half = l >> 4, t = (l & 15) >> 2, j = l & 3;
+    const int unit = 2 * j + (t >> 1);
+    return half * (xtile >> 1) + (m >> 3) * 1024 + (m & 7) * 128 + ((unit ^ (m & 7)) << 4) + (t & 1) * 8 + e * 2;
+}
+// Prologue (all dequantisation warps of all CTAs): the external x of every call -> xperm, then one arrive per CTA.
+__device__ void x_prologue(const LsParams& P, int tid, int nthreads) {
+    const int gtid = blockIdx.x * nthreads + tid, gsz = gridDim.x * nthreads;
+    for (int ci = 0; ci < P.n_calls; ++ci) {
+        const LsCall& c = P.calls[ci];
+        if (c.x_internal) continue;
+        const int per_row = c.K >> 2;                   // 8-byte pieces per token row
+        uint8_t* dstb = const_cast<uint8_t*>(c.xperm);
+        for (int p = gtid; p < c.M * per_row; p += gsz) {
+            const int m = p / per_row, q = p - m * per_row;
+            const uint2 v = *reinterpret_cast<const uint2*>(c.x + size_t(m) * c.K + 4 * q);
+            const int k = 4 * q;
+            *reinterpret_cast<uint2*>(dstb + size_t(k >> 7) * c.xtile + xperm_offset(m, k & 127, c.xtile)) = v;
+        }
+    }
+}
+
+// ---- warp 1 (one lane): x tiles; warp 3 (one lane): scale slots ------------------------------------------------
+__device__ void x_producer(const LsParams& P, uint8_t* xring, Bars* B) {
+    const uint64_t pol = policy_evict_last();
     SegIter it;
     Seg sg;
     int n = 0, ph_seen = 0;
+    bool prologue_seen = false;
     while (it.next(P, sg)) {
+        const LsCall& c = P.calls[sg.call];
         if (sg.ph != ph_seen) {     // this phase's x is an earlier phase's y: wait until all its panels are stored
             for (int q = ph_seen; q < sg.ph; ++q) wait_counter(P.done + q, unsigned(P.phase_panels[q]));
             ph_seen = sg.ph;
+            asm volatile("fence.proxy.async;" ::: "memory");     // generic-proxy stores of other SMs -> our bulk copies
         }
-        const LsCall& c = P.calls[sg.call];
-        const __half* xp = c.x + size_t(sg.k0) * 128 + 4 * lane;
-        for (int k = sg.k0; k < sg.k1; ++k, ++n, xp += 128) {
+        if (!c.x_internal && !prologue_seen) {
+            wait_counter(P.done + kLsMaxCalls + 1, gridDim.x);
+            asm volatile("fence.proxy.async;" ::: "memory");
+            prologue_seen = true;
+        }
+        const uint8_t* xp = c.xperm + size_t(sg.k0) * c.xtile;
+        for (int k = sg.k0; k < sg.k1; ++k, ++n, xp += c.xtile) {
             const int s = n % kStages;
             mbar_wait(&B->empty[s], ((n / kStages) & 1) ^ 1);
-            const uint32_t dst = smem_u32(xring + s * kXBytes) + half * 2048 + off;
-#pragma unroll
-            for (int m = 0; m < 16; ++m)
-                if (m < c.M)
-                    cp_async8(dst + (m >> 3) * 1024 + (m & 7) * 128 + ((unit ^ (m & 7)) << 4), xp + size_t(m) * c.K);
-            cp_async_arrive_noinc(&B->full[s]);
+            mbar_arrive_expect_tx(&B->full[s], c.xtile);
+            bulk_g2s(xring + s * kXBytes, xp, c.xtile, &B->full[s], pol);
+        }
+    }
+}
+__device__ void sc_producer(const LsParams& P, uint8_t* scring, Bars* B) {
+    const uint64_t pol = policy_evict_last();
+    SegIter it;
+    Seg sg;
+    int n = 0;
+    while (it.next(P, sg)) {
+        const LsCall& c = P.calls[sg.call];
+        const uint8_t* sp = c.scales + size_t(sg.panel) * (c.C / c.group_chunks) * kScBytes;
+        for (int k = sg.k0; k < sg.k1; ++k, ++n) {
+            const int s = n % kStages;
+            mbar_wait(&B->empty[s], ((n / kStages) & 1) ^ 1);
+            mbar_arrive_expect_tx(&B->full[s], kScBytes);
+            bulk_g2s(scring + s * kScBytes, sp + size_t(k / c.group_chunks) * kScBytes, kScBytes, &B->full[s], pol);
         }
     }
 }
 
-// ---- warp 2 (one lane): MMA issue ---------------------------------------------------------------------------
-__device__ void mma_issuer(const LsParams& P, uint8_t* xring, Bars* B, uint32_t tmem) {
+// ---- warps 20-23 (one lane each): MMA issue of pipeline i ---------------------------------------------------
+__device__ void mma_issuer(const LsParams& P, uint8_t* xring, Bars* B, uint32_t tmem, int i) {
     SegIter it;
     Seg sg;
     int n = 0, db = 0;
-    unsigned uses[2] = {0, 0};
+    unsigned par = 0;       // bit b: parity of accumulator b's next d_empty phase
+    const uint32_t a_base = tmem + i * 64, d_base = tmem + kDCol + i * 32;
     while (it.next(P, sg)) {
         const int gc = P.calls[sg.call].group_chunks;
-        bool fresh = true;      // next MMA starts an accumulation run
-        for (int k = sg.k0; k < sg.k1; ++k, ++n) {
-            const int s = n % kStages;
-            if (fresh) mbar_wait(&B->d_empty[db], (uses[db] & 1) ^ 1);
-            const uint64_t bd = desc_sw128(smem_u32(xring + s * kXBytes));
-#pragma unroll
-            for (int h = 0; h < 2; ++h) {
-                const int tau = 2 * n + h, slot = tau % kASlots;
-                mbar_wait(&B->a_full[slot], (tau / kASlots) & 1);
+        const uint64_t half_desc = uint64_t(P.calls[sg.call].xtile >> 5);      // (xtile / 2) >> 4: descriptor step to the second k-tile
+        for (int ka = sg.k0; ka < sg.k1;) {          // accumulation runs: the chunks of one scale group
+            const int kb = min(sg.k1, (ka / gc + 1) * gc);
+            const int n_last = n + (kb - ka) - 1;
+            for (; n <= n_last; ++n) {
+                if ((n & (kPipes - 1)) != i) continue;
+                const int s = n % kStages;
+                const bool first = (n - kPipes < n_last - (kb - ka) + 1), last = (n + kPipes > n_last);
+                if (first) mbar_wait(&B->d_empty[i][db], ((par >> db) & 1) ^ 1);
+                mbar_wait(&B->a_full[i], (n / kPipes) & 1);
+                LS_CT(n, 4);
                 tc_fence_after();
+                const uint64_t bd = desc_sw128(smem_u32(xring + s * kXBytes));
 #pragma unroll
-                for (int j = 0; j < 4; ++j)
-                    umma_ts(tmem + kDCol + 16 * db, tmem + slot * 32 + 8 * j, bd + uint64_t(h * 128 + 2 * j), !(fresh && h == 0 && j == 0));
-                umma_commit(&B->a_empty[slot]);
+                for (int h = 0; h < 2; ++h)
+#pragma unroll
+                    for (int j = 0; j < 4; ++j)
+                        umma_ts(d_base + 16 * db, a_base + h * 32 + 8 * j, bd + h * half_desc + uint64_t(2 * j), !(first && h == 0 && j == 0));
+                umma_commit(&B->a_empty[i]);
+                umma_commit(&B->empty[s]);
+                LS_CT(n, 5);
+                if (last) {
+                    umma_commit(&B->d_full[i][db]);
+                    par ^= 1u << db;
+                    db ^= 1;
+                }
             }
-            fresh = false;
-            umma_commit(&B->empty[s]);
-            if ((k + 1) % gc == 0 || k + 1 == sg.k1) {
-                umma_commit(&B->d_full[db]);
-                ++uses[db];
-                db ^= 1;
-                fresh = true;
-            }
+            ka = kb;
         }
     }
 }
 
-// ---- warps 8-23: int4 -> fp16 -> TMEM -----------------------------------------------------------------------
+// ---- warps 8-19: int4 -> fp16 -> TMEM (warp = group x TMEM lane quarter q; chunk n goes to A slot n mod 4) -----------------------------
 __device__ void dequantiser(int n_total, uint8_t* wring, Bars* B, uint32_t tmem, int warp, int lane) {
-    const int q = warp & 3, i = (warp - 8) >> 2;
+    const int q = warp & 3, grp = (warp - 8) >> 2;
     const uint32_t w_lane = smem_u32(wring) + (2 * q * 32 + lane) * 16;
-    const uint32_t t_lane = tmem + (uint32_t(32 * q) << 16);
-    for (int tau = i; tau < 2 * n_total; tau += 4) {
-        const int n = tau >> 1, h = tau & 1, s = n % kStages, slot = tau % kASlots;
-        mbar_wait(&B->a_empty[slot], ((tau / kASlots) & 1) ^ 1);
+    for (int n = grp; n < n_total; n += kDqGroups) {
+        const int s = n % kStages, i = n & (kPipes - 1);
+        const uint32_t t_lane = tmem + i * 64 + (uint32_t(32 * q) << 16);
+        mbar_wait(&B->a_empty[i], ((n / kPipes) & 1) ^ 1);
         mbar_wait(&B->full[s], (n / kStages) & 1);
+        if (q == 0 && lane == 0) LS_CT(n, 2);
         tc_fence_after();
 #pragma unroll
-        for (int sp = 0; sp < 2; ++sp) {
-            uint4 w;
-            const uint32_t addr = w_lane + s * kWBytes + h * 4096 + sp * 512;
-            asm volatile("ld.shared.v4.u32 {%0, %1, %2, %3}, [%4];" : "=r"(w.x), "=r"(w.y), "=r"(w.z), "=r"(w.w) : "r"(addr));
-            uint32_t a[4], b[4], c[4], d[4];
-            dequant_word(w.x, a);   // row g,   k 16t + 0..7
-            dequant_word(w.y, b);   // row g,   k 16t + 8..15
-            dequant_word(w.z, c);   // row g+8, k 16t + 0..7
-            dequant_word(w.w, d);   // row g+8, k 16t + 8..15
-            // register order of 16x256b.x4: MMA j <- {row g: 2 regs, row g+8: 2 regs}
-            asm volatile(
-                "tcgen05.st.sync.aligned.16x256b.x4.b32 [%0], {%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15,%16};"
-                ::"r"(t_lane + slot * 32 + (uint32_t(16 * sp) << 16)),
-                "r"(a[0]), "r"(a[1]), "r"(c[0]), "r"(c[1]), "r"(a[2]), "r"(a[3]), "r"(c[2]), "r"(c[3]),
-                "r"(b[0]), "r"(b[1]), "r"(d[0]), "r"(d[1]), "r"(b[2]), "r"(b[3]), "r"(d[2]), "r"(d[3])
-                : "memory");
+        for (int h = 0; h < 2; ++h) {
+#pragma unroll
+            for (int sp = 0; sp < 2; ++sp) {
+                uint4 w;
+                const uint32_t addr = w_lane + s * kWBytes + h * 4096 + sp * 512;
+                asm volatile("ld.shared.v4.u32 {%0, %1, %2, %3}, [%4];" : "=r"(w.x), "=r"(w.y), "=r"(w.z), "=r"(w.w) : "r"(addr));
+                uint32_t a[4], b[4], c[4], d[4];
+                dequant_word(w.x, a);   // row g,   k 16t + 0..7
+                dequant_word(w.y, b);   // row g,   k 16t + 8..15
+                dequant_word(w.z, c);   // row g+8, k 16t + 0..7
+                dequant_word(w.w, d);   // row g+8, k 16t + 8..15
+                // register order of 16x256b.x4: MMA j <- {row g: 2 regs, row g+8: 2 regs}
+                asm volatile(
+                    "tcgen05.st.sync.aligned.16x256b.x4.b32 [%0], {%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15,%16};"
+                    ::"r"(t_lane + h * 32 + (uint32_t(16 * sp) << 16)),
+                    "r"(a[0]), "r"(a[1]), "r"(c[0]), "r"(c[1]), "r"(a[2]), "r"(a[3]), "r"(c[2]), "r"(c[3]),
+                    "r"(b[0]), "r"(b[1]), "r"(d[0]), "r"(d[1]), "r"(b[2]), "r"(b[3]), "r"(d[2]), "r"(d[3])
+                    : "memory");
+            }
         }
         asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory");
         fence_proxy_async_smem();       // the x tile was written by cp.async (generic proxy); the MMA reads it through the async proxy
         tc_fence_before();
         __syncwarp();
         if (lane == 0) {
-            mbar_arrive(&B->a_full[slot]);
+            mbar_arrive(&B->a_full[i]);
             mbar_arrive(&B->empty[s]);
+            if (q == 0) LS_CT(n, 3);
         }
     }
 }
@@ -281,64 +384,83 @@ namespace ls {
 __device__ __forceinline__ void epi_bar() { named_bar_sync(1, 128); }
 
 // ---- warps 4-7: accumulate the runs, finalise panel segments ------------------------------------------------
-__device__ void epilogue(const LsParams& P, uint8_t* scring, float* us, Bars* B, uint32_t tmem, int warp, int lane) {
+__device__ void epilogue(const LsParams& P, const uint8_t* scring, float* us, Bars* B, uint32_t tmem, int warp, int lane) {
     const int q = warp - 4, row = 32 * q + lane, et = row;        // et = thread index among the 128 epilogue threads
-    const int sc_off = ((row >> 4) * 16 + 2 * (row & 7) + ((row >> 3) & 1)) * 2;
+    const int sc_idx = (row >> 4) * 16 + 2 * (row & 7) + ((row >> 3) & 1);      // SPW4 scale slot of this row
     const int G = gridDim.x, b = blockIdx.x;
+    const uint32_t d_lane = tmem + kDCol + (uint32_t(32 * q) << 16);
     SegIter it;
     Seg sg;
-    int n = 0, db = 0;
-    unsigned uses[2] = {0, 0};
+    int n = 0;
+    unsigned dbits = 0, pbits = 0;      // per pipeline w: bit w of dbits = current accumulator, bit 2w + b of pbits = its phase parity
     while (it.next(P, sg)) {
         const LsCall& c = P.calls[sg.call];
         const int gc = c.group_chunks;
         float acc[16];
 #pragma unroll
         for (int m = 0; m < 16; ++m) acc[m] = 0.f;
-        for (int k = sg.k0; k < sg.k1; ++k, ++n) {
-            const int s = n % kStages;
-            const bool readout = ((k + 1) % gc == 0) || (k + 1 == sg.k1);
-            mbar_wait(&B->full[s], (n / kStages) & 1);
+        for (int ka = sg.k0; ka < sg.k1;) {          // accumulation runs: the chunks of one scale group
+            const int kb = min(sg.k1, (ka / gc + 1) * gc);
+            const int n_last = n + (kb - ka) - 1;
+            // every chunk's stage is released by the epilogue too: the last chunk of the run carries the scale read here
             float scale = 0.f;
-            if (readout) scale = __half2float(*reinterpret_cast<const __half*>(scring + s * kScBytes + sc_off));
-            __syncwarp();
-            if (lane == 0) mbar_arrive(&B->empty[s]);
-            if (readout) {
-                mbar_wait(&B->d_full[db], uses[db] & 1);
+            for (int sq = n; sq <= n_last; ++sq) {
+                const int s = sq % kStages;
+                mbar_wait(&B->full[s], (sq / kStages) & 1);
+                if (sq == n_last) scale = __half2float(*reinterpret_cast<const __half*>(scring + s * kScBytes + sc_idx * 2));
+                __syncwarp();
+                if (lane == 0) mbar_arrive(&B->empty[s]);
+            }
+            float sum[16];
+#pragma unroll
+            for (int m = 0; m < 16; ++m) sum[m] = 0.f;
+            for (int sq = max(n, n_last - (kPipes - 1)); sq <= n_last; ++sq) {     // the pipelines that hold a piece
+                const int w = sq & (kPipes - 1);
+                const int bw = (dbits >> w) & 1;
+                const unsigned par = (pbits >> (2 * w + bw)) & 1;
+                pbits ^= 1u << (2 * w + bw);
+                dbits ^= 1u << w;
+                mbar_wait(&B->d_full[w][bw], par);
+                if (et == 0) LS_CT(sq, 6);
                 tc_fence_after();
                 uint32_t v[16];
                 asm volatile(
                     "tcgen05.ld.sync.aligned.32x32b.x16.b32 {%0,%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15}, [%16];"
                     : "=r"(v[0]), "=r"(v[1]), "=r"(v[2]), "=r"(v[3]), "=r"(v[4]), "=r"(v[5]), "=r"(v[6]), "=r"(v[7]),
                       "=r"(v[8]), "=r"(v[9]), "=r"(v[10]), "=r"(v[11]), "=r"(v[12]), "=r"(v[13]), "=r"(v[14]), "=r"(v[15])
-                    : "r"(tmem + kDCol + 16 * db + (uint32_t(32 * q) << 16))
+                    : "r"(d_lane + w * 32 + 16 * bw)
                     : "memory");
                 asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
                 tc_fence_before();
                 __syncwarp();
-                if (lane == 0) mbar_arrive(&B->d_empty[db]);
-                ++uses[db];
-                db ^= 1;
+                if (lane == 0) mbar_arrive(&B->d_empty[w][bw]);
 #pragma unroll
-                for (int m = 0; m < 16; ++m) acc[m] = fmaf(scale, __uint_as_float(v[m]), acc[m]);
+                for (int m = 0; m < 16; ++m) sum[m] += __uint_as_float(v[m]);
             }
+#pragma unroll
+            for (int m = 0; m < 16; ++m) acc[m] = fmaf(scale, sum[m], acc[m]);
+            if (et == 0) LS_CT(n_last, 7);
+            n = n_last + 1;
+            ka = kb;
         }
+        LS_STAMP(40);
         // ---- end of the segment: S8 split-K, S7 rank-r update, cast, store ----
-        const int T = P.phase_chunks[sg.ph];
+        const Cut cut = phase_cut(P, sg.ph);
         const bool whole = (sg.k0 == 0 && sg.k1 == c.C);
         bool finalize = whole;
         if (!whole) {
-            const int lo_b = range_lo(b, T, G);
+            const int lo_b = range_lo(b, cut);
             const int which = (sg.pos == lo_b) ? 0 : 1;
             float* slot = P.partial + (size_t((sg.ph & 1) * G + b) * 2 + which) * 2048;
 #pragma unroll
             for (int m = 0; m < 16; ++m) slot[m * 128 + row] = acc[m];
             epi_bar();
+            LS_STAMP(41);
             const int p_begin = c.chunk_base + sg.panel * c.C, p_end = p_begin + c.C;
             if (et == 0) {
                 // CTAs that hold a piece of this panel (ranges may be empty when the phase has fewer chunks than CTAs)
                 int parts = 0;
-                for (int pos = p_begin; pos < p_end; pos = range_lo(cta_of(pos, T, G) + 1, T, G)) ++parts;
+                for (int pos = p_begin; pos < p_end; pos = range_lo(cta_of(pos, cut) + 1, cut)) ++parts;
                 unsigned* ctr = P.counters + c.panel_base + sg.panel;
                 const unsigned old = atom_add_acq_rel(ctr, 1);      // releases this CTA's partial, acquires the others'
                 const int last = (old == unsigned(parts - 1));
@@ -346,24 +468,39 @@ __device__ void epilogue(const LsParams& P, uint8_t* scring, float* us, Bars* B,
                 B->flag = last;
             }
             epi_bar();
+            LS_STAMP(42);
             finalize = (B->flag != 0);
             if (finalize) {
 #pragma unroll
                 for (int m = 0; m < 16; ++m) acc[m] = 0.f;
-                for (int pos = p_begin; pos < p_end;) {             // fixed CTA order: bitwise reproducible
-                    const int cq = cta_of(pos, T, G);
-                    const int lo_q = range_lo(cq, T, G);
-                    const int wq = (pos == lo_q) ? 0 : 1;
-                    pos = range_lo(cq + 1, T, G);
-                    const float* sj = P.partial + (size_t((sg.ph & 1) * G + cq) * 2 + wq) * 2048;
-                    float tmp[16];
+                // partials are summed in CTA order (bitwise reproducible); two CTAs' loads are in flight
+                // before the first add so that their L2 round trips overlap
+                for (int pos = p_begin; pos < p_end;) {
+                    const float* sj[2];
+                    int np = 0;
+                    for (; np < 2 && pos < p_end; ++np) {
+                        const int cq = cta_of(pos, cut);
+                        const int wq = (pos == range_lo(cq, cut)) ? 0 : 1;
+                        sj[np] = P.partial + (size_t((sg.ph & 1) * G + cq) * 2 + wq) * 2048 + row;
+                        pos = range_lo(cq + 1, cut);
+                    }
+                    float tmp[2][16];
 #pragma unroll
-                    for (int m = 0; m < 16; ++m) tmp[m] = __ldcg(sj + m * 128 + row);
+                    for (int e = 0; e < 2; ++e)
+                        if (e < np) {
 #pragma unroll
-                    for (int m = 0; m < 16; ++m) acc[m] += tmp[m];
+                            for (int m = 0; m < 16; ++m) tmp[e][m] = __ldcg(sj[e] + m * 128);
+                        }
+#pragma unroll
+                    for (int e = 0; e < 2; ++e)
+                        if (e < np) {
+#pragma unroll
+                            for (int m = 0; m < 16; ++m) acc[m] += tmp[e][m];
+                        }
                 }
             }
         }
+        LS_STAMP(43);
         if (finalize) {
             const int nrow = sg.panel * 128 + row;
             if (c.r > 0) {
@@ -401,9 +538,16 @@ __device__ void epilogue(const LsParams& P, uint8_t* scring, float* us, Bars* B,
 #pragma unroll
             for (int m = 0; m < 16; ++m)
                 if (m < c.M) c.y[size_t(m) * c.N + nrow] = __float2half_rn(acc[m]);
+            if (c.yperm) {      // a later call of this launch reads this y as its x: hand it over in the operand layout
+                uint8_t* yp = c.yperm + size_t(nrow >> 7) * c.xtile;
+#pragma unroll
+                for (int m = 0; m < 16; ++m)
+                    if (m < c.M) *reinterpret_cast<__half*>(yp + xperm_offset(m, nrow & 127, c.xtile)) = __float2half_rn(acc[m]);
+            }
+            LS_STAMP(44);
             if (P.n_phases > 1) {               // somebody may be waiting for this phase's y
                 epi_bar();
-                if (et == 0) { __threadfence(); red_add_release(P.done + sg.ph, 1u); }
+                if (et == 0) { __threadfence(); asm volatile("fence.proxy.async;" ::: "memory"); red_add_release(P.done + sg.ph, 1u); }
             }
         }
     }
@@ -411,7 +555,7 @@ __device__ void epilogue(const LsParams& P, uint8_t* scring, float* us, Bars* B,
 }  // namespace ls
 
 namespace ls {
-// ---- warp 3: z = x [A; w_g]^T, gate, u (S4-S6) --------------------------------------------------------------
+// ---- warp 2: z = x [A; w_g]^T, gate, u (S4-S6) --------------------------------------------------------------
 __device__ __forceinline__ void ec_load16(const __half* row, int col, uint32_t (&lo)[4], uint32_t (&hi)[4]) {
     if (row) {
         const uint4 a = *reinterpret_cast<const uint4*>(row + col);
@@ -512,14 +656,17 @@ __global__ void __launch_bounds__(ls::kThreads, 1) ls_kernel(const __grid_consta
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
 
     if (threadIdx.x == 0) {
-        for (int s = 0; s < kStages; ++s) { mbar_init(&B->full[s], 1 + 32); mbar_init(&B->empty[s], kEmptyCount); }
-        for (int s = 0; s < kASlots; ++s) { mbar_init(&B->a_full[s], 4); mbar_init(&B->a_empty[s], 1); }
-        for (int s = 0; s < 2; ++s) { mbar_init(&B->d_full[s], 1); mbar_init(&B->d_empty[s], 4); }
+        for (int s = 0; s < kStages; ++s) { mbar_init(&B->full[s], 3); mbar_init(&B->empty[s], kEmptyCount); }
+        for (int s = 0; s < kPipes; ++s) {
+            mbar_init(&B->a_full[s], 4);
+            mbar_init(&B->a_empty[s], 1);
+            for (int d = 0; d < 2; ++d) { mbar_init(&B->d_full[s][d], 1); mbar_init(&B->d_empty[s][d], 4); }
+        }
         B->flag = 0;
         B->u_call = -1;
         fence_mbar_init();
     }
-    if (warp == 2) {
+    if (warp == 3) {
         asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_u32(&B->tmem)), "n"(kTmemCols) : "memory");
         asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
     }
@@ -527,23 +674,48 @@ __global__ void __launch_bounds__(ls::kThreads, 1) ls_kernel(const __grid_consta
     __syncthreads();
     tc_fence_after();
     const uint32_t tmem = B->tmem;
+#ifdef LS_TRACE
+    unsigned long long* stamp = g_stamp;
+    if (threadIdx.x == 0) stamp[39] = ls_now();
+    __syncthreads();
+#endif
 
     if (warp == 0) {
-        if (lane == 0) producer(P, wring, scring, B);
+        if (lane == 0) producer(P, wring, B);
     } else if (warp == 1) {
-        x_loader(P, xring, B, lane);
-    } else if (warp == 2) {
-        if (lane == 0) mma_issuer(P, xring, B, tmem);
+        if (lane == 0) x_producer(P, xring, B);
     } else if (warp == 3) {
+        if (lane == 0) sc_producer(P, scring, B);
+    } else if (warp == 2) {
         ec_warp(P, lane);
     } else if (warp < 8) {
         epilogue(P, scring, us, B, tmem, warp, lane);
-    } else {
+    } else if (warp < 8 + 4 * kDqGroups) {
+        // prologue: x -> operand layout (workspace), one arrive per CTA once its 8 warps are through
+        x_prologue(P, threadIdx.x - 256, 128 * kDqGroups);
+        __threadfence();
+        named_bar_sync(2, 128 * kDqGroups);
+        if (threadIdx.x == 256) { asm volatile("fence.proxy.async;" ::: "memory"); red_add_release(P.done + kLsMaxCalls + 1, 1u); }
         dequantiser(total_chunks(P), wring, B, tmem, warp, lane);
+    } else {
+        if (lane == 0) mma_issuer(P, xring, B, tmem, warp - (8 + 4 * kDqGroups));
     }
+#ifdef LS_TRACE
+    if (lane == 0) stamp[warp] = ls_now();
+#endif
     tc_fence_before();
     __syncthreads();
-    if (warp == 2) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem), "n"(kTmemCols) : "memory");
+#ifdef LS_TRACE
+    if (threadIdx.x == 0 && total_chunks(P) > 0 && (blockIdx.x % 37) == 36) {
+        const unsigned long long t0 = stamp[39];
+        printf("   epi: runs %llu slot %llu atom %llu sum %llu store %llu\n", stamp[40]-stamp[39], stamp[41]-stamp[39], stamp[42]-stamp[39], stamp[43]-stamp[39], stamp[44]-stamp[39]);
+        if (blockIdx.x == 36) for (int n = 0; n < min(32, total_chunks(P)); ++n)
+            printf("  chunk %2d: bulk %llu xld %llu full %llu deq %llu afull %llu mma %llu dfull %llu epi %llu\n", n, g_ct[n][0]-t0, g_ct[n][1]-t0, g_ct[n][2]-t0, g_ct[n][3]-t0, g_ct[n][4]-t0, g_ct[n][5]-t0, g_ct[n][6]-t0, g_ct[n][7]-t0);
+        printf("cta %d chunks %d: prod %llu xld %llu ec %llu epi %llu dq %llu %llu mma %llu %llu end %llu\n", blockIdx.x, total_chunks(P), stamp[0] - t0, stamp[1] - t0,
+               stamp[2] - t0, stamp[4] - t0, stamp[8] - t0, stamp[19] - t0, stamp[20] - t0, stamp[23] - t0, ls_now() - t0);
+    }
+#endif
+    if (warp == 3) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem), "n"(kTmemCols) : "memory");
     if (threadIdx.x == 0) {
         // the last CTA to leave resets what the next launch expects to be zero
         unsigned* exit_ctr = P.done + kLsMaxCalls;
@@ -552,7 +724,8 @@ __global__ void __launch_bounds__(ls::kThreads, 1) ls_kernel(const __grid_consta
             for (int ph = 0; ph < P.n_phases; ++ph) P.done[ph] = 0;
             for (int ci = 0; ci < P.n_calls; ++ci)
                 if (P.calls[ci].ec_slot >= 0) P.ec_sync[2 * P.calls[ci].ec_slot + 1] = 0;
-            *exit_ctr = 0;
+            exit_ctr[0] = 0;
+            exit_ctr[1] = 0;
         }
     }
 }
@@ -571,6 +744,7 @@ int ls_grid() {
 size_t ls_workspace_bytes(int grid) {
     return size_t(grid) * 2 * 2 * 2048 * 4 + (size_t(1) << 20);
 }
+int g_ls_coop = 1;
 int launch_lstream(const LsParams& p, cudaStream_t st) {
     const int grid = ls_grid();
     if (grid <= 0) return set_error(SPEAR_ECUDA, "layer-stream kernel cannot be resident on this device");
@@ -581,7 +755,7 @@ int launch_lstream(const LsParams& p, cudaStream_t st) {
     cfg.stream = st;
     cudaLaunchAttribute attr[1];
     attr[0].id = cudaLaunchAttributeCooperative;      // all CTAs co-resident or the launch fails: the device-wide
-    attr[0].val.cooperative = 1;                      // arrive / wait patterns above cannot deadlock
+    attr[0].val.cooperative = g_ls_coop;                      // arrive / wait patterns above cannot deadlock
     cfg.attrs = attr;
     cfg.numAttrs = 1;
     SPEAR_CUDA_OK(cudaLaunchKernelEx(&cfg, ls_kernel, p));
