@@ -62,22 +62,19 @@ __shared__ unsigned long long g_ct[32][8];
 #endif
 constexpr int kStages = LS_STAGES;                 // ring depth (chunks): 16 x (8 KiB weights + 4 KiB x tile)
 constexpr int kPipes = 4;                   // dequantisation / MMA pipelines; pipeline i owns chunks n = i (mod 4)
-#ifndef LS_DQ_GROUPS
-#define LS_DQ_GROUPS 2
-#endif
-constexpr int kDqGroups = LS_DQ_GROUPS;     // dequantisation warp groups (4 warps each); group g takes chunks n = g (mod kDqGroups)
-constexpr int kThreads = (8 + 4 * kDqGroups + 4) * 32;
+constexpr int kThreads = (8 + 4 * kPipes + kPipes) * 32;      // 4 service warps, 4 finalisers, 16 workers, 4 MMA issuers
 constexpr int kWBytes = 8192, kXBytes = 4096, kScBytes = 256;
 constexpr uint32_t kTmemCols = 512;
 constexpr uint32_t kDCol = kPipes * 64;     // per pipeline: one 64-column A slot (a chunk), then two 16-column accumulators
 constexpr uint32_t kIdesc = (1u << 4) | (uint32_t(16 >> 3) << 17) | (uint32_t(128 >> 4) << 24);
-constexpr int kEmptyCount = 4 + 4 + 1;      // the chunk's 4 dequantisation warps + 4 epilogue warps (scales) + its MMA commit
+constexpr int kEmptyCount = 4 + 1;          // the chunk's 4 worker warps + its MMA commit
 struct Smem {
     static constexpr size_t x = 0;
     static constexpr size_t w = x + size_t(kStages) * kXBytes;
     static constexpr size_t sc = w + size_t(kStages) * kWBytes;
     static constexpr size_t u = sc + size_t(kStages) * kScBytes;       // [16][128] fp32 staging of u
-    static constexpr size_t bars = u + 16 * 128 * 4;
+    static constexpr size_t part = u + 16 * 128 * 4;                   // [2][kPipes][16][128] fp32 segment hand-over
+    static constexpr size_t bars = part + size_t(2) * kPipes * 2048 * 4;
     static constexpr size_t total = bars + 1024;
 };
 static_assert(Smem::total + 1024 <= 232448, "layer-stream shared memory exceeds the 227 KiB opt-in limit");
@@ -194,6 +191,7 @@ __device__ __forceinline__ int total_chunks(const LsParams& P) {
 namespace ls {
 struct Bars {
     uint64_t full[kStages], empty[kStages], a_full[kPipes], a_empty[kPipes], d_full[kPipes][2], d_empty[kPipes][2];
+    uint64_t seg_full[2], seg_empty[2];      // segment hand-over (workers -> finalisers), double-buffered
     uint32_t tmem;
     int flag;       // epilogue broadcast: this CTA finalises the panel
     int u_call;     // call whose u sits in the staging buffer (-1 = none)
@@ -214,7 +212,6 @@ __device__ void producer(const LsParams& P, uint8_t* wring, Bars* B) {
             mbar_wait(&B->empty[s], ((n / kStages) & 1) ^ 1);
             mbar_arrive_expect_tx(&B->full[s], kWBytes);
             bulk_g2s(wring + s * kWBytes, wp, kWBytes, &B->full[s], pol_w);
-            LS_CT(n, 0);
         }
     }
 }
@@ -313,7 +310,6 @@ __device__ void mma_issuer(const LsParams& P, uint8_t* xring, Bars* B, uint32_t 
                 const bool first = (n - kPipes < n_last - (kb - ka) + 1), last = (n + kPipes > n_last);
                 if (first) mbar_wait(&B->d_empty[i][db], ((par >> db) & 1) ^ 1);
                 mbar_wait(&B->a_full[i], (n / kPipes) & 1);
-                LS_CT(n, 4);
                 tc_fence_after();
                 const uint64_t bd = desc_sw128(smem_u32(xring + s * kXBytes));
 #pragma unroll
@@ -323,7 +319,6 @@ __device__ void mma_issuer(const LsParams& P, uint8_t* xring, Bars* B, uint32_t 
                         umma_ts(d_base + 16 * db, a_base + h * 32 + 8 * j, bd + h * half_desc + uint64_t(2 * j), !(first && h == 0 && j == 0));
                 umma_commit(&B->a_empty[i]);
                 umma_commit(&B->empty[s]);
-                LS_CT(n, 5);
                 if (last) {
                     umma_commit(&B->d_full[i][db]);
                     par ^= 1u << db;
@@ -335,17 +330,96 @@ __device__ void mma_issuer(const LsParams& P, uint8_t* xring, Bars* B, uint32_t 
     }
 }
 
-// ---- warps 8-19: int4 -> fp16 -> TMEM (warp = group x TMEM lane quarter q; chunk n goes to A slot n mod 4) -----------------------------
-__device__ void dequantiser(int n_total, uint8_t* wring, Bars* B, uint32_t tmem, int warp, int lane) {
-    const int q = warp & 3, grp = (warp - 8) >> 2;
+// ---- warps 8-23: workers (pipeline g = chunks n = g mod 4, TMEM lane quarter q) ---------------------------------
+// Per own chunk n: first the epilogue of own chunk n - 4 (tcgen05.ld of the pipeline's accumulator at the end of each
+// scale-group run, acc += s * D, thread = output row; at the end of a segment the pipeline's partial sums go to a
+// shared-memory hand-over buffer for the finaliser warps), then the dequantisation of chunk n: LDS.128 -> exact
+// q - 8 in fp16 -> tcgen05.st.16x256b.x4 into the pipeline's A slot.  The row's scale is read from the ring stage
+// while the chunk is there and kept in a register until the run is read out.
+struct EpiState {
+    SegIter it;
+    Seg sg;
+    int n0, n1;          // stream positions [n0, n1) of the current segment's chunks
+    int m;               // next own chunk to look at
+    int seg_idx;         // segments finished (hand-over buffer = seg_idx & 1)
+    bool live, done;
+    int db;
+    unsigned par;
+};
+__device__ void worker(const LsParams& P, uint8_t* wring, const uint8_t* scring, float* part, Bars* B, uint32_t tmem,
+                       int warp, int lane) {
+    const int q = warp & 3, g = (warp - 8) >> 2;
+    const int row = 32 * q + lane;
+    const int sc_off = ((row >> 4) * 16 + 2 * (row & 7) + ((row >> 3) & 1)) * 2;       // SPW4 scale slot of this row
     const uint32_t w_lane = smem_u32(wring) + (2 * q * 32 + lane) * 16;
-    for (int n = grp; n < n_total; n += kDqGroups) {
-        const int s = n % kStages, i = n & (kPipes - 1);
-        const uint32_t t_lane = tmem + i * 64 + (uint32_t(32 * q) << 16);
-        mbar_wait(&B->a_empty[i], ((n / kPipes) & 1) ^ 1);
+    const uint32_t t_lane = tmem + g * 64 + (uint32_t(32 * q) << 16);
+    const uint32_t d_lane = tmem + kDCol + g * 32 + (uint32_t(32 * q) << 16);
+    const int n_total = total_chunks(P);
+    EpiState e;
+    e.n0 = e.n1 = 0; e.m = g; e.seg_idx = 0; e.live = false; e.done = false; e.db = 0; e.par = 0;
+    float acc[16];
+#pragma unroll
+    for (int mm = 0; mm < 16; ++mm) acc[mm] = 0.f;
+    float sc_cur = 0.f;      // scale of this row in the last dequantised own chunk's group
+
+    // epilogue of every own chunk <= limit, plus the segment hand-overs that become due
+    auto epilogue_until = [&](int limit) {
+        while (!e.done) {
+            if (!e.live) {
+                e.n0 = e.n1;
+                if (!e.it.next(P, e.sg)) { e.done = true; break; }
+                e.n1 = e.n0 + (e.sg.k1 - e.sg.k0);
+                e.live = true;
+            }
+            if (e.m < e.n1) {
+                if (e.m > limit) break;
+                // own chunk e.m of this segment: is it the pipeline's last chunk of its scale-group run?
+                const int gc = P.calls[e.sg.call].group_chunks;
+                const int k = e.sg.k0 + (e.m - e.n0);
+                const int run_end = e.n0 + (min(e.sg.k1, (k / gc + 1) * gc) - e.sg.k0);      // stream position after the run
+                if (e.m + kPipes >= run_end) {
+                    mbar_wait(&B->d_full[g][e.db], (e.par >> e.db) & 1);
+                    tc_fence_after();
+                    uint32_t v[16];
+                    asm volatile(
+                        "tcgen05.ld.sync.aligned.32x32b.x16.b32 {%0,%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15}, [%16];"
+                        : "=r"(v[0]), "=r"(v[1]), "=r"(v[2]), "=r"(v[3]), "=r"(v[4]), "=r"(v[5]), "=r"(v[6]), "=r"(v[7]),
+                          "=r"(v[8]), "=r"(v[9]), "=r"(v[10]), "=r"(v[11]), "=r"(v[12]), "=r"(v[13]), "=r"(v[14]), "=r"(v[15])
+                        : "r"(d_lane + 16 * e.db)
+                        : "memory");
+                    asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+                    tc_fence_before();
+                    __syncwarp();
+                    if (lane == 0) mbar_arrive(&B->d_empty[g][e.db]);
+                    e.par ^= 1u << e.db;
+                    e.db ^= 1;
+                    const float sc = sc_cur;      // own chunks are read out one iteration after their dequantisation
+#pragma unroll
+                    for (int mm = 0; mm < 16; ++mm) acc[mm] = fmaf(sc, __uint_as_float(v[mm]), acc[mm]);
+                }
+                e.m += kPipes;
+                continue;
+            }
+            // the segment holds no further own chunk: hand the pipeline's partial sums to the finalisers
+            const int buf = e.seg_idx & 1;
+            mbar_wait(&B->seg_empty[buf], ((e.seg_idx >> 1) & 1) ^ 1);
+            float* dst = part + size_t(buf * kPipes + g) * 2048 + row;
+#pragma unroll
+            for (int mm = 0; mm < 16; ++mm) { dst[mm * 128] = acc[mm]; acc[mm] = 0.f; }
+            __syncwarp();
+            if (lane == 0) mbar_arrive(&B->seg_full[buf]);
+            ++e.seg_idx;
+            e.live = false;
+        }
+    };
+
+    for (int n = g; n < n_total; n += kPipes) {
+        epilogue_until(n - kPipes);
+        const int s = n % kStages;
+        mbar_wait(&B->a_empty[g], ((n / kPipes) & 1) ^ 1);
         mbar_wait(&B->full[s], (n / kStages) & 1);
-        if (q == 0 && lane == 0) LS_CT(n, 2);
         tc_fence_after();
+        sc_cur = __half2float(*reinterpret_cast<const __half*>(scring + s * kScBytes + sc_off));
 #pragma unroll
         for (int h = 0; h < 2; ++h) {
 #pragma unroll
@@ -368,81 +442,41 @@ __device__ void dequantiser(int n_total, uint8_t* wring, Bars* B, uint32_t tmem,
             }
         }
         asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory");
-        fence_proxy_async_smem();       // the x tile was written by cp.async (generic proxy); the MMA reads it through the async proxy
         tc_fence_before();
         __syncwarp();
         if (lane == 0) {
-            mbar_arrive(&B->a_full[i]);
+            mbar_arrive(&B->a_full[g]);
             mbar_arrive(&B->empty[s]);
-            if (q == 0) LS_CT(n, 3);
         }
     }
+    epilogue_until(0x7fffffff - kPipes);
 }
 }  // namespace ls
 
 namespace ls {
 __device__ __forceinline__ void epi_bar() { named_bar_sync(1, 128); }
 
-// ---- warps 4-7: accumulate the runs, finalise panel segments ------------------------------------------------
-__device__ void epilogue(const LsParams& P, const uint8_t* scring, float* us, Bars* B, uint32_t tmem, int warp, int lane) {
-    const int q = warp - 4, row = 32 * q + lane, et = row;        // et = thread index among the 128 epilogue threads
-    const int sc_idx = (row >> 4) * 16 + 2 * (row & 7) + ((row >> 3) & 1);      // SPW4 scale slot of this row
+// ---- warps 4-7: finalise panel segments (thread = output row) --------------------------------------------------
+__device__ void finaliser(const LsParams& P, const float* part, float* us, Bars* B, int warp, int lane) {
+    const int q = warp - 4, row = 32 * q + lane, et = row;        // et = thread index among the 128 finaliser threads
     const int G = gridDim.x, b = blockIdx.x;
-    const uint32_t d_lane = tmem + kDCol + (uint32_t(32 * q) << 16);
     SegIter it;
     Seg sg;
-    int n = 0;
-    unsigned dbits = 0, pbits = 0;      // per pipeline w: bit w of dbits = current accumulator, bit 2w + b of pbits = its phase parity
+    int seg_idx = 0;
     while (it.next(P, sg)) {
         const LsCall& c = P.calls[sg.call];
-        const int gc = c.group_chunks;
+        // the four pipelines' partial sums of this segment
+        const int buf = seg_idx & 1;
+        mbar_wait(&B->seg_full[buf], (seg_idx >> 1) & 1);
         float acc[16];
+        {
+            const float* src = part + size_t(buf * kPipes) * 2048 + row;
 #pragma unroll
-        for (int m = 0; m < 16; ++m) acc[m] = 0.f;
-        for (int ka = sg.k0; ka < sg.k1;) {          // accumulation runs: the chunks of one scale group
-            const int kb = min(sg.k1, (ka / gc + 1) * gc);
-            const int n_last = n + (kb - ka) - 1;
-            // every chunk's stage is released by the epilogue too: the last chunk of the run carries the scale read here
-            float scale = 0.f;
-            for (int sq = n; sq <= n_last; ++sq) {
-                const int s = sq % kStages;
-                mbar_wait(&B->full[s], (sq / kStages) & 1);
-                if (sq == n_last) scale = __half2float(*reinterpret_cast<const __half*>(scring + s * kScBytes + sc_idx * 2));
-                __syncwarp();
-                if (lane == 0) mbar_arrive(&B->empty[s]);
-            }
-            float sum[16];
-#pragma unroll
-            for (int m = 0; m < 16; ++m) sum[m] = 0.f;
-            for (int sq = max(n, n_last - (kPipes - 1)); sq <= n_last; ++sq) {     // the pipelines that hold a piece
-                const int w = sq & (kPipes - 1);
-                const int bw = (dbits >> w) & 1;
-                const unsigned par = (pbits >> (2 * w + bw)) & 1;
-                pbits ^= 1u << (2 * w + bw);
-                dbits ^= 1u << w;
-                mbar_wait(&B->d_full[w][bw], par);
-                if (et == 0) LS_CT(sq, 6);
-                tc_fence_after();
-                uint32_t v[16];
-                asm volatile(
-                    "tcgen05.ld.sync.aligned.32x32b.x16.b32 {%0,%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15}, [%16];"
-                    : "=r"(v[0]), "=r"(v[1]), "=r"(v[2]), "=r"(v[3]), "=r"(v[4]), "=r"(v[5]), "=r"(v[6]), "=r"(v[7]),
-                      "=r"(v[8]), "=r"(v[9]), "=r"(v[10]), "=r"(v[11]), "=r"(v[12]), "=r"(v[13]), "=r"(v[14]), "=r"(v[15])
-                    : "r"(d_lane + w * 32 + 16 * bw)
-                    : "memory");
-                asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
-                tc_fence_before();
-                __syncwarp();
-                if (lane == 0) mbar_arrive(&B->d_empty[w][bw]);
-#pragma unroll
-                for (int m = 0; m < 16; ++m) sum[m] += __uint_as_float(v[m]);
-            }
-#pragma unroll
-            for (int m = 0; m < 16; ++m) acc[m] = fmaf(scale, sum[m], acc[m]);
-            if (et == 0) LS_CT(n_last, 7);
-            n = n_last + 1;
-            ka = kb;
+            for (int m = 0; m < 16; ++m) acc[m] = (src[m * 128] + src[2048 + m * 128]) + (src[4096 + m * 128] + src[6144 + m * 128]);
         }
+        __syncwarp();
+        if (lane == 0) mbar_arrive(&B->seg_empty[buf]);
+        ++seg_idx;
         LS_STAMP(40);
         // ---- end of the segment: S8 split-K, S7 rank-r update, cast, store ----
         const Cut cut = phase_cut(P, sg.ph);
@@ -652,6 +686,7 @@ __global__ void __launch_bounds__(ls::kThreads, 1) ls_kernel(const __grid_consta
     uint8_t* wring = base + Smem::w;
     uint8_t* scring = base + Smem::sc;
     float* us = reinterpret_cast<float*>(base + Smem::u);
+    float* part = reinterpret_cast<float*>(base + Smem::part);
     Bars* B = reinterpret_cast<Bars*>(base + Smem::bars);
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
 
@@ -662,6 +697,7 @@ __global__ void __launch_bounds__(ls::kThreads, 1) ls_kernel(const __grid_consta
             mbar_init(&B->a_empty[s], 1);
             for (int d = 0; d < 2; ++d) { mbar_init(&B->d_full[s][d], 1); mbar_init(&B->d_empty[s][d], 4); }
         }
+        for (int d = 0; d < 2; ++d) { mbar_init(&B->seg_full[d], 4 * kPipes); mbar_init(&B->seg_empty[d], 4); }
         B->flag = 0;
         B->u_call = -1;
         fence_mbar_init();
@@ -689,16 +725,16 @@ __global__ void __launch_bounds__(ls::kThreads, 1) ls_kernel(const __grid_consta
     } else if (warp == 2) {
         ec_warp(P, lane);
     } else if (warp < 8) {
-        epilogue(P, scring, us, B, tmem, warp, lane);
-    } else if (warp < 8 + 4 * kDqGroups) {
-        // prologue: x -> operand layout (workspace), one arrive per CTA once its 8 warps are through
-        x_prologue(P, threadIdx.x - 256, 128 * kDqGroups);
+        finaliser(P, part, us, B, warp, lane);
+    } else if (warp < 8 + 4 * kPipes) {
+        // prologue: x -> operand layout (workspace), one arrive per CTA once its 16 worker warps are through
+        x_prologue(P, threadIdx.x - 256, 128 * kPipes);
         __threadfence();
-        named_bar_sync(2, 128 * kDqGroups);
+        named_bar_sync(2, 128 * kPipes);
         if (threadIdx.x == 256) { asm volatile("fence.proxy.async;" ::: "memory"); red_add_release(P.done + kLsMaxCalls + 1, 1u); }
-        dequantiser(total_chunks(P), wring, B, tmem, warp, lane);
+        worker(P, wring, scring, part, B, tmem, warp, lane);
     } else {
-        if (lane == 0) mma_issuer(P, xring, B, tmem, warp - (8 + 4 * kDqGroups));
+        if (lane == 0) mma_issuer(P, xring, B, tmem, warp - (8 + 4 * kPipes));
     }
 #ifdef LS_TRACE
     if (lane == 0) stamp[warp] = ls_now();
@@ -710,9 +746,9 @@ __global__ void __launch_bounds__(ls::kThreads, 1) ls_kernel(const __grid_consta
         const unsigned long long t0 = stamp[39];
         printf("   epi: runs %llu slot %llu atom %llu sum %llu store %llu\n", stamp[40]-stamp[39], stamp[41]-stamp[39], stamp[42]-stamp[39], stamp[43]-stamp[39], stamp[44]-stamp[39]);
         if (blockIdx.x == 36) for (int n = 0; n < min(32, total_chunks(P)); ++n)
-            printf("  chunk %2d: bulk %llu xld %llu full %llu deq %llu afull %llu mma %llu dfull %llu epi %llu\n", n, g_ct[n][0]-t0, g_ct[n][1]-t0, g_ct[n][2]-t0, g_ct[n][3]-t0, g_ct[n][4]-t0, g_ct[n][5]-t0, g_ct[n][6]-t0, g_ct[n][7]-t0);
+            printf("  chunk %2d: start %llu fullwait %llu | epi: full %llu (dfull) ld-issued %llu ld-done %llu arrived %llu dfull %llu end %llu\n", n, g_ct[n][0]-t0, g_ct[n][1]-t0, g_ct[n][2]-t0, g_ct[n][3]-t0, g_ct[n][4]-t0, g_ct[n][5]-t0, g_ct[n][6]-t0, g_ct[n][7]-t0);
         printf("cta %d chunks %d: prod %llu xld %llu ec %llu epi %llu dq %llu %llu mma %llu %llu end %llu\n", blockIdx.x, total_chunks(P), stamp[0] - t0, stamp[1] - t0,
-               stamp[2] - t0, stamp[4] - t0, stamp[8] - t0, stamp[19] - t0, stamp[20] - t0, stamp[23] - t0, ls_now() - t0);
+               stamp[2] - t0, stamp[4] - t0, stamp[8] - t0, stamp[23] - t0, stamp[24] - t0, stamp[27] - t0, ls_now() - t0);
     }
 #endif
     if (warp == 3) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem), "n"(kTmemCols) : "memory");
