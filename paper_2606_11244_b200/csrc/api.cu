@@ -253,7 +253,7 @@ static bool variant_valid(int v, int M, int r, int gate) {
     switch (v) {
         case SPEAR_VARIANT_STREAM_FUSED: return M <= 16 && r > 0 && gate != SPEAR_GATE_MLP;
         case SPEAR_VARIANT_STREAM_SPLIT: return M <= 16;
-        case SPEAR_VARIANT_LSTREAM: return M <= 16 && gate != SPEAR_GATE_MLP;
+        case SPEAR_VARIANT_LSTREAM: return M <= 16 && gate != SPEAR_GATE_MLP;      // (+ group shape, checked in layer_impl)
         case SPEAR_VARIANT_TC_FUSED: return tc_available() && M >= 1;
         case SPEAR_VARIANT_TC_SPLIT: return tc_available() && r > 0;
         default: return false;
@@ -455,6 +455,8 @@ static bool ls_eligible(const spear_call& c) {
     if (c.M < 1 || c.M > 16) return false;
     if (c.r > 0 && c.ec && c.ec->gate_kind == SPEAR_GATE_MLP) return false;
     if (c.ec && c.ec->workspace) return false;
+    const int gcn = c.group / 128;
+    if (c.group != c.K && (gcn & (gcn - 1))) return false;      // scale groups: a power-of-two number of 128-column chunks, or per-channel
     return true;
 }
 static int run_lstream(const spear_call* calls, int n_calls, cudaStream_t st) {
@@ -525,6 +527,8 @@ static int run_lstream(const spear_call* calls, int n_calls, cudaStream_t st) {
                 xperm_used += need;
             }
             d.group_chunks = c.group / 128;
+            d.group_shift = 31;
+            if (c.group != c.K) { d.group_shift = 0; while ((1 << d.group_shift) < d.group_chunks) ++d.group_shift; }
             d.C = c.K / 128;
             d.P = c.N / 128;
             d.chunk_base = int(phase_chunks);
@@ -583,8 +587,15 @@ static int layer_impl(const void* x, const void* Wq, const void* scales, const v
         v = heuristic_variant(M, r, gate);
         if (!variant_valid(v, M, r, gate)) return set_error(SPEAR_EUNSUPPORTED, "no kernel variant for M=%d r=%d", M, r);
     }
-    if (v == SPEAR_VARIANT_LSTREAM && ec && ec->workspace && ec->force_variant == SPEAR_VARIANT_AUTO)
-        v = (r > 0 && gate != SPEAR_GATE_MLP) ? SPEAR_VARIANT_STREAM_FUSED : SPEAR_VARIANT_STREAM_SPLIT;   // caller-owned workspace
+    {
+        const int gcn = group / 128;
+        const bool odd_group = (group != K) && (gcn & (gcn - 1));     // lstream: power-of-two chunks per group, or per-channel
+        const bool auto_v = !(ec && ec->force_variant != SPEAR_VARIANT_AUTO);
+        if (v == SPEAR_VARIANT_LSTREAM && auto_v && ((ec && ec->workspace) || odd_group))
+            v = (r > 0 && gate != SPEAR_GATE_MLP) ? SPEAR_VARIANT_STREAM_FUSED : SPEAR_VARIANT_STREAM_SPLIT;
+        if (v == SPEAR_VARIANT_LSTREAM && odd_group)
+            return set_error(SPEAR_EUNSUPPORTED, "the layer-stream variant needs group / 128 to be a power of two (or group == K)");
+    }
     if (v == SPEAR_VARIANT_LSTREAM) {
         if (ec && ec->workspace) return set_error(SPEAR_EUNSUPPORTED, "the layer-stream variant uses the library's own workspace");
         spear_call c = {x, Wq, scales, A, B, ec, y, M, N, K, r, group};

@@ -64,6 +64,7 @@ struct LsCall {
     int x_internal;          // 1: x is an earlier call's y (xperm comes from its finalisers)
     int M, N, K, r;
     int group_chunks;        // group / 128
+    int group_shift;         // log2(group_chunks) when the group is a power-of-two number of chunks; 31: group == K
     int C;                   // K / 128 chunks per panel
     int P;                   // N / 128 panels
     int gate_kind;           // SPEAR_GATE_SCALAR_SIGMOID or SPEAR_GATE_NONE

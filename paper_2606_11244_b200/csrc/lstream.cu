@@ -65,7 +65,8 @@ constexpr int kPipes = 4;                   // dequantisation / MMA pipelines; p
 constexpr int kThreads = (8 + 4 * kPipes + kPipes) * 32;      // 4 service warps, 4 finalisers, 16 workers, 4 MMA issuers
 constexpr int kWBytes = 8192, kXBytes = 4096, kScBytes = 256;
 constexpr uint32_t kTmemCols = 512;
-constexpr uint32_t kDCol = kPipes * 64;     // per pipeline: one 64-column A slot (a chunk), then two 16-column accumulators
+constexpr int kASlots = 6;                  // A-operand slots in tensor memory (64 columns = one chunk each); chunk n -> slot n mod 6
+constexpr uint32_t kDCol = kASlots * 64;    // behind them: two 16-column fp32 accumulators per pipeline (6*64 + 4*32 = 512 columns)
 constexpr uint32_t kIdesc = (1u << 4) | (uint32_t(16 >> 3) << 17) | (uint32_t(128 >> 4) << 24);
 constexpr int kEmptyCount = 4 + 1;          // the chunk's 4 worker warps + its MMA commit
 struct Smem {
@@ -190,7 +191,7 @@ __device__ __forceinline__ int total_chunks(const LsParams& P) {
 
 namespace ls {
 struct Bars {
-    uint64_t full[kStages], empty[kStages], a_full[kPipes], a_empty[kPipes], d_full[kPipes][2], d_empty[kPipes][2];
+    uint64_t full[kStages], empty[kStages], a_full[kASlots], a_empty[kASlots], d_full[kPipes][2], d_empty[kPipes][2];
     uint64_t seg_full[2], seg_empty[2];      // segment hand-over (workers -> finalisers), double-buffered
     uint32_t tmem;
     int flag;       // epilogue broadcast: this CTA finalises the panel
@@ -212,6 +213,7 @@ __device__ void producer(const LsParams& P, uint8_t* wring, Bars* B) {
             mbar_wait(&B->empty[s], ((n / kStages) & 1) ^ 1);
             mbar_arrive_expect_tx(&B->full[s], kWBytes);
             bulk_g2s(wring + s * kWBytes, wp, kWBytes, &B->full[s], pol_w);
+            LS_CT(n, 6);
         }
     }
 }
@@ -264,6 +266,9 @@ __device__ void x_producer(const LsParams& P, uint8_t* xring, Bars* B) {
             wait_counter(P.done + kLsMaxCalls + 1, gridDim.x);
             asm volatile("fence.proxy.async;" ::: "memory");
             prologue_seen = true;
+#ifdef LS_TRACE
+            g_stamp[47] = ls_now();
+#endif
         }
         const uint8_t* xp = c.xperm + size_t(sg.k0) * c.xtile;
         for (int k = sg.k0; k < sg.k1; ++k, ++n, xp += c.xtile) {
@@ -297,36 +302,38 @@ __device__ void mma_issuer(const LsParams& P, uint8_t* xring, Bars* B, uint32_t 
     Seg sg;
     int n = 0, db = 0;
     unsigned par = 0;       // bit b: parity of accumulator b's next d_empty phase
-    const uint32_t a_base = tmem + i * 64, d_base = tmem + kDCol + i * 32;
+    const uint32_t d_base = tmem + kDCol + i * 32;
     while (it.next(P, sg)) {
-        const int gc = P.calls[sg.call].group_chunks;
+        const int gsh = P.calls[sg.call].group_shift;       // log2(chunks per scale group); >= 31: one group per row
         const uint64_t half_desc = uint64_t(P.calls[sg.call].xtile >> 5);      // (xtile / 2) >> 4: descriptor step to the second k-tile
-        for (int ka = sg.k0; ka < sg.k1;) {          // accumulation runs: the chunks of one scale group
-            const int kb = min(sg.k1, (ka / gc + 1) * gc);
-            const int n_last = n + (kb - ka) - 1;
-            for (; n <= n_last; ++n) {
-                if ((n & (kPipes - 1)) != i) continue;
-                const int s = n % kStages;
-                const bool first = (n - kPipes < n_last - (kb - ka) + 1), last = (n + kPipes > n_last);
-                if (first) mbar_wait(&B->d_empty[i][db], ((par >> db) & 1) ^ 1);
-                mbar_wait(&B->a_full[i], (n / kPipes) & 1);
-                tc_fence_after();
-                const uint64_t bd = desc_sw128(smem_u32(xring + s * kXBytes));
+        const int n_seg = n + (sg.k1 - sg.k0);
+        int m = n + ((i - n) & (kPipes - 1));                // first own chunk of the segment
+        for (; m < n_seg; m += kPipes) {
+            // the accumulation run (chunks of one scale group inside this segment) that chunk m belongs to
+            const int k = sg.k0 + (m - n);
+            const int run_lo = gsh >= 31 ? sg.k0 : max(sg.k0, (k >> gsh) << gsh);
+            const int run_hi = gsh >= 31 ? sg.k1 : min(sg.k1, ((k >> gsh) + 1) << gsh);
+            const bool first = (k - kPipes < run_lo), last = (k + kPipes >= run_hi);
+            const int s = m % kStages, slot = m % kASlots;
+            const uint32_t a_base = tmem + slot * 64;
+            if (first) mbar_wait(&B->d_empty[i][db], ((par >> db) & 1) ^ 1);
+            mbar_wait(&B->a_full[slot], (m / kASlots) & 1);
+            tc_fence_after();
+            const uint64_t bd = desc_sw128(smem_u32(xring + s * kXBytes));
 #pragma unroll
-                for (int h = 0; h < 2; ++h)
+            for (int h = 0; h < 2; ++h)
 #pragma unroll
-                    for (int j = 0; j < 4; ++j)
-                        umma_ts(d_base + 16 * db, a_base + h * 32 + 8 * j, bd + h * half_desc + uint64_t(2 * j), !(first && h == 0 && j == 0));
-                umma_commit(&B->a_empty[i]);
-                umma_commit(&B->empty[s]);
-                if (last) {
-                    umma_commit(&B->d_full[i][db]);
-                    par ^= 1u << db;
-                    db ^= 1;
-                }
+                for (int j = 0; j < 4; ++j)
+                    umma_ts(d_base + 16 * db, a_base + h * 32 + 8 * j, bd + h * half_desc + uint64_t(2 * j), !(first && h == 0 && j == 0));
+            umma_commit(&B->a_empty[slot]);
+            umma_commit(&B->empty[s]);
+            if (last) {
+                umma_commit(&B->d_full[i][db]);
+                par ^= 1u << db;
+                db ^= 1;
             }
-            ka = kb;
         }
+        n = n_seg;
     }
 }
 
@@ -352,7 +359,7 @@ __device__ void worker(const LsParams& P, uint8_t* wring, const uint8_t* scring,
     const int row = 32 * q + lane;
     const int sc_off = ((row >> 4) * 16 + 2 * (row & 7) + ((row >> 3) & 1)) * 2;       // SPW4 scale slot of this row
     const uint32_t w_lane = smem_u32(wring) + (2 * q * 32 + lane) * 16;
-    const uint32_t t_lane = tmem + g * 64 + (uint32_t(32 * q) << 16);
+    const uint32_t t_quarter = tmem + (uint32_t(32 * q) << 16);
     const uint32_t d_lane = tmem + kDCol + g * 32 + (uint32_t(32 * q) << 16);
     const int n_total = total_chunks(P);
     EpiState e;
@@ -360,7 +367,7 @@ __device__ void worker(const LsParams& P, uint8_t* wring, const uint8_t* scring,
     float acc[16];
 #pragma unroll
     for (int mm = 0; mm < 16; ++mm) acc[mm] = 0.f;
-    float sc_cur = 0.f;      // scale of this row in the last dequantised own chunk's group
+    float sc_a = 0.f, sc_b = 0.f;      // this row's scale in the groups of own chunks n - 4 and n - 8 (read out two iterations late)
 
     // epilogue of every own chunk <= limit, plus the segment hand-overs that become due
     auto epilogue_until = [&](int limit) {
@@ -374,10 +381,10 @@ __device__ void worker(const LsParams& P, uint8_t* wring, const uint8_t* scring,
             if (e.m < e.n1) {
                 if (e.m > limit) break;
                 // own chunk e.m of this segment: is it the pipeline's last chunk of its scale-group run?
-                const int gc = P.calls[e.sg.call].group_chunks;
+                const int gsh = P.calls[e.sg.call].group_shift;
                 const int k = e.sg.k0 + (e.m - e.n0);
-                const int run_end = e.n0 + (min(e.sg.k1, (k / gc + 1) * gc) - e.sg.k0);      // stream position after the run
-                if (e.m + kPipes >= run_end) {
+                const int run_hi = gsh >= 31 ? e.sg.k1 : min(e.sg.k1, ((k >> gsh) + 1) << gsh);      // chunk after the run
+                if (k + kPipes >= run_hi) {
                     mbar_wait(&B->d_full[g][e.db], (e.par >> e.db) & 1);
                     tc_fence_after();
                     uint32_t v[16];
@@ -393,7 +400,7 @@ __device__ void worker(const LsParams& P, uint8_t* wring, const uint8_t* scring,
                     if (lane == 0) mbar_arrive(&B->d_empty[g][e.db]);
                     e.par ^= 1u << e.db;
                     e.db ^= 1;
-                    const float sc = sc_cur;      // own chunks are read out one iteration after their dequantisation
+                    const float sc = sc_b;
 #pragma unroll
                     for (int mm = 0; mm < 16; ++mm) acc[mm] = fmaf(sc, __uint_as_float(v[mm]), acc[mm]);
                 }
@@ -414,12 +421,17 @@ __device__ void worker(const LsParams& P, uint8_t* wring, const uint8_t* scring,
     };
 
     for (int n = g; n < n_total; n += kPipes) {
-        epilogue_until(n - kPipes);
-        const int s = n % kStages;
-        mbar_wait(&B->a_empty[g], ((n / kPipes) & 1) ^ 1);
+        epilogue_until(n - 2 * kPipes);      // its MMAs finished long ago: no wait, and the accumulator is free for chunk n
+        const int s = n % kStages, slot = n % kASlots;
+        const uint32_t t_lane = t_quarter + slot * 64;
+        mbar_wait(&B->a_empty[slot], ((n / kASlots) & 1) ^ 1);
         mbar_wait(&B->full[s], (n / kStages) & 1);
+#ifdef LS_TRACE
+        if (n == 0 && q == 0 && lane == 0) g_stamp[46] = ls_now();
+#endif
         tc_fence_after();
-        sc_cur = __half2float(*reinterpret_cast<const __half*>(scring + s * kScBytes + sc_off));
+        sc_b = sc_a;
+        sc_a = __half2float(*reinterpret_cast<const __half*>(scring + s * kScBytes + sc_off));
 #pragma unroll
         for (int h = 0; h < 2; ++h) {
 #pragma unroll
@@ -445,11 +457,17 @@ __device__ void worker(const LsParams& P, uint8_t* wring, const uint8_t* scring,
         tc_fence_before();
         __syncwarp();
         if (lane == 0) {
-            mbar_arrive(&B->a_full[g]);
+            mbar_arrive(&B->a_full[slot]);
             mbar_arrive(&B->empty[s]);
         }
     }
-    epilogue_until(0x7fffffff - kPipes);
+    // the last two own chunks
+    {
+        const int n_next = g + ((n_total - g + kPipes - 1) / kPipes) * kPipes;      // first own position >= n_total
+        epilogue_until(n_next - 2 * kPipes);
+        sc_b = sc_a;
+        epilogue_until(0x7fffffff - kPipes);
+    }
 }
 }  // namespace ls
 
@@ -669,9 +687,17 @@ __device__ void ec_call(const LsParams& P, int ci, int lane) {
         red_add_release(sync + 1, 1u);
     }
 }
+// Phase 0 (x comes from outside the launch): its calls are shared by five warps (the EC warp and the four finaliser
+// warps, idle until the first segment is through), so that their memory round trips overlap.  Later phases (x is an
+// earlier phase's y) belong to the EC warp alone.
+__device__ void ec_phase0(const LsParams& P, int lane, int e) {
+    for (int ci = P.phase_first_call[0] + e; ci < P.phase_first_call[1]; ci += 5)
+        if (P.calls[ci].r > 0) ec_call(P, ci, lane);
+}
 __device__ void ec_warp(const LsParams& P, int lane) {
-    for (int ph = 0; ph < P.n_phases; ++ph) {
-        if (ph > 0) wait_counter(P.done + ph - 1, unsigned(P.phase_panels[ph - 1]));
+    ec_phase0(P, lane, 4);
+    for (int ph = 1; ph < P.n_phases; ++ph) {
+        wait_counter(P.done + ph - 1, unsigned(P.phase_panels[ph - 1]));
         for (int ci = P.phase_first_call[ph]; ci < P.phase_first_call[ph + 1]; ++ci)
             if (P.calls[ci].r > 0) ec_call(P, ci, lane);
     }
@@ -692,9 +718,8 @@ __global__ void __launch_bounds__(ls::kThreads, 1) ls_kernel(const __grid_consta
 
     if (threadIdx.x == 0) {
         for (int s = 0; s < kStages; ++s) { mbar_init(&B->full[s], 3); mbar_init(&B->empty[s], kEmptyCount); }
+        for (int s = 0; s < kASlots; ++s) { mbar_init(&B->a_full[s], 4); mbar_init(&B->a_empty[s], 1); }
         for (int s = 0; s < kPipes; ++s) {
-            mbar_init(&B->a_full[s], 4);
-            mbar_init(&B->a_empty[s], 1);
             for (int d = 0; d < 2; ++d) { mbar_init(&B->d_full[s][d], 1); mbar_init(&B->d_empty[s][d], 4); }
         }
         for (int d = 0; d < 2; ++d) { mbar_init(&B->seg_full[d], 4 * kPipes); mbar_init(&B->seg_empty[d], 4); }
@@ -725,6 +750,7 @@ __global__ void __launch_bounds__(ls::kThreads, 1) ls_kernel(const __grid_consta
     } else if (warp == 2) {
         ec_warp(P, lane);
     } else if (warp < 8) {
+        ec_phase0(P, lane, warp - 4);
         finaliser(P, part, us, B, warp, lane);
     } else if (warp < 8 + 4 * kPipes) {
         // prologue: x -> operand layout (workspace), one arrive per CTA once its 16 worker warps are through
@@ -732,6 +758,9 @@ __global__ void __launch_bounds__(ls::kThreads, 1) ls_kernel(const __grid_consta
         __threadfence();
         named_bar_sync(2, 128 * kPipes);
         if (threadIdx.x == 256) { asm volatile("fence.proxy.async;" ::: "memory"); red_add_release(P.done + kLsMaxCalls + 1, 1u); }
+#ifdef LS_TRACE
+        if (threadIdx.x == 256) g_stamp[45] = ls_now();
+#endif
         worker(P, wring, scring, part, B, tmem, warp, lane);
     } else {
         if (lane == 0) mma_issuer(P, xring, B, tmem, warp - (8 + 4 * kPipes));
@@ -744,9 +773,9 @@ __global__ void __launch_bounds__(ls::kThreads, 1) ls_kernel(const __grid_consta
 #ifdef LS_TRACE
     if (threadIdx.x == 0 && total_chunks(P) > 0 && (blockIdx.x % 37) == 36) {
         const unsigned long long t0 = stamp[39];
-        printf("   epi: runs %llu slot %llu atom %llu sum %llu store %llu\n", stamp[40]-stamp[39], stamp[41]-stamp[39], stamp[42]-stamp[39], stamp[43]-stamp[39], stamp[44]-stamp[39]);
+        printf("   prologue %llu xgo %llu first-full %llu | last seg: parts %llu slot %llu atom %llu sum %llu store %llu\n", stamp[45]-stamp[39], stamp[47]-stamp[39], stamp[46]-stamp[39], stamp[40]-stamp[39], stamp[41]-stamp[39], stamp[42]-stamp[39], stamp[43]-stamp[39], stamp[44]-stamp[39]);
         if (blockIdx.x == 36) for (int n = 0; n < min(32, total_chunks(P)); ++n)
-            printf("  chunk %2d: start %llu fullwait %llu | epi: full %llu (dfull) ld-issued %llu ld-done %llu arrived %llu dfull %llu end %llu\n", n, g_ct[n][0]-t0, g_ct[n][1]-t0, g_ct[n][2]-t0, g_ct[n][3]-t0, g_ct[n][4]-t0, g_ct[n][5]-t0, g_ct[n][6]-t0, g_ct[n][7]-t0);
+            printf("  chunk %2d: mma-lane: arrive %llu dempty-ok %llu (after-dfull-commit %llu run-top %llu) | mma: afull %llu commit %llu | bulk %llu mma-complete %llu\n", n, g_ct[n][0]-t0, g_ct[n][1]-t0, g_ct[n][2]-t0, g_ct[n][3]-t0, g_ct[n][4]-t0, g_ct[n][5]-t0, g_ct[n][6]-t0, g_ct[n][7]-t0);
         printf("cta %d chunks %d: prod %llu xld %llu ec %llu epi %llu dq %llu %llu mma %llu %llu end %llu\n", blockIdx.x, total_chunks(P), stamp[0] - t0, stamp[1] - t0,
                stamp[2] - t0, stamp[4] - t0, stamp[8] - t0, stamp[23] - t0, stamp[24] - t0, stamp[27] - t0, ls_now() - t0);
     }
