@@ -57,9 +57,24 @@ __shared__ unsigned long long g_ct[32][8];
 #define LS_STAMP(i)
 #define LS_CT(n, j)
 #endif
+#ifdef LS_TRACE
+__device__ __forceinline__ void ls_wait_impl(uint64_t* bar, uint32_t parity, int tag, int a, int b) {
+    long long t0 = clock64();
+    while (!mbar_try_wait(bar, parity)) {
+        if (clock64() - t0 > 400000000ll) {
+            if ((threadIdx.x & 31) == 0 || (threadIdx.x >> 5) < 4 || (threadIdx.x >> 5) >= 24) printf("STUCK mbar tag %d cta %d warp %d lane %d info %d %d\n", tag, blockIdx.x, threadIdx.x >> 5, threadIdx.x & 31, a, b);
+            t0 = clock64() + 4000000000ll;
+        }
+    }
+}
+#define LS_WAIT(bar, parity, tag, a, b) ls_wait_impl(bar, parity, tag, a, b)
+#else
+#define LS_WAIT(bar, parity, tag, a, b) mbar_wait(bar, parity)
+#endif
 #ifndef LS_STAGES
 #define LS_STAGES 16
 #endif
+static_assert(LS_STAGES % 2 == 0 && LS_STAGES >= 6, "ring depth must be even: chunk n - kStages must belong to pipeline n or n + 2 (mod 4), whose progress a worker has observed before it tests full[] by parity");
 constexpr int kStages = LS_STAGES;                 // ring depth (chunks): 16 x (8 KiB weights + 4 KiB x tile)
 constexpr int kPipes = 4;                   // dequantisation / MMA pipelines; pipeline i owns chunks n = i (mod 4)
 constexpr int kThreads = (8 + 4 * kPipes + kPipes) * 32;      // 4 service warps, 4 finalisers, 16 workers, 4 MMA issuers
@@ -117,7 +132,15 @@ __device__ __forceinline__ void red_add_release(unsigned* p, unsigned v) {
     asm volatile("red.release.gpu.global.add.u32 [%0], %1;" ::"l"(p), "r"(v) : "memory");
 }
 __device__ __forceinline__ void wait_counter(const unsigned* p, unsigned target) {
+#ifdef LS_TRACE
+    long long t0 = clock64();
+    while (ld_acquire(p) < target) {
+        __nanosleep(64);
+        if (clock64() - t0 > 400000000ll) { printf("STUCK counter cta %d warp %d have %u want %u\n", blockIdx.x, threadIdx.x >> 5, ld_acquire(p), target); t0 = clock64() + 4000000000ll; }
+    }
+#else
     while (ld_acquire(p) < target) __nanosleep(64);
+#endif
 }
 
 // ---- the work sequence of this CTA --------------------------------------------------------------------------
@@ -210,7 +233,7 @@ __device__ void producer(const LsParams& P, uint8_t* wring, Bars* B) {
         const uint8_t* wp = c.wq + (size_t(sg.panel) * c.C + sg.k0) * kWBytes;
         for (int k = sg.k0; k < sg.k1; ++k, ++n, wp += kWBytes) {
             const int s = n % kStages;
-            mbar_wait(&B->empty[s], ((n / kStages) & 1) ^ 1);
+            LS_WAIT(&B->empty[s], ((n / kStages) & 1) ^ 1, 1, n, 0);
             mbar_arrive_expect_tx(&B->full[s], kWBytes);
             bulk_g2s(wring + s * kWBytes, wp, kWBytes, &B->full[s], pol_w);
             LS_CT(n, 6);
@@ -273,7 +296,7 @@ __device__ void x_producer(const LsParams& P, uint8_t* xring, Bars* B) {
         const uint8_t* xp = c.xperm + size_t(sg.k0) * c.xtile;
         for (int k = sg.k0; k < sg.k1; ++k, ++n, xp += c.xtile) {
             const int s = n % kStages;
-            mbar_wait(&B->empty[s], ((n / kStages) & 1) ^ 1);
+            LS_WAIT(&B->empty[s], ((n / kStages) & 1) ^ 1, 2, n, 0);
             mbar_arrive_expect_tx(&B->full[s], c.xtile);
             bulk_g2s(xring + s * kXBytes, xp, c.xtile, &B->full[s], pol);
         }
@@ -289,7 +312,7 @@ __device__ void sc_producer(const LsParams& P, uint8_t* scring, Bars* B) {
         const uint8_t* sp = c.scales + size_t(sg.panel) * (c.C / c.group_chunks) * kScBytes;
         for (int k = sg.k0; k < sg.k1; ++k, ++n) {
             const int s = n % kStages;
-            mbar_wait(&B->empty[s], ((n / kStages) & 1) ^ 1);
+            LS_WAIT(&B->empty[s], ((n / kStages) & 1) ^ 1, 3, n, 0);
             mbar_arrive_expect_tx(&B->full[s], kScBytes);
             bulk_g2s(scring + s * kScBytes, sp + size_t(k / c.group_chunks) * kScBytes, kScBytes, &B->full[s], pol);
         }
@@ -316,8 +339,12 @@ __device__ void mma_issuer(const LsParams& P, uint8_t* xring, Bars* B, uint32_t 
             const bool first = (k - kPipes < run_lo), last = (k + kPipes >= run_hi);
             const int s = m % kStages, slot = m % kASlots;
             const uint32_t a_base = tmem + slot * 64;
-            if (first) mbar_wait(&B->d_empty[i][db], ((par >> db) & 1) ^ 1);
-            mbar_wait(&B->a_full[slot], (m / kASlots) & 1);
+            if (first) LS_WAIT(&B->d_empty[i][db], ((par >> db) & 1) ^ 1, 4, m, db);
+            // A slots are shared between pipelines (chunk m - 6 belongs to another issuer): a parity wait is only valid
+            // when the barrier is at most one phase behind, so first make sure MMA(m - 6) has been committed -- then
+            // a_full[slot] can only be completed by chunk m's own workers
+            LS_WAIT(&B->a_empty[slot], ((m / kASlots) & 1) ^ 1, 11, m, 0);
+            LS_WAIT(&B->a_full[slot], (m / kASlots) & 1, 5, m, 0);
             tc_fence_after();
             const uint64_t bd = desc_sw128(smem_u32(xring + s * kXBytes));
 #pragma unroll
@@ -385,7 +412,7 @@ __device__ void worker(const LsParams& P, uint8_t* wring, const uint8_t* scring,
                 const int k = e.sg.k0 + (e.m - e.n0);
                 const int run_hi = gsh >= 31 ? e.sg.k1 : min(e.sg.k1, ((k >> gsh) + 1) << gsh);      // chunk after the run
                 if (k + kPipes >= run_hi) {
-                    mbar_wait(&B->d_full[g][e.db], (e.par >> e.db) & 1);
+                    LS_WAIT(&B->d_full[g][e.db], (e.par >> e.db) & 1, 6, e.m, e.db);
                     tc_fence_after();
                     uint32_t v[16];
                     asm volatile(
@@ -409,7 +436,7 @@ __device__ void worker(const LsParams& P, uint8_t* wring, const uint8_t* scring,
             }
             // the segment holds no further own chunk: hand the pipeline's partial sums to the finalisers
             const int buf = e.seg_idx & 1;
-            mbar_wait(&B->seg_empty[buf], ((e.seg_idx >> 1) & 1) ^ 1);
+            LS_WAIT(&B->seg_empty[buf], ((e.seg_idx >> 1) & 1) ^ 1, 7, e.seg_idx, e.m);
             float* dst = part + size_t(buf * kPipes + g) * 2048 + row;
 #pragma unroll
             for (int mm = 0; mm < 16; ++mm) { dst[mm * 128] = acc[mm]; acc[mm] = 0.f; }
@@ -424,8 +451,8 @@ __device__ void worker(const LsParams& P, uint8_t* wring, const uint8_t* scring,
         epilogue_until(n - 2 * kPipes);      // its MMAs finished long ago: no wait, and the accumulator is free for chunk n
         const int s = n % kStages, slot = n % kASlots;
         const uint32_t t_lane = t_quarter + slot * 64;
-        mbar_wait(&B->a_empty[slot], ((n / kASlots) & 1) ^ 1);
-        mbar_wait(&B->full[s], (n / kStages) & 1);
+        LS_WAIT(&B->a_empty[slot], ((n / kASlots) & 1) ^ 1, 8, n, 0);
+        LS_WAIT(&B->full[s], (n / kStages) & 1, 9, n, 0);
 #ifdef LS_TRACE
         if (n == 0 && q == 0 && lane == 0) g_stamp[46] = ls_now();
 #endif
@@ -485,7 +512,7 @@ __device__ void finaliser(const LsParams& P, const float* part, float* us, Bars*
         const LsCall& c = P.calls[sg.call];
         // the four pipelines' partial sums of this segment
         const int buf = seg_idx & 1;
-        mbar_wait(&B->seg_full[buf], (seg_idx >> 1) & 1);
+        LS_WAIT(&B->seg_full[buf], (seg_idx >> 1) & 1, 10, seg_idx, 0);
         float acc[16];
         {
             const float* src = part + size_t(buf * kPipes) * 2048 + row;
@@ -771,7 +798,7 @@ __global__ void __launch_bounds__(ls::kThreads, 1) ls_kernel(const __grid_consta
     tc_fence_before();
     __syncthreads();
 #ifdef LS_TRACE
-    if (threadIdx.x == 0 && total_chunks(P) > 0 && (blockIdx.x % 37) == 36) {
+    if (false && threadIdx.x == 0 && total_chunks(P) > 0 && (blockIdx.x % 37) == 36) {
         const unsigned long long t0 = stamp[39];
         printf("   prologue %llu xgo %llu first-full %llu | last seg: parts %llu slot %llu atom %llu sum %llu store %llu\n", stamp[45]-stamp[39], stamp[47]-stamp[39], stamp[46]-stamp[39], stamp[40]-stamp[39], stamp[41]-stamp[39], stamp[42]-stamp[39], stamp[43]-stamp[39], stamp[44]-stamp[39]);
         if (blockIdx.x == 36) for (int n = 0; n < min(32, total_chunks(P)); ++n)
