@@ -80,7 +80,7 @@ struct LsParams {
     int phase_chunks[kLsMaxCalls];           // chunks of the phase (all its calls)
     int phase_per[kLsMaxCalls], phase_rem[kLsMaxCalls];   // phase_chunks / grid, phase_chunks % grid
     int phase_panels[kLsMaxCalls];           // panels of the phase = y completions to wait for
-    float* partial;          // [2 phase parities][grid][2][16][128] fp32 split-K slots
+    float* partial;          // [2 phase parities][grid][16][128] fp32 split-K accumulators of shared panels, zero between launches
     unsigned* counters;      // per-panel split-K counters, zero between launches (self-cleaning)
     unsigned* done;          // [n_phases] finalised panels per phase, [kLsMaxCalls] exit counter, [kLsMaxCalls + 1] CTAs that
                              // finished the x prologue; zeroed by the last CTA

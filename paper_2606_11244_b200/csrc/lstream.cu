@@ -504,12 +504,33 @@ __device__ __forceinline__ void epi_bar() { named_bar_sync(1, 128); }
 // ---- warps 4-7: finalise panel segments (thread = output row) --------------------------------------------------
 __device__ void finaliser(const LsParams& P, const float* part, float* us, Bars* B, int warp, int lane) {
     const int q = warp - 4, row = 32 * q + lane, et = row;        // et = thread index among the 128 finaliser threads
-    const int G = gridDim.x, b = blockIdx.x;
+    const int G = gridDim.x;
     SegIter it;
     Seg sg;
     int seg_idx = 0;
     while (it.next(P, sg)) {
         const LsCall& c = P.calls[sg.call];
+        // While the workers are still on this segment: fetch this row of B (first 32 columns) and, when the call's u has
+        // been published already, stage it -- so that the finalisation below finds both on chip.
+        uint4 bpre[4];
+        if (c.r > 0) {
+            const uint4* Brow = reinterpret_cast<const uint4*>(c.B + size_t(sg.panel * 128 + row) * c.r);
+#pragma unroll
+            for (int j8 = 0; j8 < 4; ++j8)
+                if (j8 < c.r / 8) bpre[j8] = __ldg(Brow + j8);
+            if (B->u_call != sg.call) {          // uniform across the 128 threads
+                epi_bar();
+                if (et == 0) B->flag = ld_acquire(P.ec_sync + 2 * c.ec_slot + 1) >= 1u;
+                epi_bar();
+                if (B->flag) {
+                    const float* ug = P.ubuf + size_t(c.ec_slot) * 2048;
+                    for (int idx = et; idx < c.M * c.r; idx += 128) us[idx] = __ldcg(ug + idx);
+                    epi_bar();
+                    if (et == 0) B->u_call = sg.call;
+                }
+                epi_bar();
+            }
+        }
         // the four pipelines' partial sums of this segment
         const int buf = seg_idx & 1;
         LS_WAIT(&B->seg_full[buf], (seg_idx >> 1) & 1, 10, seg_idx, 0);
@@ -528,20 +549,21 @@ __device__ void finaliser(const LsParams& P, const float* part, float* us, Bars*
         const bool whole = (sg.k0 == 0 && sg.k1 == c.C);
         bool finalize = whole;
         if (!whole) {
-            const int lo_b = range_lo(b, cut);
-            const int which = (sg.pos == lo_b) ? 0 : 1;
-            float* slot = P.partial + (size_t((sg.ph & 1) * G + b) * 2 + which) * 2048;
+            // The panel is shared with neighbouring CTAs: every holder adds its piece to the panel's fp32 accumulator in
+            // the workspace (red.add, fire and forget) and arrives; the last arriver takes the sum, leaves zeros behind
+            // and finalises.  One round trip whatever the number of pieces (the sum order, hence the last bits of y of
+            // such panels, depends on arrival order -- inside the tolerance, PAPER.md leaves the order free).
+            const int p_begin = c.chunk_base + sg.panel * c.C;
+            const int c_first = cta_of(p_begin, cut);
+            const int parts = cut.per == 0 ? c.C : cta_of(p_begin + c.C - 1, cut) - c_first + 1;
+            float* accum = P.partial + size_t((sg.ph & 1) * G + c_first) * 2048 + row;
 #pragma unroll
-            for (int m = 0; m < 16; ++m) slot[m * 128 + row] = acc[m];
+            for (int m = 0; m < 16; ++m) atomicAdd(accum + m * 128, acc[m]);
             epi_bar();
             LS_STAMP(41);
-            const int p_begin = c.chunk_base + sg.panel * c.C, p_end = p_begin + c.C;
             if (et == 0) {
-                // CTAs that hold a piece of this panel (ranges may be empty when the phase has fewer chunks than CTAs)
-                int parts = 0;
-                for (int pos = p_begin; pos < p_end; pos = range_lo(cta_of(pos, cut) + 1, cut)) ++parts;
                 unsigned* ctr = P.counters + c.panel_base + sg.panel;
-                const unsigned old = atom_add_acq_rel(ctr, 1);      // releases this CTA's partial, acquires the others'
+                const unsigned old = atom_add_acq_rel(ctr, 1);      // releases this CTA's adds, acquires the others'
                 const int last = (old == unsigned(parts - 1));
                 if (last) *ctr = 0;                                  // self-cleaning
                 B->flag = last;
@@ -551,32 +573,9 @@ __device__ void finaliser(const LsParams& P, const float* part, float* us, Bars*
             finalize = (B->flag != 0);
             if (finalize) {
 #pragma unroll
-                for (int m = 0; m < 16; ++m) acc[m] = 0.f;
-                // partials are summed in CTA order (bitwise reproducible); two CTAs' loads are in flight
-                // before the first add so that their L2 round trips overlap
-                for (int pos = p_begin; pos < p_end;) {
-                    const float* sj[2];
-                    int np = 0;
-                    for (; np < 2 && pos < p_end; ++np) {
-                        const int cq = cta_of(pos, cut);
-                        const int wq = (pos == range_lo(cq, cut)) ? 0 : 1;
-                        sj[np] = P.partial + (size_t((sg.ph & 1) * G + cq) * 2 + wq) * 2048 + row;
-                        pos = range_lo(cq + 1, cut);
-                    }
-                    float tmp[2][16];
+                for (int m = 0; m < 16; ++m) acc[m] = __ldcg(accum + m * 128);
 #pragma unroll
-                    for (int e = 0; e < 2; ++e)
-                        if (e < np) {
-#pragma unroll
-                            for (int m = 0; m < 16; ++m) tmp[e][m] = __ldcg(sj[e] + m * 128);
-                        }
-#pragma unroll
-                    for (int e = 0; e < 2; ++e)
-                        if (e < np) {
-#pragma unroll
-                            for (int m = 0; m < 16; ++m) acc[m] += tmp[e][m];
-                        }
-                }
+                for (int m = 0; m < 16; ++m) accum[m * 128] = 0.f;
             }
         }
         LS_STAMP(43);
@@ -593,9 +592,9 @@ __device__ void finaliser(const LsParams& P, const float* part, float* us, Bars*
                     epi_bar();
                 }
                 const uint4* Brow = reinterpret_cast<const uint4*>(c.B + size_t(nrow) * c.r);
-#pragma unroll 2
+#pragma unroll 4
                 for (int j8 = 0; j8 < c.r / 8; ++j8) {
-                    const uint4 bv = __ldg(Brow + j8);
+                    const uint4 bv = j8 < 4 ? bpre[j8 & 3] : __ldg(Brow + j8);
                     const __half2* bh = reinterpret_cast<const __half2*>(&bv);
                     float bf[8];
 #pragma unroll
@@ -646,7 +645,8 @@ __device__ __forceinline__ void ec_load16(const __half* row, int col, uint32_t (
         for (int i = 0; i < 4; ++i) lo[i] = hi[i] = 0u;
     }
 }
-__device__ void ec_call(const LsParams& P, int ci, int lane) {
+// this CTA's share of z = x [A; w_g]^T of call ci, added to the global fp32 z (red.add); no synchronisation here
+__device__ void ec_partial(const LsParams& P, int ci, int lane) {
     const LsCall& c = P.calls[ci];
     const int g = lane >> 2, t = lane & 3, G = gridDim.x;
     const bool scalar = (c.gate_kind == SPEAR_GATE_SCALAR_SIGMOID);
@@ -688,13 +688,14 @@ __device__ void ec_call(const LsParams& P, int ci, int lane) {
             }
         }
     }
-    __syncwarp();
+}
+// z of call ci is complete (the gate needs the fully reduced z): gate (S5), u = alpha gamma z (S6),
+// publish u behind the call's flag, leave z zeroed for the next launch
+__device__ void ec_gate(const LsParams& P, int ci, int lane) {
+    const LsCall& c = P.calls[ci];
+    const bool scalar = (c.gate_kind == SPEAR_GATE_SCALAR_SIGMOID);
+    float* z = P.zbuf + size_t(c.ec_slot) * 16 * kZStride;
     unsigned* sync = P.ec_sync + 2 * c.ec_slot;
-    unsigned old = 0;
-    if (lane == 0) old = atom_add_acq_rel(sync, 1u);
-    old = __shfl_sync(0xffffffffu, old, 0);
-    if (old != unsigned(G - 1)) return;
-    // last arriver: z is complete -> gate (S5), u = alpha gamma z (S6)
     const float bias = (scalar && c.b_g) ? __ldg(c.b_g) : 0.f;
     float* u = P.ubuf + size_t(c.ec_slot) * 2048;
     for (int idx = lane; idx < c.M * c.r; idx += 32) {
@@ -714,15 +715,26 @@ __device__ void ec_call(const LsParams& P, int ci, int lane) {
         red_add_release(sync + 1, 1u);
     }
 }
-// Phase 0 (x comes from outside the launch): its calls are shared by five warps (the EC warp and the four finaliser
-// warps, idle until the first segment is through), so that their memory round trips overlap.  Later phases (x is an
-// earlier phase's y) belong to the EC warp alone.
-__device__ void ec_phase0(const LsParams& P, int lane, int e) {
-    for (int ci = P.phase_first_call[0] + e; ci < P.phase_first_call[1]; ci += 5)
-        if (P.calls[ci].r > 0) ec_call(P, ci, lane);
+// a call of a later phase (x is an earlier phase's y): the EC warp of every CTA adds its share and arrives; the last
+// arriver applies the gate
+__device__ void ec_call(const LsParams& P, int ci, int lane) {
+    ec_partial(P, ci, lane);
+    __syncwarp();
+    unsigned* sync = P.ec_sync + 2 * P.calls[ci].ec_slot;
+    unsigned old = 0;
+    if (lane == 0) old = atom_add_acq_rel(sync, 1u);
+    old = __shfl_sync(0xffffffffu, old, 0);
+    if (old == gridDim.x - 1) ec_gate(P, ci, lane);
 }
+// Phase 0 (x comes from outside the launch): the worker warps add the z shares in the launch prologue (one arrive per CTA
+// covers them and the x rewrite); the gate of call ci is then applied by the EC warp of CTA ci mod gridDim.x.
 __device__ void ec_warp(const LsParams& P, int lane) {
-    ec_phase0(P, lane, 4);
+    bool waited = false;
+    for (int ci = P.phase_first_call[0]; ci < P.phase_first_call[1]; ++ci) {
+        if (P.calls[ci].r == 0 || ci % int(gridDim.x) != int(blockIdx.x)) continue;
+        if (!waited) { wait_counter(P.done + kLsMaxCalls + 1, gridDim.x); waited = true; }
+        ec_gate(P, ci, lane);
+    }
     for (int ph = 1; ph < P.n_phases; ++ph) {
         wait_counter(P.done + ph - 1, unsigned(P.phase_panels[ph - 1]));
         for (int ci = P.phase_first_call[ph]; ci < P.phase_first_call[ph + 1]; ++ci)
@@ -733,6 +745,9 @@ __device__ void ec_warp(const LsParams& P, int lane) {
 
 __global__ void __launch_bounds__(ls::kThreads, 1) ls_kernel(const __grid_constant__ LsParams P) {
     using namespace ls;
+#ifdef LS_TRACE
+    const unsigned long long t_entry = ls_now();
+#endif
     extern __shared__ uint8_t smem_raw[];
     uint8_t* base = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
     uint8_t* xring = base + Smem::x;
@@ -777,11 +792,12 @@ __global__ void __launch_bounds__(ls::kThreads, 1) ls_kernel(const __grid_consta
     } else if (warp == 2) {
         ec_warp(P, lane);
     } else if (warp < 8) {
-        ec_phase0(P, lane, warp - 4);
         finaliser(P, part, us, B, warp, lane);
     } else if (warp < 8 + 4 * kPipes) {
         // prologue: x -> operand layout (workspace), one arrive per CTA once its 16 worker warps are through
         x_prologue(P, threadIdx.x - 256, 128 * kPipes);
+        for (int ci = P.phase_first_call[0] + (warp - 8); ci < P.phase_first_call[1]; ci += 4 * kPipes)
+            if (P.calls[ci].r > 0) ec_partial(P, ci, lane);
         __threadfence();
         named_bar_sync(2, 128 * kPipes);
         if (threadIdx.x == 256) { asm volatile("fence.proxy.async;" ::: "memory"); red_add_release(P.done + kLsMaxCalls + 1, 1u); }
@@ -808,6 +824,9 @@ __global__ void __launch_bounds__(ls::kThreads, 1) ls_kernel(const __grid_consta
     }
 #endif
     if (warp == 3) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem), "n"(kTmemCols) : "memory");
+#ifdef LS_TRACE
+    if (threadIdx.x == 0) printf("CTA %d entry %llu setup %llu exit %llu\n", blockIdx.x, t_entry, g_stamp[39], ls_now());
+#endif
     if (threadIdx.x == 0) {
         // the last CTA to leave resets what the next launch expects to be zero
         unsigned* exit_ctr = P.done + kLsMaxCalls;
