@@ -40,7 +40,7 @@ def build(force: bool = False, verbose: bool = False) -> str:
         o = os.path.join(OBJ, src[:-3] + ".o")
         objs.append(o)
         if force or not os.path.exists(o) or os.path.getmtime(o) < max(os.path.getmtime(s), dep_m):
-            extra = (["-DLS_TRACE"] if os.environ.get("SPEAR_LS_TRACE") else []) + os.environ.get("SPEAR_NVCC_EXTRA", "").split()
+            extra = (["-DLS_TRACE"] if os.environ.get("SPEAR_LS_TRACE") else []) + (["-DLS_TIMER"] if os.environ.get("SPEAR_LS_TIMER") else []) + os.environ.get("SPEAR_NVCC_EXTRA", "").split()
             cmd = [nvcc] + NVCC_FLAGS + extra + (["-Xptxas", "-v"] if verbose else []) + ["-c", s, "-o", o]
             jobs.append(cmd)
     if jobs:

@@ -79,7 +79,7 @@ static LsWs ls_ws_layout(int grid) {
     size_t o = 0;
     L.partial = o; o += size_t(grid) * 2 * 2 * 2048 * 4;
     L.counters = o; o += size_t(kLsMaxPanels) * 4;
-    L.done = o; o += align_up(size_t(kLsMaxCalls + 2) * 4, 1024);
+    L.done = o; o += align_up(size_t(kLsMaxCalls + 4) * 4, 1024);
     L.zbuf = o; o += align_up(size_t(kLsMaxCalls) * 16 * kZStride * 4, 1024);
     L.ubuf = o; o += size_t(kLsMaxCalls) * 2048 * 4;
     L.ec_sync = o; o += align_up(size_t(kLsMaxCalls) * 2 * 4, 1024);
@@ -135,6 +135,7 @@ static void do_init() {
         const size_t ls_bytes = ls_ws_layout(g_dev.num_sms).total;
         e = cudaMalloc(&g_ls_ws, ls_bytes);
         if (e == cudaSuccess) e = cudaMemset(g_ls_ws, 0, ls_bytes);
+        if (e == cudaSuccess) e = cudaMemset(static_cast<uint8_t*>(g_ls_ws) + ls_ws_layout(g_dev.num_sms).done + (kLsMaxCalls + 2) * 4, 0xff, 8);   // trace builds: min entry time
     }
     if (e == cudaSuccess) e = cudaDeviceSynchronize();
     if (e != cudaSuccess) {

@@ -46,7 +46,10 @@ int launch_stream(const CUtensorMap& xmap, const StreamParams& p, int MT, int gr
 // ---- lstream.cu (M <= 16): persistent "layer stream" -- ONE cooperative launch consumes a table of layer
 // calls as a single queue of (call, panel, 128-column chunk) work items; int4 -> fp16 in registers -> TMEM
 // (tcgen05.st) -> tcgen05.mma with the tokens as N = 16 (A operand in tensor memory), fp32 accumulators in TMEM.
-constexpr int kLsMaxCalls = 64;
+#ifndef LS_MAX_CALLS
+#define LS_MAX_CALLS 64
+#endif
+constexpr int kLsMaxCalls = LS_MAX_CALLS;
 struct LsCall {
     const uint8_t* wq;       // SPW4 packed codes
     const uint8_t* scales;   // SPW4 packed scales

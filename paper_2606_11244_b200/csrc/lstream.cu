@@ -45,7 +45,7 @@
 namespace spear {
 
 namespace ls {
-#ifdef LS_TRACE
+#if defined(LS_TRACE) || defined(LS_TIMER)
 __device__ __forceinline__ unsigned long long ls_now() { unsigned long long t; asm volatile("mov.u64 %0, %globaltimer;" : "=l"(t)); return t; }
 #endif
 #ifdef LS_TRACE
@@ -72,10 +72,10 @@ __device__ __forceinline__ void ls_wait_impl(uint64_t* bar, uint32_t parity, int
 #define LS_WAIT(bar, parity, tag, a, b) mbar_wait(bar, parity)
 #endif
 #ifndef LS_STAGES
-#define LS_STAGES 16
+#define LS_STAGES 10
 #endif
 static_assert(LS_STAGES % 2 == 0 && LS_STAGES >= 6, "ring depth must be even: chunk n - kStages must belong to pipeline n or n + 2 (mod 4), whose progress a worker has observed before it tests full[] by parity");
-constexpr int kStages = LS_STAGES;                 // ring depth (chunks): 16 x (8 KiB weights + 4 KiB x tile)
+constexpr int kStages = LS_STAGES;          // ring depth (chunks): 10 x (8 KiB weights + 4 KiB x tile + 256 B scales); measured 6..12: within 5 %
 constexpr int kPipes = 4;                   // dequantisation / MMA pipelines; pipeline i owns chunks n = i (mod 4)
 constexpr int kThreads = (8 + 4 * kPipes + kPipes) * 32;      // 4 service warps, 4 finalisers, 16 workers, 4 MMA issuers
 constexpr int kWBytes = 8192, kXBytes = 4096, kScBytes = 256;
@@ -135,11 +135,10 @@ __device__ __forceinline__ void wait_counter(const unsigned* p, unsigned target)
 #ifdef LS_TRACE
     long long t0 = clock64();
     while (ld_acquire(p) < target) {
-        __nanosleep(64);
         if (clock64() - t0 > 400000000ll) { printf("STUCK counter cta %d warp %d have %u want %u\n", blockIdx.x, threadIdx.x >> 5, ld_acquire(p), target); t0 = clock64() + 4000000000ll; }
     }
 #else
-    while (ld_acquire(p) < target) __nanosleep(64);
+    while (ld_acquire(p) < target) {}
 #endif
 }
 
@@ -397,7 +396,7 @@ __device__ void worker(const LsParams& P, uint8_t* wring, const uint8_t* scring,
     float sc_a = 0.f, sc_b = 0.f;      // this row's scale in the groups of own chunks n - 4 and n - 8 (read out two iterations late)
 
     // epilogue of every own chunk <= limit, plus the segment hand-overs that become due
-    auto epilogue_until = [&](int limit) {
+    auto epilogue_until = [&](int limit, int old_chunk) __attribute__((always_inline)) {
         while (!e.done) {
             if (!e.live) {
                 e.n0 = e.n1;
@@ -427,7 +426,7 @@ __device__ void worker(const LsParams& P, uint8_t* wring, const uint8_t* scring,
                     if (lane == 0) mbar_arrive(&B->d_empty[g][e.db]);
                     e.par ^= 1u << e.db;
                     e.db ^= 1;
-                    const float sc = sc_b;
+                    const float sc = (e.m == old_chunk) ? sc_b : sc_a;
 #pragma unroll
                     for (int mm = 0; mm < 16; ++mm) acc[mm] = fmaf(sc, __uint_as_float(v[mm]), acc[mm]);
                 }
@@ -447,8 +446,28 @@ __device__ void worker(const LsParams& P, uint8_t* wring, const uint8_t* scring,
         }
     };
 
-    for (int n = g; n < n_total; n += kPipes) {
-        epilogue_until(n - 2 * kPipes);      // its MMAs finished long ago: no wait, and the accumulator is free for chunk n
+    // stream position at which the next phase of this CTA starts: its x tiles exist only once the previous phase is
+    // finalised, which needs this pipeline's partial sums -- so the lagging epilogue catches up before crossing it
+    int ph_next = 1;
+    int boundary = P.n_phases > 1 ? P.phase_per[0] + (int(blockIdx.x) < P.phase_rem[0] ? 1 : 0) : 0x7fffffff;
+    for (int n = g;; n += kPipes) {
+        // epilogue of own chunk n - 8 (its MMAs finished long ago: no wait, and the accumulator is free for chunk n);
+        // also of chunk n - 4 when chunk n opens a new phase; past the end of the stream: whatever is left
+        int limit = n - 2 * kPipes;
+        if (n >= boundary) {
+            limit = n - kPipes;
+            while (n >= boundary) {
+                boundary = ph_next < P.n_phases - 1 ? boundary + P.phase_per[ph_next] + (int(blockIdx.x) < P.phase_rem[ph_next] ? 1 : 0)
+                                                    : 0x7fffffff;
+                ++ph_next;
+            }
+        }
+        epilogue_until(limit, n - 2 * kPipes);
+        if (n >= n_total) {
+            if (e.done) break;
+            sc_b = sc_a;
+            continue;
+        }
         const int s = n % kStages, slot = n % kASlots;
         const uint32_t t_lane = t_quarter + slot * 64;
         LS_WAIT(&B->a_empty[slot], ((n / kASlots) & 1) ^ 1, 8, n, 0);
@@ -487,13 +506,6 @@ __device__ void worker(const LsParams& P, uint8_t* wring, const uint8_t* scring,
             mbar_arrive(&B->a_full[slot]);
             mbar_arrive(&B->empty[s]);
         }
-    }
-    // the last two own chunks
-    {
-        const int n_next = g + ((n_total - g + kPipes - 1) / kPipes) * kPipes;      // first own position >= n_total
-        epilogue_until(n_next - 2 * kPipes);
-        sc_b = sc_a;
-        epilogue_until(0x7fffffff - kPipes);
     }
 }
 }  // namespace ls
@@ -827,6 +839,9 @@ __global__ void __launch_bounds__(ls::kThreads, 1) ls_kernel(const __grid_consta
 #ifdef LS_TRACE
     if (threadIdx.x == 0) printf("CTA %d entry %llu setup %llu exit %llu\n", blockIdx.x, t_entry, g_stamp[39], ls_now());
 #endif
+#if defined(LS_TRACE) || defined(LS_TIMER)
+    if (threadIdx.x == 0) atomicMin(reinterpret_cast<unsigned long long*>(P.done + kLsMaxCalls + 2), t_entry);
+#endif
     if (threadIdx.x == 0) {
         // the last CTA to leave resets what the next launch expects to be zero
         unsigned* exit_ctr = P.done + kLsMaxCalls;
@@ -837,6 +852,11 @@ __global__ void __launch_bounds__(ls::kThreads, 1) ls_kernel(const __grid_consta
                 if (P.calls[ci].ec_slot >= 0) P.ec_sync[2 * P.calls[ci].ec_slot + 1] = 0;
             exit_ctr[0] = 0;
             exit_ctr[1] = 0;
+#if defined(LS_TRACE) || defined(LS_TIMER)
+            unsigned long long* tmin = reinterpret_cast<unsigned long long*>(P.done + kLsMaxCalls + 2);
+            printf("KERNEL %llu ns (first entry -> last exit), chunks/cta %d\n", ls_now() - *tmin, total_chunks(P));
+            *tmin = ~0ull;
+#endif
         }
     }
 }
