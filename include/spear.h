@@ -96,7 +96,7 @@ int spear_w4_ec_gemm(const void* x, const void* Wq, const void* scales, const vo
 /* Extended form: everything the paper's EC needs that the 14-argument form cannot express. */
 typedef struct {
     int gate_kind;            /* spear_gate_kind                                                    */
-    int gate_hidden;          /* h, MLP gate only (1 <= h <= 512, reading A2: default 4r)           */
+    int gate_hidden;          /* h, MLP gate only (8 <= h <= 512, h % 8 == 0; reading A2: default 4r) */
     float alpha;              /* Eq. 3 alpha (reading A3)                                           */
     const void* W1;           /* [h][r] fp16   MLP gate                                             */
     const void* b1;           /* [h]    fp32                                                        */
@@ -118,11 +118,13 @@ int spear_w4_ec_gemm_ex(const void* x, const void* Wq, const void* scales, const
                         const spear_ec_desc* ec, void* y,
                         int M, int N, int K, int r, int group, void* stream);
 
-/* A batch of INDEPENDENT layer calls (no call reads another call's y; all y buffers distinct), e.g. the
- * q/k/v or gate/up projections of one transformer block, or unrelated requests.  The calls run
- * concurrently on the library's internal lanes (up to 16 streams with their own workspaces); all of them are
- * ordered after the work already enqueued on `stream` and before anything enqueued on it afterwards
- * (fork / join with events; capturable in a CUDA graph).  ec->workspace must be NULL.  The
+/* A batch of layer calls, e.g. the projections of one or several transformer blocks, or unrelated requests.
+ * Independent calls run concurrently on the library's internal lanes (up to 16 streams with their own workspaces), or --
+ * for M <= 16, when spear_plan_batch measured it faster or spear_tune("lstream", 1) -- as ONE persistent layer-stream
+ * launch.  A call may read an earlier call's y as its x (same pointer, same M, K == that call's N): such chains are
+ * ordered (one after the other on `stream`, or as dependency phases inside the layer-stream launch).  Everything is
+ * ordered after the work already enqueued on `stream` and before anything enqueued on it afterwards (capturable in a
+ * CUDA graph).  ec->workspace must be NULL.  The
  * per-token-gated EC of every call is evaluated exactly as in spear_w4_ec_gemm_ex. */
 typedef struct {
     const void *x, *Wq, *scales, *A, *B;
@@ -152,10 +154,14 @@ int spear_w4_ec_gemm_hostio(const void* x_host, void* y_host, void* x_dev, void*
 /* Workspace a call of this shape may need (upper bound over variants). */
 int spear_workspace_bytes(int M, int N, int K, int r, int group, size_t* bytes);
 
-/* Allocates (once per process, current device) and zero-fills the default workspace and reads the
- * device properties.  Called implicitly by the first compute call; call it explicitly before
- * capturing a CUDA graph.  Synchronises the device. */
+/* Allocates (once per process, current device) and zero-fills the library's own device memory and reads the device
+ * properties: the default workspace (96 MiB), 16 batch lanes (a stream + 48 MiB workspace each) and the layer-stream
+ * kernel's workspace (~40 MiB: split-K accumulators, counters, EC state, 32 MiB of x in the MMA operand layout) --
+ * spear_memory_bytes() reports the total.  No compute call allocates anything after that; a caller who wants to own
+ * the memory passes spear_ec_desc.workspace (single calls).  Called implicitly by the first compute call; call it
+ * explicitly before capturing a CUDA graph.  Synchronises the device. */
 int spear_init(void);
+int spear_memory_bytes(size_t* bytes);   /* device bytes spear_init allocates */
 
 /* ---- S9: measured dispatch ---------------------------------------------------------------- */
 
@@ -168,6 +174,11 @@ int spear_plan(int M, int N, int K, int r, int group, int gate_kind, int gate_hi
                int* chosen_variant_out, float* times_us_out, void* stream);
 int spear_plan_save(const char* path);   /* text file, one line per planned problem (host path) */
 int spear_plan_load(const char* path);
+/* S9 for batches: times the two ways of running THIS batch of M <= 16 calls on the caller's own
+ * buffers (the y buffers are overwritten) -- 0: per-call kernels (concurrent lanes, or one after the other when calls read
+ * each other's y), 1: ONE persistent layer-stream launch -- and records the winner for every later batch with the same
+ * shapes.  times_us_out[2] (host, may be NULL): microseconds per batch, negative = not applicable.  Synchronises. */
+int spear_plan_batch(const spear_call* calls, int n_calls, int* chosen_out, float* times_us_out, void* stream);
 /* The variant AUTO would run for this problem right now (table hit or heuristic). */
 int spear_plan_query(int M, int N, int K, int r, int group, int gate_kind, int* variant_out);
 

@@ -24,8 +24,8 @@ VARIANT_NAMES = ["auto", "stream_fused", "stream_split", "tc_fused", "tc_split",
 EXPORTS = [
     "spear_pack_w4_sizes", "spear_pack_w4", "spear_unpack_w4", "spear_dequant_w4",
     "spear_w4_ec_gemm", "spear_w4_ec_gemm_ex", "spear_w4_ec_gemm_hostio", "spear_w4_ec_gemm_batch", "spear_w4_ec_gemm_batch_hostio",
-    "spear_workspace_bytes", "spear_init", "spear_plan", "spear_plan_save", "spear_plan_load",
-    "spear_plan_query", "spear_tune", "spear_last_error", "spear_launch_count",
+    "spear_workspace_bytes", "spear_init", "spear_memory_bytes", "spear_plan", "spear_plan_save", "spear_plan_load",
+    "spear_plan_query", "spear_plan_batch", "spear_tune", "spear_last_error", "spear_launch_count",
 ]
 
 
@@ -82,10 +82,12 @@ def lib():
         L.spear_w4_ec_gemm_hostio.argtypes = [vp] * 8 + [ctypes.POINTER(EcDesc)] + [ci] * 5 + [vp]
         L.spear_workspace_bytes.argtypes = [ci] * 5 + [ctypes.POINTER(ctypes.c_size_t)]
         L.spear_init.argtypes = []
+        L.spear_memory_bytes.argtypes = [ctypes.POINTER(ctypes.c_size_t)]
         L.spear_plan.argtypes = [ci] * 7 + [ctypes.POINTER(ci), ctypes.POINTER(ctypes.c_float), vp]
         L.spear_plan_save.argtypes = [ctypes.c_char_p]
         L.spear_plan_load.argtypes = [ctypes.c_char_p]
         L.spear_plan_query.argtypes = [ci] * 6 + [ctypes.POINTER(ci)]
+        L.spear_plan_batch.argtypes = [ctypes.POINTER(Call), ci, ctypes.POINTER(ci), ctypes.POINTER(ctypes.c_float), vp]
         L.spear_tune.argtypes = [ctypes.c_char_p, ci]
         L.spear_last_error.restype = ctypes.c_char_p
         L.spear_launch_count.restype = ctypes.c_ulonglong
@@ -263,6 +265,14 @@ def plan(M, N, K, r, group, gate="scalar", gate_hidden=0, stream=None):
     times = (ctypes.c_float * VARIANT_COUNT)()
     _check(lib().spear_plan(M, N, K, r, group, GATE_KINDS[gate], gate_hidden, ctypes.byref(chosen), times,
                             _stream(stream)))
+    return chosen.value, [float(t) for t in times]
+
+
+def plan_batch(batch, stream=None):
+    """spear_plan_batch: times lanes / sequential kernels vs ONE layer-stream launch for this batch; returns (chosen, [us, us])."""
+    chosen = ctypes.c_int(-1)
+    times = (ctypes.c_float * 2)()
+    _check(lib().spear_plan_batch(batch.calls, batch.n, ctypes.byref(chosen), times, _stream(stream)))
     return chosen.value, [float(t) for t in times]
 
 

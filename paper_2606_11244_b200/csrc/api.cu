@@ -181,7 +181,10 @@ int get_tensor_map_2d(const void* base, uint64_t rows, uint64_t cols, uint64_t r
         return set_error(SPEAR_ECUDA, "cuTensorMapEncodeTiled failed (%d) rows=%llu cols=%llu stride=%llu box=%ux%u",
                          int(rc), (unsigned long long)rows, (unsigned long long)cols,
                          (unsigned long long)row_stride_bytes, box_rows, box_cols);
-    if (g_maps.size() > 8192) g_maps.clear();
+    if (g_maps.size() > 8192) {      // bounded cache: drop every other entry rather than all of them at once
+        bool drop = false;
+        for (auto it2 = g_maps.begin(); it2 != g_maps.end(); drop = !drop) it2 = drop ? g_maps.erase(it2) : std::next(it2);
+    }
     g_maps[key] = m;
     *out = m;
     return SPEAR_OK;
@@ -208,7 +211,10 @@ int get_tensor_map_x3d(const void* base, uint64_t rows, uint64_t cols, uint32_t 
     if (rc != CUDA_SUCCESS)
         return set_error(SPEAR_ECUDA, "cuTensorMapEncodeTiled (3-D x view) failed (%d) rows=%llu cols=%llu", int(rc),
                          (unsigned long long)rows, (unsigned long long)cols);
-    if (g_maps.size() > 8192) g_maps.clear();
+    if (g_maps.size() > 8192) {
+        bool drop = false;
+        for (auto it2 = g_maps.begin(); it2 != g_maps.end(); drop = !drop) it2 = drop ? g_maps.erase(it2) : std::next(it2);
+    }
     g_maps[key] = m;
     *out = m;
     return SPEAR_OK;
@@ -228,16 +234,14 @@ struct Tunables {
     int tc_xslice_mb = 0;         // 0 = default (16), MiB of x per raster group
     int batch_lanes = 16;         // concurrent lanes of spear_w4_ec_gemm_batch (1..16); measured 12 > 8 > 4 on the 12-call step
     int stream_deep = -1;         // -1 = heuristic, 0 / 1 = force the shallow / deep decode ring
-    int stream_debug = 0;         // measurement hook, see StreamParams::debug
     int stream_batch_grid = 128;  // cap of the decode grid inside a batch (0 = off); measured 128 > 148 > 96
     int stream_batch_units = 8;   // target units per CTA inside a batch (0 = off); measured 8-10 > 4 > 16 > even split
     int ecbig_kdiv = 0;           // 0 = default 2 (measured 1-2 > 4): minimum k-tiles per K split of the M > 16 EC pre-pass
     int stream_units = 0;         // the same target for stream-ordered calls (0 = off: use every SM)
-    int lstream = 1;              // 1 = M <= 16 calls (single and batched) take the persistent layer-stream kernel
+    int lstream = -1;             // layer-stream kernel for M <= 16: -1 = where the plan tables measured it faster (chains always), 0 = never, 1 = always
     int stream_whole_panels = 1;  // 1 = whole-panel partition when N/128 is within 1/5 of the grid
 };
 static Tunables g_tune;
-extern int g_ls_coop;
 static thread_local bool t_in_batch = false;
 
 struct PlanKey {
@@ -262,7 +266,7 @@ static bool variant_valid(int v, int M, int r, int gate) {
     (void)r;
 }
 static int heuristic_variant(int M, int r, int gate) {
-    if (M <= 16 && g_tune.lstream && gate != SPEAR_GATE_MLP) return SPEAR_VARIANT_LSTREAM;
+    if (M <= 16 && g_tune.lstream == 1 && gate != SPEAR_GATE_MLP) return SPEAR_VARIANT_LSTREAM;
     if (M <= 16) return (r > 0 && gate != SPEAR_GATE_MLP) ? SPEAR_VARIANT_STREAM_FUSED : SPEAR_VARIANT_STREAM_SPLIT;
     return SPEAR_VARIANT_TC_FUSED;
 }
@@ -304,6 +308,25 @@ static int check_problem(const void* x, const void* Wq, const void* scales, cons
         }
     }
     if (al & 15) return set_error(SPEAR_EINVAL, "device pointers must be 16-byte aligned");
+    return SPEAR_OK;
+}
+
+// zbuf (kept zero between calls) grows up, the tcgen05 path's u16 scratch grows down from the end of the same workspace:
+// a call with a larger M than any before may find stale u16 bytes where it expects zeros.  Per workspace the lowest
+// offset that may be non-zero is tracked; a call whose zbuf reaches it clears the overlap first (stream-ordered).
+static std::map<const void*, size_t> g_ws_dirty_lo;
+static std::mutex g_ws_mutex;
+static int ws_prepare(uint8_t* ws, size_t ws_bytes, const WsLayout& L, int M, int r, bool uses_u16, cudaStream_t st) {
+    const size_t zend = L.zbuf + align_up(size_t(M > 16 ? M : 16) * kZStride * 4, 1024);
+    std::lock_guard<std::mutex> lock(g_ws_mutex);
+    auto it = g_ws_dirty_lo.find(ws);
+    size_t lo = (it == g_ws_dirty_lo.end()) ? ws_bytes : it->second;
+    if (r > 0 && zend > lo) {
+        SPEAR_CUDA_OK(cudaMemsetAsync(ws + lo, 0, zend - lo, st));
+        lo = zend;
+    }
+    if (uses_u16 && r > 0) lo = std::min(lo, L.u16);
+    g_ws_dirty_lo[ws] = lo;
     return SPEAR_OK;
 }
 
@@ -362,7 +385,7 @@ static int run_stream(const void* x, const void* Wq, const void* scales, const v
     if (g_tune.stream_deep >= 0) deep = g_tune.stream_deep != 0;
     if (deep) per_sm = 1;
     p.stages = stream_stages(MT, deep);
-    p.debug = g_tune.stream_debug;
+    per_sm = std::min(per_sm, stream_resident_ctas(MT, deep));      // what really fits (occupancy query), not an assumption
     int grid = std::min(p.U, g_dev.num_sms * per_sm);
     grid = std::min(grid, kMaxStreamGrid);
     // When the panels nearly fill the machine, give every CTA whole panels: an even stream-K split would cut almost
@@ -388,7 +411,6 @@ static int run_stream(const void* x, const void* Wq, const void* scales, const v
         p.w_g = static_cast<const __half*>(ec->w_g);
         p.b_g = static_cast<const float*>(ec->b_g);
         p.zbuf = reinterpret_cast<float*>(ws + L.zfused);
-        p.u_out = u32;
         p.gate_out = static_cast<float*>(ec->gate_out);
         p.ec_sync = counters + kEcPreCounter + 16;
     }
@@ -602,6 +624,7 @@ static int layer_impl(const void* x, const void* Wq, const void* scales, const v
         spear_call c = {x, Wq, scales, A, B, ec, y, M, N, K, r, group};
         return run_lstream(&c, 1, st);
     }
+    if (int rc = ws_prepare(ws, ws_bytes, L, M, r, v == SPEAR_VARIANT_TC_FUSED || v == SPEAR_VARIANT_TC_SPLIT, st)) return rc;
     switch (v) {
         case SPEAR_VARIANT_STREAM_FUSED:
             return run_stream(x, Wq, scales, A, B, ec, y, M, N, K, r, group, ws, L, true, st);
@@ -626,6 +649,12 @@ extern "C" int spear_init(void) {
     return SPEAR_OK;
 }
 
+extern "C" int spear_memory_bytes(size_t* bytes) {
+    if (!bytes) return set_error(SPEAR_EINVAL, "NULL bytes");
+    *bytes = kDefaultWorkspace + size_t(kBatchLanes) * kLaneWorkspace + ls_ws_layout(g_dev.num_sms > 0 ? g_dev.num_sms : SPEAR_NUM_SMS_FALLBACK).total;
+    return SPEAR_OK;
+}
+
 extern "C" const char* spear_last_error(void) { return g_err; }
 extern "C" unsigned long long spear_launch_count(void) { return g_launches.load(); }
 
@@ -641,9 +670,7 @@ extern "C" int spear_tune(const char* key, int value) {
     else if (!strcmp(key, "tc_xslice_mb")) g_tune.tc_xslice_mb = value;
     else if (!strcmp(key, "batch_lanes")) g_tune.batch_lanes = value;
     else if (!strcmp(key, "stream_deep")) g_tune.stream_deep = value;
-    else if (!strcmp(key, "stream_debug")) g_tune.stream_debug = value;
     else if (!strcmp(key, "lstream")) g_tune.lstream = value;
-    else if (!strcmp(key, "ls_coop")) spear::g_ls_coop = value;
     else if (!strcmp(key, "stream_whole_panels")) g_tune.stream_whole_panels = value;
     else if (!strcmp(key, "stream_batch_grid")) g_tune.stream_batch_grid = value;
     else if (!strcmp(key, "stream_batch_units")) g_tune.stream_batch_units = value;
@@ -679,7 +706,26 @@ extern "C" int spear_w4_ec_gemm(const void* x, const void* Wq, const void* scale
     return layer_impl(x, Wq, scales, A, B, &ec, y, M, N, K, r, group, static_cast<cudaStream_t>(stream));
 }
 
-static int batch_impl(const spear_call* calls, const spear_host_io* io, int n_calls, void* stream);
+// S9 for batches: the two ways to run a batch of M <= 16 calls -- concurrent lanes of per-call kernels, or ONE persistent
+// layer-stream launch -- are timed by spear_plan_batch and the winner is remembered per batch signature (shapes only).
+static std::map<std::vector<int>, int> g_batch_plan;      // signature -> 0 lanes, 1 layer-stream
+static std::vector<int> batch_signature(const spear_call* calls, int n) {
+    std::vector<int> sig;
+    sig.reserve(size_t(n) * 6);
+    for (int i = 0; i < n; ++i) {
+        const int gate = (calls[i].r > 0 && calls[i].ec) ? calls[i].ec->gate_kind : SPEAR_GATE_NONE;
+        const int v[6] = {calls[i].M, calls[i].N, calls[i].K, calls[i].r, calls[i].group, gate};
+        sig.insert(sig.end(), v, v + 6);
+    }
+    return sig;
+}
+static bool batch_has_chain(const spear_call* calls, int n) {
+    for (int i = 1; i < n; ++i)
+        for (int j = 0; j < i; ++j)
+            if (calls[i].x == calls[j].y) return true;
+    return false;
+}
+static int batch_impl(const spear_call* calls, const spear_host_io* io, int n_calls, void* stream, int mode = -1);
 
 extern "C" int spear_w4_ec_gemm_batch(const spear_call* calls, int n_calls, void* stream) {
     return batch_impl(calls, nullptr, n_calls, stream);
@@ -690,15 +736,37 @@ extern "C" int spear_w4_ec_gemm_batch_hostio(const spear_call* calls, const spea
     return batch_impl(calls, io, n_calls, stream);
 }
 
-static int batch_impl(const spear_call* calls, const spear_host_io* io, int n_calls, void* stream) {
+static int batch_impl(const spear_call* calls, const spear_host_io* io, int n_calls, void* stream, int mode) {
     if (!calls || n_calls < 0) return set_error(SPEAR_EINVAL, "bad batch");
     if (n_calls == 0) return SPEAR_OK;
     if (int rc = spear_init()) return rc;
     cudaStream_t st = static_cast<cudaStream_t>(stream);
-    if (!io && g_tune.lstream) {
+    const bool chain = batch_has_chain(calls, n_calls);
+    if (!io) {
         bool all = true;
         for (int i = 0; i < n_calls && all; ++i) all = ls_eligible(calls[i]);
-        if (all) return run_lstream(calls, n_calls, st);
+        bool take = false;
+        if (mode == 1) {
+            if (!all) return set_error(SPEAR_EUNSUPPORTED, "the layer-stream kernel needs M <= 16, scalar / none gates, power-of-two or per-channel groups");
+            take = true;
+        } else if (mode < 0 && all && g_tune.lstream != 0) {
+            take = (g_tune.lstream == 1);
+            if (!take) {       // ask the batch plan
+                std::lock_guard<std::mutex> lock(g_plan_mutex);
+                auto it = g_batch_plan.find(batch_signature(calls, n_calls));
+                take = (it != g_batch_plan.end() && it->second == 1);
+            }
+        }
+        if (take) return run_lstream(calls, n_calls, st);
+    }
+    if (chain) {
+        // calls that read each other's y: one after the other on the caller's stream (PDL-chained kernels)
+        if (io) return set_error(SPEAR_EUNSUPPORTED, "host-io batches must consist of independent calls");
+        for (int i = 0; i < n_calls; ++i) {
+            const spear_call& c = calls[i];
+            if (int rc = layer_impl(c.x, c.Wq, c.scales, c.A, c.B, c.ec, c.y, c.M, c.N, c.K, c.r, c.group, st)) return rc;
+        }
+        return SPEAR_OK;
     }
     const int lanes = std::max(1, std::min(kBatchLanes, std::min(n_calls, g_tune.batch_lanes)));
     // longest-processing-time-first assignment by weight bytes
@@ -747,8 +815,10 @@ static int batch_impl(const spear_call* calls, const spear_host_io* io, int n_ca
     t_in_batch = false;
     // always join, also after an error, so that `stream` stays consistent (and a capture stays valid)
     for (int l = 0; l < lanes; ++l) {
-        cudaEventRecord(g_lane_done[l], g_lane_stream[l]);
-        cudaStreamWaitEvent(st, g_lane_done[l], 0);
+        cudaError_t je = cudaEventRecord(g_lane_done[l], g_lane_stream[l]);
+        if (je == cudaSuccess) je = cudaStreamWaitEvent(st, g_lane_done[l], 0);
+        if (je != cudaSuccess && status == SPEAR_OK)
+            status = set_error(SPEAR_ECUDA, "batch join of lane %d failed: %s", l, cudaGetErrorString(je));
     }
     return status;
 }
@@ -793,19 +863,29 @@ extern "C" int spear_plan(int M, int N, int K, int r, int group, int gate_kind, 
         return set_error(SPEAR_EUNSUPPORTED, "spear_plan: unsupported problem");
     const int G = K / group;
     const int h = gate_kind == SPEAR_GATE_MLP ? (gate_hidden > 0 ? gate_hidden : 4 * r) : 0;
-    DevBuf x, wq, sc, A, B, y, wg, bg, W1, b1, W2, b2;
+    // The weights and EC factors of every timed launch come from a different copy (>= 2 x L2 in total), so that the table
+    // ranks the variants on weights read from HBM, as in serving, not on an L2-resident layer.
+    const size_t copy_bytes = size_t(N) * K / 2 + size_t(N) * G * 2 + size_t(r) * (size_t(K) + N) * 2;
+    int nc = int(std::min<size_t>(32, ((size_t(256) << 20) + copy_bytes - 1) / copy_bytes));
+    while (nc > 1 && copy_bytes * nc > (size_t(3) << 29)) --nc;
+    DevBuf x, y, wg, bg, W1, b1, W2, b2;
+    std::vector<DevBuf> wq(nc), sc(nc), A(nc), B(nc);
     // finite, small fp16 patterns: 0x2xxx..0x2fff ~ [0.008, 0.12]; codes any nibble
-    if (x.alloc(size_t(M) * K * 2) || wq.alloc(size_t(N) * K / 2) || sc.alloc(size_t(N) * G * 2) ||
-        y.alloc(size_t(M) * N * 2) || A.alloc(size_t(r) * K * 2) || B.alloc(size_t(N) * r * 2) ||
-        wg.alloc(size_t(K) * 2) || bg.alloc(16) || W1.alloc(size_t(h) * r * 2) || b1.alloc(size_t(h) * 4) ||
-        W2.alloc(size_t(r) * h * 2) || b2.alloc(size_t(r) * 4))
-        return set_error(SPEAR_ENOMEM, "spear_plan: cudaMalloc failed");
+    bool bad = x.alloc(size_t(M) * K * 2) || y.alloc(size_t(M) * N * 2) || wg.alloc(size_t(K) * 2) || bg.alloc(16) ||
+               W1.alloc(size_t(h) * r * 2) || b1.alloc(size_t(h) * 4) || W2.alloc(size_t(r) * h * 2) || b2.alloc(size_t(r) * 4);
+    for (int c = 0; c < nc && !bad; ++c)
+        bad = wq[c].alloc(size_t(N) * K / 2) || sc[c].alloc(size_t(N) * G * 2) || A[c].alloc(size_t(r) * K * 2) || B[c].alloc(size_t(N) * r * 2);
+    if (bad) return set_error(SPEAR_ENOMEM, "spear_plan: cudaMalloc failed");
     fill(x.p, size_t(M) * K * 2, 2654435761u, 0x0fff0fffu, 0x20002000u, st);
-    fill(wq.p, size_t(N) * K / 2, 2246822519u, 0xffffffffu, 0u, st);
-    fill(sc.p, size_t(N) * G * 2, 3266489917u, 0x03ff03ffu, 0x20002000u, st);
+    for (int c = 0; c < nc; ++c) {
+        fill(wq[c].p, size_t(N) * K / 2, 2246822519u + 2u * c, 0xffffffffu, 0u, st);
+        fill(sc[c].p, size_t(N) * G * 2, 3266489917u, 0x03ff03ffu, 0x20002000u, st);
+        if (r > 0) {
+            fill(A[c].p, size_t(r) * K * 2, 668265263u, 0x0fff0fffu, 0x20002000u, st);
+            fill(B[c].p, size_t(N) * r * 2, 374761393u, 0x0fff0fffu, 0x20002000u, st);
+        }
+    }
     if (r > 0) {
-        fill(A.p, size_t(r) * K * 2, 668265263u, 0x0fff0fffu, 0x20002000u, st);
-        fill(B.p, size_t(N) * r * 2, 374761393u, 0x0fff0fffu, 0x20002000u, st);
         fill(wg.p, size_t(K) * 2, 1103515245u, 0x0fff0fffu, 0x20002000u, st);
         if (h) {
             fill(W1.p, size_t(h) * r * 2, 12345u, 0x0fff0fffu, 0x20002000u, st);
@@ -834,10 +914,12 @@ extern "C" int spear_plan(int M, int N, int K, int r, int group, int gate_kind, 
     for (int v = 0; v < SPEAR_VARIANT_COUNT && status == SPEAR_OK; ++v) {
         ent.us[v] = -1.f;
         if (!variant_valid(v, M, r, r > 0 ? gate_kind : SPEAR_GATE_NONE)) continue;
+        if (v == SPEAR_VARIANT_LSTREAM && group != K && ((group / 128) & (group / 128 - 1))) continue;
         ec.force_variant = v;
         for (int i = 0; i < warm + iters && status == SPEAR_OK; ++i) {
             if (i >= warm) cudaEventRecord(e0, st);
-            status = spear_w4_ec_gemm_ex(x.p, wq.p, sc.p, A.p, B.p, &ec, y.p, M, N, K, r, group, st);
+            const int c = i % nc;
+            status = spear_w4_ec_gemm_ex(x.p, wq[c].p, sc[c].p, A[c].p, B[c].p, &ec, y.p, M, N, K, r, group, st);
             if (i >= warm) {
                 cudaEventRecord(e1, st);
                 if (cudaEventSynchronize(e1) != cudaSuccess) { status = set_error(SPEAR_ECUDA, "spear_plan: timing failed: %s", cudaGetErrorString(cudaGetLastError())); break; }
@@ -859,6 +941,43 @@ extern "C" int spear_plan(int M, int N, int K, int r, int group, int gate_kind, 
     }
     if (chosen_variant_out) *chosen_variant_out = ent.variant;
     if (times_us_out) for (int v = 0; v < SPEAR_VARIANT_COUNT; ++v) times_us_out[v] = ent.us[v];
+    return SPEAR_OK;
+}
+
+extern "C" int spear_plan_batch(const spear_call* calls, int n_calls, int* chosen_out, float* times_us_out, void* stream) {
+    if (!calls || n_calls < 1) return set_error(SPEAR_EINVAL, "bad batch");
+    if (int rc = spear_init()) return rc;
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    bool all = true;
+    for (int i = 0; i < n_calls && all; ++i) all = ls_eligible(calls[i]);
+    float us[2] = {-1.f, -1.f};
+    cudaEvent_t e0, e1;
+    SPEAR_CUDA_OK(cudaEventCreate(&e0));
+    SPEAR_CUDA_OK(cudaEventCreate(&e1));
+    int status = SPEAR_OK;
+    for (int mode = 0; mode < 2 && status == SPEAR_OK; ++mode) {
+        if (mode == 1 && !all) break;
+        const int warm = 20, iters = 100;     // PAPER.md:274 protocol scaled down: the batch is replayed back to back
+        for (int i = 0; i < warm && status == SPEAR_OK; ++i) status = batch_impl(calls, nullptr, n_calls, stream, mode);
+        if (status != SPEAR_OK) break;
+        cudaEventRecord(e0, st);
+        for (int i = 0; i < iters && status == SPEAR_OK; ++i) status = batch_impl(calls, nullptr, n_calls, stream, mode);
+        cudaEventRecord(e1, st);
+        if (cudaEventSynchronize(e1) != cudaSuccess) status = set_error(SPEAR_ECUDA, "spear_plan_batch: timing failed");
+        float ms = 0.f;
+        cudaEventElapsedTime(&ms, e0, e1);
+        us[mode] = ms * 1000.f / iters;
+    }
+    cudaEventDestroy(e0);
+    cudaEventDestroy(e1);
+    if (status != SPEAR_OK) return status;
+    const int chosen = (us[1] > 0.f && us[1] < us[0]) ? 1 : 0;
+    {
+        std::lock_guard<std::mutex> lock(g_plan_mutex);
+        g_batch_plan[batch_signature(calls, n_calls)] = chosen;
+    }
+    if (chosen_out) *chosen_out = chosen;
+    if (times_us_out) { times_us_out[0] = us[0]; times_us_out[1] = us[1]; }
     return SPEAR_OK;
 }
 

@@ -9,6 +9,8 @@
 // same k-permutation trick as the weight kernel: a lane reads 32 contiguous bytes of a row), partial
 // z goes to a global fp32 buffer with red.add, and the LAST CTA to arrive (atomic counter) applies the
 // gate, writes u and re-zeroes the buffer so the workspace is clean for the next call.
+#include <mutex>
+
 #include "common.cuh"
 #include "kernels.h"
 
@@ -383,11 +385,10 @@ __global__ void __launch_bounds__(256) ec_update_kernel(const __half* __restrict
 
 int launch_ec_update(const __half* u16, const __half* B, __half* y, int M, int N, int r, bool pdl, cudaStream_t st) {
     const size_t smem = size_t(32) * r * 4 + size_t(128) * (r + 2) * 2;
-    static bool attr_set = false;
-    if (!attr_set) {
-        SPEAR_CUDA_OK(cudaFuncSetAttribute(ec_update_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 64 * 1024));
-        attr_set = true;
-    }
+    static std::once_flag attr_once;
+    static cudaError_t attr_err = cudaSuccess;
+    std::call_once(attr_once, [] { attr_err = cudaFuncSetAttribute(ec_update_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 64 * 1024); });
+    SPEAR_CUDA_OK(attr_err);
     cudaLaunchConfig_t cfg = {};
     cfg.gridDim = dim3(N / 128, (M + 31) / 32);
     cfg.blockDim = dim3(256);

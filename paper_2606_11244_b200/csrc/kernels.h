@@ -23,9 +23,6 @@ struct StreamParams {
     int CP;                  // (C + 1) / 2 chunk pairs = work units per panel
     int U;                   // (N / 128) * CP work units
     int stages;              // ring depth (stream_stages)
-    int debug;               // measurement hooks (results are wrong): bit 0 consumers skip the arithmetic; bit 1 the
-                             // epilogue does not wait for z; bit 2 the epilogue skips the rank-r add; bit 3 every
-                             // role returns after the prologue (launch machinery only)
     // ---- fused EC (SPEAR_VARIANT_STREAM_FUSED): z = x [A; w_g]^T, gate and u are computed by this kernel ----
     int fused;               // 0: u comes from the EC pre-kernel; 1: warp 9 of every CTA produces it
     int gate_kind;           // SPEAR_GATE_SCALAR_SIGMOID or SPEAR_GATE_NONE
@@ -35,12 +32,12 @@ struct StreamParams {
     const __half* w_g;       // [K] (scalar gate)
     const float* b_g;        // 1 or NULL
     float* zbuf;             // [2][16][kZStride] fp32, double-buffered by the parity of the epoch word
-    float* u_out;            // unused by the fused variant (u is formed in shared memory)
     float* gate_out;         // optional [M]
     unsigned* ec_sync;       // [0] epoch (bumped once per fused launch), [1], [2] arrival counters of buffer 0 / 1
 };
 int stream_stages(int MT, bool deep);
 int stream_smem_bytes(int MT, int stages);
+int stream_resident_ctas(int MT, bool deep);
 int launch_stream(const CUtensorMap& xmap, const StreamParams& p, int MT, int grid, bool pdl, cudaStream_t st);
 
 // ---- lstream.cu (M <= 16): persistent "layer stream" -- ONE cooperative launch consumes a table of layer

@@ -875,7 +875,6 @@ int ls_grid() {
 size_t ls_workspace_bytes(int grid) {
     return size_t(grid) * 2 * 2 * 2048 * 4 + (size_t(1) << 20);
 }
-int g_ls_coop = 1;
 int launch_lstream(const LsParams& p, cudaStream_t st) {
     const int grid = ls_grid();
     if (grid <= 0) return set_error(SPEAR_ECUDA, "layer-stream kernel cannot be resident on this device");
@@ -886,7 +885,7 @@ int launch_lstream(const LsParams& p, cudaStream_t st) {
     cfg.stream = st;
     cudaLaunchAttribute attr[1];
     attr[0].id = cudaLaunchAttributeCooperative;      // all CTAs co-resident or the launch fails: the device-wide
-    attr[0].val.cooperative = g_ls_coop;                      // arrive / wait patterns above cannot deadlock
+    attr[0].val.cooperative = 1;                      // arrive / wait patterns above cannot deadlock
     cfg.attrs = attr;
     cfg.numAttrs = 1;
     SPEAR_CUDA_OK(cudaLaunchKernelEx(&cfg, ls_kernel, p));

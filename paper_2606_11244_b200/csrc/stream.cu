@@ -26,6 +26,8 @@
 //   * per panel segment the 8 warps reduce through shared memory; a CTA that owns a whole panel writes y
 //     directly, otherwise it parks an fp32 partial in the workspace and the last arriver (atomic counter
 //     per panel) sums the partials in CTA order, adds the EC term and casts once.
+#include <mutex>
+
 #include "common.cuh"
 #include "kernels.h"
 
@@ -164,7 +166,8 @@ __device__ __forceinline__ void stream_task(uint32_t w_addr, uint32_t x_addr, ui
 // word that the last arriver bumps: launch n uses buffer n & 1 and CTA 0 re-zeroes the other buffer for launch
 // n + 1 (its previous user, launch n - 1, is complete once griddepcontrol.wait returns), so nothing has to be
 // cleaned on the critical path.  All CTAs of the grid are co-resident (grid <= SMs x resident CTAs), so the
-// late wait cannot deadlock.
+// late wait cannot deadlock: fused launches are COOPERATIVE launches (launch_stream), so the driver starts the grid
+// only when all of its CTAs fit at once, whatever else runs on the device.
 __device__ __forceinline__ void ec_load16(const __half* row, int col, bool readonly, uint32_t (&lo)[4], uint32_t (&hi)[4]) {
     if (row) {
         uint4 a, b;
@@ -309,7 +312,6 @@ stream_kernel(const __grid_constant__ CUtensorMap xmap, const StreamParams p) {
     }
     __syncthreads();
     pdl_launch_dependents();
-    if (p.debug & 8) return;     // measurement hook: launch machinery only
 
     if (warp == 0) {
         // ------------------------------ producer: weights, scales, x tiles ------------------------------
@@ -405,7 +407,7 @@ stream_kernel(const __grid_constant__ CUtensorMap xmap, const StreamParams p) {
         const int seg_end = min(n_units, (pnl + 1) * CP - u0);
         for (int i = seg_begin; i < seg_end; ++i) {
             mbar_wait(&full[rs], rph);
-            if (2 * pr + (kq >> 1) < C && !(p.debug & 1))   // the second chunk is absent in a panel's odd tail unit
+            if (2 * pr + (kq >> 1) < C)   // the second chunk is absent in a panel's odd tail unit
                 stream_task<MT>(w_lane + rs * Cfg::kWUnit, x_base + rs * Cfg::kXTile, sc_lane + rs * Cfg::kScUnit,
                                 kq, lane, tot);
             __syncwarp();
@@ -484,27 +486,16 @@ stream_kernel(const __grid_constant__ CUtensorMap xmap, const StreamParams p) {
         }
         if (finalize) {
             const int n = pnl * 128 + row;
-            if (p.r > 0 && !(p.debug & 4)) {
+            if (p.r > 0) {
                 // S7: y += sum_j u[m][j] * B[n][j]   (u = alpha * gamma (.) z, fp32, from the pre-kernel or warp 9)
                 if (p.fused && !u_seen) {
-                    if (ct == 0 && !(p.debug & 2)) {   // wait (late) until every CTA has added its piece of z
+                    if (ct == 0) {   // wait (late) until every CTA has added its piece of z
                         mbar_wait(e_ready, 0);
                         const unsigned* ctr = p.ec_sync + 1 + flag[1];
                         unsigned f;
-                        unsigned long long t0 = 0;
-                        unsigned spins = 0;
-                        do {
+                        do {       // all CTAs of the grid are co-resident (cooperative launch), and every one arrives within
+                                   // microseconds of its start: this wait cannot deadlock
                             asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(f) : "l"(ctr) : "memory");
-                            // Watchdog: every CTA arrives within microseconds of its start, so seconds of waiting
-                            // can only mean that the grid is not co-resident (see api.cu); fail loudly (sticky launch
-                            // error) instead of hanging the device.
-                            if (f < gridDim.x) __nanosleep(200);     // do not hammer the line the arrivals need
-                            if (f < gridDim.x && (++spins & 0x3ffu) == 0) {
-                                unsigned long long now;
-                                asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(now));
-                                if (t0 == 0) t0 = now;
-                                else if (now - t0 > 4000000000ull) __trap();
-                            }
                         } while (f < gridDim.x);
                     }
                     u_seen = true;      // later panels of this CTA need not look again
@@ -573,30 +564,55 @@ int stream_smem_bytes(int MT, int stages) {
     return int(MT == 1 ? StreamCfg<1>::smem_bytes(stages) : StreamCfg<2>::smem_bytes(stages));
 }
 
+// Resident CTAs per SM of the instance a launch would take (occupancy query, cached): the fused EC's device-wide
+// arrive / wait needs the whole grid resident, so api.cu clamps the grid to num_sms x this.
+int stream_resident_ctas(int MT, bool deep) {
+    static int cache[2][2] = {{0, 0}, {0, 0}};
+    int& c = cache[MT - 1][deep ? 1 : 0];
+    if (c == 0) {
+        const int smem = stream_smem_bytes(MT, stream_stages(MT, deep));
+        const void* fn = MT == 1 ? (deep ? (const void*)stream_kernel<1, 1> : (const void*)stream_kernel<1, 2>)
+                                 : (deep ? (const void*)stream_kernel<2, 1> : (const void*)stream_kernel<2, 2>);
+        int n = 0;
+        if (cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, smem) != cudaSuccess ||
+            cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n, fn, 320, smem) != cudaSuccess || n < 1)
+            n = 1;
+        c = n;
+    }
+    return c;
+}
+
 int launch_stream(const CUtensorMap& xmap, const StreamParams& p, int MT, int grid, bool pdl,
                   cudaStream_t st) {
-    static bool attr_set = false;
-    if (!attr_set) {
-        SPEAR_CUDA_OK(cudaFuncSetAttribute(stream_kernel<1, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                           int(StreamCfg<1>::smem_bytes(StreamCfg<1>::kStagesShallow))));
-        SPEAR_CUDA_OK(cudaFuncSetAttribute(stream_kernel<2, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                           int(StreamCfg<2>::smem_bytes(StreamCfg<2>::kStagesShallow))));
-        SPEAR_CUDA_OK(cudaFuncSetAttribute(stream_kernel<1, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                           int(StreamCfg<1>::smem_bytes(StreamCfg<1>::kStagesDeep))));
-        SPEAR_CUDA_OK(cudaFuncSetAttribute(stream_kernel<2, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                           int(StreamCfg<2>::smem_bytes(StreamCfg<2>::kStagesDeep))));
-        attr_set = true;
-    }
+    static std::once_flag attr_once;
+    static cudaError_t attr_err = cudaSuccess;
+    std::call_once(attr_once, [&]() {
+        auto set = [&](const void* fn, size_t bytes) {
+            if (attr_err == cudaSuccess) attr_err = cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, int(bytes));
+        };
+        set((const void*)stream_kernel<1, 2>, StreamCfg<1>::smem_bytes(StreamCfg<1>::kStagesShallow));
+        set((const void*)stream_kernel<2, 2>, StreamCfg<2>::smem_bytes(StreamCfg<2>::kStagesShallow));
+        set((const void*)stream_kernel<1, 1>, StreamCfg<1>::smem_bytes(StreamCfg<1>::kStagesDeep));
+        set((const void*)stream_kernel<2, 1>, StreamCfg<2>::smem_bytes(StreamCfg<2>::kStagesDeep));
+    });
+    SPEAR_CUDA_OK(attr_err);
     cudaLaunchConfig_t cfg = {};
     cfg.gridDim = dim3(grid);
     cfg.blockDim = dim3(320);
     cfg.dynamicSmemBytes = stream_smem_bytes(MT, p.stages);
     cfg.stream = st;
-    cudaLaunchAttribute attr[1];
+    cudaLaunchAttribute attr[2];
     attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
     attr[0].val.programmaticStreamSerializationAllowed = pdl ? 1 : 0;
     cfg.attrs = attr;
     cfg.numAttrs = 1;
+    if (p.fused && p.r > 0) {
+        // the fused EC waits device-wide for its own grid: a cooperative launch makes the co-residency of all CTAs a
+        // guarantee of the driver instead of an assumption about dispatch order (other lanes, other tenants of the GPU)
+        attr[1].id = cudaLaunchAttributeCooperative;
+        attr[1].val.cooperative = 1;
+        cfg.numAttrs = 2;
+    }
     const bool deep = p.stages > stream_stages(MT, false);
     if (MT == 1 && !deep) SPEAR_CUDA_OK(cudaLaunchKernelEx(&cfg, stream_kernel<1, 2>, xmap, p));
     else if (MT == 1) SPEAR_CUDA_OK(cudaLaunchKernelEx(&cfg, stream_kernel<1, 1>, xmap, p));

@@ -32,6 +32,8 @@
 //               A-operand stage, fence.proxy.async, arrive.  For an EC k-block one lane TMA-loads the B slab.
 #include <algorithm>
 
+#include <mutex>
+
 #include "common.cuh"
 #include "kernels.h"
 
@@ -449,7 +451,9 @@ bool tc_available() { return true; }
 template <int BT, int CS>
 static int launch_tc(const CUtensorMap& xmap, const CUtensorMap& umap, const CUtensorMap& bmap, const TcParams& p,
                      int grid_override, bool pdl, cudaStream_t st) {
+    static std::mutex init_mutex;    // first-call query, guarded: concurrent host threads may launch the same instance
     static int max_clusters = 0;     // co-resident clusters of CS CTAs (one CTA per SM)
+    std::unique_lock<std::mutex> init_lock(init_mutex);
     if (!max_clusters) {
         SPEAR_CUDA_OK(cudaFuncSetAttribute(tc_kernel<BT, CS>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                            int(TcCfg<BT>::kSmemBytes)));
@@ -470,6 +474,7 @@ static int launch_tc(const CUtensorMap& xmap, const CUtensorMap& umap, const CUt
         }
         max_clusters = n;
     }
+    init_lock.unlock();
     int clusters = std::min(p.n_work, max_clusters);
     if (grid_override > 0) clusters = std::min(clusters, std::max(1, grid_override / CS));
     cudaLaunchConfig_t cfg = {};
@@ -525,7 +530,8 @@ int run_tc(const TcProblem& t, cudaStream_t st) {
         if (p.n_tiles > t.max_counters || !t.partial || !t.counters) ks = 1;
     }
     if (t.ksplit_override > 0) ks = std::max(1, std::min(t.ksplit_override, p.kb_w));
-    if (ks > 1 && (size_t(p.n_tiles) * ks * BT * 128 * 4 > t.partial_bytes || p.n_tiles * CS > t.max_counters))
+    if (ks > 1 && CS > 1) ks = 1;       // split-K slots are indexed per tile, the cluster variant per (tile, rank): never both
+    if (ks > 1 && (size_t(p.n_tiles) * CS * ks * BT * 128 * 4 > t.partial_bytes || p.n_tiles * CS > t.max_counters))
         return set_error(SPEAR_ENOMEM, "tc split-K %d needs more workspace", ks);
     p.ksplit = ks;
     p.n_work = p.n_tiles * ks;
