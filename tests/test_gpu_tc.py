@@ -194,3 +194,114 @@ def test_config4_M4096_r64_sampled_rows(sp):
     rng = np.random.default_rng(s.seed)
     rows = np.array(sorted({0, s.M - 1, 255, 256, *[int(v) for v in rng.integers(0, s.M, size=8)]}))
     check(li, variant=0, rows=rows, label="config4 M=4096 r=64")
+
+
+# ---------------------------------------------------------------- the remaining BASELINE.json config shapes (north_star: "on all 5 configs")
+
+@pytest.mark.parametrize("M,r", [(4096, 16), (4096, 128), (16384, 0), (16384, 64)])
+def test_config4_large_sampled_rows(sp, M, r):
+    """configs[3] at the sizes not covered above: M = 4096 with r = 16 / 128 and M = 16384 with r = 0 / 64, all N
+    columns of a seeded row sample (SURVEY.md 8(c) large-shape policy: rows are independent, sampling is exact)."""
+    s = [c for c in config_shapes(3) if c.M == M and c.r == r][0]
+    li = make_layer(s.seed, s.M, s.N, s.K, s.group, s.r, gate="scalar")
+    rng = np.random.default_rng(s.seed + 1)
+    rows = np.array(sorted({0, M - 1, 127, 128, M // 2, *[int(v) for v in rng.integers(0, M, size=5)]}))
+    check(li, variant=0, rows=rows, label=f"config4 M={M} r={r}")
+
+
+def test_config3_gate_up_M2048(sp):
+    s = config_shapes(2)[10]
+    assert s.M == 2048 and s.name == "gate_up"
+    li = make_layer(s.seed, s.M, s.N, s.K, s.group, s.r, gate="scalar")
+    check(li, variant=0, rows=sample_rows(s.M, s.seed, extra=4)[::2], label="config3 gate_up M=2048")
+
+
+@pytest.mark.parametrize("M", [64, 2048])
+def test_config5_full_stack_one_batch_in_a_graph(sp, M):
+    """configs[4]: the whole 64-call projection stack (16 layers x {qkv, o, gate_up, down}, EC r = 32 on o / down of layers
+    {0, 1, 14, 15}, reading A11), issued as ONE spear_w4_ec_gemm_batch captured in a CUDA graph -- the way bench.py
+    times it -- and every call compared with the oracle (all rows at M = 64, a row sample at M = 2048)."""
+    import torch
+    h = _h()
+    shapes = [c for c in config_shapes(4) if c.M == M]
+    assert len(shapes) == 64 and sum(1 for c in shapes if c.r > 0) == 8
+    lis = [make_layer(c.seed, c.M, c.N, c.K, c.group, c.r, gate="scalar") for c in shapes]
+    dls = [h.upload_layer(li) for li in lis]
+    xs = [h.dev(li.x) for li in lis]
+    ys = [torch.zeros((li.M, li.N), dtype=torch.float16, device="cuda") for li in lis]
+    descs = [dl.desc() if li.r else sp.make_desc(gate="none") for dl, li in zip(dls, lis)]
+    batch = sp.Batch([(x, dl.pw, dl.A if li.r else None, dl.B if li.r else None, d, y)
+                      for x, dl, li, d, y in zip(xs, dls, lis, descs, ys)])
+    st = torch.cuda.Stream()
+    with torch.cuda.stream(st):
+        sp.w4_ec_gemm_batch(batch, stream=st)
+        torch.cuda.synchronize()
+        for y in ys:
+            y.zero_()
+        g = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(g, stream=st):
+            sp.w4_ec_gemm_batch(batch, stream=st)
+        g.replay()
+        torch.cuda.synchronize()
+    rows = None if M == 64 else np.array([0, 700, M - 1])
+    for c, li, y in zip(shapes, lis, ys):
+        ref = oracle.forward_layer(li, rows=rows)["y"]
+        yg = y.cpu().numpy().astype(np.float64)
+        if rows is not None:
+            yg = yg[rows]
+        rms = float(np.sqrt(np.mean(ref ** 2)))
+        assert float(np.max(np.abs(yg - ref))) <= Y_TOL * rms, c.name
+
+
+@pytest.mark.parametrize("cfg,name,M", [(1, "gate_up", 8), (2, "qkv", 256)])
+def test_paper_mlp_gate_on_config_shapes(sp, cfg, name, M):
+    """The paper's own gate (gamma = 1 + tanh(W2 ReLU(W1 z + b1) + b2), h = 4r, reading A2) on one decode and
+    one prefill shape of the configs -- the configs themselves use the scalar gate (reading A1)."""
+    s = [c for c in config_shapes(cfg) if c.name == name and c.M == M][0]
+    li = make_layer(s.seed, s.M, s.N, s.K, s.group, s.r, gate="mlp")
+    rng = np.random.default_rng(3)
+    li.b1 = (rng.integers(-8, 9, li.W1.shape[0]) / 16.0).astype(np.float32)      # non-zero biases: the ReLU clips
+    li.b2 = (rng.integers(-4, 5, li.r) / 16.0).astype(np.float32)
+    check(li, variant=0, label=f"MLP gate, config {cfg + 1} {name} M={M}")
+
+
+def test_cluster_of_four_instance(sp):
+    """tc_kernel<256, 4>: four CTAs share the token tile by TMA multicast (reachable through spear_tune only)."""
+    li = make_layer(1900, 520, 1024, 640, 128, 24, gate="scalar")
+    sp.tune("tc_cluster", 4)
+    sp.tune("tc_bt", 256)
+    try:
+        check(li, label="cluster 4")
+    finally:
+        sp.tune("tc_cluster", 0)
+        sp.tune("tc_bt", 0)
+
+
+def test_tc_grid_and_tile_overrides(sp):
+    li = make_layer(1901, 300, 512, 640, 128, 16, gate="scalar")
+    for bt in (128, 256):
+        sp.tune("tc_bt", bt)
+        sp.tune("tc_grid", 7)
+        try:
+            check(li, label=f"tc_bt={bt} tc_grid=7")
+        finally:
+            sp.tune("tc_bt", 0)
+            sp.tune("tc_grid", 0)
+
+
+def test_single_call_hostio(sp):
+    """spear_w4_ec_gemm_hostio: pinned host x -> device -> layer -> pinned host y on one stream."""
+    import torch
+    h = _h()
+    for (M, N, K, r) in [(4, 512, 768, 16), (100, 384, 640, 8)]:
+        li = make_layer(1950 + M, M, N, K, 128, r, gate="scalar")
+        dl = h.upload_layer(li)
+        xh = torch.from_numpy(li.x).pin_memory()
+        yh = torch.zeros((M, N), dtype=torch.float16).pin_memory()
+        xd = torch.empty((M, K), dtype=torch.float16, device="cuda")
+        yd = torch.empty((M, N), dtype=torch.float16, device="cuda")
+        sp.w4_ec_gemm_hostio(xh, yh, xd, yd, dl.pw, dl.A, dl.B, dl.desc())
+        torch.cuda.synchronize()
+        ref = oracle.forward_layer(li)["y"]
+        rms = float(np.sqrt(np.mean(ref ** 2)))
+        assert float(np.max(np.abs(yh.numpy().astype(np.float64) - ref))) <= Y_TOL * rms
