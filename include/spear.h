@@ -182,6 +182,30 @@ int spear_plan_batch(const spear_call* calls, int n_calls, int* chosen_out, floa
 /* The variant AUTO would run for this problem right now (table hit or heuristic). */
 int spear_plan_query(int M, int N, int K, int r, int group, int gate_kind, int* variant_out);
 
+/* ---- PAPER.md 4.3: latency look-up tables and SLO-constrained chunk selection (host only) ------------ */
+
+/* per layer type t the offline tables l_W4[t](M), l_EC[t](M) (microseconds) on a sparse, strictly
+ * increasing grid of token counts M_grid[n_grid], row-major [n_types][n_grid]; lat_attn_us[n_grid] is the attention
+ * table the caller profiled (NULL = no attention term: this library has no attention kernel).  Tables are copied; an
+ * entry smaller than its predecessor is raised to it (T_S must be monotone for the binary search of PAPER.md:237). */
+typedef struct spear_lut spear_lut;
+int spear_lut_create(const int* M_grid, int n_grid, int n_types, const float* lat_w4_us, const float* lat_ec_us,
+                     const float* lat_attn_us, spear_lut** out);
+void spear_lut_destroy(spear_lut* lut);
+/* PAPER.md:231 online aggregator: T_S(M) = sum over the n_modules linear layers of (selected[m] ? l_EC : l_W4)[type[m]](M)
+ * + n_attn_layers * l_attn(M), linear interpolation between grid points (first entry below the grid, last segment
+ * extended above it, T_S(0) = 0).  selected may be NULL (no EC anywhere).  All pointers are host pointers. */
+int spear_lut_iteration_us(const spear_lut* lut, const int* module_type, const unsigned char* selected, int n_modules,
+                           int n_attn_layers, int M, double* us_out);
+/* the largest prefill chunk c in [c_min, c_max] with T_S(d) + T_S(c) <= t_slo_us, d = decode tokens already
+ * scheduled; binary search.  *c_out = 0 when even c_min does not fit. */
+int spear_slo_chunk(const spear_lut* lut, const int* module_type, const unsigned char* selected, int n_modules,
+                    int n_attn_layers, int d, int c_min, int c_max, double t_slo_us, int* c_out);
+/* Measures one layer type's two table rows on the device with spear_plan (fastest variant per grid point, weights read
+ * from HBM): lat_w4_us_out[n_grid] for the plain layer, lat_ec_us_out[n_grid] with the rank-r EC.  Synchronises. */
+int spear_lut_measure(const int* M_grid, int n_grid, int N, int K, int group, int r, int gate_kind, int gate_hidden,
+                      float* lat_w4_us_out, float* lat_ec_us_out, void* stream);
+
 /* Debug / sweep hook: sets a launch tunable.  Decode kernel: "stream_ctas_per_sm", "stream_deep" (-1 heuristic,
  * 0 / 1 shallow / deep ring), "stream_whole_panels", "stream_batch_grid", "stream_batch_units", "stream_units",
  * "stream_debug" (measurement bits, results are wrong); EC pre-kernels: "ecpre_ctas", "ecbig_kdiv"; tcgen05 kernel: "tc_grid",

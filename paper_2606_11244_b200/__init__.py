@@ -25,7 +25,8 @@ EXPORTS = [
     "spear_pack_w4_sizes", "spear_pack_w4", "spear_unpack_w4", "spear_dequant_w4",
     "spear_w4_ec_gemm", "spear_w4_ec_gemm_ex", "spear_w4_ec_gemm_hostio", "spear_w4_ec_gemm_batch", "spear_w4_ec_gemm_batch_hostio",
     "spear_workspace_bytes", "spear_init", "spear_memory_bytes", "spear_plan", "spear_plan_save", "spear_plan_load",
-    "spear_plan_query", "spear_plan_batch", "spear_tune", "spear_last_error", "spear_launch_count",
+    "spear_plan_query", "spear_plan_batch", "spear_lut_create", "spear_lut_destroy", "spear_lut_iteration_us",
+    "spear_slo_chunk", "spear_lut_measure", "spear_tune", "spear_last_error", "spear_launch_count",
 ]
 
 
@@ -88,11 +89,18 @@ def lib():
         L.spear_plan_load.argtypes = [ctypes.c_char_p]
         L.spear_plan_query.argtypes = [ci] * 6 + [ctypes.POINTER(ci)]
         L.spear_plan_batch.argtypes = [ctypes.POINTER(Call), ci, ctypes.POINTER(ci), ctypes.POINTER(ctypes.c_float), vp]
+        fp = ctypes.POINTER(ctypes.c_float)
+        L.spear_lut_create.argtypes = [ctypes.POINTER(ci), ci, ci, fp, fp, fp, ctypes.POINTER(vp)]
+        L.spear_lut_destroy.argtypes = [vp]
+        L.spear_lut_destroy.restype = None
+        L.spear_lut_iteration_us.argtypes = [vp, ctypes.POINTER(ci), ctypes.c_char_p, ci, ci, ci, ctypes.POINTER(ctypes.c_double)]
+        L.spear_slo_chunk.argtypes = [vp, ctypes.POINTER(ci), ctypes.c_char_p, ci, ci, ci, ci, ci, ctypes.c_double, ctypes.POINTER(ci)]
+        L.spear_lut_measure.argtypes = [ctypes.POINTER(ci), ci, ci, ci, ci, ci, ci, ci, fp, fp, vp]
         L.spear_tune.argtypes = [ctypes.c_char_p, ci]
         L.spear_last_error.restype = ctypes.c_char_p
         L.spear_launch_count.restype = ctypes.c_ulonglong
         for name in EXPORTS:
-            if name not in ("spear_last_error", "spear_launch_count"):
+            if name not in ("spear_last_error", "spear_launch_count", "spear_lut_destroy"):
                 getattr(L, name).restype = ci
         _lib = L
     return _lib
@@ -288,3 +296,52 @@ def plan_save(path: str):
 
 def plan_load(path: str):
     _check(lib().spear_plan_load(path.encode()))
+
+
+# ---- PAPER.md 4.3: latency tables and SLO-constrained chunk selection (host only; marshalling only) -------------
+class Lut:
+    """spear_lut: l_W4 / l_EC tables per layer type on a sparse M grid (+ optional attention table), microseconds."""
+
+    def __init__(self, M_grid, lat_w4_us, lat_ec_us, lat_attn_us=None):
+        n = len(M_grid)
+        n_types = len(lat_w4_us)
+        assert len(lat_ec_us) == n_types and all(len(r) == n for r in list(lat_w4_us) + list(lat_ec_us))
+        grid = (ctypes.c_int * n)(*[int(v) for v in M_grid])
+        flat = lambda rows: (ctypes.c_float * (n_types * n))(*[float(v) for r in rows for v in r])
+        attn = None if lat_attn_us is None else (ctypes.c_float * n)(*[float(v) for v in lat_attn_us])
+        self._h = ctypes.c_void_p()
+        _check(lib().spear_lut_create(grid, n, n_types, flat(lat_w4_us), flat(lat_ec_us), attn, ctypes.byref(self._h)))
+
+    def __del__(self):
+        if getattr(self, "_h", None) and _lib is not None:
+            _lib.spear_lut_destroy(self._h)
+            self._h = None
+
+    @staticmethod
+    def _modules(module_type, selected):
+        n = len(module_type)
+        types = (ctypes.c_int * n)(*[int(t) for t in module_type])
+        sel = None if selected is None else bytes(bytearray(1 if s else 0 for s in selected))
+        return types, sel, n
+
+    def iteration_us(self, module_type, selected, M, n_attn_layers=0) -> float:
+        types, sel, n = self._modules(module_type, selected)
+        out = ctypes.c_double()
+        _check(lib().spear_lut_iteration_us(self._h, types, sel, n, n_attn_layers, int(M), ctypes.byref(out)))
+        return out.value
+
+    def slo_chunk(self, module_type, selected, d, c_min, c_max, t_slo_us, n_attn_layers=0) -> int:
+        types, sel, n = self._modules(module_type, selected)
+        c = ctypes.c_int()
+        _check(lib().spear_slo_chunk(self._h, types, sel, n, n_attn_layers, int(d), int(c_min), int(c_max),
+                                     float(t_slo_us), ctypes.byref(c)))
+        return c.value
+
+
+def lut_measure(M_grid, N, K, group, r, gate="scalar", gate_hidden=0, stream=None):
+    """spear_lut_measure: (l_W4 row, l_EC row) of one layer type, measured on the device with spear_plan."""
+    n = len(M_grid)
+    grid = (ctypes.c_int * n)(*[int(v) for v in M_grid])
+    w4, ec = (ctypes.c_float * n)(), (ctypes.c_float * n)()
+    _check(lib().spear_lut_measure(grid, n, N, K, group, r, GATE_KINDS[gate], gate_hidden, w4, ec, _stream(stream)))
+    return [float(v) for v in w4], [float(v) for v in ec]
