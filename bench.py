@@ -6,7 +6,10 @@ Workload (config.workload): BASELINE.json configs[1] -- Llama-3.2-1B-shaped deco
 the scalar sigmoid gate on every projection, M in {1, 8, 16}.  One "step" = one pass of the whole hot
 path over that batch = 12 layer calls (3 token counts x 4 projections), all through the C ABI
 (spear_w4_ec_gemm_ex).  value = algorithmic bytes of the step (packed weights +
-scales + x + y + EC factors + gate vector) / device time, whole job.
+scales + x + y + EC factors + gate vector) / device time, whole job.  The headline step issues the 12 calls one
+after the other on one stream (the dependent-chain regime: in a decoder qkv -> o -> gate_up -> down depend on each
+other); the same step overlapped on the library's lanes and as one persistent layer-stream launch are reported
+beside it, and the `configs` key carries SURVEY.md 8(d)'s result rows for all five configs.
 
 L2 hygiene: every step reads a different copy of the weights and EC factors from an arena of NCOPY
 copies (> 4x the 126 MB L2), so weights always come from HBM ("inputs larger than L2").
@@ -136,6 +139,32 @@ def aggregate_value(bytes_per_rank_step, ms_per_step, world):
 # ------------------------------------------------------------------------------------------------
 # CUDA arm
 # ------------------------------------------------------------------------------------------------
+NOMINAL_HBM_GBS = 8000.0          # nominal 8 TB/s, 2.25 PFLOP/s dense fp16
+NOMINAL_TFLOPS = 2250.0
+
+
+def load_tensor_peak():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        with open(p) as f:
+            return float(json.load(f)["bf16_tflops"]), "measured (MEASURED_PEAKS.json bf16_tflops, burst)"
+    return 1590.0, "fallback (B200_PROFILING.md 1.59 PFLOP/s burst)"
+
+
+def profile_traffic():
+    """dram__bytes_read + dram__bytes_write per launch of the dominant decode kernel, from the committed ncu capture."""
+    p = os.path.join(ROOT, "profiles", "r02_dram_traffic.csv")
+    if not os.path.exists(p):
+        return None, "no capture committed"
+    import csv
+    with open(p) as f:
+        rows = list(csv.reader(l for l in f if l.strip() and not l.startswith("#")))
+    for r in rows[1:]:
+        if r[0] == "stream_kernel":
+            return int(r[3]), f"{r[1]} ({r[2]}); algorithmic {r[4]} B; profiles/r02_dram_traffic.csv"
+    return None, "stream_kernel not in profiles/r02_dram_traffic.csv"
+
+
 def run_cuda(args, rank, world):
     import torch
     import torch.distributed as dist
@@ -148,12 +177,12 @@ def run_cuda(args, rank, world):
     if world > 1:
         dist.init_process_group("nccl", device_id=torch.device(device))
     sp.init()
-    if os.environ.get("SPEAR_PDL") is not None:
-        sp.tune("pdl", int(os.environ["SPEAR_PDL"]))
-    for kv in os.environ.get("SPEAR_TUNE", "").split(","):     # sweep hook: key=value,... for spear_tune
+    tunes = {}
+    for kv in os.environ.get("SPEAR_TUNE", "").split(","):     # sweep hook: key=value,... for spear_tune; echoed in config
         if "=" in kv:
             k, v = kv.split("=")
             sp.tune(k.strip(), int(v))
+            tunes[k.strip()] = int(v)
 
     shapes = step_shapes()
     # weights / EC factors: one seeded set per projection (the M=16 entry's seed), shared by the three
@@ -186,45 +215,47 @@ def run_cuda(args, rank, world):
     descs = {}   # keep EcDesc objects alive
     batches = {}
 
-    def one_step(g, with_ec=True, batched=True):
-        """One pass over the 12 independent layer calls: as ONE spear_w4_ec_gemm_batch (the library overlaps
-        independent calls on its lanes) or as 12 stream-ordered spear_w4_ec_gemm_ex calls."""
+    def one_step(g, with_ec=True, mode="ordered", ec_resident=False):
+        """One pass over the 12 layer calls of the step.  mode: "ordered" = 12 stream-ordered spear_w4_ec_gemm_ex calls, one
+        after the other (PDL-chained kernels) -- the regime of SURVEY.md 8(d) and of a real decoder, whose projections
+        depend on each other; "lanes" = ONE spear_w4_ec_gemm_batch over the library's concurrent lanes (the 12 calls of
+        the config are independent problems); "lstream" = ONE persistent layer-stream launch.  ec_resident: the EC factors
+        come from ONE copy (L2-resident, a model's EC set is a few MB) instead of rotating with the weights (cold)."""
         entries = []
         for mi, M in enumerate(TOKENS):
             cp = copies[(3 * g + mi) % ncopy]
+            ecp = copies[0] if ec_resident else cp
             for s in shapes[M]:
-                dl = cp[s.name]
-                key = (g, mi, s.name, with_ec)
+                dl, de = cp[s.name], ecp[s.name]
+                key = (g, mi, s.name, with_ec, ec_resident)
                 if key not in descs:
-                    descs[key] = dl.desc() if with_ec else sp.make_desc(gate="none")
-                A, B = (dl.A, dl.B) if with_ec else (None, None)
-                if batched:
-                    entries.append((xs[(M, s.name)], dl.pw, A, B, descs[key], ys[(M, s.name)]))
-                else:
+                    descs[key] = de.desc() if with_ec else sp.make_desc(gate="none")
+                A, B = (de.A, de.B) if with_ec else (None, None)
+                if mode == "ordered":
                     sp.w4_ec_gemm_ex(xs[(M, s.name)], dl.pw, A, B, descs[key], y=ys[(M, s.name)])
-        if batched:
-            bk = (g, with_ec)
+                else:
+                    entries.append((xs[(M, s.name)], dl.pw, A, B, descs[key], ys[(M, s.name)]))
+        if mode != "ordered":
+            bk = (g, with_ec, ec_resident)
             if bk not in batches:
                 batches[bk] = sp.Batch(entries)
+            sp.tune("lstream", 1 if mode == "lstream" else 0)
             sp.w4_ec_gemm_batch(batches[bk])
+            sp.tune("lstream", -1)
 
     stream = torch.cuda.Stream()
     ngraph = ncopy // 3
-    use_graph = os.environ.get("SPEAR_BENCH_GRAPH", "1") != "0"
 
-    def make_graphs(with_ec, batched=True):
+    def make_graphs(with_ec, mode, ec_resident=False):
         gs = []
         with torch.cuda.stream(stream):
-            one_step(0, with_ec, batched)  # first-call work (tensor maps, attributes) outside capture
+            one_step(0, with_ec, mode, ec_resident)  # first-call work (tensor maps, attributes) outside capture
             torch.cuda.synchronize()
             for g in range(ngraph):
-                if use_graph:
-                    cg = torch.cuda.CUDAGraph()
-                    with torch.cuda.graph(cg, stream=stream):
-                        one_step(g, with_ec, batched)
-                    gs.append(cg.replay)
-                else:
-                    gs.append(lambda g=g: one_step(g, with_ec, batched))
+                cg = torch.cuda.CUDAGraph()
+                with torch.cuda.graph(cg, stream=stream):
+                    one_step(g, with_ec, mode, ec_resident)
+                gs.append(cg.replay)
         return gs
 
     def timed(fns, steps, warmup):
@@ -247,129 +278,344 @@ def run_cuda(args, rank, world):
     sampler = ClockSampler(local)
     if rank == 0:
         sampler.start()
+    b_ec, b_w4 = step_bytes(True), step_bytes(False)
+    peak, peak_src = load_peaks()
+
+    def leg(with_ec, mode, ec_resident=False, steps=None):
+        steps = steps or args.steps
+        ms = timed(make_graphs(with_ec, mode, ec_resident), steps, args.warmup) / steps
+        by = b_ec if with_ec else b_w4
+        gbs = aggregate_value(by, ms, world)
+        return {"value": round(gbs, 1), "ms_per_step": round(ms, 6), "frac_of_measured_hbm": round(gbs / world / peak, 4),
+                "frac_of_nominal_8tbs": round(gbs / world / NOMINAL_HBM_GBS, 4)}
+
+    # headline: the dependent-chain regime (stream-ordered calls), EC factors cold (rotating with the weights)
     launches0 = sp.launch_count()
-    g_ec = make_graphs(True)
+    g_head = make_graphs(True, "ordered")
     per_step_launches = (sp.launch_count() - launches0) // (ngraph + 1)
-    ms = timed(g_ec, args.steps, args.warmup)
-    g_w4 = make_graphs(False)
-    ms_w4 = timed(g_w4, args.steps, args.warmup)
-    # the same step with the 12 calls strictly stream-ordered (one after the other, PDL-chained)
-    ms_seq = timed(make_graphs(True, batched=False), args.steps, args.warmup)
-    ms_seq_w4 = timed(make_graphs(False, batched=False), args.steps, args.warmup)
-    # make the region long enough for nvidia-smi to see it under load
-    t_end = time.time() + 1.5
+    ms_head = timed(g_head, args.steps, args.warmup) / args.steps
+    sub = min(args.steps, 500)
+    ordered_w4 = leg(False, "ordered")
+    ordered_ec_res = leg(True, "ordered", ec_resident=True, steps=sub)
+    lanes_ec, lanes_w4 = leg(True, "lanes", steps=sub), leg(False, "lanes", steps=sub)
+    ls_ec, ls_w4 = leg(True, "lstream", steps=sub), leg(False, "lstream", steps=sub)
+    t_end = time.time() + 1.0      # keep the GPU under load long enough for nvidia-smi to sample it
     while rank == 0 and time.time() < t_end:
-        timed(g_ec, 200, 0)
+        timed(g_head, 200, 0)
 
     # e2e: pinned-host x -> device -> layer -> pinned-host y for every call of the step, through ONE
     # spear_w4_ec_gemm_batch_hostio (copies and kernels of different calls overlap on the lanes)
     e2e_steps = max(1, min(args.steps, 300))
+    one_step(0, True, "lanes")          # builds batches[(g, True, False)] for every rotation below
+    for g in range(ngraph):
+        one_step(g, True, "lanes")
+    torch.cuda.synchronize()
 
     def e2e_step(g):
-        # the Batch of rotation g was built (and kept) when its graph was captured
-        bt = batches[(g, True)]
+        bt = batches[(g, True, False)]
         order = [(M, s.name) for M in TOKENS for s in shapes[M]]
         sp.w4_ec_gemm_batch_hostio(bt, [xh[k] for k in order], [yh[k] for k in order], stream=stream)
 
-    ms_e2e = timed([lambda g=g: e2e_step(g) for g in range(ngraph)], e2e_steps, max(3, min(args.warmup, 20)))
+    ms_e2e = timed([lambda g=g: e2e_step(g) for g in range(ngraph)], e2e_steps, max(3, min(args.warmup, 20))) / e2e_steps
     clocks = sampler.stop() if rank == 0 else None
 
-    b_ec, b_w4 = step_bytes(True), step_bytes(False)
-    per = ms / args.steps
-    per_w4 = ms_w4 / args.steps
-    per_e2e = ms_e2e / e2e_steps
-    value = aggregate_value(b_ec, per, world)
-    peak, peak_src = load_peaks()
+    value = aggregate_value(b_ec, ms_head, world)
     ncalls = sum(len(v) for v in shapes.values())
-    ach = b_w4 / (per_w4 * 1e-3) / 1e9
+    traffic, traffic_note = profile_traffic()
+    ach = ordered_w4["value"] / world
     out = {
         "metric": METRIC, "value": round(value, 1), "unit": UNIT, "n_gpus": world, "steps": args.steps,
-        "warmup": args.warmup, "ms_per_step": round(per, 6), "higher_is_better": True, "scaling": "weak",
+        "warmup": args.warmup, "ms_per_step": round(ms_head, 6), "higher_is_better": True, "scaling": "weak",
         "vs_baseline": None, "dtype": "f16 (int4 weights, fp32 accumulate)", "data": "synthetic (seeded, workloads/)",
-        "config": {"workload": "BASELINE.json configs[1]: Llama-3.2-1B decode projections qkv/o/gate_up/down, "
-                               "group=128, EC r=32 scalar sigmoid gate, M in {1,8,16}; step = 12 independent layer calls issued as one "
-                               "spear_w4_ec_gemm_batch",
+        "config": {"workload": "BASELINE.json configs[1]: Llama-3.2-1B decode projections qkv/o/gate_up/down, group=128, EC r=32 "
+                               "scalar sigmoid gate, M in {1,8,16}; step = the 12 layer calls issued one after the other on one "
+                               "stream (dependent-chain regime of SURVEY.md 8(d); EC factors cold = rotating with the weights)",
                    "l2": f"inputs larger than L2: weights+EC rotate over {ncopy} copies ({ncopy * set_bytes >> 20} MiB)",
-                   "cuda_graph": use_graph, "bytes_per_step": b_ec, "parallelism": f"replicas x{world}"},
-        "e2e": {"value": round(world * b_ec / (per_e2e * 1e-3) / 1e9, 1), "unit": UNIT,
+                   "cuda_graph": True, "bytes_per_step": b_ec, "parallelism": f"replicas x{world}",
+                   "spear_tune_overrides": tunes, "env": {k: os.environ[k] for k in ("SPEAR_TUNE",) if k in os.environ}},
+        "e2e": {"value": round(world * b_ec / (ms_e2e * 1e-3) / 1e9, 1), "unit": UNIT,
                 "h2d_bytes_per_step": sum(t.numel() * 2 for t in xh.values()),
-                "d2h_bytes_per_step": sum(t.numel() * 2 for t in yh.values()), "ms_per_step": round(per_e2e, 6)},
+                "d2h_bytes_per_step": sum(t.numel() * 2 for t in yh.values()), "ms_per_step": round(ms_e2e, 6),
+                "path": "spear_w4_ec_gemm_batch_hostio (per call: pinned host x -> device, layer, device -> pinned host y, on the lanes)"},
         "gpu_launches": int(per_step_launches * args.steps),
         "clocks": clocks,
-        "roofline": {"bound": "hbm", "kernel": "spear::stream_kernel (plain W4 step: one launch per layer call, "
-                                                "calls overlapped on the batch lanes)",
+        "roofline": {"bound": "hbm", "kernel": "spear::stream_kernel<MT,1> (deep ring, one launch per layer call, stream-ordered; "
+                                                "plain W4 leg of the same step)",
                      "achieved": round(ach, 1), "peak": peak, "unit": "GB/s", "frac": round(ach / peak, 4),
-                     "peak_source": peak_src, "traffic": 17400320,
-                     "traffic_note": "dram__bytes_read+write of ONE launch (gate_up 2048->16384, M=8, r=0; algorithmic "
-                                     "17.35 MB) from profiles/r01_ncu_summary.md; the step is 12 such launches of 4 shapes",
-                     "avg_launch_us": round(per_w4 * 1e3 / ncalls, 3), "launches_per_step": ncalls},
-        "no_ec": {"value": round(world * b_w4 / (per_w4 * 1e-3) / 1e9, 1), "ms_per_step": round(per_w4, 6)},
-        "ec_overhead_time_frac": round(per / per_w4 - 1.0, 4),
-        "stream_ordered": {"note": "same step, 12 calls one after the other on one stream (PDL-chained) instead of "
-                                   "one spear_w4_ec_gemm_batch",
-                           "value": round(world * b_ec / (ms_seq / args.steps * 1e-3) / 1e9, 1),
-                           "no_ec_value": round(world * b_w4 / (ms_seq_w4 / args.steps * 1e-3) / 1e9, 1),
-                           "ms_per_step": round(ms_seq / args.steps, 6)},
+                     "peak_source": peak_src, "traffic": traffic, "traffic_note": traffic_note,
+                     "avg_launch_us": round(ordered_w4["ms_per_step"] * 1e3 / ncalls, 3), "launches_per_step": ncalls,
+                     "frac_with_ec": round(value / world / peak, 4)},
+        "no_ec": ordered_w4,
+        "ec_overhead_time_frac": round(ms_head / ordered_w4["ms_per_step"] - 1.0, 4),
+        "ec_l2_resident": dict(ordered_ec_res, ec_overhead_time_frac=round(ordered_ec_res["ms_per_step"] / ordered_w4["ms_per_step"] - 1.0, 4)),
+        "overlapped_lanes": {"note": "same step as ONE spear_w4_ec_gemm_batch: the 12 calls are independent problems, the library overlaps "
+                                     "them on 12 concurrent lanes (round 1's headline; not a dependent chain)",
+                             "ec": lanes_ec, "no_ec": lanes_w4,
+                             "ec_overhead_time_frac": round(lanes_ec["ms_per_step"] / lanes_w4["ms_per_step"] - 1.0, 4)},
+        "layer_stream": {"note": "same step as ONE persistent cooperative launch of spear::ls_kernel (tcgen05, weights through tensor "
+                                 "memory); kernel durations are multiples of ~2.05 us on this path (DESIGN.md 6.5)",
+                         "ec": ls_ec, "no_ec": ls_w4,
+                         "ec_overhead_time_frac": round(ls_ec["ms_per_step"] / ls_w4["ms_per_step"] - 1.0, 4)},
     }
     if rank == 0:
-        out["prefill"] = prefill_numbers(sp, device)
+        del copies, base
+        torch.cuda.empty_cache()
+        out["prefill"] = None
+        if not args.no_table:
+            out["configs"] = configs_table(sp, device)
+            p4 = out["configs"]["config4"]
+            best = max((e for e in p4 if e["M"] == 4096 and e["r"] == 0), key=lambda e: e["tflops"])
+            ec64 = [e for e in p4 if e["M"] == 4096 and e["r"] == 64][0]
+            out["prefill"] = {"workload": "BASELINE.json configs[3]: M=4096, K=8192, N=28672, group=128 (see configs.config4 for the sweep)",
+                              "kernel": "spear::tc_kernel<256,2> (tcgen05, TMEM accumulators, EC folded in as extra k-blocks)",
+                              "tflops_no_ec": best["tflops"], "tflops_ec_r64": ec64["tflops"],
+                              "ec_overhead_time_frac": ec64.get("ec_overhead_time_frac"),
+                              "roofline": {"bound": "tensor", "achieved": best["tflops"], "peak": load_tensor_peak()[0], "unit": "TFLOP/s",
+                                           "frac": best["frac_of_measured_roofline"], "peak_source": load_tensor_peak()[1],
+                                           "frac_of_nominal_2250": best["frac_of_nominal_roofline"]}}
         out["cpu_baseline"] = cpu_baseline_sample()
         print(json.dumps(out), flush=True)
     if world > 1:
         dist.destroy_process_group()
 
 
-def prefill_numbers(sp, device):
-    """The other half of BASELINE.json's metric: prefill TFLOP/s of the tcgen05 kernel on configs[3]
-    (M=4096, K=8192, N=28672, group=128), without and with the EC (r=64, scalar gate), against the measured
-    dense bf16 tensor peak.  Inputs (117 MB weights + 67 MB x + 235 MB y) exceed the 126 MB L2.  Device-side
-    seeded torch RNG with the config's value distributions (parity on this shape: tests/test_gpu_tc.py)."""
+# ------------------------------------------------------------------------------------------------
+# SURVEY.md 8(d) result rows for all five configs (perf only: seeded device-side generator with the configs' value
+# distributions -- parity on every one of these shapes is tests/test_gpu_*.py with workloads/ inputs)
+# ------------------------------------------------------------------------------------------------
+def configs_table(sp, device):
     import torch
     from workloads import algorithmic_flops
-    M, N, K, group = 4096, 28672, 8192, 128
+    hbm, _ = load_peaks()
+    tpk, _ = load_tensor_peak()
     gen = torch.Generator(device=device)
-    gen.manual_seed(4096)
-    codes = torch.randint(0, 16, (N, K), dtype=torch.uint8, device=device, generator=gen)
-    scales = (torch.randn(N, K // group, device=device, generator=gen).abs() * 0.02 + 1e-3).half()
-    pw = sp.pack_w4(codes, scales, group)
-    del codes
-    x = torch.randn(M, K, device=device, generator=gen).half()
-    y = torch.empty(M, N, dtype=torch.float16, device=device)
-    res = {}
-    for r in (0, 64):
-        A = B = wg = bg = None
+    gen.manual_seed(20260611)
+
+    def rand_layer(N, K, group, r, gate="scalar"):
+        codes = torch.randint(0, 16, (N, K), dtype=torch.uint8, device=device, generator=gen)
+        scales = (torch.randn(N, K // group, device=device, generator=gen).abs() * 0.02 + 1e-3).half()
+        pw = sp.pack_w4(codes, scales, group)
+        del codes
+        L = {"pw": pw, "r": r, "gate": gate if r else "none"}
         if r:
-            A = (torch.randn(r, K, device=device, generator=gen) / K ** 0.5).half()
-            B = (torch.randn(N, r, device=device, generator=gen) / r ** 0.5).half()
-            wg = (torch.randn(K, device=device, generator=gen) / K ** 0.5).half()
-            bg = torch.zeros(1, device=device)
-        d = sp.make_desc(gate="scalar" if r else "none", w_g=wg, b_g=bg)
-        for _ in range(3):
-            sp.w4_ec_gemm_ex(x, pw, A, B, d, y=y)
-        torch.cuda.synchronize()
+            L["A"] = (torch.randn(r, K, device=device, generator=gen) / K ** 0.5).half()
+            L["B"] = (torch.randn(N, r, device=device, generator=gen) / r ** 0.5).half()
+            if gate == "scalar":
+                L["w_g"] = (torch.randn(K, device=device, generator=gen) / K ** 0.5).half()
+                L["b_g"] = torch.zeros(1, device=device)
+            elif gate == "mlp":
+                h = 4 * r
+                L["W1"] = (torch.randn(h, r, device=device, generator=gen) / r ** 0.5).half()
+                L["W2"] = (torch.randn(r, h, device=device, generator=gen) / h ** 0.5).half()
+                L["b1"], L["b2"] = torch.zeros(h, device=device), torch.zeros(r, device=device)
+        return L
+
+    def clones(L, n, ec_too=True):
+        out = [L]
+        for _ in range(n - 1):
+            C = dict(L)
+            C["pw"] = sp.PackedW4(L["pw"].wq.clone(), L["pw"].scales.clone(), L["pw"].N, L["pw"].K, L["pw"].group)
+            if L["r"] and ec_too:
+                C["A"], C["B"] = L["A"].clone(), L["B"].clone()
+            out.append(C)
+        return out
+
+    def desc_of(L):
+        return sp.make_desc(gate=L["gate"], w_g=L.get("w_g"), b_g=L.get("b_g"), W1=L.get("W1"), b1=L.get("b1"),
+                            W2=L.get("W2"), b2=L.get("b2"))
+
+    stream = torch.cuda.Stream()
+
+    def steady_us(M, arena, n_calls, plain=False, reps=5):
+        """Steady state (SURVEY.md 8(d) regime 1): a CUDA graph of n_calls back-to-back stream-ordered calls cycling through
+        the arena (>= 512 MB of weights unless the layer alone exceeds L2); microseconds per call, median of `reps` replays."""
+        K, N = arena[0]["pw"].K, arena[0]["pw"].N
+        x = torch.randn(M, K, device=device, generator=gen).half()
+        y = torch.empty(M, N, dtype=torch.float16, device=device)
+        ds = [sp.make_desc(gate="none") if plain else desc_of(L) for L in arena]
+
+        def body():
+            for i in range(n_calls):
+                L = arena[i % len(arena)]
+                sp.w4_ec_gemm_ex(x, L["pw"], None if plain else L.get("A"), None if plain else L.get("B"), ds[i % len(arena)], y=y)
+
+        with torch.cuda.stream(stream):
+            body()
+            torch.cuda.synchronize()
+            g = torch.cuda.CUDAGraph()
+            with torch.cuda.graph(g, stream=stream):
+                body()
+            g.replay()
+            torch.cuda.synchronize()
+            ts = []
+            for _ in range(reps):
+                e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                e0.record(stream)
+                g.replay()
+                e1.record(stream)
+                e1.synchronize()
+                ts.append(e0.elapsed_time(e1) * 1e3 / n_calls)
+        return sorted(ts)[len(ts) // 2]
+
+    def row(name, M, N, K, group, r, us, gate="scalar", extra=None):
+        by = algorithmic_bytes(M, N, K, group, r, gate, 4 * r if gate == "mlp" else 0)
+        fl = algorithmic_flops(M, N, K, group, r, gate, 4 * r if gate == "mlp" else 0)
+        t_meas = max(by / (hbm * 1e3), fl / (tpk * 1e6))          # us at the measured peaks
+        t_nom = max(by / (NOMINAL_HBM_GBS * 1e3), fl / (NOMINAL_TFLOPS * 1e6))
+        e = {"name": name, "M": M, "N": N, "K": K, "group": group, "r": r, "gate": gate if r else "none", "us": round(us, 2),
+             "gbs": round(by / us * 1e-3, 1), "tflops": round(fl / us * 1e-6, 2),
+             "bound": "hbm" if by / hbm / 1e3 >= fl / tpk / 1e6 else "tensor",
+             "frac_of_measured_roofline": round(t_meas / us, 4), "frac_of_nominal_roofline": round(t_nom / us, 4)}
+        if extra:
+            e.update(extra)
+        return e
+
+    def arena_for(L, M):
+        wbytes = L["pw"].wq.numel() + L["pw"].scales.numel() * 2
+        n = max(2, min(40, -(-(512 << 20) // wbytes)))
+        return clones(L, n), (64 if M <= 16 else max(n, 4))
+
+    def sweep(shapes, gate="scalar"):
+        rows = []
+        layers = {}
+        for s in shapes:
+            key = (s.N, s.K, s.group, s.r)
+            if key not in layers:
+                layers.clear()
+                torch.cuda.empty_cache()
+                layers[key] = rand_layer(s.N, s.K, s.group, s.r, gate)
+            L = layers[key]
+            arena, n_calls = arena_for(L, s.M)
+            us0 = steady_us(s.M, arena, n_calls, plain=True)
+            rows.append(row(s.name, s.M, s.N, s.K, s.group, 0, us0))
+            if s.r:
+                us1 = steady_us(s.M, arena, n_calls)
+                rows.append(row(s.name, s.M, s.N, s.K, s.group, s.r, us1, gate, {"ec_overhead_time_frac": round(us1 / us0 - 1.0, 4)}))
+            del arena
+        return rows
+
+    table = {"protocol": "steady state: CUDA graph of back-to-back stream-ordered calls of one shape cycling through >= 512 MB of weight "
+                         "copies (EC factors cold), median of 5 replays; us per call; roofline = max(bytes / HBM peak, flops / tensor peak) "
+                         "at the measured and at the nominal (8 TB/s, 2.25 PFLOP/s) peaks",
+             "peaks": {"hbm_gbs_measured": hbm, "tensor_tflops_measured": tpk}}
+    table["config1"] = sweep(config_shapes(0))
+    table["config2"] = sweep(config_shapes(1))
+    table["config3"] = sweep(config_shapes(2))
+    # config 4: one weight arena per r, all three token counts.  The EC overhead of a row is taken against the plain layer
+    # timed on the SAME arena right before it (the part power-caps under these GEMMs: rows measured minutes apart do not
+    # share a clock state)
+    rows4 = []
+    s0 = config_shapes(3)[0]
+    for r in (0, 16, 64, 128):
+        torch.cuda.empty_cache()
+        L = rand_layer(s0.N, s0.K, s0.group, r)
+        arena = clones(L, 5)
+        for M in (512, 4096, 16384):
+            reps = 3 if M == 16384 else 5
+            us0 = steady_us(M, arena, 5, plain=True, reps=reps)
+            if r == 0:
+                rows4.append(row("mlp70b", M, s0.N, s0.K, s0.group, 0, us0))
+            else:
+                us1 = steady_us(M, arena, 5, reps=reps)
+                rows4.append(row("mlp70b", M, s0.N, s0.K, s0.group, r, us1, "scalar",
+                                 {"ec_overhead_time_frac": round(us1 / us0 - 1.0, 4), "plain_us_same_arena": round(us0, 2)}))
+        del arena, L
+    table["config4"] = rows4
+    torch.cuda.empty_cache()
+    table["mlp_gate_cost"] = mlp_gate_rows(sp, rand_layer, arena_for, steady_us, row)
+    table["single_cold_launch"] = cold_launch_rows(sp, device, rand_layer, desc_of, row, gen)
+    torch.cuda.empty_cache()
+    table["config5"] = stack_rows(sp, device, rand_layer, desc_of, gen, hbm, tpk)
+    return table
+
+
+def mlp_gate_rows(sp, rand_layer, arena_for, steady_us, row):
+    """The paper's MLP gate (h = 4r) against the scalar gate of the configs (reading A1): config 1, one decode and
+    one prefill shape."""
+    out = []
+    for (name, M, N, K, group, r) in (("config1", 4, 2048, 2048, 128, 16), ("config2 gate_up", 8, 16384, 2048, 128, 32),
+                                      ("config3 qkv", 256, 6144, 4096, 4096, 64)):
+        for gate in ("scalar", "mlp"):
+            L = rand_layer(N, K, group, r, gate)
+            arena, n_calls = arena_for(L, M)
+            out.append(row(name, M, N, K, group, r, steady_us(M, arena, n_calls), gate))
+            del arena, L
+    return out
+
+
+def cold_launch_rows(sp, device, rand_layer, desc_of, row, gen):
+    """SURVEY.md 8(d) regime 2: ONE call after the L2 has been flushed by a 256 MB write; median of 15."""
+    import torch
+    out = []
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device=device)
+    for (name, M, N, K, group, r) in (("config2 o", 1, 2048, 2048, 128, 32), ("config2 gate_up", 8, 16384, 2048, 128, 32),
+                                      ("config3 gate_up", 16, 28672, 4096, 4096, 64)):
+        L = rand_layer(N, K, group, r)
+        x = torch.randn(M, K, device=device, generator=gen).half()
+        y = torch.empty(M, N, dtype=torch.float16, device=device)
+        d = desc_of(L)
         ts = []
-        for _ in range(7):
+        for i in range(18):
+            flush.fill_(i & 0xff)
             e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
             e0.record()
-            sp.w4_ec_gemm_ex(x, pw, A, B, d, y=y)
+            sp.w4_ec_gemm_ex(x, L["pw"], L["A"], L["B"], d, y=y)
             e1.record()
             e1.synchronize()
-            ts.append(e0.elapsed_time(e1))
-        res[r] = sorted(ts)[len(ts) // 2]
-    peak, src = 1590.0, "fallback (B200_PROFILING.md 1.59 PFLOP/s burst)"
-    pth = os.path.join(ROOT, "MEASURED_PEAKS.json")
-    if os.path.exists(pth):
-        with open(pth) as f:
-            peak, src = float(json.load(f)["bf16_tflops"]), "measured (MEASURED_PEAKS.json bf16_tflops, burst)"
-    tf0 = algorithmic_flops(M, N, K, group, 0) / (res[0] * 1e-3) / 1e12
-    tf1 = algorithmic_flops(M, N, K, group, 64, "scalar") / (res[64] * 1e-3) / 1e12
-    return {"workload": "BASELINE.json configs[3]: M=4096, K=8192, N=28672, group=128, one layer call, median of 7",
-            "kernel": "spear::tc_kernel<256,2> (tcgen05, TMEM accumulators, EC folded in as extra k-blocks)",
-            "tflops_no_ec": round(tf0, 1), "ms_no_ec": round(res[0], 4),
-            "tflops_ec_r64": round(tf1, 1), "ms_ec_r64": round(res[64], 4),
-            "ec_overhead_time_frac": round(res[64] / res[0] - 1.0, 4),
-            "roofline": {"bound": "tensor", "achieved": round(tf0, 1), "peak": peak, "unit": "TFLOP/s",
-                         "frac": round(tf0 / peak, 4), "peak_source": src, "frac_of_nominal_2250": round(tf0 / 2250.0, 4)}}
+            if i >= 3:
+                ts.append(e0.elapsed_time(e1) * 1e3)
+        out.append(row(name, M, N, K, group, r, sorted(ts)[len(ts) // 2]))
+        del L
+    return out
+
+
+def stack_rows(sp, device, rand_layer, desc_of, gen, hbm, tpk):
+    """configs[4]: the 64-call projection stack as ONE spear_w4_ec_gemm_batch captured in ONE CUDA graph (reading A11), with the
+    ECs on o / down of layers {0, 1, 14, 15} and with no EC at all; the stack's own weights (579 MB) exceed L2."""
+    import torch
+    from workloads import algorithmic_flops
+    from workloads.configs import stack_shapes
+    out = []
+    for M in (64, 2048):
+        shapes = stack_shapes(M)
+        layers = [rand_layer(s.N, s.K, s.group, s.r) for s in shapes]
+        xs = [torch.randn(M, s.K, device=device, generator=gen).half() for s in shapes]
+        ys = [torch.empty(M, s.N, dtype=torch.float16, device=device) for s in shapes]
+        for with_ec in (False, True):
+            ds = [desc_of(L) if with_ec else sp.make_desc(gate="none") for L in layers]
+            batch = sp.Batch([(x, L["pw"], L.get("A") if with_ec else None, L.get("B") if with_ec else None, d, y)
+                              for x, L, d, y in zip(xs, layers, ds, ys)])
+            st = torch.cuda.Stream()
+            with torch.cuda.stream(st):
+                sp.w4_ec_gemm_batch(batch, stream=st)
+                torch.cuda.synchronize()
+                g = torch.cuda.CUDAGraph()
+                with torch.cuda.graph(g, stream=st):
+                    sp.w4_ec_gemm_batch(batch, stream=st)
+                g.replay()
+                torch.cuda.synchronize()
+                ts = []
+                for _ in range(5):
+                    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                    e0.record(st)
+                    g.replay()
+                    e1.record(st)
+                    e1.synchronize()
+                    ts.append(e0.elapsed_time(e1) * 1e3)
+            us = sorted(ts)[len(ts) // 2]
+            by = sum(algorithmic_bytes(M, s.N, s.K, s.group, s.r if with_ec else 0, "scalar") for s in shapes)
+            fl = sum(algorithmic_flops(M, s.N, s.K, s.group, s.r if with_ec else 0, "scalar") for s in shapes)
+            t_meas = sum(max(algorithmic_bytes(M, s.N, s.K, s.group, s.r if with_ec else 0, "scalar") / (hbm * 1e3),
+                             algorithmic_flops(M, s.N, s.K, s.group, s.r if with_ec else 0, "scalar") / (tpk * 1e6)) for s in shapes)
+            t_nom = sum(max(algorithmic_bytes(M, s.N, s.K, s.group, s.r if with_ec else 0, "scalar") / (NOMINAL_HBM_GBS * 1e3),
+                            algorithmic_flops(M, s.N, s.K, s.group, s.r if with_ec else 0, "scalar") / (NOMINAL_TFLOPS * 1e6)) for s in shapes)
+            out.append({"name": "16-layer stack, 64 calls, one batch in one CUDA graph", "M": M, "ec_on_8_calls": with_ec,
+                        "us": round(us, 1), "gbs": round(by / us * 1e-3, 1), "tflops": round(fl / us * 1e-6, 2),
+                        "sum_t_roof_measured_us": round(t_meas, 1), "frac_of_measured_roofline": round(t_meas / us, 4),
+                        "frac_of_nominal_roofline": round(t_nom / us, 4)})
+        del layers, xs, ys
+        torch.cuda.empty_cache()
+    return out
 
 
 # ------------------------------------------------------------------------------------------------
@@ -449,6 +695,7 @@ def main():
     ap.add_argument("--steps", type=int, default=2000)
     ap.add_argument("--warmup", type=int, default=50)
     ap.add_argument("--impl", default="cuda", choices=["cuda", "reference"])
+    ap.add_argument("--no-table", action="store_true", help="skip the per-config result table (configs key)")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "cuda" else args.warmup
     rank = int(os.environ.get("RANK", "0"))
