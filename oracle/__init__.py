@@ -51,6 +51,9 @@ def lib():
         L.spo_forward.restype = ctypes.c_int
         L.spo_forward.argtypes = [ctypes.c_void_p] * 4 + [ctypes.c_int, ctypes.c_int, ctypes.c_double] + \
             [ctypes.c_void_p] * 5 + [ctypes.c_double] + [ctypes.c_int] * 4 + [ctypes.c_void_p] * 4
+        L.spo_forward_q8.restype = ctypes.c_int
+        L.spo_forward_q8.argtypes = [ctypes.c_void_p] * 6 + [ctypes.c_int, ctypes.c_int, ctypes.c_double] + \
+            [ctypes.c_void_p] * 5 + [ctypes.c_double] + [ctypes.c_int] * 4 + [ctypes.c_void_p] * 4
         for name in ("spo_dequant", "spo_dequant16"):
             f = getattr(L, name)
             f.restype = ctypes.c_int
@@ -123,7 +126,7 @@ def dequant16(codes: np.ndarray, scales: np.ndarray, group: int) -> np.ndarray:
 
 
 def forward(x, What, A=None, B=None, gate="scalar", alpha=1.0, w_g=None, b_g=0.0,
-            W1=None, b1=None, W2=None, b2=None):
+            W1=None, b1=None, W2=None, b2=None, A_scale=None, B_scale=None):
     """O2..O6 on fp16 inputs (numpy float16 arrays) and an fp64 What from dequant().
 
     Returns dict(y, ybase, z, gam) in fp64; gam is [M][r] for the MLP gate, [M]
@@ -141,11 +144,21 @@ def forward(x, What, A=None, B=None, gate="scalar", alpha=1.0, w_g=None, b_g=0.0
     gam = np.zeros((M, max(r, 1)), np.float64)
     b1c = None if b1 is None else np.ascontiguousarray(b1, dtype=np.float32)
     b2c = None if b2 is None else np.ascontiguousarray(b2, dtype=np.float32)
-    rc = lib().spo_forward(_p(_bits(x)), _p(What), _p(_bits(A)), _p(_bits(B)),
-                           _GATE[gate], h, float(alpha),
-                           _p(_bits(W1)), _p(b1c), _p(_bits(W2)), _p(b2c),
-                           _p(_bits(w_g)), float(b_g), M, N, K, r,
-                           _p(y), _p(ybase), _p(z), _p(gam))
+    if A is not None and A.dtype == np.int8:       # INT8 per-channel symmetric EC factors
+        assert B.dtype == np.int8 and A_scale is not None and B_scale is not None
+        assert A_scale.shape == (r,) and B_scale.shape == (N,)
+        rc = lib().spo_forward_q8(_p(_bits(x)), _p(What), _p(np.ascontiguousarray(A)), _p(_bits(A_scale)),
+                                  _p(np.ascontiguousarray(B)), _p(_bits(B_scale)),
+                                  _GATE[gate], h, float(alpha),
+                                  _p(_bits(W1)), _p(b1c), _p(_bits(W2)), _p(b2c),
+                                  _p(_bits(w_g)), float(b_g), M, N, K, r,
+                                  _p(y), _p(ybase), _p(z), _p(gam))
+    else:
+        rc = lib().spo_forward(_p(_bits(x)), _p(What), _p(_bits(A)), _p(_bits(B)),
+                               _GATE[gate], h, float(alpha),
+                               _p(_bits(W1)), _p(b1c), _p(_bits(W2)), _p(b2c),
+                               _p(_bits(w_g)), float(b_g), M, N, K, r,
+                               _p(y), _p(ybase), _p(z), _p(gam))
     if rc:
         raise ValueError("spo_forward: bad arguments")
     out = {"y": y, "ybase": ybase, "z": None, "gam": None}
@@ -166,7 +179,8 @@ def forward_layer(li, rows=None):
     if li.r == 0:
         return forward(x, What, gate="none")
     return forward(x, What, li.A, li.B, gate=li.gate, alpha=li.alpha, w_g=li.w_g, b_g=li.b_g,
-                   W1=li.W1, b1=li.b1, W2=li.W2, b2=li.b2)
+                   W1=li.W1, b1=li.b1, W2=li.W2, b2=li.b2,
+                   A_scale=getattr(li, "A_scale", None), B_scale=getattr(li, "B_scale", None))
 
 
 def pack_w4(codes: np.ndarray, scales: np.ndarray, group: int):

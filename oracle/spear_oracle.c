@@ -16,6 +16,7 @@
  *              none   gamma = 1                                    Eq. 2, :96
  *   O5  u[m][j]     = gamma[m][j] * z[m][j]                        Eq. 3, :107
  *   O6  y[m][n]     = ybase[m][n] + alpha * sum_j B[n][j] u[m][j]  Eq. 3, :107
+ *   O3', O6'  the same with INT8 per-channel symmetric factors A8*sA, B8*sB   :603 (spo_forward_q8)
  *
  * Everything is fp64, plain left-to-right loops, no blocking, no reordering.
  * fp16 inputs arrive as raw uint16 bit patterns and are decoded by the decoder
@@ -152,7 +153,7 @@ enum { SPO_GATE_SCALAR_SIGMOID = 0, SPO_GATE_MLP = 1, SPO_GATE_NONE = 2 };
  * Outputs (any may be NULL): y[M][N], ybase[M][N], z[M][r], gam[M][r] (scalar/none gates are
  * broadcast along r).  Returns 0, or -1 on bad arguments.
  */
-int spo_forward(const uint16_t *x, const double *What, const uint16_t *A, const uint16_t *B,
+static int spo_forward_core(const uint16_t *x, const double *What, const double *A, const double *B,
                 int gate_kind, int h, double alpha,
                 const uint16_t *W1, const float *b1, const uint16_t *W2, const float *b2,
                 const uint16_t *w_g, double b_g,
@@ -178,7 +179,7 @@ int spo_forward(const uint16_t *x, const double *What, const uint16_t *A, const 
             for (int j = 0; j < r; ++j) {
                 double acc = 0.0;
                 for (int k = 0; k < K; ++k)
-                    acc += spo_f16_to_f64(A[(size_t)j * K + k]) * xd[(size_t)m * K + k];
+                    acc += A[(size_t)j * K + k] * xd[(size_t)m * K + k];
                 zz[(size_t)m * r + j] = acc;
             }
         }
@@ -227,7 +228,7 @@ int spo_forward(const uint16_t *x, const double *What, const uint16_t *A, const 
             for (int k = 0; k < K; ++k) acc += xr[k] * wr[k];
             double ec = 0.0;
             for (int j = 0; j < r; ++j)
-                ec += spo_f16_to_f64(B[(size_t)n * r + j]) * uu[(size_t)m * r + j];
+                ec += B[(size_t)n * r + j] * uu[(size_t)m * r + j];
             if (ybase) ybase[(size_t)m * N + n] = acc;
             if (y) y[(size_t)m * N + n] = acc + alpha * ec;
         }
@@ -236,6 +237,58 @@ int spo_forward(const uint16_t *x, const double *What, const uint16_t *A, const 
     if (gam && r > 0) memcpy(gam, gg, sizeof(double) * (size_t)M * r);
     free(xd); free(zz); free(uu); free(gg);
     return 0;
+}
+
+/* fp16 EC factors (the exact fp64 value of every fp16 entry) */
+int spo_forward(const uint16_t *x, const double *What, const uint16_t *A, const uint16_t *B,
+                int gate_kind, int h, double alpha,
+                const uint16_t *W1, const float *b1, const uint16_t *W2, const float *b2,
+                const uint16_t *w_g, double b_g,
+                int M, int N, int K, int r,
+                double *y, double *ybase, double *z, double *gam)
+{
+    double *Ad = NULL, *Bd = NULL;
+    if (r > 0) {
+        if (!A || !B) return -1;
+        Ad = (double *)malloc(sizeof(double) * (size_t)r * K);
+        Bd = (double *)malloc(sizeof(double) * (size_t)N * r);
+        if (!Ad || !Bd) { free(Ad); free(Bd); return -1; }
+        spo_f16_to_f64_array(A, Ad, (size_t)r * K);
+        spo_f16_to_f64_array(B, Bd, (size_t)N * r);
+    }
+    int rc = spo_forward_core(x, What, Ad, Bd, gate_kind, h, alpha, W1, b1, W2, b2, w_g, b_g, M, N, K, r, y, ybase, z, gam);
+    free(Ad); free(Bd);
+    return rc;
+}
+
+/*
+ * INT8 EC factors, "INT8 per-channel symmetric" (PAPER.md:603, Table 7; :585, :607): the stored factors are
+ *   Ahat[j][k] = A8[j][k] * sA[j]      (one fp16 scale per row of A, i.e. per rank channel j)
+ *   Bhat[n][j] = B8[n][j] * sB[n]      (one fp16 scale per row of B, i.e. per output channel n)
+ * (reading A17 of DESIGN.md: "per-channel" = per output channel of each factor); everything else is Eq. 3 unchanged.
+ * The products int8 * fp16 are exact in fp64.
+ */
+int spo_forward_q8(const uint16_t *x, const double *What, const int8_t *A8, const uint16_t *sA,
+                   const int8_t *B8, const uint16_t *sB,
+                   int gate_kind, int h, double alpha,
+                   const uint16_t *W1, const float *b1, const uint16_t *W2, const float *b2,
+                   const uint16_t *w_g, double b_g,
+                   int M, int N, int K, int r,
+                   double *y, double *ybase, double *z, double *gam)
+{
+    if (r <= 0 || !A8 || !sA || !B8 || !sB) return -1;
+    double *Ad = (double *)malloc(sizeof(double) * (size_t)r * K);
+    double *Bd = (double *)malloc(sizeof(double) * (size_t)N * r);
+    if (!Ad || !Bd) { free(Ad); free(Bd); return -1; }
+    for (int j = 0; j < r; ++j)
+        for (int k = 0; k < K; ++k)
+            Ad[(size_t)j * K + k] = (double)A8[(size_t)j * K + k] * spo_f16_to_f64(sA[j]);
+    for (int n = 0; n < N; ++n)
+        for (int j = 0; j < r; ++j)
+            Bd[(size_t)n * r + j] = (double)B8[(size_t)n * r + j] * spo_f16_to_f64(sB[n]);
+    int rc = spo_forward_core(x, What, Ad, Bd, gate_kind, h, alpha, W1, b1, W2, b2, w_g, b_g, M, N, K, r, y, ybase, z, gam);
+    free(Ad); free(Bd);
+    return rc;
 }
 
 /* ---- Q1: packed layout, from the layout document ---------------------------------------- */

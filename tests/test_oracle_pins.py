@@ -233,6 +233,57 @@ def test_P8_bruteforce_rational_with_the_gate(gate, h):
         assert n_clipped > 0          # the ReLU really clips on this input
 
 
+# ---------------------------------------------------------------- INT8 EC factors
+
+def test_int8_ec_worked_example():
+    with open(os.path.join(GOLD, "int8_ec_worked_example.json")) as f:
+        g = json.load(f)
+    What = oracle.dequant(np.array(g["codes"], np.uint8), f16(g["scales"]), g["group"])
+    for c in g["cases"]:
+        out = oracle.forward(f16(g["x"]), What, np.array(g["A8"], np.int8), np.array(g["B8"], np.int8), gate="none",
+                             alpha=g["alpha"], A_scale=f16(c["sA"]), B_scale=f16(c["sB"]))
+        assert np.array_equal(out["ybase"], np.array(g["ybase"]))
+        assert np.array_equal(out["z"], np.array(c["z"]))
+        assert np.array_equal(out["y"], np.array(c["y"]))
+
+
+def test_int8_ec_equals_fp16_ec_when_the_products_are_representable():
+    """code * scale with a power-of-two scale is an exact fp16: the int8 path must then give the fp16 path's result bit for
+    bit (same fp64 operands, same loops) -- pins the dequantisation of the factors against the already pinned fp16 path."""
+    from workloads import with_int8_ec
+    li = make_layer(seed=31, M=4, N=128, K=256, group=128, r=8, gate="mlp")
+    l8 = with_int8_ec(li)
+    l8.A_scale = np.full(li.r, 2.0 ** -7, np.float16)
+    l8.B_scale = np.full(li.N, 2.0 ** -5, np.float16)
+    l8.B_scale[::3] = np.float16(2.0 ** -4)          # unequal per-row scales
+    lf = make_layer(seed=31, M=4, N=128, K=256, group=128, r=8, gate="mlp")
+    lf.A = (l8.A.astype(np.float64) * l8.A_scale.astype(np.float64)[:, None]).astype(np.float16)
+    lf.B = (l8.B.astype(np.float64) * l8.B_scale.astype(np.float64)[:, None]).astype(np.float16)
+    assert np.array_equal(lf.A.astype(np.float64), l8.A.astype(np.float64) * l8.A_scale.astype(np.float64)[:, None])
+    a, b = oracle.forward_layer(l8), oracle.forward_layer(lf)
+    for k in ("y", "z", "gam"):
+        assert np.array_equal(a[k], b[k]), k
+
+
+def test_int8_ec_bruteforce_rational():
+    from workloads import with_int8_ec
+    li = with_int8_ec(make_layer(seed=33, M=2, N=128, K=256, group=128, r=8, gate="none"))
+    Nn = 4
+    What = oracle.dequant(li.codes[:Nn], li.scales[:Nn], li.group)
+    out = oracle.forward(li.x, What, li.A, li.B[:Nn], gate="none", alpha=1.5, A_scale=li.A_scale, B_scale=li.B_scale[:Nn])
+    X, S = _frac(li.x), _frac(li.scales[:Nn])
+    sA = [Fraction(float(v)) for v in li.A_scale]
+    sB = [Fraction(float(v)) for v in li.B_scale[:Nn]]
+    for m in range(li.M):
+        z = [sA[j] * sum(int(li.A[j][k]) * X[m][k] for k in range(li.K)) for j in range(li.r)]
+        for j in range(li.r):
+            assert abs(out["z"][m][j] - float(z[j])) <= 1e-13 * max(1.0, abs(float(z[j])))
+        for n in range(Nn):
+            base = sum(X[m][k] * (int(li.codes[n][k]) - 8) * S[n][k // li.group] for k in range(li.K))
+            y = base + Fraction(3, 2) * sB[n] * sum(int(li.B[n][j]) * z[j] for j in range(li.r))
+            assert abs(out["y"][m][n] - float(y)) <= 1e-12 * max(1.0, abs(float(y)))
+
+
 # ---------------------------------------------------------------- P2 reductions to plain W4
 
 def test_P2_zero_A_or_B_or_closed_gate_is_plain_w4():

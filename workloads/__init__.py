@@ -9,6 +9,7 @@ from .synth import (  # noqa: F401
     TAGS,
     LayerInputs,
     make_layer,
+    with_int8_ec,
     codes_uniform,
     normal_f64,
     uniform_f64,

@@ -77,12 +77,12 @@ def stack_shapes(M: int) -> List[LayerShape]:
 CONFIGS = [config_shapes(i) for i in range(5)]
 
 
-def algorithmic_bytes(M, N, K, group, r, gate="scalar", h=0) -> int:
-    """bytes_W4 + bytes_EC of SURVEY.md 8(d) (what the method must move)."""
+def algorithmic_bytes(M, N, K, group, r, gate="scalar", h=0, ec_int8=False) -> int:
+    """bytes_W4 + bytes_EC of SURVEY.md 8(d) (what the method must move); ec_int8: INT8 factors + their fp16 row scales."""
     G = K // group
     b = N * K // 2 + 2 * N * G + 2 * M * K + 2 * M * N
     if r > 0:
-        b += 2 * r * (K + N)
+        b += (r * (K + N) + 2 * (r + N)) if ec_int8 else 2 * r * (K + N)
         if gate == "scalar":
             b += 2 * K + 4
         elif gate == "mlp":

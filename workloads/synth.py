@@ -112,6 +112,8 @@ class LayerInputs:
     b1: Optional[np.ndarray] = None
     W2: Optional[np.ndarray] = None
     b2: Optional[np.ndarray] = None
+    A_scale: Optional[np.ndarray] = None      # INT8 EC factors: A is int8 [r][K] with one fp16 scale per row
+    B_scale: Optional[np.ndarray] = None      # B is int8 [N][r] with one fp16 scale per row (output channel)
     outlier_channels: np.ndarray = field(default_factory=lambda: np.zeros(0, np.int64))
 
 
@@ -155,3 +157,24 @@ def make_layer(seed: int, M: int, N: int, K: int, group: int, r: int,
             li.b1 = np.zeros(hh, np.float32)
             li.b2 = np.zeros(r, np.float32)
     return li
+
+
+def with_int8_ec(li: LayerInputs) -> LayerInputs:
+    """The same layer with its EC factors stored the way the paper stores them after calibration: "INT8 per-channel
+    symmetric".  Input preparation only: per row, scale = fp16(max|v| / 127), code = clamp(round-half-even
+    (v / scale), -127, 127).  The quantised factors (code * scale) are the layer's EC from here on -- the oracle and the
+    GPU both consume the int8 codes and the fp16 scales."""
+    import copy
+    assert li.r > 0 and li.A.dtype == np.float16
+    out = copy.copy(li)
+
+    def q(mat):
+        m = mat.astype(np.float64)
+        s = np.max(np.abs(m), axis=1) / 127.0
+        s = np.where(s > 0, s, 1.0).astype(np.float16)
+        codes = np.clip(np.rint(m / s.astype(np.float64)[:, None]), -127, 127).astype(np.int8)
+        return np.ascontiguousarray(codes), np.ascontiguousarray(s)
+
+    out.A, out.A_scale = q(li.A)
+    out.B, out.B_scale = q(li.B)
+    return out
