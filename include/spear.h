@@ -54,6 +54,8 @@ typedef enum {
 
 /* Execution variants.  AUTO consults the table filled by spear_plan and
  * otherwise a size heuristic. */
+typedef enum { SPEAR_EC_FP16 = 0, SPEAR_EC_INT8 = 1 } spear_ec_dtype;
+
 typedef enum {
     SPEAR_VARIANT_AUTO = 0,
     SPEAR_VARIANT_STREAM_FUSED = 1,  /* one kernel: weight stream (mma.sync) + x.A^T, gate, B add inside; M <= 16, scalar / none gate */
@@ -112,6 +114,11 @@ typedef struct {
                                  relative to the END of the buffer).                                    */
     size_t workspace_bytes;
     int force_variant;        /* spear_variant; SPEAR_VARIANT_AUTO = use the plan                   */
+    int ec_dtype;             /* spear_ec_dtype: storage of A and B.  SPEAR_EC_INT8 = "INT8 per-channel symmetric"
+                                 (PAPER.md:603): A is int8 [r][K], B is int8 [N][r], Ahat[j][k] = A[j][k] * A_scale[j],
+                                 Bhat[n][j] = B[n][j] * B_scale[n] (reading A17)                                        */
+    const void* A_scale;      /* [r] fp16, SPEAR_EC_INT8 only                                        */
+    const void* B_scale;      /* [N] fp16, SPEAR_EC_INT8 only                                        */
 } spear_ec_desc;
 
 int spear_w4_ec_gemm_ex(const void* x, const void* Wq, const void* scales, const void* A, const void* B,

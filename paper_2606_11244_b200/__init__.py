@@ -43,6 +43,7 @@ class EcDesc(ctypes.Structure):
         ("W1", ctypes.c_void_p), ("b1", ctypes.c_void_p), ("W2", ctypes.c_void_p), ("b2", ctypes.c_void_p),
         ("w_g", ctypes.c_void_p), ("b_g", ctypes.c_void_p), ("gate_out", ctypes.c_void_p),
         ("workspace", ctypes.c_void_p), ("workspace_bytes", ctypes.c_size_t), ("force_variant", ctypes.c_int),
+        ("ec_dtype", ctypes.c_int), ("A_scale", ctypes.c_void_p), ("B_scale", ctypes.c_void_p),
     ]
 
 
@@ -190,7 +191,7 @@ def w4_ec_gemm(x, pw: PackedW4, A=None, B=None, gate_w=None, gate_b=None, y=None
 
 
 def make_desc(gate="scalar", alpha=1.0, w_g=None, b_g=None, W1=None, b1=None, W2=None, b2=None,
-              gate_out=None, workspace=None, variant=VARIANT_AUTO) -> EcDesc:
+              gate_out=None, workspace=None, variant=VARIANT_AUTO, A_scale=None, B_scale=None) -> EcDesc:
     d = EcDesc()
     d.gate_kind = GATE_KINDS[gate] if isinstance(gate, str) else int(gate)
     d.gate_hidden = 0 if W1 is None else int(W1.shape[0])
@@ -200,6 +201,8 @@ def make_desc(gate="scalar", alpha=1.0, w_g=None, b_g=None, W1=None, b1=None, W2
     d.workspace = _ptr(workspace)
     d.workspace_bytes = 0 if workspace is None else workspace.numel() * workspace.element_size()
     d.force_variant = int(variant)
+    d.ec_dtype = 0 if A_scale is None else 1          # SPEAR_EC_INT8: A / B are int8 with one fp16 scale per row
+    d.A_scale, d.B_scale = _ptr(A_scale), _ptr(B_scale)
     return d
 
 

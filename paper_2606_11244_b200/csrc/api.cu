@@ -41,7 +41,7 @@ const DeviceInfo& device_info() { return g_dev; }
 
 // workspace layout (byte offsets); every region is 1 KiB aligned
 struct WsLayout {
-    size_t counters, zbuf, zfused, u32, partial, u16, total;
+    size_t counters, zbuf, zfused, u32, partial, ec16, u16, total;
 };
 constexpr size_t kCounterBytes = 64 * 1024;          // 16384 u32
 constexpr int kEcPreCounter = 8192;                  // index into counters[]
@@ -50,7 +50,7 @@ static size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
 // Fixed-size regions first; the two regions whose size depends on M must never alias a region that a
 // call with another M leaves non-zero: zbuf (kept zero between calls) grows up from a fixed offset and
 // u16 (scratch) grows DOWN from the end of the workspace.
-static WsLayout ws_layout(int M, int r, size_t ws_bytes) {
+static WsLayout ws_layout(int M, int r, size_t ws_bytes, size_t ec16_bytes = 0) {
     WsLayout L;
     size_t o = 0;
     L.counters = o; o += kCounterBytes;
@@ -58,6 +58,7 @@ static WsLayout ws_layout(int M, int r, size_t ws_bytes) {
     L.zfused = o; o += align_up(size_t(2) * 16 * kZStride * 4, 1024);   // fused decode EC: z, double-buffered by epoch parity
     L.partial = o; o += size_t(kMaxStreamGrid) * 2 * 16 * 128 * 4;
     L.zbuf = o; o += align_up(size_t(M > 16 ? M : 16) * kZStride * 4, 1024);
+    L.ec16 = o; o += align_up(ec16_bytes, 1024);      // INT8 EC factors dequantised to fp16 (M > 16 path only)
     const size_t u16_bytes = align_up(size_t(M) * size_t(r) * 2 + 1024, 1024);
     L.total = o + u16_bytes;
     L.u16 = ws_bytes >= L.total ? (ws_bytes - u16_bytes) & ~size_t(1023) : o;
@@ -295,6 +296,12 @@ static int check_problem(const void* x, const void* Wq, const void* scales, cons
     if (r > 0) {
         if (!A || !B || !ec) return set_error(SPEAR_EINVAL, "r > 0 needs A, B and the EC descriptor");
         al |= uintptr_t(A) | uintptr_t(B);
+        if (ec->ec_dtype == SPEAR_EC_INT8) {
+            if (!ec->A_scale || !ec->B_scale) return set_error(SPEAR_EINVAL, "INT8 EC factors need A_scale[r] and B_scale[N]");
+            if ((uintptr_t(ec->A_scale) | uintptr_t(ec->B_scale)) & 1) return set_error(SPEAR_EINVAL, "A_scale / B_scale must be fp16-aligned");
+        } else if (ec->ec_dtype != SPEAR_EC_FP16) {
+            return set_error(SPEAR_EINVAL, "unknown ec_dtype %d", ec->ec_dtype);
+        }
         if (ec->gate_kind == SPEAR_GATE_SCALAR_SIGMOID) {
             if (!ec->w_g) return set_error(SPEAR_EINVAL, "scalar gate needs w_g");
             al |= uintptr_t(ec->w_g);
@@ -325,7 +332,7 @@ static int ws_prepare(uint8_t* ws, size_t ws_bytes, const WsLayout& L, int M, in
         SPEAR_CUDA_OK(cudaMemsetAsync(ws + lo, 0, zend - lo, st));
         lo = zend;
     }
-    if (uses_u16 && r > 0) lo = std::min(lo, L.u16);
+    if (uses_u16 && r > 0) lo = std::min(lo, std::min(L.u16, L.ec16));
     g_ws_dirty_lo[ws] = lo;
     return SPEAR_OK;
 }
@@ -340,6 +347,8 @@ static int run_stream(const void* x, const void* Wq, const void* scales, const v
         EcPreParams e = {};
         e.x = static_cast<const __half*>(x);
         e.A = static_cast<const __half*>(A);
+        e.ec_int8 = ec->ec_dtype == SPEAR_EC_INT8;
+        e.A_scale = static_cast<const __half*>(ec->A_scale);
         e.w_g = static_cast<const __half*>(ec->w_g);
         e.b_g = static_cast<const float*>(ec->b_g);
         e.W1 = static_cast<const __half*>(ec->W1);
@@ -367,6 +376,11 @@ static int run_stream(const void* x, const void* Wq, const void* scales, const v
     p.y = static_cast<__half*>(y);
     p.u = u32;
     p.B = static_cast<const __half*>(B);
+    if (r > 0 && ec && ec->ec_dtype == SPEAR_EC_INT8) {
+        p.ec_int8 = 1;
+        p.A_scale = static_cast<const __half*>(ec->A_scale);
+        p.B_scale = static_cast<const __half*>(ec->B_scale);
+    }
     p.partial = reinterpret_cast<float*>(ws + L.partial);
     p.counters = counters;
     p.M = M; p.N = N; p.K = K; p.r = r;
@@ -423,6 +437,15 @@ static int run_tc_fused(const void* x, const void* Wq, const void* scales, const
                         const spear_ec_desc* ec, void* y, int M, int N, int K, int r, int group,
                         uint8_t* ws, const WsLayout& L, bool split, cudaStream_t st) {
     const bool pdl = g_tune.pdl != 0;
+    if (r > 0 && ec->ec_dtype == SPEAR_EC_INT8) {
+        // INT8 EC factors: code * row scale -> fp16 scratch in the workspace, then the fp16 path (r (K + N) elements)
+        __half* A16 = reinterpret_cast<__half*>(ws + L.ec16);
+        __half* B16 = A16 + size_t(r) * K;
+        if (int rc = launch_ec_dequant_i8(static_cast<const int8_t*>(A), static_cast<const __half*>(ec->A_scale), A16, r, K, st)) return rc;
+        if (int rc = launch_ec_dequant_i8(static_cast<const int8_t*>(B), static_cast<const __half*>(ec->B_scale), B16, N, r, st)) return rc;
+        A = A16;
+        B = B16;
+    }
     if (r > 0) {
         EcBigParams e = {};
         e.x = static_cast<const __half*>(x);
@@ -477,6 +500,7 @@ static bool overlaps(const void* a, size_t an, const void* b, size_t bn) {
 static bool ls_eligible(const spear_call& c) {
     if (c.M < 1 || c.M > 16) return false;
     if (c.r > 0 && c.ec && c.ec->gate_kind == SPEAR_GATE_MLP) return false;
+    if (c.r > 0 && c.ec && c.ec->ec_dtype == SPEAR_EC_INT8) return false;
     if (c.ec && c.ec->workspace) return false;
     const int gcn = c.group / 128;
     if (c.group != c.K && (gcn & (gcn - 1))) return false;      // scale groups: a power-of-two number of 128-column chunks, or per-channel
@@ -599,7 +623,8 @@ static int layer_impl(const void* x, const void* Wq, const void* scales, const v
         ws_bytes = ec->workspace_bytes;
         if (uintptr_t(ws) & 1023) return set_error(SPEAR_EINVAL, "workspace must be 1024-byte aligned");
     }
-    const WsLayout L = ws_layout(M, r, ws_bytes);
+    const bool ec_i8 = (r > 0 && ec && ec->ec_dtype == SPEAR_EC_INT8);
+    const WsLayout L = ws_layout(M, r, ws_bytes, (ec_i8 && M > 16) ? size_t(r) * (size_t(K) + N) * 2 : 0);
     if (ws_bytes < L.total + 1024)
         return set_error(SPEAR_ENOMEM, "workspace too small: need %zu bytes, have %zu (pass spear_ec_desc.workspace)", L.total, ws_bytes);
     const int gate = (r > 0 && ec) ? ec->gate_kind : SPEAR_GATE_NONE;
@@ -619,6 +644,12 @@ static int layer_impl(const void* x, const void* Wq, const void* scales, const v
         if (v == SPEAR_VARIANT_LSTREAM && odd_group)
             return set_error(SPEAR_EUNSUPPORTED, "the layer-stream variant needs group / 128 to be a power of two (or group == K)");
     }
+    if (v == SPEAR_VARIANT_LSTREAM && ec_i8) {
+        if (ec->force_variant != SPEAR_VARIANT_AUTO) return set_error(SPEAR_EUNSUPPORTED, "the layer-stream variant takes fp16 EC factors");
+        v = (gate != SPEAR_GATE_MLP) ? SPEAR_VARIANT_STREAM_FUSED : SPEAR_VARIANT_STREAM_SPLIT;
+    }
+    if (ec_i8 && M <= 16 && (v == SPEAR_VARIANT_TC_FUSED || v == SPEAR_VARIANT_TC_SPLIT))
+        return set_error(SPEAR_EUNSUPPORTED, "INT8 EC factors on the tcgen05 variants need M > 16 (workspace scratch is sized for that path)");
     if (v == SPEAR_VARIANT_LSTREAM) {
         if (ec && ec->workspace) return set_error(SPEAR_EUNSUPPORTED, "the layer-stream variant uses the library's own workspace");
         spear_call c = {x, Wq, scales, A, B, ec, y, M, N, K, r, group};
@@ -681,9 +712,9 @@ extern "C" int spear_tune(const char* key, int value) {
 }
 
 extern "C" int spear_workspace_bytes(int M, int N, int K, int r, int group, size_t* bytes) {
-    (void)N; (void)K; (void)group;
+    (void)group;
     if (!bytes || M < 1 || r < 0) return set_error(SPEAR_EINVAL, "bad arguments");
-    *bytes = ws_layout(M, r, 0).total + 1024;
+    *bytes = ws_layout(M, r, 0, M > 16 ? size_t(r) * (size_t(K) + N) * 2 : 0).total + 1024;      // incl. the INT8-EC scratch
     return SPEAR_OK;
 }
 
@@ -791,7 +822,8 @@ static int batch_impl(const spear_call* calls, const spear_host_io* io, int n_ca
         const spear_call& c = calls[i];
         if (c.ec && c.ec->workspace) { status = set_error(SPEAR_EINVAL, "batch calls use the library's lane workspaces (ec->workspace must be NULL)"); break; }
         size_t need = 0;
-        if (c.M >= 1 && c.r >= 0) need = ws_layout(c.M, c.r, 0).total + 1024;
+        if (c.M >= 1 && c.r >= 0)
+            need = ws_layout(c.M, c.r, 0, (c.M > 16 && c.ec && c.ec->ec_dtype == SPEAR_EC_INT8) ? size_t(c.r) * (size_t(c.K) + c.N) * 2 : 0).total + 1024;
         const int l = lane_of[i];
         if (io && (!io[i].x_host || !io[i].y_host || c.M < 1 || c.N < 1 || c.K < 1)) {
             status = set_error(SPEAR_EINVAL, "batch call %d: NULL host buffer", i);

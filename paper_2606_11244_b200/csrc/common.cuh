@@ -178,6 +178,17 @@ __device__ __forceinline__ void dequant_word(uint32_t w, uint32_t (&out)[4]) {
     asm("sub.f16x2 %0, %1, %2;" : "=r"(out[2]) : "r"(lo1), "r"(kSub));
     asm("fma.rn.f16x2 %0, %1, %2, %3;" : "=r"(out[3]) : "r"(hi1), "r"(kSixteenth), "r"(kNeg72));
 }
+// ---- int8 -> fp16 (INT8 EC factors): four signed bytes of one word -> two half2, exact ----
+// b ^ 0x80 is b + 128 as an unsigned byte; spliced under the exponent byte 0x64 it is the fp16 value 1024 + (b + 128);
+// minus 1152 gives b.
+__device__ __forceinline__ void cvt_i8x4_f16x2(uint32_t w, uint32_t& lo, uint32_t& hi) {
+    const uint32_t x = w ^ 0x80808080u;
+    uint32_t a, b;
+    asm("prmt.b32 %0, %1, %2, 0x5140;" : "=r"(a) : "r"(x), "r"(0x64646464u));     // bytes: x0, 0x64, x1, 0x64
+    asm("prmt.b32 %0, %1, %2, 0x7362;" : "=r"(b) : "r"(x), "r"(0x64646464u));     // bytes: x2, 0x64, x3, 0x64
+    asm("sub.f16x2 %0, %1, %2;" : "=r"(lo) : "r"(a), "r"(0x64806480u));
+    asm("sub.f16x2 %0, %1, %2;" : "=r"(hi) : "r"(b), "r"(0x64806480u));
+}
 __device__ __forceinline__ uint32_t hmul2_u32(uint32_t a, uint32_t b) {
     uint32_t d;
     asm("mul.rn.f16x2 %0, %1, %2;" : "=r"(d) : "r"(a), "r"(b));

@@ -9,6 +9,7 @@
 // same k-permutation trick as the weight kernel: a lane reads 32 contiguous bytes of a row), partial
 // z goes to a global fp32 buffer with red.add, and the LAST CTA to arrive (atomic counter) applies the
 // gate, writes u and re-zeroes the buffer so the workspace is clean for the next call.
+#include <algorithm>
 #include <mutex>
 
 #include "common.cuh"
@@ -22,6 +23,19 @@ __device__ __forceinline__ void load_row32(const __half* row, int col, uint32_t 
         const uint4 b = __ldg(reinterpret_cast<const uint4*>(row + col + 8));
         lo[0] = a.x; lo[1] = a.y; lo[2] = a.z; lo[3] = a.w;
         hi[0] = b.x; hi[1] = b.y; hi[2] = b.z; hi[3] = b.w;
+    } else {
+#pragma unroll
+        for (int i = 0; i < 4; ++i) lo[i] = hi[i] = 0u;
+    }
+}
+// INT8 factor row: 16 columns = 16 bytes, converted exactly to the fp16 fragment registers
+__device__ __forceinline__ void load_row32_i8(const int8_t* row, int col, uint32_t (&lo)[4], uint32_t (&hi)[4]) {
+    if (row) {
+        const uint4 a = __ldg(reinterpret_cast<const uint4*>(row + col));
+        cvt_i8x4_f16x2(a.x, lo[0], lo[1]);
+        cvt_i8x4_f16x2(a.y, lo[2], lo[3]);
+        cvt_i8x4_f16x2(a.z, hi[0], hi[1]);
+        cvt_i8x4_f16x2(a.w, hi[2], hi[3]);
     } else {
 #pragma unroll
         for (int i = 0; i < 4; ++i) lo[i] = hi[i] = 0u;
@@ -154,8 +168,10 @@ __global__ void __launch_bounds__(128) ec_pre_kernel(const EcPreParams p) {
     for (int kt = kt_begin + warp; kt < kt_end; kt += 4) {
         const int col = kt * 64 + 16 * t;
         uint32_t a0l[4], a0h[4], a1l[4], a1h[4], x0l[4], x0h[4], x1l[4], x1h[4];
-        load_row32(pa0, col, a0l, a0h);
-        load_row32(pa1, col, a1l, a1h);
+        if (p.ec_int8 && rho0 < p.r) load_row32_i8(reinterpret_cast<const int8_t*>(p.A) + size_t(rho0) * p.K, col, a0l, a0h);
+        else load_row32(pa0, col, a0l, a0h);
+        if (p.ec_int8 && rho1 < p.r) load_row32_i8(reinterpret_cast<const int8_t*>(p.A) + size_t(rho1) * p.K, col, a1l, a1h);
+        else load_row32(pa1, col, a1l, a1h);
         load_x32(px0, col, x0l, x0h);
         load_x32(px1, col, x1l, x1h);
 #pragma unroll
@@ -174,7 +190,8 @@ __global__ void __launch_bounds__(128) ec_pre_kernel(const EcPreParams p) {
         const int row = o & 15, tok = o >> 4;
         const int rho = strip * 16 + row;
         if (tok < p.M && rho < rows_total) {
-            const float v = red[0][row][tok] + red[1][row][tok] + red[2][row][tok] + red[3][row][tok];
+            float v = red[0][row][tok] + red[1][row][tok] + red[2][row][tok] + red[3][row][tok];
+            if (p.ec_int8 && rho < p.r) v *= __half2float(__ldg(p.A_scale + rho));     // per-row scale of the INT8 factor
             atomicAdd(p.zbuf + tok * kZStride + rho, v);
         }
     }
@@ -381,6 +398,29 @@ __global__ void __launch_bounds__(256) ec_update_kernel(const __half* __restrict
             *yp = __float2half_rn(__half2float(*yp) + acc[t]);
         }
     }
+}
+
+// INT8 EC factors on the M > 16 path: code * per-row scale -> fp16 scratch (one rounding; the tcgen05 path consumes fp16
+// operand tiles through TMA).  r (K + N) elements per call, < 1 % of the layer's weight bytes.
+__global__ void ec_dequant_i8_kernel(const int8_t* __restrict__ q, const __half* __restrict__ scale, __half* __restrict__ out,
+                                     int rows, int cols) {
+    const size_t n = size_t(rows) * cols;
+    for (size_t i = (blockIdx.x * size_t(blockDim.x) + threadIdx.x) * 4; i < n; i += size_t(gridDim.x) * blockDim.x * 4) {
+        const int row = int(i / cols);          // cols % 8 == 0: the four elements share a row
+        const float s = __half2float(__ldg(scale + row));
+        const char4 c = *reinterpret_cast<const char4*>(q + i);
+        __half2 a = __floats2half2_rn(float(c.x) * s, float(c.y) * s), b = __floats2half2_rn(float(c.z) * s, float(c.w) * s);
+        *reinterpret_cast<__half2*>(out + i) = a;
+        *reinterpret_cast<__half2*>(out + i + 2) = b;
+    }
+}
+int launch_ec_dequant_i8(const int8_t* q, const __half* scale, __half* out, int rows, int cols, cudaStream_t st) {
+    const size_t n = size_t(rows) * cols;
+    const int blocks = int(std::min<size_t>(1184, (n / 4 + 255) / 256));
+    ec_dequant_i8_kernel<<<std::max(blocks, 1), 256, 0, st>>>(q, scale, out, rows, cols);
+    SPEAR_CUDA_OK(cudaGetLastError());
+    count_launch();
+    return SPEAR_OK;
 }
 
 int launch_ec_update(const __half* u16, const __half* B, __half* y, int M, int N, int r, bool pdl, cudaStream_t st) {

@@ -13,7 +13,10 @@ struct StreamParams {
     const void* scales;      // SPW4 packed scales
     __half* y;               // [M][N]
     const float* u;          // [16][r] fp32, alpha * gamma (.) z (EC pre-kernel); unused when r == 0
-    const __half* B;         // [N][r]
+    const __half* B;         // [N][r] (int8 [N][r] when ec_int8)
+    int ec_int8;             // 1: A and B are int8 with one fp16 scale per row
+    const __half* A_scale;   // [r]
+    const __half* B_scale;   // [N]
     float* partial;          // [grid * 2][8*MT][128] fp32 split-K slots
     unsigned* counters;      // [N / 128], zero between calls
     int M, N, K, r;
@@ -95,7 +98,9 @@ int launch_lstream(const LsParams& p, cudaStream_t st);
 // ---- ec_pre.cu (M <= 16): z = x A^T, gate, u = alpha * gamma (.) z ------------------------------
 struct EcPreParams {
     const __half* x;         // [M][K]
-    const __half* A;         // [r][K]
+    const __half* A;         // [r][K] (int8 [r][K] when ec_int8)
+    int ec_int8;
+    const __half* A_scale;   // [r]
     const __half* w_g;       // [K]       scalar gate
     const float* b_g;        // 1 (device) or NULL
     const __half* W1;        // [h][r]    MLP gate
@@ -129,6 +134,8 @@ struct EcBigParams {
 int launch_ec_big(const EcBigParams& p, bool pdl, cudaStream_t st);
 // split arm for M > 16: y += u16 . B^T as a separate pass (SPEAR_VARIANT_TC_SPLIT)
 int launch_ec_update(const __half* u16, const __half* B, __half* y, int M, int N, int r, bool pdl, cudaStream_t st);
+// INT8 EC factors on the M > 16 path: rows * cols int8 codes times one fp16 scale per row -> fp16 scratch
+int launch_ec_dequant_i8(const int8_t* q, const __half* scale, __half* out, int rows, int cols, cudaStream_t st);
 
 // ---- tc.cu (M > 16): tcgen05 GEMM, int4 dequantised into shared memory, EC folded in as extra K blocks
 struct TcProblem {

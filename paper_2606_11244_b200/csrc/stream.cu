@@ -186,6 +186,20 @@ __device__ __forceinline__ void ec_load16(const __half* row, int col, bool reado
     }
 }
 
+// the same 16 columns of an INT8 factor row (16 bytes): exact conversion to the fp16 fragment registers
+__device__ __forceinline__ void ec_load16_i8(const int8_t* row, int col, uint32_t (&lo)[4], uint32_t (&hi)[4]) {
+    if (row) {
+        const uint4 a = __ldg(reinterpret_cast<const uint4*>(row + col));
+        cvt_i8x4_f16x2(a.x, lo[0], lo[1]);
+        cvt_i8x4_f16x2(a.y, lo[2], lo[3]);
+        cvt_i8x4_f16x2(a.z, hi[0], hi[1]);
+        cvt_i8x4_f16x2(a.w, hi[2], hi[3]);
+    } else {
+#pragma unroll
+        for (int i = 0; i < 4; ++i) lo[i] = hi[i] = 0u;
+    }
+}
+
 // Before griddepcontrol.wait: pull this CTA's slice of [A; w_g] (the rows / K range of its phase-A tasks) into
 // L2, so that the loads after the wait do not pay an HBM round trip on the critical path.
 __device__ void ec_prefetch_factors(const StreamParams& p, int lane) {
@@ -203,6 +217,10 @@ __device__ void ec_prefetch_factors(const StreamParams& p, int lane) {
         const int lines = kt_end - kt_begin;           // 128-byte lines per row
         for (int i = lane; i < 16 * lines; i += 32) {
             const int rho = strip * 16 + i / lines, kt = kt_begin + i % lines;
+            if (p.ec_int8 && rho < p.r) {
+                if ((kt & 1) == 0) prefetch_l2(reinterpret_cast<const int8_t*>(p.A) + size_t(rho) * p.K + kt * 64);
+                continue;
+            }
             const __half* row = rho < p.r ? p.A + size_t(rho) * p.K : (rho == p.r && scalar ? p.w_g : nullptr);
             if (row) prefetch_l2(row + kt * 64);
         }
@@ -230,16 +248,22 @@ __device__ void ec_reduce_and_arrive(const StreamParams& p, int lane, int* par_s
     for (int task = blockIdx.x; task < n_tasks; task += G) {
         const int strip = task % strips, ks = task / strips;
         const int rho0 = strip * 16 + g, rho1 = rho0 + 8;
+        const bool q0 = p.ec_int8 && rho0 < p.r, q1 = p.ec_int8 && rho1 < p.r;      // INT8 factor rows; the gate row w_g stays fp16
+        const int8_t* A8 = reinterpret_cast<const int8_t*>(p.A);
         const __half* pa0 = rho0 < p.r ? p.A + size_t(rho0) * p.K : (rho0 == p.r && scalar ? p.w_g : nullptr);
         const __half* pa1 = rho1 < p.r ? p.A + size_t(rho1) * p.K : (rho1 == p.r && scalar ? p.w_g : nullptr);
+        // per-row scale of the INT8 factors, applied once to the K-reduced partial sum (1 for fp16 rows)
+        const float sa0 = q0 ? __half2float(__ldg(p.A_scale + rho0)) : 1.f, sa1 = q1 ? __half2float(__ldg(p.A_scale + rho1)) : 1.f;
         const int kt_begin = int((long long)ks * ktiles / ksplit);
         const int kt_end = int((long long)(ks + 1) * ktiles / ksplit);
         float acc0[4] = {0.f, 0.f, 0.f, 0.f}, acc1[4] = {0.f, 0.f, 0.f, 0.f};
         for (int kt = kt_begin; kt < kt_end; ++kt) {
             const int col = kt * 64 + 16 * t;
             uint32_t a0l[4], a0h[4], a1l[4], a1h[4], x0l[4], x0h[4], x1l[4], x1h[4];
-            ec_load16(pa0, col, true, a0l, a0h);     // EC factors are parameters: never written by a kernel
-            ec_load16(pa1, col, true, a1l, a1h);
+            if (q0) ec_load16_i8(A8 + size_t(rho0) * p.K, col, a0l, a0h);
+            else ec_load16(pa0, col, true, a0l, a0h);     // EC factors are parameters: never written by a kernel
+            if (q1) ec_load16_i8(A8 + size_t(rho1) * p.K, col, a1l, a1h);
+            else ec_load16(pa1, col, true, a1l, a1h);
             ec_load16(px0, col, false, x0l, x0h);
             ec_load16(px1, col, false, x1l, x1h);
 #pragma unroll
@@ -259,8 +283,9 @@ __device__ void ec_reduce_and_arrive(const StreamParams& p, int lane, int* par_s
             const int rho = (i & 2) ? rho1 : rho0;
             const int tok = 2 * t + (i & 1);
             if (rho < rows_total) {
-                if (tok < p.M) atomicAdd(zpar + tok * kZStride + rho, acc0[i]);
-                if (tok + 8 < p.M) atomicAdd(zpar + (tok + 8) * kZStride + rho, acc1[i]);
+                const float sa = (i & 2) ? sa1 : sa0;
+                if (tok < p.M) atomicAdd(zpar + tok * kZStride + rho, sa * acc0[i]);
+                if (tok + 8 < p.M) atomicAdd(zpar + (tok + 8) * kZStride + rho, sa * acc1[i]);
             }
         }
     }
@@ -362,7 +387,7 @@ stream_kernel(const __grid_constant__ CUtensorMap xmap, const StreamParams p) {
             // warm L2 with the B rows of every panel this CTA may finalise (read only in the epilogue)
             const int p_first = u0 / CP, p_last = (u0 + n_units - 1) / CP;
             const uint8_t* Bb = reinterpret_cast<const uint8_t*>(p.B);
-            const size_t slab = size_t(128) * p.r * 2;
+            const size_t slab = size_t(128) * p.r * (p.ec_int8 ? 1 : 2);
             for (int pnl = p_first; pnl <= p_last; ++pnl)
                 for (size_t off = size_t(lane - 1) * 128; off < slab; off += 31 * 128)
                     prefetch_l2(Bb + size_t(pnl) * slab + off);
@@ -522,15 +547,25 @@ stream_kernel(const __grid_constant__ CUtensorMap xmap, const StreamParams p) {
                 }
                 named_bar_sync(2, 256);
                 const uint4* Brow = reinterpret_cast<const uint4*>(p.B + size_t(n) * p.r);
+                const uint2* Brow8 = reinterpret_cast<const uint2*>(reinterpret_cast<const int8_t*>(p.B) + size_t(n) * p.r);
+                const float sb = p.ec_int8 ? __half2float(__ldg(p.B_scale + n)) : 1.f;     // INT8 factors: per-row scale of B
 #pragma unroll 4
                 for (int j8 = 0; j8 < p.r / 8; ++j8) {
-                    const uint4 bv = __ldg(Brow + j8);
-                    const __half2* bh = reinterpret_cast<const __half2*>(&bv);
+                    uint32_t bw[4];
+                    if (p.ec_int8) {
+                        const uint2 b8 = __ldg(Brow8 + j8);
+                        cvt_i8x4_f16x2(b8.x, bw[0], bw[1]);
+                        cvt_i8x4_f16x2(b8.y, bw[2], bw[3]);
+                    } else {
+                        const uint4 bv = __ldg(Brow + j8);
+                        bw[0] = bv.x; bw[1] = bv.y; bw[2] = bv.z; bw[3] = bv.w;
+                    }
+                    const __half2* bh = reinterpret_cast<const __half2*>(bw);
                     float bf[8];
 #pragma unroll
                     for (int q = 0; q < 4; ++q) {
                         const float2 f = __half22float2(bh[q]);
-                        bf[2 * q] = f.x; bf[2 * q + 1] = f.y;
+                        bf[2 * q] = f.x * sb; bf[2 * q + 1] = f.y * sb;
                     }
 #pragma unroll
                     for (int i = 0; i < 4 * MT; ++i) {

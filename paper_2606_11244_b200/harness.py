@@ -37,10 +37,13 @@ class DeviceLayer:
     b1: Optional[torch.Tensor] = None
     W2: Optional[torch.Tensor] = None
     b2: Optional[torch.Tensor] = None
+    A_scale: Optional[torch.Tensor] = None     # INT8 EC factors: A / B are int8, one fp16 scale per row
+    B_scale: Optional[torch.Tensor] = None
 
     def desc(self, gate_out=None, variant=VARIANT_AUTO) -> EcDesc:
         return make_desc(gate=self.gate if self.r > 0 else "none", alpha=self.alpha, w_g=self.w_g, b_g=self.b_g,
-                         W1=self.W1, b1=self.b1, W2=self.W2, b2=self.b2, gate_out=gate_out, variant=variant)
+                         W1=self.W1, b1=self.b1, W2=self.W2, b2=self.b2, gate_out=gate_out, variant=variant,
+                         A_scale=self.A_scale, B_scale=self.B_scale)
 
 
 def upload_layer(li, device="cuda:0") -> DeviceLayer:
@@ -50,6 +53,8 @@ def upload_layer(li, device="cuda:0") -> DeviceLayer:
     dl = DeviceLayer(pw=pw, M=li.M, N=li.N, K=li.K, r=li.r, group=li.group, gate=li.gate, alpha=li.alpha)
     if li.r > 0:
         dl.A, dl.B = dev(li.A, device), dev(li.B, device)
+        if getattr(li, "A_scale", None) is not None:
+            dl.A_scale, dl.B_scale = dev(li.A_scale, device), dev(li.B_scale, device)
         if li.gate == "scalar":
             dl.w_g = dev(li.w_g, device)
             dl.b_g = torch.tensor([li.b_g], dtype=torch.float32, device=device)

@@ -376,3 +376,35 @@ def test_config2_step_in_the_bench_launch_configuration(sp):
         rms = float(np.sqrt(np.mean(ref ** 2)))
         err = float(np.max(np.abs(y.cpu().numpy().astype(np.float64) - ref)))
         assert err <= Y_TOL * rms, f"config2 {s.name} M={s.M} in the batch: {err:.4g} > {Y_TOL} * {rms:.4g}"
+
+
+# ---------------------------------------------------------------- INT8 EC factors
+
+@pytest.mark.parametrize("idx", [0, 1, 2, 3, 6, 9, 10, 11])
+def test_int8_ec_config2(sp, idx):
+    """configs[1] shapes with the EC factors stored INT8 per-channel symmetric: the GPU reads the int8 codes directly
+    (fused decode kernel) and must match the oracle's spo_forward_q8 within the usual bars."""
+    from workloads import with_int8_ec
+    s = config_shapes(1)[idx]
+    li = with_int8_ec(make_layer(s.seed, s.M, s.N, s.K, s.group, s.r, gate="scalar"))
+    check_layer(li, label=f"int8 EC config2 {s.name} M={s.M}")
+
+
+def test_int8_ec_config1_and_variants(sp):
+    from workloads import with_int8_ec
+    s = config_shapes(0)[0]
+    li = with_int8_ec(make_layer(s.seed, s.M, s.N, s.K, s.group, s.r, gate="scalar"))
+    check_layer(li, variant=1, label="int8 EC config1 fused")
+    check_layer(li, variant=2, label="int8 EC config1 split")
+    lm = with_int8_ec(make_layer(77, 5, 512, 1024, 128, 24, gate="mlp"))
+    check_layer(lm, label="int8 EC, MLP gate (split arm)")
+    ln = with_int8_ec(make_layer(78, 16, 384, 640, 128, 128, gate="none", alpha=0.75))
+    check_layer(ln, label="int8 EC, r = 128, gate none")
+
+
+@pytest.mark.parametrize("M", [40, 300])
+def test_int8_ec_prefill_path(sp, M):
+    """M > 16: the factors are dequantised to an fp16 scratch (one rounding) and take the tcgen05 path."""
+    from workloads import with_int8_ec
+    li = with_int8_ec(make_layer(79 + M, M, 384, 640, 128, 24, gate="scalar"))
+    check_layer(li, label=f"int8 EC M={M}")
