@@ -35,7 +35,7 @@ if ROOT not in sys.path:
 
 import numpy as np
 
-from workloads import algorithmic_bytes, config_shapes, make_layer
+from workloads import algorithmic_bytes, config_shapes, make_layer, with_int8_ec
 from workloads.synth import make_x
 
 METRIC = "W4A16+gated-EC layer: decode HBM GB/s (Llama-3.2-1B decode projections, r=32, M in {1,8,16})"
@@ -59,11 +59,11 @@ def step_shapes():
     return {M: [s for s in shapes if s.M == M] for M in TOKENS}
 
 
-def step_bytes(with_ec=True):
+def step_bytes(with_ec=True, ec_int8=False):
     tot = 0
     for M, ss in step_shapes().items():
         for s in ss:
-            tot += algorithmic_bytes(s.M, s.N, s.K, s.group, s.r if with_ec else 0, "scalar")
+            tot += algorithmic_bytes(s.M, s.N, s.K, s.group, s.r if with_ec else 0, "scalar", ec_int8=ec_int8)
     return tot
 
 
@@ -187,10 +187,12 @@ def run_cuda(args, rank, world):
     shapes = step_shapes()
     # weights / EC factors: one seeded set per projection (the M=16 entry's seed), shared by the three
     # token counts; activations per (M, projection) from that entry's own seed
-    base = {}
+    base, base8 = {}, {}
     for s in shapes[16]:
         li = make_layer(s.seed, 16, s.N, s.K, s.group, s.r, gate="scalar")
         base[s.name] = harness.upload_layer(li, device)
+        l8 = with_int8_ec(li)          # the same EC stored INT8 per-channel symmetric
+        base8[s.name] = tuple(harness.dev(a, device) for a in (l8.A, l8.B, l8.A_scale, l8.B_scale))
     set_bytes = sum(dl.pw.wq.numel() + dl.pw.scales.numel() * 2 + (dl.A.numel() + dl.B.numel() + dl.w_g.numel()) * 2
                     for dl in base.values())
     ncopy = max(3, -(-NCOPY_TARGET_BYTES // set_bytes))
@@ -202,6 +204,9 @@ def run_cuda(args, rank, world):
             pw = sp.PackedW4(dl.pw.wq.clone(), dl.pw.scales.clone(), dl.pw.N, dl.pw.K, dl.pw.group)
             d[name] = harness.DeviceLayer(pw=pw, M=0, N=dl.N, K=dl.K, r=dl.r, group=dl.group, gate="scalar",
                                           alpha=1.0, A=dl.A.clone(), B=dl.B.clone(), w_g=dl.w_g.clone(), b_g=dl.b_g)
+            A8, B8, sA, sB = base8[name]
+            d[name + "/i8"] = harness.DeviceLayer(pw=pw, M=0, N=dl.N, K=dl.K, r=dl.r, group=dl.group, gate="scalar", alpha=1.0,
+                                                  A=A8.clone(), B=B8.clone(), w_g=d[name].w_g, b_g=dl.b_g, A_scale=sA.clone(), B_scale=sB.clone())
         copies.append(d)
     xs, ys, xh, yh = {}, {}, {}, {}
     for M in TOKENS:
@@ -215,7 +220,7 @@ def run_cuda(args, rank, world):
     descs = {}   # keep EcDesc objects alive
     batches = {}
 
-    def one_step(g, with_ec=True, mode="ordered", ec_resident=False):
+    def one_step(g, with_ec=True, mode="ordered", ec_resident=False, ec_int8=False):
         """One pass over the 12 layer calls of the step.  mode: "ordered" = 12 stream-ordered spear_w4_ec_gemm_ex calls, one
         after the other (PDL-chained kernels) -- the regime of SURVEY.md 8(d) and of a real decoder, whose projections
         depend on each other; "lanes" = ONE spear_w4_ec_gemm_batch over the library's concurrent lanes (the 12 calls of
@@ -226,8 +231,8 @@ def run_cuda(args, rank, world):
             cp = copies[(3 * g + mi) % ncopy]
             ecp = copies[0] if ec_resident else cp
             for s in shapes[M]:
-                dl, de = cp[s.name], ecp[s.name]
-                key = (g, mi, s.name, with_ec, ec_resident)
+                dl, de = cp[s.name], ecp[s.name + ("/i8" if ec_int8 else "")]
+                key = (g, mi, s.name, with_ec, ec_resident, ec_int8)
                 if key not in descs:
                     descs[key] = de.desc() if with_ec else sp.make_desc(gate="none")
                 A, B = (de.A, de.B) if with_ec else (None, None)
@@ -236,7 +241,7 @@ def run_cuda(args, rank, world):
                 else:
                     entries.append((xs[(M, s.name)], dl.pw, A, B, descs[key], ys[(M, s.name)]))
         if mode != "ordered":
-            bk = (g, with_ec, ec_resident)
+            bk = (g, with_ec, ec_resident, ec_int8)
             if bk not in batches:
                 batches[bk] = sp.Batch(entries)
             sp.tune("lstream", 1 if mode == "lstream" else 0)
@@ -246,15 +251,15 @@ def run_cuda(args, rank, world):
     stream = torch.cuda.Stream()
     ngraph = ncopy // 3
 
-    def make_graphs(with_ec, mode, ec_resident=False):
+    def make_graphs(with_ec, mode, ec_resident=False, ec_int8=False):
         gs = []
         with torch.cuda.stream(stream):
-            one_step(0, with_ec, mode, ec_resident)  # first-call work (tensor maps, attributes) outside capture
+            one_step(0, with_ec, mode, ec_resident, ec_int8)  # first-call work (tensor maps, attributes) outside capture
             torch.cuda.synchronize()
             for g in range(ngraph):
                 cg = torch.cuda.CUDAGraph()
                 with torch.cuda.graph(cg, stream=stream):
-                    one_step(g, with_ec, mode, ec_resident)
+                    one_step(g, with_ec, mode, ec_resident, ec_int8)
                 gs.append(cg.replay)
         return gs
 
@@ -281,10 +286,10 @@ def run_cuda(args, rank, world):
     b_ec, b_w4 = step_bytes(True), step_bytes(False)
     peak, peak_src = load_peaks()
 
-    def leg(with_ec, mode, ec_resident=False, steps=None):
+    def leg(with_ec, mode, ec_resident=False, steps=None, ec_int8=False):
         steps = steps or args.steps
-        ms = timed(make_graphs(with_ec, mode, ec_resident), steps, args.warmup) / steps
-        by = b_ec if with_ec else b_w4
+        ms = timed(make_graphs(with_ec, mode, ec_resident, ec_int8), steps, args.warmup) / steps
+        by = (step_bytes(True, True) if ec_int8 else b_ec) if with_ec else b_w4
         gbs = aggregate_value(by, ms, world)
         return {"value": round(gbs, 1), "ms_per_step": round(ms, 6), "frac_of_measured_hbm": round(gbs / world / peak, 4),
                 "frac_of_nominal_8tbs": round(gbs / world / NOMINAL_HBM_GBS, 4)}
@@ -297,6 +302,8 @@ def run_cuda(args, rank, world):
     sub = min(args.steps, 500)
     ordered_w4 = leg(False, "ordered")
     ordered_ec_res = leg(True, "ordered", ec_resident=True, steps=sub)
+    ordered_ec_i8 = leg(True, "ordered", steps=sub, ec_int8=True)
+    lanes_ec_i8 = leg(True, "lanes", steps=sub, ec_int8=True)
     lanes_ec, lanes_w4 = leg(True, "lanes", steps=sub), leg(False, "lanes", steps=sub)
     ls_ec, ls_w4 = leg(True, "lstream", steps=sub), leg(False, "lstream", steps=sub)
     t_end = time.time() + 1.0      # keep the GPU under load long enough for nvidia-smi to sample it
@@ -312,7 +319,7 @@ def run_cuda(args, rank, world):
     torch.cuda.synchronize()
 
     def e2e_step(g):
-        bt = batches[(g, True, False)]
+        bt = batches[(g, True, False, False)]
         order = [(M, s.name) for M in TOKENS for s in shapes[M]]
         sp.w4_ec_gemm_batch_hostio(bt, [xh[k] for k in order], [yh[k] for k in order], stream=stream)
 
@@ -348,6 +355,9 @@ def run_cuda(args, rank, world):
         "no_ec": ordered_w4,
         "ec_overhead_time_frac": round(ms_head / ordered_w4["ms_per_step"] - 1.0, 4),
         "ec_l2_resident": dict(ordered_ec_res, ec_overhead_time_frac=round(ordered_ec_res["ms_per_step"] / ordered_w4["ms_per_step"] - 1.0, 4)),
+        "ec_int8": {"note": "the same step with the EC factors stored INT8 per-channel symmetric (PAPER.md:603): bytes_EC halve; cold factors",
+                    "ordered": dict(ordered_ec_i8, ec_overhead_time_frac=round(ordered_ec_i8["ms_per_step"] / ordered_w4["ms_per_step"] - 1.0, 4)),
+                    "lanes": dict(lanes_ec_i8, ec_overhead_time_frac=round(lanes_ec_i8["ms_per_step"] / lanes_w4["ms_per_step"] - 1.0, 4))},
         "overlapped_lanes": {"note": "same step as ONE spear_w4_ec_gemm_batch: the 12 calls are independent problems, the library overlaps "
                                      "them on 12 concurrent lanes (round 1's headline; not a dependent chain)",
                              "ec": lanes_ec, "no_ec": lanes_w4,

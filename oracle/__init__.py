@@ -51,6 +51,8 @@ def lib():
         L.spo_forward.restype = ctypes.c_int
         L.spo_forward.argtypes = [ctypes.c_void_p] * 4 + [ctypes.c_int, ctypes.c_int, ctypes.c_double] + \
             [ctypes.c_void_p] * 5 + [ctypes.c_double] + [ctypes.c_int] * 4 + [ctypes.c_void_p] * 4
+        L.spo_tail.restype = ctypes.c_int
+        L.spo_tail.argtypes = [ctypes.c_void_p] * 3 + [ctypes.c_double, ctypes.c_int, ctypes.c_int, ctypes.c_void_p, ctypes.c_void_p]
         L.spo_forward_q8.restype = ctypes.c_int
         L.spo_forward_q8.argtypes = [ctypes.c_void_p] * 6 + [ctypes.c_int, ctypes.c_int, ctypes.c_double] + \
             [ctypes.c_void_p] * 5 + [ctypes.c_double] + [ctypes.c_int] * 4 + [ctypes.c_void_p] * 4
@@ -181,6 +183,18 @@ def forward_layer(li, rows=None):
     return forward(x, What, li.A, li.B, gate=li.gate, alpha=li.alpha, w_g=li.w_g, b_g=li.b_g,
                    W1=li.W1, b1=li.b1, W2=li.W2, b2=li.b2,
                    A_scale=getattr(li, "A_scale", None), B_scale=getattr(li, "B_scale", None))
+
+
+def tail(y: np.ndarray, residual: np.ndarray, rms_weight: np.ndarray, eps: float):
+    """T1 / T2 (PAPER.md:217): returns (s = residual + y, h = RMSNorm(s) * weight), fp64."""
+    M, N = y.shape
+    y = np.ascontiguousarray(y, dtype=np.float64)
+    s = np.empty((M, N), np.float64)
+    h = np.empty((M, N), np.float64)
+    rc = lib().spo_tail(_p(y), _p(_bits(residual)), _p(_bits(rms_weight)), float(eps), M, N, _p(s), _p(h))
+    if rc:
+        raise ValueError("spo_tail: bad arguments")
+    return s, h
 
 
 def pack_w4(codes: np.ndarray, scales: np.ndarray, group: int):

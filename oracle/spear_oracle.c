@@ -16,6 +16,7 @@
  *              none   gamma = 1                                    Eq. 2, :96
  *   O5  u[m][j]     = gamma[m][j] * z[m][j]                        Eq. 3, :107
  *   O6  y[m][n]     = ybase[m][n] + alpha * sum_j B[n][j] u[m][j]  Eq. 3, :107
+ *   T1, T2  residual add + next-layer RMSNorm of the fused post-EC tail   :217 (spo_tail)
  *   O3', O6'  the same with INT8 per-channel symmetric factors A8*sA, B8*sB   :603 (spo_forward_q8)
  *
  * Everything is fp64, plain left-to-right loops, no blocking, no reordering.
@@ -289,6 +290,34 @@ int spo_forward_q8(const uint16_t *x, const double *What, const int8_t *A8, cons
     int rc = spo_forward_core(x, What, Ad, Bd, gate_kind, h, alpha, W1, b1, W2, b2, w_g, b_g, M, N, K, r, y, ybase, z, gam);
     free(Ad); free(Bd);
     return rc;
+}
+
+/* ---- post-EC tail: residual add + next-layer RMSNorm ------------------------ */
+/*
+ * "residual addition, and next-layer RMSNorm ... as a single fused tail".  Given the layer output y (fp64,
+ * from spo_forward), the residual stream res[M][N] (f16 bits) and the next layer's RMSNorm weight g[N] (f16 bits):
+ *   T1  s[m][n] = res[m][n] + y[m][n]                                  the new residual stream
+ *   T2  h[m][n] = s[m][n] / sqrt( (1/N) sum_n s[m][n]^2 + eps ) * g[n]  RMSNorm (Zhang & Sennrich), eps as given
+ * Plain loops, fp64.
+ */
+int spo_tail(const double *y, const uint16_t *res, const uint16_t *g, double eps, int M, int N,
+             double *s_out, double *h_out)
+{
+    if (M < 0 || N <= 0 || !y || !res || !g) return -1;
+    for (int m = 0; m < M; ++m) {
+        double ssq = 0.0;
+        for (int n = 0; n < N; ++n) {
+            double s = spo_f16_to_f64(res[(size_t)m * N + n]) + y[(size_t)m * N + n];
+            if (s_out) s_out[(size_t)m * N + n] = s;
+            ssq += s * s;
+        }
+        double inv = 1.0 / sqrt(ssq / (double)N + eps);
+        for (int n = 0; n < N; ++n) {
+            double s = spo_f16_to_f64(res[(size_t)m * N + n]) + y[(size_t)m * N + n];
+            if (h_out) h_out[(size_t)m * N + n] = s * inv * spo_f16_to_f64(g[n]);
+        }
+    }
+    return 0;
 }
 
 /* ---- Q1: packed layout, from the layout document ---------------------------------------- */

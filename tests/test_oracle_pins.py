@@ -284,6 +284,36 @@ def test_int8_ec_bruteforce_rational():
             assert abs(out["y"][m][n] - float(y)) <= 1e-12 * max(1.0, abs(float(y)))
 
 
+# ---------------------------------------------------------------- post-EC tail: residual add + RMSNorm
+
+def test_tail_hand_example_and_invariants():
+    # hand example: y = [3, -1, 2, 0.5], residual = [1, 1, -2, 1.5], g = [1, 2, 0.5, 1], eps = 0
+    # s = [4, 0, 0, 2]; mean(s^2) = (16 + 0 + 0 + 4) / 4 = 5; h = s / sqrt(5) * g = [4/sqrt5, 0, 0, 2/sqrt5]
+    y = np.array([[3.0, -1.0, 2.0, 0.5]])
+    s, h = oracle.tail(y, f16([[1.0, 1.0, -2.0, 1.5]]), f16([1.0, 2.0, 0.5, 1.0]), 0.0)
+    assert np.array_equal(s, [[4.0, 0.0, 0.0, 2.0]])
+    np.testing.assert_allclose(h, [[4 / 5 ** 0.5, 0.0, 0.0, 2 / 5 ** 0.5]], rtol=0, atol=1e-15)
+    # eps enters under the root: s = [2, 2], eps = 12 -> h = 2 / sqrt(4 + 12) = 0.5
+    _, h = oracle.tail(np.array([[1.0, 3.0]]), f16([[1.0, -1.0]]), f16([1.0, 1.0]), 12.0)
+    assert np.array_equal(h, [[0.5, 0.5]])
+    # invariants on random data: unit weight and eps = 0 -> mean(h^2) = 1 per token; h is invariant to scaling s;
+    # tokens are independent; numpy cross-check in a vectorised formulation
+    rng = np.random.default_rng(6)
+    y = rng.standard_normal((5, 96)) * 7
+    res = f16(rng.standard_normal((5, 96)))
+    g = f16(rng.uniform(0.5, 1.5, 96))
+    s, h = oracle.tail(y, res, g, 1e-5)
+    s_np = res.astype(np.float64) + y
+    np.testing.assert_allclose(s, s_np, rtol=0, atol=0)
+    np.testing.assert_allclose(h, s_np / np.sqrt((s_np ** 2).mean(axis=1, keepdims=True) + 1e-5) * g.astype(np.float64), rtol=1e-13, atol=1e-13)
+    _, h1 = oracle.tail(y, res, f16(np.ones(96)), 0.0)
+    np.testing.assert_allclose((h1 ** 2).mean(axis=1), 1.0, rtol=1e-12)
+    _, h2 = oracle.tail(4.0 * y, f16(4.0 * res.astype(np.float64)), f16(np.ones(96)), 0.0)
+    np.testing.assert_allclose(h2, h1, rtol=1e-12, atol=1e-12)
+    _, hp = oracle.tail(y[[3, 0]], res[[3, 0]], g, 1e-5)
+    assert np.array_equal(hp, h[[3, 0]])
+
+
 # ---------------------------------------------------------------- P2 reductions to plain W4
 
 def test_P2_zero_A_or_B_or_closed_gate_is_plain_w4():
