@@ -125,6 +125,24 @@ int spear_w4_ec_gemm_ex(const void* x, const void* Wq, const void* scales, const
                         const spear_ec_desc* ec, void* y,
                         int M, int N, int K, int r, int group, void* stream);
 
+/* The layer followed by the rest of the paper's fused post-EC tail ("residual addition, and next-layer
+ * RMSNorm ... as a single fused tail"):
+ *     y[m][n]     = residual[m][n] + (What x + alpha B (gamma (.) A x))[m][n]          the new residual stream, fp16
+ *     h_out[m][n] = y[m][n] / sqrt(mean_n(y[m][:]^2) + eps) * rms_weight[n]            input of the next layer, fp16
+ * Both are formed from the fp32 accumulators (one rounding each; the mean of squares is taken before rounding).  For
+ * M <= 16 on the weight-stream variants this happens inside the layer kernel's epilogue (the row-wide mean needs every
+ * output panel: arrive / wait across the co-resident CTAs of a cooperative launch); the other variants run the layer and a
+ * row kernel.  residual [M][N] fp16 (may alias y), rms_weight [N] fp16, h_out [M][N] fp16 (must not alias y or x). */
+typedef struct {
+    const void* residual;
+    const void* rms_weight;
+    float eps;
+    void* h_out;
+} spear_tail_desc;
+int spear_w4_ec_gemm_tail(const void* x, const void* Wq, const void* scales, const void* A, const void* B,
+                          const spear_ec_desc* ec, const spear_tail_desc* tail, void* y,
+                          int M, int N, int K, int r, int group, void* stream);
+
 /* A batch of layer calls, e.g. the projections of one or several transformer blocks, or unrelated requests.
  * Independent calls run concurrently on the library's internal lanes (up to 16 streams with their own workspaces), or --
  * for M <= 16, when spear_plan_batch measured it faster or spear_tune("lstream", 1) -- as ONE persistent layer-stream

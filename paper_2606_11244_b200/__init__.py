@@ -23,7 +23,7 @@ VARIANT_NAMES = ["auto", "stream_fused", "stream_split", "tc_fused", "tc_split",
 
 EXPORTS = [
     "spear_pack_w4_sizes", "spear_pack_w4", "spear_unpack_w4", "spear_dequant_w4",
-    "spear_w4_ec_gemm", "spear_w4_ec_gemm_ex", "spear_w4_ec_gemm_hostio", "spear_w4_ec_gemm_batch", "spear_w4_ec_gemm_batch_hostio",
+    "spear_w4_ec_gemm", "spear_w4_ec_gemm_ex", "spear_w4_ec_gemm_hostio", "spear_w4_ec_gemm_tail", "spear_w4_ec_gemm_batch", "spear_w4_ec_gemm_batch_hostio",
     "spear_workspace_bytes", "spear_init", "spear_memory_bytes", "spear_plan", "spear_plan_save", "spear_plan_load",
     "spear_plan_query", "spear_plan_batch", "spear_lut_create", "spear_lut_destroy", "spear_lut_iteration_us",
     "spear_slo_chunk", "spear_lut_measure", "spear_tune", "spear_last_error", "spear_launch_count",
@@ -45,6 +45,11 @@ class EcDesc(ctypes.Structure):
         ("workspace", ctypes.c_void_p), ("workspace_bytes", ctypes.c_size_t), ("force_variant", ctypes.c_int),
         ("ec_dtype", ctypes.c_int), ("A_scale", ctypes.c_void_p), ("B_scale", ctypes.c_void_p),
     ]
+
+
+class TailDesc(ctypes.Structure):
+    """struct spear_tail_desc of include/spear.h."""
+    _fields_ = [("residual", ctypes.c_void_p), ("rms_weight", ctypes.c_void_p), ("eps", ctypes.c_float), ("h_out", ctypes.c_void_p)]
 
 
 class Call(ctypes.Structure):
@@ -79,6 +84,7 @@ def lib():
         L.spear_dequant_w4.argtypes = [vp, vp, vp, ci, ci, ci, vp]
         L.spear_w4_ec_gemm.argtypes = [vp] * 8 + [ci] * 5 + [vp]
         L.spear_w4_ec_gemm_ex.argtypes = [vp] * 5 + [ctypes.POINTER(EcDesc), vp] + [ci] * 5 + [vp]
+        L.spear_w4_ec_gemm_tail.argtypes = [vp] * 5 + [ctypes.POINTER(EcDesc), ctypes.POINTER(TailDesc), vp] + [ci] * 5 + [vp]
         L.spear_w4_ec_gemm_batch.argtypes = [ctypes.POINTER(Call), ci, vp]
         L.spear_w4_ec_gemm_batch_hostio.argtypes = [ctypes.POINTER(Call), ctypes.POINTER(HostIO), ci, vp]
         L.spear_w4_ec_gemm_hostio.argtypes = [vp] * 8 + [ctypes.POINTER(EcDesc)] + [ci] * 5 + [vp]
@@ -219,6 +225,24 @@ def w4_ec_gemm_ex(x, pw: PackedW4, A=None, B=None, desc: Optional[EcDesc] = None
     _check(lib().spear_w4_ec_gemm_ex(_ptr(x), _ptr(pw.wq), _ptr(pw.scales), _ptr(A), _ptr(B),
                                      ctypes.byref(desc), _ptr(y), M, pw.N, K, r, pw.group, _stream(stream)))
     return y
+
+
+def w4_ec_gemm_tail(x, pw: PackedW4, A, B, desc: Optional[EcDesc], residual, rms_weight, eps, y=None, h_out=None, stream=None):
+    """spear_w4_ec_gemm_tail: the layer + residual add + next-layer RMSNorm; returns (y, h_out)."""
+    import torch
+    M, K = x.shape
+    r = 0 if A is None else A.shape[0]
+    if desc is None:
+        desc = make_desc(gate="none")
+    if y is None:
+        y = torch.empty((M, pw.N), dtype=torch.float16, device=x.device)
+    if h_out is None:
+        h_out = torch.empty((M, pw.N), dtype=torch.float16, device=x.device)
+    t = TailDesc()
+    t.residual, t.rms_weight, t.eps, t.h_out = _ptr(residual), _ptr(rms_weight), float(eps), _ptr(h_out)
+    _check(lib().spear_w4_ec_gemm_tail(_ptr(x), _ptr(pw.wq), _ptr(pw.scales), _ptr(A), _ptr(B), ctypes.byref(desc), ctypes.byref(t),
+                                       _ptr(y), M, pw.N, K, r, pw.group, _stream(stream)))
+    return y, h_out
 
 
 def w4_ec_gemm_hostio(x_host, y_host, x_dev, y_dev, pw: PackedW4, A=None, B=None,

@@ -339,7 +339,7 @@ static int ws_prepare(uint8_t* ws, size_t ws_bytes, const WsLayout& L, int M, in
 
 static int run_stream(const void* x, const void* Wq, const void* scales, const void* A, const void* B,
                       const spear_ec_desc* ec, void* y, int M, int N, int K, int r, int group,
-                      uint8_t* ws, const WsLayout& L, bool fused, cudaStream_t st) {
+                      uint8_t* ws, const WsLayout& L, bool fused, cudaStream_t st, const spear_tail_desc* tail = nullptr) {
     unsigned* counters = reinterpret_cast<unsigned*>(ws + L.counters);
     float* u32 = reinterpret_cast<float*>(ws + L.u32);
     const bool pdl = g_tune.pdl != 0;
@@ -427,6 +427,14 @@ static int run_stream(const void* x, const void* Wq, const void* scales, const v
         p.zbuf = reinterpret_cast<float*>(ws + L.zfused);
         p.gate_out = static_cast<float*>(ec->gate_out);
         p.ec_sync = counters + kEcPreCounter + 16;
+    }
+    if (tail) {       // fused post-EC tail: state lives in the (zero-kept) counter block
+        p.resid = static_cast<const __half*>(tail->residual);
+        p.rms_w = static_cast<const __half*>(tail->rms_weight);
+        p.h_out = static_cast<__half*>(tail->h_out);
+        p.rms_eps = tail->eps;
+        p.tail_ctr = counters + kEcPreCounter + 32;
+        p.tail_ssq = reinterpret_cast<float*>(counters + kEcPreCounter + 64);
     }
     return launch_stream(xmap, p, MT, grid, pdl, st);
 }
@@ -612,7 +620,7 @@ static int run_lstream(const spear_call* calls, int n_calls, cudaStream_t st) {
 
 static int layer_impl(const void* x, const void* Wq, const void* scales, const void* A, const void* B,
                       const spear_ec_desc* ec, void* y, int M, int N, int K, int r, int group, cudaStream_t st,
-                      void* lane_ws = nullptr, size_t lane_ws_bytes = 0) {
+                      void* lane_ws = nullptr, size_t lane_ws_bytes = 0, const spear_tail_desc* tail = nullptr) {
     if (int rc = spear_init()) return rc;
     if (r == 0) { A = nullptr; B = nullptr; }
     if (int rc = check_problem(x, Wq, scales, A, B, ec, y, M, N, K, r, group)) return rc;
@@ -653,18 +661,22 @@ static int layer_impl(const void* x, const void* Wq, const void* scales, const v
     if (v == SPEAR_VARIANT_LSTREAM) {
         if (ec && ec->workspace) return set_error(SPEAR_EUNSUPPORTED, "the layer-stream variant uses the library's own workspace");
         spear_call c = {x, Wq, scales, A, B, ec, y, M, N, K, r, group};
-        return run_lstream(&c, 1, st);
+        if (int rc = run_lstream(&c, 1, st)) return rc;
+        return tail ? launch_tail_rows(static_cast<__half*>(y), static_cast<const __half*>(tail->residual), static_cast<const __half*>(tail->rms_weight),
+                                       static_cast<__half*>(tail->h_out), tail->eps, M, N, false, st) : SPEAR_OK;
     }
     if (int rc = ws_prepare(ws, ws_bytes, L, M, r, v == SPEAR_VARIANT_TC_FUSED || v == SPEAR_VARIANT_TC_SPLIT, st)) return rc;
     switch (v) {
-        case SPEAR_VARIANT_STREAM_FUSED:
-            return run_stream(x, Wq, scales, A, B, ec, y, M, N, K, r, group, ws, L, true, st);
+        case SPEAR_VARIANT_STREAM_FUSED:       // the weight-stream kernel fuses the tail into its epilogue
+            return run_stream(x, Wq, scales, A, B, ec, y, M, N, K, r, group, ws, L, true, st, tail);
         case SPEAR_VARIANT_STREAM_SPLIT:
-            return run_stream(x, Wq, scales, A, B, ec, y, M, N, K, r, group, ws, L, false, st);
+            return run_stream(x, Wq, scales, A, B, ec, y, M, N, K, r, group, ws, L, false, st, tail);
         case SPEAR_VARIANT_TC_FUSED:
-            return run_tc_fused(x, Wq, scales, A, B, ec, y, M, N, K, r, group, ws, L, false, st);
-        case SPEAR_VARIANT_TC_SPLIT:
-            return run_tc_fused(x, Wq, scales, A, B, ec, y, M, N, K, r, group, ws, L, true, st);
+        case SPEAR_VARIANT_TC_SPLIT: {
+            if (int rc = run_tc_fused(x, Wq, scales, A, B, ec, y, M, N, K, r, group, ws, L, v == SPEAR_VARIANT_TC_SPLIT, st)) return rc;
+            return tail ? launch_tail_rows(static_cast<__half*>(y), static_cast<const __half*>(tail->residual), static_cast<const __half*>(tail->rms_weight),
+                                           static_cast<__half*>(tail->h_out), tail->eps, M, N, g_tune.pdl != 0, st) : SPEAR_OK;
+        }
         default:
             return set_error(SPEAR_EUNSUPPORTED, "variant %d not implemented", v);
     }
@@ -722,6 +734,16 @@ extern "C" int spear_w4_ec_gemm_ex(const void* x, const void* Wq, const void* sc
                                    const spear_ec_desc* ec, void* y, int M, int N, int K, int r, int group,
                                    void* stream) {
     return layer_impl(x, Wq, scales, A, B, ec, y, M, N, K, r, group, static_cast<cudaStream_t>(stream));
+}
+
+extern "C" int spear_w4_ec_gemm_tail(const void* x, const void* Wq, const void* scales, const void* A, const void* B,
+                                     const spear_ec_desc* ec, const spear_tail_desc* tail, void* y,
+                                     int M, int N, int K, int r, int group, void* stream) {
+    if (!tail || !tail->residual || !tail->rms_weight || !tail->h_out) return set_error(SPEAR_EINVAL, "tail needs residual, rms_weight and h_out");
+    if (tail->h_out == y || tail->h_out == x) return set_error(SPEAR_EINVAL, "h_out must not alias y or x");
+    if ((uintptr_t(tail->residual) | uintptr_t(tail->rms_weight) | uintptr_t(tail->h_out)) & 15) return set_error(SPEAR_EINVAL, "tail pointers must be 16-byte aligned");
+    if (!(tail->eps >= 0.f)) return set_error(SPEAR_EINVAL, "eps must be >= 0");
+    return layer_impl(x, Wq, scales, A, B, ec, y, M, N, K, r, group, static_cast<cudaStream_t>(stream), nullptr, 0, tail);
 }
 
 extern "C" int spear_w4_ec_gemm(const void* x, const void* Wq, const void* scales, const void* A, const void* B,

@@ -423,6 +423,56 @@ int launch_ec_dequant_i8(const int8_t* q, const __half* scale, __half* out, int 
     return SPEAR_OK;
 }
 
+// ---- the post-EC tail as a row kernel, for the variants whose layer kernel does not fuse it ----------
+// One CTA per token: y <- residual + y (one more rounding of the layer's output: the fused decode epilogue avoids it),
+// mean of squares over the row from the fp32 sums, h_out <- y * rsqrt(mean + eps) * w.
+__global__ void __launch_bounds__(256) tail_rows_kernel(__half* __restrict__ y, const __half* resid, const __half* __restrict__ w,
+                                                        __half* __restrict__ h_out, float eps, int N) {
+    __shared__ float red[8];
+    __shared__ float inv_s;
+    pdl_launch_dependents();
+    pdl_wait();
+    const size_t base = size_t(blockIdx.x) * N;
+    float ssq = 0.f;
+    for (int n = threadIdx.x * 2; n < N; n += 512) {
+        const float2 a = __half22float2(*reinterpret_cast<const __half2*>(y + base + n));
+        const float2 b = __half22float2(*reinterpret_cast<const __half2*>(resid + base + n));
+        const float s0 = a.x + b.x, s1 = a.y + b.y;
+        ssq += s0 * s0 + s1 * s1;
+        *reinterpret_cast<__half2*>(y + base + n) = __floats2half2_rn(s0, s1);
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) ssq += __shfl_xor_sync(0xffffffffu, ssq, o);
+    if ((threadIdx.x & 31) == 0) red[threadIdx.x >> 5] = ssq;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        float t = 0.f;
+        for (int i = 0; i < 8; ++i) t += red[i];
+        inv_s = rsqrtf(t / float(N) + eps);
+    }
+    __syncthreads();
+    const float inv = inv_s;
+    for (int n = threadIdx.x * 2; n < N; n += 512) {       // the same elements this thread stored above
+        const float2 a = __half22float2(*reinterpret_cast<const __half2*>(y + base + n));
+        const float2 g = __half22float2(*reinterpret_cast<const __half2*>(w + n));
+        *reinterpret_cast<__half2*>(h_out + base + n) = __floats2half2_rn(a.x * inv * g.x, a.y * inv * g.y);
+    }
+}
+int launch_tail_rows(__half* y, const __half* resid, const __half* rms_w, __half* h_out, float eps, int M, int N, bool pdl, cudaStream_t st) {
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3(M);
+    cfg.blockDim = dim3(256);
+    cfg.stream = st;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr[0].val.programmaticStreamSerializationAllowed = pdl ? 1 : 0;
+    cfg.attrs = attr;
+    cfg.numAttrs = 1;
+    SPEAR_CUDA_OK(cudaLaunchKernelEx(&cfg, tail_rows_kernel, y, resid, rms_w, h_out, eps, N));
+    count_launch();
+    return SPEAR_OK;
+}
+
 int launch_ec_update(const __half* u16, const __half* B, __half* y, int M, int N, int r, bool pdl, cudaStream_t st) {
     const size_t smem = size_t(32) * r * 4 + size_t(128) * (r + 2) * 2;
     static std::once_flag attr_once;

@@ -26,6 +26,13 @@ struct StreamParams {
     int CP;                  // (C + 1) / 2 chunk pairs = work units per panel
     int U;                   // (N / 128) * CP work units
     int stages;              // ring depth (stream_stages)
+    // ---- fused tail: y = residual + layer, h_out = RMSNorm(y) * rms_w; NULL resid = off ----
+    const __half* resid;     // [M][N]
+    const __half* rms_w;     // [N]
+    __half* h_out;           // [M][N]
+    float rms_eps;
+    float* tail_ssq;         // [16] fp32 sum of squares per token, zero between calls
+    unsigned* tail_ctr;      // [0] finalised panels, [1] CTAs that left; zero between calls
     // ---- fused EC (SPEAR_VARIANT_STREAM_FUSED): z = x [A; w_g]^T, gate and u are computed by this kernel ----
     int fused;               // 0: u comes from the EC pre-kernel; 1: warp 9 of every CTA produces it
     int gate_kind;           // SPEAR_GATE_SCALAR_SIGMOID or SPEAR_GATE_NONE
@@ -133,6 +140,8 @@ struct EcBigParams {
 };
 int launch_ec_big(const EcBigParams& p, bool pdl, cudaStream_t st);
 // split arm for M > 16: y += u16 . B^T as a separate pass (SPEAR_VARIANT_TC_SPLIT)
+// the tail as a row kernel (variants whose layer kernel does not fuse it): y <- residual + y, h_out <- RMSNorm(y) * w
+int launch_tail_rows(__half* y, const __half* resid, const __half* rms_w, __half* h_out, float eps, int M, int N, bool pdl, cudaStream_t st);
 int launch_ec_update(const __half* u16, const __half* B, __half* y, int M, int N, int r, bool pdl, cudaStream_t st);
 // INT8 EC factors on the M > 16 path: rows * cols int8 codes times one fp16 scale per row -> fp16 scratch
 int launch_ec_dequant_i8(const int8_t* q, const __half* scale, __half* out, int rows, int cols, cudaStream_t st);

@@ -426,6 +426,10 @@ stream_kernel(const __grid_constant__ CUtensorMap xmap, const StreamParams p) {
     const uint32_t x_base = smem_u32(xring);
     bool u_seen = false;
     int it = 0;
+    constexpr int kMaxMine = 128;      // panels one CTA may finalise with the fused tail on (grid >= N / 128 / kMaxMine, checked on the host)
+    __shared__ float tail_s[16];
+    __shared__ int mine[kMaxMine];
+    int n_mine = 0;
     while (it < n_units) {
         const int pnl = (u0 + it) / CP;
         const int seg_begin = it;
@@ -579,15 +583,76 @@ stream_kernel(const __grid_constant__ CUtensorMap xmap, const StreamParams p) {
                     }
                 }
             }
+            if (p.resid) {
+                // fused tail, first half: residual add on the fp32 sums, and this panel's share of the
+                // per-token sum of squares that the next layer's RMSNorm needs (taken before the rounding)
+                if (ct < 16) tail_s[ct] = 0.f;
+                named_bar_sync(2, 256);
+#pragma unroll
+                for (int i = 0; i < 4 * MT; ++i) {
+                    const int tok = (ct >> 7) + 2 * i;
+                    float sq = 0.f;
+                    if (tok < p.M) {
+                        val[i] += __half2float(p.resid[size_t(tok) * p.N + n]);
+                        sq = val[i] * val[i];
+                    }
+#pragma unroll
+                    for (int o = 16; o > 0; o >>= 1) sq += __shfl_xor_sync(0xffffffffu, sq, o);
+                    if (lane == 0 && tok < p.M) atomicAdd(&tail_s[tok], sq);
+                }
+                named_bar_sync(2, 256);
+                if (ct < p.M) atomicAdd(p.tail_ssq + ct, tail_s[ct]);
+                if (ct == 0 && n_mine < kMaxMine) mine[n_mine] = pnl;
+                ++n_mine;       // (every thread counts; only ct == 0 writes the list)
+            }
             // S8: one RN-even cast, coalesced store of 128 consecutive n per token
 #pragma unroll
             for (int i = 0; i < 4 * MT; ++i) {
                 const int tok = (ct >> 7) + 2 * i;
                 if (tok < p.M) p.y[size_t(tok) * p.N + n] = __float2half_rn(val[i]);
             }
+            if (p.resid) {
+                named_bar_sync(2, 256);      // the panel's y stores and ssq adds are issued
+                if (ct == 0) { __threadfence(); atomicAdd(p.tail_ctr, 1u); }
+            }
         }
         named_bar_sync(1, 256);     // red[] and flag are reused by the next segment
         it = seg_end;
+    }
+    if (p.resid) {
+        // fused tail, second half: once every panel of the layer has contributed (all CTAs are co-resident: cooperative
+        // launch), normalise the panels this CTA finalised.  y is re-read as stored (fp16).
+        if (n_mine > 0) {
+            if (ct == 0) {
+                unsigned f;
+                do { asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(f) : "l"(p.tail_ctr) : "memory"); } while (f < unsigned(p.N >> 7));
+            }
+            named_bar_sync(2, 256);
+            if (ct < 16) tail_s[ct] = ct < p.M ? rsqrtf(__ldcg(p.tail_ssq + ct) / float(p.N) + p.rms_eps) : 0.f;
+            named_bar_sync(2, 256);
+            const int row = ct & 127;
+            for (int q = 0; q < min(n_mine, kMaxMine); ++q) {
+                const int n = mine[q] * 128 + row;
+                const float gw = __half2float(__ldg(p.rms_w + n));
+#pragma unroll
+                for (int i = 0; i < 4 * MT; ++i) {
+                    const int tok = (ct >> 7) + 2 * i;
+                    if (tok < p.M) {
+                        const float yv = __half2float(__ldcg(p.y + size_t(tok) * p.N + n));
+                        p.h_out[size_t(tok) * p.N + n] = __float2half_rn(yv * tail_s[tok] * gw);
+                    }
+                }
+            }
+        }
+        named_bar_sync(2, 256);
+        if (ct == 0) {      // the last CTA to leave resets the tail state for the next call
+            __threadfence();
+            if (atomicAdd(p.tail_ctr + 1, 1u) == gridDim.x - 1) {
+                for (int m = 0; m < 16; ++m) p.tail_ssq[m] = 0.f;
+                p.tail_ctr[0] = 0;
+                p.tail_ctr[1] = 0;
+            }
+        }
     }
 }
 
@@ -641,8 +706,8 @@ int launch_stream(const CUtensorMap& xmap, const StreamParams& p, int MT, int gr
     attr[0].val.programmaticStreamSerializationAllowed = pdl ? 1 : 0;
     cfg.attrs = attr;
     cfg.numAttrs = 1;
-    if (p.fused && p.r > 0) {
-        // the fused EC waits device-wide for its own grid: a cooperative launch makes the co-residency of all CTAs a
+    if ((p.fused && p.r > 0) || p.resid) {
+        // the fused EC (and the fused tail's row-wide mean) wait device-wide for their own grid: a cooperative launch makes the co-residency of all CTAs a
         // guarantee of the driver instead of an assumption about dispatch order (other lanes, other tenants of the GPU)
         attr[1].id = cudaLaunchAttributeCooperative;
         attr[1].val.cooperative = 1;

@@ -34,9 +34,11 @@ def test_header_symbols_all_exported(spear):
 
 
 def test_ec_desc_layout_matches_header(spear):
-    # 2 ints + float + pad, 7 pointers, void* + size_t, int + pad
-    assert ctypes.sizeof(spear.EcDesc) == 16 + 7 * 8 + 16 + 8
+    # 2 ints + float + pad, 7 pointers, void* + size_t, 2 ints (force_variant, ec_dtype), 2 pointers (INT8 EC scales)
+    assert ctypes.sizeof(spear.EcDesc) == 16 + 7 * 8 + 16 + 8 + 16
     assert spear.EcDesc.W1.offset == 16 and spear.EcDesc.force_variant.offset == 88
+    assert spear.EcDesc.ec_dtype.offset == 92 and spear.EcDesc.A_scale.offset == 96 and spear.EcDesc.B_scale.offset == 104
+    assert ctypes.sizeof(spear.TailDesc) == 32 and spear.TailDesc.h_out.offset == 24
 
 
 def test_sizes_and_shape_errors_need_no_gpu(spear):

@@ -408,3 +408,60 @@ def test_int8_ec_prefill_path(sp, M):
     from workloads import with_int8_ec
     li = with_int8_ec(make_layer(79 + M, M, 384, 640, 128, 24, gate="scalar"))
     check_layer(li, label=f"int8 EC M={M}")
+
+
+# ---------------------------------------------------------------- fused post-EC tail
+
+def check_tail(li, variant=0, rows=None, label=""):
+    """Layer + residual add + next-layer RMSNorm against the oracle (spo_forward + spo_tail)."""
+    import torch
+    import paper_2606_11244_b200 as sp
+    h = _harness()
+    rng = np.random.default_rng(li.seed + 99)
+    res = (rng.standard_normal((li.M, li.N)) * 4.0).astype(np.float16)
+    gw = rng.uniform(0.5, 1.5, li.N).astype(np.float16)
+    eps = 1e-5
+    dl = h.upload_layer(li)
+    y, hn = sp.w4_ec_gemm_tail(h.dev(li.x), dl.pw, dl.A, dl.B, dl.desc(variant=variant), h.dev(res), h.dev(gw), eps)
+    torch.cuda.synchronize()
+    ref = oracle.forward_layer(li)
+    s_ref, h_ref = oracle.tail(ref["y"], res, gw, eps)
+    for name, got, want in (("residual stream", y, s_ref), ("rmsnorm", hn, h_ref)):
+        g64 = got.cpu().numpy().astype(np.float64)
+        rms = float(np.sqrt(np.mean(want ** 2)))
+        err = float(np.max(np.abs(g64 - want)))
+        assert err <= Y_TOL * rms, f"{label} {name}: max err {err:.4g} > {Y_TOL} * rms {rms:.4g}"
+
+
+@pytest.mark.parametrize("idx", [0, 2, 3, 5, 7, 8, 10, 11])
+def test_fused_tail_config2(sp, idx):
+    s = config_shapes(1)[idx]
+    check_tail(make_layer(s.seed, s.M, s.N, s.K, s.group, s.r, gate="scalar"), label=f"tail config2 {s.name} M={s.M}")
+
+
+def test_fused_tail_variants_and_back_to_back(sp):
+    li = make_layer(300, 7, 1024, 768, 128, 16, gate="scalar")
+    for v in (1, 2, 5, 3):          # fused in the decode epilogue (1, 2); layer + row kernel (layer-stream, tcgen05)
+        check_tail(li, variant=v, label=f"tail variant {v}")
+        check_tail(li, variant=v, label=f"tail variant {v} again")       # the tail state must come back clean
+    check_tail(make_layer(301, 3, 256, 256, 128, 0), label="tail r=0")
+    check_tail(make_layer(302, 16, 128 * 19, 256, 128, 8, gate="mlp"), label="tail mlp, more panels than CTAs have units")
+    check_tail(make_layer(303, 100, 384, 640, 128, 8, gate="scalar"), label="tail M=100 (tcgen05 + row kernel)")
+
+
+def test_fused_tail_in_place_residual(sp):
+    """The residual stream may be updated in place (residual == y)."""
+    import torch
+    import paper_2606_11244_b200 as sp_
+    h = _harness()
+    li = make_layer(304, 5, 512, 512, 128, 8, gate="scalar")
+    rng = np.random.default_rng(1)
+    res = (rng.standard_normal((5, 512)) * 3).astype(np.float16)
+    gw = np.ones(512, np.float16)
+    dl = h.upload_layer(li)
+    stream = h.dev(res)
+    y, hn = sp_.w4_ec_gemm_tail(h.dev(li.x), dl.pw, dl.A, dl.B, dl.desc(), stream, h.dev(gw), 1e-5, y=stream)
+    torch.cuda.synchronize()
+    s_ref, h_ref = oracle.tail(oracle.forward_layer(li)["y"], res, gw, 1e-5)
+    assert float(np.max(np.abs(y.cpu().numpy().astype(np.float64) - s_ref))) <= Y_TOL * float(np.sqrt(np.mean(s_ref ** 2)))
+    assert float(np.max(np.abs(hn.cpu().numpy().astype(np.float64) - h_ref))) <= Y_TOL * float(np.sqrt(np.mean(h_ref ** 2)))
