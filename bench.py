@@ -436,9 +436,7 @@ def configs_table(sp, device):
 
     stream = torch.cuda.Stream()
 
-    def steady_us(M, arena, n_calls, plain=False, reps=5):
-        """Steady state (SURVEY.md 8(d) regime 1): a CUDA graph of n_calls back-to-back stream-ordered calls cycling through
-        the arena (>= 512 MB of weights unless the layer alone exceeds L2); microseconds per call, median of `reps` replays."""
+    def steady_graph(M, arena, n_calls, plain):
         K, N = arena[0]["pw"].K, arena[0]["pw"].N
         x = torch.randn(M, K, device=device, generator=gen).half()
         y = torch.empty(M, N, dtype=torch.float16, device=device)
@@ -457,15 +455,30 @@ def configs_table(sp, device):
                 body()
             g.replay()
             torch.cuda.synchronize()
-            ts = []
+        return g, (x, y, ds)
+
+    def time_graphs(graphs, n_calls, reps):
+        """Medians (us per call) of `reps` replays of each graph, the graphs taken in turn (same clock / power state)."""
+        ts = [[] for _ in graphs]
+        with torch.cuda.stream(stream):
             for _ in range(reps):
-                e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-                e0.record(stream)
-                g.replay()
-                e1.record(stream)
-                e1.synchronize()
-                ts.append(e0.elapsed_time(e1) * 1e3 / n_calls)
-        return sorted(ts)[len(ts) // 2]
+                for gi, (g, _) in enumerate(graphs):
+                    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                    e0.record(stream)
+                    g.replay()
+                    e1.record(stream)
+                    e1.synchronize()
+                    ts[gi].append(e0.elapsed_time(e1) * 1e3 / n_calls)
+        return [sorted(t)[len(t) // 2] for t in ts]
+
+    def steady_us(M, arena, n_calls, plain=False, reps=5):
+        """Steady state (SURVEY.md 8(d) regime 1): a CUDA graph of n_calls back-to-back stream-ordered calls cycling through
+        the arena (>= 512 MB of weights unless the layer alone exceeds L2); microseconds per call, median of `reps` replays."""
+        return time_graphs([steady_graph(M, arena, n_calls, plain)], n_calls, reps)[0]
+
+    def steady_pair_us(M, arena, n_calls, reps=5):
+        """(plain, with EC) on the same arena, replays interleaved."""
+        return time_graphs([steady_graph(M, arena, n_calls, True), steady_graph(M, arena, n_calls, False)], n_calls, reps)
 
     def row(name, M, N, K, group, r, us, gate="scalar", extra=None):
         by = algorithmic_bytes(M, N, K, group, r, gate, 4 * r if gate == "mlp" else 0)
@@ -496,10 +509,12 @@ def configs_table(sp, device):
                 layers[key] = rand_layer(s.N, s.K, s.group, s.r, gate)
             L = layers[key]
             arena, n_calls = arena_for(L, s.M)
-            us0 = steady_us(s.M, arena, n_calls, plain=True)
+            if s.r:
+                us0, us1 = steady_pair_us(s.M, arena, n_calls)
+            else:
+                us0 = steady_us(s.M, arena, n_calls, plain=True)
             rows.append(row(s.name, s.M, s.N, s.K, s.group, 0, us0))
             if s.r:
-                us1 = steady_us(s.M, arena, n_calls)
                 rows.append(row(s.name, s.M, s.N, s.K, s.group, s.r, us1, gate, {"ec_overhead_time_frac": round(us1 / us0 - 1.0, 4)}))
             del arena
         return rows
@@ -512,8 +527,8 @@ def configs_table(sp, device):
     table["config2"] = sweep(config_shapes(1))
     table["config3"] = sweep(config_shapes(2))
     # config 4: one weight arena per r, all three token counts.  The EC overhead of a row is taken against the plain layer
-    # timed on the SAME arena right before it (the part power-caps under these GEMMs: rows measured minutes apart do not
-    # share a clock state)
+    # timed on the SAME arena with interleaved replays (the part power-caps under these GEMMs: rows measured seconds apart
+    # do not share a clock state)
     rows4 = []
     s0 = config_shapes(3)[0]
     for r in (0, 16, 64, 128):
@@ -521,12 +536,12 @@ def configs_table(sp, device):
         L = rand_layer(s0.N, s0.K, s0.group, r)
         arena = clones(L, 5)
         for M in (512, 4096, 16384):
-            reps = 3 if M == 16384 else 5
-            us0 = steady_us(M, arena, 5, plain=True, reps=reps)
+            reps = 3 if M == 16384 else 7
             if r == 0:
+                us0 = steady_us(M, arena, 5, plain=True, reps=reps)
                 rows4.append(row("mlp70b", M, s0.N, s0.K, s0.group, 0, us0))
             else:
-                us1 = steady_us(M, arena, 5, reps=reps)
+                us0, us1 = steady_pair_us(M, arena, 5, reps=reps)
                 rows4.append(row("mlp70b", M, s0.N, s0.K, s0.group, r, us1, "scalar",
                                  {"ec_overhead_time_frac": round(us1 / us0 - 1.0, 4), "plain_us_same_arena": round(us0, 2)}))
         del arena, L
@@ -534,6 +549,7 @@ def configs_table(sp, device):
     torch.cuda.empty_cache()
     table["mlp_gate_cost"] = mlp_gate_rows(sp, rand_layer, arena_for, steady_us, row)
     table["single_cold_launch"] = cold_launch_rows(sp, device, rand_layer, desc_of, row, gen)
+    table["fused_tail"] = tail_rows(sp, device, rand_layer, desc_of, clones, gen)
     torch.cuda.empty_cache()
     table["config5"] = stack_rows(sp, device, rand_layer, desc_of, gen, hbm, tpk)
     return table
@@ -550,6 +566,55 @@ def mlp_gate_rows(sp, rand_layer, arena_for, steady_us, row):
             arena, n_calls = arena_for(L, M)
             out.append(row(name, M, N, K, group, r, steady_us(M, arena, n_calls), gate))
             del arena, L
+    return out
+
+
+def tail_rows(sp, device, rand_layer, desc_of, clones, gen):
+    """the layer with the residual add + next-layer RMSNorm fused into its epilogue (spear_w4_ec_gemm_tail) against
+    the layer alone, on the two projections of configs[1] that write the residual stream (o, down), M = 8, steady state."""
+    import torch
+    out = []
+    stream = torch.cuda.Stream()
+    for (name, N, K) in (("o", 2048, 2048), ("down", 2048, 8192)):
+        M, r = 8, 32
+        L = rand_layer(N, K, 128, r)
+        arena = clones(L, max(2, -(-(512 << 20) // (N * K // 2))))
+        x = torch.randn(M, K, device=device, generator=gen).half()
+        y = torch.empty(M, N, dtype=torch.float16, device=device)
+        res = torch.randn(M, N, device=device, generator=gen).half()
+        gw = torch.ones(N, dtype=torch.float16, device=device)
+        hn = torch.empty(M, N, dtype=torch.float16, device=device)
+        ds = [desc_of(C) for C in arena]
+        us = {}
+        for mode in ("layer", "layer+tail"):
+            def body():
+                for i in range(64):
+                    C = arena[i % len(arena)]
+                    if mode == "layer":
+                        sp.w4_ec_gemm_ex(x, C["pw"], C["A"], C["B"], ds[i % len(arena)], y=y)
+                    else:
+                        sp.w4_ec_gemm_tail(x, C["pw"], C["A"], C["B"], ds[i % len(arena)], res, gw, 1e-5, y=y, h_out=hn)
+            with torch.cuda.stream(stream):
+                body()
+                torch.cuda.synchronize()
+                g = torch.cuda.CUDAGraph()
+                with torch.cuda.graph(g, stream=stream):
+                    body()
+                g.replay()
+                torch.cuda.synchronize()
+                ts = []
+                for _ in range(5):
+                    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                    e0.record(stream)
+                    g.replay()
+                    e1.record(stream)
+                    e1.synchronize()
+                    ts.append(e0.elapsed_time(e1) * 1e3 / 64)
+            us[mode] = sorted(ts)[2]
+        out.append({"name": f"config2 {name}", "M": M, "N": N, "K": K, "r": r, "us_layer": round(us["layer"], 2),
+                    "us_layer_plus_fused_tail": round(us["layer+tail"], 2),
+                    "tail_overhead_time_frac": round(us["layer+tail"] / us["layer"] - 1.0, 4)})
+        del arena, L
     return out
 
 
