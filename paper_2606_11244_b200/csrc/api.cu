@@ -398,8 +398,14 @@ static int run_stream(const void* x, const void* Wq, const void* scales, const v
     (void)units_per_cta;
     if (g_tune.stream_deep >= 0) deep = g_tune.stream_deep != 0;
     if (deep) per_sm = 1;
-    p.stages = stream_stages(MT, deep);
-    per_sm = std::min(per_sm, stream_resident_ctas(MT, deep));      // what really fits (occupancy query), not an assumption
+    p.deep = deep ? 1 : 0;
+    p.stages = stream_fit_stages(MT, deep, r);
+    if (r > 0) {      // the panel's B slab rides in the ring: one item of <= 16 KiB, or two
+        const int slab = 128 * r * (p.ec_int8 ? 1 : 2);
+        p.b_slots = slab > 16384 ? 2 : 1;
+        p.b_slot_bytes = slab / p.b_slots;
+    }
+    per_sm = std::min(per_sm, stream_resident_ctas(MT, deep, r));      // what really fits (occupancy query), not an assumption
     int grid = std::min(p.U, g_dev.num_sms * per_sm);
     grid = std::min(grid, kMaxStreamGrid);
     // When the panels nearly fill the machine, give every CTA whole panels: an even stream-K split would cut almost

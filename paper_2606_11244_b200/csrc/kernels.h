@@ -25,7 +25,10 @@ struct StreamParams {
     int C;                   // K / 128 chunks per panel
     int CP;                  // (C + 1) / 2 chunk pairs = work units per panel
     int U;                   // (N / 128) * CP work units
-    int stages;              // ring depth (stream_stages)
+    int stages;              // ring depth (stream_stages, minus what the u buffer needs: stream_fit_stages)
+    int deep;                // 1: the one-CTA-per-SM instance (deep ring), 0: the two-CTA instance
+    int b_slots;             // r > 0: ring items that carry one panel's B slab (1, or 2 when 128 r elements exceed 16 KiB)
+    int b_slot_bytes;        // bytes of one such item (128 r esize / b_slots)
     // ---- fused tail: y = residual + layer, h_out = RMSNorm(y) * rms_w; NULL resid = off ----
     const __half* resid;     // [M][N]
     const __half* rms_w;     // [N]
@@ -46,8 +49,9 @@ struct StreamParams {
     unsigned* ec_sync;       // [0] epoch (bumped once per fused launch), [1], [2] arrival counters of buffer 0 / 1
 };
 int stream_stages(int MT, bool deep);
-int stream_smem_bytes(int MT, int stages);
-int stream_resident_ctas(int MT, bool deep);
+int stream_smem_bytes(int MT, int stages, int r);
+int stream_fit_stages(int MT, bool deep, int r);          // deepest ring <= stream_stages whose CTA (ring + u buffer) fits
+int stream_resident_ctas(int MT, bool deep, int r);
 int launch_stream(const CUtensorMap& xmap, const StreamParams& p, int MT, int grid, bool pdl, cudaStream_t st);
 
 // ---- lstream.cu (M <= 16): persistent "layer stream" -- ONE cooperative launch consumes a table of layer

@@ -19,13 +19,17 @@
 //     the previous kernel): under programmatic dependent launch the ring of layer i+1 fills while layer i
 //     drains.  After the wait the same lane adds one 3-D TMA tensor copy per unit for the x tile (8*MT tokens x
 //     4 k-tiles x 64 columns, 128-byte swizzle, zero-filled beyond M and K);
-//   * warp 9 (fused variant only): reduces this CTA's share of z = x [A; w_g]^T and arrives (see below);
+//   * warp 9 (r > 0): fused variant: reduces this CTA's share of z = x [A; w_g]^T and arrives; in the CTAs that
+//     finalise a panel it then stages u = alpha gamma (.) z in shared memory (split variant: copies the pre-kernel's u);
 //   * 8 consumer warps, all on the same unit: warp (h, kq) takes strips 4h..4h+3 (64 rows) x k-tile kq
 //     (64 columns): 4 LDS.128 of int4, lop3/sub dequantisation in registers, mma.sync.m16n8k16 with the
 //     tokens as the n=8 operand (fp32 accumulate), group scale applied to the fp32 accumulator;
 //   * per panel segment the 8 warps reduce through shared memory; a CTA that owns a whole panel writes y
-//     directly, otherwise it parks an fp32 partial in the workspace and the last arriver (atomic counter
-//     per panel) sums the partials in CTA order, adds the EC term and casts once.
+//     directly, otherwise the parts meet through fp32 slots in the workspace and a counter per panel.  Plain layer: the
+//     last arriver sums them in CTA order (nobody waits).  With an EC: the CTA that owns the panel's FIRST unit
+//     finalises -- the ring brings the panel's B slab (128 x r, <= 2 items of 16 KiB) to it right behind that
+//     segment's weights, and the same 8 warps add B u^T as r / 16 extra mma.sync k-steps (u split into an fp16 head
+//     and remainder) before the single cast: S7 costs one ring item per panel instead of a scalar epilogue.
 #include <mutex>
 
 #include "common.cuh"
@@ -69,6 +73,10 @@ __device__ __forceinline__ unsigned arrive_acq_rel(unsigned* ctr) {
     asm volatile("atom.add.acq_rel.gpu.global.u32 %0, [%1], 1;" : "=r"(old) : "l"(ctr) : "memory");
     return old;
 }
+// ... and the same arrive when nobody needs the count it returns: fire and forget, the issuing thread does not wait
+__device__ __forceinline__ void arrive_release(unsigned* ctr) {
+    asm volatile("red.release.gpu.global.add.u32 [%0], 1;" :: "l"(ctr) : "memory");
+}
 
 // ---- the consumer inner loop -------------------------------------------------------------------------
 // Explicit shared-window loads (32-bit addresses; the generic-pointer form compiles to LD.E + 64-bit math).
@@ -93,6 +101,53 @@ __device__ __forceinline__ void biased_word(uint32_t w, uint32_t (&out)[4]) {
     const uint32_t w8 = w >> 8;
     asm("lop3.b32 %0, %1, 0x000f000f, %2, 0xea;" : "=r"(out[2]) : "r"(w8), "r"(kMagic));
     asm("lop3.b32 %0, %1, 0x00f000f0, %2, 0xea;" : "=r"(out[3]) : "r"(w8), "r"(kMagic));
+}
+
+__device__ __forceinline__ uint32_t lds16(uint32_t addr) {
+    uint32_t v;
+    asm volatile("ld.shared.u16 %0, [%1];" : "=r"(v) : "r"(addr));
+    return v;
+}
+__device__ __forceinline__ uint32_t pack_half2(float lo, float hi) {
+    const __half2 h = __floats2half2_rn(lo, hi);
+    return *reinterpret_cast<const uint32_t*>(&h);
+}
+
+// S7 on the tensor cores (the B (gamma (.) A x) term of Eq. 3): one 16-row strip of the panel's B slab
+// (fp16 [row][r], or int8 [row][r]; b_addr = the strip's first row in the ring slot) times u^T, into acc.
+//   A operand = the strip (rows g / g + 8, k = 16 ks + 2t.. and + 8), B operand = u[token][k] split into an fp16 head
+//   and an fp16 remainder (two mma per k-step: u keeps ~22 bits, the products are exact, fp32 accumulate).
+// r % 16 == 8: the upper half of the last k-step is absent and fed as zeros on both operands.
+template <int MT>
+__device__ __forceinline__ void ec_up(uint32_t b_addr, int r, bool int8, const float* us, int lane, float (&acc)[MT][4]) {
+    const int g = lane >> 2, t = lane & 3;
+    for (int k0 = 2 * t; k0 < r; k0 += 16) {
+        const bool up = k0 + 8 < r;
+        uint32_t a0, a1, a2, a3;
+        if (!int8) {
+            a0 = lds32(b_addr + (g * r + k0) * 2);
+            a1 = lds32(b_addr + ((g + 8) * r + k0) * 2);
+            a2 = up ? lds32(b_addr + (g * r + k0 + 8) * 2) : 0u;
+            a3 = up ? lds32(b_addr + ((g + 8) * r + k0 + 8) * 2) : 0u;
+        } else {
+            const uint32_t w0 = lds16(b_addr + g * r + k0) | (up ? lds16(b_addr + g * r + k0 + 8) << 16 : 0u);
+            const uint32_t w1 = lds16(b_addr + (g + 8) * r + k0) | (up ? lds16(b_addr + (g + 8) * r + k0 + 8) << 16 : 0u);
+            cvt_i8x4_f16x2(w0, a0, a2);
+            cvt_i8x4_f16x2(w1, a1, a3);
+        }
+#pragma unroll
+        for (int mt = 0; mt < MT; ++mt) {
+            const float* up_ = us + (mt * 8 + g) * r + k0;
+            const float2 u0 = *reinterpret_cast<const float2*>(up_);
+            const float2 u1 = up ? *reinterpret_cast<const float2*>(up_ + 8) : make_float2(0.f, 0.f);
+            const __half2 h0 = __floats2half2_rn(u0.x, u0.y), h1 = __floats2half2_rn(u1.x, u1.y);
+            const float2 f0 = __half22float2(h0), f1 = __half22float2(h1);
+            const uint32_t hi0 = *reinterpret_cast<const uint32_t*>(&h0), hi1 = *reinterpret_cast<const uint32_t*>(&h1);
+            const uint32_t lo0 = pack_half2(u0.x - f0.x, u0.y - f0.y), lo1 = pack_half2(u1.x - f1.x, u1.y - f1.y);
+            mma_m16n8k16(acc[mt], a0, a1, a2, a3, hi0, hi1);
+            mma_m16n8k16(acc[mt], a0, a1, a2, a3, lo0, lo1);
+        }
+    }
 }
 
 // One (4 strips = 64 rows) x (64 columns) task of a warp.  w_addr: this lane's first 16 bytes of the
@@ -158,16 +213,17 @@ __device__ __forceinline__ void stream_task(uint32_t w_addr, uint32_t x_addr, ui
 
 // ---- fused EC (warp 9): S4-S6 of SURVEY.md 8(a) inside the weight-stream kernel ---------------------
 // Every CTA reduces one (16-row strip of [A; w_g]) x (K slice) piece of z = x [A; w_g]^T with mma.sync,
-// adds it to the global fp32 z with red.add and ARRIVES on a device-wide counter right away; nobody waits
-// there.  A CTA that finalises a panel looks at the counter only in its epilogue, long after everybody has
-// arrived (arrive early / wait late), then reads the complete z (z must be complete before the gate,
-// PAPER.md:199-211), applies the gate (PAPER.md:107-109 / BASELINE.json scalar gate) and forms
-// u = alpha * gamma (.) z in shared memory.  z and the counter are double-buffered by the parity of an epoch
-// word that the last arriver bumps: launch n uses buffer n & 1 and CTA 0 re-zeroes the other buffer for launch
-// n + 1 (its previous user, launch n - 1, is complete once griddepcontrol.wait returns), so nothing has to be
-// cleaned on the critical path.  All CTAs of the grid are co-resident (grid <= SMs x resident CTAs), so the
-// late wait cannot deadlock: fused launches are COOPERATIVE launches (launch_stream), so the driver starts the grid
-// only when all of its CTAs fit at once, whatever else runs on the device.
+// adds it to the global fp32 z with red.add and ARRIVES on a device-wide counter (red.release, fire and forget).
+// Only warp 9 of the CTAs that FINALISE a panel goes on: it waits until the counter shows every CTA of the grid,
+// reads the complete z (z must be complete before the gate), applies the gate (PAPER.md:107-109 /
+// BASELINE.json scalar gate) and stages u = alpha * gamma (.) z in shared memory -- all of it beside the consumers'
+// main loop, which meets u on a shared-memory barrier when it reaches the panel's B slab (S7, see the kernel).
+// z and the counter are double-buffered by the parity of an epoch word: launch n uses buffer n & 1, CTA 0
+// re-zeroes the other buffer for launch n + 1 (its previous user, launch n - 1, is complete once
+// griddepcontrol.wait returns) and bumps the epoch once everybody has arrived, so nothing has to be cleaned on
+// the critical path.  All CTAs of the grid are co-resident (grid <= SMs x resident CTAs) and launches with an EC are
+// COOPERATIVE launches (launch_stream): the driver starts the grid only when all of its CTAs fit at once, whatever
+// else runs on the device, so the waits (this one, and a panel's head CTA for the panel's other parts) cannot deadlock.
 __device__ __forceinline__ void ec_load16(const __half* row, int col, bool readonly, uint32_t (&lo)[4], uint32_t (&hi)[4]) {
     if (row) {
         uint4 a, b;
@@ -229,7 +285,7 @@ __device__ void ec_prefetch_factors(const StreamParams& p, int lane) {
 
 // Phase A (whole warp, after griddepcontrol.wait): this CTA's piece of z, red.add, arrive.  Returns true in
 // the last CTA to arrive.
-__device__ void ec_reduce_and_arrive(const StreamParams& p, int lane, int* par_smem, uint64_t* e_ready) {
+__device__ unsigned ec_reduce_and_arrive(const StreamParams& p, int lane) {
     const int g = lane >> 2, t = lane & 3;
     const bool scalar = (p.gate_kind == SPEAR_GATE_SCALAR_SIGMOID);
     const int rows_total = p.r + (scalar ? 1 : 0);
@@ -274,7 +330,6 @@ __device__ void ec_reduce_and_arrive(const StreamParams& p, int lane, int* par_s
         }
         if (!announced) {
             zpar = p.zbuf + (epoch & 1u) * (16 * kZStride);
-            if (lane == 0) { *par_smem = int(epoch & 1u); mbar_arrive(e_ready); }
             announced = true;
         }
         // C fragment: rows rho0 / rho1 of [A; w_g], tokens 2t, 2t+1 (acc0) and 8+2t, 9+2t (acc1)
@@ -290,18 +345,64 @@ __device__ void ec_reduce_and_arrive(const StreamParams& p, int lane, int* par_s
         }
     }
     const unsigned par = epoch & 1u;
-    if (!announced && lane == 0) { *par_smem = int(par); mbar_arrive(e_ready); }
+    __syncwarp();
+    if (lane == 0) arrive_release(p.ec_sync + 1 + par);     // (CTA 0 bumps the epoch once it has seen everybody: ec_stage_u)
     if (blockIdx.x == 0) {
-        // prepare the other buffer for the next fused launch on this workspace
+        // prepare the other buffer for the next fused launch on this workspace (after the arrive: everybody waits for it)
         float* zo = p.zbuf + (par ^ 1u) * (16 * kZStride);
         for (int i = lane; i < 16 * kZStride; i += 32) zo[i] = 0.f;
         if (lane == 0) p.ec_sync[1 + (par ^ 1u)] = 0;
     }
-    __syncwarp();
-    if (lane == 0) {
-        const unsigned old = arrive_acq_rel(p.ec_sync + 1 + par);
-        if (old == unsigned(G - 1)) p.ec_sync[0] = epoch + 1u;      // the next launch takes the other buffer
+    return par;
+}
+
+// S5 + S6 (warp 9 of the CTAs that finalise a panel): u = alpha * gamma (.) z into shared memory, from the COMPLETE z
+// (fused variant: after every CTA of the grid has arrived) or from the pre-kernel's u (split variant).
+// Runs beside the consumers' main loop, so the device-wide wait and the z round trip stay off their critical path; they
+// meet it on the u_ready barrier when they reach the panel's B items.
+template <int KTOK>
+__device__ void ec_stage_u(const StreamParams& p, int lane, unsigned par, float* us, uint64_t* u_ready) {
+    const int n = KTOK * p.r;
+    if (p.fused) {
+        if (lane == 0) {
+            const unsigned* ctr = p.ec_sync + 1 + par;
+            unsigned f;
+            do {       // all CTAs of the grid are co-resident (cooperative launch), and every one arrives within
+                       // microseconds of its start: this wait cannot deadlock
+                asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(f) : "l"(ctr) : "memory");
+            } while (f < gridDim.x);
+            if (blockIdx.x == 0) p.ec_sync[0] += 1u;       // everybody has arrived: the next fused launch takes the other buffer
+        }
+        __syncwarp();
+        const bool scalar = (p.gate_kind == SPEAR_GATE_SCALAR_SIGMOID);
+        const float* zc = p.zbuf + par * (16 * kZStride);
+        const float bias = (scalar && p.b_g) ? __ldg(p.b_g) : 0.f;
+        const float rinv = 1.f / float(p.r);
+        for (int i0 = lane; i0 < n; i0 += 8 * 32) {
+            float zz[8], zg[8];
+#pragma unroll
+            for (int q = 0; q < 8; ++q) {       // eight independent L2 round trips in flight per lane
+                const int idx = i0 + 32 * q;
+                const int m = int((float(idx) + 0.5f) * rinv), j = idx - m * p.r;
+                const bool on = idx < n && m < p.M;
+                zz[q] = on ? __ldcg(zc + m * kZStride + j) : 0.f;
+                zg[q] = (on && scalar) ? __ldcg(zc + m * kZStride + p.r) : 0.f;
+            }
+#pragma unroll
+            for (int q = 0; q < 8; ++q) {
+                const int idx = i0 + 32 * q;
+                if (idx >= n) break;
+                const int m = int((float(idx) + 0.5f) * rinv), j = idx - m * p.r;
+                const float gam = scalar ? 1.f / (1.f + expf(-(zg[q] + bias))) : 1.f;
+                us[idx] = m < p.M ? p.alpha * gam * zz[q] : 0.f;
+                if (scalar && p.gate_out && blockIdx.x == 0 && j == 0 && m < p.M) p.gate_out[m] = gam;
+            }
+        }
+    } else {
+        for (int idx = lane; idx < n; idx += 32) us[idx] = idx < p.M * p.r ? __ldcg(p.u + idx) : 0.f;
     }
+    __syncwarp();
+    if (lane == 0) mbar_arrive(u_ready);
 }
 
 // MINB = resident CTAs per SM the register allocation must allow: 2 for the shallow ring (96 registers), 1 for the
@@ -320,7 +421,8 @@ stream_kernel(const __grid_constant__ CUtensorMap xmap, const StreamParams p) {
     uint64_t* full = reinterpret_cast<uint64_t*>(reinterpret_cast<uint8_t*>(red) + Cfg::kRedBytes);
     uint64_t* empty = full + Cfg::kMaxStages;
     int* flag = reinterpret_cast<int*>(empty + Cfg::kMaxStages);
-    uint64_t* e_ready = reinterpret_cast<uint64_t*>(flag + 2);     // fused EC: flag[1] holds the epoch to wait past
+    uint64_t* u_ready = reinterpret_cast<uint64_t*>(flag + 2);     // EC: warp 9 has staged u in us[]
+    float* us = reinterpret_cast<float*>(reinterpret_cast<uint8_t*>(full) + Cfg::kBarBytes);      // u = alpha gamma (.) z, [8 MT][r] fp32 (r > 0 only)
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int G = gridDim.x, b = blockIdx.x;
@@ -331,7 +433,7 @@ stream_kernel(const __grid_constant__ CUtensorMap xmap, const StreamParams p) {
 
     if (threadIdx.x == 0) {
         for (int s = 0; s < S; ++s) { mbar_init(&full[s], 2); mbar_init(&empty[s], 8); }
-        mbar_init(e_ready, 1);
+        mbar_init(u_ready, 1);
         fence_mbar_init();
         tma_prefetch_desc(&xmap);
     }
@@ -347,8 +449,21 @@ stream_kernel(const __grid_constant__ CUtensorMap xmap, const StreamParams p) {
             const uint64_t pol_w = policy_evict_first(), pol_s = policy_evict_last();
             const uint8_t* wq = reinterpret_cast<const uint8_t*>(p.wq);
             const uint8_t* sc = reinterpret_cast<const uint8_t*>(p.scales);
-            int pnl = u0 / CP, pr = u0 - pnl * CP, s = 0;
+            // ring items of this CTA: its units in order; a segment (the CTA's units of one panel) that starts its panel is followed by the
+            // panel's B slab (p.b_slots items of p.b_slot_bytes), consumed by the same warps as r / 16 extra k-steps
+            const uint8_t* Bb = reinterpret_cast<const uint8_t*>(p.B);
+            const int nb = p.r > 0 ? p.b_slots : 0;
+            // (B follows the segment that STARTS the panel: its CTA is the one that finalises the panel, see below)
+            int pnl = u0 / CP, pr = u0 - pnl * CP, bs = 0, s = 0;       // bs: 0 = weight unit, 1..nb = B item
+            int done = 0;                                               // units issued
+            bool head = (pr == 0);                                      // the current segment starts its panel
+            const int n_items = n_units + nb * ((u0 + n_units - 1) / CP - u0 / CP + (pr == 0 ? 1 : 0));
             auto issue_w = [&]() {
+                if (bs > 0) {
+                    mbar_arrive_expect_tx(&full[s], p.b_slot_bytes);
+                    bulk_g2s(wring + s * Cfg::kWUnit, Bb + (size_t(pnl) * nb + (bs - 1)) * p.b_slot_bytes, p.b_slot_bytes, &full[s], pol_w);
+                    return;
+                }
                 const int c0 = 2 * pr, nch = (c0 + 1 < C) ? 2 : 1;
                 mbar_arrive_expect_tx(&full[s], nch * (8192 + 256));
                 bulk_g2s(wring + s * Cfg::kWUnit, wq + (size_t(pnl) * C + c0) * 8192, nch * 8192, &full[s], pol_w);
@@ -363,43 +478,50 @@ stream_kernel(const __grid_constant__ CUtensorMap xmap, const StreamParams p) {
                 }
             };
             auto issue_x = [&]() {
+                if (bs > 0) { mbar_arrive(&full[s]); return; }      // a B item has no x tile
                 mbar_arrive_expect_tx(&full[s], Cfg::kXTile);
                 tma_load_3d(xring + s * Cfg::kXTile, &xmap, 0, pr * 4, 0, &full[s], pol_s);
             };
             auto advance = [&]() {
-                if (++pr == CP) { pr = 0; ++pnl; }
                 if (++s == S) s = 0;
+                if (bs == 0) {
+                    ++done;
+                    const bool seg_end = (pr == CP - 1) || (done == n_units);
+                    if (nb > 0 && seg_end && head) { bs = 1; return; }
+                    if (seg_end) head = true;        // every later segment starts at a panel boundary
+                } else if (bs < nb) {
+                    ++bs;
+                    return;
+                }
+                bs = 0;
+                if (++pr == CP) { pr = 0; ++pnl; }
             };
-            const int nfirst = min(n_units, S);
+            const int nfirst = min(n_items, S);
             for (int it = 0; it < nfirst; ++it) { issue_w(); advance(); }
             pdl_wait();   // x may be written by the previous kernel in the stream
-            pnl = u0 / CP; pr = u0 - pnl * CP; s = 0;
+            pnl = u0 / CP; pr = u0 - pnl * CP; bs = 0; s = 0; done = 0; head = (pr == 0);
             for (int it = 0; it < nfirst; ++it) { issue_x(); advance(); }
             uint32_t eph = 0;     // parity of the first completion of empty[]
-            for (int it = nfirst; it < n_units; ++it) {
+            for (int it = nfirst; it < n_items; ++it) {
                 mbar_wait(&empty[s], eph);
                 issue_w();
                 issue_x();
                 advance();
                 if (s == 0) eph ^= 1;
             }
-        } else if (p.r > 0) {
-            // warm L2 with the B rows of every panel this CTA may finalise (read only in the epilogue)
-            const int p_first = u0 / CP, p_last = (u0 + n_units - 1) / CP;
-            const uint8_t* Bb = reinterpret_cast<const uint8_t*>(p.B);
-            const size_t slab = size_t(128) * p.r * (p.ec_int8 ? 1 : 2);
-            for (int pnl = p_first; pnl <= p_last; ++pnl)
-                for (size_t off = size_t(lane - 1) * 128; off < slab; off += 31 * 128)
-                    prefetch_l2(Bb + size_t(pnl) * slab + off);
         }
         return;
     }
     if (warp == 9) {
         // ------------------------------ EC warp (fused variant only) ------------------------------
-        if (!(p.fused && p.r > 0)) return;
-        ec_prefetch_factors(p, lane);   // EC factors are parameters: warm L2 before the wait
+        if (p.r == 0) return;
+        // this CTA finalises the panels whose first unit it owns (every segment but a first one that starts mid-panel)
+        const bool finalises = (u0 + n_units - 1) / CP - u0 / CP + (u0 % CP == 0 ? 1 : 0) > 0;
+        unsigned par = 0;
+        if (p.fused) ec_prefetch_factors(p, lane);   // EC factors are parameters: warm L2 before the wait
         pdl_wait();
-        ec_reduce_and_arrive(p, lane, flag + 1, e_ready);
+        if (p.fused) par = ec_reduce_and_arrive(p, lane);
+        if (finalises) ec_stage_u<Cfg::kTok>(p, lane, par, us, u_ready);
         return;
     }
 
@@ -470,30 +592,52 @@ stream_kernel(const __grid_constant__ CUtensorMap xmap, const StreamParams p) {
             val[i] = v;
         }
         const bool whole = ((u0 + seg_begin) % CP == 0) && (seg_end - seg_begin == CP);
+        // Who finalises a split panel.  Plain layer (r == 0): the last CTA to arrive (nobody ever waits).  With an EC: the
+        // CTA that owns the panel's first unit -- the ring brought the panel's B slab to ITS shared memory -- which waits
+        // for the other parts; those were started earlier (a CTA's mid-panel segment is its first) and the launch is
+        // cooperative, so the wait is short and cannot deadlock.
+        const bool head = (u0 + seg_begin) % CP == 0;
+        const bool waits = p.r > 0 && head;
         bool finalize = whole;
         int c_first = b, c_last = b;
         if (!whole) {
             const int which = ((u0 / CP) == pnl) ? 0 : 1;
             float* slot = p.partial + size_t(b * 2 + which) * Cfg::kTok * 128;
+            if (!waits) {
 #pragma unroll
-            for (int i = 0; i < 4 * MT; ++i) slot[((ct >> 7) + 2 * i) * 128 + row] = val[i];
+                for (int i = 0; i < 4 * MT; ++i) slot[((ct >> 7) + 2 * i) * 128 + row] = val[i];
+            }
             named_bar_sync(2, 256);
             c_first = cta_of_unit(pnl * CP, per, rem);
             c_last = cta_of_unit(pnl * CP + CP - 1, per, rem);
             if (ct == 0) {
-                const unsigned old = arrive_acq_rel(p.counters + pnl);   // releases the CTA's partial, acquires the others'
-                const int last = (old == unsigned(c_last - c_first));
-                if (last) p.counters[pnl] = 0;      // self-cleaning: the next call finds zero
-                *flag = last;
+                if (waits) {
+                    unsigned f;
+                    do { asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(f) : "l"(p.counters + pnl) : "memory"); } while (f < unsigned(c_last - c_first));
+                    p.counters[pnl] = 0;            // self-cleaning: the next call finds zero
+                    *flag = 1;
+                } else {
+                    int last = 0;
+                    if (p.r > 0) {
+                        arrive_release(p.counters + pnl);        // the panel's head CTA is waiting for this
+                    } else {
+                        const unsigned old = arrive_acq_rel(p.counters + pnl);   // releases the CTA's partial, acquires the others'
+                        last = (old == unsigned(c_last - c_first));
+                        if (last) p.counters[pnl] = 0;
+                    }
+                    *flag = last;
+                }
             }
             named_bar_sync(2, 256);
             finalize = (*flag != 0);
             if (finalize) {
+                if (!waits) {
 #pragma unroll
-                for (int i = 0; i < 4 * MT; ++i) val[i] = 0.f;
-                // partials are summed in CTA order; four CTAs' loads are issued before the first add so that their
-                // L2 round trips overlap instead of queueing one behind the other
-                for (int cj = c_first; cj <= c_last; cj += 4) {
+                    for (int i = 0; i < 4 * MT; ++i) val[i] = 0.f;
+                }
+                // partials are summed in CTA order (a waiting head CTA keeps its own part in registers and adds the others);
+                // four CTAs' loads are issued before the first add so that their L2 round trips overlap
+                for (int cj = waits ? c_first + 1 : c_first; cj <= c_last; cj += 4) {
                     float tmp[4][4 * MT];
 #pragma unroll
                     for (int q = 0; q < 4; ++q) {
@@ -513,76 +657,46 @@ stream_kernel(const __grid_constant__ CUtensorMap xmap, const StreamParams p) {
                 }
             }
         }
+        if (waits) {
+            // ---- S7: the next ring item(s) hold this panel's B slab; every warp multiplies its 16-row strip by u^T on
+            // the tensor cores (u staged by warp 9, met here on u_ready) and the strips go through red[] once more to
+            // reach the row-per-thread layout of val[].
+            if (!u_seen) { mbar_wait(u_ready, 0); u_seen = true; }
+            const int nb = p.b_slots;
+            const int esz = p.ec_int8 ? 1 : 2;
+            const int row0 = 64 * h + 16 * kq;                   // this warp's strip of the panel
+            float sb0 = 1.f, sb1 = 1.f;
+            if (p.ec_int8) {                                     // INT8 factors: per-row scale of B
+                sb0 = __half2float(__ldg(p.B_scale + pnl * 128 + row0 + g));
+                sb1 = __half2float(__ldg(p.B_scale + pnl * 128 + row0 + g + 8));
+            }
+            float acc[MT][4];
+#pragma unroll
+            for (int mt = 0; mt < MT; ++mt) acc[mt][0] = acc[mt][1] = acc[mt][2] = acc[mt][3] = 0.f;
+            for (int k = 0; k < nb; ++k) {
+                mbar_wait(&full[rs], rph);
+                if (nb == 1 || h == k)
+                    ec_up<MT>(smem_u32(wring) + rs * Cfg::kWUnit + (nb == 1 ? row0 : 16 * kq) * p.r * esz, p.r, p.ec_int8 != 0, us, lane, acc);
+                __syncwarp();
+                if (lane == 0) mbar_arrive(&empty[rs]);
+                if (++rs == S) { rs = 0; rph ^= 1; }
+            }
+            constexpr int kEcStride = 132;                       // [token][row]: conflict-free fragment stores
+            named_bar_sync(2, 256);                              // every thread has taken its sums out of red[]
+#pragma unroll
+            for (int mt = 0; mt < MT; ++mt) {
+                const int tok = mt * 8 + 2 * t;
+                red[tok * kEcStride + row0 + g] = sb0 * acc[mt][0];
+                red[(tok + 1) * kEcStride + row0 + g] = sb0 * acc[mt][1];
+                red[tok * kEcStride + row0 + g + 8] = sb1 * acc[mt][2];
+                red[(tok + 1) * kEcStride + row0 + g + 8] = sb1 * acc[mt][3];
+            }
+            named_bar_sync(2, 256);
+#pragma unroll
+            for (int i = 0; i < 4 * MT; ++i) val[i] += red[((ct >> 7) + 2 * i) * kEcStride + row];
+        }
         if (finalize) {
             const int n = pnl * 128 + row;
-            if (p.r > 0) {
-                // S7: y += sum_j u[m][j] * B[n][j]   (u = alpha * gamma (.) z, fp32, from the pre-kernel or warp 9)
-                if (p.fused && !u_seen) {
-                    if (ct == 0) {   // wait (late) until every CTA has added its piece of z
-                        mbar_wait(e_ready, 0);
-                        const unsigned* ctr = p.ec_sync + 1 + flag[1];
-                        unsigned f;
-                        do {       // all CTAs of the grid are co-resident (cooperative launch), and every one arrives within
-                                   // microseconds of its start: this wait cannot deadlock
-                            asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(f) : "l"(ctr) : "memory");
-                        } while (f < gridDim.x);
-                    }
-                    u_seen = true;      // later panels of this CTA need not look again
-                }
-                // u (M x r fp32, <= 8 KiB) is staged in the idle reduction buffer: every lane of a warp then reads
-                // the same word (broadcast) instead of paying an L2 round trip per term
-                float* us = red;
-                named_bar_sync(2, 256);      // every thread has taken its sums out of red[]; the counter was seen
-                if (p.fused) {
-                    // S5 + S6 here: gamma from the complete z, u = alpha * gamma (.) z
-                    const bool scalar = (p.gate_kind == SPEAR_GATE_SCALAR_SIGMOID);
-                    const float* zc = p.zbuf + flag[1] * (16 * kZStride);
-                    const float bias = (scalar && p.b_g) ? __ldg(p.b_g) : 0.f;
-                    for (int idx = ct; idx < p.M * p.r; idx += 256) {
-                        const int m = idx / p.r, j = idx - m * p.r;
-                        const float zz = __ldcg(zc + m * kZStride + j);
-                        float gam = 1.f;
-                        if (scalar) gam = 1.f / (1.f + expf(-(__ldcg(zc + m * kZStride + p.r) + bias)));
-                        us[idx] = p.alpha * gam * zz;
-                        if (scalar && p.gate_out && pnl == 0 && j == 0) p.gate_out[m] = gam;
-                    }
-                } else {
-                    for (int idx = ct; idx < p.M * p.r; idx += 256) us[idx] = __ldcg(p.u + idx);
-                }
-                named_bar_sync(2, 256);
-                const uint4* Brow = reinterpret_cast<const uint4*>(p.B + size_t(n) * p.r);
-                const uint2* Brow8 = reinterpret_cast<const uint2*>(reinterpret_cast<const int8_t*>(p.B) + size_t(n) * p.r);
-                const float sb = p.ec_int8 ? __half2float(__ldg(p.B_scale + n)) : 1.f;     // INT8 factors: per-row scale of B
-#pragma unroll 4
-                for (int j8 = 0; j8 < p.r / 8; ++j8) {
-                    uint32_t bw[4];
-                    if (p.ec_int8) {
-                        const uint2 b8 = __ldg(Brow8 + j8);
-                        cvt_i8x4_f16x2(b8.x, bw[0], bw[1]);
-                        cvt_i8x4_f16x2(b8.y, bw[2], bw[3]);
-                    } else {
-                        const uint4 bv = __ldg(Brow + j8);
-                        bw[0] = bv.x; bw[1] = bv.y; bw[2] = bv.z; bw[3] = bv.w;
-                    }
-                    const __half2* bh = reinterpret_cast<const __half2*>(bw);
-                    float bf[8];
-#pragma unroll
-                    for (int q = 0; q < 4; ++q) {
-                        const float2 f = __half22float2(bh[q]);
-                        bf[2 * q] = f.x * sb; bf[2 * q + 1] = f.y * sb;
-                    }
-#pragma unroll
-                    for (int i = 0; i < 4 * MT; ++i) {
-                        const int tok = (ct >> 7) + 2 * i;
-                        if (tok < p.M) {
-                            const float4* up = reinterpret_cast<const float4*>(us + tok * p.r + j8 * 8);
-                            const float4 ua = up[0], ub = up[1];
-                            val[i] += ua.x * bf[0] + ua.y * bf[1] + ua.z * bf[2] + ua.w * bf[3] +
-                                      ub.x * bf[4] + ub.y * bf[5] + ub.z * bf[6] + ub.w * bf[7];
-                        }
-                    }
-                }
-            }
             if (p.resid) {
                 // fused tail, first half: residual add on the fp32 sums, and this panel's share of the
                 // per-token sum of squares that the next layer's RMSNorm needs (taken before the rounding)
@@ -660,21 +774,31 @@ int stream_stages(int MT, bool deep) {
     if (MT == 1) return deep ? StreamCfg<1>::kStagesDeep : StreamCfg<1>::kStagesShallow;
     return deep ? StreamCfg<2>::kStagesDeep : StreamCfg<2>::kStagesShallow;
 }
-int stream_smem_bytes(int MT, int stages) {
-    return int(MT == 1 ? StreamCfg<1>::smem_bytes(stages) : StreamCfg<2>::smem_bytes(stages));
+// u buffer behind the barriers: [8 MT][r] fp32
+static int stream_u_bytes(int MT, int r) { return r > 0 ? ((8 * MT * r * 4 + 127) & ~127) : 0; }
+int stream_smem_bytes(int MT, int stages, int r) {
+    return int(MT == 1 ? StreamCfg<1>::smem_bytes(stages) : StreamCfg<2>::smem_bytes(stages)) + stream_u_bytes(MT, r);
+}
+int stream_fit_stages(int MT, bool deep, int r) {
+    constexpr int kLimit = 232448 - 1024;      // opt-in shared memory per CTA minus the kernel's static shared variables
+    int S = stream_stages(MT, deep);
+    while (S > 2 && stream_smem_bytes(MT, S, r) > kLimit) --S;
+    return S;
 }
 
-// Resident CTAs per SM of the instance a launch would take (occupancy query, cached): the fused EC's device-wide
-// arrive / wait needs the whole grid resident, so api.cu clamps the grid to num_sms x this.
-int stream_resident_ctas(int MT, bool deep) {
-    static int cache[2][2] = {{0, 0}, {0, 0}};
-    int& c = cache[MT - 1][deep ? 1 : 0];
+// Resident CTAs per SM of the instance a launch would take (occupancy query, cached per u-buffer size): the fused EC's
+// device-wide arrive / wait needs the whole grid resident, so api.cu clamps the grid to num_sms x this.
+int stream_resident_ctas(int MT, bool deep, int r) {
+    static std::mutex mu;
+    static int cache[2][2][130] = {};
+    std::lock_guard<std::mutex> lock(mu);
+    int& c = cache[MT - 1][deep ? 1 : 0][std::min(r, 129)];
     if (c == 0) {
-        const int smem = stream_smem_bytes(MT, stream_stages(MT, deep));
+        const int smem = stream_smem_bytes(MT, stream_fit_stages(MT, deep, r), r);
         const void* fn = MT == 1 ? (deep ? (const void*)stream_kernel<1, 1> : (const void*)stream_kernel<1, 2>)
                                  : (deep ? (const void*)stream_kernel<2, 1> : (const void*)stream_kernel<2, 2>);
         int n = 0;
-        if (cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, smem) != cudaSuccess ||
+        if (cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, 232448 - 1024) != cudaSuccess ||
             cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n, fn, 320, smem) != cudaSuccess || n < 1)
             n = 1;
         c = n;
@@ -690,30 +814,31 @@ int launch_stream(const CUtensorMap& xmap, const StreamParams& p, int MT, int gr
         auto set = [&](const void* fn, size_t bytes) {
             if (attr_err == cudaSuccess) attr_err = cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, int(bytes));
         };
-        set((const void*)stream_kernel<1, 2>, StreamCfg<1>::smem_bytes(StreamCfg<1>::kStagesShallow));
-        set((const void*)stream_kernel<2, 2>, StreamCfg<2>::smem_bytes(StreamCfg<2>::kStagesShallow));
-        set((const void*)stream_kernel<1, 1>, StreamCfg<1>::smem_bytes(StreamCfg<1>::kStagesDeep));
-        set((const void*)stream_kernel<2, 1>, StreamCfg<2>::smem_bytes(StreamCfg<2>::kStagesDeep));
+        // every instance may take up to the opt-in maximum (ring + u buffer; stream_fit_stages keeps it below)
+        set((const void*)stream_kernel<1, 2>, 232448 - 1024);
+        set((const void*)stream_kernel<2, 2>, 232448 - 1024);
+        set((const void*)stream_kernel<1, 1>, 232448 - 1024);
+        set((const void*)stream_kernel<2, 1>, 232448 - 1024);
     });
     SPEAR_CUDA_OK(attr_err);
     cudaLaunchConfig_t cfg = {};
     cfg.gridDim = dim3(grid);
     cfg.blockDim = dim3(320);
-    cfg.dynamicSmemBytes = stream_smem_bytes(MT, p.stages);
+    cfg.dynamicSmemBytes = stream_smem_bytes(MT, p.stages, p.r);
     cfg.stream = st;
     cudaLaunchAttribute attr[2];
     attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
     attr[0].val.programmaticStreamSerializationAllowed = pdl ? 1 : 0;
     cfg.attrs = attr;
     cfg.numAttrs = 1;
-    if ((p.fused && p.r > 0) || p.resid) {
+    if (p.r > 0 || p.resid) {
         // the fused EC (and the fused tail's row-wide mean) wait device-wide for their own grid: a cooperative launch makes the co-residency of all CTAs a
         // guarantee of the driver instead of an assumption about dispatch order (other lanes, other tenants of the GPU)
         attr[1].id = cudaLaunchAttributeCooperative;
         attr[1].val.cooperative = 1;
         cfg.numAttrs = 2;
     }
-    const bool deep = p.stages > stream_stages(MT, false);
+    const bool deep = p.deep != 0;
     if (MT == 1 && !deep) SPEAR_CUDA_OK(cudaLaunchKernelEx(&cfg, stream_kernel<1, 2>, xmap, p));
     else if (MT == 1) SPEAR_CUDA_OK(cudaLaunchKernelEx(&cfg, stream_kernel<1, 1>, xmap, p));
     else if (!deep) SPEAR_CUDA_OK(cudaLaunchKernelEx(&cfg, stream_kernel<2, 2>, xmap, p));

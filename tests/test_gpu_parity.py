@@ -465,3 +465,39 @@ def test_fused_tail_in_place_residual(sp):
     s_ref, h_ref = oracle.tail(oracle.forward_layer(li)["y"], res, gw, 1e-5)
     assert float(np.max(np.abs(y.cpu().numpy().astype(np.float64) - s_ref))) <= Y_TOL * float(np.sqrt(np.mean(s_ref ** 2)))
     assert float(np.max(np.abs(hn.cpu().numpy().astype(np.float64) - h_ref))) <= Y_TOL * float(np.sqrt(np.mean(h_ref ** 2)))
+
+
+def test_config2_step_stream_ordered_as_bench_headline(sp):
+    """The headline leg of bench.py: the 12 calls of BASELINE.json configs[1] one after the other on one stream
+    (spear_w4_ec_gemm_ex, AUTO dispatch: deep-ring weight-stream kernel with the fused EC, cooperative + PDL-chained),
+    captured in a CUDA graph and replayed; every call, every output element against the oracle."""
+    import torch
+    h = _harness()
+    shapes = config_shapes(1)
+    lis = [make_layer(s.seed, s.M, s.N, s.K, s.group, s.r, gate="scalar") for s in shapes]
+    dls = [h.upload_layer(li) for li in lis]
+    xs = [h.dev(li.x) for li in lis]
+    ys = [torch.zeros((li.M, li.N), dtype=torch.float16, device="cuda:0") for li in lis]
+    ds = [dl.desc() for dl in dls]
+
+    def step():
+        for x, dl, d, y in zip(xs, dls, ds, ys):
+            sp.w4_ec_gemm_ex(x, dl.pw, dl.A, dl.B, d, y=y)
+
+    st = torch.cuda.Stream()
+    with torch.cuda.stream(st):
+        step()
+        torch.cuda.synchronize()
+        g = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(g, stream=st):
+            step()
+        for y in ys:
+            y.zero_()
+        for _ in range(5):
+            g.replay()
+    torch.cuda.synchronize()
+    for s, li, y in zip(shapes, lis, ys):
+        ref = oracle.forward_layer(li)["y"]
+        rms = float(np.sqrt(np.mean(ref ** 2)))
+        err = float(np.max(np.abs(y.cpu().numpy().astype(np.float64) - ref)))
+        assert err <= Y_TOL * rms, f"config2 {s.name} M={s.M} stream-ordered: {err:.4g} > {Y_TOL} * {rms:.4g}"
