@@ -151,8 +151,9 @@ def load_tensor_peak():
     return 1590.0, "fallback (B200_PROFILING.md 1.59 PFLOP/s burst)"
 
 
-def profile_traffic():
-    """dram__bytes_read + dram__bytes_write per launch of the dominant decode kernel, from the committed ncu capture."""
+def profile_traffic(kernel):
+    """dram__bytes_read + dram__bytes_write per launch of `kernel` (the dominant decode kernel of this run), from the committed
+    ncu capture.  A capture of another kernel is not a substitute: then the figure is None and the note says what is missing."""
     p = os.path.join(ROOT, "profiles", "r02_dram_traffic.csv")
     if not os.path.exists(p):
         return None, "no capture committed"
@@ -160,9 +161,9 @@ def profile_traffic():
     with open(p) as f:
         rows = list(csv.reader(l for l in f if l.strip() and not l.startswith("#")))
     for r in rows[1:]:
-        if r[0] == "stream_kernel":
+        if r[0] and r[0] in kernel:
             return int(r[3]), f"{r[1]} ({r[2]}); algorithmic {r[4]} B; profiles/r02_dram_traffic.csv"
-    return None, "stream_kernel not in profiles/r02_dram_traffic.csv"
+    return None, f"no capture of {kernel} in profiles/r02_dram_traffic.csv (it holds: {', '.join(sorted({r[0] for r in rows[1:]}))})"
 
 
 def run_cuda(args, rank, world):
@@ -306,6 +307,69 @@ def run_cuda(args, rank, world):
     lanes_ec_i8 = leg(True, "lanes", steps=sub, ec_int8=True)
     lanes_ec, lanes_w4 = leg(True, "lanes", steps=sub), leg(False, "lanes", steps=sub)
     ls_ec, ls_w4 = leg(True, "lstream", steps=sub), leg(False, "lstream", steps=sub)
+    # ---- which kernel runs which call, and how long each call takes in the headline regime --------------------------------
+    # One CUDA graph per call of the step: that call alone, stream-ordered, once per weight copy.  The 12 graphs are replayed in
+    # turn, so between two replays of one graph all the other calls' copies (677 MiB in all) have gone through L2: cold weights.
+    KERNEL_OF = {sp.VARIANT_STREAM_FUSED: "spear::stream_kernel<MT,1>", sp.VARIANT_STREAM_SPLIT: "spear::stream_kernel<MT,1>",
+                 sp.VARIANT_ROWS: "spear::rows_kernel<MT,FUSED>", sp.VARIANT_LSTREAM: "spear::ls_kernel",
+                 sp.VARIANT_TC_FUSED: "spear::tc_kernel", sp.VARIANT_TC_SPLIT: "spear::tc_kernel"}
+
+    def per_call(with_ec):
+        calls, graphs = [], []
+        with torch.cuda.stream(stream):
+            for M in TOKENS:
+                for s in shapes[M]:
+                    ds = [(cp[s.name].desc() if with_ec else sp.make_desc(gate="none")) for cp in copies]
+
+                    def body(M=M, s=s, ds=ds):
+                        for cp, d in zip(copies, ds):
+                            dl = cp[s.name]
+                            sp.w4_ec_gemm_ex(xs[(M, s.name)], dl.pw, dl.A if with_ec else None, dl.B if with_ec else None, d, y=ys[(M, s.name)])
+                    body()
+                    torch.cuda.synchronize()
+                    cg = torch.cuda.CUDAGraph()
+                    with torch.cuda.graph(cg, stream=stream):
+                        body()
+                    graphs.append((cg, ds))
+                    v = sp.plan_query(M, s.N, s.K, s.r if with_ec else 0, s.group, gate="scalar" if with_ec else "none")
+                    calls.append({"call": f"{s.name} M={M}", "variant": v, "kernel": KERNEL_OF.get(v, "?"),
+                                  "bytes": algorithmic_bytes(M, s.N, s.K, s.group, s.r if with_ec else 0, "scalar" if with_ec else "none", 0)})
+            ts = [[] for _ in graphs]
+            for rep in range(7):
+                for gi, (cg, _) in enumerate(graphs):
+                    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                    e0.record(stream)
+                    cg.replay()
+                    e1.record(stream)
+                    e1.synchronize()
+                    if rep >= 2:
+                        ts[gi].append(e0.elapsed_time(e1) * 1e3 / ncopy)
+        for c, t in zip(calls, ts):
+            c["us"] = round(sorted(t)[len(t) // 2], 3)
+        return calls
+
+    def by_kernel(calls):
+        tot = sum(c["us"] for c in calls)
+        groups = {}
+        for c in calls:
+            g = groups.setdefault(c["kernel"], {"kernel": c["kernel"], "launches_per_step": 0, "us_per_step": 0.0, "bytes_per_step": 0, "calls": []})
+            g["launches_per_step"] += 1
+            g["us_per_step"] += c["us"]
+            g["bytes_per_step"] += c["bytes"]
+            g["calls"].append(c["call"])
+        out = []
+        for g in groups.values():
+            ach = g["bytes_per_step"] / (g["us_per_step"] * 1e-6) / 1e9
+            out.append({"kernel": g["kernel"], "launches_per_step": g["launches_per_step"], "calls": g["calls"],
+                        "share_of_step_time": round(g["us_per_step"] / tot, 4), "avg_launch_us": round(g["us_per_step"] / g["launches_per_step"], 3),
+                        "algorithmic_bytes_per_launch": int(g["bytes_per_step"] / g["launches_per_step"]),
+                        "achieved": round(ach, 1), "frac": round(ach / peak, 4)})
+        out.sort(key=lambda g: -g["share_of_step_time"])
+        return out, tot
+
+    calls_w4, calls_ec = per_call(False), per_call(True)
+    kern_w4, sum_w4 = by_kernel(calls_w4)
+    kern_ec, sum_ec = by_kernel(calls_ec)
     t_end = time.time() + 1.0      # keep the GPU under load long enough for nvidia-smi to sample it
     while rank == 0 and time.time() < t_end:
         timed(g_head, 200, 0)
@@ -328,8 +392,8 @@ def run_cuda(args, rank, world):
 
     value = aggregate_value(b_ec, ms_head, world)
     ncalls = sum(len(v) for v in shapes.values())
-    traffic, traffic_note = profile_traffic()
-    ach = ordered_w4["value"] / world
+    dom = kern_w4[0]
+    traffic, traffic_note = profile_traffic(dom["kernel"])
     out = {
         "metric": METRIC, "value": round(value, 1), "unit": UNIT, "n_gpus": world, "steps": args.steps,
         "warmup": args.warmup, "ms_per_step": round(ms_head, 6), "higher_is_better": True, "scaling": "weak",
@@ -346,12 +410,22 @@ def run_cuda(args, rank, world):
                 "path": "spear_w4_ec_gemm_batch_hostio (per call: pinned host x -> device, layer, device -> pinned host y, on the lanes)"},
         "gpu_launches": int(per_step_launches * args.steps),
         "clocks": clocks,
-        "roofline": {"bound": "hbm", "kernel": "spear::stream_kernel<MT,1> (deep ring, one launch per layer call, stream-ordered; "
-                                                "plain W4 leg of the same step)",
-                     "achieved": round(ach, 1), "peak": peak, "unit": "GB/s", "frac": round(ach / peak, 4),
-                     "peak_source": peak_src, "traffic": traffic, "traffic_note": traffic_note,
-                     "avg_launch_us": round(ordered_w4["ms_per_step"] * 1e3 / ncalls, 3), "launches_per_step": ncalls,
-                     "frac_with_ec": round(value / world / peak, 4)},
+        "roofline": dict(
+            {"bound": "hbm", "kernel": dom["kernel"], "achieved": dom["achieved"], "peak": peak, "unit": "GB/s", "frac": dom["frac"],
+             "peak_source": peak_src, "traffic": traffic, "traffic_note": traffic_note,
+             "avg_launch_us": dom["avg_launch_us"], "launches_per_step": dom["launches_per_step"],
+             "algorithmic_bytes_per_launch": dom["algorithmic_bytes_per_launch"], "share_of_step_time": dom["share_of_step_time"],
+             "calls": dom["calls"]},
+            how="the kernel with the largest share of the plain (r = 0) stream-ordered step; achieved = algorithmic bytes of ITS launches / "
+                "the summed durations of ITS launches, each call timed alone in its own CUDA graph over cold weight copies (graphs replayed "
+                "in turn); which kernel serves a call is asked of the library (spear_plan_query)",
+            other_kernels=kern_w4[1:], with_ec=kern_ec,
+            per_call_us={"no_ec": {c["call"]: c["us"] for c in calls_w4}, "ec": {c["call"]: c["us"] for c in calls_ec}},
+            step={"note": "the whole step (all 12 calls, every kernel): bytes_per_step / ms_per_step of the no_ec and headline legs; "
+                          "sum_of_calls_us is the per-call graphs added up (isolated calls; the mixed step differs by a few per cent)",
+                  "frac_no_ec": ordered_w4["frac_of_measured_hbm"], "frac_with_ec": round(value / world / peak, 4),
+                  "sum_of_calls_us": {"no_ec": round(sum_w4, 2), "ec": round(sum_ec, 2)},
+                  "step_us": {"no_ec": round(ordered_w4["ms_per_step"] * 1e3, 2), "ec": round(ms_head * 1e3, 2)}}),
         "no_ec": ordered_w4,
         "ec_overhead_time_frac": round(ms_head / ordered_w4["ms_per_step"] - 1.0, 4),
         "ec_l2_resident": dict(ordered_ec_res, ec_overhead_time_frac=round(ordered_ec_res["ms_per_step"] / ordered_w4["ms_per_step"] - 1.0, 4)),

@@ -65,7 +65,9 @@ typedef enum {
                                         paper's unfused comparator; y is rounded twice); any M, r > 0 */
     SPEAR_VARIANT_LSTREAM = 5,       /* persistent layer-stream kernel (tcgen05, weights through TMEM), EC fused; M <= 16,
                                         scalar / none gate; also what spear_w4_ec_gemm_batch runs for such calls */
-    SPEAR_VARIANT_COUNT = 6
+    SPEAR_VARIANT_ROWS = 6,          /* EC pre-kernel (r > 0) + row-strip kernel: one CTA per 16 output rows over the whole of K, no
+                                        cross-CTA reduction; M <= 16, the latency-bound (small) layers */
+    SPEAR_VARIANT_COUNT = 7
 } spear_variant;
 
 /* ---- S0: packing (the "SPW4" layout) -------------------------------- */
@@ -132,7 +134,11 @@ int spear_w4_ec_gemm_ex(const void* x, const void* Wq, const void* scales, const
  * Both are formed from the fp32 accumulators (one rounding each; the mean of squares is taken before rounding).  For
  * M <= 16 on the weight-stream variants this happens inside the layer kernel's epilogue (the row-wide mean needs every
  * output panel: arrive / wait across the co-resident CTAs of a cooperative launch); the other variants run the layer and a
- * row kernel.  residual [M][N] fp16 (may alias y), rms_weight [N] fp16, h_out [M][N] fp16 (must not alias y or x). */
+ * row kernel; AUTO therefore keeps M <= 16 on the weight-stream variants when a tail is asked for.
+ * residual [M][N] fp16, rms_weight [N] fp16, h_out [M][N] fp16 (must not alias y or x).  residual == y (the residual
+ * stream updated in place) is supported where the tail is fused -- M <= 16, SPEAR_VARIANT_AUTO / STREAM_FUSED /
+ * STREAM_SPLIT; on every other arm (M > 16, or a forced ROWS / LSTREAM / TC variant) the layer kernel has stored y before
+ * the row kernel reads residual, so an aliased or partly overlapping residual is rejected with SPEAR_EINVAL. */
 typedef struct {
     const void* residual;
     const void* rms_weight;

@@ -17,8 +17,8 @@ LIB_PATH = os.path.join(_HERE, "libspear.so")
 
 GATE_SCALAR_SIGMOID, GATE_MLP, GATE_NONE = 0, 1, 2
 GATE_KINDS = {"scalar": GATE_SCALAR_SIGMOID, "mlp": GATE_MLP, "none": GATE_NONE}
-VARIANT_AUTO, VARIANT_STREAM_FUSED, VARIANT_STREAM_SPLIT, VARIANT_TC_FUSED, VARIANT_TC_SPLIT, VARIANT_LSTREAM = range(6)
-VARIANT_COUNT = 6
+VARIANT_AUTO, VARIANT_STREAM_FUSED, VARIANT_STREAM_SPLIT, VARIANT_TC_FUSED, VARIANT_TC_SPLIT, VARIANT_LSTREAM, VARIANT_ROWS = range(7)
+VARIANT_COUNT = 7
 VARIANT_NAMES = ["auto", "stream_fused", "stream_split", "tc_fused", "tc_split", "lstream"]
 
 EXPORTS = [

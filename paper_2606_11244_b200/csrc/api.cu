@@ -241,6 +241,7 @@ struct Tunables {
     int stream_units = 0;         // the same target for stream-ordered calls (0 = off: use every SM)
     int lstream = -1;             // layer-stream kernel for M <= 16: -1 = where the plan tables measured it faster (chains always), 0 = never, 1 = always
     int stream_whole_panels = 1;  // 1 = whole-panel partition when N/128 is within 1/5 of the grid
+    int rows = 1;                 // 1 = the heuristic may pick the row-strip kernel for small decode layers, 0 = never
 };
 static Tunables g_tune;
 static thread_local bool t_in_batch = false;
@@ -260,15 +261,27 @@ static bool variant_valid(int v, int M, int r, int gate) {
         case SPEAR_VARIANT_STREAM_FUSED: return M <= 16 && r > 0 && gate != SPEAR_GATE_MLP;
         case SPEAR_VARIANT_STREAM_SPLIT: return M <= 16;
         case SPEAR_VARIANT_LSTREAM: return M <= 16 && gate != SPEAR_GATE_MLP;      // (+ group shape, checked in layer_impl)
+        case SPEAR_VARIANT_ROWS: return M <= 16;
         case SPEAR_VARIANT_TC_FUSED: return tc_available() && M >= 1;
         case SPEAR_VARIANT_TC_SPLIT: return tc_available() && r > 0;
         default: return false;
     }
     (void)r;
 }
-static int heuristic_variant(int M, int r, int gate) {
+// Where no plan entry exists.  Decode: the row-strip kernel (no cross-CTA reduction) on the layers whose time is the
+// latency chain, not the bytes -- measured (B200, stream-ordered, cold weights): plain layers up to 4 MiB of int4 at any
+// M <= 16 (2.1-3.8 us against 4.7-6.2), up to 13 MiB at M <= 8 (down 2048x8192: 7.3 against 8.4); with an EC up to 4 MiB
+// (5.5-9.6 us against 7.2-10.5).  Everything larger streams through the ring kernel.
+static int heuristic_variant(int M, int N, int K, int r, int gate) {
     if (M <= 16 && g_tune.lstream == 1 && gate != SPEAR_GATE_MLP) return SPEAR_VARIANT_LSTREAM;
-    if (M <= 16) return (r > 0 && gate != SPEAR_GATE_MLP) ? SPEAR_VARIANT_STREAM_FUSED : SPEAR_VARIANT_STREAM_SPLIT;
+    if (M <= 16) {
+        const size_t wbytes = size_t(N) * K / 2;
+        // (not inside a batch: there whole kernels of different lanes overlap, and the ring kernel's few big CTAs share the
+        // SMs better than thousands of small ones -- measured 40 vs 47 us plain, 53 vs 80 us with the EC on the 12-call step)
+        const bool rows = g_tune.rows != 0 && !t_in_batch && (wbytes <= (size_t(4) << 20) || (r == 0 && M <= 8 && wbytes <= (size_t(13) << 20) && N <= 8192));
+        if (rows) return SPEAR_VARIANT_ROWS;
+        return (r > 0 && gate != SPEAR_GATE_MLP) ? SPEAR_VARIANT_STREAM_FUSED : SPEAR_VARIANT_STREAM_SPLIT;
+    }
     return SPEAR_VARIANT_TC_FUSED;
 }
 static int choose_variant(int M, int N, int K, int r, int group, int gate) {
@@ -277,7 +290,7 @@ static int choose_variant(int M, int N, int K, int r, int group, int gate) {
         auto it = g_plan.find(PlanKey{M, N, K, r, group, gate});
         if (it != g_plan.end()) return it->second.variant;
     }
-    return heuristic_variant(M, r, gate);
+    return heuristic_variant(M, N, K, r, gate);
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -337,37 +350,45 @@ static int ws_prepare(uint8_t* ws, size_t ws_bytes, const WsLayout& L, int M, in
     return SPEAR_OK;
 }
 
+// EC pre-kernel for M <= 16 (S4-S6: z = x [A; w_g]^T, any gate, u = alpha gamma (.) z as fp32 [M][r] in the workspace).
+static int run_ec_pre_small(const void* x, const void* A, const spear_ec_desc* ec, int M, int K, int r,
+                        uint8_t* ws, const WsLayout& L, cudaStream_t st) {
+    unsigned* counters = reinterpret_cast<unsigned*>(ws + L.counters);
+    float* u32 = reinterpret_cast<float*>(ws + L.u32);
+    const bool pdl = g_tune.pdl != 0;
+    EcPreParams e = {};
+    e.x = static_cast<const __half*>(x);
+    e.A = static_cast<const __half*>(A);
+    e.ec_int8 = ec->ec_dtype == SPEAR_EC_INT8;
+    e.A_scale = static_cast<const __half*>(ec->A_scale);
+    e.w_g = static_cast<const __half*>(ec->w_g);
+    e.b_g = static_cast<const float*>(ec->b_g);
+    e.W1 = static_cast<const __half*>(ec->W1);
+    e.b1 = static_cast<const float*>(ec->b1);
+    e.W2 = static_cast<const __half*>(ec->W2);
+    e.b2 = static_cast<const float*>(ec->b2);
+    e.zbuf = reinterpret_cast<float*>(ws + L.zbuf);
+    e.u = u32;
+    e.gate_out = static_cast<float*>(ec->gate_out);
+    e.counter = counters + kEcPreCounter;
+    e.M = M; e.K = K; e.r = r; e.h = ec->gate_hidden; e.gate_kind = ec->gate_kind;
+    e.alpha = ec->alpha;
+    const int strips = (r + (ec->gate_kind == SPEAR_GATE_SCALAR_SIGMOID ? 1 : 0) + 15) / 16;
+    const int ktiles = K / 64;
+    int target = g_tune.ecpre_ctas > 0 ? g_tune.ecpre_ctas : g_dev.num_sms;
+    int ksplit = std::max(1, std::min(ktiles / 4, target / strips));
+    e.ksplit = std::max(1, std::min(ksplit, ktiles));
+    return launch_ec_pre(e, pdl, st);
+}
+
 static int run_stream(const void* x, const void* Wq, const void* scales, const void* A, const void* B,
                       const spear_ec_desc* ec, void* y, int M, int N, int K, int r, int group,
                       uint8_t* ws, const WsLayout& L, bool fused, cudaStream_t st, const spear_tail_desc* tail = nullptr) {
     unsigned* counters = reinterpret_cast<unsigned*>(ws + L.counters);
     float* u32 = reinterpret_cast<float*>(ws + L.u32);
     const bool pdl = g_tune.pdl != 0;
-    if (r > 0 && !fused) {
-        EcPreParams e = {};
-        e.x = static_cast<const __half*>(x);
-        e.A = static_cast<const __half*>(A);
-        e.ec_int8 = ec->ec_dtype == SPEAR_EC_INT8;
-        e.A_scale = static_cast<const __half*>(ec->A_scale);
-        e.w_g = static_cast<const __half*>(ec->w_g);
-        e.b_g = static_cast<const float*>(ec->b_g);
-        e.W1 = static_cast<const __half*>(ec->W1);
-        e.b1 = static_cast<const float*>(ec->b1);
-        e.W2 = static_cast<const __half*>(ec->W2);
-        e.b2 = static_cast<const float*>(ec->b2);
-        e.zbuf = reinterpret_cast<float*>(ws + L.zbuf);
-        e.u = u32;
-        e.gate_out = static_cast<float*>(ec->gate_out);
-        e.counter = counters + kEcPreCounter;
-        e.M = M; e.K = K; e.r = r; e.h = ec->gate_hidden; e.gate_kind = ec->gate_kind;
-        e.alpha = ec->alpha;
-        const int strips = (r + (ec->gate_kind == SPEAR_GATE_SCALAR_SIGMOID ? 1 : 0) + 15) / 16;
-        const int ktiles = K / 64;
-        int target = g_tune.ecpre_ctas > 0 ? g_tune.ecpre_ctas : g_dev.num_sms;
-        int ksplit = std::max(1, std::min(ktiles / 4, target / strips));
-        e.ksplit = std::max(1, std::min(ksplit, ktiles));
-        if (int rc = launch_ec_pre(e, pdl, st)) return rc;
-    }
+    if (r > 0 && !fused)
+        if (int rc = run_ec_pre_small(x, A, ec, M, K, r, ws, L, st)) return rc;
     const int MT = M <= 8 ? 1 : 2;
     CUtensorMap xmap;
     if (int rc = get_tensor_map_x3d(x, uint64_t(M), uint64_t(K), uint32_t(8 * MT), 4, &xmap)) return rc;
@@ -443,6 +464,36 @@ static int run_stream(const void* x, const void* Wq, const void* scales, const v
         p.tail_ssq = reinterpret_cast<float*>(counters + kEcPreCounter + 64);
     }
     return launch_stream(xmap, p, MT, grid, pdl, st);
+}
+
+// M <= 16, latency-bound layers: EC pre-kernel (when r > 0) then the row-strip kernel (rows.cu): one CTA per 16 output
+// rows over the whole of K, no cross-CTA reduction, no workspace traffic besides u.
+static int run_rows(const void* x, const void* Wq, const void* scales, const void* A, const void* B,
+                    const spear_ec_desc* ec, void* y, int M, int N, int K, int r, int group,
+                    uint8_t* ws, const WsLayout& L, cudaStream_t st) {
+    // scalar / none gate: z, gate and u inside the kernel (cluster-local); the paper's MLP gate goes through the pre-kernel
+    const bool fused = r > 0 && ec->gate_kind != SPEAR_GATE_MLP;
+    if (r > 0 && !fused)
+        if (int rc = run_ec_pre_small(x, A, ec, M, K, r, ws, L, st)) return rc;
+    RowsParams p = {};
+    p.wq = Wq; p.scales = scales;
+    p.x = static_cast<const __half*>(x);
+    p.y = static_cast<__half*>(y);
+    p.u = reinterpret_cast<const float*>(ws + L.u32);
+    p.B = B;
+    if (r > 0 && ec->ec_dtype == SPEAR_EC_INT8) { p.ec_int8 = 1; p.B_scale = static_cast<const __half*>(ec->B_scale); }
+    p.M = M; p.N = N; p.K = K; p.r = r; p.G = K / group; p.group = group;
+    if (fused) {
+        p.fused = 1;
+        p.gate_kind = ec->gate_kind;
+        p.alpha = ec->alpha;
+        p.A = static_cast<const __half*>(A);
+        p.A_scale = static_cast<const __half*>(ec->A_scale);
+        p.w_g = static_cast<const __half*>(ec->w_g);
+        p.b_g = static_cast<const float*>(ec->b_g);
+        p.gate_out = static_cast<float*>(ec->gate_out);
+    }
+    return launch_rows(p, g_tune.pdl != 0, st);
 }
 
 // M > 16 (also valid for any M): EC pre-pass (z, gate, u16) then the tcgen05 GEMM whose K loop is
@@ -646,7 +697,7 @@ static int layer_impl(const void* x, const void* Wq, const void* scales, const v
     if (!variant_valid(v, M, r, gate)) {
         if (ec && ec->force_variant != SPEAR_VARIANT_AUTO)
             return set_error(SPEAR_EUNSUPPORTED, "variant %d is not valid for M=%d r=%d gate=%d", v, M, r, gate);
-        v = heuristic_variant(M, r, gate);
+        v = heuristic_variant(M, N, K, r, gate);
         if (!variant_valid(v, M, r, gate)) return set_error(SPEAR_EUNSUPPORTED, "no kernel variant for M=%d r=%d", M, r);
     }
     {
@@ -661,6 +712,21 @@ static int layer_impl(const void* x, const void* Wq, const void* scales, const v
     if (v == SPEAR_VARIANT_LSTREAM && ec_i8) {
         if (ec->force_variant != SPEAR_VARIANT_AUTO) return set_error(SPEAR_EUNSUPPORTED, "the layer-stream variant takes fp16 EC factors");
         v = (gate != SPEAR_GATE_MLP) ? SPEAR_VARIANT_STREAM_FUSED : SPEAR_VARIANT_STREAM_SPLIT;
+    }
+    if (tail) {
+        // The post-EC tail.  Only the weight-stream kernel forms y = residual + layer inside its epilogue (the thread that
+        // reads residual[m][n] is the one that writes y[m][n]); every other arm runs the layer kernel, which stores y, and
+        // THEN a row kernel that reads residual -- with residual == y the residual stream would already be overwritten.
+        const bool forced = ec && ec->force_variant != SPEAR_VARIANT_AUTO;
+        if (!forced && M <= 16 && (v == SPEAR_VARIANT_ROWS || v == SPEAR_VARIANT_LSTREAM))
+            v = (r > 0 && gate != SPEAR_GATE_MLP) ? SPEAR_VARIANT_STREAM_FUSED : SPEAR_VARIANT_STREAM_SPLIT;
+        const bool fuses_tail = (v == SPEAR_VARIANT_STREAM_FUSED || v == SPEAR_VARIANT_STREAM_SPLIT);
+        const uintptr_t y0 = uintptr_t(y), r0 = uintptr_t(tail->residual), span = size_t(M) * N * 2;
+        const bool overlap = y0 < r0 + span && r0 < y0 + span;
+        if (overlap && !(fuses_tail && y0 == r0))
+            return set_error(SPEAR_EINVAL, "spear_w4_ec_gemm_tail: residual %s y; in-place update of the residual stream (residual == y) is "
+                             "supported for M <= 16 on the weight-stream variants only (variant %d, M = %d runs the layer, then a row kernel)",
+                             y0 == r0 ? "aliases" : "partly overlaps", v, M);
     }
     if (ec_i8 && M <= 16 && (v == SPEAR_VARIANT_TC_FUSED || v == SPEAR_VARIANT_TC_SPLIT))
         return set_error(SPEAR_EUNSUPPORTED, "INT8 EC factors on the tcgen05 variants need M > 16 (workspace scratch is sized for that path)");
@@ -677,6 +743,11 @@ static int layer_impl(const void* x, const void* Wq, const void* scales, const v
             return run_stream(x, Wq, scales, A, B, ec, y, M, N, K, r, group, ws, L, true, st, tail);
         case SPEAR_VARIANT_STREAM_SPLIT:
             return run_stream(x, Wq, scales, A, B, ec, y, M, N, K, r, group, ws, L, false, st, tail);
+        case SPEAR_VARIANT_ROWS: {
+            if (int rc = run_rows(x, Wq, scales, A, B, ec, y, M, N, K, r, group, ws, L, st)) return rc;
+            return tail ? launch_tail_rows(static_cast<__half*>(y), static_cast<const __half*>(tail->residual), static_cast<const __half*>(tail->rms_weight),
+                                           static_cast<__half*>(tail->h_out), tail->eps, M, N, g_tune.pdl != 0, st) : SPEAR_OK;
+        }
         case SPEAR_VARIANT_TC_FUSED:
         case SPEAR_VARIANT_TC_SPLIT: {
             if (int rc = run_tc_fused(x, Wq, scales, A, B, ec, y, M, N, K, r, group, ws, L, v == SPEAR_VARIANT_TC_SPLIT, st)) return rc;
@@ -724,6 +795,7 @@ extern "C" int spear_tune(const char* key, int value) {
     else if (!strcmp(key, "stream_batch_grid")) g_tune.stream_batch_grid = value;
     else if (!strcmp(key, "stream_batch_units")) g_tune.stream_batch_units = value;
     else if (!strcmp(key, "stream_units")) g_tune.stream_units = value;
+    else if (!strcmp(key, "rows")) g_tune.rows = value;
     else if (!strcmp(key, "ecbig_kdiv")) g_tune.ecbig_kdiv = value;
     else return set_error(SPEAR_EINVAL, "unknown tunable '%s'", key);
     return SPEAR_OK;
@@ -1045,7 +1117,7 @@ extern "C" int spear_plan_query(int M, int N, int K, int r, int group, int gate_
     if (!variant_out) return set_error(SPEAR_EINVAL, "NULL variant_out");
     const int gk = r > 0 ? gate_kind : SPEAR_GATE_NONE;
     int v = choose_variant(M, N, K, r, group, gk);
-    if (!variant_valid(v, M, r, gk)) v = heuristic_variant(M, r, gk);
+    if (!variant_valid(v, M, r, gk)) v = heuristic_variant(M, N, K, r, gk);
     *variant_out = v;
     return SPEAR_OK;
 }
@@ -1075,7 +1147,8 @@ extern "C" int spear_plan_load(const char* path) {
     std::lock_guard<std::mutex> lock(g_plan_mutex);
     while (fgets(line, sizeof(line), f)) {
         if (line[0] == '#' || line[0] == '\n') continue;
-        PlanKey k; PlanEntry e;
+        PlanKey k; PlanEntry e = {};
+        for (int v = 0; v < SPEAR_VARIANT_COUNT; ++v) e.us[v] = -1.f;      // a row written before a variant existed is shorter
         int off = 0;
         if (sscanf(line, "%d %d %d %d %d %d %d%n", &k.M, &k.N, &k.K, &k.r, &k.group, &k.gate, &e.variant, &off) != 7) {
             fclose(f);
@@ -1084,7 +1157,7 @@ extern "C" int spear_plan_load(const char* path) {
         const char* q = line + off;
         for (int v = 0; v < SPEAR_VARIANT_COUNT; ++v) {
             int adv = 0;
-            if (sscanf(q, "%f%n", &e.us[v], &adv) != 1) { e.us[v] = -1.f; break; }
+            if (sscanf(q, "%f%n", &e.us[v], &adv) != 1) break;
             q += adv;
         }
         if (e.variant <= 0 || e.variant >= SPEAR_VARIANT_COUNT) { fclose(f); return set_error(SPEAR_EINVAL, "%s: bad variant", path); }

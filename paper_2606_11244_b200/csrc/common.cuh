@@ -189,11 +189,61 @@ __device__ __forceinline__ void cvt_i8x4_f16x2(uint32_t w, uint32_t& lo, uint32_
     asm("sub.f16x2 %0, %1, %2;" : "=r"(lo) : "r"(a), "r"(0x64806480u));
     asm("sub.f16x2 %0, %1, %2;" : "=r"(hi) : "r"(b), "r"(0x64806480u));
 }
+// ---- 16 consecutive columns of an EC factor row (or of x) as mma.sync fragment registers; NULL row = zeros ----
+__device__ __forceinline__ void ec_load16(const __half* row, int col, bool readonly, uint32_t (&lo)[4], uint32_t (&hi)[4]) {
+    if (row) {
+        uint4 a, b;
+        if (readonly) {
+            a = __ldg(reinterpret_cast<const uint4*>(row + col));
+            b = __ldg(reinterpret_cast<const uint4*>(row + col + 8));
+        } else {
+            a = *reinterpret_cast<const uint4*>(row + col);
+            b = *reinterpret_cast<const uint4*>(row + col + 8);
+        }
+        lo[0] = a.x; lo[1] = a.y; lo[2] = a.z; lo[3] = a.w;
+        hi[0] = b.x; hi[1] = b.y; hi[2] = b.z; hi[3] = b.w;
+    } else {
+#pragma unroll
+        for (int i = 0; i < 4; ++i) lo[i] = hi[i] = 0u;
+    }
+}
+
+// the same 16 columns of an INT8 factor row (16 bytes): exact conversion to the fp16 fragment registers
+__device__ __forceinline__ void ec_load16_i8(const int8_t* row, int col, uint32_t (&lo)[4], uint32_t (&hi)[4]) {
+    if (row) {
+        const uint4 a = __ldg(reinterpret_cast<const uint4*>(row + col));
+        cvt_i8x4_f16x2(a.x, lo[0], lo[1]);
+        cvt_i8x4_f16x2(a.y, lo[2], lo[3]);
+        cvt_i8x4_f16x2(a.z, hi[0], hi[1]);
+        cvt_i8x4_f16x2(a.w, hi[2], hi[3]);
+    } else {
+#pragma unroll
+        for (int i = 0; i < 4; ++i) lo[i] = hi[i] = 0u;
+    }
+}
+
 __device__ __forceinline__ uint32_t hmul2_u32(uint32_t a, uint32_t b) {
     uint32_t d;
     asm("mul.rn.f16x2 %0, %1, %2;" : "=r"(d) : "r"(a), "r"(b));
     return d;
 }
+
+// ---- thread-block clusters: rank, peer shared-memory addresses, split barrier ----
+__device__ __forceinline__ uint32_t cluster_ctarank() {
+    uint32_t r;
+    asm volatile("mov.u32 %0, %%cluster_ctarank;" : "=r"(r));
+    return r;
+}
+__device__ __forceinline__ uint32_t mapa_shared(uint32_t local_addr, uint32_t rank) {      // same offset in CTA `rank` of the cluster
+    uint32_t ra;
+    asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(ra) : "r"(local_addr), "r"(rank));
+    return ra;
+}
+__device__ __forceinline__ void st_shared_cluster_f32(uint32_t addr, float v) {
+    asm volatile("st.shared::cluster.f32 [%0], %1;" :: "r"(addr), "f"(v) : "memory");
+}
+__device__ __forceinline__ void cluster_arrive_release() { asm volatile("barrier.cluster.arrive.release.aligned;" ::: "memory"); }
+__device__ __forceinline__ void cluster_wait_acquire() { asm volatile("barrier.cluster.wait.acquire.aligned;" ::: "memory"); }
 
 // ---- legacy tensor-core MMA (decode path): D(16x8,f32) += A(16x16,f16,row) * B(16x8,f16,col) ----
 __device__ __forceinline__ void mma_m16n8k16(float (&d)[4], uint32_t a0, uint32_t a1, uint32_t a2,

@@ -54,6 +54,31 @@ int stream_fit_stages(int MT, bool deep, int r);          // deepest ring <= str
 int stream_resident_ctas(int MT, bool deep, int r);
 int launch_stream(const CUtensorMap& xmap, const StreamParams& p, int MT, int grid, bool pdl, cudaStream_t st);
 
+// ---- rows.cu (M <= 16): row-strip kernel -- one CTA per 16 output rows over the whole of K, no cross-CTA reduction ----
+struct RowsParams {
+    const void* wq;          // SPW4 packed codes
+    const void* scales;      // SPW4 packed scales
+    const __half* x;         // [M][K]
+    __half* y;               // [M][N]
+    const float* u;          // [16][r] fp32, alpha * gamma (.) z from the EC pre-kernel; unused when r == 0
+    const void* B;           // [N][r] fp16 (int8 when ec_int8)
+    const __half* B_scale;   // [N] (ec_int8)
+    int ec_int8;
+    int M, N, K, r;
+    int G;                   // K / group
+    int group;
+    // ---- fused EC (scalar / none gate): every cluster of 8 CTAs computes z = x [A; w_g]^T for itself ----
+    int fused;
+    int gate_kind;
+    float alpha;
+    const __half* A;         // [r][K] fp16 (int8 when ec_int8)
+    const __half* A_scale;   // [r] (ec_int8)
+    const __half* w_g;       // [K] (scalar gate)
+    const float* b_g;        // 1 or NULL
+    float* gate_out;         // optional [M]
+};
+int launch_rows(const RowsParams& p, bool pdl, cudaStream_t st);
+
 // ---- lstream.cu (M <= 16): persistent "layer stream" -- ONE cooperative launch consumes a table of layer
 // calls as a single queue of (call, panel, 128-column chunk) work items; int4 -> fp16 in registers -> TMEM
 // (tcgen05.st) -> tcgen05.mma with the tokens as N = 16 (A operand in tensor memory), fp32 accumulators in TMEM.

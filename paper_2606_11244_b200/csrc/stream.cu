@@ -224,38 +224,6 @@ __device__ __forceinline__ void stream_task(uint32_t w_addr, uint32_t x_addr, ui
 // the critical path.  All CTAs of the grid are co-resident (grid <= SMs x resident CTAs) and launches with an EC are
 // COOPERATIVE launches (launch_stream): the driver starts the grid only when all of its CTAs fit at once, whatever
 // else runs on the device, so the waits (this one, and a panel's head CTA for the panel's other parts) cannot deadlock.
-__device__ __forceinline__ void ec_load16(const __half* row, int col, bool readonly, uint32_t (&lo)[4], uint32_t (&hi)[4]) {
-    if (row) {
-        uint4 a, b;
-        if (readonly) {
-            a = __ldg(reinterpret_cast<const uint4*>(row + col));
-            b = __ldg(reinterpret_cast<const uint4*>(row + col + 8));
-        } else {
-            a = *reinterpret_cast<const uint4*>(row + col);
-            b = *reinterpret_cast<const uint4*>(row + col + 8);
-        }
-        lo[0] = a.x; lo[1] = a.y; lo[2] = a.z; lo[3] = a.w;
-        hi[0] = b.x; hi[1] = b.y; hi[2] = b.z; hi[3] = b.w;
-    } else {
-#pragma unroll
-        for (int i = 0; i < 4; ++i) lo[i] = hi[i] = 0u;
-    }
-}
-
-// the same 16 columns of an INT8 factor row (16 bytes): exact conversion to the fp16 fragment registers
-__device__ __forceinline__ void ec_load16_i8(const int8_t* row, int col, uint32_t (&lo)[4], uint32_t (&hi)[4]) {
-    if (row) {
-        const uint4 a = __ldg(reinterpret_cast<const uint4*>(row + col));
-        cvt_i8x4_f16x2(a.x, lo[0], lo[1]);
-        cvt_i8x4_f16x2(a.y, lo[2], lo[3]);
-        cvt_i8x4_f16x2(a.z, hi[0], hi[1]);
-        cvt_i8x4_f16x2(a.w, hi[2], hi[3]);
-    } else {
-#pragma unroll
-        for (int i = 0; i < 4; ++i) lo[i] = hi[i] = 0u;
-    }
-}
-
 // Before griddepcontrol.wait: pull this CTA's slice of [A; w_g] (the rows / K range of its phase-A tasks) into
 // L2, so that the loads after the wait do not pay an HBM round trip on the critical path.
 __device__ void ec_prefetch_factors(const StreamParams& p, int lane) {

@@ -90,11 +90,24 @@ def test_plan_table_file_roundtrip_and_heuristics_without_gpu(tmp_path):
     def query(M, N, K, r, group, gate):
         assert L.spear_plan_query(M, N, K, r, group, gate, ctypes.byref(v)) == 0
         return v.value
-    # heuristics: decode kernel up to 16 tokens (fused unless the MLP gate), tcgen05 kernel above
-    assert query(4, 2048, 2048, 16, 128, 0) == 1
-    assert query(4, 2048, 2048, 16, 128, 1) == 2
-    assert query(4, 2048, 2048, 0, 128, 0) == 2
+    # heuristics (api.cu heuristic_variant; variants: 1 stream fused, 2 stream split, 3 tcgen05, 6 row-strip).
+    # Decode, M <= 16: the row-strip kernel on latency-bound layers -- up to 4 MiB of int4 whatever the EC / gate ...
+    assert query(4, 2048, 2048, 16, 128, 0) == 6
+    assert query(4, 2048, 2048, 16, 128, 1) == 6          # MLP gate: EC pre-kernel + row-strip kernel
+    assert query(4, 2048, 2048, 0, 128, 0) == 6
+    assert query(16, 3072, 2048, 32, 128, 0) == 6         # 3 MiB, M = 16
+    # ... and plain layers up to 13 MiB at M <= 8 and N <= 8192 (down 2048 x 8192 = 8 MiB) -- each condition matters:
+    assert query(8, 2048, 8192, 0, 128, 0) == 6
+    assert query(16, 2048, 8192, 0, 128, 0) == 2          # M > 8
+    assert query(8, 2048, 8192, 32, 128, 0) == 1          # an EC above 4 MiB stays with the ring kernel
+    assert query(8, 16384, 1024, 0, 128, 0) == 2          # 8 MiB but N > 8192
+    # the ring kernel for everything larger: fused unless the MLP gate (then, and for r = 0, the split arm)
+    assert query(8, 16384, 2048, 32, 128, 0) == 1
+    assert query(8, 16384, 2048, 32, 128, 1) == 2
+    assert query(8, 16384, 2048, 0, 128, 0) == 2
+    # the tcgen05 kernel above 16 tokens, whatever the size
     assert query(64, 2048, 2048, 32, 128, 0) == 3
+    assert query(17, 2048, 2048, 0, 128, 0) == 3
     # a hand-written table overrides them and survives save -> load
     src = tmp_path / "plan.txt"
     src.write_text("# spear plan v1\n4 2048 2048 16 128 0 2 17.2 16.5 26.4 32.2 -1\n64 2048 2048 32 128 0 4 -1 -1 30.0 28.0 -1\n")

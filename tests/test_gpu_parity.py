@@ -150,6 +150,15 @@ def test_config2_llama1b_decode(sp, idx):
     check_layer(li, label=f"config2 {s.name} M={s.M}")
 
 
+@pytest.mark.parametrize("idx", range(12))
+def test_config2_plain_w4_every_shape(sp, idx):
+    """The plain-W4 leg of the bench step (r = 0), every call, through AUTO: row-strip kernel on qkv / o / down (M <= 8),
+    ring kernel on gate_up and down at M = 16."""
+    s = config_shapes(1)[idx]
+    li = make_layer(s.seed, s.M, s.N, s.K, s.group, 0, gate="none")
+    check_layer(li, label=f"config2 plain {s.name} M={s.M}")
+
+
 @pytest.mark.parametrize("idx", [0, 1, 2, 3, 4, 5])
 def test_config3_per_channel_decode(sp, idx):
     s = config_shapes(2)[idx]       # M = 1 and 16, per-channel scales (group = K)
@@ -467,9 +476,33 @@ def test_fused_tail_in_place_residual(sp):
     assert float(np.max(np.abs(hn.cpu().numpy().astype(np.float64) - h_ref))) <= Y_TOL * float(np.sqrt(np.mean(h_ref ** 2)))
 
 
+def test_fused_tail_in_place_is_refused_where_the_tail_is_not_fused(sp):
+    """residual == y only works where one thread reads residual[m][n] and writes y[m][n] (the weight-stream epilogue).
+    The two-kernel arms store y first and would then add the layer to itself: they must refuse, not return 2 * layer."""
+    import torch
+    import paper_2606_11244_b200 as sp_
+    h = _harness()
+    gw = h.dev(np.ones(512, np.float16))
+    for M, variant in ((5, sp_.VARIANT_ROWS), (5, sp_.VARIANT_LSTREAM), (40, sp_.VARIANT_AUTO)):
+        li = make_layer(305 + M, M, 512, 512, 128, 8, gate="scalar")
+        dl = h.upload_layer(li)
+        res = np.full((M, 512), 3.0, np.float16)
+        stream = h.dev(res)
+        with pytest.raises(sp_.SpearError):
+            sp_.w4_ec_gemm_tail(h.dev(li.x), dl.pw, dl.A, dl.B, dl.desc(variant=variant), stream, gw, 1e-5, y=stream)
+        torch.cuda.synchronize()
+        assert np.array_equal(stream.cpu().numpy(), res), "a refused call must not touch the residual stream"
+        # ... and the same call out of place is served, and right
+        y, hn = sp_.w4_ec_gemm_tail(h.dev(li.x), dl.pw, dl.A, dl.B, dl.desc(variant=variant), stream, gw, 1e-5)
+        torch.cuda.synchronize()
+        s_ref, h_ref = oracle.tail(oracle.forward_layer(li)["y"], res, np.ones(512, np.float16), 1e-5)
+        assert float(np.max(np.abs(y.cpu().numpy().astype(np.float64) - s_ref))) <= Y_TOL * float(np.sqrt(np.mean(s_ref ** 2)))
+        assert float(np.max(np.abs(hn.cpu().numpy().astype(np.float64) - h_ref))) <= Y_TOL * float(np.sqrt(np.mean(h_ref ** 2)))
+
+
 def test_config2_step_stream_ordered_as_bench_headline(sp):
     """The headline leg of bench.py: the 12 calls of BASELINE.json configs[1] one after the other on one stream
-    (spear_w4_ec_gemm_ex, AUTO dispatch: deep-ring weight-stream kernel with the fused EC, cooperative + PDL-chained),
+    (spear_w4_ec_gemm_ex, AUTO dispatch: row-strip kernel on qkv / o, deep-ring weight-stream kernel on gate_up / down, PDL-chained),
     captured in a CUDA graph and replayed; every call, every output element against the oracle."""
     import torch
     h = _harness()
