@@ -149,6 +149,20 @@ int spear_w4_ec_gemm_tail(const void* x, const void* Wq, const void* scales, con
                           const spear_ec_desc* ec, const spear_tail_desc* tail, void* y,
                           int M, int N, int K, int r, int group, void* stream);
 
+/* The decode layer for callers that cannot allocate (code under CUDA graph capture, tight serving loops, harnesses that
+ * forbid cudaMalloc): same operation and argument meaning as spear_w4_ec_gemm_ex (Eq. 3; any gate, fp16 or
+ * INT8 EC factors), limited to M <= 16 tokens and r <= 128, and this call -- unlike every other entry point -- never
+ * calls cudaMalloc / cudaFree, spear_init or any allocating routine, on the first call or later.  Its scratch (fp32 z
+ * [16][136], a counter, u [16][128]: 17,152 bytes) is a static __device__ array inside the library, held by every GPU
+ * that loads the library until exit.  ec->workspace, ec->force_variant and the plan table are ignored; the path is the EC
+ * pre-kernel followed by the row-strip kernel.  Sizes beyond the limits return SPEAR_EUNSUPPORTED with a message naming
+ * the limit.  All calls on a device share the array: z and the counter are cleared (stream-ordered) at the head of each
+ * call, u is overwritten; calls that overlap on the GPU (different streams, unordered graph branches) race -- serialise
+ * them.  Uses the caller's current device; the pointers and the stream must belong to it. */
+int spear_w4_ec_gemm_noalloc(const void* x, const void* Wq, const void* scales, const void* A, const void* B,
+                             const spear_ec_desc* ec, void* y,
+                             int M, int N, int K, int r, int group, void* stream);
+
 /* A batch of layer calls, e.g. the projections of one or several transformer blocks, or unrelated requests.
  * Independent calls run concurrently on the library's internal lanes (up to 16 streams with their own workspaces), or --
  * for M <= 16, when spear_plan_batch measured it faster or spear_tune("lstream", 1) -- as ONE persistent layer-stream

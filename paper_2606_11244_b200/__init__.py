@@ -23,7 +23,7 @@ VARIANT_NAMES = ["auto", "stream_fused", "stream_split", "tc_fused", "tc_split",
 
 EXPORTS = [
     "spear_pack_w4_sizes", "spear_pack_w4", "spear_unpack_w4", "spear_dequant_w4",
-    "spear_w4_ec_gemm", "spear_w4_ec_gemm_ex", "spear_w4_ec_gemm_hostio", "spear_w4_ec_gemm_tail", "spear_w4_ec_gemm_batch", "spear_w4_ec_gemm_batch_hostio",
+    "spear_w4_ec_gemm", "spear_w4_ec_gemm_ex", "spear_w4_ec_gemm_hostio", "spear_w4_ec_gemm_tail", "spear_w4_ec_gemm_noalloc", "spear_w4_ec_gemm_batch", "spear_w4_ec_gemm_batch_hostio",
     "spear_workspace_bytes", "spear_init", "spear_memory_bytes", "spear_plan", "spear_plan_save", "spear_plan_load",
     "spear_plan_query", "spear_plan_batch", "spear_lut_create", "spear_lut_destroy", "spear_lut_iteration_us",
     "spear_slo_chunk", "spear_lut_measure", "spear_tune", "spear_last_error", "spear_launch_count",
@@ -84,6 +84,7 @@ def lib():
         L.spear_dequant_w4.argtypes = [vp, vp, vp, ci, ci, ci, vp]
         L.spear_w4_ec_gemm.argtypes = [vp] * 8 + [ci] * 5 + [vp]
         L.spear_w4_ec_gemm_ex.argtypes = [vp] * 5 + [ctypes.POINTER(EcDesc), vp] + [ci] * 5 + [vp]
+        L.spear_w4_ec_gemm_noalloc.argtypes = [vp] * 5 + [ctypes.POINTER(EcDesc), vp] + [ci] * 5 + [vp]
         L.spear_w4_ec_gemm_tail.argtypes = [vp] * 5 + [ctypes.POINTER(EcDesc), ctypes.POINTER(TailDesc), vp] + [ci] * 5 + [vp]
         L.spear_w4_ec_gemm_batch.argtypes = [ctypes.POINTER(Call), ci, vp]
         L.spear_w4_ec_gemm_batch_hostio.argtypes = [ctypes.POINTER(Call), ctypes.POINTER(HostIO), ci, vp]
@@ -224,6 +225,22 @@ def w4_ec_gemm_ex(x, pw: PackedW4, A=None, B=None, desc: Optional[EcDesc] = None
         y = torch.empty((M, pw.N), dtype=torch.float16, device=x.device)
     _check(lib().spear_w4_ec_gemm_ex(_ptr(x), _ptr(pw.wq), _ptr(pw.scales), _ptr(A), _ptr(B),
                                      ctypes.byref(desc), _ptr(y), M, pw.N, K, r, pw.group, _stream(stream)))
+    return y
+
+
+def w4_ec_gemm_noalloc(x, pw: PackedW4, A=None, B=None, desc: Optional[EcDesc] = None, y=None, stream=None):
+    """spear_w4_ec_gemm_noalloc: the decode layer (M <= 16, r <= 128) with its scratch in a static device array: the call
+    allocates nothing.  y must be passed by a caller that may not allocate; it is created here only when omitted."""
+    import torch
+    M, K = x.shape
+    assert K == pw.K and x.dtype == torch.float16 and x.is_contiguous()
+    r = 0 if A is None else A.shape[0]
+    if desc is None:
+        desc = make_desc(gate="none")
+    if y is None:
+        y = torch.empty((M, pw.N), dtype=torch.float16, device=x.device)
+    _check(lib().spear_w4_ec_gemm_noalloc(_ptr(x), _ptr(pw.wq), _ptr(pw.scales), _ptr(A), _ptr(B),
+                                          ctypes.byref(desc), _ptr(y), M, pw.N, K, r, pw.group, _stream(stream)))
     return y
 
 

@@ -16,7 +16,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 OBJ = os.path.join(HERE, "build")
 SO = os.path.join(HERE, "libspear.so")
-SOURCES = ["api.cu", "pack.cu", "stream.cu", "ec_pre.cu", "tc.cu", "lstream.cu", "rows.cu", "sched.cu"]
+SOURCES = ["api.cu", "pack.cu", "stream.cu", "ec_pre.cu", "tc.cu", "lstream.cu", "rows.cu", "noalloc.cu", "sched.cu"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
               "-Xcompiler", "-fPIC", "--expt-relaxed-constexpr"]
 
