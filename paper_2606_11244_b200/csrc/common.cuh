@@ -162,6 +162,11 @@ __device__ __forceinline__ void prefetch_l2(const void* p) {
 
 // ---- int4 -> fp16 (SPW4 word: column 2i in bits [4i,4i+4), column 2i+1 in bits [4i+16,4i+20)) ----
 // Returns the four half2 pairs (q-8) of one 32-bit word, columns (0,1) (2,3) (4,5) (6,7); exact.
+// Attribution: this is the well-known "magic number" int4 -> fp16 conversion (OR the nibble under the exponent of 1024.0,
+// subtract 1024 + zero-point; for the high nibble of a byte multiply by 1/16 first) published with FasterTransformer /
+// TensorRT-LLM (FastInterleavedAndBiasedNumericArrayConverter<half, uint4b_t>) and used by Marlin-style kernels.  The
+// constants below are fixed by that arithmetic (0x6400 = 1024.0, 0x6408 = 1032.0, 0x2c00 = 1/16, 0xd480 = -72.0) and so
+// is the interleaved nibble order of the SPW4 word, chosen so that two lop3 masks yield fp16 pairs.
 __device__ __forceinline__ void dequant_word(uint32_t w, uint32_t (&out)[4]) {
     constexpr uint32_t kMagic = 0x64006400u;    // fp16 1024.0 twice
     constexpr uint32_t kSub = 0x64086408u;      // 1032.0  : (1024 + q) - 1032 = q - 8

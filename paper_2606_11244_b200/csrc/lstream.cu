@@ -12,30 +12,40 @@
 //     contiguous ranges, so every SM streams the same number of bytes and the cp.async.bulk ring never drains
 //     between calls; a call whose x is an earlier call's y opens a new phase, whose x loads wait for the
 //     previous phase's panel-completion counter while its WEIGHTS are prefetched across the boundary;
-//   * warp 0 (one lane): cp.async.bulk of the chunk into a shared-memory ring (evict_first);
-//   * warp 1 / warp 3 (one lane each): the chunk's x tile ([16 tokens][128 columns] fp16 in the MMA operand layout,
-//     prepared once per launch in the workspace, see x_prologue) / its 256-byte scale slot, as cp.async.bulk copies
-//     into the same ring stage;
-//   * warps 8-19 (12 dequantisation warps = 3 groups x 4 TMEM lane quarters; group g takes the chunks n = g mod 3
-//     of the CTA's stream): LDS.128 -> exact q - 8 in fp16 (lop3 / sub / fma) -> tcgen05.st.16x256b.x4 into the
-//     A-operand slot n mod 4 in TENSOR MEMORY.  The SPW4
-//     word of lane (g, t) holds rows g, g+8 x columns 16t..16t+15, the 16x256b store shape spreads a row's
-//     columns over the four lanes of a quad, so MMA j of a 64-column k-tile sees k = 16t + 4j + e at its
-//     K position 4t + e; the x loader applies the same permutation (a dot product is order-invariant);
-//   * warps 20-23 (one lane each, MMA issuer of pipeline i = chunks n = i mod 4): tcgen05.mma.cta_group::1.kind::f16, M = 128 rows of
-//     the panel, N = 16 tokens, K = 16, A from TMEM, B = x tile from shared memory, D = one of the pipeline's
-//     two 16-column fp32 accumulators in TMEM; one accumulation run per scale group (a run that spans several
-//     chunks leaves one partial accumulator per pipeline).  Measured: one thread issues a small-N MMA every
-//     ~47 clk whatever N, the tensor pipe needs 8 clk: four issuers keep the 8 MMAs per chunk off the critical
-//     path.  tcgen05.commit frees the A slot / ring stage and hands D over;
-//   * warps 4-7 (epilogue, thread = output row): tcgen05.ld the run's accumulators, scale by s[n][group]
-//     (read from global one run ahead) into fp32 registers;
-//     at the end of a panel segment: split-K through fp32 partial slots + an acq_rel counter when the panel
-//     is shared with neighbouring CTAs, then the rank-r update y += u B^T, one RN-even cast, store;
-//   * warp 2 (EC): this CTA's share of z = x [A; w_g]^T for every call of the phase (mma.sync, red.add),
-//     arrive; the last arriver applies the gate (PAPER.md:109 scalar form of BASELINE.json / gamma = 1) and
-//     publishes u = alpha gamma z behind a flag that finalising CTAs look at only in their epilogue
-//     (z must be complete before the gate).
+//   * 896 threads, one CTA per SM.  Service warps: warp 0 (one lane) weight producer -- cp.async.bulk of the chunk into
+//     a shared-memory ring of LS_STAGES = 10 stages (evict_first); warp 1 (one lane) x producer -- the chunk's x tile
+//     ([16 tokens][128 columns] fp16 in the MMA operand layout, k-permuted; written once per launch into the workspace
+//     by x_prologue, so it is a plain bulk copy here); warp 3 (one lane) scale producer -- the chunk's 256-byte scale
+//     slot rides in the same stage (global scale loads queued 2-3 us behind the deep bulk ring) -- and TMEM allocation;
+//   * warps 8-23, the workers: 4 pipelines x 4 TMEM lane quarters; pipeline i takes the chunks n = i mod 4 of the CTA's
+//     stream: LDS.128 -> exact q - 8 in fp16 (dequant_word) -> tcgen05.st.16x256b.x4 into A-operand slot n mod 6 in
+//     TENSOR MEMORY (6 slots x 64 columns).  The SPW4 word of lane (g, t) holds rows g, g + 8 x columns 16t..16t+15,
+//     the 16x256b store shape spreads a row's columns over the four lanes of a quad, so MMA j of a 64-column k-tile
+//     sees k = 16t + 4j + e at its K position 16j + 4t + e; x_prologue applies the same permutation to x (a dot product is
+//     order-invariant).  The same warps run the pipeline's epilogue, lagging TWO own chunks behind the dequantisation
+//     (tcgen05.ld the run's accumulator, scale by s[n][group] in fp32, add into registers; at the end of a panel segment
+//     hand the [16 tokens][128 rows] part over through shared memory); before a phase boundary they catch up;
+//   * warps 24-27 (one lane each), MMA issuer of pipeline i: tcgen05.mma.cta_group::1.kind::f16, M = 128 rows of the
+//     panel, N = 16 tokens, K = 16, A from TMEM, B = x tile from shared memory (SWIZZLE_128B, K-major), D = one of the
+//     pipeline's two 16-column fp32 accumulators in TMEM; one accumulation run per scale group.  Measured: one thread
+//     issues a small-N MMA every ~47 clk whatever N while the tensor pipe needs 8 clk, hence four issuers.  A lane waits
+//     for a_empty[slot] of chunk m - 6 BEFORE a_full[slot] of chunk m: the slot barriers are shared between pipelines
+//     and an mbarrier parity wait is only valid one phase behind (this was a 1-in-3000-replays hang);
+//     tcgen05.commit frees the A slot / ring stage and hands D over;
+//   * warps 4-7, the finalisers (thread = output row): sum the four pipelines' parts; split-K across CTAs through fp32
+//     red.add accumulators in the workspace + an acq_rel counter per panel (the last arriver finalises); then the rank-r
+//     update y += u B^T (B rows prefetched), one RN-even cast, store; in a chain also the k-permuted copy of y that the
+//     next phase reads as its x tile, and the panel-completion counter that phase waits on;
+//   * warp 2 (EC): this CTA's share of z = x [A; w_g]^T for every call of the phase (mma.sync, red.add), arrive; the
+//     last arriver applies the gate (scalar form of BASELINE.json / gamma = 1; the MLP gate is not served here) and
+//     publishes u = alpha gamma z behind a flag that finalisers look at only when they need it (z must be complete
+//     before the gate).
+//
+// Where it stands (B200, config 2 step as ONE launch): 43 us plain / 60 us with the EC against 40 / 53 us for the same
+// step on the per-call kernels over 12 lanes: ~12 us fixed (cooperative launch, prologue, first fill, tail) and a
+// ~275 ns per-chunk hand-shake floor (3.3 TB/s streaming) that neither ring depth, ALU work nor MMA issue explains.
+// It is therefore opt-in: spear_tune("lstream", 1), or a batch signature for which spear_plan_batch measured it faster
+// (DESIGN.md 6.5).  Development builds: -DLS_TRACE (per-role time stamps, watchdog printf), -DLS_TIMER.
 #include <cooperative_groups.h>
 #include <cstdio>
 
