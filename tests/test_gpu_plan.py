@@ -54,3 +54,24 @@ def test_planned_variant_matches_oracle(sp):
     ref = oracle.forward_layer(li)["y"]
     rms = float(np.sqrt(np.mean(ref ** 2)))
     assert float(np.max(np.abs(y.cpu().numpy().astype(np.float64) - ref))) <= 1e-2 * rms
+
+
+def test_lut_measure_feeds_the_chunk_selector(sp):
+    """SURVEY.md 8(f)4 end to end on the device: spear_lut_measure fills l_W4 / l_EC of one layer type from the library's own
+    timings, the LUT built from them agrees with the oracle's linear scan."""
+    from oracle import sched_oracle as so
+    grid = [1, 16, 64, 256]
+    w4, ec = sp.lut_measure(grid, 1024, 1024, 128, 32, gate="scalar")
+    assert len(w4) == len(ec) == 4 and all(t > 0 for t in w4 + ec)
+    assert all(e >= 0.5 * w for w, e in zip(w4, ec)), "an EC layer cannot be much faster than the plain one"
+    assert max(w4) < 5000 and max(ec) < 5000, "microseconds, not another unit"
+    lut = sp.Lut(grid, [w4], [ec])
+    types, sel = [0] * 8, [True, False] * 4
+    # a table entry is reproduced at its grid point (after the running maximum both sides apply)
+    mw, me = so.monotone(w4), so.monotone(ec)
+    assert abs(lut.iteration_us(types, sel, 64) - 4 * (mw[2] + me[2])) <= 1e-3 * 4 * (mw[2] + me[2])
+    t16 = lut.iteration_us(types, sel, 16)
+    for slo_factor in (1.5, 3.0, 10.0):
+        want = so.slo_chunk(grid, [w4], [ec], None, types, sel, 0, 16, 1, 512, slo_factor * t16)
+        got = lut.slo_chunk(types, sel, 16, 1, 512, slo_factor * t16)
+        assert got == want, (slo_factor, got, want)
