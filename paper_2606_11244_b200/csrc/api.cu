@@ -241,6 +241,9 @@ struct Tunables {
     int stream_units = 0;         // the same target for stream-ordered calls (0 = off: use every SM)
     int lstream = -1;             // layer-stream kernel for M <= 16: -1 = where the plan tables measured it faster (chains always), 0 = never, 1 = always
     int stream_whole_panels = 1;  // 1 = whole-panel partition when N/128 is within 1/5 of the grid
+    int stream_aligned = 1;       // 1 = panel-aligned partition for stream-ordered calls with fewer panels than SMs
+    int stream_grid = 0;          // 0 = heuristic, else the decode ring kernel's grid for stream-ordered calls (sweeps)
+    int rows_ec = 1;              // row-strip kernel's EC (scalar / none gate): 1 = z once by a one-cluster pre-kernel, 0 = z per cluster inside the layer kernel
     int rows = 1;                 // 1 = the heuristic may pick the row-strip kernel for small decode layers, 0 = never
 };
 static Tunables g_tune;
@@ -269,16 +272,16 @@ static bool variant_valid(int v, int M, int r, int gate) {
     (void)r;
 }
 // Where no plan entry exists.  Decode: the row-strip kernel (no cross-CTA reduction) on the layers whose time is the
-// latency chain, not the bytes -- measured (B200, stream-ordered, cold weights): plain layers up to 4 MiB of int4 at any
-// M <= 16 (2.1-3.8 us against 4.7-6.2), up to 13 MiB at M <= 8 (down 2048x8192: 7.3 against 8.4); with an EC up to 4 MiB
-// (5.5-9.6 us against 7.2-10.5).  Everything larger streams through the ring kernel.
+// latency chain, not the bytes -- measured (B200, stream-ordered, cold weights): up to 4 MiB of int4, any M <= 16, with or without
+// an EC (plain 2.1-3.8 us against 4.7-6.2; with an EC 5.8-8.5 against 7.2-10.5).  Everything larger streams through the ring kernel
+// (down 2048 x 8192 = 8 MiB: 6.3 us there with the panel-aligned partition, 7.3 on the row-strip kernel).
 static int heuristic_variant(int M, int N, int K, int r, int gate) {
     if (M <= 16 && g_tune.lstream == 1 && gate != SPEAR_GATE_MLP) return SPEAR_VARIANT_LSTREAM;
     if (M <= 16) {
         const size_t wbytes = size_t(N) * K / 2;
         // (not inside a batch: there whole kernels of different lanes overlap, and the ring kernel's few big CTAs share the
         // SMs better than thousands of small ones -- measured 40 vs 47 us plain, 53 vs 80 us with the EC on the 12-call step)
-        const bool rows = g_tune.rows != 0 && !t_in_batch && (wbytes <= (size_t(4) << 20) || (r == 0 && M <= 8 && wbytes <= (size_t(13) << 20) && N <= 8192));
+        const bool rows = g_tune.rows != 0 && !t_in_batch && wbytes <= (size_t(4) << 20);
         if (rows) return SPEAR_VARIANT_ROWS;
         return (r > 0 && gate != SPEAR_GATE_MLP) ? SPEAR_VARIANT_STREAM_FUSED : SPEAR_VARIANT_STREAM_SPLIT;
     }
@@ -443,6 +446,18 @@ static int run_stream(const void* x, const void* Wq, const void* scales, const v
         const int parts = (p.CP + units_target - 1) / units_target;
         grid = std::max(1, std::min(grid, n_panels * parts));
     }
+    // Fewer panels than SMs (stream-ordered call): cut every panel into the same number p of EQUAL parts, p the largest divisor of
+    // the panel's units with n_panels x p CTAs fitting -- then no CTA straddles two panels (one cross-CTA reduction per CTA instead
+    // of two, no ragged first / last segment).  Measured against the even split over all SMs: down 8192 -> 2048 (16 panels x 8 = 128
+    // CTAs) 8.3 -> 6.3 us at M = 8, 10.3 -> 8.2 at M = 16; config 3 qkv (48 x 2 = 96) 9.4 -> 9.0; config 3 down (32 x 4 = 128) 14.6 -> 13.5.
+    if (!t_in_batch && units_target == 0 && g_tune.stream_aligned && n_panels < grid && grid != n_panels) {
+        const int cap = g_dev.num_sms * per_sm;
+        int best = 0;
+        for (int parts = 1; parts <= p.CP && n_panels * parts <= cap; ++parts)
+            if (p.CP % parts == 0) best = parts;
+        if (best > 0 && n_panels * best * 5 >= cap * 3) grid = n_panels * best;
+    }
+    if (g_tune.stream_grid > 0 && !t_in_batch) grid = std::max(1, std::min(g_tune.stream_grid, std::min(p.U, g_dev.num_sms * per_sm)));
     if (fused && r > 0) {
         p.fused = 1;
         p.gate_kind = ec->gate_kind;
@@ -472,8 +487,16 @@ static int run_rows(const void* x, const void* Wq, const void* scales, const voi
                     const spear_ec_desc* ec, void* y, int M, int N, int K, int r, int group,
                     uint8_t* ws, const WsLayout& L, cudaStream_t st) {
     // scalar / none gate: z, gate and u inside the kernel (cluster-local); the paper's MLP gate goes through the pre-kernel
-    const bool fused = r > 0 && ec->gate_kind != SPEAR_GATE_MLP;
-    if (r > 0 && !fused)
+    const bool mlp = r > 0 && ec->gate_kind == SPEAR_GATE_MLP;
+    // scalar / none gate: z inside the layer kernel, recomputed by each of its N / 128 clusters ("rows_ec" 0) -- or once, by a
+    // one-cluster pre-kernel that the layer kernel overlaps under PDL (1, the default).  Measured (us per call alone, M = 1 / 8 / 16):
+    // o 2048^2 (16 clusters) 5.5 / 5.9 / 8.6 fused against 5.8 / 6.2 / 8.3; qkv 2048 -> 3072 (24 clusters) 6.6 / 7.1 / 9.6 against
+    // 5.8 / 6.4 / 8.5; gate_up (128 clusters) 32 against 14.  Inside the 12-call stream-ordered step of config 2 the pre-kernel arm
+    // wins on both (114.9 -> 111.3 us): a cluster launch of the big fused grid does not overlap its predecessor as well.
+    const bool want_pre = g_tune.rows_ec != 0;
+    const bool fused = r > 0 && !mlp && !want_pre;           // z per cluster inside the layer kernel
+    const bool pre_cluster = r > 0 && !mlp && want_pre;      // z once, by a one-cluster pre-kernel
+    if (mlp)
         if (int rc = run_ec_pre_small(x, A, ec, M, K, r, ws, L, st)) return rc;
     RowsParams p = {};
     p.wq = Wq; p.scales = scales;
@@ -483,8 +506,8 @@ static int run_rows(const void* x, const void* Wq, const void* scales, const voi
     p.B = B;
     if (r > 0 && ec->ec_dtype == SPEAR_EC_INT8) { p.ec_int8 = 1; p.B_scale = static_cast<const __half*>(ec->B_scale); }
     p.M = M; p.N = N; p.K = K; p.r = r; p.G = K / group; p.group = group;
-    if (fused) {
-        p.fused = 1;
+    if (fused || pre_cluster) {
+        p.fused = fused ? 1 : 0;
         p.gate_kind = ec->gate_kind;
         p.alpha = ec->alpha;
         p.A = static_cast<const __half*>(A);
@@ -493,6 +516,8 @@ static int run_rows(const void* x, const void* Wq, const void* scales, const voi
         p.b_g = static_cast<const float*>(ec->b_g);
         p.gate_out = static_cast<float*>(ec->gate_out);
     }
+    if (pre_cluster)
+        if (int rc = launch_ecz_cluster(p, g_tune.pdl != 0, st)) return rc;
     return launch_rows(p, g_tune.pdl != 0, st);
 }
 
@@ -796,6 +821,9 @@ extern "C" int spear_tune(const char* key, int value) {
     else if (!strcmp(key, "stream_batch_units")) g_tune.stream_batch_units = value;
     else if (!strcmp(key, "stream_units")) g_tune.stream_units = value;
     else if (!strcmp(key, "rows")) g_tune.rows = value;
+    else if (!strcmp(key, "rows_ec")) g_tune.rows_ec = value;
+    else if (!strcmp(key, "stream_grid")) g_tune.stream_grid = value;
+    else if (!strcmp(key, "stream_aligned")) g_tune.stream_aligned = value;
     else if (!strcmp(key, "ecbig_kdiv")) g_tune.ecbig_kdiv = value;
     else return set_error(SPEAR_EINVAL, "unknown tunable '%s'", key);
     return SPEAR_OK;

@@ -78,6 +78,7 @@ struct RowsParams {
     float* gate_out;         // optional [M]
 };
 int launch_rows(const RowsParams& p, bool pdl, cudaStream_t st);
+int launch_ecz_cluster(const RowsParams& p, bool pdl, cudaStream_t st);      // z, gate, u once, by one cluster of 8 CTAs -> p.u
 
 // ---- lstream.cu (M <= 16): persistent "layer stream" -- ONE cooperative launch consumes a table of layer
 // calls as a single queue of (call, panel, 128-column chunk) work items; int4 -> fp16 in registers -> TMEM

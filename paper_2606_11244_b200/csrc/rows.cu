@@ -31,6 +31,12 @@
 // workspace, no co-residency requirement beyond the cluster's own.  Price: A is read once per cluster (L2 hits after
 // the first), N / 128 times in all.
 //
+// Measured and NOT kept (round 2): a persistent form (2 CTAs per SM walking strips, first with a one-batch register look-ahead across
+// strips, then with lane-private cp.async rings of 12 k-tile slots = 96 KiB in flight per SM).  gate_up 2048 -> 16384 went 9.05 ->
+// 9.2 -> 8.4 us (the ring kernel: 7.4), small layers got 0.1-0.6 us slower.  Bytes in flight are therefore not what bounds this
+// kernel on big layers; the L1 wavefronts of the x fragment loads (8 lines per LDG.128, twice per k-tile, four times at M > 8)
+// and the legacy mma.sync rate (~3.9 clk per m16n8k16 per SM) are.
+//
 // What it costs: x is re-read by every CTA (L2 traffic 2 M / 16 times the weight bytes) and a strip of a K = 8192 layer
 // is 64 KiB through one CTA -- fine while the layer is small, wrong for the big ones, which stay with stream.cu
 // (api.cu: heuristic_variant / spear_plan decide).
@@ -316,6 +322,113 @@ __global__ void __launch_bounds__(256, 2) rows_kernel(const RowsParams p) {
         p.y[size_t(tok) * p.N + n] = __float2half_rn(v);      // S8: one RN-even cast
     }
 }
+
+// ---- z, gate and u ONCE, by one cluster of 8 CTAs (S4-S6 for the split arm of the row-strip kernel) -----------------------------
+// The fused instance above makes every cluster of the layer recompute z (N / 128 times the work, and it sits in front of
+// each CTA's main loop).  Here z = x [A; w_g]^T is computed once: CTA c of ONE cluster takes the c-th eighth of K (its
+// slice of A is requested before griddepcontrol.wait, x after), the eight partial z land in the slots of rank 0 through
+// distributed shared memory, rank 0 sums them in rank order, applies the gate (scalar / none) and writes
+// u = alpha gamma (.) z as fp32 [8 MT][r] to global memory for the layer kernel that is already running behind it under
+// programmatic dependent launch (its weight requests are in flight; it reads u after its own griddepcontrol.wait).
+template <int MT>
+__global__ void __launch_bounds__(256, 1) ecz_cluster_kernel(const RowsParams p) {
+    constexpr int kTok = 8 * MT;
+    constexpr int kSG = 2;
+    extern __shared__ float zs[];                 // [8 ranks][kTok][r + 1] (used in rank 0), then [kTok][r + 1] own partial
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int g = lane >> 2, t = lane & 3;
+    const int KT = p.K >> 6;
+    const bool scalar = (p.gate_kind == SPEAR_GATE_SCALAR_SIGMOID);
+    const int zr = p.r + 1;
+    const int strips = (p.r + (scalar ? 1 : 0) + 15) >> 4;
+    const int sgroups = (strips + kSG - 1) / kSG;
+    const uint32_t rank = cluster_ctarank();
+    const int kt0 = int(rank) * KT / 8, kt1 = (int(rank) + 1) * KT / 8;
+    const int n_items = (kt1 - kt0) * sgroups;
+    float* zmine = zs + 8 * kTok * zr;
+    pdl_launch_dependents();                      // the layer kernel may start (and request its weights) right away
+    uint32_t al[2][kSG][2][4], ah[2][kSG][2][4];  // two items in flight: [buffer][strip][row g / g + 8][k16 step]
+    float sa[2][kSG][2];
+    auto load_A = [&](int buf, int item) {
+        const int kt = kt0 + item / sgroups, s0 = (item % sgroups) * kSG;
+        const int col = kt * 64 + 16 * t;
+        const int8_t* A8 = reinterpret_cast<const int8_t*>(p.A);
+#pragma unroll
+        for (int s = 0; s < kSG; ++s)
+#pragma unroll
+            for (int hrow = 0; hrow < 2; ++hrow) {
+                const int rho = (s0 + s) * 16 + g + 8 * hrow;
+                const bool q = p.ec_int8 && rho < p.r;                 // the gate row w_g stays fp16
+                const __half* pa = rho < p.r ? p.A + size_t(rho) * p.K : (rho == p.r && scalar ? p.w_g : nullptr);
+                if (q) ec_load16_i8(A8 + size_t(rho) * p.K, col, al[buf][s][hrow], ah[buf][s][hrow]);
+                else ec_load16(pa, col, true, al[buf][s][hrow], ah[buf][s][hrow]);
+                sa[buf][s][hrow] = q ? __half2float(__ldg(p.A_scale + rho)) : 1.f;
+            }
+    };
+    for (int i = threadIdx.x; i < kTok * zr; i += 256) zmine[i] = 0.f;
+    cluster_arrive_release();                     // "this CTA runs": matched before the first peer store below
+    if (warp < n_items) load_A(0, warp);          // the factors are parameters: before the wait
+    pdl_wait();                                   // x may be the previous kernel's output
+    __syncthreads();                              // zmine is zero
+    int buf = 0;
+    for (int item = warp; item < n_items; item += 8, buf ^= 1) {
+        const int kt = kt0 + item / sgroups, s0 = (item % sgroups) * kSG;
+        uint32_t xl[MT][4], xh[MT][4];
+#pragma unroll
+        for (int mt = 0; mt < MT; ++mt)
+            ec_load16(mt * 8 + g < p.M ? p.x + size_t(mt * 8 + g) * p.K : nullptr, kt * 64 + 16 * t, false, xl[mt], xh[mt]);
+        if (item + 8 < n_items) {                 // the next item's factors are in flight while this one is consumed
+            if (buf == 0) load_A(1, item + 8); else load_A(0, item + 8);
+        }
+#pragma unroll
+        for (int bsel = 0; bsel < 2; ++bsel) {
+            if (bsel != buf) continue;
+#pragma unroll
+            for (int s = 0; s < kSG; ++s) {
+                if (s0 + s >= strips) break;
+#pragma unroll
+                for (int mt = 0; mt < MT; ++mt) {
+                    float acc[4] = {0.f, 0.f, 0.f, 0.f};
+#pragma unroll
+                    for (int jj = 0; jj < 4; ++jj)
+                        mma_m16n8k16(acc, al[bsel][s][0][jj], al[bsel][s][1][jj], ah[bsel][s][0][jj], ah[bsel][s][1][jj], xl[mt][jj], xh[mt][jj]);
+#pragma unroll
+                    for (int i = 0; i < 4; ++i) {
+                        const int rho = (s0 + s) * 16 + g + ((i & 2) ? 8 : 0);
+                        if (rho < zr) atomicAdd(zmine + (mt * 8 + 2 * t + (i & 1)) * zr + rho, sa[bsel][s][(i & 2) ? 1 : 0] * acc[i]);
+                    }
+                }
+            }
+        }
+    }
+    __syncthreads();
+    cluster_wait_acquire();                       // every CTA of the cluster has started: rank 0's shared memory may be written
+    const uint32_t slot0 = mapa_shared(smem_u32(zs + int(rank) * kTok * zr), 0);
+    for (int i = threadIdx.x; i < kTok * zr; i += 256) st_shared_cluster_f32(slot0 + 4 * i, zmine[i]);
+    cluster_arrive_release();
+    cluster_wait_acquire();                       // all eight parts are in rank 0
+    if (rank != 0) return;
+    float* zsum = zmine;
+    for (int i = threadIdx.x; i < kTok * zr; i += 256) {
+        float z = 0.f;
+#pragma unroll
+        for (int c = 0; c < 8; ++c) z += zs[c * kTok * zr + i];
+        zsum[i] = z;
+    }
+    __syncthreads();
+    if (scalar && threadIdx.x < kTok) {
+        const int m = threadIdx.x;
+        const float gam = 1.f / (1.f + expf(-(zsum[m * zr + p.r] + (p.b_g ? __ldg(p.b_g) : 0.f))));
+        zsum[m * zr + p.r] = gam;
+        if (p.gate_out && m < p.M) p.gate_out[m] = gam;
+    }
+    __syncthreads();
+    float* uo = const_cast<float*>(p.u);
+    for (int i = threadIdx.x; i < p.M * p.r; i += 256) {
+        const int m = i / p.r, j = i - m * p.r;
+        uo[i] = p.alpha * (scalar ? zsum[m * zr + p.r] : 1.f) * zsum[m * zr + j];
+    }
+}
 }  // namespace
 
 int launch_rows(const RowsParams& p, bool pdl, cudaStream_t st) {
@@ -350,6 +463,36 @@ int launch_rows(const RowsParams& p, bool pdl, cudaStream_t st) {
         if (MT == 1) SPEAR_CUDA_OK(cudaLaunchKernelEx(&cfg, rows_kernel<1, false>, p));
         else SPEAR_CUDA_OK(cudaLaunchKernelEx(&cfg, rows_kernel<2, false>, p));
     }
+    count_launch();
+    return SPEAR_OK;
+}
+
+int launch_ecz_cluster(const RowsParams& p, bool pdl, cudaStream_t st) {
+    const int MT = p.M <= 8 ? 1 : 2;
+    static std::once_flag once;
+    static cudaError_t err = cudaSuccess;
+    std::call_once(once, [&]() {
+        err = cudaFuncSetAttribute((const void*)ecz_cluster_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, 9 * 8 * 129 * 4);
+        if (err == cudaSuccess)
+            err = cudaFuncSetAttribute((const void*)ecz_cluster_kernel<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, 9 * 16 * 129 * 4);
+    });
+    SPEAR_CUDA_OK(err);
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3(8);
+    cfg.blockDim = dim3(256);
+    cfg.dynamicSmemBytes = size_t(9) * 8 * MT * (p.r + 1) * 4;
+    cfg.stream = st;
+    cudaLaunchAttribute attr[2];
+    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr[0].val.programmaticStreamSerializationAllowed = pdl ? 1 : 0;
+    attr[1].id = cudaLaunchAttributeClusterDimension;
+    attr[1].val.clusterDim.x = 8;
+    attr[1].val.clusterDim.y = 1;
+    attr[1].val.clusterDim.z = 1;
+    cfg.attrs = attr;
+    cfg.numAttrs = 2;
+    if (MT == 1) SPEAR_CUDA_OK(cudaLaunchKernelEx(&cfg, ecz_cluster_kernel<1>, p));
+    else SPEAR_CUDA_OK(cudaLaunchKernelEx(&cfg, ecz_cluster_kernel<2>, p));
     count_launch();
     return SPEAR_OK;
 }

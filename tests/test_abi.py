@@ -91,16 +91,17 @@ def test_plan_table_file_roundtrip_and_heuristics_without_gpu(tmp_path):
         assert L.spear_plan_query(M, N, K, r, group, gate, ctypes.byref(v)) == 0
         return v.value
     # heuristics (api.cu heuristic_variant; variants: 1 stream fused, 2 stream split, 3 tcgen05, 6 row-strip).
-    # Decode, M <= 16: the row-strip kernel on latency-bound layers -- up to 4 MiB of int4 whatever the EC / gate ...
+    # Decode, M <= 16: the row-strip kernel on latency-bound layers -- up to 4 MiB of int4 whatever M, the EC or the gate ...
     assert query(4, 2048, 2048, 16, 128, 0) == 6
     assert query(4, 2048, 2048, 16, 128, 1) == 6          # MLP gate: EC pre-kernel + row-strip kernel
     assert query(4, 2048, 2048, 0, 128, 0) == 6
     assert query(16, 3072, 2048, 32, 128, 0) == 6         # 3 MiB, M = 16
-    # ... and plain layers up to 13 MiB at M <= 8 and N <= 8192 (down 2048 x 8192 = 8 MiB) -- each condition matters:
-    assert query(8, 2048, 8192, 0, 128, 0) == 6
-    assert query(16, 2048, 8192, 0, 128, 0) == 2          # M > 8
-    assert query(8, 2048, 8192, 32, 128, 0) == 1          # an EC above 4 MiB stays with the ring kernel
-    assert query(8, 16384, 1024, 0, 128, 0) == 2          # 8 MiB but N > 8192
+    # ... and nothing above 4 MiB (down 2048 x 8192 = 8 MiB), whatever M or the EC
+    assert query(8, 2048, 8192, 0, 128, 0) == 2
+    assert query(16, 2048, 8192, 0, 128, 0) == 2
+    assert query(8, 2048, 8192, 32, 128, 0) == 1
+    assert query(8, 4096, 2048, 0, 128, 0) == 6           # exactly 4 MiB
+    assert query(8, 4224, 2048, 0, 128, 0) == 2           # just above
     # the ring kernel for everything larger: fused unless the MLP gate (then, and for r = 0, the split arm)
     assert query(8, 16384, 2048, 32, 128, 0) == 1
     assert query(8, 16384, 2048, 32, 128, 1) == 2
