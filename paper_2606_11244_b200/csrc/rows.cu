@@ -37,6 +37,11 @@
 // kernel on big layers; the L1 wavefronts of the x fragment loads (8 lines per LDG.128, twice per k-tile, four times at M > 8)
 // and the legacy mma.sync rate (~3.9 clk per m16n8k16 per SM) are.
 //
+// Also measured and not kept: the EC cluster INSIDE the layer kernel's grid (8 extra CTAs compute z once and raise a flag; the strips
+// poll it after their main loop, with a bounded wait and a compute-it-yourself fallback so that progress never rests on dispatch
+// order).  One launch instead of two, but slower than the one-cluster pre-kernel: qkv 7.0 / 7.4 / 8.6 us against 5.8 / 6.4 / 8.5 --
+// fence + flag + poll + reload of u is a longer chain than the PDL hand-over between two kernels.
+//
 // What it costs: x is re-read by every CTA (L2 traffic 2 M / 16 times the weight bytes) and a strip of a K = 8192 layer
 // is 64 KiB through one CTA -- fine while the layer is small, wrong for the big ones, which stay with stream.cu
 // (api.cu: heuristic_variant / spear_plan decide).
