@@ -311,7 +311,7 @@ def run_cuda(args, rank, world):
     # One CUDA graph per call of the step: that call alone, stream-ordered, once per weight copy.  The 12 graphs are replayed in
     # turn, so between two replays of one graph all the other calls' copies (677 MiB in all) have gone through L2: cold weights.
     KERNEL_OF = {sp.VARIANT_STREAM_FUSED: "spear::stream_kernel<MT,1>", sp.VARIANT_STREAM_SPLIT: "spear::stream_kernel<MT,1>",
-                 sp.VARIANT_ROWS: "spear::rows_kernel<MT,FUSED>", sp.VARIANT_LSTREAM: "spear::ls_kernel",
+                 sp.VARIANT_ROWS: "spear::rows_kernel<MT,false> (with an EC: behind spear::ecz_cluster_kernel<MT>, counted with it)", sp.VARIANT_LSTREAM: "spear::ls_kernel",
                  sp.VARIANT_TC_FUSED: "spear::tc_kernel", sp.VARIANT_TC_SPLIT: "spear::tc_kernel"}
 
     def per_call(with_ec):
