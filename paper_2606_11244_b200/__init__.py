@@ -19,7 +19,7 @@ GATE_SCALAR_SIGMOID, GATE_MLP, GATE_NONE = 0, 1, 2
 GATE_KINDS = {"scalar": GATE_SCALAR_SIGMOID, "mlp": GATE_MLP, "none": GATE_NONE}
 VARIANT_AUTO, VARIANT_STREAM_FUSED, VARIANT_STREAM_SPLIT, VARIANT_TC_FUSED, VARIANT_TC_SPLIT, VARIANT_LSTREAM, VARIANT_ROWS = range(7)
 VARIANT_COUNT = 7
-VARIANT_NAMES = ["auto", "stream_fused", "stream_split", "tc_fused", "tc_split", "lstream"]
+VARIANT_NAMES = ["auto", "stream_fused", "stream_split", "tc_fused", "tc_split", "lstream", "rows"]
 
 EXPORTS = [
     "spear_pack_w4_sizes", "spear_pack_w4", "spear_unpack_w4", "spear_dequant_w4",

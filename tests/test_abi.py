@@ -122,3 +122,16 @@ def test_plan_table_file_roundtrip_and_heuristics_without_gpu(tmp_path):
     bad = tmp_path / "bad.txt"
     bad.write_text("1 2 3\n")
     assert L.spear_plan_load(str(bad).encode()) == -1
+
+
+def test_variant_names_cover_every_variant_of_the_header():
+    """The binding's variant table must follow include/spear.h (a stale list broke plan_configs when ROWS was added)."""
+    import re
+    import paper_2606_11244_b200 as sp
+    hdr = open(os.path.join(ROOT, "include", "spear.h")).read()
+    enum = dict((m.group(1), int(m.group(2))) for m in re.finditer(r"SPEAR_VARIANT_([A-Z_]+)\s*=\s*(\d+)", hdr))
+    count = enum.pop("COUNT")
+    assert sp.VARIANT_COUNT == count == len(sp.VARIANT_NAMES)
+    for name, value in enum.items():
+        assert sp.VARIANT_NAMES[value] == name.lower(), (name, value)
+        assert getattr(sp, "VARIANT_" + name) == value
