@@ -534,3 +534,43 @@ def test_config2_step_stream_ordered_as_bench_headline(sp):
         rms = float(np.sqrt(np.mean(ref ** 2)))
         err = float(np.max(np.abs(y.cpu().numpy().astype(np.float64) - ref)))
         assert err <= Y_TOL * rms, f"config2 {s.name} M={s.M} stream-ordered: {err:.4g} > {Y_TOL} * {rms:.4g}"
+
+
+def test_stream_ordered_step_replay_stress(sp):
+    """5000 back-to-back replays of the headline step (row-strip kernel behind its one-cluster EC pre-kernel, cooperative ring
+    kernel with the fused EC, all PDL-chained): every replay must finish, the workspace state (z buffers, epoch word, split-K
+    and panel counters) must come back clean every time, and the last results must still match the oracle."""
+    import torch
+    h = _harness()
+    shapes = config_shapes(1)
+    lis = [make_layer(s.seed, s.M, s.N, s.K, s.group, s.r, gate="scalar") for s in shapes]
+    dls = [h.upload_layer(li) for li in lis]
+    xs = [h.dev(li.x) for li in lis]
+    ys = [torch.zeros((li.M, li.N), dtype=torch.float16, device="cuda:0") for li in lis]
+    ds = [dl.desc() for dl in dls]
+
+    def step():
+        for x, dl, d, y in zip(xs, dls, ds, ys):
+            sp.w4_ec_gemm_ex(x, dl.pw, dl.A, dl.B, d, y=y)
+
+    st = torch.cuda.Stream()
+    with torch.cuda.stream(st):
+        step()
+        torch.cuda.synchronize()
+        g = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(g, stream=st):
+            step()
+        for _ in range(5000):
+            g.replay()
+        torch.cuda.synchronize()
+        snap = [y.clone() for y in ys]
+        for y in ys:
+            y.zero_()
+        g.replay()
+        torch.cuda.synchronize()
+    for s, li, y, y0 in zip(shapes, lis, ys, snap):
+        ref = oracle.forward_layer(li)["y"]
+        rms = float(np.sqrt(np.mean(ref ** 2)))
+        for lab, t in (("after 5000 replays", y0), ("replay 5001 into zeroed y", y)):
+            err = float(np.max(np.abs(t.cpu().numpy().astype(np.float64) - ref)))
+            assert err <= Y_TOL * rms, f"{s.name} M={s.M} {lab}: {err:.4g} > {Y_TOL} * {rms:.4g}"
