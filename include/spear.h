@@ -257,7 +257,7 @@ int spear_lut_measure(const int* M_grid, int n_grid, int N, int K, int group, in
  * the heuristic may pick the row-strip kernel for small layers, 0 = never), "rows_ec" (the row-strip kernel's EC: 0 = z per cluster inside
  * the kernel, 1 = z once by a one-cluster pre-kernel (default)), "lstream" (-1 = the layer-stream kernel only
  * where spear_plan_batch measured it faster, 0 = never, 1 = always for M <= 16); EC pre-kernels: "ecpre_ctas", "ecbig_kdiv";
- * tcgen05 kernel: "tc_grid", "tc_cluster", "tc_ksplit", "tc_bt", "tc_xslice_mb"; all: "pdl"; batch: "batch_lanes".
+ * tcgen05 kernel: "tc_grid", "tc_cluster", "tc_ksplit", "tc_tail" (split the tiles of a small partial last wave along K), "tc_bt", "tc_xslice_mb"; all: "pdl"; batch: "batch_lanes".
  * Unknown key -> SPEAR_EINVAL.  Host-only, process-wide, not thread-safe against concurrent compute calls.  bench.py
  * echoes every override it was run with (config.spear_tune_overrides). */
 int spear_tune(const char* key, int value);

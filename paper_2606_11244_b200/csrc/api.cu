@@ -231,6 +231,7 @@ struct Tunables {
     int tc_grid = 0;              // 0 = heuristic
     int tc_cluster = 0;           // 0 = heuristic, else 1 / 2 / 4
     int tc_ksplit = 0;            // 0 = heuristic, else the tcgen05 kernel's split-K factor
+    int tc_tail = 1;              // 1 = split the tiles of a small partial last wave along K over the idle CTAs, 0 = off
     int tc_bt = 0;                // 0 = heuristic, else the tcgen05 kernel's token-tile width
     int tc_xslice_mb = 0;         // 0 = default (16), MiB of x per raster group
     int batch_lanes = 16;         // concurrent lanes of spear_w4_ec_gemm_batch (1..16); measured 12 > 8 > 4 on the 12-call step
@@ -565,6 +566,7 @@ static int run_tc_fused(const void* x, const void* Wq, const void* scales, const
     t.grid_override = g_tune.tc_grid;
     t.cluster_override = g_tune.tc_cluster;
     t.ksplit_override = g_tune.tc_ksplit;
+    t.tail_split = g_tune.tc_tail;
     t.bt_override = g_tune.tc_bt;
     t.xslice_mb = g_tune.tc_xslice_mb;
     t.partial = ws + L.partial;
@@ -822,6 +824,7 @@ extern "C" int spear_tune(const char* key, int value) {
     else if (!strcmp(key, "stream_units")) g_tune.stream_units = value;
     else if (!strcmp(key, "rows")) g_tune.rows = value;
     else if (!strcmp(key, "rows_ec")) g_tune.rows_ec = value;
+    else if (!strcmp(key, "tc_tail")) g_tune.tc_tail = value;
     else if (!strcmp(key, "stream_grid")) g_tune.stream_grid = value;
     else if (!strcmp(key, "stream_aligned")) g_tune.stream_aligned = value;
     else if (!strcmp(key, "ecbig_kdiv")) g_tune.ecbig_kdiv = value;

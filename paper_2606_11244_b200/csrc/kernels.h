@@ -185,6 +185,7 @@ struct TcProblem {
     int grid_override;
     int cluster_override;    // 0 = heuristic, else 1 / 2 / 4 CTAs sharing x tiles by TMA multicast
     int ksplit_override;     // 0 = heuristic, else the split-K factor
+    int tail_split;          // 0 = off, else: split the tiles of a small partial last wave along K over the idle CTAs
     int bt_override;         // 0 = heuristic, else the token-tile width (32 / 64 need M <= width)
     int xslice_mb;           // 0 = default: MiB of x a raster group of token tiles may cover (L2 residency)
     void* partial;           // fp32 split-K slots (workspace)

@@ -110,9 +110,11 @@ struct TcParams {
     int n_pp, n_mt;          // N / (128 * CS) panel groups (CS = cluster size), ceil(M / BT)
     int mt_group;            // token tiles per raster group (keeps the x slice L2-resident)
     int n_tiles;             // n_pp * n_mt output tiles; each is taken by one cluster (CTA rank c -> panel pp * CS + c)
-    int ksplit;              // split-K factor: a tile's weight k-blocks are shared by `ksplit` work items
-    int n_work;              // n_tiles * ksplit
-    float* partial;          // [n_tiles * CS][ksplit][BT][128] fp32, split-K partial sums (ksplit > 1)
+    int ksplit;              // split-K factor: a (split) tile's weight k-blocks are shared by `ksplit` work items
+    int n_whole;             // the first n_whole tiles are ONE work item each; the tiles behind them are split `ksplit` ways
+                             // (0 with a uniform split; with a split tail: the tiles of the last, partial wave)
+    int n_work;              // n_whole + (n_tiles - n_whole) * ksplit
+    float* partial;          // [(n_tiles - n_whole) * CS][ksplit][BT][128] fp32, split-K partial sums (ksplit > 1)
     unsigned* counters;      // [n_tiles * CS], zero between calls
 };
 
@@ -120,16 +122,23 @@ struct TcParams {
 // belong to the last split.
 struct TcWork {
     int panel, mt, ks, kb0, nw, ne;
+    int tile, nsplit;        // output tile; number of work items that share it (1 = the item owns the tile)
 };
 __device__ __forceinline__ void tile_coords(const TcParams& p, int tile, int& panel, int& mt);
 __device__ __forceinline__ TcWork get_work(const TcParams& p, int w) {
     TcWork t;
-    const int tile = w / p.ksplit;
-    t.ks = w - tile * p.ksplit;
-    tile_coords(p, tile, t.panel, t.mt);
-    t.kb0 = int((long long)t.ks * p.kb_w / p.ksplit);
-    t.nw = int((long long)(t.ks + 1) * p.kb_w / p.ksplit) - t.kb0;
-    t.ne = (t.ks == p.ksplit - 1) ? p.kb_ec : 0;
+    if (w < p.n_whole) {
+        t.tile = w; t.ks = 0; t.nsplit = 1;
+    } else {
+        const int idx = w - p.n_whole;
+        t.tile = p.n_whole + idx / p.ksplit;
+        t.ks = idx - (t.tile - p.n_whole) * p.ksplit;
+        t.nsplit = p.ksplit;
+    }
+    tile_coords(p, t.tile, t.panel, t.mt);
+    t.kb0 = int((long long)t.ks * p.kb_w / t.nsplit);
+    t.nw = int((long long)(t.ks + 1) * p.kb_w / t.nsplit) - t.kb0;
+    t.ne = (t.ks == t.nsplit - 1) ? p.kb_ec : 0;
     return t;
 }
 
@@ -304,7 +313,7 @@ tc_kernel(const __grid_constant__ CUtensorMap xmap, const __grid_constant__ CUte
             const int n = panel * 128 + nl;
             const int m0 = t.mt * BT;
             __half* yp = p.y + size_t(m0) * p.N + n;
-            if (p.ksplit == 1) {
+            if (t.nsplit == 1) {
 #pragma unroll 1
                 for (int c = 0; c < BT; c += 32) {
                     if (m0 + c >= p.M) break;       // warp-uniform: nothing left in this tile
@@ -321,8 +330,8 @@ tc_kernel(const __grid_constant__ CUtensorMap xmap, const __grid_constant__ CUte
             } else {
                 // split-K: park the fp32 partial, the last of the tile's `ksplit` work items to arrive sums them
                 // in split order, casts once and stores y (same pattern as the decode kernel's panels)
-                const int out_id = (w / p.ksplit) * CS + cta_rank;
-                float* slots = p.partial + size_t(out_id) * p.ksplit * (BT * 128);
+                const int out_id = t.tile * CS + cta_rank;                          // counter of this (tile, rank)
+                float* slots = p.partial + size_t((t.tile - p.n_whole) * CS + cta_rank) * p.ksplit * (BT * 128);
                 float* mine = slots + size_t(t.ks) * (BT * 128);
 #pragma unroll 1
                 for (int c = 0; c < BT; c += 32) {
@@ -525,11 +534,29 @@ int run_tc(const TcProblem& t, cudaStream_t st) {
         if (p.n_tiles > t.max_counters || !t.partial || !t.counters) ks = 1;
     }
     if (t.ksplit_override > 0) ks = std::max(1, std::min(t.ksplit_override, p.kb_w));
-    if (ks > 1 && CS > 1) ks = 1;       // split-K slots are indexed per tile, the cluster variant per (tile, rank): never both
-    if (ks > 1 && (size_t(p.n_tiles) * CS * ks * BT * 128 * 4 > t.partial_bytes || p.n_tiles * CS > t.max_counters))
+    if (ks > 1 && CS > 1) ks = 1;       // a uniform split is for problems with fewer tiles than SMs; clusters are for many tiles
+    p.n_whole = 0;
+    // Partial last wave (e.g. 224 cluster-tiles on 74 clusters = 3.03 waves: the 4th round keeps 2 clusters busy and 72 idle):
+    // the tiles of that round are split along K over the idle clusters, `ks` ways each, so the round lasts 1 / ks of a tile.
+    // Only when the tail is small (<= half a wave) and a share keeps >= 32 k-tiles (a split must pay for its reduction).
+    if (ks == 1 && t.tail_split != 0 && t.partial && t.counters) {
+        const int slots = std::max(1, device_info().num_sms / CS);
+        const int rem = p.n_tiles % slots;
+        // ... and only for a few waves: with many (M >= 2048 on the big layers) the CTAs drift apart, the "last wave" is no longer a
+        // wave, and the split costs 5-9 % (measured: M = 4096 config 4 1237 -> 1121 TFLOP/s; M = 512 1031 -> 1079, M = 1024 1168 -> 1179)
+        if (p.n_tiles > slots && (p.n_tiles <= 8 * slots || t.tail_split == 2) && rem > 0 && 2 * rem <= slots) {
+            int kt = std::min(std::min(slots / rem, std::max(1, p.kb_w * KT / 32)), 16);
+            while (kt > 1 && size_t(rem) * CS * kt * BT * 128 * 4 > t.partial_bytes) --kt;
+            if (kt > 1 && p.n_tiles * CS <= t.max_counters) {
+                ks = kt;
+                p.n_whole = p.n_tiles - rem;
+            }
+        }
+    }
+    if (ks > 1 && (size_t(p.n_tiles - p.n_whole) * CS * ks * BT * 128 * 4 > t.partial_bytes || p.n_tiles * CS > t.max_counters))
         return set_error(SPEAR_ENOMEM, "tc split-K %d needs more workspace", ks);
     p.ksplit = ks;
-    p.n_work = p.n_tiles * ks;
+    p.n_work = p.n_whole + (p.n_tiles - p.n_whole) * ks;
     p.partial = static_cast<float*>(t.partial);
     p.counters = t.counters;
     CUtensorMap xmap, umap, bmap;

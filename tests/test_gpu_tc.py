@@ -305,3 +305,20 @@ def test_single_call_hostio(sp):
         ref = oracle.forward_layer(li)["y"]
         rms = float(np.sqrt(np.mean(ref ** 2)))
         assert float(np.max(np.abs(yh.numpy().astype(np.float64) - ref))) <= Y_TOL * rms
+
+
+@pytest.mark.parametrize("M,r", [(256, 32), (512, 0), (512, 64)])
+def test_split_tail_of_a_partial_last_wave(sp, M, r):
+    """150 panels: one more wave than the 148 SMs (M = 256, single CTAs: 150 tiles) or than the 74 CTA pairs (M = 512, clusters
+    of 2: 150 cluster tiles) hold -- the 2 tiles of the last, nearly empty wave are split along K over idle CTAs (fp32 partial
+    slots + last-arriver sum, also with the cluster variant and with the EC k-blocks riding on the last share).  Sampled rows
+    against the oracle, with the split on and off, and twice in a row (the tile counters must come back to zero)."""
+    N, K = 128 * 150, 4096
+    li = make_layer(700 + M + r, M, N, K, 128, r, gate="scalar")
+    rows = np.array(sorted({0, 1, M - 1, M // 2, 255, min(256, M - 1)}))
+    try:
+        for tail in (1, 1, 0):
+            sp.tune("tc_tail", tail)
+            check(li, variant=0, rows=rows, label=f"split tail={tail} M={M} r={r}")
+    finally:
+        sp.tune("tc_tail", 1)
