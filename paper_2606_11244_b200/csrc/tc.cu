@@ -358,16 +358,23 @@ tc_kernel(const __grid_constant__ CUtensorMap xmap, const __grid_constant__ CUte
                 if (tmem_slot[1]) {
                     __threadfence();
                     const int rows = min(BT, p.M - m0);
-                    for (int mm = 0; mm < rows; mm += 4) {
-                        float sum[4] = {0.f, 0.f, 0.f, 0.f};
+                    // 16 token rows per pass: every load of a pass is issued before the first add, so that 16 L2 round trips
+                    // overlap (with 4 the sum of a 128-token tile took ~10 us per share and made a 2-way split a loss)
+                    constexpr int kRows = 16;
+                    for (int mm = 0; mm < rows; mm += kRows) {
+                        float sum[kRows];
+#pragma unroll
+                        for (int u = 0; u < kRows; ++u) sum[u] = 0.f;
                         for (int ks = 0; ks < p.ksplit; ++ks) {
                             const float* sk = slots + size_t(ks) * (BT * 128) + nl;
+                            float v[kRows];
 #pragma unroll
-                            for (int u = 0; u < 4; ++u)
-                                if (mm + u < rows) sum[u] += __ldcg(sk + (mm + u) * 128);
+                            for (int u = 0; u < kRows; ++u) v[u] = (mm + u < rows) ? __ldcg(sk + (mm + u) * 128) : 0.f;
+#pragma unroll
+                            for (int u = 0; u < kRows; ++u) sum[u] += v[u];
                         }
 #pragma unroll
-                        for (int u = 0; u < 4; ++u)
+                        for (int u = 0; u < kRows; ++u)
                             if (mm + u < rows) yp[size_t(mm + u) * p.N] = __float2half_rn(sum[u]);
                     }
                 }
@@ -529,7 +536,15 @@ int run_tc(const TcProblem& t, cudaStream_t st) {
     // split-K when there are fewer output tiles than SMs (mid-M on small layers): work items = tiles x ksplit
     int ks = 1;
     if (CS == 1 && p.n_tiles < device_info().num_sms) {
-        ks = std::min(std::min(device_info().num_sms / p.n_tiles, std::max(1, p.kb_w * KT / 32)), 16);   // measured: a split must keep >= 32 k-tiles to pay for its reduction
+        // A share saves K-loop time (one ~0.45 us barrier round trip per stage) and pays for parking and re-reading fp32 partials
+        // (~0.035 us per token row of the tile and per share, measured): take the factor that minimises the sum.  E.g. 128 tokens,
+        // 4096 -> 6144: no split (23.4 us; 2-way 25.2); 64 tokens, 8192 -> 2048: 4-way (20.7 us; none 33.7, 2-way 24.6).
+        const int ks_max = std::min(std::min(device_info().num_sms / p.n_tiles, p.kb_w), 16);
+        double best_t = 0.45 * p.kb_w;
+        for (int c = 2; c <= ks_max; ++c) {
+            const double tc_us = 0.45 * p.kb_w / c + 0.035 * BT * c;
+            if (tc_us < best_t) { best_t = tc_us; ks = c; }
+        }
         while (ks > 1 && size_t(p.n_tiles) * ks * BT * 128 * 4 > t.partial_bytes) --ks;
         if (p.n_tiles > t.max_counters || !t.partial || !t.counters) ks = 1;
     }
