@@ -266,8 +266,8 @@ static bool variant_valid(int v, int M, int r, int gate) {
         case SPEAR_VARIANT_STREAM_SPLIT: return M <= 16;
         case SPEAR_VARIANT_LSTREAM: return M <= 16 && gate != SPEAR_GATE_MLP;      // (+ group shape, checked in layer_impl)
         case SPEAR_VARIANT_ROWS: return M <= 16;
-        case SPEAR_VARIANT_TC_FUSED: return tc_available() && M >= 1;
-        case SPEAR_VARIANT_TC_SPLIT: return tc_available() && r > 0;
+        case SPEAR_VARIANT_TC_FUSED: return M >= 1;
+        case SPEAR_VARIANT_TC_SPLIT: return r > 0;
         default: return false;
     }
     (void)r;

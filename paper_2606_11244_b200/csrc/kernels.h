@@ -193,7 +193,6 @@ struct TcProblem {
     unsigned* counters;      // zero between calls
     int max_counters;
 };
-bool tc_available();
 int run_tc(const TcProblem& t, cudaStream_t st);
 
 }  // namespace spear

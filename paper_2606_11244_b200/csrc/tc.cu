@@ -457,7 +457,6 @@ tc_kernel(const __grid_constant__ CUtensorMap xmap, const __grid_constant__ CUte
 }
 
 // ---- host side -----------------------------------------------------------------------------------
-bool tc_available() { return true; }
 
 template <int BT, int CS>
 static int launch_tc(const CUtensorMap& xmap, const CUtensorMap& umap, const CUtensorMap& bmap, const TcParams& p,
