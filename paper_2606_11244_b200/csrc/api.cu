@@ -552,7 +552,7 @@ static int run_tc_fused(const void* x, const void* Wq, const void* scales, const
         e.gate_out = static_cast<float*>(ec->gate_out);
         e.M = M; e.K = K; e.r = r; e.h = ec->gate_hidden; e.gate_kind = ec->gate_kind;
         e.alpha = ec->alpha;
-        const int mtiles = (M + 63) / 64, ktiles = K / 64;
+        const int mtiles = (M + 127) / 128, ktiles = K / 64;
         int target = (g_tune.ecpre_ctas > 0 ? g_tune.ecpre_ctas : 2 * g_dev.num_sms);
         int ksplit = std::max(1, target / mtiles);
         e.ksplit = std::max(1, std::min(ksplit, ktiles / (g_tune.ecbig_kdiv > 0 ? g_tune.ecbig_kdiv : 2)));

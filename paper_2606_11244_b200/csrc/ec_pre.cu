@@ -243,44 +243,79 @@ int launch_ec_pre(const EcPreParams& p, bool pdl, cudaStream_t st) {
 // M > 16: z = x [A; w_g]^T as a split-K mma.sync GEMM (tokens are the 16-row operand here), then a
 // gate kernel per 16 tokens.  Cost is r/N of the main GEMM (SURVEY.md section 7 "Prefill EC fold").
 // ------------------------------------------------------------------------------------------------
+// A CTA of 8 warps takes 128 tokens (16 per warp) x every row of [A; w_g] x one K slice.  Per 64-column k-tile the block of
+// [A; w_g] (NT x 8 rows x 128 bytes) is staged ONCE per CTA in shared memory by cp.async (three stages in flight) and read by all
+// 8 warps; the x fragments are each warp's own and come straight from global memory.  (The first version let every warp fetch its
+// A fragments from global memory: at M = 2048, K = 14336, r = 64 that is 128 warps x 1.8 MB through L2 -- 74 us on a 210 us layer.)
+constexpr int kEzRowBytes = 144;      // 128 bytes of a k-tile row + 16 bytes of padding: the 8 rows x 4 column groups of a quarter-warp hit distinct banks
+constexpr int kEzStages = 3;
+
 template <int NT>   // NT = number of 8-row tiles of [A; w_g] (rows beyond r [+1] read as zero)
-__global__ void __launch_bounds__(128) ec_big_z_kernel(const EcBigParams p) {
+__global__ void __launch_bounds__(256) ec_big_z_kernel(const EcBigParams p) {
+    extern __shared__ __align__(16) uint8_t ez_smem[];      // [kEzStages][NT * 8][kEzRowBytes]
+    constexpr int kStageBytes = NT * 8 * kEzRowBytes;
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int g = lane >> 2, t = lane & 3;
     const bool scalar = (p.gate_kind == SPEAR_GATE_SCALAR_SIGMOID);
     const int rows_total = p.r + (scalar ? 1 : 0);
-    const int m0 = blockIdx.x * 64 + warp * 16;
-    pdl_launch_dependents();
-    if (m0 >= p.M) { pdl_wait(); return; }
-    const __half* px0 = (m0 + g) < p.M ? p.x + size_t(m0 + g) * p.K : nullptr;
-    const __half* px1 = (m0 + g + 8) < p.M ? p.x + size_t(m0 + g + 8) * p.K : nullptr;
-    const __half* pa[NT];
-#pragma unroll
-    for (int nt = 0; nt < NT; ++nt) {
-        const int rho = nt * 8 + g;
-        pa[nt] = rho < p.r ? p.A + size_t(rho) * p.K : (rho == p.r && scalar ? p.w_g : nullptr);
-    }
+    const int m0 = blockIdx.x * 128 + warp * 16;
     const int ktiles = p.K >> 6;
     const int kt_begin = int((long long)blockIdx.y * ktiles / p.ksplit);
     const int kt_end = int((long long)(blockIdx.y + 1) * ktiles / p.ksplit);
+    const int n_kt = kt_end - kt_begin;
+    pdl_launch_dependents();
+    // rows beyond [A; w_g] stay zero in every stage
+    for (int i = threadIdx.x; i < kEzStages * NT * 8; i += 256) {
+        const int row = i % (NT * 8);
+        if (row >= rows_total) {
+            uint4* dst = reinterpret_cast<uint4*>(ez_smem + size_t(i / (NT * 8)) * kStageBytes + row * kEzRowBytes);
+#pragma unroll
+            for (int q = 0; q < 8; ++q) dst[q] = make_uint4(0u, 0u, 0u, 0u);
+        }
+    }
+    auto stage_in = [&](int j) {        // k-tile kt_begin + j -> stage j % kEzStages (one commit group, possibly empty)
+        if (j < n_kt) {
+            const int kt = kt_begin + j;
+            uint8_t* st = ez_smem + size_t(j % kEzStages) * kStageBytes;
+            for (int i = threadIdx.x; i < rows_total * 8; i += 256) {
+                const int row = i >> 3, pc = i & 7;
+                const __half* src = row < p.r ? p.A + size_t(row) * p.K : p.w_g;
+                const uint32_t dst = smem_u32(st + row * kEzRowBytes + pc * 16);
+                asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(dst), "l"(src + kt * 64 + pc * 8) : "memory");
+            }
+        }
+        asm volatile("cp.async.commit_group;" ::: "memory");
+    };
+    // [A; w_g] are parameters: the first stages are requested before griddepcontrol.wait
+    for (int j = 0; j < kEzStages - 1; ++j) stage_in(j);
+    const __half* px0 = (m0 + g) < p.M ? p.x + size_t(m0 + g) * p.K : nullptr;
+    const __half* px1 = (m0 + g + 8) < p.M ? p.x + size_t(m0 + g + 8) * p.K : nullptr;
     float acc[NT][4];
 #pragma unroll
     for (int nt = 0; nt < NT; ++nt) acc[nt][0] = acc[nt][1] = acc[nt][2] = acc[nt][3] = 0.f;
     pdl_wait();
-    for (int kt = kt_begin; kt < kt_end; ++kt) {
-        const int col = kt * 64 + 16 * t;
+    for (int j = 0; j < n_kt; ++j) {
+        const int col = (kt_begin + j) * 64 + 16 * t;
         uint32_t x0l[4], x0h[4], x1l[4], x1h[4];
         load_x32(px0, col, x0l, x0h);
         load_x32(px1, col, x1l, x1h);
+        asm volatile("cp.async.wait_group %0;" ::"n"(kEzStages - 2) : "memory");      // this thread's pieces of stage j have landed
+        __syncthreads();                                     // ... and everybody's; everybody is also done with stage j - 1
+        stage_in(j + kEzStages - 1);                         // refill the stage read in iteration j - 1
+        const uint8_t* st = ez_smem + size_t(j % kEzStages) * kStageBytes + g * kEzRowBytes + t * 32;
+        if (m0 < p.M) {
 #pragma unroll
-        for (int nt = 0; nt < NT; ++nt) {
-            uint32_t al[4], ah[4];
-            load_row32(pa[nt], col, al, ah);
-#pragma unroll
-            for (int jj = 0; jj < 4; ++jj)
-                mma_m16n8k16(acc[nt], x0l[jj], x1l[jj], x0h[jj], x1h[jj], al[jj], ah[jj]);
+            for (int nt = 0; nt < NT; ++nt) {
+                const uint4 lo = *reinterpret_cast<const uint4*>(st + nt * 8 * kEzRowBytes);
+                const uint4 hi = *reinterpret_cast<const uint4*>(st + nt * 8 * kEzRowBytes + 16);
+                mma_m16n8k16(acc[nt], x0l[0], x1l[0], x0h[0], x1h[0], lo.x, hi.x);
+                mma_m16n8k16(acc[nt], x0l[1], x1l[1], x0h[1], x1h[1], lo.y, hi.y);
+                mma_m16n8k16(acc[nt], x0l[2], x1l[2], x0h[2], x1h[2], lo.z, hi.z);
+                mma_m16n8k16(acc[nt], x0l[3], x1l[3], x0h[3], x1h[3], lo.w, hi.w);
+            }
         }
     }
+    if (m0 >= p.M) return;
     // C fragment: rows = tokens g, g+8; columns = EC rows nt*8 + 2t, +1
 #pragma unroll
     for (int nt = 0; nt < NT; ++nt) {
@@ -325,6 +360,12 @@ __global__ void __launch_bounds__(128) ec_big_gate_kernel(const EcBigParams p) {
 
 template <int NT>
 static int launch_ec_big_z(const EcBigParams& p, cudaLaunchConfig_t& cfg) {
+    constexpr int kBytes = kEzStages * NT * 8 * kEzRowBytes;      // <= 58,752 B (NT = 17)
+    static std::once_flag once;
+    static cudaError_t err = cudaSuccess;
+    std::call_once(once, [] { err = cudaFuncSetAttribute(ec_big_z_kernel<NT>, cudaFuncAttributeMaxDynamicSharedMemorySize, kBytes); });
+    SPEAR_CUDA_OK(err);
+    cfg.dynamicSmemBytes = kBytes;
     SPEAR_CUDA_OK(cudaLaunchKernelEx(&cfg, ec_big_z_kernel<NT>, p));
     return SPEAR_OK;
 }
@@ -333,8 +374,8 @@ int launch_ec_big(const EcBigParams& p, bool pdl, cudaStream_t st) {
     const bool scalar = (p.gate_kind == SPEAR_GATE_SCALAR_SIGMOID);
     const int nt = (p.r + (scalar ? 1 : 0) + 7) / 8;
     cudaLaunchConfig_t cfg = {};
-    cfg.gridDim = dim3((p.M + 63) / 64, p.ksplit);
-    cfg.blockDim = dim3(128);
+    cfg.gridDim = dim3((p.M + 127) / 128, p.ksplit);
+    cfg.blockDim = dim3(256);
     cfg.stream = st;
     cudaLaunchAttribute attr[1];
     attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
@@ -349,6 +390,8 @@ int launch_ec_big(const EcBigParams& p, bool pdl, cudaStream_t st) {
     else rc = launch_ec_big_z<17>(p, cfg);
     if (rc) return rc;
     cfg.gridDim = dim3((p.M + 15) / 16);
+    cfg.blockDim = dim3(128);
+    cfg.dynamicSmemBytes = 0;
     SPEAR_CUDA_OK(cudaLaunchKernelEx(&cfg, ec_big_gate_kernel, p));
     count_launch(2);
     return SPEAR_OK;
