@@ -247,6 +247,8 @@ int launch_ec_pre(const EcPreParams& p, bool pdl, cudaStream_t st) {
 // [A; w_g] (NT x 8 rows x 128 bytes) is staged ONCE per CTA in shared memory by cp.async (three stages in flight) and read by all
 // 8 warps; the x fragments are each warp's own and come straight from global memory.  (The first version let every warp fetch its
 // A fragments from global memory: at M = 2048, K = 14336, r = 64 that is 128 warps x 1.8 MB through L2 -- 74 us on a 210 us layer.)
+// (Measured and not kept: applying the scalar gate in this kernel's last arriver per 128-token block instead of the separate gate
+// kernel -- fence + counter + a serial tail in one CTA cost more than the launch they save: M = 256, 4096 -> 6144 36 -> 41 us.)
 constexpr int kEzRowBytes = 144;      // 128 bytes of a k-tile row + 16 bytes of padding: the 8 rows x 4 column groups of a quarter-warp hit distinct banks
 constexpr int kEzStages = 3;
 
