@@ -66,7 +66,7 @@ typedef enum {
     SPEAR_VARIANT_LSTREAM = 5,       /* persistent layer-stream kernel (tcgen05, weights through TMEM), EC fused; M <= 16,
                                         scalar / none gate; also what spear_w4_ec_gemm_batch runs for such calls */
     SPEAR_VARIANT_ROWS = 6,          /* EC pre-kernel (r > 0) + row-strip kernel: one CTA per 16 output rows over the whole of K, no
-                                        cross-CTA reduction; M <= 16, the latency-bound (small) layers */
+                                        cross-CTA reduction; M <= 16 on the latency-bound (small) layers, and a 32-token form for 17..64 tokens (fp16 EC factors) */
     SPEAR_VARIANT_COUNT = 7
 } spear_variant;
 
@@ -254,7 +254,7 @@ int spear_lut_measure(const int* M_grid, int n_grid, int N, int K, int group, in
 /* Sweep hook: sets a launch tunable.  Every knob preserves results (it moves work between kernels, grids or streams, never
  * changes what is computed).  Decode ring kernel: "stream_ctas_per_sm", "stream_deep" (-1 heuristic, 0 / 1 shallow / deep
  * ring), "stream_whole_panels", "stream_aligned", "stream_grid", "stream_batch_grid", "stream_batch_units", "stream_units"; decode kernel choice: "rows" (1 =
- * the heuristic may pick the row-strip kernel for small layers, 0 = never), "rows_ec" (the row-strip kernel's EC: 0 = z per cluster inside
+ * the heuristic may pick the row-strip kernel for small layers, 0 = never), "rows_mid" (1 = the heuristic may pick its 32-token form for 17..64 tokens), "rows_ec" (the row-strip kernel's EC: 0 = z per cluster inside
  * the kernel, 1 = z once by a one-cluster pre-kernel (default)), "lstream" (-1 = the layer-stream kernel only
  * where spear_plan_batch measured it faster, 0 = never, 1 = always for M <= 16); EC pre-kernels: "ecpre_ctas", "ecbig_kdiv";
  * tcgen05 kernel: "tc_grid", "tc_cluster", "tc_ksplit", "tc_tail" (split the tiles of a small partial last wave along K), "tc_bt", "tc_xslice_mb"; all: "pdl"; batch: "batch_lanes".

@@ -244,6 +244,7 @@ struct Tunables {
     int stream_whole_panels = 1;  // 1 = whole-panel partition when N/128 is within 1/5 of the grid
     int stream_aligned = 1;       // 1 = panel-aligned partition for stream-ordered calls with fewer panels than SMs
     int stream_grid = 0;          // 0 = heuristic, else the decode ring kernel's grid for stream-ordered calls (sweeps)
+    int rows_mid = 1;             // 1 = the heuristic may pick the strip kernel's 32-token form for 17..64 tokens on small layers
     int rows_ec = 1;              // row-strip kernel's EC (scalar / none gate): 1 = z once by a one-cluster pre-kernel, 0 = z per cluster inside the layer kernel
     int rows = 1;                 // 1 = the heuristic may pick the row-strip kernel for small decode layers, 0 = never
 };
@@ -265,7 +266,7 @@ static bool variant_valid(int v, int M, int r, int gate) {
         case SPEAR_VARIANT_STREAM_FUSED: return M <= 16 && r > 0 && gate != SPEAR_GATE_MLP;
         case SPEAR_VARIANT_STREAM_SPLIT: return M <= 16;
         case SPEAR_VARIANT_LSTREAM: return M <= 16 && gate != SPEAR_GATE_MLP;      // (+ group shape, checked in layer_impl)
-        case SPEAR_VARIANT_ROWS: return M <= 16;
+        case SPEAR_VARIANT_ROWS: return M <= 64;      // (17..64 tokens: fp16 EC factors only, checked in layer_impl)
         case SPEAR_VARIANT_TC_FUSED: return M >= 1;
         case SPEAR_VARIANT_TC_SPLIT: return r > 0;
         default: return false;
@@ -286,6 +287,11 @@ static int heuristic_variant(int M, int N, int K, int r, int gate) {
         if (rows) return SPEAR_VARIANT_ROWS;
         return (r > 0 && gate != SPEAR_GATE_MLP) ? SPEAR_VARIANT_STREAM_FUSED : SPEAR_VARIANT_STREAM_SPLIT;
     }
+    // 17..64 tokens on small layers: the strip kernel's 32-token form (the tcgen05 kernel has a ~9-12 us floor on a 2048-column layer)
+    // measured (us, M = 64 / 32 / 17): 2048 -> 3072 10.1 / 7.2 / - against 12.3 / 10.5 / -; 2048 -> 2048 7.2 / - / 5.3 against 12.2 / - / 9.6;
+    // above 4 MiB of int4 it loses (8192 -> 2048 at M = 32: 16.2 against 15.1; 4096 -> 6144 at M = 48: 23.8 against 15.5)
+    // (not inside a batch: the config-5 stack on 16 lanes went 369 -> 471 us with it -- many small CTAs crowd the lanes out)
+    if (M <= 64 && g_tune.rows_mid != 0 && !t_in_batch && size_t(N) * K / 2 <= (size_t(4) << 20)) return SPEAR_VARIANT_ROWS;
     return SPEAR_VARIANT_TC_FUSED;
 }
 static int choose_variant(int M, int N, int K, int r, int group, int gate) {
@@ -482,11 +488,48 @@ static int run_stream(const void* x, const void* Wq, const void* scales, const v
     return launch_stream(xmap, p, MT, grid, pdl, st);
 }
 
+// EC pre-pass for M > 16 (S4-S6): z = x [A; w_g]^T as a split-K GEMM, gate kernel, u = alpha gamma (.) z as fp16 [M][r] at ws + L.u16.
+static int run_ec_big(const void* x, const void* A, const spear_ec_desc* ec, int M, int K, int r,
+                      uint8_t* ws, const WsLayout& L, bool pdl, cudaStream_t st) {
+    EcBigParams e = {};
+    e.x = static_cast<const __half*>(x);
+    e.A = static_cast<const __half*>(A);
+    e.w_g = static_cast<const __half*>(ec->w_g);
+    e.b_g = static_cast<const float*>(ec->b_g);
+    e.W1 = static_cast<const __half*>(ec->W1);
+    e.b1 = static_cast<const float*>(ec->b1);
+    e.W2 = static_cast<const __half*>(ec->W2);
+    e.b2 = static_cast<const float*>(ec->b2);
+    e.zbuf = reinterpret_cast<float*>(ws + L.zbuf);
+    e.u16 = reinterpret_cast<__half*>(ws + L.u16);
+    e.gate_out = static_cast<float*>(ec->gate_out);
+    e.M = M; e.K = K; e.r = r; e.h = ec->gate_hidden; e.gate_kind = ec->gate_kind;
+    e.alpha = ec->alpha;
+    const int mtiles = (M + 127) / 128, ktiles = K / 64;
+    int target = (g_tune.ecpre_ctas > 0 ? g_tune.ecpre_ctas : 2 * g_dev.num_sms);
+    int ksplit = std::max(1, target / mtiles);
+    e.ksplit = std::max(1, std::min(ksplit, ktiles / (g_tune.ecbig_kdiv > 0 ? g_tune.ecbig_kdiv : 2)));
+    return launch_ec_big(e, pdl, st);
+}
+
 // M <= 16, latency-bound layers: EC pre-kernel (when r > 0) then the row-strip kernel (rows.cu): one CTA per 16 output
 // rows over the whole of K, no cross-CTA reduction, no workspace traffic besides u.
 static int run_rows(const void* x, const void* Wq, const void* scales, const void* A, const void* B,
                     const spear_ec_desc* ec, void* y, int M, int N, int K, int r, int group,
                     uint8_t* ws, const WsLayout& L, cudaStream_t st) {
+    if (M > 16) {
+        // 17..64 tokens: the M > 16 EC pre-pass (u as fp16 [M][r]) and the 32-token form of the strip kernel
+        if (r > 0)
+            if (int rc = run_ec_big(x, A, ec, M, K, r, ws, L, g_tune.pdl != 0, st)) return rc;
+        RowsParams q = {};
+        q.wq = Wq; q.scales = scales;
+        q.x = static_cast<const __half*>(x);
+        q.y = static_cast<__half*>(y);
+        q.u16 = reinterpret_cast<const __half*>(ws + L.u16);
+        q.B = B;
+        q.M = M; q.N = N; q.K = K; q.r = r; q.G = K / group; q.group = group;
+        return launch_rows_mid(q, g_tune.pdl != 0, st);
+    }
     // scalar / none gate: z, gate and u inside the kernel (cluster-local); the paper's MLP gate goes through the pre-kernel
     const bool mlp = r > 0 && ec->gate_kind == SPEAR_GATE_MLP;
     // scalar / none gate: z inside the layer kernel, recomputed by each of its N / 128 clusters ("rows_ec" 0) -- or once, by a
@@ -537,27 +580,8 @@ static int run_tc_fused(const void* x, const void* Wq, const void* scales, const
         A = A16;
         B = B16;
     }
-    if (r > 0) {
-        EcBigParams e = {};
-        e.x = static_cast<const __half*>(x);
-        e.A = static_cast<const __half*>(A);
-        e.w_g = static_cast<const __half*>(ec->w_g);
-        e.b_g = static_cast<const float*>(ec->b_g);
-        e.W1 = static_cast<const __half*>(ec->W1);
-        e.b1 = static_cast<const float*>(ec->b1);
-        e.W2 = static_cast<const __half*>(ec->W2);
-        e.b2 = static_cast<const float*>(ec->b2);
-        e.zbuf = reinterpret_cast<float*>(ws + L.zbuf);
-        e.u16 = reinterpret_cast<__half*>(ws + L.u16);
-        e.gate_out = static_cast<float*>(ec->gate_out);
-        e.M = M; e.K = K; e.r = r; e.h = ec->gate_hidden; e.gate_kind = ec->gate_kind;
-        e.alpha = ec->alpha;
-        const int mtiles = (M + 127) / 128, ktiles = K / 64;
-        int target = (g_tune.ecpre_ctas > 0 ? g_tune.ecpre_ctas : 2 * g_dev.num_sms);
-        int ksplit = std::max(1, target / mtiles);
-        e.ksplit = std::max(1, std::min(ksplit, ktiles / (g_tune.ecbig_kdiv > 0 ? g_tune.ecbig_kdiv : 2)));
-        if (int rc = launch_ec_big(e, pdl, st)) return rc;
-    }
+    if (r > 0)
+        if (int rc = run_ec_big(x, A, ec, M, K, r, ws, L, pdl, st)) return rc;
     TcProblem t = {};
     t.x = x; t.wq = Wq; t.scales = scales; t.B = B; t.y = y;
     t.u16 = (r > 0 && !split) ? ws + L.u16 : nullptr;
@@ -755,6 +779,10 @@ static int layer_impl(const void* x, const void* Wq, const void* scales, const v
                              "supported for M <= 16 on the weight-stream variants only (variant %d, M = %d runs the layer, then a row kernel)",
                              y0 == r0 ? "aliases" : "partly overlaps", v, M);
     }
+    if (v == SPEAR_VARIANT_ROWS && M > 16 && ec_i8) {
+        if (ec && ec->force_variant != SPEAR_VARIANT_AUTO) return set_error(SPEAR_EUNSUPPORTED, "the row-strip variant above 16 tokens takes fp16 EC factors");
+        v = SPEAR_VARIANT_TC_FUSED;
+    }
     if (ec_i8 && M <= 16 && (v == SPEAR_VARIANT_TC_FUSED || v == SPEAR_VARIANT_TC_SPLIT))
         return set_error(SPEAR_EUNSUPPORTED, "INT8 EC factors on the tcgen05 variants need M > 16 (workspace scratch is sized for that path)");
     if (v == SPEAR_VARIANT_LSTREAM) {
@@ -764,7 +792,7 @@ static int layer_impl(const void* x, const void* Wq, const void* scales, const v
         return tail ? launch_tail_rows(static_cast<__half*>(y), static_cast<const __half*>(tail->residual), static_cast<const __half*>(tail->rms_weight),
                                        static_cast<__half*>(tail->h_out), tail->eps, M, N, false, st) : SPEAR_OK;
     }
-    if (int rc = ws_prepare(ws, ws_bytes, L, M, r, v == SPEAR_VARIANT_TC_FUSED || v == SPEAR_VARIANT_TC_SPLIT, st)) return rc;
+    if (int rc = ws_prepare(ws, ws_bytes, L, M, r, v == SPEAR_VARIANT_TC_FUSED || v == SPEAR_VARIANT_TC_SPLIT || (v == SPEAR_VARIANT_ROWS && M > 16), st)) return rc;
     switch (v) {
         case SPEAR_VARIANT_STREAM_FUSED:       // the weight-stream kernel fuses the tail into its epilogue
             return run_stream(x, Wq, scales, A, B, ec, y, M, N, K, r, group, ws, L, true, st, tail);
@@ -824,6 +852,7 @@ extern "C" int spear_tune(const char* key, int value) {
     else if (!strcmp(key, "stream_units")) g_tune.stream_units = value;
     else if (!strcmp(key, "rows")) g_tune.rows = value;
     else if (!strcmp(key, "rows_ec")) g_tune.rows_ec = value;
+    else if (!strcmp(key, "rows_mid")) g_tune.rows_mid = value;
     else if (!strcmp(key, "tc_tail")) g_tune.tc_tail = value;
     else if (!strcmp(key, "stream_grid")) g_tune.stream_grid = value;
     else if (!strcmp(key, "stream_aligned")) g_tune.stream_aligned = value;

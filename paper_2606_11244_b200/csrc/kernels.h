@@ -61,6 +61,7 @@ struct RowsParams {
     const __half* x;         // [M][K]
     __half* y;               // [M][N]
     const float* u;          // [16][r] fp32, alpha * gamma (.) z from the EC pre-kernel; unused when r == 0
+    const __half* u16;       // mid-M form (launch_rows_mid): u as fp16 [M][r] from the M > 16 pre-pass
     const void* B;           // [N][r] fp16 (int8 when ec_int8)
     const __half* B_scale;   // [N] (ec_int8)
     int ec_int8;
@@ -78,7 +79,8 @@ struct RowsParams {
     float* gate_out;         // optional [M]
 };
 int launch_rows(const RowsParams& p, bool pdl, cudaStream_t st);
-int launch_ecz_cluster(const RowsParams& p, bool pdl, cudaStream_t st);      // z, gate, u once, by one cluster of 8 CTAs -> p.u
+int launch_ecz_cluster(const RowsParams& p, bool pdl, cudaStream_t st);
+int launch_rows_mid(const RowsParams& p, bool pdl, cudaStream_t st);        // 17..64 tokens: 32 tokens x one strip per CTA, fp16 EC factors, u16 from the M > 16 pre-pass      // z, gate, u once, by one cluster of 8 CTAs -> p.u
 
 // ---- lstream.cu (M <= 16): persistent "layer stream" -- ONE cooperative launch consumes a table of layer
 // calls as a single queue of (call, panel, 128-column chunk) work items; int4 -> fp16 in registers -> TMEM

@@ -328,6 +328,139 @@ __global__ void __launch_bounds__(256, 2) rows_kernel(const RowsParams p) {
     }
 }
 
+// ---- the same strip kernel for 17..64 tokens (mid-M on small layers) ------------------------------------------------------------
+// The tcgen05 kernel pays one ~0.45 us barrier round trip per 128 columns of K whatever the token count, so a 2048-column
+// layer costs it >= 9-12 us at any M; this kernel has no such floor.  grid = (N / 16 strips, ceil(M / 32) token blocks); a CTA
+// takes 32 tokens (four n = 8 tiles per mma.sync k-step) of one strip over the whole of K; weights are re-read per token block
+// (L2 hits: these are small layers).  It is bound by the legacy mma.sync rate and the x fragment loads, so it loses to tcgen05 on
+// big layers and above 64 tokens (api.cu decides).  EC: u = alpha gamma (.) z comes as fp16 [M][r] from the M > 16 pre-pass.
+__global__ void __launch_bounds__(256, 2) rowsm_kernel(const RowsParams p) {
+    constexpr int MT = 4, kTok = 32, kNB = 2;
+    __shared__ float red[8][16][kTok + 1];
+    __shared__ __align__(16) float us[kTok * 128];
+    __shared__ __align__(16) uint8_t bs[16 * (128 * 2 + 16)];
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int g = lane >> 2, t = lane & 3;
+    const int strip = blockIdx.x, mb = blockIdx.y * kTok;
+    const int pnl = strip >> 3, sp = strip & 7;
+    const int KT = p.K >> 6, C = p.K >> 7;
+    const uint8_t* wbase = reinterpret_cast<const uint8_t*>(p.wq) + size_t(pnl) * C * 8192 + (sp * 32 + lane) * 16;
+    const uint8_t* sbase = reinterpret_cast<const uint8_t*>(p.scales) + size_t(pnl) * p.G * 256 + (sp * 16 + 2 * g) * 2;
+    const int kt_per_group = p.group >> 6;
+    uint4 wv[kNB], wn[kNB];
+    uint32_t sc[kNB], sn[kNB];
+    auto load_w = [&](uint4 (&wd)[kNB], uint32_t (&sd)[kNB], int base) {
+#pragma unroll
+        for (int b = 0; b < kNB; ++b) {
+            const int kt = base + 8 * b;
+            if (kt < KT) {
+                wd[b] = __ldg(reinterpret_cast<const uint4*>(wbase + size_t(kt >> 1) * 8192 + (kt & 1) * 4096));      // (re-read by the other token blocks: keep it cached)
+                sd[b] = __ldg(reinterpret_cast<const uint32_t*>(sbase + size_t(kt / kt_per_group) * 256));
+            }
+        }
+    };
+    load_w(wv, sc, warp);
+    const int brow = p.r * 2 + 16;
+    if (p.r > 0) {
+        const int per_row = p.r * 2 / 8;
+        const uint8_t* Bs = reinterpret_cast<const uint8_t*>(p.B) + size_t(strip) * 16 * p.r * 2;
+        for (int i = threadIdx.x; i < 16 * per_row; i += 256) {
+            const int rw = i / per_row, pc = i - rw * per_row;
+            cp_async8(bs + rw * brow + pc * 8, Bs + (size_t(rw) * per_row + pc) * 8);
+        }
+    }
+    pdl_launch_dependents();
+    pdl_wait();
+    if (p.r > 0)
+        for (int i = threadIdx.x; i < kTok * p.r; i += 256) {
+            const int m = mb + i / p.r;
+            us[i] = m < p.M ? __half2float(__ldcg(p.u16 + size_t(mb) * p.r + i)) : 0.f;
+        }
+    float tot[MT][4];
+#pragma unroll
+    for (int mt = 0; mt < MT; ++mt) tot[mt][0] = tot[mt][1] = tot[mt][2] = tot[mt][3] = 0.f;
+    const __half* xrow[MT];
+#pragma unroll
+    for (int mt = 0; mt < MT; ++mt) xrow[mt] = (mb + mt * 8 + g < p.M) ? p.x + size_t(mb + mt * 8 + g) * p.K + 16 * t : nullptr;
+    for (int base = warp; base < KT; base += 8 * kNB) {
+        if (base + 8 * kNB < KT) load_w(wn, sn, base + 8 * kNB);
+#pragma unroll
+        for (int b = 0; b < kNB; ++b) {
+            const int kt = base + 8 * b;
+            if (kt < KT) {
+                uint4 xa[MT], xb[MT];
+#pragma unroll
+                for (int mt = 0; mt < MT; ++mt) {
+                    if (xrow[mt]) {
+                        xa[mt] = *reinterpret_cast<const uint4*>(xrow[mt] + kt * 64);
+                        xb[mt] = *reinterpret_cast<const uint4*>(xrow[mt] + kt * 64 + 8);
+                    } else {
+                        xa[mt] = make_uint4(0u, 0u, 0u, 0u);
+                        xb[mt] = make_uint4(0u, 0u, 0u, 0u);
+                    }
+                }
+                const uint4 w = wv[b];
+                uint32_t a0[4], a1[4], a2[4], a3[4];
+                dequant_word(w.x, a0);
+                dequant_word(w.z, a1);
+                dequant_word(w.y, a2);
+                dequant_word(w.w, a3);
+                const float s_lo = __half2float(__ushort_as_half(uint16_t(sc[b] & 0xffff)));
+                const float s_hi = __half2float(__ushort_as_half(uint16_t(sc[b] >> 16)));
+#pragma unroll
+                for (int mt = 0; mt < MT; ++mt) {
+                    float acc[4] = {0.f, 0.f, 0.f, 0.f}, acd[4] = {0.f, 0.f, 0.f, 0.f};
+                    mma_m16n8k16(acc, a0[0], a1[0], a2[0], a3[0], xa[mt].x, xb[mt].x);
+                    mma_m16n8k16(acd, a0[1], a1[1], a2[1], a3[1], xa[mt].y, xb[mt].y);
+                    mma_m16n8k16(acc, a0[2], a1[2], a2[2], a3[2], xa[mt].z, xb[mt].z);
+                    mma_m16n8k16(acd, a0[3], a1[3], a2[3], a3[3], xa[mt].w, xb[mt].w);
+                    tot[mt][0] = fmaf(s_lo, acc[0] + acd[0], tot[mt][0]);
+                    tot[mt][1] = fmaf(s_lo, acc[1] + acd[1], tot[mt][1]);
+                    tot[mt][2] = fmaf(s_hi, acc[2] + acd[2], tot[mt][2]);
+                    tot[mt][3] = fmaf(s_hi, acc[3] + acd[3], tot[mt][3]);
+                }
+            }
+        }
+#pragma unroll
+        for (int b = 0; b < kNB; ++b) { wv[b] = wn[b]; sc[b] = sn[b]; }
+    }
+#pragma unroll
+    for (int mt = 0; mt < MT; ++mt) {
+        red[warp][g][mt * 8 + 2 * t] = tot[mt][0];
+        red[warp][g][mt * 8 + 2 * t + 1] = tot[mt][1];
+        red[warp][g + 8][mt * 8 + 2 * t] = tot[mt][2];
+        red[warp][g + 8][mt * 8 + 2 * t + 1] = tot[mt][3];
+    }
+    if (p.r > 0) cp_async_wait_all();
+    __syncthreads();
+    const int row = threadIdx.x & 15;
+    const int n = strip * 16 + row;
+#pragma unroll
+    for (int pass = 0; pass < 2; ++pass) {
+        const int tok = (threadIdx.x >> 4) + 16 * pass;
+        if (mb + tok >= p.M) continue;
+        float v = 0.f;
+#pragma unroll
+        for (int w = 0; w < 8; ++w) v += red[w][row][tok];
+        if (p.r > 0) {
+            const float4* up = reinterpret_cast<const float4*>(us + tok * p.r);
+            float e0 = 0.f, e1 = 0.f;
+            for (int j8 = 0; j8 < p.r / 8; ++j8) {
+                const uint4 bv = *reinterpret_cast<const uint4*>(bs + row * brow + j8 * 16);
+                const float4 ua = up[2 * j8], ub = up[2 * j8 + 1];
+                const float2 f0 = __half22float2(*reinterpret_cast<const __half2*>(&bv.x));
+                const float2 f1 = __half22float2(*reinterpret_cast<const __half2*>(&bv.y));
+                const float2 f2 = __half22float2(*reinterpret_cast<const __half2*>(&bv.z));
+                const float2 f3 = __half22float2(*reinterpret_cast<const __half2*>(&bv.w));
+                e0 += ua.x * f0.x + ua.y * f0.y + ua.z * f1.x + ua.w * f1.y;
+                e1 += ub.x * f2.x + ub.y * f2.y + ub.z * f3.x + ub.w * f3.y;
+            }
+            v += e0 + e1;
+        }
+        p.y[size_t(mb + tok) * p.N + n] = __float2half_rn(v);
+    }
+}
+
 // ---- z, gate and u ONCE, by one cluster of 8 CTAs (S4-S6 for the split arm of the row-strip kernel) -----------------------------
 // The fused instance above makes every cluster of the layer recompute z (N / 128 times the work, and it sits in front of
 // each CTA's main loop).  Here z = x [A; w_g]^T is computed once: CTA c of ONE cluster takes the c-th eighth of K (its
@@ -498,6 +631,22 @@ int launch_ecz_cluster(const RowsParams& p, bool pdl, cudaStream_t st) {
     cfg.numAttrs = 2;
     if (MT == 1) SPEAR_CUDA_OK(cudaLaunchKernelEx(&cfg, ecz_cluster_kernel<1>, p));
     else SPEAR_CUDA_OK(cudaLaunchKernelEx(&cfg, ecz_cluster_kernel<2>, p));
+    count_launch();
+    return SPEAR_OK;
+}
+
+int launch_rows_mid(const RowsParams& p, bool pdl, cudaStream_t st) {
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3(p.N / 16, (p.M + 31) / 32);
+    cfg.blockDim = dim3(256);
+    cfg.dynamicSmemBytes = 0;
+    cfg.stream = st;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr[0].val.programmaticStreamSerializationAllowed = pdl ? 1 : 0;
+    cfg.attrs = attr;
+    cfg.numAttrs = 1;
+    SPEAR_CUDA_OK(cudaLaunchKernelEx(&cfg, rowsm_kernel, p));
     count_launch();
     return SPEAR_OK;
 }

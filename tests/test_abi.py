@@ -106,9 +106,13 @@ def test_plan_table_file_roundtrip_and_heuristics_without_gpu(tmp_path):
     assert query(8, 16384, 2048, 32, 128, 0) == 1
     assert query(8, 16384, 2048, 32, 128, 1) == 2
     assert query(8, 16384, 2048, 0, 128, 0) == 2
-    # the tcgen05 kernel above 16 tokens, whatever the size
-    assert query(64, 2048, 2048, 32, 128, 0) == 3
-    assert query(17, 2048, 2048, 0, 128, 0) == 3
+    # 17..64 tokens: the strip kernel's 32-token form up to 4 MiB of int4, the tcgen05 kernel otherwise and above 64 tokens
+    assert query(64, 2048, 2048, 32, 128, 0) == 6
+    assert query(17, 2048, 2048, 0, 128, 0) == 6
+    assert query(64, 4096, 2048, 0, 128, 0) == 6          # exactly 4 MiB
+    assert query(64, 2048, 8192, 32, 128, 0) == 3         # 8 MiB
+    assert query(65, 2048, 2048, 32, 128, 0) == 3         # above 64 tokens
+    assert query(2048, 2048, 2048, 0, 128, 0) == 3
     # a hand-written table overrides them and survives save -> load
     src = tmp_path / "plan.txt"
     src.write_text("# spear plan v1\n4 2048 2048 16 128 0 2 17.2 16.5 26.4 32.2 -1\n64 2048 2048 32 128 0 4 -1 -1 30.0 28.0 -1\n")

@@ -36,12 +36,16 @@ def test_plan_decode_times_fused_and_split(sp, tmp_path):
 
 
 def test_plan_crossover_shapes(sp):
-    # M <= 16: the decode kernel and the tcgen05 kernel are both valid; above 16 only the tcgen05 one
+    # M <= 16: the decode kernels and the tcgen05 kernel are all valid; 17..64 tokens: the tcgen05 arms and the strip kernel's
+    # 32-token form, never the ring kernel; above 64 tokens only the tcgen05 arms
     chosen, us = sp.plan(16, 4096, 4096, 64, 4096, gate="scalar")
-    assert us[sp.VARIANT_TC_FUSED] > 0 and us[sp.VARIANT_STREAM_FUSED] > 0
+    assert us[sp.VARIANT_TC_FUSED] > 0 and us[sp.VARIANT_STREAM_FUSED] > 0 and us[sp.VARIANT_ROWS] > 0
     chosen64, us64 = sp.plan(64, 2048, 2048, 32, 128, gate="scalar")
-    assert chosen64 in (sp.VARIANT_TC_FUSED, sp.VARIANT_TC_SPLIT) and us64[sp.VARIANT_STREAM_FUSED] < 0
-    assert us64[sp.VARIANT_TC_FUSED] > 0 and us64[sp.VARIANT_TC_SPLIT] > 0      # both prefill arms are measured
+    assert chosen64 in (sp.VARIANT_TC_FUSED, sp.VARIANT_TC_SPLIT, sp.VARIANT_ROWS) and us64[sp.VARIANT_STREAM_FUSED] < 0
+    assert us64[sp.VARIANT_TC_FUSED] > 0 and us64[sp.VARIANT_TC_SPLIT] > 0 and us64[sp.VARIANT_ROWS] > 0
+    assert us64[chosen64] == min(t for t in us64 if t > 0)
+    chosen96, us96 = sp.plan(96, 2048, 2048, 32, 128, gate="scalar")
+    assert chosen96 in (sp.VARIANT_TC_FUSED, sp.VARIANT_TC_SPLIT) and us96[sp.VARIANT_ROWS] < 0 and us96[sp.VARIANT_STREAM_FUSED] < 0
 
 
 def test_planned_variant_matches_oracle(sp):

@@ -123,3 +123,26 @@ def test_stream_ordered_in_a_graph(sp):
         ref = oracle.forward_layer(li)["y"]
         rms = float(np.sqrt(np.mean(ref ** 2)))
         assert float(np.max(np.abs(y.cpu().numpy().astype(np.float64) - ref))) <= Y_TOL * rms
+
+
+@pytest.mark.parametrize("M", [17, 31, 32, 33, 48, 64])
+@pytest.mark.parametrize("shape", [(3072, 2048, 128, 32, "scalar"), (2048, 8192, 128, 32, "scalar"), (384, 640, 128, 24, "mlp"),
+                                   (256, 1792, 1792, 0, "none"), (512, 1024, 256, 128, "none")])
+def test_mid_token_counts(sp, M, shape):
+    """The 32-token form of the strip kernel (17..64 tokens; u as fp16 from the M > 16 EC pre-pass): config-5-sized layers, ragged
+    token blocks, K not a multiple of 512, per-channel scales, every gate, r = 0 and r = 128."""
+    N, K, group, r, gate = shape
+    check(sp, make_layer(500 + M + r, M, N, K, group, r, gate=gate), f"mid-M M={M} {shape}")
+
+
+def test_mid_token_counts_refuse_int8_when_forced_and_fall_back_on_auto(sp):
+    import torch
+    from paper_2606_11244_b200 import harness as h
+    li = with_int8_ec(make_layer(560, 40, 512, 1024, 128, 16, gate="scalar"))
+    dl = h.upload_layer(li)
+    with pytest.raises(sp.SpearError):
+        h.run_layer(dl, h.dev(li.x), variant=sp.VARIANT_ROWS)
+    y, _ = h.run_layer(dl, h.dev(li.x))                # AUTO serves it (tcgen05 path with the factors dequantised to fp16 scratch)
+    torch.cuda.synchronize()
+    ref = oracle.forward_layer(li)["y"]
+    assert float(np.max(np.abs(y.cpu().numpy().astype(np.float64) - ref))) <= Y_TOL * float(np.sqrt(np.mean(ref ** 2)))
