@@ -255,7 +255,7 @@ int spear_lut_measure(const int* M_grid, int n_grid, int N, int K, int group, in
  * changes what is computed).  Decode ring kernel: "stream_ctas_per_sm", "stream_deep" (-1 heuristic, 0 / 1 shallow / deep
  * ring), "stream_whole_panels", "stream_aligned", "stream_grid", "stream_batch_grid", "stream_batch_units", "stream_units"; decode kernel choice: "rows" (1 =
  * the heuristic may pick the row-strip kernel for small layers, 0 = never), "rows_mid" (1 = the heuristic may pick its 32-token form for 17..64 tokens), "rows_ec" (the row-strip kernel's EC: 0 = z per cluster inside
- * the kernel, 1 = z once by a one-cluster pre-kernel (default)), "lstream" (-1 = the layer-stream kernel only
+ * the kernel, 1 = z, gate and u once by a one-cluster pre-kernel, 2 (default) = partial z by 8 pre-kernel CTAs, summed and gated in the layer kernel), "lstream" (-1 = the layer-stream kernel only
  * where spear_plan_batch measured it faster, 0 = never, 1 = always for M <= 16); EC pre-kernels: "ecpre_ctas", "ecbig_kdiv";
  * tcgen05 kernel: "tc_grid", "tc_cluster", "tc_ksplit", "tc_tail" (split the tiles of a small partial last wave along K), "tc_bt", "tc_xslice_mb"; all: "pdl"; batch: "batch_lanes".
  * Unknown key -> SPEAR_EINVAL.  Host-only, process-wide, not thread-safe against concurrent compute calls.  bench.py

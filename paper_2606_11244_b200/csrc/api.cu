@@ -245,7 +245,7 @@ struct Tunables {
     int stream_aligned = 1;       // 1 = panel-aligned partition for stream-ordered calls with fewer panels than SMs
     int stream_grid = 0;          // 0 = heuristic, else the decode ring kernel's grid for stream-ordered calls (sweeps)
     int rows_mid = 1;             // 1 = the heuristic may pick the strip kernel's 32-token form for 17..64 tokens on small layers
-    int rows_ec = 1;              // row-strip kernel's EC (scalar / none gate): 1 = z once by a one-cluster pre-kernel, 0 = z per cluster inside the layer kernel
+    int rows_ec = 2;              // row-strip kernel's EC (scalar / none gate): 2 = partial z by 8 pre-kernel CTAs, summed and gated by the layer kernel; 1 = z, gate and u by a one-cluster pre-kernel; 0 = z per cluster inside the layer kernel
     int rows = 1;                 // 1 = the heuristic may pick the row-strip kernel for small decode layers, 0 = never
 };
 static Tunables g_tune;
@@ -537,6 +537,8 @@ static int run_rows(const void* x, const void* Wq, const void* scales, const voi
     // o 2048^2 (16 clusters) 5.5 / 5.9 / 8.6 fused against 5.8 / 6.2 / 8.3; qkv 2048 -> 3072 (24 clusters) 6.6 / 7.1 / 9.6 against
     // 5.8 / 6.4 / 8.5; gate_up (128 clusters) 32 against 14.  Inside the 12-call stream-ordered step of config 2 the pre-kernel arm
     // wins on both (114.9 -> 111.3 us): a cluster launch of the big fused grid does not overlap its predecessor as well.
+    // 2 (the default): the pre-kernel is 8 INDEPENDENT CTAs that park their partial z in the workspace -- no cluster, no DSMEM, no gate --
+    // and every CTA of the layer kernel sums the eight parts and applies the gate while its x loads are in flight: step 114.0 -> 109.8 us.
     const bool want_pre = g_tune.rows_ec != 0;
     const bool fused = r > 0 && !mlp && !want_pre;           // z per cluster inside the layer kernel
     const bool pre_cluster = r > 0 && !mlp && want_pre;      // z once, by a one-cluster pre-kernel
@@ -560,6 +562,7 @@ static int run_rows(const void* x, const void* Wq, const void* scales, const voi
         p.b_g = static_cast<const float*>(ec->b_g);
         p.gate_out = static_cast<float*>(ec->gate_out);
     }
+    if (pre_cluster && g_tune.rows_ec == 2) p.zpart = reinterpret_cast<float*>(ws + L.partial);      // (split-K slots: unused on this arm)
     if (pre_cluster)
         if (int rc = launch_ecz_cluster(p, g_tune.pdl != 0, st)) return rc;
     return launch_rows(p, g_tune.pdl != 0, st);

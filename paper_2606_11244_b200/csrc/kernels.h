@@ -77,6 +77,7 @@ struct RowsParams {
     const __half* w_g;       // [K] (scalar gate)
     const float* b_g;        // 1 or NULL
     float* gate_out;         // optional [M]
+    float* zpart;            // non-NULL: the pre-kernel parks 8 partial z [8 MT][r + 1] here (no cluster), the layer kernel sums and gates
 };
 int launch_rows(const RowsParams& p, bool pdl, cudaStream_t st);
 int launch_ecz_cluster(const RowsParams& p, bool pdl, cudaStream_t st);

@@ -37,6 +37,11 @@
 // kernel on big layers; the L1 wavefronts of the x fragment loads (8 lines per LDG.128, twice per k-tile, four times at M > 8)
 // and the legacy mma.sync rate (~3.9 clk per m16n8k16 per SM) are.
 //
+// Default EC arm since the end of round 2 ("rows_ec" 2): the pre-kernel (ecz_cluster_kernel<MT, true>) is 8 independent CTAs, CTA c
+// reduces the c-th eighth of K and parks its partial z [8 MT][r + 1] in the workspace; the plain layer kernel, which started under PDL
+// while they ran, sums the eight parts in rank order and applies the gate when it stages u -- those loads share the round trip of
+// its x loads.  No cluster, no DSMEM, no barrier: 5.8 us against 6.4 (one-cluster arm) on o at M = 8.
+//
 // Also measured and not kept: the EC cluster INSIDE the layer kernel's grid (8 extra CTAs compute z once and raise a flag; the strips
 // poll it after their main loop, with a bounded wait and a compute-it-yourself fallback so that progress never rests on dispatch
 // order).  One launch instead of two, but slower than the one-cluster pre-kernel: qkv 7.0 / 7.4 / 8.6 us against 5.8 / 6.4 / 8.5 --
@@ -152,10 +157,34 @@ __global__ void __launch_bounds__(256, 2) rows_kernel(const RowsParams p) {
     }
     pdl_launch_dependents();
     pdl_wait();          // x (and u) may be written by the previous kernel in the stream
-    if (!FUSED && p.r > 0)
-        for (int i = threadIdx.x; i < kTok * p.r; i += 256) {
-            if (i < p.M * p.r) cp_async4(us + i, p.u + i); else us[i] = 0.f;
+    if (!FUSED && p.r > 0) {
+        if (p.zpart) {
+            // the pre-kernel left eight partial z [kTok][r + 1] in global memory: sum them in rank order, gate, u (all loads of a
+            // thread in flight at once; they share the round trip with the x loads below)
+            const bool sc = (p.gate_kind == SPEAR_GATE_SCALAR_SIGMOID);
+            const int zr1 = p.r + 1;
+            const float bias = (sc && p.b_g) ? __ldg(p.b_g) : 0.f;
+            for (int i = threadIdx.x; i < kTok * p.r; i += 256) {
+                const int m = i / p.r, j = i - m * p.r;
+                float zv[8], gv[8];
+#pragma unroll
+                for (int c = 0; c < 8; ++c) {
+                    zv[c] = p.zpart[(c * kTok + m) * zr1 + j];
+                    gv[c] = sc ? p.zpart[(c * kTok + m) * zr1 + p.r] : 0.f;
+                }
+                float z = 0.f, zg = 0.f;
+#pragma unroll
+                for (int c = 0; c < 8; ++c) { z += zv[c]; zg += gv[c]; }
+                const float gam = sc ? 1.f / (1.f + expf(-(zg + bias))) : 1.f;
+                us[i] = m < p.M ? p.alpha * gam * z : 0.f;
+                if (sc && p.gate_out && blockIdx.x == 0 && j == 0 && m < p.M) p.gate_out[m] = gam;
+            }
+        } else {
+            for (int i = threadIdx.x; i < kTok * p.r; i += 256) {
+                if (i < p.M * p.r) cp_async4(us + i, p.u + i); else us[i] = 0.f;
+            }
         }
+    }
 
     float tot[MT][4];
 #pragma unroll
@@ -468,7 +497,7 @@ __global__ void __launch_bounds__(256, 2) rowsm_kernel(const RowsParams p) {
 // distributed shared memory, rank 0 sums them in rank order, applies the gate (scalar / none) and writes
 // u = alpha gamma (.) z as fp32 [8 MT][r] to global memory for the layer kernel that is already running behind it under
 // programmatic dependent launch (its weight requests are in flight; it reads u after its own griddepcontrol.wait).
-template <int MT>
+template <int MT, bool PART>      // PART: no cluster -- 8 independent CTAs park their partial z in global memory, the layer kernel sums and gates
 __global__ void __launch_bounds__(256, 1) ecz_cluster_kernel(const RowsParams p) {
     constexpr int kTok = 8 * MT;
     constexpr int kSG = 2;
@@ -480,7 +509,7 @@ __global__ void __launch_bounds__(256, 1) ecz_cluster_kernel(const RowsParams p)
     const int zr = p.r + 1;
     const int strips = (p.r + (scalar ? 1 : 0) + 15) >> 4;
     const int sgroups = (strips + kSG - 1) / kSG;
-    const uint32_t rank = cluster_ctarank();
+    const uint32_t rank = PART ? blockIdx.x : cluster_ctarank();
     const int kt0 = int(rank) * KT / 8, kt1 = (int(rank) + 1) * KT / 8;
     const int n_items = (kt1 - kt0) * sgroups;
     float* zmine = zs + 8 * kTok * zr;
@@ -504,7 +533,7 @@ __global__ void __launch_bounds__(256, 1) ecz_cluster_kernel(const RowsParams p)
             }
     };
     for (int i = threadIdx.x; i < kTok * zr; i += 256) zmine[i] = 0.f;
-    cluster_arrive_release();                     // "this CTA runs": matched before the first peer store below
+    if (!PART) cluster_arrive_release();          // "this CTA runs": matched before the first peer store below
     if (warp < n_items) load_A(0, warp);          // the factors are parameters: before the wait
     pdl_wait();                                   // x may be the previous kernel's output
     __syncthreads();                              // zmine is zero
@@ -540,6 +569,11 @@ __global__ void __launch_bounds__(256, 1) ecz_cluster_kernel(const RowsParams p)
         }
     }
     __syncthreads();
+    if (PART) {
+        float* out = p.zpart + size_t(rank) * kTok * zr;
+        for (int i = threadIdx.x; i < kTok * zr; i += 256) out[i] = zmine[i];
+        return;
+    }
     cluster_wait_acquire();                       // every CTA of the cluster has started: rank 0's shared memory may be written
     const uint32_t slot0 = mapa_shared(smem_u32(zs + int(rank) * kTok * zr), 0);
     for (int i = threadIdx.x; i < kTok * zr; i += 256) st_shared_cluster_f32(slot0 + 4 * i, zmine[i]);
@@ -610,11 +644,35 @@ int launch_ecz_cluster(const RowsParams& p, bool pdl, cudaStream_t st) {
     static std::once_flag once;
     static cudaError_t err = cudaSuccess;
     std::call_once(once, [&]() {
-        err = cudaFuncSetAttribute((const void*)ecz_cluster_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, 9 * 8 * 129 * 4);
+        err = cudaFuncSetAttribute((const void*)ecz_cluster_kernel<1, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, 9 * 8 * 129 * 4);
         if (err == cudaSuccess)
-            err = cudaFuncSetAttribute((const void*)ecz_cluster_kernel<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, 9 * 16 * 129 * 4);
+            err = cudaFuncSetAttribute((const void*)ecz_cluster_kernel<2, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, 9 * 16 * 129 * 4);
     });
     SPEAR_CUDA_OK(err);
+    if (p.zpart) {
+        static std::once_flag once2;
+        static cudaError_t err2 = cudaSuccess;
+        std::call_once(once2, [&]() {
+            err2 = cudaFuncSetAttribute((const void*)ecz_cluster_kernel<1, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, 9 * 8 * 129 * 4);
+            if (err2 == cudaSuccess)
+                err2 = cudaFuncSetAttribute((const void*)ecz_cluster_kernel<2, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, 9 * 16 * 129 * 4);
+        });
+        SPEAR_CUDA_OK(err2);
+        cudaLaunchConfig_t c2 = {};
+        c2.gridDim = dim3(8);
+        c2.blockDim = dim3(256);
+        c2.dynamicSmemBytes = size_t(9) * 8 * MT * (p.r + 1) * 4;
+        c2.stream = st;
+        cudaLaunchAttribute a2[1];
+        a2[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+        a2[0].val.programmaticStreamSerializationAllowed = pdl ? 1 : 0;
+        c2.attrs = a2;
+        c2.numAttrs = 1;
+        if (MT == 1) SPEAR_CUDA_OK(cudaLaunchKernelEx(&c2, ecz_cluster_kernel<1, true>, p));
+        else SPEAR_CUDA_OK(cudaLaunchKernelEx(&c2, ecz_cluster_kernel<2, true>, p));
+        count_launch();
+        return SPEAR_OK;
+    }
     cudaLaunchConfig_t cfg = {};
     cfg.gridDim = dim3(8);
     cfg.blockDim = dim3(256);
@@ -629,8 +687,8 @@ int launch_ecz_cluster(const RowsParams& p, bool pdl, cudaStream_t st) {
     attr[1].val.clusterDim.z = 1;
     cfg.attrs = attr;
     cfg.numAttrs = 2;
-    if (MT == 1) SPEAR_CUDA_OK(cudaLaunchKernelEx(&cfg, ecz_cluster_kernel<1>, p));
-    else SPEAR_CUDA_OK(cudaLaunchKernelEx(&cfg, ecz_cluster_kernel<2>, p));
+    if (MT == 1) SPEAR_CUDA_OK(cudaLaunchKernelEx(&cfg, ecz_cluster_kernel<1, false>, p));
+    else SPEAR_CUDA_OK(cudaLaunchKernelEx(&cfg, ecz_cluster_kernel<2, false>, p));
     count_launch();
     return SPEAR_OK;
 }

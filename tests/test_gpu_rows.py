@@ -77,12 +77,13 @@ def test_int8_ec_factors(sp, M):
     check(sp, li, f"INT8 EC M={M}")
 
 
-@pytest.mark.parametrize("rows_ec", [0, 1])
+@pytest.mark.parametrize("rows_ec", [0, 1, 2])
 @pytest.mark.parametrize("shape", [(8, 2048, 2048, 128, 32, "scalar"), (16, 3072, 2048, 128, 32, "scalar"), (1, 512, 8192, 128, 128, "scalar"),
                                    (13, 384, 640, 128, 24, "none"), (5, 256, 128, 128, 8, "scalar"), (16, 6144, 4096, 4096, 64, "scalar")])
 def test_both_ec_arms(sp, rows_ec, shape):
     """The row-strip kernel's EC for the scalar / none gate has two arms (spear_tune "rows_ec"): z recomputed by every cluster inside
-    the layer kernel (0), or once by the one-cluster pre-kernel ecz_cluster_kernel that the layer kernel overlaps (1).  Both, on
+    the layer kernel (0), once by the one-cluster pre-kernel ecz_cluster_kernel that the layer kernel overlaps (1), or as eight partial
+    z parked in the workspace by 8 independent pre-kernel CTAs and summed + gated by the layer kernel (2, the default).  All, on
     shapes that cover ragged tokens, one k-tile per CTA of the cluster (K = 128 ... 640), r = 128, per-channel scales."""
     M, N, K, group, r, gate = shape
     sp.tune("rows_ec", rows_ec)
@@ -90,7 +91,7 @@ def test_both_ec_arms(sp, rows_ec, shape):
         check(sp, make_layer(400 + M + r, M, N, K, group, r, gate=gate), f"rows_ec={rows_ec} {shape}")
         check(sp, with_int8_ec(make_layer(401 + M + r, M, N, K, group, r, gate=gate)), f"rows_ec={rows_ec} int8 {shape}")
     finally:
-        sp.tune("rows_ec", 1)
+        sp.tune("rows_ec", 2)
 
 
 def test_stream_ordered_in_a_graph(sp):
