@@ -574,3 +574,20 @@ def test_stream_ordered_step_replay_stress(sp):
         for lab, t in (("after 5000 replays", y0), ("replay 5001 into zeroed y", y)):
             err = float(np.max(np.abs(t.cpu().numpy().astype(np.float64) - ref)))
             assert err <= Y_TOL * rms, f"{s.name} M={s.M} {lab}: {err:.4g} > {Y_TOL} * {rms:.4g}"
+
+
+@pytest.mark.parametrize("shape", [(8, 2048, 8192, 128, 32), (16, 2048, 8192, 128, 0), (1, 6144, 4096, 4096, 64), (16, 4096, 14336, 14336, 64),
+                                   (5, 1280, 1792, 128, 16), (8, 384, 7168, 128, 8), (16, 2432, 4608, 256, 24)])
+@pytest.mark.parametrize("knob", [("stream_aligned", 0), ("stream_aligned", 1), ("stream_grid", 37), ("stream_grid", 101)])
+def test_ring_kernel_partitions(sp, shape, knob):
+    """The ring kernel's result must not depend on how the units are cut over CTAs: panel-aligned equal parts (default when a layer has
+    fewer panels than SMs), the even stream-K split (stream_aligned = 0), and two odd forced grids whose CTAs straddle panels with
+    ragged first / last segments -- with and without the EC (whose B slab follows the segment that starts a panel)."""
+    M, N, K, group, r = shape
+    li = make_layer(800 + M + r, M, N, K, group, r, gate="scalar")
+    sp.tune(knob[0], knob[1])
+    try:
+        check_layer(li, variant=1 if r else 2, label=f"{knob} {shape}")
+    finally:
+        sp.tune("stream_aligned", 1)
+        sp.tune("stream_grid", 0)
